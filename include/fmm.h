@@ -1,0 +1,171 @@
+/*
+ * fmm.h -- C ABI of libfmm_b200.so: the B200 (sm_100a, FP64) hot path of the
+ * interpolation-based fast multipole method for the lab-frame relativistic space-charge
+ * field (arXiv 2302.07567; citations are PAPER.md:<line> + equation / algorithm, or a
+ * DESIGN.md reading where the paper is silent or garbled).
+ *
+ * Problem (eq. (3.1)-(3.2)): N particles with positions x_i, normalised
+ * momenta p_i = gamma_i beta_i and charges q_i.  Wanted at every particle:
+ *     E_i = 1/(4 pi eps0)    * sum_{j != i} q_j gamma_j g(x_i, x_j)
+ *     B_i = 1/(4 pi eps0 c0) * sum_{j != i} q_j p_j x g(x_i, x_j)
+ *     g(x_i, x_j) = (x_i - x_j) / (dx^2 + dy^2 + gamma_bar^2 dz^2)^{3/2},
+ *     gamma_j = sqrt(1 + p_j.p_j),  gamma_bar^2 = 1 + pbar.pbar,  pbar = mean momentum.
+ * Method (Alg 5.12): cluster tree (Alg 5.1/5.2) -> dual tree traversal
+ * with the stretched admissibility condition (Alg 5.6-5.8, Alg 9.1) -> P2M/M2M (Alg 5.3-5.5)
+ * -> M2L (Alg 5.9) + P2P (Alg 5.10) -> L2L/L2P (Alg 5.13-5.15).
+ *
+ * Conventions
+ *   Pointers   every array pointer is a DEVICE pointer unless the name of the call ends in
+ *              _host.  Arrays are structure-of-arrays FP64 of length N, caller-owned; inputs
+ *              are read-only and need not outlive the call that takes them.
+ *   Workspace  every byte of device workspace is obtained through the caller's allocator
+ *              (fmm_alloc_fn / fmm_free_fn, e.g. PyTorch's caching allocator).  If both are
+ *              NULL the library uses cudaMalloc / cudaFree.  A plan frees its workspace in
+ *              fmm_plan_destroy.
+ *   Stream     all work is enqueued on `cuda_stream` (a cudaStream_t passed as void*; NULL =
+ *              the legacy default stream).  fmm_plan_create / fmm_plan_update synchronise the
+ *              stream internally (the interaction-list lengths must be read back to size the
+ *              lists); fmm_eval and fmm_direct only enqueue and return.
+ *   Errors     0 on success, a negative FMM_E* code otherwise; no exceptions, no exit(), no
+ *              global state.  Outputs are unspecified after an error.
+ *   Order      outputs are in the caller's particle order.
+ *   Units      SI; eps0 = 8.8541878128e-12 F/m, c0 = 299792458 m/s (CODATA 2018), unless
+ *              FMM_RAW_SUMS is set (then the bare sums without prefactors are returned).
+ *   Determinism  accumulation is target-owned (every target gathers over its own list in a
+ *              fixed order); there are no floating-point atomics: identical inputs give
+ *              bit-identical outputs run to run.
+ */
+#ifndef FMM_B200_H
+#define FMM_B200_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define FMM_MAX_ORDER 12            /* interpolation degree n <= 12 (P = (n+1)^3 <= 2197)        */
+
+/* flags word of fmm_params_t / fmm_direct */
+#define FMM_TREE_KD            0u   /* Alg 5.2: median split along the axis of
+                                       largest stretched extent (default)                        */
+#define FMM_TREE_MORTON_MEDIAN 1u   /* particle order = 63-bit Morton key of the stretched, cube-
+                                       normalised coordinates, same closed-form ranges (DESIGN T-3') */
+#define FMM_TREE_MASK          1u
+#define FMM_RAW_SUMS           4u   /* skip the prefactors of eq. (3.1)                          */
+
+#define FMM_OK          0
+#define FMM_EINVAL     -1           /* bad argument: N < 1, order out of range, leaf_size < 1,
+                                       theta <= 0 or non-finite, NULL pointer                    */
+#define FMM_ENOMEM     -2           /* the allocator returned NULL                               */
+#define FMM_ECUDA      -3           /* a CUDA call failed; text in fmm_last_error                */
+#define FMM_ENONFINITE -4           /* gamma_bar came out non-finite (NaN / Inf in the momenta)  */
+#define FMM_EOVERFLOW  -5           /* an interaction list exceeds 2^31-1 entries                */
+
+typedef struct fmm_plan fmm_plan_t; /* opaque; owns its device workspace                          */
+
+typedef void *(*fmm_alloc_fn)(size_t bytes, void *user); /* returns a device pointer (256-B aligned) or NULL */
+typedef void (*fmm_free_fn)(void *ptr, void *user);
+
+typedef struct {
+    int64_t N;                      /* number of particles, >= 1                                 */
+    const double *x, *y, *z;        /* positions [m]                                             */
+    const double *px, *py, *pz;     /* normalised momenta gamma*beta [1]        */
+    const double *q;                /* charges [C], or NULL: every particle carries q_scalar      */
+    double q_scalar;
+} fmm_particles_t;
+
+typedef struct {
+    int order_n;                    /* interpolation degree n, 1 <= n <= FMM_MAX_ORDER           */
+    int leaf_size;                  /* N0 >= 1: maximum particles per leaf (Alg 5.2)             */
+    double theta;                   /* admissibility parameter eta > 0 (eq. (4.3)) */
+    double gamma_bar;               /* <= 0: computed from the mean momentum;
+                                       > 0: use this value                                       */
+    uint32_t flags;                 /* FMM_TREE_* | FMM_RAW_SUMS                                 */
+} fmm_params_t;
+
+/* Per-stage device times are CUDA-event times of the last fmm_plan_create/_update (tree, lists)
+ * and of the last fmm_eval that ran with timing switched on (fmm_plan_set_timing). */
+typedef struct {
+    int64_t N;
+    int32_t order_n, P, leaf_size, kappa;   /* P = (n+1)^3; kappa = tree depth     */
+    int64_t nodes, leaves;                  /* 2^{kappa+1}-1, 2^kappa              */
+    int64_t n_p2p, n_m2l;                   /* lengths of the two interaction lists (Alg 9.1)     */
+    int64_t p2p_pairs, m2l_pairs;           /* kernel evaluations: particle pairs, proxy pairs    */
+    double gamma_bar, theta;
+    uint32_t flags;
+    int32_t timing_valid;                   /* 1 if the eval times below were measured            */
+    float ms_tree;                          /* a0-a2: gamma_bar, order, permute, bounding boxes    */
+    float ms_lists;                         /* a3: traversal, sort, CSR                            */
+    float ms_p2m, ms_m2m, ms_m2l, ms_l2l, ms_p2p, ms_l2p;  /* a4-a10 (l2p includes finalise)      */
+    int64_t workspace_bytes;                /* device bytes currently held by the plan            */
+} fmm_stats_t;
+
+/* Copies of the plan's integer structures and (optionally) expansions, for bit-exact
+ * comparison with the oracle.  Every non-NULL field is a HOST pointer to caller memory of the
+ * stated length; NULL fields are skipped.  Node ids are heap indices, root = 1
+ * (PAPER.md:578-584); row i-1 describes node i. */
+typedef struct {
+    int64_t *perm;      /* [N]         tree position -> caller index                              */
+    int64_t *node_lo;   /* [nodes]     half-open range [lo, hi) of tree positions                 */
+    int64_t *node_hi;   /* [nodes]                                                                */
+    double *bbox;       /* [nodes][6]  ax ay az bx by bz (tight)                  */
+    int32_t *p2p_off;   /* [nodes+1]   CSR by target node (row i-1 = node i), P2P list            */
+    int32_t *p2p_src;   /* [n_p2p]     source leaf ids, ascending within a target                 */
+    int32_t *m2l_off;   /* [nodes+1]   CSR by target node, M2L list                               */
+    int32_t *m2l_src;   /* [n_m2l]                                                                */
+    double *M;          /* [nodes][P][4]  multipole moments (q gamma, q px, q py, q pz) after the
+                                          upward pass of the last fmm_eval; nu = (nu1*(n+1)+nu2)*(n+1)+nu3 */
+    double *L;          /* [nodes][P][6]  local fields (E, B sums) after the downward pass         */
+} fmm_export_t;
+
+/* a0-a3: mean momentum -> gamma_bar, tree order, bounding boxes, dual tree traversal, CSR lists.
+ * Synchronises the stream.  *out is NULL on error. */
+int fmm_plan_create(fmm_plan_t **out, const fmm_particles_t *particles, const fmm_params_t *params,
+                    fmm_alloc_fn alloc, fmm_free_fn free_, void *user, void *cuda_stream);
+
+/* Same N and parameters, new positions / momenta / charges: rebuilds tree and lists in place,
+ * reusing the workspace where sizes allow. */
+int fmm_plan_update(fmm_plan_t *plan, const fmm_particles_t *particles);
+
+/* a4-a10: P2M, M2M, M2L, P2P, L2L, L2P, prefactors, scatter to caller order.  Enqueue only.
+ * Ex..Bz: device arrays of length N, overwritten. */
+int fmm_eval(fmm_plan_t *plan, double *Ex, double *Ey, double *Ez, double *Bx, double *By, double *Bz);
+
+/* a11: direct O(N * n_targets) summation (Alg 5.10 with S_t = S_s = S).
+ * target_idx: device array of n_targets particle indices, or NULL = all N particles in order
+ * (then n_targets must be N).  gamma_bar <= 0: computed from the mean momentum.
+ * Outputs: device arrays of length n_targets.  Enqueue only (synchronises only if gamma_bar <= 0). */
+int fmm_direct(const fmm_particles_t *particles, double gamma_bar, uint32_t flags,
+               int64_t n_targets, const int64_t *target_idx,
+               double *Ex, double *Ey, double *Ez, double *Bx, double *By, double *Bz,
+               fmm_alloc_fn alloc, fmm_free_fn free_, void *user, void *cuda_stream);
+
+/* Whole of Alg 5.12 from HOST memory: copies the particles to the device, fmm_plan_create,
+ * fmm_eval, copies E and B back, destroys the plan.  All pointers in `particles` and the six
+ * outputs are HOST pointers (pinned memory makes the copies asynchronous).  Returns after the
+ * results are in host memory.  stats (may be NULL) receives the plan's statistics. */
+int fmm_field_host(const fmm_particles_t *particles_host, const fmm_params_t *params,
+                   double *Ex, double *Ey, double *Ez, double *Bx, double *By, double *Bz,
+                   fmm_stats_t *stats,
+                   fmm_alloc_fn alloc, fmm_free_fn free_, void *user, void *cuda_stream);
+
+/* on != 0: fmm_eval brackets every stage with CUDA events (adds a few microseconds) and
+ * fmm_plan_stats synchronises on the last one. */
+int fmm_plan_set_timing(fmm_plan_t *plan, int on);
+int fmm_plan_stats(fmm_plan_t *plan, fmm_stats_t *stats);
+int fmm_plan_export(fmm_plan_t *plan, fmm_export_t *out);  /* synchronises the stream */
+void fmm_plan_destroy(fmm_plan_t *plan);
+
+/* Number of kernel launches the library has enqueued in this process (bench.py's gpu_launches). */
+int64_t fmm_launch_count(void);
+
+const char *fmm_strerror(int code);
+const char *fmm_last_error(const fmm_plan_t *plan);  /* plan may be NULL: last error of a plan-less call */
+const char *fmm_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* FMM_B200_H */

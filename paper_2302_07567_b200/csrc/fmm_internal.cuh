@@ -1,0 +1,170 @@
+// fmm_internal.cuh -- plan layout, launch bookkeeping and device helpers shared by the
+// kernels of libfmm_b200.so (include/fmm.h).  Nothing here is shared with oracle/.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <stdio.h>
+#include <string.h>
+#include <atomic>
+#include <vector>
+
+#include "../../include/fmm.h"
+
+#define FMM_SM_COUNT 148           // B200: 2 dies x 74 SMs (grids are sized in multiples of this)
+#define FMM_EPS0 8.8541878128e-12  // F/m, CODATA 2018 (eq. (3.1))
+#define FMM_C0 299792458.0         // m/s
+#define FMM_PI 3.14159265358979323846
+
+extern std::atomic<int64_t> g_fmm_launches;
+#define FMM_COUNT_LAUNCH() (g_fmm_launches.fetch_add(1, std::memory_order_relaxed))
+
+struct fmm_ctx {  // allocator + stream + error text, shared by plans and plan-less calls
+    fmm_alloc_fn alloc;
+    fmm_free_fn free_;
+    void *user;
+    cudaStream_t stream;
+    char err[256];
+    int64_t bytes;
+    std::vector<void *> owned;
+    std::vector<size_t> owned_bytes;
+};
+
+void *ctx_alloc(fmm_ctx *c, size_t bytes);  // NULL on failure (err set)
+void ctx_free(fmm_ctx *c, void *p);
+void ctx_free_all(fmm_ctx *c);
+int ctx_cuda_fail(fmm_ctx *c, cudaError_t e, const char *what);
+#define FMM_CUDA(c, call)                                                  \
+    do {                                                                   \
+        cudaError_t e__ = (call);                                          \
+        if (e__ != cudaSuccess) return ctx_cuda_fail((c), e__, #call);     \
+    } while (0)
+#define FMM_LAUNCH_CHECK(c, name)                                          \
+    do {                                                                   \
+        FMM_COUNT_LAUNCH();                                                \
+        cudaError_t e__ = cudaGetLastError();                              \
+        if (e__ != cudaSuccess) return ctx_cuda_fail((c), e__, name);      \
+    } while (0)
+#define FMM_TRY(expr)                    \
+    do {                                 \
+        int rc__ = (expr);               \
+        if (rc__ != FMM_OK) return rc__; \
+    } while (0)
+
+enum { EV_P2M = 0, EV_M2M, EV_M2L, EV_L2L, EV_P2P, EV_L2P, EV_END, EV_COUNT };
+
+struct fmm_plan {
+    fmm_ctx ctx;
+    int64_t N;
+    int n, n1, P, N0, kappa;
+    int64_t nodes, leaves;
+    double theta, gamma_bar, gamma_bar_param;
+    uint32_t flags;
+    // particles in tree order (SoA), source weights w0 = q gamma, w1..3 = q p
+    double *tx, *ty, *tz, *w0, *w1, *w2, *w3;
+    int32_t *perm;          // [N] tree position -> caller index
+    // nodes, heap index 1..nodes (entry 0 unused)
+    int32_t *node_lo;       // [nodes+2] range start; node_hi(i) stored separately
+    int32_t *node_hi;
+    double *bbox;           // [nodes+1][6]
+    double *node_geo;       // [nodes+1][4] : r^2 (Alg 5.6 squared), cx, cy, cz (box centres)
+    // interaction lists, CSR by target node id (offset arrays indexed by node id, length nodes+2)
+    int32_t *p2p_off, *p2p_src, *m2l_off, *m2l_src;
+    int64_t n_p2p, n_m2l, cap_p2p, cap_m2l;
+    int64_t p2p_pairs, m2l_pairs;
+    int32_t *p2p_order, *m2l_order;  // target ids sorted by descending work (LPT block order)
+    int32_t n_p2p_targets, n_m2l_targets;
+    // expansions
+    double *M;              // [nodes+1][P][4]
+    double *L;              // [nodes+1][P][6]
+    double *near_;          // [6][N] tree order, P2P result
+    // timing
+    int timing;
+    cudaEvent_t ev[EV_COUNT];
+    cudaEvent_t ev_plan[3];
+    int ev_valid;
+    float ms_tree, ms_lists;
+};
+
+// ---- kernels_tree.cu ----------------------------------------------------------------
+int tree_gamma_bar(fmm_ctx *c, int64_t N, const double *px, const double *py, const double *pz,
+                   double *gamma_bar_out /* host */);
+int tree_build(fmm_plan *p, const fmm_particles_t *in);
+// ---- kernels_dtt.cu -----------------------------------------------------------------
+int dtt_build_lists(fmm_plan *p);
+// ---- kernels_interp.cu --------------------------------------------------------------
+int interp_p2m(fmm_plan *p);
+int interp_m2m(fmm_plan *p);
+int interp_l2l(fmm_plan *p);
+int interp_l2p_finalize(fmm_plan *p, double *Ex, double *Ey, double *Ez, double *Bx, double *By, double *Bz);
+// ---- kernels_pairs.cu ---------------------------------------------------------------
+int pairs_p2p(fmm_plan *p);
+int pairs_m2l(fmm_plan *p);
+int pairs_direct(fmm_ctx *c, int64_t N, const double *x, const double *y, const double *z,
+                 const double *w0, const double *w1, const double *w2, const double *w3,
+                 double gamma_bar, int raw, int64_t nt, const int64_t *tidx,
+                 double *Ex, double *Ey, double *Ez, double *Bx, double *By, double *Bz);
+int pairs_source_weights(fmm_ctx *c, int64_t N, const double *px, const double *py, const double *pz,
+                         const double *q, double q_scalar, double *w0, double *w1, double *w2, double *w3);
+// ---- sort.cu --------------------------------------------------------------------------
+// Stable LSD radix sort of (key, value) pairs on bits [bit_lo, bit_hi) of the key.  keys/vals are
+// overwritten with the sorted sequence; tmp_* are scratch of the same length.
+int sort_pairs_u64(fmm_ctx *c, uint64_t *keys, uint32_t *vals, uint64_t *tmp_keys, uint32_t *tmp_vals,
+                   int64_t n, int bit_lo, int bit_hi);
+int scan_exclusive_i32(fmm_ctx *c, const int32_t *in, int32_t *out, int64_t n);  // out may alias in
+
+#ifdef __CUDACC__
+// ---- device helpers -------------------------------------------------------------------
+
+// w = D^{-3/2} for D > 0, and 0 for D == 0 (reading G17: a coincident pair contributes nothing,
+// which also removes i == j).  One MUFU.RSQ64H seed y0 (relative error ~2^-20) and one cubic
+// correction of y0^3:  D y0^2 = 1 - e  =>  D^{-3/2} = y0^3 (1-e)^{-3/2} = y0^3 (1 + 3/2 e + 15/8 e^2 + O(e^3)),
+// truncation 35/16 e^3 < 1e-17 relative.  6 FP64 instructions.  Subnormal D is flushed to 0 by the seed.
+__device__ __forceinline__ double inv_r3(double D)
+{
+    double y0;
+    asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y0) : "d"(D));
+    int hi = __double2hiint(y0);
+    hi = (hi == 0x7ff00000) ? 0 : hi;          // D == 0 -> seed +inf -> 0 (integer pipe, no FP64 slot)
+    y0 = __hiloint2double(hi, 0);
+    double t = y0 * y0;
+    double e = fma(-D, t, 1.0);
+    double c = y0 * t;
+    double p = fma(1.875, e, 1.5);
+    double pe = p * e;
+    return fma(c, pe, c);
+}
+
+// One source (x, y, z, m0..m3) acting on one target: eq. (3.1)-(3.2) without prefactors,
+// E += m0 g, B += (m1,m2,m3) x g.  25 FP64 instructions.
+__device__ __forceinline__ void pair_accumulate(double xt, double yt, double zt, double g2,
+                                                double xs, double ys, double zs,
+                                                double m0, double m1, double m2, double m3,
+                                                double &ex, double &ey, double &ez,
+                                                double &bx, double &by, double &bz)
+{
+    double dx = xt - xs, dy = yt - ys, dz = zt - zs;
+    double D = dx * dx;
+    D = fma(dy, dy, D);
+    D = fma(g2 * dz, dz, D);
+    double w = inv_r3(D);
+    double gx = w * dx, gy = w * dy, gz = w * dz;
+    ex = fma(m0, gx, ex);
+    ey = fma(m0, gy, ey);
+    ez = fma(m0, gz, ez);
+    bx = fma(m2, gz, bx);
+    bx = fma(-m3, gy, bx);
+    by = fma(m3, gx, by);
+    by = fma(-m1, gz, by);
+    bz = fma(m1, gy, bz);
+    bz = fma(-m2, gx, bz);
+}
+
+// Reference Chebyshev points of the second kind on [-1,1] (reading I-1): c_k = cos(k pi / n)
+// written as sin(pi (n - 2k) / (2n)) so that c_k = -c_{n-k}; c_0 = 1, c_n = -1 exactly.
+__device__ __forceinline__ double cheb_ref(int n, int k)
+{
+    if (k == 0) return 1.0;
+    if (k == n) return -1.0;
+    return sin(FMM_PI * (double)(n - 2 * k) / (double)(2 * n));
+}
+#endif

@@ -1,0 +1,204 @@
+// kernels_dtt.cu -- step a3: dual tree traversal (Alg 9.1; same logic as Alg 5.11,
+// PAPER.md:400-435) with the stretched admissibility condition of Alg 5.6-5.8 (PAPER.md:337-366,
+// eq. (4.3)), emitting the two interaction lists, then sorting them by
+// (target, source) into CSR form (readings D-4, G20).
+//
+// The recursion is run level-synchronously: a frontier of (target, source) node pairs is
+// classified by one kernel per step (P2P / M2L / split), children are appended to the next frontier
+// through INTEGER atomic counters (order inside a frontier is irrelevant: the lists are sorted
+// afterwards, so the result is unique and bit-reproducible).  No host round trip until the final
+// list lengths are read back.
+#include "fmm_internal.cuh"
+
+struct dtt_counters {           // device
+    unsigned int n_p2p, n_m2l, overflow, pad;
+    unsigned int n_front[72];   // frontier sizes per step (at most 2*kappa+2 steps)
+};
+
+__global__ void dtt_init(dtt_counters *cnt, uint64_t *front0)
+{
+    if (threadIdx.x == 0 && blockIdx.x == 0) {
+        cnt->n_p2p = cnt->n_m2l = cnt->overflow = cnt->pad = 0;
+        for (int k = 0; k < 72; ++k) cnt->n_front[k] = 0;
+        cnt->n_front[0] = 1;
+        front0[0] = (1ull << 32) | 1ull;  // (root, root)
+    }
+}
+
+__global__ void __launch_bounds__(256) dtt_step(int step, int leaves, double gamma_bar, double theta2,
+                                                const int32_t *__restrict__ node_lo, const int32_t *__restrict__ node_hi,
+                                                const double *__restrict__ geo, const uint64_t *__restrict__ front_in,
+                                                uint64_t *__restrict__ front_out, unsigned int cap_front,
+                                                uint64_t *__restrict__ p2p, unsigned int cap_p2p,
+                                                uint64_t *__restrict__ m2l, unsigned int cap_m2l,
+                                                int key_shift, dtt_counters *cnt)
+{
+    unsigned int nin = cnt->n_front[step];
+    if (nin > cap_front) nin = cap_front;
+    for (unsigned int k = blockIdx.x * blockDim.x + threadIdx.x; k < nin; k += gridDim.x * blockDim.x) {
+        uint64_t pr = front_in[k];
+        int i = (int)(pr >> 32), j = (int)(pr & 0xffffffffu);  // i = target, j = source
+        if (node_hi[i] <= node_lo[i] || node_hi[j] <= node_lo[j]) continue;  // empty cluster
+        bool leaf_i = i >= leaves, leaf_j = j >= leaves;
+        if (leaf_i && leaf_j) {  // D-1: leaf-leaf -> P2P, no admissibility test
+            unsigned int pos = atomicAdd(&cnt->n_p2p, 1u);
+            if (pos < cap_p2p) p2p[pos] = ((uint64_t)i << key_shift) | (uint64_t)j; else cnt->overflow = 1;
+            continue;
+        }
+        // D-2: Alg 5.6-5.8 squared; every product and sum rounded separately, in this order
+        const double *gi = geo + 4 * (int64_t)i, *gj = geo + 4 * (int64_t)j;
+        double ri = gi[0], rj = gj[0];
+        double ex = __dmul_rn(1.0, __dsub_rn(gi[1], gj[1]));
+        double ey = __dmul_rn(1.0, __dsub_rn(gi[2], gj[2]));
+        double ez = __dmul_rn(gamma_bar, __dsub_rn(gi[3], gj[3]));
+        double d2 = __dadd_rn(__dadd_rn(__dmul_rn(ex, ex), __dmul_rn(ey, ey)), __dmul_rn(ez, ez));
+        double rmax = (ri > rj) ? ri : rj;
+        if (rmax < __dmul_rn(theta2, d2)) {  // admissible -> M2L
+            unsigned int pos = atomicAdd(&cnt->n_m2l, 1u);
+            if (pos < cap_m2l) m2l[pos] = ((uint64_t)i << key_shift) | (uint64_t)j; else cnt->overflow = 1;
+            continue;
+        }
+        // D-3: which side to split
+        bool split_target = leaf_i ? false : (leaf_j ? true : (ri > rj));
+        unsigned int pos = atomicAdd(&cnt->n_front[step + 1], 2u);
+        if (pos + 1 < cap_front) {
+            if (split_target) {
+                front_out[pos] = ((uint64_t)(2 * i) << 32) | (uint64_t)j;
+                front_out[pos + 1] = ((uint64_t)(2 * i + 1) << 32) | (uint64_t)j;
+            } else {
+                front_out[pos] = ((uint64_t)i << 32) | (uint64_t)(2 * j);
+                front_out[pos + 1] = ((uint64_t)i << 32) | (uint64_t)(2 * j + 1);
+            }
+        } else {
+            cnt->overflow = 1;
+        }
+    }
+}
+
+// sorted keys (target << shift | source) -> CSR: off[t] = first position with target >= t
+__global__ void csr_from_sorted(const uint64_t *__restrict__ keys, int64_t n, int key_shift, int nodes,
+                                int32_t *__restrict__ off /* [nodes+2] */, int32_t *__restrict__ src)
+{
+    int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (k > n) return;
+    uint64_t mask = (1ull << key_shift) - 1ull;
+    int t_prev = (k == 0) ? -1 : (int)(keys[k - 1] >> key_shift);
+    int t_cur = (k == n) ? nodes + 1 : (int)(keys[k] >> key_shift);
+    for (int t = t_prev + 1; t <= t_cur; ++t) off[t] = (int32_t)k;
+    if (k < n) src[k] = (int32_t)(keys[k] & mask);
+}
+
+// LPT block order: targets by descending work (number of source clusters x their sizes)
+__global__ void list_work_keys(int first, int count, const int32_t *__restrict__ off, const int32_t *__restrict__ src,
+                               const int32_t *__restrict__ node_lo, const int32_t *__restrict__ node_hi, int by_size,
+                               uint64_t *__restrict__ keys, uint32_t *__restrict__ vals, unsigned long long *__restrict__ total)
+{
+    int k = blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= count) return;
+    int t = first + k;
+    unsigned long long work = 0;
+    if (by_size) {
+        unsigned long long nt = (unsigned long long)(node_hi[t] - node_lo[t]);
+        for (int e = off[t]; e < off[t + 1]; ++e) work += nt * (unsigned long long)(node_hi[src[e]] - node_lo[src[e]]);
+        atomicAdd(total, work);
+    } else {
+        work = (unsigned long long)(off[t + 1] - off[t]);
+    }
+    if (work > 0xffffffffull) work = 0xffffffffull;
+    keys[k] = 0xffffffffull - work;  // ascending sort of this = descending work
+    vals[k] = (uint32_t)t;
+}
+
+__global__ void copy_u32_to_i32(int n, const uint32_t *__restrict__ a, int32_t *__restrict__ b)
+{
+    int k = blockIdx.x * blockDim.x + threadIdx.x;
+    if (k < n) b[k] = (int32_t)a[k];
+}
+
+static int make_order(fmm_plan *p, int first, int count, const int32_t *off, const int32_t *src, int by_size,
+                      int32_t *order_out, unsigned long long *total_dev)
+{
+    fmm_ctx *c = &p->ctx;
+    uint64_t *keys = (uint64_t *)ctx_alloc(c, sizeof(uint64_t) * count);
+    uint64_t *tkeys = (uint64_t *)ctx_alloc(c, sizeof(uint64_t) * count);
+    uint32_t *vals = (uint32_t *)ctx_alloc(c, sizeof(uint32_t) * count);
+    uint32_t *tvals = (uint32_t *)ctx_alloc(c, sizeof(uint32_t) * count);
+    if (!keys || !tkeys || !vals || !tvals) return FMM_ENOMEM;
+    list_work_keys<<<(count + 255) / 256, 256, 0, c->stream>>>(first, count, off, src, p->node_lo, p->node_hi, by_size, keys, vals, total_dev);
+    FMM_LAUNCH_CHECK(c, "list_work_keys");
+    FMM_TRY(sort_pairs_u64(c, keys, vals, tkeys, tvals, count, 0, 32));
+    copy_u32_to_i32<<<(count + 255) / 256, 256, 0, c->stream>>>(count, vals, order_out);
+    FMM_LAUNCH_CHECK(c, "copy_u32_to_i32");
+    ctx_free(c, keys); ctx_free(c, tkeys); ctx_free(c, vals); ctx_free(c, tvals);
+    return FMM_OK;
+}
+
+int dtt_build_lists(fmm_plan *p)
+{
+    fmm_ctx *c = &p->ctx;
+    cudaStream_t st = c->stream;
+    const int key_shift = p->kappa + 2;  // node ids < 2^(kappa+1)
+    const int nsteps = 2 * p->kappa + 1;
+    dtt_counters *cnt = (dtt_counters *)ctx_alloc(c, sizeof(dtt_counters) + sizeof(unsigned long long));
+    if (!cnt) return FMM_ENOMEM;
+    unsigned long long *total_dev = (unsigned long long *)(cnt + 1);
+    dtt_counters h;
+    int64_t cap = p->leaves * 128;  // first guess; doubled until nothing overflows
+    if (cap < 4096) cap = 4096;
+    uint64_t *f0 = NULL, *f1 = NULL, *kp2p = NULL, *km2l = NULL;
+    for (int attempt = 0;; ++attempt) {
+        if (cap >= ((int64_t)1 << 31)) return FMM_EOVERFLOW;
+        f0 = (uint64_t *)ctx_alloc(c, sizeof(uint64_t) * cap);
+        f1 = (uint64_t *)ctx_alloc(c, sizeof(uint64_t) * cap);
+        kp2p = (uint64_t *)ctx_alloc(c, sizeof(uint64_t) * cap);
+        km2l = (uint64_t *)ctx_alloc(c, sizeof(uint64_t) * cap);
+        if (!f0 || !f1 || !kp2p || !km2l) return FMM_ENOMEM;
+        dtt_init<<<1, 32, 0, st>>>(cnt, f0);
+        FMM_LAUNCH_CHECK(c, "dtt_init");
+        uint64_t *fin = f0, *fout = f1;
+        for (int step = 0; step < nsteps; ++step) {
+            dtt_step<<<2 * FMM_SM_COUNT, 256, 0, st>>>(step, (int)p->leaves, p->gamma_bar, p->theta * p->theta, p->node_lo, p->node_hi,
+                                                       p->node_geo, fin, fout, (unsigned)cap, kp2p, (unsigned)cap, km2l, (unsigned)cap,
+                                                       key_shift, cnt);
+            FMM_LAUNCH_CHECK(c, "dtt_step");
+            uint64_t *t = fin; fin = fout; fout = t;
+        }
+        FMM_CUDA(c, cudaMemcpyAsync(&h, cnt, sizeof(h), cudaMemcpyDeviceToHost, st));
+        FMM_CUDA(c, cudaStreamSynchronize(st));
+        ctx_free(c, f0); ctx_free(c, f1);
+        if (!h.overflow) break;
+        ctx_free(c, kp2p); ctx_free(c, km2l);
+        cap *= 4;
+    }
+    p->n_p2p = h.n_p2p;
+    p->n_m2l = h.n_m2l;
+
+    // sort by (target, source), then CSR
+    int64_t nmax = (p->n_p2p > p->n_m2l) ? p->n_p2p : p->n_m2l;
+    uint64_t *tkeys = (uint64_t *)ctx_alloc(c, sizeof(uint64_t) * (nmax > 0 ? nmax : 1));
+    if (!tkeys) return FMM_ENOMEM;
+    if (p->p2p_src) ctx_free(c, p->p2p_src);
+    if (p->m2l_src) ctx_free(c, p->m2l_src);
+    p->p2p_src = (int32_t *)ctx_alloc(c, sizeof(int32_t) * (p->n_p2p > 0 ? p->n_p2p : 1));
+    p->m2l_src = (int32_t *)ctx_alloc(c, sizeof(int32_t) * (p->n_m2l > 0 ? p->n_m2l : 1));
+    if (!p->p2p_src || !p->m2l_src) return FMM_ENOMEM;
+    FMM_TRY(sort_pairs_u64(c, kp2p, NULL, tkeys, NULL, p->n_p2p, 0, 2 * key_shift));
+    FMM_TRY(sort_pairs_u64(c, km2l, NULL, tkeys, NULL, p->n_m2l, 0, 2 * key_shift));
+    csr_from_sorted<<<(unsigned)((p->n_p2p + 256) / 256), 256, 0, st>>>(kp2p, p->n_p2p, key_shift, (int)p->nodes, p->p2p_off, p->p2p_src);
+    FMM_LAUNCH_CHECK(c, "csr_from_sorted");
+    csr_from_sorted<<<(unsigned)((p->n_m2l + 256) / 256), 256, 0, st>>>(km2l, p->n_m2l, key_shift, (int)p->nodes, p->m2l_off, p->m2l_src);
+    FMM_LAUNCH_CHECK(c, "csr_from_sorted");
+    ctx_free(c, tkeys); ctx_free(c, kp2p); ctx_free(c, km2l);
+
+    // block orders (descending work) and evaluation counts
+    FMM_CUDA(c, cudaMemsetAsync(total_dev, 0, sizeof(unsigned long long), st));
+    FMM_TRY(make_order(p, (int)p->leaves, (int)p->leaves, p->p2p_off, p->p2p_src, 1, p->p2p_order, total_dev));
+    FMM_TRY(make_order(p, 1, (int)p->nodes, p->m2l_off, p->m2l_src, 0, p->m2l_order, total_dev));
+    unsigned long long total_h = 0;
+    FMM_CUDA(c, cudaMemcpyAsync(&total_h, total_dev, sizeof(total_h), cudaMemcpyDeviceToHost, st));
+    FMM_CUDA(c, cudaStreamSynchronize(st));
+    p->p2p_pairs = (int64_t)total_h;
+    p->m2l_pairs = p->n_m2l * (int64_t)p->P * (int64_t)p->P;
+    ctx_free(c, cnt);
+    return FMM_OK;
+}

@@ -1,0 +1,365 @@
+// kernels_interp.cu -- the interpolation passes of the hot path:
+//   a4  P2M  Alg 5.3 / eq. (2.4)
+//   a5  M2M  Alg 5.4 / eq. (2.9), level by level upward (Alg 5.5)
+//   a8  L2L  Alg 5.13 / eq. (2.11), level by level downward (Alg 5.15)
+//   a9  L2P  Alg 5.14 / eq. (2.10)  + a10 prefactors of eq. (3.1) and the
+//       scatter back to the caller's particle order
+// Barycentric Lagrange basis on Chebyshev points of the second kind (readings I-1..I-5).
+// M2M / L2L use the tensor-product structure: three 1-D contractions with (n+1)x(n+1) transfer
+// matrices instead of the (n+1)^6 form.  All of it is < 2 % of the run time; the passes are
+// HBM / launch-latency-bound (M2M, L2L) or small FP64 loops (P2M, L2P).
+#include "fmm_internal.cuh"
+
+struct cheb_t {
+    double c[FMM_MAX_ORDER + 1];
+};
+
+static cheb_t host_cheb(int n)
+{
+    cheb_t t;
+    memset(&t, 0, sizeof(t));
+    for (int k = 0; k <= n; ++k) t.c[k] = sin(FMM_PI * (double)(n - 2 * k) / (double)(2 * n));  // I-1
+    t.c[0] = 1.0;
+    t.c[n] = -1.0;
+    return t;
+}
+
+// I-3: xi_k = (a+b)/2 + (b-a)/2 c_k, product and sum rounded separately
+__device__ __forceinline__ double node_point(double mid, double half, double ck) { return __dadd_rn(mid, __dmul_rn(half, ck)); }
+
+// I-2, I-4: l_k(x) = (w_k/(x-xi_k)) / sum_m (w_m/(x-xi_m)), w_k = (-1)^k delta_k, delta_0 = delta_n = 1/2;
+// exact hit x == xi_k: l_k = 1 for the first such k, 0 elsewhere.  out has stride `stride`.
+__device__ __forceinline__ void basis_1d(int n, const cheb_t &ch, double a, double b, double x, double *out, int stride)
+{
+    double mid = __dmul_rn(__dadd_rn(a, b), 0.5), half = __dmul_rn(__dsub_rn(b, a), 0.5);
+    int hit = -1;
+    double S = 0.0;
+    for (int k = 0; k <= n; ++k) {
+        double xi = node_point(mid, half, ch.c[k]);
+        double d = x - xi;
+        if (d == 0.0 && hit < 0) hit = k;
+        double wk = (k == 0 || k == n) ? 0.5 : 1.0;
+        if (k & 1) wk = -wk;
+        double t = wk / d;
+        out[k * stride] = t;
+        S += t;
+    }
+    if (hit >= 0) {
+        for (int k = 0; k <= n; ++k) out[k * stride] = (k == hit) ? 1.0 : 0.0;
+    } else {
+        for (int k = 0; k <= n; ++k) out[k * stride] = out[k * stride] / S;
+    }
+}
+
+// ---------------------------------------------------------------------------------------
+// a4: P2M.  One block per leaf; thread nu accumulates M_{S,nu} = sum_j l_nu(x_j) m_j over the leaf's
+// particles in tree order.  The 1-D basis values of a chunk of particles are staged in shared memory.
+// ---------------------------------------------------------------------------------------
+#define P2M_THREADS 256
+#define P2M_CHUNK 128
+
+__global__ void __launch_bounds__(P2M_THREADS) p2m_kernel(int n, cheb_t ch, int leaves, const int32_t *__restrict__ node_lo,
+                                                          const int32_t *__restrict__ node_hi, const double *__restrict__ bbox,
+                                                          const double *__restrict__ tx, const double *__restrict__ ty,
+                                                          const double *__restrict__ tz, const double *__restrict__ w0,
+                                                          const double *__restrict__ w1, const double *__restrict__ w2,
+                                                          const double *__restrict__ w3, double *__restrict__ M)
+{
+    extern __shared__ double sm[];
+    const int n1 = n + 1, P = n1 * n1 * n1;
+    double *bas = sm;                            // [3][n1][P2M_CHUNK]
+    double *wts = sm + 3 * n1 * P2M_CHUNK;       // [4][P2M_CHUNK]
+    int node = leaves + blockIdx.x;
+    int lo = node_lo[node], hi = node_hi[node];
+    const double *bb = bbox + 6 * (int64_t)node;
+    double *Mn = M + 4 * (int64_t)P * node;
+    for (int nu0 = 0; nu0 < P; nu0 += P2M_THREADS) {
+        int nu = nu0 + threadIdx.x;
+        int a = nu / (n1 * n1), b = (nu / n1) % n1, c3 = nu % n1;
+        double acc0 = 0.0, acc1 = 0.0, acc2 = 0.0, acc3 = 0.0;
+        for (int j0 = lo; j0 < hi; j0 += P2M_CHUNK) {
+            int cnt = min(P2M_CHUNK, hi - j0);
+            __syncthreads();
+            for (int t = threadIdx.x; t < 3 * cnt; t += P2M_THREADS) {
+                int g = t / cnt, jj = t - g * cnt;
+                const double *coord = (g == 0) ? tx : (g == 1) ? ty : tz;
+                basis_1d(n, ch, bb[g], bb[3 + g], coord[j0 + jj], bas + (size_t)g * n1 * P2M_CHUNK + jj, P2M_CHUNK);
+            }
+            for (int t = threadIdx.x; t < cnt; t += P2M_THREADS) {
+                wts[t] = w0[j0 + t];
+                wts[P2M_CHUNK + t] = w1[j0 + t];
+                wts[2 * P2M_CHUNK + t] = w2[j0 + t];
+                wts[3 * P2M_CHUNK + t] = w3[j0 + t];
+            }
+            __syncthreads();
+            if (nu < P) {
+                const double *la = bas + (size_t)a * P2M_CHUNK, *lb = bas + (size_t)(n1 + b) * P2M_CHUNK,
+                             *lc = bas + (size_t)(2 * n1 + c3) * P2M_CHUNK;
+                for (int jj = 0; jj < cnt; ++jj) {
+                    double l = la[jj] * lb[jj] * lc[jj];
+                    acc0 = fma(l, wts[jj], acc0);
+                    acc1 = fma(l, wts[P2M_CHUNK + jj], acc1);
+                    acc2 = fma(l, wts[2 * P2M_CHUNK + jj], acc2);
+                    acc3 = fma(l, wts[3 * P2M_CHUNK + jj], acc3);
+                }
+            }
+        }
+        if (nu < P) {
+            double *m = Mn + 4 * (int64_t)nu;
+            m[0] = acc0; m[1] = acc1; m[2] = acc2; m[3] = acc3;
+        }
+    }
+}
+
+// ---------------------------------------------------------------------------------------
+// 1-D transfer matrices T_g[k][k'] = l_{S,k}(xi_{S',k'}) on the three axes (S = parent, S' = child)
+// ---------------------------------------------------------------------------------------
+__device__ __forceinline__ void transfer_matrices(int n, const cheb_t &ch, const double *bS, const double *bC, double *T /* [3][n1][n1] */)
+{
+    const int n1 = n + 1;
+    for (int t = threadIdx.x; t < 3 * n1; t += blockDim.x) {
+        int g = t / n1, kc = t - g * n1;
+        double mid = __dmul_rn(__dadd_rn(bC[g], bC[3 + g]), 0.5), half = __dmul_rn(__dsub_rn(bC[3 + g], bC[g]), 0.5);
+        double xi = node_point(mid, half, ch.c[kc]);
+        basis_1d(n, ch, bS[g], bS[3 + g], xi, T + (size_t)g * n1 * n1 + kc, n1);  // column kc
+    }
+}
+
+// ---------------------------------------------------------------------------------------
+// a5: M2M for one level.  One block per parent; for each non-empty child three 1-D contractions:
+//   M_S[a,b,c] += sum_{a',b',c'} Tx[a][a'] Ty[b][b'] Tz[c][c'] M_S'[a',b',c']
+// ---------------------------------------------------------------------------------------
+#define XFER_THREADS 256
+
+__global__ void __launch_bounds__(XFER_THREADS) m2m_kernel(int n, cheb_t ch, int first, const int32_t *__restrict__ node_lo,
+                                                           const int32_t *__restrict__ node_hi, const double *__restrict__ bbox,
+                                                           double *__restrict__ M)
+{
+    extern __shared__ double sm[];
+    const int n1 = n + 1, P = n1 * n1 * n1, P4 = 4 * P;
+    double *T = sm;                   // [3][n1][n1]
+    double *A = sm + 3 * n1 * n1;     // [P][4]
+    double *B = A + P4;               // [P][4]
+    int S = first + blockIdx.x;
+    double *MS = M + (int64_t)P4 * S;
+    // parent accumulators live in registers across the two children: element e = threadIdx.x + k*blockDim
+    for (int e0 = 0; e0 < P4; e0 += XFER_THREADS * 8) {
+        // (P4 <= 8788; with 256 threads at most 35 elements per thread -> process in slabs of 8 per thread)
+        double acc[8];
+#pragma unroll
+        for (int k = 0; k < 8; ++k) acc[k] = 0.0;
+        for (int child = 0; child < 2; ++child) {
+            int C = 2 * S + child;
+            if (node_hi[C] <= node_lo[C]) continue;  // uniform per block
+            __syncthreads();
+            transfer_matrices(n, ch, bbox + 6 * (int64_t)S, bbox + 6 * (int64_t)C, T);
+            const double *MC = M + (int64_t)P4 * C;
+            for (int e = threadIdx.x; e < P4; e += XFER_THREADS) A[e] = MC[e];
+            __syncthreads();
+            const double *Tx = T, *Ty = T + n1 * n1, *Tz = T + 2 * n1 * n1;
+            // z: B[a',b',c] = sum_c' Tz[c][c'] A[a',b',c']
+            for (int e = threadIdx.x; e < P4; e += XFER_THREADS) {
+                int f = e & 3, nu = e >> 2, c3 = nu % n1, ab = nu / n1;
+                double s = 0.0;
+                for (int k = 0; k < n1; ++k) s = fma(Tz[c3 * n1 + k], A[4 * (ab * n1 + k) + f], s);
+                B[e] = s;
+            }
+            __syncthreads();
+            // y: A[a',b,c] = sum_b' Ty[b][b'] B[a',b',c]
+            for (int e = threadIdx.x; e < P4; e += XFER_THREADS) {
+                int f = e & 3, nu = e >> 2, c3 = nu % n1, b = (nu / n1) % n1, a = nu / (n1 * n1);
+                double s = 0.0;
+                for (int k = 0; k < n1; ++k) s = fma(Ty[b * n1 + k], B[4 * ((a * n1 + k) * n1 + c3) + f], s);
+                A[e] = s;
+            }
+            __syncthreads();
+            // x: out[a,b,c] = sum_a' Tx[a][a'] A[a',b,c]
+#pragma unroll
+            for (int k8 = 0; k8 < 8; ++k8) {
+                int e = e0 + threadIdx.x + k8 * XFER_THREADS;
+                if (e < P4) {
+                    int f = e & 3, nu = e >> 2, bc = nu % (n1 * n1), a = nu / (n1 * n1);
+                    double s = 0.0;
+                    for (int k = 0; k < n1; ++k) s = fma(Tx[a * n1 + k], A[4 * (k * n1 * n1 + bc) + f], s);
+                    acc[k8] += s;
+                }
+            }
+        }
+#pragma unroll
+        for (int k8 = 0; k8 < 8; ++k8) {
+            int e = e0 + threadIdx.x + k8 * XFER_THREADS;
+            if (e < P4) MS[e] = acc[k8];
+        }
+    }
+}
+
+// ---------------------------------------------------------------------------------------
+// a8: L2L for one level.  One block per child S' (parent S = S'/2):
+//   L_S'[a',b',c'] += sum_{a,b,c} Tx[a][a'] Ty[b][b'] Tz[c][c'] L_S[a,b,c]
+// ---------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(XFER_THREADS) l2l_kernel(int n, cheb_t ch, int first, const int32_t *__restrict__ node_lo,
+                                                           const int32_t *__restrict__ node_hi, const double *__restrict__ bbox,
+                                                           double *__restrict__ L)
+{
+    extern __shared__ double sm[];
+    const int n1 = n + 1, P = n1 * n1 * n1, P6 = 6 * P;
+    double *T = sm;
+    double *A = sm + 3 * n1 * n1;  // [P][6]
+    double *B = A + P6;
+    int C = first + blockIdx.x, S = C >> 1;
+    if (node_hi[C] <= node_lo[C]) return;
+    transfer_matrices(n, ch, bbox + 6 * (int64_t)S, bbox + 6 * (int64_t)C, T);
+    const double *LS = L + (int64_t)P6 * S;
+    double *LC = L + (int64_t)P6 * C;
+    for (int e = threadIdx.x; e < P6; e += XFER_THREADS) A[e] = LS[e];
+    __syncthreads();
+    const double *Tx = T, *Ty = T + n1 * n1, *Tz = T + 2 * n1 * n1;
+    // z: B[a,b,c'] = sum_c Tz[c][c'] A[a,b,c]
+    for (int e = threadIdx.x; e < P6; e += XFER_THREADS) {
+        int f = e % 6, nu = e / 6, c3 = nu % n1, ab = nu / n1;
+        double s = 0.0;
+        for (int k = 0; k < n1; ++k) s = fma(Tz[k * n1 + c3], A[6 * (ab * n1 + k) + f], s);
+        B[e] = s;
+    }
+    __syncthreads();
+    // y: A[a,b',c'] = sum_b Ty[b][b'] B[a,b,c']
+    for (int e = threadIdx.x; e < P6; e += XFER_THREADS) {
+        int f = e % 6, nu = e / 6, c3 = nu % n1, b = (nu / n1) % n1, a = nu / (n1 * n1);
+        double s = 0.0;
+        for (int k = 0; k < n1; ++k) s = fma(Ty[k * n1 + b], B[6 * ((a * n1 + k) * n1 + c3) + f], s);
+        A[e] = s;
+    }
+    __syncthreads();
+    // x: L_S'[a',b',c'] += sum_a Tx[a][a'] A[a,b',c']
+    for (int e = threadIdx.x; e < P6; e += XFER_THREADS) {
+        int f = e % 6, nu = e / 6, bc = nu % (n1 * n1), a = nu / (n1 * n1);
+        double s = 0.0;
+        for (int k = 0; k < n1; ++k) s = fma(Tx[k * n1 + a], A[6 * (k * n1 * n1 + bc) + f], s);
+        LC[e] += s;
+    }
+}
+
+// ---------------------------------------------------------------------------------------
+// a9 + a10: L2P, add the near field, prefactors, scatter to caller order.  One block per leaf, one thread
+// per particle; the leaf's local fields sit in shared memory and are read as broadcasts.
+// ---------------------------------------------------------------------------------------
+#define L2P_THREADS 128
+
+__global__ void __launch_bounds__(L2P_THREADS) l2p_kernel(int n, cheb_t ch, int leaves, int N, const int32_t *__restrict__ node_lo,
+                                                          const int32_t *__restrict__ node_hi, const double *__restrict__ bbox,
+                                                          const double *__restrict__ tx, const double *__restrict__ ty,
+                                                          const double *__restrict__ tz, const double *__restrict__ L,
+                                                          const double *__restrict__ near_, const int32_t *__restrict__ perm,
+                                                          double cE, double cB, double *__restrict__ Ex, double *__restrict__ Ey,
+                                                          double *__restrict__ Ez, double *__restrict__ Bx, double *__restrict__ By,
+                                                          double *__restrict__ Bz)
+{
+    extern __shared__ double sm[];
+    const int n1 = n + 1, P = n1 * n1 * n1, P6 = 6 * P;
+    double *Ls = sm;                 // [P][6]
+    double *bas = sm + P6;           // [3][n1][L2P_THREADS]
+    int node = leaves + blockIdx.x;
+    int lo = node_lo[node], hi = node_hi[node];
+    const double *bb = bbox + 6 * (int64_t)node;
+    const double *Ln = L + (int64_t)P6 * node;
+    for (int e = threadIdx.x; e < P6; e += L2P_THREADS) Ls[e] = Ln[e];
+    __syncthreads();
+    for (int k = lo + threadIdx.x; k < hi; k += L2P_THREADS) {
+        double *lx = bas + threadIdx.x, *ly = lx + n1 * L2P_THREADS, *lz = ly + n1 * L2P_THREADS;
+        basis_1d(n, ch, bb[0], bb[3], tx[k], lx, L2P_THREADS);
+        basis_1d(n, ch, bb[1], bb[4], ty[k], ly, L2P_THREADS);
+        basis_1d(n, ch, bb[2], bb[5], tz[k], lz, L2P_THREADS);
+        double fx[6] = {0, 0, 0, 0, 0, 0};
+        for (int a = 0; a < n1; ++a) {
+            double fy[6] = {0, 0, 0, 0, 0, 0};
+            for (int b = 0; b < n1; ++b) {
+                double fz[6] = {0, 0, 0, 0, 0, 0};
+                const double *row = Ls + 6 * (size_t)((a * n1 + b) * n1);
+                for (int c3 = 0; c3 < n1; ++c3) {
+                    double l = lz[c3 * L2P_THREADS];
+#pragma unroll
+                    for (int f = 0; f < 6; ++f) fz[f] = fma(l, row[6 * c3 + f], fz[f]);
+                }
+                double l = ly[b * L2P_THREADS];
+#pragma unroll
+                for (int f = 0; f < 6; ++f) fy[f] = fma(l, fz[f], fy[f]);
+            }
+            double l = lx[a * L2P_THREADS];
+#pragma unroll
+            for (int f = 0; f < 6; ++f) fx[f] = fma(l, fy[f], fx[f]);
+        }
+        int i = perm[k];
+        // fixed order: near + far, then the prefactors of eq. (3.1)
+        Ex[i] = cE * (near_[k] + fx[0]);
+        Ey[i] = cE * (near_[(size_t)N + k] + fx[1]);
+        Ez[i] = cE * (near_[2 * (size_t)N + k] + fx[2]);
+        Bx[i] = cB * (near_[3 * (size_t)N + k] + fx[3]);
+        By[i] = cB * (near_[4 * (size_t)N + k] + fx[4]);
+        Bz[i] = cB * (near_[5 * (size_t)N + k] + fx[5]);
+    }
+}
+
+// ---------------------------------------------------------------------------------------
+static int set_smem(fmm_ctx *c, const void *fn, size_t bytes)
+{
+    if (bytes > 48 * 1024) FMM_CUDA(c, cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes));
+    return FMM_OK;
+}
+
+int interp_p2m(fmm_plan *p)
+{
+    fmm_ctx *c = &p->ctx;
+    cheb_t ch = host_cheb(p->n);
+    size_t smem = sizeof(double) * (3 * (size_t)p->n1 * P2M_CHUNK + 4 * P2M_CHUNK);
+    FMM_TRY(set_smem(c, (const void *)p2m_kernel, smem));
+    p2m_kernel<<<(unsigned)p->leaves, P2M_THREADS, smem, c->stream>>>(p->n, ch, (int)p->leaves, p->node_lo, p->node_hi, p->bbox,
+                                                                      p->tx, p->ty, p->tz, p->w0, p->w1, p->w2, p->w3, p->M);
+    FMM_LAUNCH_CHECK(c, "p2m_kernel");
+    return FMM_OK;
+}
+
+int interp_m2m(fmm_plan *p)
+{
+    fmm_ctx *c = &p->ctx;
+    cheb_t ch = host_cheb(p->n);
+    size_t smem = sizeof(double) * (3 * (size_t)p->n1 * p->n1 + 8 * (size_t)p->P);
+    FMM_TRY(set_smem(c, (const void *)m2m_kernel, smem));
+    for (int level = p->kappa - 1; level >= 0; --level) {
+        int first = 1 << level;
+        m2m_kernel<<<first, XFER_THREADS, smem, c->stream>>>(p->n, ch, first, p->node_lo, p->node_hi, p->bbox, p->M);
+        FMM_LAUNCH_CHECK(c, "m2m_kernel");
+    }
+    return FMM_OK;
+}
+
+int interp_l2l(fmm_plan *p)
+{
+    fmm_ctx *c = &p->ctx;
+    cheb_t ch = host_cheb(p->n);
+    size_t smem = sizeof(double) * (3 * (size_t)p->n1 * p->n1 + 12 * (size_t)p->P);
+    FMM_TRY(set_smem(c, (const void *)l2l_kernel, smem));
+    for (int level = 1; level <= p->kappa; ++level) {
+        int first = 1 << level;
+        l2l_kernel<<<first, XFER_THREADS, smem, c->stream>>>(p->n, ch, first, p->node_lo, p->node_hi, p->bbox, p->L);
+        FMM_LAUNCH_CHECK(c, "l2l_kernel");
+    }
+    return FMM_OK;
+}
+
+int interp_l2p_finalize(fmm_plan *p, double *Ex, double *Ey, double *Ez, double *Bx, double *By, double *Bz)
+{
+    fmm_ctx *c = &p->ctx;
+    cheb_t ch = host_cheb(p->n);
+    double cE = 1.0, cB = 1.0;
+    if (!(p->flags & FMM_RAW_SUMS)) {  // eq. (3.1)
+        cE = 1.0 / (4.0 * FMM_PI * FMM_EPS0);
+        cB = 1.0 / (4.0 * FMM_PI * FMM_EPS0 * FMM_C0);
+    }
+    size_t smem = sizeof(double) * (6 * (size_t)p->P + 3 * (size_t)p->n1 * L2P_THREADS);
+    FMM_TRY(set_smem(c, (const void *)l2p_kernel, smem));
+    l2p_kernel<<<(unsigned)p->leaves, L2P_THREADS, smem, c->stream>>>(p->n, ch, (int)p->leaves, (int)p->N, p->node_lo, p->node_hi, p->bbox,
+                                                                      p->tx, p->ty, p->tz, p->L, p->near_, p->perm, cE, cB, Ex, Ey, Ez,
+                                                                      Bx, By, Bz);
+    FMM_LAUNCH_CHECK(c, "l2p_kernel");
+    return FMM_OK;
+}

@@ -1,0 +1,459 @@
+// kernels_tree.cu -- steps a0-a2 of the hot path:
+//   a0  mean momentum -> gamma_bar, source weights q gamma, q p
+//   a1  particle order of the balanced cluster tree: mode KD = Alg 5.1/5.2 (PAPER.md:255-289,
+//       App. B) on the array tree of section 8;
+//       mode MORTON_MEDIAN = 63-bit Morton order of the stretched coordinates (DESIGN T-3')
+//   a2  tight bounding boxes, stretched radii and centres (Alg 5.6/5.7)
+// Everything here is integer / compare / min-max work: HBM- and launch-latency-bound.
+#include "fmm_internal.cuh"
+
+// ---------------------------------------------------------------------------------------
+// closed-form node ranges (DESIGN T-2): root [0,N); left child gets ceil(size/2)
+// ---------------------------------------------------------------------------------------
+__host__ __device__ __forceinline__ void node_at_level(int N, int level, int pos, int &node, int &lo, int &hi)
+{
+    lo = 0;
+    hi = N;
+    node = 1;
+    for (int l = 0; l < level; ++l) {
+        int mid = lo + (hi - lo + 1) / 2;
+        if (pos < mid) {
+            hi = mid;
+            node = 2 * node;
+        } else {
+            lo = mid;
+            node = 2 * node + 1;
+        }
+    }
+}
+
+__global__ void node_ranges_kernel(int N, int kappa, int nodes, int32_t *__restrict__ node_lo, int32_t *__restrict__ node_hi)
+{
+    int i = blockIdx.x * blockDim.x + threadIdx.x + 1;  // heap id
+    if (i > nodes) return;
+    int level = 31 - __clz(i);
+    int lo = 0, hi = N;
+    for (int b = level - 1; b >= 0; --b) {
+        int mid = lo + (hi - lo + 1) / 2;
+        if ((i >> b) & 1) lo = mid; else hi = mid;
+    }
+    node_lo[i] = lo;
+    node_hi[i] = hi;
+}
+
+// ---------------------------------------------------------------------------------------
+// a0: deterministic mean momentum (fixed grid, fixed reduction tree)
+// ---------------------------------------------------------------------------------------
+#define RED_BLOCKS (2 * FMM_SM_COUNT)
+#define RED_THREADS 256
+
+__device__ __forceinline__ double block_sum_256(double v, double *sm /* [8] */)
+{
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
+    int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    __syncthreads();
+    if (lane == 0) sm[warp] = v;
+    __syncthreads();
+    double t = 0.0;
+    if (threadIdx.x == 0)
+        for (int w = 0; w < RED_THREADS / 32; ++w) t += sm[w];
+    return t;  // valid in thread 0
+}
+
+__global__ void __launch_bounds__(RED_THREADS) momentum_partial(int64_t N, const double *__restrict__ px, const double *__restrict__ py,
+                                                                const double *__restrict__ pz, double *__restrict__ partial)
+{
+    __shared__ double sm[8];
+    double sx = 0.0, sy = 0.0, sz = 0.0;
+    for (int64_t j = (int64_t)blockIdx.x * RED_THREADS + threadIdx.x; j < N; j += (int64_t)RED_BLOCKS * RED_THREADS) {
+        sx += px[j];
+        sy += py[j];
+        sz += pz[j];
+    }
+    sx = block_sum_256(sx, sm);
+    sy = block_sum_256(sy, sm);
+    sz = block_sum_256(sz, sm);
+    if (threadIdx.x == 0) {
+        partial[3 * blockIdx.x + 0] = sx;
+        partial[3 * blockIdx.x + 1] = sy;
+        partial[3 * blockIdx.x + 2] = sz;
+    }
+}
+
+__global__ void momentum_final(int64_t N, const double *__restrict__ partial, double *__restrict__ out)
+{
+    if (threadIdx.x != 0 || blockIdx.x != 0) return;
+    double sx = 0.0, sy = 0.0, sz = 0.0;
+    for (int b = 0; b < RED_BLOCKS; ++b) {
+        sx += partial[3 * b + 0];
+        sy += partial[3 * b + 1];
+        sz += partial[3 * b + 2];
+    }
+    double mx = sx / (double)N, my = sy / (double)N, mz = sz / (double)N;
+    out[0] = sqrt(1.0 + (mx * mx + my * my + mz * mz));  // gamma_bar^2 = 1 + pbar.pbar
+}
+
+int tree_gamma_bar(fmm_ctx *c, int64_t N, const double *px, const double *py, const double *pz, double *gamma_bar_out)
+{
+    double *partial = (double *)ctx_alloc(c, sizeof(double) * (3 * RED_BLOCKS + 1));
+    if (!partial) return FMM_ENOMEM;
+    momentum_partial<<<RED_BLOCKS, RED_THREADS, 0, c->stream>>>(N, px, py, pz, partial);
+    FMM_LAUNCH_CHECK(c, "momentum_partial");
+    momentum_final<<<1, 32, 0, c->stream>>>(N, partial, partial + 3 * RED_BLOCKS);
+    FMM_LAUNCH_CHECK(c, "momentum_final");
+    FMM_CUDA(c, cudaMemcpyAsync(gamma_bar_out, partial + 3 * RED_BLOCKS, sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+    FMM_CUDA(c, cudaStreamSynchronize(c->stream));
+    ctx_free(c, partial);
+    return FMM_OK;
+}
+
+// ---------------------------------------------------------------------------------------
+// a1, mode KD
+// ---------------------------------------------------------------------------------------
+// total order of doubles as unsigned keys; -0.0 == +0.0 (the oracle compares with <, so they tie)
+__device__ __forceinline__ uint64_t sortable_key(double v)
+{
+    v = v + 0.0;  // -0.0 -> +0.0
+    uint64_t b = (uint64_t)__double_as_longlong(v);
+    return (b >> 63) ? ~b : (b | 0x8000000000000000ull);
+}
+
+__global__ void kd_make_keys(int N, const double *__restrict__ coord, uint64_t *__restrict__ keys, uint32_t *__restrict__ vals)
+{
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= N) return;
+    keys[i] = sortable_key(coord[i]);
+    vals[i] = (uint32_t)i;
+}
+
+__global__ void kd_iota(int N, uint32_t *__restrict__ v)
+{
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < N) v[i] = (uint32_t)i;
+}
+
+// Alg 5.1: split axis = first maximiser of s_k (b_k - a_k) (reading G9).  The lists
+// are sorted by coordinate inside every node segment, so the bounding box is read off the segment ends.
+__global__ void kd_choose_axis(int N, int level, const double *__restrict__ x, const double *__restrict__ y, const double *__restrict__ z,
+                               const uint32_t *__restrict__ LX, const uint32_t *__restrict__ LY, const uint32_t *__restrict__ LZ,
+                               double gamma_bar, int8_t *__restrict__ axis /* [2^level] */)
+{
+    int k = blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= (1 << level)) return;
+    int lo = 0, hi = N;
+    for (int b = level - 1; b >= 0; --b) {
+        int mid = lo + (hi - lo + 1) / 2;
+        if ((k >> b) & 1) lo = mid; else hi = mid;
+    }
+    int a = 0;
+    if (hi > lo) {
+        double ex = __dmul_rn(1.0, __dsub_rn(x[LX[hi - 1]], x[LX[lo]]));
+        double ey = __dmul_rn(1.0, __dsub_rn(y[LY[hi - 1]], y[LY[lo]]));
+        double ez = __dmul_rn(gamma_bar, __dsub_rn(z[LZ[hi - 1]], z[LZ[lo]]));
+        double best = ex;
+        if (ey > best) { best = ey; a = 1; }
+        if (ez > best) { best = ez; a = 2; }
+    }
+    axis[k] = (int8_t)a;
+}
+
+// Alg 5.2 (readings G7, G8): in the list of the chosen axis the first ceil(size/2)
+// members of the node (ranked by (coordinate, index)) go to the left child.
+__global__ void kd_mark_left(int N, int level, const int8_t *__restrict__ axis, const uint32_t *__restrict__ LX,
+                             const uint32_t *__restrict__ LY, const uint32_t *__restrict__ LZ, uint8_t *__restrict__ left)
+{
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= N) return;
+    int node, lo, hi;
+    node_at_level(N, level, i, node, lo, hi);
+    int a = axis[node - (1 << level)];
+    int mid = lo + (hi - lo + 1) / 2;
+    uint32_t part = (a == 0) ? LX[i] : (a == 1) ? LY[i] : LZ[i];
+    left[part] = (i < mid) ? 1 : 0;
+}
+
+__global__ void kd_gather_flags(int N, const uint8_t *__restrict__ left, const uint32_t *__restrict__ lists /* [4][N] */,
+                                int32_t *__restrict__ f /* [4N] */)
+{
+    int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= 4ll * N) return;
+    f[i] = left[lists[i]];
+}
+
+// stable partition of every node segment of the four lists: left members first
+__global__ void kd_partition(int N, int level, const uint8_t *__restrict__ left, const int32_t *__restrict__ scan /* [4N] */,
+                             const uint32_t *__restrict__ lists, uint32_t *__restrict__ out)
+{
+    int64_t g = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (g >= 4ll * N) return;
+    int li = (int)(g / N), i = (int)(g - (int64_t)li * N);
+    int node, lo, hi;
+    node_at_level(N, level, i, node, lo, hi);
+    int mid = lo + (hi - lo + 1) / 2;
+    uint32_t part = lists[g];
+    int nleft_before = scan[g] - scan[(int64_t)li * N + lo];
+    int dest = left[part] ? (lo + nleft_before) : (mid + (i - lo - nleft_before));
+    out[(int64_t)li * N + dest] = part;
+}
+
+// ---------------------------------------------------------------------------------------
+// a1', mode MORTON_MEDIAN (DESIGN T-3')
+// ---------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(RED_THREADS) minmax_partial(int64_t N, const double *__restrict__ x, const double *__restrict__ y,
+                                                              const double *__restrict__ z, double *__restrict__ partial /* [RED_BLOCKS][6] */)
+{
+    __shared__ double sm[6][8];
+    double lo[3] = {INFINITY, INFINITY, INFINITY}, hi[3] = {-INFINITY, -INFINITY, -INFINITY};
+    for (int64_t j = (int64_t)blockIdx.x * RED_THREADS + threadIdx.x; j < N; j += (int64_t)RED_BLOCKS * RED_THREADS) {
+        lo[0] = fmin(lo[0], x[j]); hi[0] = fmax(hi[0], x[j]);
+        lo[1] = fmin(lo[1], y[j]); hi[1] = fmax(hi[1], y[j]);
+        lo[2] = fmin(lo[2], z[j]); hi[2] = fmax(hi[2], z[j]);
+    }
+    int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+#pragma unroll
+    for (int k = 0; k < 3; ++k) {
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+            lo[k] = fmin(lo[k], __shfl_down_sync(0xffffffffu, lo[k], o));
+            hi[k] = fmax(hi[k], __shfl_down_sync(0xffffffffu, hi[k], o));
+        }
+        if (lane == 0) { sm[k][warp] = lo[k]; sm[3 + k][warp] = hi[k]; }
+    }
+    __syncthreads();
+    if (threadIdx.x < 6) {
+        double v = sm[threadIdx.x][0];
+        for (int w = 1; w < 8; ++w) v = (threadIdx.x < 3) ? fmin(v, sm[threadIdx.x][w]) : fmax(v, sm[threadIdx.x][w]);
+        partial[6 * blockIdx.x + threadIdx.x] = v;
+    }
+}
+
+__global__ void minmax_final(const double *__restrict__ partial, double *__restrict__ out /* [6] */)
+{
+    if (threadIdx.x >= 6) return;
+    double v = partial[threadIdx.x];
+    for (int b = 1; b < RED_BLOCKS; ++b)
+        v = (threadIdx.x < 3) ? fmin(v, partial[6 * b + threadIdx.x]) : fmax(v, partial[6 * b + threadIdx.x]);
+    out[threadIdx.x] = v;
+}
+
+__device__ __forceinline__ uint64_t spread3(uint64_t v)  // 21 bits -> every third bit
+{
+    v &= 0x1fffffull;
+    v = (v | (v << 32)) & 0x1f00000000ffffull;
+    v = (v | (v << 16)) & 0x1f0000ff0000ffull;
+    v = (v | (v << 8)) & 0x100f00f00f00f00full;
+    v = (v | (v << 4)) & 0x10c30c30c30c30c3ull;
+    v = (v | (v << 2)) & 0x1249249249249249ull;
+    return v;
+}
+
+__global__ void morton_keys(int N, const double *__restrict__ x, const double *__restrict__ y, const double *__restrict__ z,
+                            const double *__restrict__ mm /* [6] min xyz, max xyz of the raw coordinates */, double gamma_bar,
+                            uint64_t *__restrict__ keys, uint32_t *__restrict__ vals)
+{
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= N) return;
+    // u = s o x; s > 0 so min/max commute with the scaling (every operation rounded separately)
+    double s[3] = {1.0, 1.0, gamma_bar};
+    double lo[3], L = 0.0;
+#pragma unroll
+    for (int k = 0; k < 3; ++k) {
+        lo[k] = __dmul_rn(s[k], mm[k]);
+        double ext = __dsub_rn(__dmul_rn(s[k], mm[3 + k]), lo[k]);
+        if (k == 0 || ext > L) L = ext;
+    }
+    double c[3] = {x[i], y[i], z[i]};
+    uint64_t q[3];
+#pragma unroll
+    for (int k = 0; k < 3; ++k) {
+        double u = __dmul_rn(s[k], c[k]);
+        double f = (L > 0.0) ? floor(__dmul_rn(__ddiv_rn(__dsub_rn(u, lo[k]), L), 2097152.0)) : 0.0;
+        if (f > 2097151.0) f = 2097151.0;
+        if (f < 0.0) f = 0.0;
+        q[k] = (uint64_t)f;
+    }
+    keys[i] = spread3(q[0]) | (spread3(q[1]) << 1) | (spread3(q[2]) << 2);  // z most significant
+    vals[i] = (uint32_t)i;
+}
+
+// ---------------------------------------------------------------------------------------
+// a1 end: physical permutation into tree order + source weights (a0)
+// ---------------------------------------------------------------------------------------
+__global__ void permute_particles(int N, const uint32_t *__restrict__ order, const double *__restrict__ x, const double *__restrict__ y,
+                                  const double *__restrict__ z, const double *__restrict__ px, const double *__restrict__ py,
+                                  const double *__restrict__ pz, const double *__restrict__ q, double q_scalar,
+                                  int32_t *__restrict__ perm, double *__restrict__ tx, double *__restrict__ ty, double *__restrict__ tz,
+                                  double *__restrict__ w0, double *__restrict__ w1, double *__restrict__ w2, double *__restrict__ w3)
+{
+    int k = blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= N) return;
+    uint32_t j = order[k];
+    perm[k] = (int32_t)j;
+    tx[k] = x[j];
+    ty[k] = y[j];
+    tz[k] = z[j];
+    double ax = px[j], ay = py[j], az = pz[j];
+    double qj = q ? q[j] : q_scalar;
+    double gam = sqrt(1.0 + (ax * ax + ay * ay + az * az));  // gamma_j = sqrt(1 + p.p)
+    w0[k] = qj * gam;
+    w1[k] = qj * ax;
+    w2[k] = qj * ay;
+    w3[k] = qj * az;
+}
+
+// ---------------------------------------------------------------------------------------
+// a2: bounding boxes
+// ---------------------------------------------------------------------------------------
+// one warp per leaf: tight min/max over its members (exact, order-free)
+__global__ void leaf_bbox(int leaves, const int32_t *__restrict__ node_lo, const int32_t *__restrict__ node_hi,
+                          const double *__restrict__ tx, const double *__restrict__ ty, const double *__restrict__ tz,
+                          double *__restrict__ bbox)
+{
+    int w = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
+    if (w >= leaves) return;
+    int node = leaves + w;
+    int lo = node_lo[node], hi = node_hi[node];
+    double a[3] = {INFINITY, INFINITY, INFINITY}, b[3] = {-INFINITY, -INFINITY, -INFINITY};
+    for (int k = lo + lane; k < hi; k += 32) {
+        double vx = tx[k], vy = ty[k], vz = tz[k];
+        a[0] = fmin(a[0], vx); b[0] = fmax(b[0], vx);
+        a[1] = fmin(a[1], vy); b[1] = fmax(b[1], vy);
+        a[2] = fmin(a[2], vz); b[2] = fmax(b[2], vz);
+    }
+#pragma unroll
+    for (int k = 0; k < 3; ++k)
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+            a[k] = fmin(a[k], __shfl_xor_sync(0xffffffffu, a[k], o));
+            b[k] = fmax(b[k], __shfl_xor_sync(0xffffffffu, b[k], o));
+        }
+    if (lane == 0) {
+        double *bb = bbox + 6 * (int64_t)node;
+        bool empty = hi <= lo;  // empty cluster: zeros (it takes part in nothing)
+        for (int k = 0; k < 3; ++k) {
+            bb[k] = empty ? 0.0 : a[k];
+            bb[3 + k] = empty ? 0.0 : b[k];
+        }
+    }
+}
+
+// one block: parents = union of the non-empty children, level by level upward; then the stretched
+// squared radius (Alg 5.6) and the box centre (Alg 5.7) of every node, each
+// product and sum rounded separately (reading D-2) so that the traversal is bit-reproducible.
+__global__ void __launch_bounds__(1024) upper_bbox_and_geometry(int kappa, int nodes, const int32_t *__restrict__ node_lo,
+                                                                const int32_t *__restrict__ node_hi, double gamma_bar,
+                                                                double *__restrict__ bbox, double *__restrict__ geo)
+{
+    for (int level = kappa - 1; level >= 0; --level) {
+        int first = 1 << level;
+        for (int i = first + threadIdx.x; i < 2 * first; i += blockDim.x) {
+            int c0 = 2 * i, c1 = 2 * i + 1;
+            bool e0 = node_hi[c0] <= node_lo[c0], e1 = node_hi[c1] <= node_lo[c1];
+            double *bb = bbox + 6 * (int64_t)i;
+            const double *b0 = bbox + 6 * (int64_t)c0, *b1 = bbox + 6 * (int64_t)c1;
+            for (int k = 0; k < 3; ++k) {
+                double lo, hi;
+                if (e0 && e1) { lo = 0.0; hi = 0.0; }
+                else if (e1) { lo = b0[k]; hi = b0[3 + k]; }
+                else if (e0) { lo = b1[k]; hi = b1[3 + k]; }
+                else { lo = fmin(b0[k], b1[k]); hi = fmax(b0[3 + k], b1[3 + k]); }
+                bb[k] = lo;
+                bb[3 + k] = hi;
+            }
+        }
+        __syncthreads();
+    }
+    for (int i = 1 + threadIdx.x; i <= nodes; i += blockDim.x) {
+        const double *bb = bbox + 6 * (int64_t)i;
+        double hx = __dmul_rn(__dsub_rn(bb[3], bb[0]), 0.5), hy = __dmul_rn(__dsub_rn(bb[4], bb[1]), 0.5),
+               hz = __dmul_rn(__dsub_rn(bb[5], bb[2]), 0.5);
+        double ex = __dmul_rn(1.0, hx), ey = __dmul_rn(1.0, hy), ez = __dmul_rn(gamma_bar, hz);
+        double *g = geo + 4 * (int64_t)i;
+        g[0] = __dadd_rn(__dadd_rn(__dmul_rn(ex, ex), __dmul_rn(ey, ey)), __dmul_rn(ez, ez));
+        g[1] = __dmul_rn(__dadd_rn(bb[0], bb[3]), 0.5);
+        g[2] = __dmul_rn(__dadd_rn(bb[1], bb[4]), 0.5);
+        g[3] = __dmul_rn(__dadd_rn(bb[2], bb[5]), 0.5);
+    }
+}
+
+// ---------------------------------------------------------------------------------------
+int tree_build(fmm_plan *p, const fmm_particles_t *in)
+{
+    fmm_ctx *c = &p->ctx;
+    cudaStream_t st = c->stream;
+    const int N = (int)p->N;
+    const int T = 256;
+    const int gN = (N + T - 1) / T;
+
+    node_ranges_kernel<<<(unsigned)((p->nodes + T - 1) / T), T, 0, st>>>(N, p->kappa, (int)p->nodes, p->node_lo, p->node_hi);
+    FMM_LAUNCH_CHECK(c, "node_ranges_kernel");
+
+    uint64_t *keys = (uint64_t *)ctx_alloc(c, sizeof(uint64_t) * N);
+    uint64_t *tkeys = (uint64_t *)ctx_alloc(c, sizeof(uint64_t) * N);
+    uint32_t *tvals = (uint32_t *)ctx_alloc(c, sizeof(uint32_t) * N);
+    uint32_t *lists = (uint32_t *)ctx_alloc(c, sizeof(uint32_t) * 4 * (size_t)N);  // LX, LY, LZ, LI
+    if (!keys || !tkeys || !tvals || !lists) return FMM_ENOMEM;
+    const uint32_t *order = NULL;
+
+    if ((p->flags & FMM_TREE_MASK) == FMM_TREE_KD) {
+        uint32_t *lists2 = (uint32_t *)ctx_alloc(c, sizeof(uint32_t) * 4 * (size_t)N);
+        int32_t *scan = (int32_t *)ctx_alloc(c, sizeof(int32_t) * 4 * (size_t)N);
+        uint8_t *left = (uint8_t *)ctx_alloc(c, (size_t)N);
+        int8_t *axis = (int8_t *)ctx_alloc(c, (size_t)((p->leaves > 1) ? p->leaves : 1));
+        if (!lists2 || !scan || !left || !axis) return FMM_ENOMEM;
+        if (p->kappa > 0) {
+            const double *coord[3] = {in->x, in->y, in->z};
+            for (int a = 0; a < 3; ++a) {
+                kd_make_keys<<<gN, T, 0, st>>>(N, coord[a], keys, lists + (size_t)a * N);
+                FMM_LAUNCH_CHECK(c, "kd_make_keys");
+                FMM_TRY(sort_pairs_u64(c, keys, lists + (size_t)a * N, tkeys, tvals, N, 0, 64));
+            }
+        }
+        kd_iota<<<gN, T, 0, st>>>(N, lists + 3 * (size_t)N);
+        FMM_LAUNCH_CHECK(c, "kd_iota");
+        uint32_t *cur = lists, *nxt = lists2;
+        const int g4 = (int)((4ll * N + T - 1) / T);
+        for (int level = 0; level < p->kappa; ++level) {
+            int nn = 1 << level;
+            kd_choose_axis<<<(nn + T - 1) / T, T, 0, st>>>(N, level, in->x, in->y, in->z, cur, cur + N, cur + 2 * (size_t)N,
+                                                           p->gamma_bar, axis);
+            FMM_LAUNCH_CHECK(c, "kd_choose_axis");
+            kd_mark_left<<<gN, T, 0, st>>>(N, level, axis, cur, cur + N, cur + 2 * (size_t)N, left);
+            FMM_LAUNCH_CHECK(c, "kd_mark_left");
+            kd_gather_flags<<<g4, T, 0, st>>>(N, left, cur, scan);
+            FMM_LAUNCH_CHECK(c, "kd_gather_flags");
+            FMM_TRY(scan_exclusive_i32(c, scan, scan, 4ll * N));
+            kd_partition<<<g4, T, 0, st>>>(N, level, left, scan, cur, nxt);
+            FMM_LAUNCH_CHECK(c, "kd_partition");
+            uint32_t *t = cur; cur = nxt; nxt = t;
+        }
+        order = cur + 3 * (size_t)N;  // the index-ordered list: leaves in heap order, ascending index inside (T-3)
+        permute_particles<<<gN, T, 0, st>>>(N, order, in->x, in->y, in->z, in->px, in->py, in->pz, in->q, in->q_scalar,
+                                            p->perm, p->tx, p->ty, p->tz, p->w0, p->w1, p->w2, p->w3);
+        FMM_LAUNCH_CHECK(c, "permute_particles");
+        ctx_free(c, lists2); ctx_free(c, scan); ctx_free(c, left); ctx_free(c, axis);
+    } else {
+        double *mm = (double *)ctx_alloc(c, sizeof(double) * (6 * RED_BLOCKS + 6));
+        if (!mm) return FMM_ENOMEM;
+        minmax_partial<<<RED_BLOCKS, RED_THREADS, 0, st>>>(N, in->x, in->y, in->z, mm);
+        FMM_LAUNCH_CHECK(c, "minmax_partial");
+        minmax_final<<<1, 32, 0, st>>>(mm, mm + 6 * RED_BLOCKS);
+        FMM_LAUNCH_CHECK(c, "minmax_final");
+        morton_keys<<<gN, T, 0, st>>>(N, in->x, in->y, in->z, mm + 6 * RED_BLOCKS, p->gamma_bar, keys, lists);
+        FMM_LAUNCH_CHECK(c, "morton_keys");
+        FMM_TRY(sort_pairs_u64(c, keys, lists, tkeys, tvals, N, 0, 64));
+        order = lists;
+        permute_particles<<<gN, T, 0, st>>>(N, order, in->x, in->y, in->z, in->px, in->py, in->pz, in->q, in->q_scalar,
+                                            p->perm, p->tx, p->ty, p->tz, p->w0, p->w1, p->w2, p->w3);
+        FMM_LAUNCH_CHECK(c, "permute_particles");
+        ctx_free(c, mm);
+    }
+    ctx_free(c, keys); ctx_free(c, tkeys); ctx_free(c, tvals); ctx_free(c, lists);
+
+    leaf_bbox<<<(unsigned)((p->leaves * 32 + T - 1) / T), T, 0, st>>>((int)p->leaves, p->node_lo, p->node_hi, p->tx, p->ty, p->tz, p->bbox);
+    FMM_LAUNCH_CHECK(c, "leaf_bbox");
+    upper_bbox_and_geometry<<<1, 1024, 0, st>>>(p->kappa, (int)p->nodes, p->node_lo, p->node_hi, p->gamma_bar, p->bbox, p->node_geo);
+    FMM_LAUNCH_CHECK(c, "upper_bbox_and_geometry");
+    return FMM_OK;
+}
