@@ -1,0 +1,390 @@
+// fmm_api.cu -- the C-ABI entry points of include/fmm.h and the host orchestration of
+// Alg 5.12: fmm_plan_create = subdivide + dualtraversefillitl (a0-a3),
+// fmm_eval = upward pass, M2L + P2P over the lists, downward pass (a4-a10).
+#include "fmm_internal.cuh"
+
+#include <math.h>
+#include <new>
+
+std::atomic<int64_t> g_fmm_launches{0};
+static thread_local char g_last_error[256] = "";
+
+// ---------------------------------------------------------------------------------------
+// context: allocator, stream, error text
+// ---------------------------------------------------------------------------------------
+static void ctx_init(fmm_ctx *c, fmm_alloc_fn alloc, fmm_free_fn free_, void *user, void *stream)
+{
+    c->alloc = alloc;
+    c->free_ = free_;
+    c->user = user;
+    c->stream = (cudaStream_t)stream;
+    c->err[0] = 0;
+    c->bytes = 0;
+}
+
+static void ctx_set_error(fmm_ctx *c, const char *msg)
+{
+    snprintf(c->err, sizeof(c->err), "%s", msg);
+    snprintf(g_last_error, sizeof(g_last_error), "%s", msg);
+}
+
+int ctx_cuda_fail(fmm_ctx *c, cudaError_t e, const char *what)
+{
+    char buf[256];
+    snprintf(buf, sizeof(buf), "%s: %s", what, cudaGetErrorString(e));
+    ctx_set_error(c, buf);
+    return FMM_ECUDA;
+}
+
+void *ctx_alloc(fmm_ctx *c, size_t bytes)
+{
+    if (bytes == 0) bytes = 8;
+    void *p = NULL;
+    if (c->alloc) {
+        p = c->alloc(bytes, c->user);
+    } else {
+        if (cudaMallocAsync(&p, bytes, c->stream) != cudaSuccess) p = NULL;
+    }
+    if (!p) {
+        char buf[128];
+        snprintf(buf, sizeof(buf), "allocator returned NULL for %zu bytes", bytes);
+        ctx_set_error(c, buf);
+        return NULL;
+    }
+    c->owned.push_back(p);
+    c->owned_bytes.push_back(bytes);
+    c->bytes += (int64_t)bytes;
+    return p;
+}
+
+void ctx_free(fmm_ctx *c, void *p)
+{
+    if (!p) return;
+    for (size_t k = c->owned.size(); k-- > 0;) {
+        if (c->owned[k] == p) {
+            c->bytes -= (int64_t)c->owned_bytes[k];
+            c->owned.erase(c->owned.begin() + k);
+            c->owned_bytes.erase(c->owned_bytes.begin() + k);
+            break;
+        }
+    }
+    if (c->free_) c->free_(p, c->user);
+    else cudaFreeAsync(p, c->stream);
+}
+
+void ctx_free_all(fmm_ctx *c)
+{
+    while (!c->owned.empty()) ctx_free(c, c->owned.back());
+}
+
+static int check_particles(const fmm_particles_t *in)
+{
+    if (!in || in->N < 1 || in->N >= ((int64_t)1 << 31)) return FMM_EINVAL;
+    if (!in->x || !in->y || !in->z || !in->px || !in->py || !in->pz) return FMM_EINVAL;
+    return FMM_OK;
+}
+
+extern "C" const char *fmm_strerror(int code)
+{
+    switch (code) {
+        case FMM_OK: return "ok";
+        case FMM_EINVAL: return "invalid argument";
+        case FMM_ENOMEM: return "device allocator returned NULL";
+        case FMM_ECUDA: return "CUDA error";
+        case FMM_ENONFINITE: return "gamma_bar is not finite (NaN/Inf in the momenta)";
+        case FMM_EOVERFLOW: return "interaction list exceeds 2^31-1 entries";
+    }
+    return "unknown error code";
+}
+
+extern "C" const char *fmm_last_error(const fmm_plan_t *plan) { return plan ? plan->ctx.err : g_last_error; }
+extern "C" const char *fmm_version(void) { return "fmm_b200 0.1 (sm_100a, FP64)"; }
+extern "C" int64_t fmm_launch_count(void) { return g_fmm_launches.load(); }
+
+// ---------------------------------------------------------------------------------------
+// plan: a0-a3
+// ---------------------------------------------------------------------------------------
+static int plan_alloc_fixed(fmm_plan *p)
+{
+    fmm_ctx *c = &p->ctx;
+    const size_t N = (size_t)p->N, nodes1 = (size_t)p->nodes + 2;
+#define ALLOC(field, type, count)                                         \
+    do {                                                                  \
+        p->field = (type *)ctx_alloc(c, sizeof(type) * (size_t)(count));  \
+        if (!p->field) return FMM_ENOMEM;                                 \
+    } while (0)
+    ALLOC(tx, double, N); ALLOC(ty, double, N); ALLOC(tz, double, N);
+    ALLOC(w0, double, N); ALLOC(w1, double, N); ALLOC(w2, double, N); ALLOC(w3, double, N);
+    ALLOC(perm, int32_t, N);
+    ALLOC(node_lo, int32_t, nodes1); ALLOC(node_hi, int32_t, nodes1);
+    ALLOC(bbox, double, 6 * nodes1); ALLOC(node_geo, double, 4 * nodes1);
+    ALLOC(p2p_off, int32_t, nodes1 + 1); ALLOC(m2l_off, int32_t, nodes1 + 1);
+    ALLOC(p2p_order, int32_t, nodes1); ALLOC(m2l_order, int32_t, nodes1);
+    ALLOC(M, double, 4 * (size_t)p->P * nodes1);
+    ALLOC(L, double, 6 * (size_t)p->P * nodes1);
+    ALLOC(near_, double, 6 * N);
+#undef ALLOC
+    return FMM_OK;
+}
+
+static int plan_build(fmm_plan *p, const fmm_particles_t *in)
+{
+    fmm_ctx *c = &p->ctx;
+    FMM_CUDA(c, cudaEventRecord(p->ev_plan[0], c->stream));
+    if (p->gamma_bar_param > 0.0) {
+        p->gamma_bar = p->gamma_bar_param;
+    } else {
+        FMM_TRY(tree_gamma_bar(c, p->N, in->px, in->py, in->pz, &p->gamma_bar));
+        if (!isfinite(p->gamma_bar)) return FMM_ENONFINITE;
+    }
+    FMM_TRY(tree_build(p, in));
+    FMM_CUDA(c, cudaEventRecord(p->ev_plan[1], c->stream));
+    FMM_TRY(dtt_build_lists(p));
+    FMM_CUDA(c, cudaEventRecord(p->ev_plan[2], c->stream));
+    FMM_CUDA(c, cudaStreamSynchronize(c->stream));
+    FMM_CUDA(c, cudaEventElapsedTime(&p->ms_tree, p->ev_plan[0], p->ev_plan[1]));
+    FMM_CUDA(c, cudaEventElapsedTime(&p->ms_lists, p->ev_plan[1], p->ev_plan[2]));
+    p->ev_valid = 0;
+    return FMM_OK;
+}
+
+extern "C" void fmm_plan_destroy(fmm_plan_t *p)
+{
+    if (!p) return;
+    cudaStreamSynchronize(p->ctx.stream);
+    ctx_free_all(&p->ctx);
+    for (int k = 0; k < EV_COUNT; ++k)
+        if (p->ev[k]) cudaEventDestroy(p->ev[k]);
+    for (int k = 0; k < 3; ++k)
+        if (p->ev_plan[k]) cudaEventDestroy(p->ev_plan[k]);
+    delete p;
+}
+
+extern "C" int fmm_plan_create(fmm_plan_t **out, const fmm_particles_t *in, const fmm_params_t *prm,
+                               fmm_alloc_fn alloc, fmm_free_fn free_, void *user, void *cuda_stream)
+{
+    if (!out) return FMM_EINVAL;
+    *out = NULL;
+    if (check_particles(in) != FMM_OK || !prm) return FMM_EINVAL;
+    if (prm->order_n < 1 || prm->order_n > FMM_MAX_ORDER || prm->leaf_size < 1) return FMM_EINVAL;
+    if (!(prm->theta > 0.0) || !isfinite(prm->theta)) return FMM_EINVAL;
+    if ((alloc == NULL) != (free_ == NULL)) return FMM_EINVAL;
+    if (isnan(prm->gamma_bar) || isinf(prm->gamma_bar)) return FMM_EINVAL;
+    fmm_plan *p = new (std::nothrow) fmm_plan();
+    if (!p) return FMM_ENOMEM;
+    ctx_init(&p->ctx, alloc, free_, user, cuda_stream);
+    p->N = in->N;
+    p->n = prm->order_n;
+    p->n1 = p->n + 1;
+    p->P = p->n1 * p->n1 * p->n1;
+    p->N0 = prm->leaf_size;
+    p->theta = prm->theta;
+    p->gamma_bar_param = prm->gamma_bar;
+    p->flags = prm->flags;
+    int kappa = 0;  // T-1: smallest kappa with N0 2^kappa >= N
+    while (((int64_t)p->N0 << kappa) < p->N) ++kappa;
+    p->kappa = kappa;
+    p->leaves = (int64_t)1 << kappa;
+    p->nodes = ((int64_t)2 << kappa) - 1;
+    int rc = FMM_OK;
+    for (int k = 0; k < EV_COUNT && rc == FMM_OK; ++k)
+        if (cudaEventCreate(&p->ev[k]) != cudaSuccess) rc = FMM_ECUDA;
+    for (int k = 0; k < 3 && rc == FMM_OK; ++k)
+        if (cudaEventCreate(&p->ev_plan[k]) != cudaSuccess) rc = FMM_ECUDA;
+    if (rc == FMM_OK) rc = plan_alloc_fixed(p);
+    if (rc == FMM_OK) rc = plan_build(p, in);
+    if (rc != FMM_OK) {
+        snprintf(g_last_error, sizeof(g_last_error), "%s", p->ctx.err);
+        fmm_plan_destroy(p);
+        return rc;
+    }
+    *out = p;
+    return FMM_OK;
+}
+
+extern "C" int fmm_plan_update(fmm_plan_t *p, const fmm_particles_t *in)
+{
+    if (!p || check_particles(in) != FMM_OK || in->N != p->N) return FMM_EINVAL;
+    return plan_build(p, in);
+}
+
+extern "C" int fmm_plan_set_timing(fmm_plan_t *p, int on)
+{
+    if (!p) return FMM_EINVAL;
+    p->timing = on ? 1 : 0;
+    p->ev_valid = 0;
+    return FMM_OK;
+}
+
+// ---------------------------------------------------------------------------------------
+// evaluation: a4-a10
+// ---------------------------------------------------------------------------------------
+#define MARK(p, id)                                                                   \
+    do {                                                                              \
+        if ((p)->timing) FMM_CUDA(&(p)->ctx, cudaEventRecord((p)->ev[id], (p)->ctx.stream)); \
+    } while (0)
+
+extern "C" int fmm_eval(fmm_plan_t *p, double *Ex, double *Ey, double *Ez, double *Bx, double *By, double *Bz)
+{
+    if (!p || !Ex || !Ey || !Ez || !Bx || !By || !Bz) return FMM_EINVAL;
+    MARK(p, EV_P2M);
+    FMM_TRY(interp_p2m(p));          // Alg 5.3 at the leaves
+    MARK(p, EV_M2M);
+    FMM_TRY(interp_m2m(p));          // Alg 5.4, levels kappa-1 .. 0 (Alg 5.5)
+    MARK(p, EV_M2L);
+    FMM_TRY(pairs_m2l(p));           // Alg 5.9 over m2l_itl
+    MARK(p, EV_L2L);
+    FMM_TRY(interp_l2l(p));          // Alg 5.13, levels 1 .. kappa (Alg 5.15)
+    MARK(p, EV_P2P);
+    FMM_TRY(pairs_p2p(p));           // Alg 5.10 over p2p_itl
+    MARK(p, EV_L2P);
+    FMM_TRY(interp_l2p_finalize(p, Ex, Ey, Ez, Bx, By, Bz));  // Alg 5.14 + eq. (3.1) prefactors
+    MARK(p, EV_END);
+    if (p->timing) p->ev_valid = 1;
+    return FMM_OK;
+}
+
+extern "C" int fmm_plan_stats(fmm_plan_t *p, fmm_stats_t *s)
+{
+    if (!p || !s) return FMM_EINVAL;
+    memset(s, 0, sizeof(*s));
+    s->N = p->N;
+    s->order_n = p->n;
+    s->P = p->P;
+    s->leaf_size = p->N0;
+    s->kappa = p->kappa;
+    s->nodes = p->nodes;
+    s->leaves = p->leaves;
+    s->n_p2p = p->n_p2p;
+    s->n_m2l = p->n_m2l;
+    s->p2p_pairs = p->p2p_pairs;
+    s->m2l_pairs = p->m2l_pairs;
+    s->gamma_bar = p->gamma_bar;
+    s->theta = p->theta;
+    s->flags = p->flags;
+    s->ms_tree = p->ms_tree;
+    s->ms_lists = p->ms_lists;
+    s->workspace_bytes = p->ctx.bytes;
+    if (p->timing && p->ev_valid) {
+        fmm_ctx *c = &p->ctx;
+        FMM_CUDA(c, cudaEventSynchronize(p->ev[EV_END]));
+        FMM_CUDA(c, cudaEventElapsedTime(&s->ms_p2m, p->ev[EV_P2M], p->ev[EV_M2M]));
+        FMM_CUDA(c, cudaEventElapsedTime(&s->ms_m2m, p->ev[EV_M2M], p->ev[EV_M2L]));
+        FMM_CUDA(c, cudaEventElapsedTime(&s->ms_m2l, p->ev[EV_M2L], p->ev[EV_L2L]));
+        FMM_CUDA(c, cudaEventElapsedTime(&s->ms_l2l, p->ev[EV_L2L], p->ev[EV_P2P]));
+        FMM_CUDA(c, cudaEventElapsedTime(&s->ms_p2p, p->ev[EV_P2P], p->ev[EV_L2P]));
+        FMM_CUDA(c, cudaEventElapsedTime(&s->ms_l2p, p->ev[EV_L2P], p->ev[EV_END]));
+        s->timing_valid = 1;
+    }
+    return FMM_OK;
+}
+
+extern "C" int fmm_plan_export(fmm_plan_t *p, fmm_export_t *o)
+{
+    if (!p || !o) return FMM_EINVAL;
+    fmm_ctx *c = &p->ctx;
+    FMM_CUDA(c, cudaStreamSynchronize(c->stream));
+    const size_t N = (size_t)p->N, nodes = (size_t)p->nodes;
+    std::vector<int32_t> tmp;
+    auto get_i32 = [&](const int32_t *dev, size_t count) -> int {
+        tmp.resize(count);
+        FMM_CUDA(c, cudaMemcpy(tmp.data(), dev, sizeof(int32_t) * count, cudaMemcpyDeviceToHost));
+        return FMM_OK;
+    };
+    if (o->perm) {
+        FMM_TRY(get_i32(p->perm, N));
+        for (size_t k = 0; k < N; ++k) o->perm[k] = tmp[k];
+    }
+    if (o->node_lo) {
+        FMM_TRY(get_i32(p->node_lo + 1, nodes));
+        for (size_t k = 0; k < nodes; ++k) o->node_lo[k] = tmp[k];
+    }
+    if (o->node_hi) {
+        FMM_TRY(get_i32(p->node_hi + 1, nodes));
+        for (size_t k = 0; k < nodes; ++k) o->node_hi[k] = tmp[k];
+    }
+    if (o->bbox) FMM_CUDA(c, cudaMemcpy(o->bbox, p->bbox + 6, sizeof(double) * 6 * nodes, cudaMemcpyDeviceToHost));
+    if (o->p2p_off) FMM_CUDA(c, cudaMemcpy(o->p2p_off, p->p2p_off + 1, sizeof(int32_t) * (nodes + 1), cudaMemcpyDeviceToHost));
+    if (o->m2l_off) FMM_CUDA(c, cudaMemcpy(o->m2l_off, p->m2l_off + 1, sizeof(int32_t) * (nodes + 1), cudaMemcpyDeviceToHost));
+    if (o->p2p_src && p->n_p2p > 0)
+        FMM_CUDA(c, cudaMemcpy(o->p2p_src, p->p2p_src, sizeof(int32_t) * (size_t)p->n_p2p, cudaMemcpyDeviceToHost));
+    if (o->m2l_src && p->n_m2l > 0)
+        FMM_CUDA(c, cudaMemcpy(o->m2l_src, p->m2l_src, sizeof(int32_t) * (size_t)p->n_m2l, cudaMemcpyDeviceToHost));
+    if (o->M) FMM_CUDA(c, cudaMemcpy(o->M, p->M + 4 * (size_t)p->P, sizeof(double) * 4 * (size_t)p->P * nodes, cudaMemcpyDeviceToHost));
+    if (o->L) FMM_CUDA(c, cudaMemcpy(o->L, p->L + 6 * (size_t)p->P, sizeof(double) * 6 * (size_t)p->P * nodes, cudaMemcpyDeviceToHost));
+    return FMM_OK;
+}
+
+// ---------------------------------------------------------------------------------------
+// a11: direct summation
+// ---------------------------------------------------------------------------------------
+extern "C" int fmm_direct(const fmm_particles_t *in, double gamma_bar, uint32_t flags, int64_t nt, const int64_t *tidx,
+                          double *Ex, double *Ey, double *Ez, double *Bx, double *By, double *Bz,
+                          fmm_alloc_fn alloc, fmm_free_fn free_, void *user, void *cuda_stream)
+{
+    if (check_particles(in) != FMM_OK || nt < 1 || !Ex || !Ey || !Ez || !Bx || !By || !Bz) return FMM_EINVAL;
+    if (!tidx && nt != in->N) return FMM_EINVAL;
+    if ((alloc == NULL) != (free_ == NULL)) return FMM_EINVAL;
+    fmm_ctx ctx;
+    ctx_init(&ctx, alloc, free_, user, cuda_stream);
+    fmm_ctx *c = &ctx;
+    int rc = FMM_OK;
+    if (!(gamma_bar > 0.0)) {
+        rc = tree_gamma_bar(c, in->N, in->px, in->py, in->pz, &gamma_bar);
+        if (rc == FMM_OK && !isfinite(gamma_bar)) rc = FMM_ENONFINITE;
+    }
+    double *w = NULL;
+    if (rc == FMM_OK) {
+        w = (double *)ctx_alloc(c, sizeof(double) * 4 * (size_t)in->N);
+        if (!w) rc = FMM_ENOMEM;
+    }
+    const size_t N = (size_t)in->N;
+    if (rc == FMM_OK) rc = pairs_source_weights(c, in->N, in->px, in->py, in->pz, in->q, in->q_scalar, w, w + N, w + 2 * N, w + 3 * N);
+    if (rc == FMM_OK)
+        rc = pairs_direct(c, in->N, in->x, in->y, in->z, w, w + N, w + 2 * N, w + 3 * N, gamma_bar, (flags & FMM_RAW_SUMS) ? 1 : 0, nt,
+                          tidx, Ex, Ey, Ez, Bx, By, Bz);
+    ctx_free_all(c);
+    return rc;
+}
+
+// ---------------------------------------------------------------------------------------
+// whole of Alg 5.12 from host memory
+// ---------------------------------------------------------------------------------------
+extern "C" int fmm_field_host(const fmm_particles_t *h, const fmm_params_t *prm, double *Ex, double *Ey, double *Ez,
+                              double *Bx, double *By, double *Bz, fmm_stats_t *stats,
+                              fmm_alloc_fn alloc, fmm_free_fn free_, void *user, void *cuda_stream)
+{
+    if (check_particles(h) != FMM_OK || !prm || !Ex || !Ey || !Ez || !Bx || !By || !Bz) return FMM_EINVAL;
+    if ((alloc == NULL) != (free_ == NULL)) return FMM_EINVAL;
+    fmm_ctx ctx;
+    ctx_init(&ctx, alloc, free_, user, cuda_stream);
+    fmm_ctx *c = &ctx;
+    const size_t N = (size_t)h->N, bytes = sizeof(double) * N;
+    const int nin = h->q ? 7 : 6;
+    double *din = (double *)ctx_alloc(c, bytes * nin);
+    double *dout = (double *)ctx_alloc(c, bytes * 6);
+    fmm_plan_t *plan = NULL;
+    int rc = (din && dout) ? FMM_OK : FMM_ENOMEM;
+    auto body = [&]() -> int {
+        const double *src[7] = {h->x, h->y, h->z, h->px, h->py, h->pz, h->q};
+        for (int k = 0; k < nin; ++k)
+            FMM_CUDA(c, cudaMemcpyAsync(din + k * N, src[k], bytes, cudaMemcpyHostToDevice, c->stream));
+        fmm_particles_t d = *h;
+        d.x = din; d.y = din + N; d.z = din + 2 * N;
+        d.px = din + 3 * N; d.py = din + 4 * N; d.pz = din + 5 * N;
+        d.q = h->q ? din + 6 * N : NULL;
+        FMM_TRY(fmm_plan_create(&plan, &d, prm, alloc, free_, user, cuda_stream));
+        FMM_TRY(fmm_eval(plan, dout, dout + N, dout + 2 * N, dout + 3 * N, dout + 4 * N, dout + 5 * N));
+        double *dst[6] = {Ex, Ey, Ez, Bx, By, Bz};
+        for (int k = 0; k < 6; ++k)
+            FMM_CUDA(c, cudaMemcpyAsync(dst[k], dout + k * N, bytes, cudaMemcpyDeviceToHost, c->stream));
+        FMM_CUDA(c, cudaStreamSynchronize(c->stream));
+        if (stats) FMM_TRY(fmm_plan_stats(plan, stats));
+        return FMM_OK;
+    };
+    if (rc == FMM_OK) rc = body();
+    if (plan) fmm_plan_destroy(plan);
+    cudaStreamSynchronize(c->stream);
+    ctx_free_all(c);
+    return rc;
+}
