@@ -1,0 +1,212 @@
+"""GPU parity tests (-m gpu): the CUDA path, called through the C ABI (binding -> libfmm_b200.so),
+against the CPU oracle on the same seeded inputs.
+
+Bars:
+  * tree permutation, node ranges, bounding boxes, both CSR lists: bit-exact;
+  * fields (and M, L expansions): err2 (eq. (6.1)) <= 1e-12 and
+    max_i |f_i - fref_i| / max_i |fref_i| <= 1e-12, for E and for B;
+  * FMM-vs-direct error of the GPU equals the oracle's to 3 significant digits.
+The oracle is given the plan's gamma_bar (reading D-5) so that both sides share every bit of it.
+"""
+import numpy as np
+import pytest
+
+import oracle
+from paper_2302_07567_b200 import workloads
+
+pytestmark = pytest.mark.gpu
+
+TOL = 1e-12
+
+
+@pytest.fixture(scope="module")
+def fmm():
+    from paper_2302_07567_b200 import binding, build
+    build.build_library()
+    binding.load_library()
+    return binding
+
+
+def measures(f, fref):
+    """(err2 of eq. (6.1), max-norm relative error); f, fref are [N,3]."""
+    f, fref = np.asarray(f), np.asarray(fref)
+    e2 = np.sqrt(np.sum((f - fref) ** 2) / np.sum(fref ** 2))
+    d = np.linalg.norm(f - fref, axis=1).max() / np.linalg.norm(fref, axis=1).max()
+    return float(e2), float(d)
+
+
+def assert_close(f, fref, what, tol=TOL):
+    e2, d = measures(f, fref)
+    assert e2 <= tol and d <= tol, f"{what}: err2={e2:.3e} max={d:.3e} > {tol}"
+
+
+def to_np(EB):
+    E, B = EB
+    return E.cpu().numpy().T.copy(), B.cpu().numpy().T.copy()
+
+
+def small_cases():
+    """(label, workload, n, N0, theta): several tiles, ragged tails, degenerate trees."""
+    c1 = workloads.config(1)
+    yield "config1", c1, 4, 64, 0.5
+    w = workloads.config(2, N=20011)          # ragged: leaf sizes 78 / 79
+    yield "config2_ragged", w, 5, 128, 0.5
+    w = workloads.config(3, N=30000)
+    yield "config3_small_n3", w, 3, 100, 0.4
+    w = workloads.config(4, N=9000)           # gamma = 100: strongly stretched boxes
+    yield "config4_small", w, 6, 256, 0.4
+    w = workloads.paper_cube(N=6000, order_n=2)  # identical momenta, N0 = 27
+    yield "paper_cube_n2", w, 2, 27, 0.5
+    w = workloads.config(1, N=50)             # N <= N0: the root is a leaf (G23)
+    yield "single_leaf", w, 4, 64, 0.5
+    w = workloads.config(1, N=3)              # N0 = 1: an empty leaf appears
+    yield "three_particles", w, 2, 1, 0.5
+    w = workloads.config(1, N=1)
+    yield "one_particle", w, 2, 8, 0.5
+
+
+CASES = list(small_cases())
+IDS = [c[0] for c in CASES]
+
+
+# ---------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("N,targets", [(4096, None), (5003, 777), (1, None), (300, None)])
+def test_direct_matches_oracle(fmm, N, targets):
+    w = workloads.config(1, N=N)
+    gb = oracle.gamma_bar(w.px, w.py, w.pz)
+    tidx = None
+    if targets:
+        tidx = np.random.default_rng(5).choice(N, size=targets, replace=False).astype(np.int64)
+    E, B = to_np(fmm.fmm_direct(*w.arrays(), w.q, gamma_bar=gb, targets=tidx))
+    Eo, Bo = oracle.direct(*w.arrays(), w.q, gamma_bar_value=gb, targets=tidx)
+    if N == 1:
+        assert np.all(E == 0) and np.all(B == 0) and np.all(Eo == 0)
+        return
+    assert_close(E, Eo, "direct E")
+    assert_close(B, Bo, "direct B")
+
+
+def test_direct_own_gamma_bar_and_charges(fmm):
+    w = workloads.config(2, N=3000)
+    q = np.random.default_rng(11).uniform(0.5, 2.0, w.N) * workloads.ELECTRON_CHARGE
+    E, B = to_np(fmm.fmm_direct(*w.arrays(), q))          # gamma_bar computed on the device
+    Eo, Bo = oracle.direct(*w.arrays(), q)                # and by the oracle (serial sum)
+    assert_close(E, Eo, "direct E (own gamma_bar, per-particle q)", 1e-11)
+    assert_close(B, Bo, "direct B (own gamma_bar, per-particle q)", 1e-11)
+
+
+# ---------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("mode", ["kd", "morton"])
+@pytest.mark.parametrize("case", CASES, ids=IDS)
+def test_tree_and_lists_bit_exact(fmm, case, mode):
+    _, w, n, N0, theta = case
+    flags = fmm.FMM_TREE_KD if mode == "kd" else fmm.FMM_TREE_MORTON_MEDIAN
+    plan = fmm.fmm_plan_create(*w.arrays(), w.q, order_n=n, leaf_size=N0, theta=theta, flags=flags)
+    st = plan.stats()
+    ex = plan.export()
+    op = oracle.Plan(*w.arrays(), w.q, order_n=n, leaf_size=N0, theta=theta, gamma_bar_value=st["gamma_bar"],
+                     tree_mode=oracle.TREE_KD if mode == "kd" else oracle.TREE_MORTON_MEDIAN)
+    assert (st["kappa"], st["nodes"], st["leaves"], st["P"]) == (op.kappa, op.nodes, op.leaves, op.P)
+    assert abs(st["gamma_bar"] - oracle.gamma_bar(w.px, w.py, w.pz)) <= 1e-13 * st["gamma_bar"]
+    assert np.array_equal(ex["perm"], op.perm()), "permutation differs"
+    lo, hi, bb = op.node_arrays()
+    assert np.array_equal(ex["node_lo"], lo) and np.array_equal(ex["node_hi"], hi)
+    assert np.array_equal(ex["bbox"].view(np.uint64), bb.view(np.uint64)), "bounding boxes differ"
+    p2p, m2l = op.lists()
+    assert st["n_p2p"] == len(p2p) and st["n_m2l"] == len(m2l)
+    for name, ref in (("p2p", p2p), ("m2l", m2l)):
+        off, src = ex[name + "_off"], ex[name + "_src"]
+        tgt = np.repeat(np.arange(1, st["nodes"] + 1, dtype=np.int32), np.diff(off))
+        assert off[0] == 0 and off[-1] == len(ref)
+        assert np.array_equal(tgt, ref[:, 0]) and np.array_equal(src, ref[:, 1]), f"{name} list differs"
+    plan.close()
+
+
+@pytest.mark.parametrize("mode", ["kd", "morton"])
+@pytest.mark.parametrize("case", CASES, ids=IDS)
+def test_fmm_fields_match_serial_oracle(fmm, case, mode):
+    _, w, n, N0, theta = case
+    flags = fmm.FMM_TREE_KD if mode == "kd" else fmm.FMM_TREE_MORTON_MEDIAN
+    plan = fmm.fmm_plan_create(*w.arrays(), w.q, order_n=n, leaf_size=N0, theta=theta, flags=flags)
+    st = plan.stats()
+    E, B = to_np(plan.eval())
+    ex = plan.export(want_M=True, want_L=True)
+    op = oracle.Plan(*w.arrays(), w.q, order_n=n, leaf_size=N0, theta=theta, gamma_bar_value=st["gamma_bar"],
+                     tree_mode=oracle.TREE_KD if mode == "kd" else oracle.TREE_MORTON_MEDIAN)
+    Eo, Bo, Lo = op.eval(want_L=True)
+    Mo = op.upward()
+    if w.N == 1:
+        assert np.all(E == 0) and np.all(B == 0)
+        return
+    assert_close(E, Eo, "FMM E")
+    assert_close(B, Bo, "FMM B")
+    lo, hi, _ = op.node_arrays()
+    live = hi > lo
+    scale = np.abs(Mo).max()
+    assert np.abs(ex["M"][live] - Mo[live]).max() <= TOL * scale, "multipole moments differ"
+    if st["n_m2l"] > 0:
+        for f in (slice(0, 3), slice(3, 6)):
+            scale = np.abs(Lo[live][..., f]).max()
+            assert np.abs(ex["L"][live][..., f] - Lo[live][..., f]).max() <= TOL * scale, "local fields differ"
+    # FMM-vs-direct error: the GPU's equals the oracle's to 3 significant digits
+    Ed, Bd = oracle.direct(*w.arrays(), w.q, gamma_bar_value=st["gamma_bar"])
+    if st["n_m2l"] > 0:
+        for f, fo, fd in ((E, Eo, Ed), (B, Bo, Bd)):
+            a, b = oracle.err2(f, fd), oracle.err2(fo, fd)
+            assert abs(a - b) <= 5e-3 * b + 1e-13
+    else:  # pin P9: empty far list => FMM == direct
+        assert_close(E, Ed, "FMM(no far field) vs direct E", 1e-11)
+    plan.close()
+
+
+def test_raw_sums_and_charges(fmm):
+    w = workloads.config(1, N=3000)
+    q = np.random.default_rng(3).uniform(-2.0, 2.0, w.N)
+    plan = fmm.fmm_plan_create(*w.arrays(), q, order_n=3, leaf_size=50, theta=0.5, flags=fmm.FMM_RAW_SUMS)
+    st = plan.stats()
+    E, B = to_np(plan.eval())
+    op = oracle.Plan(*w.arrays(), q, order_n=3, leaf_size=50, theta=0.5, gamma_bar_value=st["gamma_bar"], raw=True)
+    Eo, Bo = op.eval()
+    assert_close(E, Eo, "raw E")
+    assert_close(B, Bo, "raw B")
+    plan.close()
+
+
+def test_deterministic_and_update(fmm):
+    w = workloads.config(2, N=12000)
+    plan = fmm.fmm_plan_create(*w.arrays(), w.q, order_n=4, leaf_size=64, theta=0.5)
+    E1, B1 = to_np(plan.eval())
+    E2, B2 = to_np(plan.eval())
+    assert np.array_equal(E1, E2) and np.array_equal(B1, B2), "not bit-reproducible run to run"
+    w2 = workloads.gaussian_bunch(12000, 20.0, 0.01, 77, order_n=4, leaf_size=64, theta=0.5)
+    plan.update(*w2.arrays(), w2.q)
+    st = plan.stats()
+    E3, B3 = to_np(plan.eval())
+    op = oracle.Plan(*w2.arrays(), w2.q, order_n=4, leaf_size=64, theta=0.5, gamma_bar_value=st["gamma_bar"])
+    Eo, Bo = op.eval()
+    assert_close(E3, Eo, "updated plan E")
+    assert_close(B3, Bo, "updated plan B")
+    plan.close()
+
+
+def test_field_host_entry(fmm):
+    w = workloads.config(1)
+    E, B, st = fmm.fmm_field_host(*w.arrays(), w.q, order_n=w.order_n, leaf_size=w.leaf_size, theta=w.theta)
+    op = oracle.Plan(*w.arrays(), w.q, order_n=w.order_n, leaf_size=w.leaf_size, theta=w.theta,
+                     gamma_bar_value=st["gamma_bar"])
+    Eo, Bo = op.eval()
+    assert_close(E.numpy().T, Eo, "host entry E")
+    assert_close(B.numpy().T, Bo, "host entry B")
+
+
+def test_bad_arguments(fmm):
+    w = workloads.config(1, N=100)
+    for kw in (dict(order_n=0, leaf_size=8, theta=0.5), dict(order_n=13, leaf_size=8, theta=0.5),
+               dict(order_n=2, leaf_size=0, theta=0.5), dict(order_n=2, leaf_size=8, theta=0.0),
+               dict(order_n=2, leaf_size=8, theta=float("nan"))):
+        with pytest.raises(fmm.FmmError):
+            fmm.fmm_plan_create(*w.arrays(), w.q, **kw)
+    bad = w.pz.copy()
+    bad[3] = np.nan
+    with pytest.raises(fmm.FmmError):
+        fmm.fmm_plan_create(w.x, w.y, w.z, w.px, w.py, bad, w.q, order_n=2, leaf_size=8, theta=0.5)
