@@ -161,6 +161,11 @@ void fmm_plan_destroy(fmm_plan_t *plan);
 /* Number of kernel launches the library has enqueued in this process (bench.py's gpu_launches). */
 int64_t fmm_launch_count(void);
 
+/* Diagnostic: sustained rate of dependent-free DFMA chains on the FP64 pipe, in TFLOP/s (2 flop per
+ * DFMA), best of 3 timed launches of ~1.2e12 flop.  The roofline denominator bench.py quotes beside
+ * the nominal 148 SM x 64 lanes x 2 x clock.  Synchronises the stream. */
+int fmm_probe_fp64_peak(double *tflops, double *ms, void *cuda_stream);
+
 const char *fmm_strerror(int code);
 const char *fmm_last_error(const fmm_plan_t *plan);  /* plan may be NULL: last error of a plan-less call */
 const char *fmm_version(void);

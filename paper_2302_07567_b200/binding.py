@@ -63,7 +63,7 @@ class fmm_export_t(C.Structure):
 
 EXPORTED_SYMBOLS = ["fmm_plan_create", "fmm_plan_update", "fmm_eval", "fmm_direct", "fmm_field_host",
                     "fmm_plan_set_timing", "fmm_plan_stats", "fmm_plan_export", "fmm_plan_destroy",
-                    "fmm_launch_count", "fmm_strerror", "fmm_last_error", "fmm_version"]
+                    "fmm_launch_count", "fmm_probe_fp64_peak", "fmm_strerror", "fmm_last_error", "fmm_version"]
 
 _lib = None
 
@@ -104,6 +104,8 @@ def load_library():
     lib.fmm_plan_destroy.restype = None
     lib.fmm_plan_destroy.argtypes = [vp]
     lib.fmm_launch_count.restype = C.c_int64
+    lib.fmm_probe_fp64_peak.restype = C.c_int
+    lib.fmm_probe_fp64_peak.argtypes = [_dp, _dp, vp]
     lib.fmm_strerror.restype = C.c_char_p
     lib.fmm_strerror.argtypes = [C.c_int]
     lib.fmm_last_error.restype = C.c_char_p
@@ -340,3 +342,11 @@ def fmm_field_host(x, y, z, px, py, pz, q=None, *, order_n, leaf_size, theta, ga
 
 def fmm_launch_count() -> int:
     return int(load_library().fmm_launch_count())
+
+
+def fmm_probe_fp64_peak() -> float:
+    """Sustained DFMA rate of the device in TFLOP/s (diagnostic; roofline denominator)."""
+    _require_cuda()
+    t, ms = C.c_double(), C.c_double()
+    _check(load_library().fmm_probe_fp64_peak(C.byref(t), C.byref(ms), _stream_ptr()))
+    return float(t.value)
