@@ -67,6 +67,7 @@ struct fmm_plan {
     int32_t *node_hi;
     double *bbox;           // [nodes+1][6]
     double *node_geo;       // [nodes+1][4] : r^2 (Alg 5.6 squared), cx, cy, cz (box centres)
+    double *node_xi;        // [nodes+1][3][16] : proxy points per axis (I-3), filled by pairs_m2l
     // interaction lists, CSR by target node id (offset arrays indexed by node id, length nodes+2)
     int32_t *p2p_off, *p2p_src, *m2l_off, *m2l_src;
     int64_t n_p2p, n_m2l, cap_p2p, cap_m2l;
@@ -76,6 +77,7 @@ struct fmm_plan {
     // expansions
     double *M;              // [nodes+1][P][4]
     double *L;              // [nodes+1][P][6]
+    double *MZ;             // [nodes+1][P][4] (m0, m1, m2, 0) x relative z proxy coordinate, filled by pairs_m2l
     double *near_;          // [6][N] tree order, P2P result
     // timing
     int timing;

@@ -210,23 +210,115 @@ struct m2l_cfg {
     static constexpr int BATCHES = (P + 1023) / 1024;
     static constexpr int PER = (P + BATCHES - 1) / BATCHES;
     static constexpr int THREADS = ((PER + 31) / 32) * 32;
+    // two resident blocks per SM while 2 x THREADS x 88 registers fit the register file (the dependent
+    // seed -> series chain of inv_r3 needs >= 5 warps per sub-partition to keep the FP64 pipe fed)
+#ifndef M2L_MINB
+#define M2L_MINB 2
+#endif
+    static constexpr int MINB = (THREADS <= 372) ? M2L_MINB : 1;
 };
 
 struct cheb13 {
     double c[FMM_MAX_ORDER + 1];
 };
 
+// ---- 1-D bulk TMA copy (global -> shared, completion on an mbarrier) ----------------------------
+__device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint64_t *bar, int count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t *bar, uint32_t bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(void *dst, const void *src, uint32_t bytes, uint64_t *bar)
+{
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(smem_u32(dst)),
+                 "l"(src), "r"(bytes), "r"(smem_u32(bar))
+                 : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity)
+{
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "WAIT_LOOP:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@p bra WAIT_DONE;\n"
+        "bra WAIT_LOOP;\n"
+        "WAIT_DONE:\n"
+        "}\n" ::"r"(smem_u32(bar)),
+        "r"(parity)
+        : "memory");
+}
+
+__device__ __forceinline__ void mbar_arrive(uint64_t *bar)
+{
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+
+// Per-node tables for M2L, filled once per evaluation:
+//   xi[node][g][k]  proxy points per axis (reading I-3), row stride M2L_XI_STRIDE.  Row 2 (z) holds the points
+//                   RELATIVE to the box centre z0 = (a_z + b_z)/2, and z0 itself sits in xi[node][2][15].
+//   MZ[node][nu][4] = (m0, m1, m2, 0) * zrel_{nu3}: with it  sum_nu m_k w dz = (zt - z0) sum_nu m_k w - sum_nu MZ_k w,
+//                   so the innermost loop needs no dz and all of its accumulate-FMAs share the operand w.
+#define M2L_XI_STRIDE 16
+#define M2L_XI_BYTES (3 * M2L_XI_STRIDE * 8)
+__global__ void m2l_proxy_points(int nodes, int n1, cheb13 ch, const double *__restrict__ bbox, double *__restrict__ xi)
+{
+    int q = blockIdx.x * blockDim.x + threadIdx.x;
+    if (q >= (nodes + 1) * 3 * M2L_XI_STRIDE) return;
+    int k = q % M2L_XI_STRIDE, g = (q / M2L_XI_STRIDE) % 3, i = q / (3 * M2L_XI_STRIDE);
+    const double *bs = bbox + 6 * (size_t)i;
+    double v = 0.0;
+    if (i >= 1) {
+        const double mid = __dmul_rn(__dadd_rn(bs[g], bs[3 + g]), 0.5);
+        if (k < n1) {  // xi = (a+b)/2 + (b-a)/2 c_k, rounded as the sequence mul, mul, add
+            v = __dadd_rn(mid, __dmul_rn(__dmul_rn(__dsub_rn(bs[3 + g], bs[g]), 0.5), ch.c[k]));
+            if (g == 2) v = __dsub_rn(v, mid);
+        } else if (g == 2 && k == M2L_XI_STRIDE - 1) {
+            v = mid;
+        }
+    }
+    xi[q] = v;
+}
+
+__global__ void m2l_moment_z(int64_t count, int P, int n1, const double *__restrict__ xi, const double *__restrict__ M, double *__restrict__ MZ)
+{
+    int64_t q = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;  // (node, nu)
+    if (q >= count) return;
+    int64_t node = q / P;
+    int nu = (int)(q - node * P);
+    const double zr = xi[(size_t)node * 3 * M2L_XI_STRIDE + 2 * M2L_XI_STRIDE + nu % n1];
+    const double2 *m = reinterpret_cast<const double2 *>(M + 4 * q);
+    double2 m01 = m[0], m23 = m[1];
+    double2 *o = reinterpret_cast<double2 *>(MZ + 4 * q);
+    o[0] = make_double2(m01.x * zr, m01.y * zr);
+    o[1] = make_double2(m23.x * zr, 0.0);
+}
+
+// Shared memory of one block: M2L_STAGES stages, each = the source node's moments (P x 4 doubles, one contiguous
+// 32 P byte tile of M) + its proxy coordinates per axis, both fetched by 1-D bulk TMA copies that complete on the
+// stage's `full` mbarrier.  There is no block-wide barrier in the source loop: every warp walks the CSR row at its
+// own pace, waits on full[stage], and releases the stage on empty[stage] (one arrival per warp); thread 0 refills a
+// stage as soon as all warps have left it, so warps may drift up to M2L_STAGES-1 sources apart.
+#define M2L_STAGES 3
 template <int N1>
-__global__ void __launch_bounds__(m2l_cfg<N1>::THREADS) m2l_kernel(cheb13 ch, double g2, const int32_t *__restrict__ order,
-                                                                   const int32_t *__restrict__ off, const int32_t *__restrict__ src,
-                                                                   const double *__restrict__ bbox, const double *__restrict__ M,
-                                                                   double *__restrict__ L)
+__global__ void __launch_bounds__(m2l_cfg<N1>::THREADS, m2l_cfg<N1>::MINB) m2l_kernel(double g2, const int32_t *__restrict__ order,
+                                                                                      const int32_t *__restrict__ off, const int32_t *__restrict__ src,
+                                                                                      const double *__restrict__ xi, const double *__restrict__ M,
+                                                                                      const double *__restrict__ MZ, double *__restrict__ L)
 {
     constexpr int P = m2l_cfg<N1>::P;
     constexpr int THREADS = m2l_cfg<N1>::THREADS;
-    extern __shared__ double2 m2l_smem[];
-    double2 *Ms = m2l_smem;                                                    // (m0,m1) (m2,m3) per source proxy
-    double(*xs)[N1 + 1] = reinterpret_cast<double(*)[N1 + 1]>(m2l_smem + 2 * P);  // source proxy coordinates per axis
+    constexpr int WARPS = THREADS / 32;
+    constexpr int S = M2L_STAGES;
+    constexpr uint32_t TILE_BYTES = 32u * P;
+    constexpr uint32_t STAGE_BYTES = 2 * TILE_BYTES + M2L_XI_BYTES;
+    extern __shared__ __align__(128) unsigned char m2l_smem_raw[];
+    uint64_t *full = reinterpret_cast<uint64_t *>(m2l_smem_raw + S * STAGE_BYTES);
+    uint64_t *empty = full + S;
     const int t = order[blockIdx.x];
     const int e0 = off[t], e1 = off[t + 1];
     double *Lt = L + 6 * (size_t)P * t;
@@ -234,66 +326,100 @@ __global__ void __launch_bounds__(m2l_cfg<N1>::THREADS) m2l_kernel(cheb13 ch, do
         for (int k = threadIdx.x; k < 6 * P; k += THREADS) Lt[k] = 0.0;
         return;
     }
-    const double *bt = bbox + 6 * (size_t)t;
+    if (threadIdx.x == 0) {
+        for (int k = 0; k < S; ++k) {
+            mbar_init(&full[k], 1);
+            mbar_init(&empty[k], WARPS);
+        }
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+    const int ne = e1 - e0;
+    const int total = m2l_cfg<N1>::BATCHES * ne;  // loads in the order they are consumed
+    auto issue = [&](int q) {                     // thread 0 only
+        const int st = q % S;
+        const int sn = src[e0 + q % ne];
+        unsigned char *dst = m2l_smem_raw + (size_t)st * STAGE_BYTES;
+        mbar_expect_tx(&full[st], STAGE_BYTES);
+        bulk_g2s(dst, M + 4 * (size_t)P * sn, TILE_BYTES, &full[st]);
+        bulk_g2s(dst + TILE_BYTES, MZ + 4 * (size_t)P * sn, TILE_BYTES, &full[st]);
+        bulk_g2s(dst + 2 * TILE_BYTES, xi + (size_t)sn * 3 * M2L_XI_STRIDE, M2L_XI_BYTES, &full[st]);
+    };
+    if (threadIdx.x == 0)
+        for (int q = 0; q < S - 1 && q < total; ++q) issue(q);
+    const double *xt3 = xi + (size_t)t * 3 * M2L_XI_STRIDE;
+    int i = 0;  // consumed loads so far
     for (int mu0 = 0; mu0 < P; mu0 += THREADS) {
         const int mu = mu0 + threadIdx.x;
         const bool live = mu < P;
         const int a = live ? mu / (N1 * N1) : 0, b = live ? (mu / N1) % N1 : 0, c3 = live ? mu % N1 : 0;
-        // I-3: xi = (a+b)/2 + (b-a)/2 c_k, rounded as the sequence mul, mul, add
-        const double xt = __dadd_rn(__dmul_rn(__dadd_rn(bt[0], bt[3]), 0.5), __dmul_rn(__dmul_rn(__dsub_rn(bt[3], bt[0]), 0.5), ch.c[a]));
-        const double yt = __dadd_rn(__dmul_rn(__dadd_rn(bt[1], bt[4]), 0.5), __dmul_rn(__dmul_rn(__dsub_rn(bt[4], bt[1]), 0.5), ch.c[b]));
-        const double zt = __dadd_rn(__dmul_rn(__dadd_rn(bt[2], bt[5]), 0.5), __dmul_rn(__dmul_rn(__dsub_rn(bt[5], bt[2]), 0.5), ch.c[c3]));
+        // the target's z proxy point: centre + relative part, exactly as the oracle's xi (mid + half c_k)
+        const double xt = xt3[a], yt = xt3[M2L_XI_STRIDE + b];
+        const double zt = __dadd_rn(xt3[2 * M2L_XI_STRIDE + M2L_XI_STRIDE - 1], xt3[2 * M2L_XI_STRIDE + c3]);
         double ex = 0, ey = 0, ez = 0, bx = 0, by = 0, bz = 0;
-        for (int e = e0; e < e1; ++e) {
-            const int s = src[e];
-            __syncthreads();
-            {
-                const double2 *Mg = reinterpret_cast<const double2 *>(M + 4 * (size_t)P * s);
-                for (int k = threadIdx.x; k < 2 * P; k += THREADS) Ms[k] = Mg[k];
-                if (threadIdx.x < 3 * N1) {
-                    int g = threadIdx.x / N1, k = threadIdx.x - g * N1;
-                    const double *bs = bbox + 6 * (size_t)s;
-                    xs[g][k] = __dadd_rn(__dmul_rn(__dadd_rn(bs[g], bs[3 + g]), 0.5),
-                                         __dmul_rn(__dmul_rn(__dsub_rn(bs[3 + g], bs[g]), 0.5), ch.c[k]));
+        for (int e = 0; e < ne; ++e, ++i) {
+            const int st = i % S;
+            if (threadIdx.x == 0) {
+                const int q = i + S - 1;
+                if (q < total) {
+                    if (q >= S) mbar_wait(&empty[q % S], (uint32_t)((q / S - 1) & 1));  // all warps left that stage
+                    issue(q);
                 }
             }
-            __syncthreads();
-            double dz[N1], gz2[N1];
+            __syncwarp();
+            mbar_wait(&full[st], (uint32_t)((i / S) & 1));
+            const double2 *Ms = reinterpret_cast<const double2 *>(m2l_smem_raw + (size_t)st * STAGE_BYTES);
+            const double2 *Zs = reinterpret_cast<const double2 *>(m2l_smem_raw + (size_t)st * STAGE_BYTES + TILE_BYTES);
+            const double *xs = reinterpret_cast<const double *>(m2l_smem_raw + (size_t)st * STAGE_BYTES + 2 * TILE_BYTES);
+            const double ztr = zt - xs[2 * M2L_XI_STRIDE + M2L_XI_STRIDE - 1];  // target z relative to the source box centre
+            double gz2[N1];
 #pragma unroll
             for (int k = 0; k < N1; ++k) {
-                dz[k] = zt - xs[2][k];
-                gz2[k] = (g2 * dz[k]) * dz[k];
+                const double dz = ztr - xs[2 * M2L_XI_STRIDE + k];
+                gz2[k] = (g2 * dz) * dz;
             }
+            double T0 = 0, T1 = 0, T2 = 0;          // sum over the whole source of A0, A1, A2
+            double S0 = 0, S1 = 0, S2 = 0;          // sum over the whole source of MZ_k w
             for (int a2 = 0; a2 < N1; ++a2) {
-                const double dx = xt - xs[0][a2];
+                const double dx = xt - xs[a2];
                 const double dx2 = dx * dx;
 #pragma unroll 1
                 for (int b2 = 0; b2 < N1; ++b2) {
-                    const double dy = yt - xs[1][b2];
+                    const double dy = yt - xs[M2L_XI_STRIDE + b2];
                     const double s2 = fma(dy, dy, dx2);
                     const double2 *row = Ms + 2 * ((a2 * N1 + b2) * N1);
-                    double A0 = 0, A1 = 0, A2 = 0, A3 = 0, Z0 = 0, Z1 = 0, Z2 = 0;
+                    const double2 *rowz = Zs + 2 * ((a2 * N1 + b2) * N1);
+                    double A0 = 0, A1 = 0, A2 = 0, A3 = 0;
 #pragma unroll
                     for (int c2 = 0; c2 < N1; ++c2) {
                         const double w = inv_r3(s2 + gz2[c2]);
                         const double2 m01 = row[2 * c2], m23 = row[2 * c2 + 1];
-                        const double wz = w * dz[c2];
+                        const double2 z01 = rowz[2 * c2];
+                        const double z2 = rowz[2 * c2 + 1].x;
                         A0 = fma(m01.x, w, A0);
                         A1 = fma(m01.y, w, A1);
                         A2 = fma(m23.x, w, A2);
                         A3 = fma(m23.y, w, A3);
-                        Z0 = fma(m01.x, wz, Z0);
-                        Z1 = fma(m01.y, wz, Z1);
-                        Z2 = fma(m23.x, wz, Z2);
+                        S0 = fma(z01.x, w, S0);
+                        S1 = fma(z01.y, w, S1);
+                        S2 = fma(z2, w, S2);
                     }
                     ex = fma(A0, dx, ex);
                     ey = fma(A0, dy, ey);
-                    ez += Z0;
-                    bx = fma(-A3, dy, bx + Z2);
-                    by = fma(A3, dx, by - Z1);
+                    bx = fma(-A3, dy, bx);
+                    by = fma(A3, dx, by);
                     bz = fma(A1, dy, fma(-A2, dx, bz));
+                    T0 += A0;
+                    T1 += A1;
+                    T2 += A2;
                 }
             }
+            // sum m_k w dz = ztr sum m_k w - sum MZ_k w:  E_z += Z0,  B_x += Z2,  B_y -= Z1
+            ez += fma(ztr, T0, -S0);
+            bx += fma(ztr, T2, -S2);
+            by -= fma(ztr, T1, -S1);
+            __syncwarp();
+            if ((threadIdx.x & 31) == 0) mbar_arrive(&empty[st]);
         }
         if (live) {
             double *o = Lt + 6 * (size_t)mu;
@@ -303,14 +429,16 @@ __global__ void __launch_bounds__(m2l_cfg<N1>::THREADS) m2l_kernel(cheb13 ch, do
 }
 
 template <int N1>
-static int launch_m2l(fmm_plan *p, const cheb13 &ch)
+static int launch_m2l(fmm_plan *p)
 {
     fmm_ctx *c = &p->ctx;
-    const size_t smem = sizeof(double2) * 2 * m2l_cfg<N1>::P + sizeof(double) * 3 * (N1 + 1);
+    const size_t smem = M2L_STAGES * ((size_t)64 * m2l_cfg<N1>::P + M2L_XI_BYTES) + 2 * M2L_STAGES * sizeof(uint64_t);
     if (smem > 48 * 1024)
         FMM_CUDA(c, cudaFuncSetAttribute((const void *)m2l_kernel<N1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    m2l_kernel<N1><<<(unsigned)p->nodes, m2l_cfg<N1>::THREADS, smem, c->stream>>>(ch, p->gamma_bar * p->gamma_bar, p->m2l_order, p->m2l_off,
-                                                                               p->m2l_src, p->bbox, p->M, p->L);
+    // the default carveout leaves room for one block only; ask for enough shared memory for every resident block
+    FMM_CUDA(c, cudaFuncSetAttribute((const void *)m2l_kernel<N1>, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared));
+    m2l_kernel<N1><<<(unsigned)p->nodes, m2l_cfg<N1>::THREADS, smem, c->stream>>>(p->gamma_bar * p->gamma_bar, p->m2l_order, p->m2l_off,
+                                                                               p->m2l_src, p->node_xi, p->M, p->MZ, p->L);
     FMM_LAUNCH_CHECK(c, "m2l_kernel");
     return FMM_OK;
 }
@@ -322,19 +450,28 @@ int pairs_m2l(fmm_plan *p)
     for (int k = 0; k <= p->n; ++k) ch.c[k] = sin(FMM_PI * (double)(p->n - 2 * k) / (double)(2 * p->n));  // I-1
     ch.c[0] = 1.0;
     ch.c[p->n] = -1.0;
+    {
+        fmm_ctx *c = &p->ctx;
+        int count = (int)(p->nodes + 1) * 3 * M2L_XI_STRIDE;
+        m2l_proxy_points<<<(count + 255) / 256, 256, 0, c->stream>>>((int)p->nodes, p->n1, ch, p->bbox, p->node_xi);
+        FMM_LAUNCH_CHECK(c, "m2l_proxy_points");
+        int64_t cnt = (p->nodes + 1) * (int64_t)p->P;
+        m2l_moment_z<<<(unsigned)((cnt + 255) / 256), 256, 0, c->stream>>>(cnt, p->P, p->n1, p->node_xi, p->M, p->MZ);
+        FMM_LAUNCH_CHECK(c, "m2l_moment_z");
+    }
     switch (p->n1) {
-        case 2: return launch_m2l<2>(p, ch);
-        case 3: return launch_m2l<3>(p, ch);
-        case 4: return launch_m2l<4>(p, ch);
-        case 5: return launch_m2l<5>(p, ch);
-        case 6: return launch_m2l<6>(p, ch);
-        case 7: return launch_m2l<7>(p, ch);
-        case 8: return launch_m2l<8>(p, ch);
-        case 9: return launch_m2l<9>(p, ch);
-        case 10: return launch_m2l<10>(p, ch);
-        case 11: return launch_m2l<11>(p, ch);
-        case 12: return launch_m2l<12>(p, ch);
-        case 13: return launch_m2l<13>(p, ch);
+        case 2: return launch_m2l<2>(p);
+        case 3: return launch_m2l<3>(p);
+        case 4: return launch_m2l<4>(p);
+        case 5: return launch_m2l<5>(p);
+        case 6: return launch_m2l<6>(p);
+        case 7: return launch_m2l<7>(p);
+        case 8: return launch_m2l<8>(p);
+        case 9: return launch_m2l<9>(p);
+        case 10: return launch_m2l<10>(p);
+        case 11: return launch_m2l<11>(p);
+        case 12: return launch_m2l<12>(p);
+        case 13: return launch_m2l<13>(p);
     }
     return FMM_EINVAL;
 }
