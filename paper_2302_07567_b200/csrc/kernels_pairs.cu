@@ -215,7 +215,11 @@ struct m2l_cfg {
 #ifndef M2L_MINB
 #define M2L_MINB 2
 #endif
-    static constexpr int MINB = (THREADS <= 372) ? M2L_MINB : 1;
+    static constexpr int MINB = (THREADS + 32 <= 400) ? M2L_MINB : 1;
+    // pipeline depth: as many stages of (M tile + MZ tile + proxy coordinates) as fit 227 KB, at most 3
+    static constexpr int STAGE_BYTES = 64 * P + 3 * 16 * 8;
+    static constexpr int FIT = (227 * 1024 - 64) / STAGE_BYTES;
+    static constexpr int STAGES = FIT >= 3 ? 3 : (FIT >= 2 ? 2 : 1);
 };
 
 struct cheb13 {
@@ -298,14 +302,13 @@ __global__ void m2l_moment_z(int64_t count, int P, int n1, const double *__restr
     o[1] = make_double2(m23.x * zr, 0.0);
 }
 
-// Shared memory of one block: M2L_STAGES stages, each = the source node's moments (P x 4 doubles, one contiguous
+// Shared memory of one block: m2l_cfg::STAGES stages, each = the source node's moments (P x 4 doubles, one contiguous
 // 32 P byte tile of M) + its proxy coordinates per axis, both fetched by 1-D bulk TMA copies that complete on the
 // stage's `full` mbarrier.  There is no block-wide barrier in the source loop: every warp walks the CSR row at its
-// own pace, waits on full[stage], and releases the stage on empty[stage] (one arrival per warp); thread 0 refills a
-// stage as soon as all warps have left it, so warps may drift up to M2L_STAGES-1 sources apart.
-#define M2L_STAGES 3
+// own pace, waits on full[stage], and releases the stage on empty[stage] (one arrival per warp); an extra producer
+// warp refills a stage as soon as all consumer warps have left it, so warps may drift up to STAGES-1 sources apart.
 template <int N1>
-__global__ void __launch_bounds__(m2l_cfg<N1>::THREADS, m2l_cfg<N1>::MINB) m2l_kernel(double g2, const int32_t *__restrict__ order,
+__global__ void __launch_bounds__(m2l_cfg<N1>::THREADS + 32, m2l_cfg<N1>::MINB) m2l_kernel(double g2, const int32_t *__restrict__ order,
                                                                                       const int32_t *__restrict__ off, const int32_t *__restrict__ src,
                                                                                       const double *__restrict__ xi, const double *__restrict__ M,
                                                                                       const double *__restrict__ MZ, double *__restrict__ L)
@@ -313,7 +316,7 @@ __global__ void __launch_bounds__(m2l_cfg<N1>::THREADS, m2l_cfg<N1>::MINB) m2l_k
     constexpr int P = m2l_cfg<N1>::P;
     constexpr int THREADS = m2l_cfg<N1>::THREADS;
     constexpr int WARPS = THREADS / 32;
-    constexpr int S = M2L_STAGES;
+    constexpr int S = m2l_cfg<N1>::STAGES;
     constexpr uint32_t TILE_BYTES = 32u * P;
     constexpr uint32_t STAGE_BYTES = 2 * TILE_BYTES + M2L_XI_BYTES;
     extern __shared__ __align__(128) unsigned char m2l_smem_raw[];
@@ -323,7 +326,7 @@ __global__ void __launch_bounds__(m2l_cfg<N1>::THREADS, m2l_cfg<N1>::MINB) m2l_k
     const int e0 = off[t], e1 = off[t + 1];
     double *Lt = L + 6 * (size_t)P * t;
     if (e0 == e1) {  // no far-field sources: the local expansion starts at zero (L2L adds into it)
-        for (int k = threadIdx.x; k < 6 * P; k += THREADS) Lt[k] = 0.0;
+        for (int k = threadIdx.x; k < 6 * P; k += THREADS + 32) Lt[k] = 0.0;
         return;
     }
     if (threadIdx.x == 0) {
@@ -345,8 +348,14 @@ __global__ void __launch_bounds__(m2l_cfg<N1>::THREADS, m2l_cfg<N1>::MINB) m2l_k
         bulk_g2s(dst + TILE_BYTES, MZ + 4 * (size_t)P * sn, TILE_BYTES, &full[st]);
         bulk_g2s(dst + 2 * TILE_BYTES, xi + (size_t)sn * 3 * M2L_XI_STRIDE, M2L_XI_BYTES, &full[st]);
     };
-    if (threadIdx.x == 0)
-        for (int q = 0; q < S - 1 && q < total; ++q) issue(q);
+    if (threadIdx.x >= THREADS) {  // producer warp: one lane keeps the stages filled, then the warp retires
+        if (threadIdx.x == THREADS)
+            for (int q = 0; q < total; ++q) {
+                if (q >= S) mbar_wait(&empty[q % S], (uint32_t)((q / S - 1) & 1));  // all consumer warps left that stage
+                issue(q);
+            }
+        return;
+    }
     const double *xt3 = xi + (size_t)t * 3 * M2L_XI_STRIDE;
     int i = 0;  // consumed loads so far
     for (int mu0 = 0; mu0 < P; mu0 += THREADS) {
@@ -359,14 +368,6 @@ __global__ void __launch_bounds__(m2l_cfg<N1>::THREADS, m2l_cfg<N1>::MINB) m2l_k
         double ex = 0, ey = 0, ez = 0, bx = 0, by = 0, bz = 0;
         for (int e = 0; e < ne; ++e, ++i) {
             const int st = i % S;
-            if (threadIdx.x == 0) {
-                const int q = i + S - 1;
-                if (q < total) {
-                    if (q >= S) mbar_wait(&empty[q % S], (uint32_t)((q / S - 1) & 1));  // all warps left that stage
-                    issue(q);
-                }
-            }
-            __syncwarp();
             mbar_wait(&full[st], (uint32_t)((i / S) & 1));
             const double2 *Ms = reinterpret_cast<const double2 *>(m2l_smem_raw + (size_t)st * STAGE_BYTES);
             const double2 *Zs = reinterpret_cast<const double2 *>(m2l_smem_raw + (size_t)st * STAGE_BYTES + TILE_BYTES);
@@ -432,12 +433,12 @@ template <int N1>
 static int launch_m2l(fmm_plan *p)
 {
     fmm_ctx *c = &p->ctx;
-    const size_t smem = M2L_STAGES * ((size_t)64 * m2l_cfg<N1>::P + M2L_XI_BYTES) + 2 * M2L_STAGES * sizeof(uint64_t);
+    const size_t smem = m2l_cfg<N1>::STAGES * ((size_t)64 * m2l_cfg<N1>::P + M2L_XI_BYTES) + 2 * m2l_cfg<N1>::STAGES * sizeof(uint64_t);
     if (smem > 48 * 1024)
         FMM_CUDA(c, cudaFuncSetAttribute((const void *)m2l_kernel<N1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     // the default carveout leaves room for one block only; ask for enough shared memory for every resident block
     FMM_CUDA(c, cudaFuncSetAttribute((const void *)m2l_kernel<N1>, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared));
-    m2l_kernel<N1><<<(unsigned)p->nodes, m2l_cfg<N1>::THREADS, smem, c->stream>>>(p->gamma_bar * p->gamma_bar, p->m2l_order, p->m2l_off,
+    m2l_kernel<N1><<<(unsigned)p->nodes, m2l_cfg<N1>::THREADS + 32, smem, c->stream>>>(p->gamma_bar * p->gamma_bar, p->m2l_order, p->m2l_off,
                                                                                p->m2l_src, p->node_xi, p->M, p->MZ, p->L);
     FMM_LAUNCH_CHECK(c, "m2l_kernel");
     return FMM_OK;

@@ -57,6 +57,12 @@ def small_cases():
     yield "config4_small", w, 6, 256, 0.4
     w = workloads.paper_cube(N=6000, order_n=2)  # identical momenta, N0 = 27
     yield "paper_cube_n2", w, 2, 27, 0.5
+    w = workloads.config(2, N=3000)           # n = 8: P = 729, M2L threads = 736 (one block per SM)
+    yield "order8", w, 8, 200, 0.5
+    w = workloads.config(3, N=2500)           # n = 10: P = 1331 > 1024 -> two proxy batches per target node, 2 pipeline stages
+    yield "order10_batches", w, 10, 300, 0.5
+    w = workloads.config(1, N=1500)           # n = 12 (FMM_MAX_ORDER): P = 2197, three batches, single-stage pipeline
+    yield "order12_max", w, 12, 200, 0.45
     w = workloads.config(1, N=50)             # N <= N0: the root is a leaf (G23)
     yield "single_leaf", w, 4, 64, 0.5
     w = workloads.config(1, N=3)              # N0 = 1: an empty leaf appears
