@@ -165,6 +165,23 @@ class ClockSampler:
 
 
 # ------------------------------------------------------------------------------------------------
+# N > 1: replicas only.  The only cross-rank traffic is the barrier and this MAX.
+# ------------------------------------------------------------------------------------------------
+def max_over_ranks(ms, world, device=None):
+    """Slowest rank's device time in ms (all_reduce MAX over the default process group when world > 1)."""
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([float(ms)], dtype=torch.float64, device=device if device is not None else "cpu")
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def aggregate_throughput(world, n_per_rank, steps, ms_total):
+    """Whole-job particles/s: every rank evaluates its own replica of n_per_rank particles `steps` times."""
+    return world * n_per_rank * steps / (ms_total * 1e-3)
+
+
 def run_cuda(args):
     import torch
     import torch.distributed as dist
@@ -221,12 +238,8 @@ def run_cuda(args):
                 stage_ms.setdefault(key, []).append(st[key])
         barrier()
     launches = fmm.fmm_launch_count() - l0
-    ms_total = sum(a.elapsed_time(b) for a, b in ev)
-    t = torch.tensor([ms_total], dtype=torch.float64, device=dev)
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    ms_total = float(t.item())
-    value = world * w.N * args.steps / (ms_total * 1e-3)
+    ms_total = max_over_ranks(sum(a.elapsed_time(b) for a, b in ev), world, dev)
+    value = aggregate_throughput(world, w.N, args.steps, ms_total)
     clocks = clk.summary()
 
     # ---- end to end through the host entry point (pinned host buffers, copies inside the timed region)
@@ -241,10 +254,7 @@ def run_cuda(args):
         fmm.fmm_field_host(*h_in, w.q, out=h_out, **prm)
     e1.record()
     barrier()
-    t = torch.tensor([e0.elapsed_time(e1)], dtype=torch.float64, device=dev)
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    e2e_value = world * w.N * args.steps / (float(t.item()) * 1e-3)
+    e2e_value = aggregate_throughput(world, w.N, args.steps, max_over_ranks(e0.elapsed_time(e1), world, dev))
 
     if rank != 0:
         if world > 1:
