@@ -52,62 +52,102 @@ __device__ __forceinline__ void basis_1d(int n, const cheb_t &ch, double a, doub
 }
 
 // ---------------------------------------------------------------------------------------
-// a4: P2M.  One block per leaf; thread nu accumulates M_{S,nu} = sum_j l_nu(x_j) m_j over the leaf's
-// particles in tree order.  The 1-D basis values of a chunk of particles are staged in shared memory.
+// a4: P2M.  One block per leaf.  A thread owns one (nu1, nu2) column of the proxy grid and keeps the
+// 4 x (n+1) moments of that column in registers:  M[nu1,nu2,:][k] += (l_x l_y m_k) l_z[:]  per particle.
+// The block's threads form G = THREADS / (n+1)^2 groups that take the particles of a chunk round-robin;
+// the groups' partial sums are then added in group order (fixed order: deterministic, no atomics).
+// 1-D basis values and weights of a chunk of particles are staged in shared memory.
 // ---------------------------------------------------------------------------------------
 #define P2M_THREADS 256
-#define P2M_CHUNK 128
+#define P2M_CHUNK 64
 
-__global__ void __launch_bounds__(P2M_THREADS) p2m_kernel(int n, cheb_t ch, int leaves, const int32_t *__restrict__ node_lo,
+template <int N1>
+struct p2m_cfg {
+    static constexpr int COLS = N1 * N1;
+    static constexpr int G0 = P2M_THREADS / COLS;
+    static constexpr int G = G0 > 8 ? 8 : (G0 < 1 ? 1 : G0);
+    static constexpr int P = N1 * N1 * N1;
+    static constexpr size_t SMEM = sizeof(double) * (3 * N1 * P2M_CHUNK + 4 * P2M_CHUNK + (G > 1 ? 4 * P : 0));
+};
+
+template <int N1>
+__global__ void __launch_bounds__(P2M_THREADS) p2m_kernel(cheb_t ch, int leaves, const int32_t *__restrict__ node_lo,
                                                           const int32_t *__restrict__ node_hi, const double *__restrict__ bbox,
                                                           const double *__restrict__ tx, const double *__restrict__ ty,
                                                           const double *__restrict__ tz, const double *__restrict__ w0,
                                                           const double *__restrict__ w1, const double *__restrict__ w2,
                                                           const double *__restrict__ w3, double *__restrict__ M)
 {
+    constexpr int COLS = p2m_cfg<N1>::COLS, G = p2m_cfg<N1>::G, P = p2m_cfg<N1>::P, n = N1 - 1;
     extern __shared__ double sm[];
-    const int n1 = n + 1, P = n1 * n1 * n1;
-    double *bas = sm;                            // [3][n1][P2M_CHUNK]
-    double *wts = sm + 3 * n1 * P2M_CHUNK;       // [4][P2M_CHUNK]
-    int node = leaves + blockIdx.x;
-    int lo = node_lo[node], hi = node_hi[node];
+    double *bas = sm;                                  // [3][P2M_CHUNK][N1]
+    double *wts = sm + 3 * N1 * P2M_CHUNK;             // [P2M_CHUNK][4]
+    double *red = wts + 4 * P2M_CHUNK;                 // [P][4] (only if G > 1)
+    const int node = leaves + blockIdx.x;
+    const int lo = node_lo[node], hi = node_hi[node];
     const double *bb = bbox + 6 * (int64_t)node;
     double *Mn = M + 4 * (int64_t)P * node;
-    for (int nu0 = 0; nu0 < P; nu0 += P2M_THREADS) {
-        int nu = nu0 + threadIdx.x;
-        int a = nu / (n1 * n1), b = (nu / n1) % n1, c3 = nu % n1;
-        double acc0 = 0.0, acc1 = 0.0, acc2 = 0.0, acc3 = 0.0;
-        for (int j0 = lo; j0 < hi; j0 += P2M_CHUNK) {
-            int cnt = min(P2M_CHUNK, hi - j0);
-            __syncthreads();
-            for (int t = threadIdx.x; t < 3 * cnt; t += P2M_THREADS) {
-                int g = t / cnt, jj = t - g * cnt;
-                const double *coord = (g == 0) ? tx : (g == 1) ? ty : tz;
-                basis_1d(n, ch, bb[g], bb[3 + g], coord[j0 + jj], bas + (size_t)g * n1 * P2M_CHUNK + jj, P2M_CHUNK);
-            }
-            for (int t = threadIdx.x; t < cnt; t += P2M_THREADS) {
-                wts[t] = w0[j0 + t];
-                wts[P2M_CHUNK + t] = w1[j0 + t];
-                wts[2 * P2M_CHUNK + t] = w2[j0 + t];
-                wts[3 * P2M_CHUNK + t] = w3[j0 + t];
-            }
-            __syncthreads();
-            if (nu < P) {
-                const double *la = bas + (size_t)a * P2M_CHUNK, *lb = bas + (size_t)(n1 + b) * P2M_CHUNK,
-                             *lc = bas + (size_t)(2 * n1 + c3) * P2M_CHUNK;
-                for (int jj = 0; jj < cnt; ++jj) {
-                    double l = la[jj] * lb[jj] * lc[jj];
-                    acc0 = fma(l, wts[jj], acc0);
-                    acc1 = fma(l, wts[P2M_CHUNK + jj], acc1);
-                    acc2 = fma(l, wts[2 * P2M_CHUNK + jj], acc2);
-                    acc3 = fma(l, wts[3 * P2M_CHUNK + jj], acc3);
+    const int grp = threadIdx.x / COLS, col = threadIdx.x - grp * COLS;
+    const bool active = grp < G;
+    const int a = col / N1, b = col - a * N1;
+    double acc[4][N1];
+#pragma unroll
+    for (int k = 0; k < 4; ++k)
+#pragma unroll
+        for (int c = 0; c < N1; ++c) acc[k][c] = 0.0;
+    for (int j0 = lo; j0 < hi; j0 += P2M_CHUNK) {
+        const int cnt = min(P2M_CHUNK, hi - j0);
+        __syncthreads();
+        for (int t = threadIdx.x; t < 3 * cnt; t += P2M_THREADS) {
+            int g = t / cnt, jj = t - g * cnt;
+            const double *coord = (g == 0) ? tx : (g == 1) ? ty : tz;
+            basis_1d(n, ch, bb[g], bb[3 + g], coord[j0 + jj], bas + ((size_t)g * P2M_CHUNK + jj) * N1, 1);
+        }
+        for (int t = threadIdx.x; t < cnt; t += P2M_THREADS) {
+            wts[4 * t + 0] = w0[j0 + t];
+            wts[4 * t + 1] = w1[j0 + t];
+            wts[4 * t + 2] = w2[j0 + t];
+            wts[4 * t + 3] = w3[j0 + t];
+        }
+        __syncthreads();
+        if (active) {
+            for (int jj = grp; jj < cnt; jj += G) {
+                const double lab = bas[(size_t)jj * N1 + a] * bas[((size_t)P2M_CHUNK + jj) * N1 + b];
+                const double *lc = bas + ((size_t)2 * P2M_CHUNK + jj) * N1;
+                const double t0 = lab * wts[4 * jj], t1 = lab * wts[4 * jj + 1], t2 = lab * wts[4 * jj + 2], t3 = lab * wts[4 * jj + 3];
+#pragma unroll
+                for (int c = 0; c < N1; ++c) {
+                    const double l = lc[c];
+                    acc[0][c] = fma(t0, l, acc[0][c]);
+                    acc[1][c] = fma(t1, l, acc[1][c]);
+                    acc[2][c] = fma(t2, l, acc[2][c]);
+                    acc[3][c] = fma(t3, l, acc[3][c]);
                 }
             }
         }
-        if (nu < P) {
-            double *m = Mn + 4 * (int64_t)nu;
-            m[0] = acc0; m[1] = acc1; m[2] = acc2; m[3] = acc3;
+    }
+    // M[nu][k], nu = (a N1 + b) N1 + c
+    if (G == 1) {
+        if (active)
+#pragma unroll
+            for (int c = 0; c < N1; ++c) {
+                double *m = Mn + 4 * (int64_t)(col * N1 + c);
+                m[0] = acc[0][c]; m[1] = acc[1][c]; m[2] = acc[2][c]; m[3] = acc[3][c];
+            }
+    } else {
+        for (int g = 0; g < G; ++g) {  // group partial sums added in group order
+            __syncthreads();
+            if (grp == g)
+#pragma unroll
+                for (int c = 0; c < N1; ++c)
+#pragma unroll
+                    for (int k = 0; k < 4; ++k) {
+                        double *r = red + 4 * (col * N1 + c) + k;
+                        *r = (g == 0) ? acc[k][c] : (*r + acc[k][c]);
+                    }
         }
+        __syncthreads();
+        for (int e = threadIdx.x; e < 4 * P; e += P2M_THREADS) Mn[e] = red[e];
     }
 }
 
@@ -306,16 +346,36 @@ static int set_smem(fmm_ctx *c, const void *fn, size_t bytes)
     return FMM_OK;
 }
 
-int interp_p2m(fmm_plan *p)
+template <int N1>
+static int launch_p2m(fmm_plan *p, const cheb_t &ch)
 {
     fmm_ctx *c = &p->ctx;
-    cheb_t ch = host_cheb(p->n);
-    size_t smem = sizeof(double) * (3 * (size_t)p->n1 * P2M_CHUNK + 4 * P2M_CHUNK);
-    FMM_TRY(set_smem(c, (const void *)p2m_kernel, smem));
-    p2m_kernel<<<(unsigned)p->leaves, P2M_THREADS, smem, c->stream>>>(p->n, ch, (int)p->leaves, p->node_lo, p->node_hi, p->bbox,
-                                                                      p->tx, p->ty, p->tz, p->w0, p->w1, p->w2, p->w3, p->M);
+    const size_t smem = p2m_cfg<N1>::SMEM;
+    FMM_TRY(set_smem(c, (const void *)p2m_kernel<N1>, smem));
+    p2m_kernel<N1><<<(unsigned)p->leaves, P2M_THREADS, smem, c->stream>>>(ch, (int)p->leaves, p->node_lo, p->node_hi, p->bbox, p->tx, p->ty,
+                                                                        p->tz, p->w0, p->w1, p->w2, p->w3, p->M);
     FMM_LAUNCH_CHECK(c, "p2m_kernel");
     return FMM_OK;
+}
+
+int interp_p2m(fmm_plan *p)
+{
+    cheb_t ch = host_cheb(p->n);
+    switch (p->n1) {
+        case 2: return launch_p2m<2>(p, ch);
+        case 3: return launch_p2m<3>(p, ch);
+        case 4: return launch_p2m<4>(p, ch);
+        case 5: return launch_p2m<5>(p, ch);
+        case 6: return launch_p2m<6>(p, ch);
+        case 7: return launch_p2m<7>(p, ch);
+        case 8: return launch_p2m<8>(p, ch);
+        case 9: return launch_p2m<9>(p, ch);
+        case 10: return launch_p2m<10>(p, ch);
+        case 11: return launch_p2m<11>(p, ch);
+        case 12: return launch_p2m<12>(p, ch);
+        case 13: return launch_p2m<13>(p, ch);
+    }
+    return FMM_EINVAL;
 }
 
 int interp_m2m(fmm_plan *p)
