@@ -66,6 +66,11 @@ __device__ __forceinline__ void tile_interact(const double2 *tile, int count, do
 // a7: P2P.  One block per target leaf (blocks issued in descending-work order); one thread per
 // target particle; the source leaves of the CSR row are staged tile by tile.
 // ---------------------------------------------------------------------------------------
+// P2P_NT target particles per thread: the source tile is read once from shared memory for P2P_NT evaluations and the
+// accumulate-FMAs of the P2P_NT targets that share a source weight are adjacent (operand reuse).
+#ifndef P2P_NT
+#define P2P_NT 4
+#endif
 __global__ void __launch_bounds__(256) p2p_kernel(int N, double g2, const int32_t *__restrict__ order, const int32_t *__restrict__ off,
                                                   const int32_t *__restrict__ src, const int32_t *__restrict__ node_lo,
                                                   const int32_t *__restrict__ node_hi, const double *__restrict__ tx,
@@ -77,11 +82,15 @@ __global__ void __launch_bounds__(256) p2p_kernel(int N, double g2, const int32_
     const int t = order[blockIdx.x];
     const int tlo = node_lo[t], thi = node_hi[t];
     const int e0 = off[t], e1 = off[t + 1];
-    for (int i0 = tlo; i0 < thi; i0 += blockDim.x) {
-        int i = i0 + threadIdx.x;
-        bool live = i < thi;
-        double xt = live ? tx[i] : 0.0, yt = live ? ty[i] : 0.0, zt = live ? tz[i] : 0.0;
-        double ex = 0, ey = 0, ez = 0, bx = 0, by = 0, bz = 0;
+    for (int i0 = tlo; i0 < thi; i0 += P2P_NT * blockDim.x) {
+        double xt[P2P_NT], yt[P2P_NT], zt[P2P_NT], ex[P2P_NT], ey[P2P_NT], ez[P2P_NT], bx[P2P_NT], by[P2P_NT], bz[P2P_NT];
+#pragma unroll
+        for (int k = 0; k < P2P_NT; ++k) {
+            int i = i0 + k * blockDim.x + threadIdx.x;
+            bool live = i < thi;
+            xt[k] = live ? tx[i] : 0.0; yt[k] = live ? ty[i] : 0.0; zt[k] = live ? tz[i] : 0.0;
+            ex[k] = ey[k] = ez[k] = bx[k] = by[k] = bz[k] = 0.0;
+        }
         for (int e = e0; e < e1; ++e) {
             int s = src[e];
             int slo = node_lo[s], shi = node_hi[s];
@@ -90,16 +99,42 @@ __global__ void __launch_bounds__(256) p2p_kernel(int N, double g2, const int32_
                 __syncthreads();
                 stage_tile(tile, count, tx, ty, tz, w0, w1, w2, w3, j0);
                 __syncthreads();
-                tile_interact(tile, count, xt, yt, zt, g2, ex, ey, ez, bx, by, bz);
+#pragma unroll 2
+                for (int j = 0; j < count; ++j) {
+                    double2 a = tile[4 * j + 0], b = tile[4 * j + 1], c = tile[4 * j + 2], d = tile[4 * j + 3];
+                    double gx[P2P_NT], gy[P2P_NT], gz[P2P_NT];
+#pragma unroll
+                    for (int k = 0; k < P2P_NT; ++k) {
+                        double dx = xt[k] - a.x, dy = yt[k] - a.y, dz = zt[k] - b.x;
+                        double D = dx * dx;
+                        D = fma(dy, dy, D);
+                        D = fma(g2 * dz, dz, D);
+                        double w = inv_r3(D);
+                        gx[k] = w * dx; gy[k] = w * dy; gz[k] = w * dz;
+                    }
+                    const double m0 = b.y, m1 = c.x, m2 = c.y, m3 = d.x;
+#pragma unroll
+                    for (int k = 0; k < P2P_NT; ++k) { ex[k] = fma(m0, gx[k], ex[k]); ey[k] = fma(m0, gy[k], ey[k]); ez[k] = fma(m0, gz[k], ez[k]); }
+#pragma unroll
+                    for (int k = 0; k < P2P_NT; ++k) { bx[k] = fma(m2, gz[k], bx[k]); bz[k] = fma(-m2, gx[k], bz[k]); }
+#pragma unroll
+                    for (int k = 0; k < P2P_NT; ++k) { by[k] = fma(m3, gx[k], by[k]); bx[k] = fma(-m3, gy[k], bx[k]); }
+#pragma unroll
+                    for (int k = 0; k < P2P_NT; ++k) { bz[k] = fma(m1, gy[k], bz[k]); by[k] = fma(-m1, gz[k], by[k]); }
+                }
             }
         }
-        if (live) {
-            near_[i] = ex;
-            near_[(size_t)N + i] = ey;
-            near_[2 * (size_t)N + i] = ez;
-            near_[3 * (size_t)N + i] = bx;
-            near_[4 * (size_t)N + i] = by;
-            near_[5 * (size_t)N + i] = bz;
+#pragma unroll
+        for (int k = 0; k < P2P_NT; ++k) {
+            int i = i0 + k * blockDim.x + threadIdx.x;
+            if (i < thi) {
+                near_[i] = ex[k];
+                near_[(size_t)N + i] = ey[k];
+                near_[2 * (size_t)N + i] = ez[k];
+                near_[3 * (size_t)N + i] = bx[k];
+                near_[4 * (size_t)N + i] = by[k];
+                near_[5 * (size_t)N + i] = bz[k];
+            }
         }
     }
 }
@@ -108,7 +143,8 @@ int pairs_p2p(fmm_plan *p)
 {
     fmm_ctx *c = &p->ctx;
     int maxleaf = (int)((p->N + p->leaves - 1) / p->leaves);
-    int threads = ((maxleaf + 31) / 32) * 32;
+    int per = (maxleaf + P2P_NT - 1) / P2P_NT;
+    int threads = ((per + 31) / 32) * 32;
     if (threads > 256) threads = 256;
     if (threads < 32) threads = 32;
     p2p_kernel<<<(unsigned)p->leaves, threads, 0, c->stream>>>((int)p->N, p->gamma_bar * p->gamma_bar, p->p2p_order, p->p2p_off, p->p2p_src,
