@@ -243,9 +243,13 @@ int pairs_direct(fmm_ctx *c, int64_t N, const double *x, const double *y, const 
 template <int N1>
 struct m2l_cfg {
     static constexpr int P = N1 * N1 * N1;
-    static constexpr int BATCHES = (P + 1023) / 1024;
+#ifndef M2L_NT
+#define M2L_NT 1
+#endif
+    static constexpr int NT = M2L_NT;                      // target proxy points per thread
+    static constexpr int BATCHES = (P + 1024 * NT - 1) / (1024 * NT);
     static constexpr int PER = (P + BATCHES - 1) / BATCHES;
-    static constexpr int THREADS = ((PER + 31) / 32) * 32;
+    static constexpr int THREADS = (((PER + NT - 1) / NT + 31) / 32) * 32;
     // two resident blocks per SM while 2 x THREADS x 88 registers fit the register file (the dependent
     // seed -> series chain of inv_r3 needs >= 5 warps per sub-partition to keep the FP64 pipe fed)
 #ifndef M2L_MINB
@@ -394,73 +398,104 @@ __global__ void __launch_bounds__(m2l_cfg<N1>::THREADS + 32, m2l_cfg<N1>::MINB) 
     }
     const double *xt3 = xi + (size_t)t * 3 * M2L_XI_STRIDE;
     int i = 0;  // consumed loads so far
-    for (int mu0 = 0; mu0 < P; mu0 += THREADS) {
-        const int mu = mu0 + threadIdx.x;
-        const bool live = mu < P;
-        const int a = live ? mu / (N1 * N1) : 0, b = live ? (mu / N1) % N1 : 0, c3 = live ? mu % N1 : 0;
-        // the target's z proxy point: centre + relative part, exactly as the oracle's xi (mid + half c_k)
-        const double xt = xt3[a], yt = xt3[M2L_XI_STRIDE + b];
-        const double zt = __dadd_rn(xt3[2 * M2L_XI_STRIDE + M2L_XI_STRIDE - 1], xt3[2 * M2L_XI_STRIDE + c3]);
-        double ex = 0, ey = 0, ez = 0, bx = 0, by = 0, bz = 0;
+    constexpr int NT = m2l_cfg<N1>::NT;
+    for (int mu0 = 0; mu0 < P; mu0 += NT * THREADS) {
+        // the thread's NT target proxy points; z = centre + relative part, as the oracle's xi (mid + half c_k)
+        double xt[NT], yt[NT], zt[NT], ex[NT], ey[NT], ez[NT], bx[NT], by[NT], bz[NT];
+#pragma unroll
+        for (int k = 0; k < NT; ++k) {
+            const int mu = mu0 + k * THREADS + threadIdx.x;
+            const bool live = mu < P;
+            const int a = live ? mu / (N1 * N1) : 0, b = live ? (mu / N1) % N1 : 0, c3 = live ? mu % N1 : 0;
+            xt[k] = xt3[a];
+            yt[k] = xt3[M2L_XI_STRIDE + b];
+            zt[k] = __dadd_rn(xt3[2 * M2L_XI_STRIDE + M2L_XI_STRIDE - 1], xt3[2 * M2L_XI_STRIDE + c3]);
+            ex[k] = ey[k] = ez[k] = bx[k] = by[k] = bz[k] = 0.0;
+        }
         for (int e = 0; e < ne; ++e, ++i) {
             const int st = i % S;
             mbar_wait(&full[st], (uint32_t)((i / S) & 1));
             const double2 *Ms = reinterpret_cast<const double2 *>(m2l_smem_raw + (size_t)st * STAGE_BYTES);
             const double2 *Zs = reinterpret_cast<const double2 *>(m2l_smem_raw + (size_t)st * STAGE_BYTES + TILE_BYTES);
             const double *xs = reinterpret_cast<const double *>(m2l_smem_raw + (size_t)st * STAGE_BYTES + 2 * TILE_BYTES);
-            const double ztr = zt - xs[2 * M2L_XI_STRIDE + M2L_XI_STRIDE - 1];  // target z relative to the source box centre
-            double gz2[N1];
+            double ztr[NT], gz2[NT][N1];
+            double T0[NT], T1[NT], T2[NT];  // sum over the whole source of A0, A1, A2
+            double S0[NT], S1[NT], S2[NT];  // sum over the whole source of MZ_k w
 #pragma unroll
-            for (int k = 0; k < N1; ++k) {
-                const double dz = ztr - xs[2 * M2L_XI_STRIDE + k];
-                gz2[k] = (g2 * dz) * dz;
+            for (int k = 0; k < NT; ++k) {
+                ztr[k] = zt[k] - xs[2 * M2L_XI_STRIDE + M2L_XI_STRIDE - 1];  // target z relative to the source box centre
+#pragma unroll
+                for (int c = 0; c < N1; ++c) {
+                    const double dz = ztr[k] - xs[2 * M2L_XI_STRIDE + c];
+                    gz2[k][c] = (g2 * dz) * dz;
+                }
+                T0[k] = T1[k] = T2[k] = S0[k] = S1[k] = S2[k] = 0.0;
             }
-            double T0 = 0, T1 = 0, T2 = 0;          // sum over the whole source of A0, A1, A2
-            double S0 = 0, S1 = 0, S2 = 0;          // sum over the whole source of MZ_k w
             for (int a2 = 0; a2 < N1; ++a2) {
-                const double dx = xt - xs[a2];
-                const double dx2 = dx * dx;
+                double dx[NT], dx2[NT];
+#pragma unroll
+                for (int k = 0; k < NT; ++k) {
+                    dx[k] = xt[k] - xs[a2];
+                    dx2[k] = dx[k] * dx[k];
+                }
 #pragma unroll 1
                 for (int b2 = 0; b2 < N1; ++b2) {
-                    const double dy = yt - xs[M2L_XI_STRIDE + b2];
-                    const double s2 = fma(dy, dy, dx2);
                     const double2 *row = Ms + 2 * ((a2 * N1 + b2) * N1);
                     const double2 *rowz = Zs + 2 * ((a2 * N1 + b2) * N1);
-                    double A0 = 0, A1 = 0, A2 = 0, A3 = 0;
+                    double dy[NT], s2[NT], A0[NT], A1[NT], A2[NT], A3[NT];
+#pragma unroll
+                    for (int k = 0; k < NT; ++k) {
+                        dy[k] = yt[k] - xs[M2L_XI_STRIDE + b2];
+                        s2[k] = fma(dy[k], dy[k], dx2[k]);
+                        A0[k] = A1[k] = A2[k] = A3[k] = 0.0;
+                    }
 #pragma unroll
                     for (int c2 = 0; c2 < N1; ++c2) {
-                        const double w = inv_r3(s2 + gz2[c2]);
                         const double2 m01 = row[2 * c2], m23 = row[2 * c2 + 1];
                         const double2 z01 = rowz[2 * c2];
                         const double z2 = rowz[2 * c2 + 1].x;
-                        A0 = fma(m01.x, w, A0);
-                        A1 = fma(m01.y, w, A1);
-                        A2 = fma(m23.x, w, A2);
-                        A3 = fma(m23.y, w, A3);
-                        S0 = fma(z01.x, w, S0);
-                        S1 = fma(z01.y, w, S1);
-                        S2 = fma(z2, w, S2);
+#pragma unroll
+                        for (int k = 0; k < NT; ++k) {
+                            const double w = inv_r3(s2[k] + gz2[k][c2]);
+                            A0[k] = fma(m01.x, w, A0[k]);
+                            A1[k] = fma(m01.y, w, A1[k]);
+                            A2[k] = fma(m23.x, w, A2[k]);
+                            A3[k] = fma(m23.y, w, A3[k]);
+                            S0[k] = fma(z01.x, w, S0[k]);
+                            S1[k] = fma(z01.y, w, S1[k]);
+                            S2[k] = fma(z2, w, S2[k]);
+                        }
                     }
-                    ex = fma(A0, dx, ex);
-                    ey = fma(A0, dy, ey);
-                    bx = fma(-A3, dy, bx);
-                    by = fma(A3, dx, by);
-                    bz = fma(A1, dy, fma(-A2, dx, bz));
-                    T0 += A0;
-                    T1 += A1;
-                    T2 += A2;
+#pragma unroll
+                    for (int k = 0; k < NT; ++k) {
+                        ex[k] = fma(A0[k], dx[k], ex[k]);
+                        ey[k] = fma(A0[k], dy[k], ey[k]);
+                        bx[k] = fma(-A3[k], dy[k], bx[k]);
+                        by[k] = fma(A3[k], dx[k], by[k]);
+                        bz[k] = fma(A1[k], dy[k], fma(-A2[k], dx[k], bz[k]));
+                        T0[k] += A0[k];
+                        T1[k] += A1[k];
+                        T2[k] += A2[k];
+                    }
                 }
             }
             // sum m_k w dz = ztr sum m_k w - sum MZ_k w:  E_z += Z0,  B_x += Z2,  B_y -= Z1
-            ez += fma(ztr, T0, -S0);
-            bx += fma(ztr, T2, -S2);
-            by -= fma(ztr, T1, -S1);
+#pragma unroll
+            for (int k = 0; k < NT; ++k) {
+                ez[k] += fma(ztr[k], T0[k], -S0[k]);
+                bx[k] += fma(ztr[k], T2[k], -S2[k]);
+                by[k] -= fma(ztr[k], T1[k], -S1[k]);
+            }
             __syncwarp();
             if ((threadIdx.x & 31) == 0) mbar_arrive(&empty[st]);
         }
-        if (live) {
-            double *o = Lt + 6 * (size_t)mu;
-            o[0] = ex; o[1] = ey; o[2] = ez; o[3] = bx; o[4] = by; o[5] = bz;
+#pragma unroll
+        for (int k = 0; k < NT; ++k) {
+            const int mu = mu0 + k * THREADS + threadIdx.x;
+            if (mu < P) {
+                double *o = Lt + 6 * (size_t)mu;
+                o[0] = ex[k]; o[1] = ey[k]; o[2] = ez[k]; o[3] = bx[k]; o[4] = by[k]; o[5] = bz[k];
+            }
         }
     }
 }
