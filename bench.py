@@ -46,7 +46,8 @@ def parse_args():
     ap.add_argument("--config", type=int, default=3, help="BASELINE.json configs[i-1] (1-based)")
     ap.add_argument("--tree", default="kd", choices=["kd", "morton"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--cpu-sample-leaves", type=int, default=256)
+    ap.add_argument("--cpu-sample-leaves", type=int, default=2048,
+                    help="target leaves the oracle evaluates in the cpu_baseline leg (the reference arm uses 1/8 of it per step)")
     return ap.parse_args()
 
 
@@ -97,11 +98,12 @@ def run_reference(args):
         return
     import oracle
     w = workloads.config(args.config)
+    per_step = max(8, args.cpu_sample_leaves // 8)   # bounded sample: K steps must end within minutes
     for _ in range(min(args.warmup, 1)):
-        oracle_step(w, args.tree, max(8, args.cpu_sample_leaves // 8))
+        oracle_step(w, args.tree, max(8, per_step // 4))
     tot, spent_tot, info = 0.0, 0.0, None
     for _ in range(args.steps):
-        full, spent, info = oracle_step(w, args.tree, args.cpu_sample_leaves)
+        full, spent, info = oracle_step(w, args.tree, per_step)
         tot += full
         spent_tot += spent
     value = w.N * args.steps / tot
@@ -180,6 +182,20 @@ def max_over_ranks(ms, world, device=None):
 def aggregate_throughput(world, n_per_rank, steps, ms_total):
     """Whole-job particles/s: every rank evaluates its own replica of n_per_rank particles `steps` times."""
     return world * n_per_rank * steps / (ms_total * 1e-3)
+
+
+def ncu_traffic(kernel, w, tree):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of `kernel`, from the committed `ncu --set full`
+    capture (profiles/ncu_traffic.csv; the .md beside it names the command).  None if the capture is of another workload."""
+    try:
+        import csv
+        with open(os.path.join(ROOT, "profiles", "ncu_traffic.csv")) as f:
+            for row in csv.DictReader(f):
+                if row["kernel"] == kernel and row["workload"] == w.name and row["tree"] == tree:
+                    return int(row["dram_bytes_read"]) + int(row["dram_bytes_write"])
+    except Exception:
+        pass
+    return None
 
 
 def run_cuda(args):
@@ -275,7 +291,8 @@ def run_cuda(args):
     evals = {"p2p": st["p2p_pairs"], "m2l": st["m2l_pairs"]}
     ach = {k: evals[k] * FLOP_PER_EVAL / (stages[k] * 1e-3) / 1e12 for k in ("p2p", "m2l")}
     roofline = {"bound": "alu", "kernel": dom + "_kernel", "achieved": ach[dom], "peak": nominal, "unit": "TFLOP/s",
-                "frac": ach[dom] / nominal, "traffic": None,
+                "frac": ach[dom] / nominal, "traffic": ncu_traffic(dom + "_kernel", w, args.tree),
+                "traffic_unit": "bytes per launch (ncu dram__bytes_read.sum + dram__bytes_write.sum, profiles/ncu_traffic.csv)",
                 "peak_source": f"FP64 vector pipe: {SM_COUNT} SMs x {FP64_LANES_PER_SM} lanes x 2 flop x {sm_max:.0f} MHz (DESIGN.md); "
                                "MEASURED_PEAKS.json has no FP64 entry",
                 "measured_dfma_tflops": measured_dfma, "frac_of_measured_dfma": ach[dom] / measured_dfma,

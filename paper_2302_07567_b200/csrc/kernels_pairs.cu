@@ -402,6 +402,7 @@ __global__ void __launch_bounds__(m2l_cfg<N1>::THREADS + 32, m2l_cfg<N1>::MINB) 
     for (int mu0 = 0; mu0 < P; mu0 += NT * THREADS) {
         // the thread's NT target proxy points; z = centre + relative part, as the oracle's xi (mid + half c_k)
         double xt[NT], yt[NT], zt[NT], ex[NT], ey[NT], ez[NT], bx[NT], by[NT], bz[NT];
+        double S0[NT], S1[NT], S2[NT];  // sum over all sources of MZ_k w (subtracted once, after the last source)
 #pragma unroll
         for (int k = 0; k < NT; ++k) {
             const int mu = mu0 + k * THREADS + threadIdx.x;
@@ -410,7 +411,7 @@ __global__ void __launch_bounds__(m2l_cfg<N1>::THREADS + 32, m2l_cfg<N1>::MINB) 
             xt[k] = xt3[a];
             yt[k] = xt3[M2L_XI_STRIDE + b];
             zt[k] = __dadd_rn(xt3[2 * M2L_XI_STRIDE + M2L_XI_STRIDE - 1], xt3[2 * M2L_XI_STRIDE + c3]);
-            ex[k] = ey[k] = ez[k] = bx[k] = by[k] = bz[k] = 0.0;
+            ex[k] = ey[k] = ez[k] = bx[k] = by[k] = bz[k] = S0[k] = S1[k] = S2[k] = 0.0;
         }
         for (int e = 0; e < ne; ++e, ++i) {
             const int st = i % S;
@@ -419,8 +420,6 @@ __global__ void __launch_bounds__(m2l_cfg<N1>::THREADS + 32, m2l_cfg<N1>::MINB) 
             const double2 *Zs = reinterpret_cast<const double2 *>(m2l_smem_raw + (size_t)st * STAGE_BYTES + TILE_BYTES);
             const double *xs = reinterpret_cast<const double *>(m2l_smem_raw + (size_t)st * STAGE_BYTES + 2 * TILE_BYTES);
             double ztr[NT], gz2[NT][N1];
-            double T0[NT], T1[NT], T2[NT];  // sum over the whole source of A0, A1, A2
-            double S0[NT], S1[NT], S2[NT];  // sum over the whole source of MZ_k w
 #pragma unroll
             for (int k = 0; k < NT; ++k) {
                 ztr[k] = zt[k] - xs[2 * M2L_XI_STRIDE + M2L_XI_STRIDE - 1];  // target z relative to the source box centre
@@ -429,7 +428,6 @@ __global__ void __launch_bounds__(m2l_cfg<N1>::THREADS + 32, m2l_cfg<N1>::MINB) 
                     const double dz = ztr[k] - xs[2 * M2L_XI_STRIDE + c];
                     gz2[k][c] = (g2 * dz) * dz;
                 }
-                T0[k] = T1[k] = T2[k] = S0[k] = S1[k] = S2[k] = 0.0;
             }
             for (int a2 = 0; a2 < N1; ++a2) {
                 double dx[NT], dx2[NT];
@@ -468,23 +466,15 @@ __global__ void __launch_bounds__(m2l_cfg<N1>::THREADS + 32, m2l_cfg<N1>::MINB) 
                     }
 #pragma unroll
                     for (int k = 0; k < NT; ++k) {
+                        // sum m_k w dz = ztr sum m_k w - sum MZ_k w:  E_z += Z0,  B_x += Z2,  B_y -= Z1
                         ex[k] = fma(A0[k], dx[k], ex[k]);
                         ey[k] = fma(A0[k], dy[k], ey[k]);
-                        bx[k] = fma(-A3[k], dy[k], bx[k]);
-                        by[k] = fma(A3[k], dx[k], by[k]);
+                        ez[k] = fma(A0[k], ztr[k], ez[k]);
+                        bx[k] = fma(-A3[k], dy[k], fma(A2[k], ztr[k], bx[k]));
+                        by[k] = fma(A3[k], dx[k], fma(-A1[k], ztr[k], by[k]));
                         bz[k] = fma(A1[k], dy[k], fma(-A2[k], dx[k], bz[k]));
-                        T0[k] += A0[k];
-                        T1[k] += A1[k];
-                        T2[k] += A2[k];
                     }
                 }
-            }
-            // sum m_k w dz = ztr sum m_k w - sum MZ_k w:  E_z += Z0,  B_x += Z2,  B_y -= Z1
-#pragma unroll
-            for (int k = 0; k < NT; ++k) {
-                ez[k] += fma(ztr[k], T0[k], -S0[k]);
-                bx[k] += fma(ztr[k], T2[k], -S2[k]);
-                by[k] -= fma(ztr[k], T1[k], -S1[k]);
             }
             __syncwarp();
             if ((threadIdx.x & 31) == 0) mbar_arrive(&empty[st]);
@@ -494,7 +484,7 @@ __global__ void __launch_bounds__(m2l_cfg<N1>::THREADS + 32, m2l_cfg<N1>::MINB) 
             const int mu = mu0 + k * THREADS + threadIdx.x;
             if (mu < P) {
                 double *o = Lt + 6 * (size_t)mu;
-                o[0] = ex[k]; o[1] = ey[k]; o[2] = ez[k]; o[3] = bx[k]; o[4] = by[k]; o[5] = bz[k];
+                o[0] = ex[k]; o[1] = ey[k]; o[2] = ez[k] - S0[k]; o[3] = bx[k] - S2[k]; o[4] = by[k] + S1[k]; o[5] = bz[k];
             }
         }
     }
