@@ -52,25 +52,43 @@ __device__ __forceinline__ void stage_tile(double2 *tile, int count, const doubl
     }
 }
 
-__device__ __forceinline__ void tile_interact(const double2 *tile, int count, double xt, double yt, double zt, double g2,
-                                              double &ex, double &ey, double &ez, double &bx, double &by, double &bz)
+// One staged tile acting on the thread's NT targets: the tile is read once from shared memory for NT evaluations
+// (4 LDS.128 per source), and the accumulate-FMAs of the NT targets that share a source weight are adjacent.
+template <int NT>
+__device__ __forceinline__ void tile_interact(const double2 *tile, int count, const double (&xt)[NT], const double (&yt)[NT],
+                                              const double (&zt)[NT], double g2, double (&ex)[NT], double (&ey)[NT], double (&ez)[NT],
+                                              double (&bx)[NT], double (&by)[NT], double (&bz)[NT])
 {
-#pragma unroll 4
+#pragma unroll 2
     for (int j = 0; j < count; ++j) {
         double2 a = tile[4 * j + 0], b = tile[4 * j + 1], c = tile[4 * j + 2], d = tile[4 * j + 3];
-        pair_accumulate(xt, yt, zt, g2, a.x, a.y, b.x, b.y, c.x, c.y, d.x, ex, ey, ez, bx, by, bz);
+        double gx[NT], gy[NT], gz[NT];
+#pragma unroll
+        for (int k = 0; k < NT; ++k) {
+            double dx = xt[k] - a.x, dy = yt[k] - a.y, dz = zt[k] - b.x;
+            double D = dx * dx;
+            D = fma(dy, dy, D);
+            D = fma(g2 * dz, dz, D);
+            double w = inv_r3(D);
+            gx[k] = w * dx; gy[k] = w * dy; gz[k] = w * dz;
+        }
+        const double m0 = b.y, m1 = c.x, m2 = c.y, m3 = d.x;
+#pragma unroll
+        for (int k = 0; k < NT; ++k) { ex[k] = fma(m0, gx[k], ex[k]); ey[k] = fma(m0, gy[k], ey[k]); ez[k] = fma(m0, gz[k], ez[k]); }
+#pragma unroll
+        for (int k = 0; k < NT; ++k) { bx[k] = fma(m2, gz[k], bx[k]); bz[k] = fma(-m2, gx[k], bz[k]); }
+#pragma unroll
+        for (int k = 0; k < NT; ++k) { by[k] = fma(m3, gx[k], by[k]); bx[k] = fma(-m3, gy[k], bx[k]); }
+#pragma unroll
+        for (int k = 0; k < NT; ++k) { bz[k] = fma(m1, gy[k], bz[k]); by[k] = fma(-m1, gz[k], by[k]); }
     }
 }
 
 // ---------------------------------------------------------------------------------------
-// a7: P2P.  One block per target leaf (blocks issued in descending-work order); one thread per
-// target particle; the source leaves of the CSR row are staged tile by tile.
+// a7: P2P.  One block per target leaf (blocks issued in descending-work order); NT target particles per
+// thread; the source leaves of the CSR row are staged tile by tile.
 // ---------------------------------------------------------------------------------------
-// P2P_NT target particles per thread: the source tile is read once from shared memory for P2P_NT evaluations and the
-// accumulate-FMAs of the P2P_NT targets that share a source weight are adjacent (operand reuse).
-#ifndef P2P_NT
-#define P2P_NT 4
-#endif
+template <int NT>
 __global__ void __launch_bounds__(256) p2p_kernel(int N, double g2, const int32_t *__restrict__ order, const int32_t *__restrict__ off,
                                                   const int32_t *__restrict__ src, const int32_t *__restrict__ node_lo,
                                                   const int32_t *__restrict__ node_hi, const double *__restrict__ tx,
@@ -82,10 +100,10 @@ __global__ void __launch_bounds__(256) p2p_kernel(int N, double g2, const int32_
     const int t = order[blockIdx.x];
     const int tlo = node_lo[t], thi = node_hi[t];
     const int e0 = off[t], e1 = off[t + 1];
-    for (int i0 = tlo; i0 < thi; i0 += P2P_NT * blockDim.x) {
-        double xt[P2P_NT], yt[P2P_NT], zt[P2P_NT], ex[P2P_NT], ey[P2P_NT], ez[P2P_NT], bx[P2P_NT], by[P2P_NT], bz[P2P_NT];
+    for (int i0 = tlo; i0 < thi; i0 += NT * blockDim.x) {
+        double xt[NT], yt[NT], zt[NT], ex[NT], ey[NT], ez[NT], bx[NT], by[NT], bz[NT];
 #pragma unroll
-        for (int k = 0; k < P2P_NT; ++k) {
+        for (int k = 0; k < NT; ++k) {
             int i = i0 + k * blockDim.x + threadIdx.x;
             bool live = i < thi;
             xt[k] = live ? tx[i] : 0.0; yt[k] = live ? ty[i] : 0.0; zt[k] = live ? tz[i] : 0.0;
@@ -99,33 +117,11 @@ __global__ void __launch_bounds__(256) p2p_kernel(int N, double g2, const int32_
                 __syncthreads();
                 stage_tile(tile, count, tx, ty, tz, w0, w1, w2, w3, j0);
                 __syncthreads();
-#pragma unroll 2
-                for (int j = 0; j < count; ++j) {
-                    double2 a = tile[4 * j + 0], b = tile[4 * j + 1], c = tile[4 * j + 2], d = tile[4 * j + 3];
-                    double gx[P2P_NT], gy[P2P_NT], gz[P2P_NT];
-#pragma unroll
-                    for (int k = 0; k < P2P_NT; ++k) {
-                        double dx = xt[k] - a.x, dy = yt[k] - a.y, dz = zt[k] - b.x;
-                        double D = dx * dx;
-                        D = fma(dy, dy, D);
-                        D = fma(g2 * dz, dz, D);
-                        double w = inv_r3(D);
-                        gx[k] = w * dx; gy[k] = w * dy; gz[k] = w * dz;
-                    }
-                    const double m0 = b.y, m1 = c.x, m2 = c.y, m3 = d.x;
-#pragma unroll
-                    for (int k = 0; k < P2P_NT; ++k) { ex[k] = fma(m0, gx[k], ex[k]); ey[k] = fma(m0, gy[k], ey[k]); ez[k] = fma(m0, gz[k], ez[k]); }
-#pragma unroll
-                    for (int k = 0; k < P2P_NT; ++k) { bx[k] = fma(m2, gz[k], bx[k]); bz[k] = fma(-m2, gx[k], bz[k]); }
-#pragma unroll
-                    for (int k = 0; k < P2P_NT; ++k) { by[k] = fma(m3, gx[k], by[k]); bx[k] = fma(-m3, gy[k], bx[k]); }
-#pragma unroll
-                    for (int k = 0; k < P2P_NT; ++k) { bz[k] = fma(m1, gy[k], bz[k]); by[k] = fma(-m1, gz[k], by[k]); }
-                }
+                tile_interact<NT>(tile, count, xt, yt, zt, g2, ex, ey, ez, bx, by, bz);
             }
         }
 #pragma unroll
-        for (int k = 0; k < P2P_NT; ++k) {
+        for (int k = 0; k < NT; ++k) {
             int i = i0 + k * blockDim.x + threadIdx.x;
             if (i < thi) {
                 near_[i] = ex[k];
@@ -139,37 +135,71 @@ __global__ void __launch_bounds__(256) p2p_kernel(int N, double g2, const int32_
     }
 }
 
+// Targets per thread: the largest NT <= 4 that still leaves >= 8 warps per SM in flight, among those the one that
+// wastes the fewest lanes (a leaf of 78 particles fills 3 x 32 slots at NT = 3 but only 78 of 128 at NT = 4).
+static void p2p_shape(int64_t leaves, int maxleaf, int *nt_out, int *threads_out)
+{
+    int best_nt = 1, best_threads = 32;
+    double best_score = -1.0;
+    for (int nt = 1; nt <= 4; ++nt) {
+        int per = (maxleaf + nt - 1) / nt;
+        int threads = ((per + 31) / 32) * 32;
+        if (threads > 256) threads = 256;
+        int passes = (maxleaf + nt * threads - 1) / (nt * threads);
+        double eff = (double)maxleaf / ((double)passes * nt * threads);
+        double warps = (double)leaves * (threads / 32);
+        double fill = warps >= 8.0 * FMM_SM_COUNT ? 1.0 : warps / (8.0 * FMM_SM_COUNT);
+        double score = eff * fill * (1.0 + 0.02 * nt);  // ties: more targets per thread
+        if (score > best_score) { best_score = score; best_nt = nt; best_threads = threads; }
+    }
+    *nt_out = best_nt;
+    *threads_out = best_threads;
+}
+
 int pairs_p2p(fmm_plan *p)
 {
     fmm_ctx *c = &p->ctx;
     int maxleaf = (int)((p->N + p->leaves - 1) / p->leaves);
-    int per = (maxleaf + P2P_NT - 1) / P2P_NT;
-    int threads = ((per + 31) / 32) * 32;
-    if (threads > 256) threads = 256;
-    if (threads < 32) threads = 32;
-    p2p_kernel<<<(unsigned)p->leaves, threads, 0, c->stream>>>((int)p->N, p->gamma_bar * p->gamma_bar, p->p2p_order, p->p2p_off, p->p2p_src,
-                                                               p->node_lo, p->node_hi, p->tx, p->ty, p->tz, p->w0, p->w1, p->w2, p->w3,
-                                                               p->near_);
+    int nt, threads;
+    p2p_shape(p->leaves, maxleaf, &nt, &threads);
+#define P2P_LAUNCH(NT)                                                                                                              \
+    p2p_kernel<NT><<<(unsigned)p->leaves, threads, 0, c->stream>>>((int)p->N, p->gamma_bar * p->gamma_bar, p->p2p_order, p->p2p_off, \
+                                                                   p->p2p_src, p->node_lo, p->node_hi, p->tx, p->ty, p->tz, p->w0,   \
+                                                                   p->w1, p->w2, p->w3, p->near_)
+    switch (nt) {
+        case 1: P2P_LAUNCH(1); break;
+        case 2: P2P_LAUNCH(2); break;
+        case 3: P2P_LAUNCH(3); break;
+        default: P2P_LAUNCH(4); break;
+    }
+#undef P2P_LAUNCH
     FMM_LAUNCH_CHECK(c, "p2p_kernel");
     return FMM_OK;
 }
 
 // ---------------------------------------------------------------------------------------
-// a11: direct summation.  grid = (target blocks, source splits); each block sums its slice of the
-// sources for 256 targets; the slices are then added in a fixed order by direct_reduce.
+// a11: direct summation.  grid = (target blocks, source splits); each block sums its slice of the sources for
+// DIRECT_NT x 128 targets; the slices are then added in a fixed order by direct_reduce.
 // ---------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(256) direct_kernel(int64_t N, double g2, int64_t nt, const int64_t *__restrict__ tidx,
-                                                     int64_t chunk, const double *__restrict__ x, const double *__restrict__ y,
-                                                     const double *__restrict__ z, const double *__restrict__ w0,
-                                                     const double *__restrict__ w1, const double *__restrict__ w2,
-                                                     const double *__restrict__ w3, double *__restrict__ part /* [splits][6][nt] */)
+#define DIRECT_NT 4
+#define DIRECT_THREADS 128
+#define DIRECT_TARGETS (DIRECT_NT * DIRECT_THREADS)
+__global__ void __launch_bounds__(DIRECT_THREADS) direct_kernel(int64_t N, double g2, int64_t nt, const int64_t *__restrict__ tidx,
+                                                                int64_t chunk, const double *__restrict__ x, const double *__restrict__ y,
+                                                                const double *__restrict__ z, const double *__restrict__ w0,
+                                                                const double *__restrict__ w1, const double *__restrict__ w2,
+                                                                const double *__restrict__ w3, double *__restrict__ part /* [splits][6][nt] */)
 {
     __shared__ double2 tile[4 * PAIR_TILE];
-    int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    bool live = k < nt;
-    int64_t i = live ? (tidx ? tidx[k] : k) : 0;
-    double xt = live ? x[i] : 0.0, yt = live ? y[i] : 0.0, zt = live ? z[i] : 0.0;
-    double ex = 0, ey = 0, ez = 0, bx = 0, by = 0, bz = 0;
+    double xt[DIRECT_NT], yt[DIRECT_NT], zt[DIRECT_NT], ex[DIRECT_NT], ey[DIRECT_NT], ez[DIRECT_NT], bx[DIRECT_NT], by[DIRECT_NT], bz[DIRECT_NT];
+#pragma unroll
+    for (int k = 0; k < DIRECT_NT; ++k) {
+        int64_t q = (int64_t)blockIdx.x * DIRECT_TARGETS + k * DIRECT_THREADS + threadIdx.x;
+        bool live = q < nt;
+        int64_t i = live ? (tidx ? tidx[q] : q) : 0;
+        xt[k] = live ? x[i] : 0.0; yt[k] = live ? y[i] : 0.0; zt[k] = live ? z[i] : 0.0;
+        ex[k] = ey[k] = ez[k] = bx[k] = by[k] = bz[k] = 0.0;
+    }
     int64_t s0 = (int64_t)blockIdx.y * chunk, s1 = s0 + chunk;
     if (s1 > N) s1 = N;
     for (int64_t j0 = s0; j0 < s1; j0 += PAIR_TILE) {
@@ -177,11 +207,15 @@ __global__ void __launch_bounds__(256) direct_kernel(int64_t N, double g2, int64
         __syncthreads();
         stage_tile(tile, count, x, y, z, w0, w1, w2, w3, j0);
         __syncthreads();
-        tile_interact(tile, count, xt, yt, zt, g2, ex, ey, ez, bx, by, bz);
+        tile_interact<DIRECT_NT>(tile, count, xt, yt, zt, g2, ex, ey, ez, bx, by, bz);
     }
-    if (live) {
-        double *o = part + (size_t)blockIdx.y * 6 * nt + k;
-        o[0] = ex; o[nt] = ey; o[2 * nt] = ez; o[3 * nt] = bx; o[4 * nt] = by; o[5 * nt] = bz;
+#pragma unroll
+    for (int k = 0; k < DIRECT_NT; ++k) {
+        int64_t q = (int64_t)blockIdx.x * DIRECT_TARGETS + k * DIRECT_THREADS + threadIdx.x;
+        if (q < nt) {
+            double *o = part + (size_t)blockIdx.y * 6 * nt + q;
+            o[0] = ex[k]; o[nt] = ey[k]; o[2 * nt] = ez[k]; o[3 * nt] = bx[k]; o[4 * nt] = by[k]; o[5 * nt] = bz[k];
+        }
     }
 }
 
@@ -204,7 +238,7 @@ int pairs_direct(fmm_ctx *c, int64_t N, const double *x, const double *y, const 
                  double gamma_bar, int raw, int64_t nt, const int64_t *tidx,
                  double *Ex, double *Ey, double *Ez, double *Bx, double *By, double *Bz)
 {
-    int64_t tblocks = (nt + 255) / 256;
+    int64_t tblocks = (nt + DIRECT_TARGETS - 1) / DIRECT_TARGETS;
     // enough blocks for ~8 waves of 148 SMs x 4 resident blocks, source slices in whole tiles
     int64_t want = 8 * 4 * FMM_SM_COUNT;
     int64_t splits = (want + tblocks - 1) / tblocks;
@@ -217,14 +251,14 @@ int pairs_direct(fmm_ctx *c, int64_t N, const double *x, const double *y, const 
     double *part = (double *)ctx_alloc(c, sizeof(double) * 6 * (size_t)nt * (size_t)splits);
     if (!part) return FMM_ENOMEM;
     dim3 grid((unsigned)tblocks, (unsigned)splits);
-    direct_kernel<<<grid, 256, 0, c->stream>>>(N, gamma_bar * gamma_bar, nt, tidx, chunk, x, y, z, w0, w1, w2, w3, part);
+    direct_kernel<<<grid, DIRECT_THREADS, 0, c->stream>>>(N, gamma_bar * gamma_bar, nt, tidx, chunk, x, y, z, w0, w1, w2, w3, part);
     FMM_LAUNCH_CHECK(c, "direct_kernel");
     double cE = 1.0, cB = 1.0;
     if (!raw) {
         cE = 1.0 / (4.0 * FMM_PI * FMM_EPS0);
         cB = 1.0 / (4.0 * FMM_PI * FMM_EPS0 * FMM_C0);
     }
-    direct_reduce<<<(unsigned)tblocks, 256, 0, c->stream>>>(nt, (int)splits, part, cE, cB, Ex, Ey, Ez, Bx, By, Bz);
+    direct_reduce<<<(unsigned)((nt + 255) / 256), 256, 0, c->stream>>>(nt, (int)splits, part, cE, cB, Ex, Ey, Ez, Bx, By, Bz);
     FMM_LAUNCH_CHECK(c, "direct_reduce");
     ctx_free(c, part);
     return FMM_OK;

@@ -119,6 +119,12 @@ def config(i: int, N: int | None = None) -> Workload:
     elif i == 6:  # "5b": all-pairs ceiling
         w = gaussian_bunch(N or 262_144, 10.0, 0.01, 1006, order_n=4, leaf_size=256, theta=0.5,
                            name="config5b_allpairs_256k")
+    elif i == 7:  # stand-in for the paper's Fig. 2-4 workload
+        w = paper_cube(N or 1_280_000, order_n=4, theta=0.5)
+        w.name = "paperP_cube_1p28m"
+    elif i == 8:  # the paper's CPU-vs-GPU run: N = 2.56e7, n = 4, N0 = 125, eta = 0.5
+        w = paper_cube(N or 25_600_000, order_n=4, theta=0.5)
+        w.name = "paperP_cube_25p6m"
     else:
         raise ValueError(f"no such config: {i}")
     return w
