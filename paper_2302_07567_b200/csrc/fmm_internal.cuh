@@ -112,6 +112,8 @@ int pairs_source_weights(fmm_ctx *c, int64_t N, const double *px, const double *
 // overwritten with the sorted sequence; tmp_* are scratch of the same length.
 int sort_pairs_u64(fmm_ctx *c, uint64_t *keys, uint32_t *vals, uint64_t *tmp_keys, uint32_t *tmp_vals,
                    int64_t n, int bit_lo, int bit_hi);
+int sort_pairs_u64_batched(fmm_ctx *c, uint64_t *keys, uint32_t *vals, uint64_t *tmp_keys, uint32_t *tmp_vals,
+                           int64_t n, int batch, int bit_lo, int bit_hi);  // `batch` segments of length n, back to back
 int scan_exclusive_i32(fmm_ctx *c, const int32_t *in, int32_t *out, int64_t n);  // out may alias in
 
 #ifdef __CUDACC__

@@ -389,9 +389,10 @@ int tree_build(fmm_plan *p, const fmm_particles_t *in)
     node_ranges_kernel<<<(unsigned)((p->nodes + T - 1) / T), T, 0, st>>>(N, p->kappa, (int)p->nodes, p->node_lo, p->node_hi);
     FMM_LAUNCH_CHECK(c, "node_ranges_kernel");
 
-    uint64_t *keys = (uint64_t *)ctx_alloc(c, sizeof(uint64_t) * N);
-    uint64_t *tkeys = (uint64_t *)ctx_alloc(c, sizeof(uint64_t) * N);
-    uint32_t *tvals = (uint32_t *)ctx_alloc(c, sizeof(uint32_t) * N);
+    const int nsort = ((p->flags & FMM_TREE_MASK) == FMM_TREE_KD) ? 3 : 1;  // KD: the three axes are sorted in one batch
+    uint64_t *keys = (uint64_t *)ctx_alloc(c, sizeof(uint64_t) * N * nsort);
+    uint64_t *tkeys = (uint64_t *)ctx_alloc(c, sizeof(uint64_t) * N * nsort);
+    uint32_t *tvals = (uint32_t *)ctx_alloc(c, sizeof(uint32_t) * N * nsort);
     uint32_t *lists = (uint32_t *)ctx_alloc(c, sizeof(uint32_t) * 4 * (size_t)N);  // LX, LY, LZ, LI
     if (!keys || !tkeys || !tvals || !lists) return FMM_ENOMEM;
     const uint32_t *order = NULL;
@@ -405,10 +406,10 @@ int tree_build(fmm_plan *p, const fmm_particles_t *in)
         if (p->kappa > 0) {
             const double *coord[3] = {in->x, in->y, in->z};
             for (int a = 0; a < 3; ++a) {
-                kd_make_keys<<<gN, T, 0, st>>>(N, coord[a], keys, lists + (size_t)a * N);
+                kd_make_keys<<<gN, T, 0, st>>>(N, coord[a], keys + (size_t)a * N, lists + (size_t)a * N);
                 FMM_LAUNCH_CHECK(c, "kd_make_keys");
-                FMM_TRY(sort_pairs_u64(c, keys, lists + (size_t)a * N, tkeys, tvals, N, 0, 64));
             }
+            FMM_TRY(sort_pairs_u64_batched(c, keys, lists, tkeys, tvals, N, 3, 0, 64));
         }
         kd_iota<<<gN, T, 0, st>>>(N, lists + 3 * (size_t)N);
         FMM_LAUNCH_CHECK(c, "kd_iota");

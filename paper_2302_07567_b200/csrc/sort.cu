@@ -137,6 +137,8 @@ __global__ void __launch_bounds__(RS_THREADS) rs_histogram(const uint64_t *__res
     __shared__ int cnt[RS_RADIX];
     cnt[threadIdx.x] = 0;
     __syncthreads();
+    keys += (int64_t)blockIdx.y * n;                       // batch segment
+    table += (int64_t)blockIdx.y * RS_RADIX * nblocks;
     int64_t base = (int64_t)blockIdx.x * RS_TILE;
 #pragma unroll
     for (int r = 0; r < RS_ROUNDS; ++r) {
@@ -155,6 +157,12 @@ __global__ void __launch_bounds__(RS_THREADS) rs_scatter(const uint64_t *__restr
     int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     for (int k = threadIdx.x; k < RS_WARPS * RS_RADIX; k += RS_THREADS) (&cnt[0][0])[k] = 0;
     __syncthreads();
+    // batch segment: the scan ran over the concatenated tables, so segment b's positions start at b * n
+    const int64_t seg = (int64_t)blockIdx.y * n;
+    keys += seg; okeys += seg;
+    if (vals) { vals += seg; ovals += seg; }
+    table += (int64_t)blockIdx.y * RS_RADIX * nblocks;
+    const int seg_base = (int)seg;
     int64_t wbase = (int64_t)blockIdx.x * RS_TILE + (int64_t)warp * (RS_TILE / RS_WARPS);
     uint64_t key[RS_ROUNDS];
     int rank[RS_ROUNDS];
@@ -179,7 +187,7 @@ __global__ void __launch_bounds__(RS_THREADS) rs_scatter(const uint64_t *__restr
     __syncthreads();
     {  // digit d = threadIdx.x: exclusive prefix over warps + global base of this block
         int d = threadIdx.x;
-        int run = table[(int64_t)d * nblocks + blockIdx.x];
+        int run = table[(int64_t)d * nblocks + blockIdx.x] - seg_base;
 #pragma unroll
         for (int w = 0; w < RS_WARPS; ++w) {
             int t = cnt[w][d];
@@ -203,26 +211,34 @@ __global__ void __launch_bounds__(RS_THREADS) rs_scatter(const uint64_t *__restr
 int sort_pairs_u64(fmm_ctx *c, uint64_t *keys, uint32_t *vals, uint64_t *tmp_keys, uint32_t *tmp_vals,
                    int64_t n, int bit_lo, int bit_hi)
 {
-    if (n <= 1 || bit_hi <= bit_lo) return FMM_OK;
-    if (n >= (int64_t)1 << 31) return FMM_EOVERFLOW;
+    return sort_pairs_u64_batched(c, keys, vals, tmp_keys, tmp_vals, n, 1, bit_lo, bit_hi);
+}
+
+// `batch` independent sorts of equal length n laid out back to back (segment b = [b n, (b+1) n)), one launch per pass
+// for all of them (grid.y = batch): the passes of a 1M-key sort are latency-bound, so three sorts cost little more than one.
+int sort_pairs_u64_batched(fmm_ctx *c, uint64_t *keys, uint32_t *vals, uint64_t *tmp_keys, uint32_t *tmp_vals,
+                           int64_t n, int batch, int bit_lo, int bit_hi)
+{
+    if (n <= 1 || bit_hi <= bit_lo || batch < 1) return FMM_OK;
+    if (n * batch >= (int64_t)1 << 31) return FMM_EOVERFLOW;
     int nblocks = (int)((n + RS_TILE - 1) / RS_TILE);
-    int64_t tlen = (int64_t)RS_RADIX * nblocks;
+    int64_t tlen = (int64_t)RS_RADIX * nblocks * batch;
     int32_t *table = (int32_t *)ctx_alloc(c, sizeof(int32_t) * tlen);
     if (!table) return FMM_ENOMEM;
     uint64_t *ki = keys, *ko = tmp_keys;
     uint32_t *vi = vals, *vo = tmp_vals;
     for (int shift = bit_lo; shift < bit_hi; shift += 8) {
-        rs_histogram<<<nblocks, RS_THREADS, 0, c->stream>>>(ki, n, shift, table, nblocks);
+        rs_histogram<<<dim3(nblocks, batch), RS_THREADS, 0, c->stream>>>(ki, n, shift, table, nblocks);
         FMM_LAUNCH_CHECK(c, "rs_histogram");
         FMM_TRY(scan_exclusive_i32(c, table, table, tlen));
-        rs_scatter<<<nblocks, RS_THREADS, 0, c->stream>>>(ki, vi, ko, vo, n, shift, table, nblocks);
+        rs_scatter<<<dim3(nblocks, batch), RS_THREADS, 0, c->stream>>>(ki, vi, ko, vo, n, shift, table, nblocks);
         FMM_LAUNCH_CHECK(c, "rs_scatter");
         uint64_t *tk = ki; ki = ko; ko = tk;
         uint32_t *tv = vi; vi = vo; vo = tv;
     }
     if (ki != keys) {
-        FMM_CUDA(c, cudaMemcpyAsync(keys, ki, sizeof(uint64_t) * n, cudaMemcpyDeviceToDevice, c->stream));
-        if (vals) FMM_CUDA(c, cudaMemcpyAsync(vals, vi, sizeof(uint32_t) * n, cudaMemcpyDeviceToDevice, c->stream));
+        FMM_CUDA(c, cudaMemcpyAsync(keys, ki, sizeof(uint64_t) * n * batch, cudaMemcpyDeviceToDevice, c->stream));
+        if (vals) FMM_CUDA(c, cudaMemcpyAsync(vals, vi, sizeof(uint32_t) * n * batch, cudaMemcpyDeviceToDevice, c->stream));
     }
     ctx_free(c, table);
     return FMM_OK;
