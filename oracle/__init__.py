@@ -109,7 +109,7 @@ def _charges(q, N):
     return qa, qp, 0.0
 
 
-def direct(x, y, z, px, py, pz, q=None, gamma_bar_value=None, raw=False, targets=None):
+def direct(x, y, z, px, py, pz, q=None, gamma_bar_value=None, raw=False, targets=None, source_momentum=False):
     """O1: returns (E[nt,3], B[nt,3]) at ``targets`` (default: all particles)."""
     arrs = [_d(a) for a in (x, y, z, px, py, pz)]
     N = len(arrs[0][0])
@@ -121,7 +121,7 @@ def direct(x, y, z, px, py, pz, q=None, gamma_bar_value=None, raw=False, targets
         t = np.ascontiguousarray(targets, dtype=np.int64)
         nt, tp = len(t), t.ctypes.data_as(_i64p)
     out = [np.empty(nt) for _ in range(6)]
-    rc = lib().orc_direct(N, *[p for _, p in arrs], qp, qs, gb, int(bool(raw)), nt, tp,
+    rc = lib().orc_direct(N, *[p for _, p in arrs], qp, qs, gb, int(bool(raw)) | (2 if source_momentum else 0), nt, tp,
                           *[o.ctypes.data_as(_dp) for o in out])
     assert rc == 0
     return np.stack(out[:3], axis=1), np.stack(out[3:], axis=1)
@@ -131,13 +131,13 @@ class Plan:
     """O2: tree + interaction lists, then upward / eval (serial FMM of Alg 5.12)."""
 
     def __init__(self, x, y, z, px, py, pz, q=None, *, order_n, leaf_size, theta,
-                 gamma_bar_value=None, tree_mode=TREE_KD, raw=False):
+                 gamma_bar_value=None, tree_mode=TREE_KD, raw=False, source_momentum=False):
         arrs = [_d(a) for a in (x, y, z, px, py, pz)]
         self.N = len(arrs[0][0])
         qa, qp, qs = _charges(q, self.N)
         gb = -1.0 if gamma_bar_value is None else float(gamma_bar_value)
         self._h = lib().orc_plan_create(self.N, *[p for _, p in arrs], qp, qs, int(order_n),
-                                        int(leaf_size), float(theta), gb, int(tree_mode), int(bool(raw)))
+                                        int(leaf_size), float(theta), gb, int(tree_mode), int(bool(raw)) | (2 if source_momentum else 0))
         if not self._h:
             raise ValueError("orc_plan_create: invalid arguments")
         s = np.empty(6, dtype=np.int64)

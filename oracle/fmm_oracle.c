@@ -31,6 +31,7 @@ struct orc_plan {
     double s[3];
     double *x, *y, *z;    /* caller order */
     double *w;            /* [N][4] source weights q*gamma, q*px, q*py, q*pz, caller order */
+    double *pm;           /* [N][3] plain momenta px, py, pz, caller order (source-momentum near field) */
     int64_t *perm;        /* tree position -> caller index */
     int64_t *lo, *hi;     /* [nodes+1], heap index, half open */
     double *bbox;         /* [nodes+1][6] ax ay az bx by bz */
@@ -86,9 +87,28 @@ static inline void accumulate(double dx, double dy, double dz, double g2, const 
     acc[5] += m[1] * gy - m[2] * gx; /* (p x g)_z = px gy - py gx */
 }
 
+/* Alternative reading of Alg 5.10 (PAPER.md:393-394 write g(x_i, x_j, p_j); G6):
+ * the NEAR field of source j is stretched along j's own momentum, D = |d|^2 + (p_j . d)^2 with p_j = gamma_j beta_j.
+ * For p_j = (0, 0, p) this is dx^2 + dy^2 + (1 + p^2) dz^2 = dx^2 + dy^2 + gamma_j^2 dz^2: eq. (3.2) with the
+ * source's own gamma, i.e. the exact field of a uniformly moving charge.  pj = plain momentum of the source. */
+static inline void accumulate_sm(double dx, double dy, double dz, const double *pj, const double *m, double *acc)
+{
+    double pd = pj[0] * dx + pj[1] * dy + pj[2] * dz;
+    double D = (dx * dx + dy * dy + dz * dz) + pd * pd;
+    double w = (D > 0.0) ? 1.0 / (D * sqrt(D)) : 0.0;
+    double gx = w * dx, gy = w * dy, gz = w * dz;
+    acc[0] += m[0] * gx;
+    acc[1] += m[0] * gy;
+    acc[2] += m[0] * gz;
+    acc[3] += m[2] * gz - m[3] * gy;
+    acc[4] += m[3] * gx - m[1] * gz;
+    acc[5] += m[1] * gy - m[2] * gx;
+}
+
+/* `raw` is a flags word: bit 0 = no SI prefactors, bit 1 = source-momentum near field (ORC_KERNEL_SOURCE_MOMENTUM). */
 static void prefactors(int raw, double *cE, double *cB)
 {
-    if (raw) {
+    if (raw & 1) {
         *cE = 1.0;
         *cB = 1.0;
     } else {
@@ -121,8 +141,15 @@ int orc_direct(int64_t N, const double *x, const double *y, const double *z,
     for (int64_t k = 0; k < T; ++k) {
         int64_t i = tidx ? tidx[k] : k;
         double acc[6] = {0, 0, 0, 0, 0, 0};
-        for (int64_t j = 0; j < N; ++j)
-            accumulate(x[i] - x[j], y[i] - y[j], z[i] - z[j], g2, &w[4 * j], acc);
+        if (raw & 2) {
+            for (int64_t j = 0; j < N; ++j) {
+                double pj[3] = {px[j], py[j], pz[j]};
+                accumulate_sm(x[i] - x[j], y[i] - y[j], z[i] - z[j], pj, &w[4 * j], acc);
+            }
+        } else {
+            for (int64_t j = 0; j < N; ++j)
+                accumulate(x[i] - x[j], y[i] - y[j], z[i] - z[j], g2, &w[4 * j], acc);
+        }
         Ex[k] = cE * acc[0];
         Ey[k] = cE * acc[1];
         Ez[k] = cE * acc[2];
@@ -430,6 +457,12 @@ orc_plan_t *orc_plan_create(int64_t N, const double *x, const double *y, const d
         p->w[4 * j + 2] = qj * py[j];
         p->w[4 * j + 3] = qj * pz[j];
     }
+    p->pm = (double *)malloc(3 * sz);
+    for (int64_t j = 0; j < N; ++j) {
+        p->pm[3 * j + 0] = px[j];
+        p->pm[3 * j + 1] = py[j];
+        p->pm[3 * j + 2] = pz[j];
+    }
     p->perm = (int64_t *)malloc(sizeof(int64_t) * (size_t)N);
     for (int64_t j = 0; j < N; ++j)
         p->perm[j] = j;
@@ -451,7 +484,7 @@ orc_plan_t *orc_plan_create(int64_t N, const double *x, const double *y, const d
 void orc_plan_destroy(orc_plan_t *p)
 {
     if (!p) return;
-    free(p->x); free(p->y); free(p->z); free(p->w); free(p->perm);
+    free(p->x); free(p->y); free(p->z); free(p->w); free(p->pm); free(p->perm);
     free(p->lo); free(p->hi); free(p->bbox); free(p->p2p); free(p->m2l); free(p->M);
     free(p);
 }
@@ -693,7 +726,10 @@ static void p2p(const orc_plan_t *p, int64_t t, int64_t s, double *near /* [N][6
         double *acc = &near[6 * ki];
         for (int64_t kj = p->lo[s]; kj < p->hi[s]; ++kj) {
             int64_t j = p->perm[kj];
-            accumulate(p->x[i] - p->x[j], p->y[i] - p->y[j], p->z[i] - p->z[j], g2, &p->w[4 * j], acc);
+            if (p->raw & 2)
+                accumulate_sm(p->x[i] - p->x[j], p->y[i] - p->y[j], p->z[i] - p->z[j], &p->pm[3 * j], &p->w[4 * j], acc);
+            else
+                accumulate(p->x[i] - p->x[j], p->y[i] - p->y[j], p->z[i] - p->z[j], g2, &p->w[4 * j], acc);
         }
     }
 }

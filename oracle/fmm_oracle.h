@@ -35,6 +35,12 @@ extern "C" {
 #define ORC_TREE_KD            0  /* Alg 5.2, reading T-3   */
 #define ORC_TREE_MORTON_MEDIAN 1  /* DESIGN.md reading T-3' (north_star's Morton order)  */
 
+/* flags word passed as `raw`: */
+#define ORC_RAW_SUMS               1  /* no SI prefactors                                                  */
+#define ORC_KERNEL_SOURCE_MOMENTUM 2  /* near field (P2P, direct) stretched along the source's own momentum,
+                                         D = |d|^2 + (p_j.d)^2 (alternative reading of Alg 5.10, G6);
+                                         the far field keeps eq. (3.2) with gamma_bar                      */
+
 typedef struct orc_plan orc_plan_t;
 
 /* gamma_bar^2 = 1 + pbar.pbar, pbar = plain mean momentum (reading G16). */

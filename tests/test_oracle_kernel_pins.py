@@ -144,3 +144,71 @@ def test_raw_and_targets_subset():
     t = np.array([5, 0, 63, 5])
     Et, Bt = oracle.direct(*a, q=QE, targets=t)
     np.testing.assert_array_equal(Et, E[t]); np.testing.assert_array_equal(Bt, B[t])
+
+
+# ---------------------------------------------------------------------------------------------
+# Source-momentum near field (alternative reading of Alg 5.10, G6)
+# ---------------------------------------------------------------------------------------------
+def _heaviside_field(q, R, p):
+    """Textbook (Heaviside / Lienard-Wiechert, uniform motion) field at R from a charge with momentum p = gamma beta,
+    in the cross-product form  E = q (1 - beta^2) R / (4 pi eps0 (R^2 - |R x beta|^2)^(3/2)),  B = beta x E / c0."""
+    gam = np.sqrt(1.0 + p @ p)
+    beta = p / gam
+    den = (R @ R - np.sum(np.cross(R, beta) ** 2)) ** 1.5
+    E = q / (4 * np.pi * EPS0) * (1.0 - beta @ beta) * R / den
+    return E, np.cross(beta, E) / C0
+
+
+def test_source_momentum_is_the_exact_field_of_each_moving_charge():
+    """Each source's near field is stretched along ITS OWN momentum (any direction): for two particles with
+    different momenta the field at one is the exact field of the other as a uniformly moving charge."""
+    rng = np.random.default_rng(7)
+    for _ in range(5):
+        X = rng.normal(size=(2, 3)) * 1e-3
+        Pm = np.stack([rng.normal(size=3) * [0.5, 0.5, 20.0], rng.normal(size=3) * [2.0, 1.0, 5.0]])
+        E, B = oracle.direct(X[:, 0].copy(), X[:, 1].copy(), X[:, 2].copy(), Pm[:, 0].copy(), Pm[:, 1].copy(),
+                             Pm[:, 2].copy(), q=QE, source_momentum=True)
+        for i, j in ((0, 1), (1, 0)):
+            E_exp, B_exp = _heaviside_field(QE, X[i] - X[j], Pm[j])
+            # (1 - beta^2) and R^2 - |R x beta|^2 cancel to ~1/gamma^2: allow gamma^2 ulps in the textbook form
+            tol = 1e-13 * (1.0 + Pm[j] @ Pm[j])
+            np.testing.assert_allclose(E[i], E_exp, rtol=tol)
+            np.testing.assert_allclose(B[i], B_exp, rtol=tol, atol=1e-30)
+
+
+def test_source_momentum_reduces_to_mean_gamma_for_identical_momenta():
+    """All p_j = (0, 0, p): D = dx^2 + dy^2 + (1 + p^2) dz^2 = eq. (3.2) with gamma_bar: both readings coincide
+    ('they coincide when all momenta are identical', the only case the paper measures)."""
+    rng = np.random.default_rng(8)
+    N = 300
+    x, y, z = rng.random(N), rng.random(N), rng.random(N)
+    pz = np.full(N, np.sqrt(50.0 ** 2 - 1.0))
+    zero = np.zeros(N)
+    Ea, Ba = oracle.direct(x, y, z, zero, zero, pz, q=QE)
+    Eb, Bb = oracle.direct(x, y, z, zero, zero, pz, q=QE, source_momentum=True)
+    assert oracle.err2(Eb, Ea) < 1e-13 and oracle.err2(Bb, Ba) < 1e-13
+
+
+def test_source_momentum_differs_for_an_energy_spread_and_fmm_near_field_uses_it():
+    """With an energy spread the two readings differ at the 1e-3 level; the serial FMM in this mode
+    equals the source-momentum direct sum when the far list is empty (pin P9 for the new near field)."""
+    from paper_2302_07567_b200 import workloads
+    w = workloads.config(1, N=1500)
+    Ea, _ = oracle.direct(*w.arrays(), w.q)
+    Eb, Bb = oracle.direct(*w.arrays(), w.q, source_momentum=True)
+    d = oracle.err2(Eb, Ea)
+    assert 1e-4 < d < 5e-2, d
+    op = oracle.Plan(*w.arrays(), w.q, order_n=3, leaf_size=64, theta=0.05, source_momentum=True)
+    assert op.n_m2l == 0
+    E, B = op.eval()
+    assert oracle.err2(E, Eb) < 1e-13 and oracle.err2(B, Bb) < 1e-13
+    # with a far field: near part in the new mode, far part unchanged (mean gamma)
+    op2 = oracle.Plan(*w.arrays(), w.q, order_n=4, leaf_size=64, theta=0.5, source_momentum=True)
+    op3 = oracle.Plan(*w.arrays(), w.q, order_n=4, leaf_size=64, theta=0.5)
+    assert op2.n_m2l > 0
+    Ef2, _ = op2.eval(part="far")
+    Ef3, _ = op3.eval(part="far")
+    assert np.array_equal(Ef2, Ef3)
+    En2, _ = op2.eval(part="near")
+    En3, _ = op3.eval(part="near")
+    assert oracle.err2(En2, En3) > 1e-5
