@@ -45,6 +45,8 @@ def parse_args():
     ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
     ap.add_argument("--config", type=int, default=3, help="BASELINE.json configs[i-1] (1-based)")
     ap.add_argument("--tree", default="kd", choices=["kd", "morton"])
+    ap.add_argument("--kernel", default="mean_gamma", choices=["mean_gamma", "source_momentum"],
+                    help="near-field kernel: eq. (3.2) with gamma_bar (default) or the G6 alternative (SURVEY 8(f) rank 2)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cpu-sample-leaves", type=int, default=2048,
                     help="target leaves the oracle evaluates in the cpu_baseline leg (the reference arm uses 1/8 of it per step)")
@@ -225,6 +227,8 @@ def run_cuda(args):
 
     w = workloads.config(args.config)
     flags = fmm.FMM_TREE_KD if args.tree == "kd" else fmm.FMM_TREE_MORTON_MEDIAN
+    if args.kernel == "source_momentum":
+        flags |= fmm.FMM_KERNEL_SOURCE_MOMENTUM
     d_in = [torch.as_tensor(a).to(dev) for a in w.arrays()]
     out = torch.empty((6, w.N), dtype=torch.float64, device=dev)
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
@@ -302,7 +306,7 @@ def run_cuda(args):
     hbm = float(peaks.get("hbm_gbs", 6650.0))
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": ms_total / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-            "dtype": "f64", "data": "synthetic", "config": workload_config(w, args.tree),
+            "dtype": "f64", "data": "synthetic", "config": dict(workload_config(w, args.tree), kernel=args.kernel),
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": 6 * 8 * w.N, "d2h_bytes_per_step": 6 * 8 * w.N},
             "gpu_launches": int(launches), "clocks": clocks, "roofline": roofline,
             "stages_ms": {k: round(v, 4) for k, v in stages.items()},

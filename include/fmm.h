@@ -54,6 +54,12 @@ extern "C" {
                                        normalised coordinates, same closed-form ranges (DESIGN T-3') */
 #define FMM_TREE_MASK          1u
 #define FMM_RAW_SUMS           4u   /* skip the prefactors of eq. (3.1)                          */
+#define FMM_KERNEL_MEAN_GAMMA      0u  /* eq. (3.2) with gamma_bar in near and far field (default)    */
+#define FMM_KERNEL_SOURCE_MOMENTUM 8u  /* alternative reading of Alg 5.10 (PAPER.md:393-394 write
+                                          g(x_i, x_j, p_j); G6): the NEAR field (P2P, fmm_direct)
+                                          of source j is stretched along j's own momentum,
+                                          D = |d|^2 + (p_j . d)^2, the exact field of a uniformly moving
+                                          charge; the far field (M2L) keeps eq. (3.2) with gamma_bar      */
 
 #define FMM_OK          0
 #define FMM_EINVAL     -1           /* bad argument: N < 1, order out of range, leaf_size < 1,
@@ -82,7 +88,7 @@ typedef struct {
     double theta;                   /* admissibility parameter eta > 0 (eq. (4.3)) */
     double gamma_bar;               /* <= 0: computed from the mean momentum;
                                        > 0: use this value                                       */
-    uint32_t flags;                 /* FMM_TREE_* | FMM_RAW_SUMS                                 */
+    uint32_t flags;                 /* FMM_TREE_* | FMM_RAW_SUMS | FMM_KERNEL_*                  */
 } fmm_params_t;
 
 /* Per-stage device times are CUDA-event times of the last fmm_plan_create/_update (tree, lists)

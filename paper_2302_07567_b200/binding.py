@@ -23,6 +23,8 @@ FMM_MAX_ORDER = 12
 FMM_TREE_KD = 0
 FMM_TREE_MORTON_MEDIAN = 1
 FMM_RAW_SUMS = 4
+FMM_KERNEL_MEAN_GAMMA = 0
+FMM_KERNEL_SOURCE_MOMENTUM = 8
 
 _dp = C.POINTER(C.c_double)
 _i64p = C.POINTER(C.c_int64)

@@ -115,6 +115,9 @@ static int plan_alloc_fixed(fmm_plan *p)
     } while (0)
     ALLOC(tx, double, N); ALLOC(ty, double, N); ALLOC(tz, double, N);
     ALLOC(w0, double, N); ALLOC(w1, double, N); ALLOC(w2, double, N); ALLOC(w3, double, N);
+    if (p->flags & FMM_KERNEL_SOURCE_MOMENTUM) {
+        ALLOC(pmx, double, N); ALLOC(pmy, double, N); ALLOC(pmz, double, N);
+    }
     ALLOC(perm, int32_t, N);
     ALLOC(node_lo, int32_t, nodes1); ALLOC(node_hi, int32_t, nodes1);
     ALLOC(bbox, double, 6 * nodes1); ALLOC(node_geo, double, 4 * nodes1);
@@ -331,7 +334,7 @@ extern "C" int fmm_direct(const fmm_particles_t *in, double gamma_bar, uint32_t 
     ctx_init(&ctx, alloc, free_, user, cuda_stream);
     fmm_ctx *c = &ctx;
     int rc = FMM_OK;
-    if (!(gamma_bar > 0.0)) {
+    if (!(gamma_bar > 0.0) && !(flags & FMM_KERNEL_SOURCE_MOMENTUM)) {  // the source-momentum kernel has no gamma_bar
         rc = tree_gamma_bar(c, in->N, in->px, in->py, in->pz, &gamma_bar);
         if (rc == FMM_OK && !isfinite(gamma_bar)) rc = FMM_ENONFINITE;
     }
@@ -342,9 +345,10 @@ extern "C" int fmm_direct(const fmm_particles_t *in, double gamma_bar, uint32_t 
     }
     const size_t N = (size_t)in->N;
     if (rc == FMM_OK) rc = pairs_source_weights(c, in->N, in->px, in->py, in->pz, in->q, in->q_scalar, w, w + N, w + 2 * N, w + 3 * N);
+    const bool sm = (flags & FMM_KERNEL_SOURCE_MOMENTUM) != 0;
     if (rc == FMM_OK)
-        rc = pairs_direct(c, in->N, in->x, in->y, in->z, w, w + N, w + 2 * N, w + 3 * N, gamma_bar, (flags & FMM_RAW_SUMS) ? 1 : 0, nt,
-                          tidx, Ex, Ey, Ez, Bx, By, Bz);
+        rc = pairs_direct(c, in->N, in->x, in->y, in->z, w, w + N, w + 2 * N, w + 3 * N, sm ? in->px : NULL, sm ? in->py : NULL,
+                          sm ? in->pz : NULL, gamma_bar, (flags & FMM_RAW_SUMS) ? 1 : 0, nt, tidx, Ex, Ey, Ez, Bx, By, Bz);
     ctx_free_all(c);
     return rc;
 }

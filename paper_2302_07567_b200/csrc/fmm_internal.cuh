@@ -61,6 +61,7 @@ struct fmm_plan {
     uint32_t flags;
     // particles in tree order (SoA), source weights w0 = q gamma, w1..3 = q p
     double *tx, *ty, *tz, *w0, *w1, *w2, *w3;
+    double *pmx, *pmy, *pmz;  // plain momenta in tree order, only with FMM_KERNEL_SOURCE_MOMENTUM (else NULL)
     int32_t *perm;          // [N] tree position -> caller index
     // nodes, heap index 1..nodes (entry 0 unused)
     int32_t *node_lo;       // [nodes+2] range start; node_hi(i) stored separately
@@ -103,6 +104,7 @@ int pairs_p2p(fmm_plan *p);
 int pairs_m2l(fmm_plan *p);
 int pairs_direct(fmm_ctx *c, int64_t N, const double *x, const double *y, const double *z,
                  const double *w0, const double *w1, const double *w2, const double *w3,
+                 const double *px, const double *py, const double *pz /* non-NULL: source-momentum kernel */,
                  double gamma_bar, int raw, int64_t nt, const int64_t *tidx,
                  double *Ex, double *Ey, double *Ez, double *Bx, double *By, double *Bz);
 int pairs_source_weights(fmm_ctx *c, int64_t N, const double *px, const double *py, const double *pz,

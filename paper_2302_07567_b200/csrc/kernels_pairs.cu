@@ -40,35 +40,48 @@ int pairs_source_weights(fmm_ctx *c, int64_t N, const double *px, const double *
 // ---------------------------------------------------------------------------------------
 #define PAIR_TILE 256
 
+// SM (FMM_KERNEL_SOURCE_MOMENTUM): a fifth double2 carries the source's plain momentum, (m3,px) (py,pz).
+template <bool SM>
 __device__ __forceinline__ void stage_tile(double2 *tile, int count, const double *__restrict__ x, const double *__restrict__ y,
                                            const double *__restrict__ z, const double *__restrict__ w0, const double *__restrict__ w1,
-                                           const double *__restrict__ w2, const double *__restrict__ w3, int64_t base)
+                                           const double *__restrict__ w2, const double *__restrict__ w3, const double *__restrict__ px,
+                                           const double *__restrict__ py, const double *__restrict__ pz, int64_t base)
 {
+    constexpr int ST = SM ? 5 : 4;
     for (int j = threadIdx.x; j < count; j += blockDim.x) {
-        tile[4 * j + 0] = make_double2(x[base + j], y[base + j]);
-        tile[4 * j + 1] = make_double2(z[base + j], w0[base + j]);
-        tile[4 * j + 2] = make_double2(w1[base + j], w2[base + j]);
-        tile[4 * j + 3] = make_double2(w3[base + j], 0.0);
+        tile[ST * j + 0] = make_double2(x[base + j], y[base + j]);
+        tile[ST * j + 1] = make_double2(z[base + j], w0[base + j]);
+        tile[ST * j + 2] = make_double2(w1[base + j], w2[base + j]);
+        tile[ST * j + 3] = make_double2(w3[base + j], SM ? px[base + j] : 0.0);
+        if (SM) tile[ST * j + 4] = make_double2(py[base + j], pz[base + j]);
     }
 }
 
 // One staged tile acting on the thread's NT targets: the tile is read once from shared memory for NT evaluations
 // (4 LDS.128 per source), and the accumulate-FMAs of the NT targets that share a source weight are adjacent.
-template <int NT>
+template <int NT, bool SM>
 __device__ __forceinline__ void tile_interact(const double2 *tile, int count, const double (&xt)[NT], const double (&yt)[NT],
                                               const double (&zt)[NT], double g2, double (&ex)[NT], double (&ey)[NT], double (&ez)[NT],
                                               double (&bx)[NT], double (&by)[NT], double (&bz)[NT])
 {
 #pragma unroll 2
     for (int j = 0; j < count; ++j) {
-        double2 a = tile[4 * j + 0], b = tile[4 * j + 1], c = tile[4 * j + 2], d = tile[4 * j + 3];
+        constexpr int ST = SM ? 5 : 4;
+        double2 a = tile[ST * j + 0], b = tile[ST * j + 1], c = tile[ST * j + 2], d = tile[ST * j + 3];
+        double2 pyz = SM ? tile[ST * j + (SM ? 4 : 0)] : make_double2(0.0, 0.0);
         double gx[NT], gy[NT], gz[NT];
 #pragma unroll
         for (int k = 0; k < NT; ++k) {
             double dx = xt[k] - a.x, dy = yt[k] - a.y, dz = zt[k] - b.x;
             double D = dx * dx;
             D = fma(dy, dy, D);
-            D = fma(g2 * dz, dz, D);
+            if (SM) {  // D = |d|^2 + (p_j . d)^2 (G6 alternative)
+                D = fma(dz, dz, D);
+                double pd = fma(pyz.y, dz, fma(pyz.x, dy, d.y * dx));
+                D = fma(pd, pd, D);
+            } else {   // eq. (3.2): D = dx^2 + dy^2 + gamma_bar^2 dz^2
+                D = fma(g2 * dz, dz, D);
+            }
             double w = inv_r3(D);
             gx[k] = w * dx; gy[k] = w * dy; gz[k] = w * dz;
         }
@@ -88,15 +101,17 @@ __device__ __forceinline__ void tile_interact(const double2 *tile, int count, co
 // a7: P2P.  One block per target leaf (blocks issued in descending-work order); NT target particles per
 // thread; the source leaves of the CSR row are staged tile by tile.
 // ---------------------------------------------------------------------------------------
-template <int NT>
+template <int NT, bool SM>
 __global__ void __launch_bounds__(256) p2p_kernel(int N, double g2, const int32_t *__restrict__ order, const int32_t *__restrict__ off,
                                                   const int32_t *__restrict__ src, const int32_t *__restrict__ node_lo,
                                                   const int32_t *__restrict__ node_hi, const double *__restrict__ tx,
                                                   const double *__restrict__ ty, const double *__restrict__ tz,
                                                   const double *__restrict__ w0, const double *__restrict__ w1,
-                                                  const double *__restrict__ w2, const double *__restrict__ w3, double *__restrict__ near_)
+                                                  const double *__restrict__ w2, const double *__restrict__ w3,
+                                                  const double *__restrict__ pmx, const double *__restrict__ pmy,
+                                                  const double *__restrict__ pmz, double *__restrict__ near_)
 {
-    __shared__ double2 tile[4 * PAIR_TILE];
+    __shared__ double2 tile[(SM ? 5 : 4) * PAIR_TILE];
     const int t = order[blockIdx.x];
     const int tlo = node_lo[t], thi = node_hi[t];
     const int e0 = off[t], e1 = off[t + 1];
@@ -115,9 +130,9 @@ __global__ void __launch_bounds__(256) p2p_kernel(int N, double g2, const int32_
             for (int j0 = slo; j0 < shi; j0 += PAIR_TILE) {
                 int count = min(PAIR_TILE, shi - j0);
                 __syncthreads();
-                stage_tile(tile, count, tx, ty, tz, w0, w1, w2, w3, j0);
+                stage_tile<SM>(tile, count, tx, ty, tz, w0, w1, w2, w3, pmx, pmy, pmz, j0);
                 __syncthreads();
-                tile_interact<NT>(tile, count, xt, yt, zt, g2, ex, ey, ez, bx, by, bz);
+                tile_interact<NT, SM>(tile, count, xt, yt, zt, g2, ex, ey, ez, bx, by, bz);
             }
         }
 #pragma unroll
@@ -162,15 +177,16 @@ int pairs_p2p(fmm_plan *p)
     int maxleaf = (int)((p->N + p->leaves - 1) / p->leaves);
     int nt, threads;
     p2p_shape(p->leaves, maxleaf, &nt, &threads);
-#define P2P_LAUNCH(NT)                                                                                                              \
-    p2p_kernel<NT><<<(unsigned)p->leaves, threads, 0, c->stream>>>((int)p->N, p->gamma_bar * p->gamma_bar, p->p2p_order, p->p2p_off, \
-                                                                   p->p2p_src, p->node_lo, p->node_hi, p->tx, p->ty, p->tz, p->w0,   \
-                                                                   p->w1, p->w2, p->w3, p->near_)
+    const bool sm = (p->flags & FMM_KERNEL_SOURCE_MOMENTUM) != 0;
+#define P2P_LAUNCH(NT, SM)                                                                                                               \
+    p2p_kernel<NT, SM><<<(unsigned)p->leaves, threads, 0, c->stream>>>((int)p->N, p->gamma_bar * p->gamma_bar, p->p2p_order, p->p2p_off, \
+                                                                       p->p2p_src, p->node_lo, p->node_hi, p->tx, p->ty, p->tz, p->w0,   \
+                                                                       p->w1, p->w2, p->w3, p->pmx, p->pmy, p->pmz, p->near_)
     switch (nt) {
-        case 1: P2P_LAUNCH(1); break;
-        case 2: P2P_LAUNCH(2); break;
-        case 3: P2P_LAUNCH(3); break;
-        default: P2P_LAUNCH(4); break;
+        case 1: if (sm) P2P_LAUNCH(1, true); else P2P_LAUNCH(1, false); break;
+        case 2: if (sm) P2P_LAUNCH(2, true); else P2P_LAUNCH(2, false); break;
+        case 3: if (sm) P2P_LAUNCH(3, true); else P2P_LAUNCH(3, false); break;
+        default: if (sm) P2P_LAUNCH(4, true); else P2P_LAUNCH(4, false); break;
     }
 #undef P2P_LAUNCH
     FMM_LAUNCH_CHECK(c, "p2p_kernel");
@@ -184,13 +200,16 @@ int pairs_p2p(fmm_plan *p)
 #define DIRECT_NT 4
 #define DIRECT_THREADS 128
 #define DIRECT_TARGETS (DIRECT_NT * DIRECT_THREADS)
+template <bool SM>
 __global__ void __launch_bounds__(DIRECT_THREADS) direct_kernel(int64_t N, double g2, int64_t nt, const int64_t *__restrict__ tidx,
                                                                 int64_t chunk, const double *__restrict__ x, const double *__restrict__ y,
                                                                 const double *__restrict__ z, const double *__restrict__ w0,
                                                                 const double *__restrict__ w1, const double *__restrict__ w2,
-                                                                const double *__restrict__ w3, double *__restrict__ part /* [splits][6][nt] */)
+                                                                const double *__restrict__ w3, const double *__restrict__ px,
+                                                                const double *__restrict__ py, const double *__restrict__ pz,
+                                                                double *__restrict__ part /* [splits][6][nt] */)
 {
-    __shared__ double2 tile[4 * PAIR_TILE];
+    __shared__ double2 tile[(SM ? 5 : 4) * PAIR_TILE];
     double xt[DIRECT_NT], yt[DIRECT_NT], zt[DIRECT_NT], ex[DIRECT_NT], ey[DIRECT_NT], ez[DIRECT_NT], bx[DIRECT_NT], by[DIRECT_NT], bz[DIRECT_NT];
 #pragma unroll
     for (int k = 0; k < DIRECT_NT; ++k) {
@@ -205,9 +224,9 @@ __global__ void __launch_bounds__(DIRECT_THREADS) direct_kernel(int64_t N, doubl
     for (int64_t j0 = s0; j0 < s1; j0 += PAIR_TILE) {
         int count = (int)((s1 - j0 < PAIR_TILE) ? (s1 - j0) : PAIR_TILE);
         __syncthreads();
-        stage_tile(tile, count, x, y, z, w0, w1, w2, w3, j0);
+        stage_tile<SM>(tile, count, x, y, z, w0, w1, w2, w3, px, py, pz, j0);
         __syncthreads();
-        tile_interact<DIRECT_NT>(tile, count, xt, yt, zt, g2, ex, ey, ez, bx, by, bz);
+        tile_interact<DIRECT_NT, SM>(tile, count, xt, yt, zt, g2, ex, ey, ez, bx, by, bz);
     }
 #pragma unroll
     for (int k = 0; k < DIRECT_NT; ++k) {
@@ -235,6 +254,7 @@ __global__ void direct_reduce(int64_t nt, int splits, const double *__restrict__
 
 int pairs_direct(fmm_ctx *c, int64_t N, const double *x, const double *y, const double *z,
                  const double *w0, const double *w1, const double *w2, const double *w3,
+                 const double *px, const double *py, const double *pz,
                  double gamma_bar, int raw, int64_t nt, const int64_t *tidx,
                  double *Ex, double *Ey, double *Ez, double *Bx, double *By, double *Bz)
 {
@@ -251,7 +271,10 @@ int pairs_direct(fmm_ctx *c, int64_t N, const double *x, const double *y, const 
     double *part = (double *)ctx_alloc(c, sizeof(double) * 6 * (size_t)nt * (size_t)splits);
     if (!part) return FMM_ENOMEM;
     dim3 grid((unsigned)tblocks, (unsigned)splits);
-    direct_kernel<<<grid, DIRECT_THREADS, 0, c->stream>>>(N, gamma_bar * gamma_bar, nt, tidx, chunk, x, y, z, w0, w1, w2, w3, part);
+    if (px)
+        direct_kernel<true><<<grid, DIRECT_THREADS, 0, c->stream>>>(N, gamma_bar * gamma_bar, nt, tidx, chunk, x, y, z, w0, w1, w2, w3, px, py, pz, part);
+    else
+        direct_kernel<false><<<grid, DIRECT_THREADS, 0, c->stream>>>(N, gamma_bar * gamma_bar, nt, tidx, chunk, x, y, z, w0, w1, w2, w3, px, py, pz, part);
     FMM_LAUNCH_CHECK(c, "direct_kernel");
     double cE = 1.0, cB = 1.0;
     if (!raw) {

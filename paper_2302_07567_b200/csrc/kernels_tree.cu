@@ -284,7 +284,8 @@ __global__ void permute_particles(int N, const uint32_t *__restrict__ order, con
                                   const double *__restrict__ z, const double *__restrict__ px, const double *__restrict__ py,
                                   const double *__restrict__ pz, const double *__restrict__ q, double q_scalar,
                                   int32_t *__restrict__ perm, double *__restrict__ tx, double *__restrict__ ty, double *__restrict__ tz,
-                                  double *__restrict__ w0, double *__restrict__ w1, double *__restrict__ w2, double *__restrict__ w3)
+                                  double *__restrict__ w0, double *__restrict__ w1, double *__restrict__ w2, double *__restrict__ w3,
+                                  double *__restrict__ pmx, double *__restrict__ pmy, double *__restrict__ pmz)
 {
     int k = blockIdx.x * blockDim.x + threadIdx.x;
     if (k >= N) return;
@@ -300,6 +301,11 @@ __global__ void permute_particles(int N, const uint32_t *__restrict__ order, con
     w1[k] = qj * ax;
     w2[k] = qj * ay;
     w3[k] = qj * az;
+    if (pmx) {  // FMM_KERNEL_SOURCE_MOMENTUM: the near field needs the plain momenta of the sources
+        pmx[k] = ax;
+        pmy[k] = ay;
+        pmz[k] = az;
+    }
 }
 
 // ---------------------------------------------------------------------------------------
@@ -431,7 +437,7 @@ int tree_build(fmm_plan *p, const fmm_particles_t *in)
         }
         order = cur + 3 * (size_t)N;  // the index-ordered list: leaves in heap order, ascending index inside (T-3)
         permute_particles<<<gN, T, 0, st>>>(N, order, in->x, in->y, in->z, in->px, in->py, in->pz, in->q, in->q_scalar,
-                                            p->perm, p->tx, p->ty, p->tz, p->w0, p->w1, p->w2, p->w3);
+                                            p->perm, p->tx, p->ty, p->tz, p->w0, p->w1, p->w2, p->w3, p->pmx, p->pmy, p->pmz);
         FMM_LAUNCH_CHECK(c, "permute_particles");
         ctx_free(c, lists2); ctx_free(c, scan); ctx_free(c, left); ctx_free(c, axis);
     } else {
@@ -446,7 +452,7 @@ int tree_build(fmm_plan *p, const fmm_particles_t *in)
         FMM_TRY(sort_pairs_u64(c, keys, lists, tkeys, tvals, N, 0, 64));
         order = lists;
         permute_particles<<<gN, T, 0, st>>>(N, order, in->x, in->y, in->z, in->px, in->py, in->pz, in->q, in->q_scalar,
-                                            p->perm, p->tx, p->ty, p->tz, p->w0, p->w1, p->w2, p->w3);
+                                            p->perm, p->tx, p->ty, p->tz, p->w0, p->w1, p->w2, p->w3, p->pmx, p->pmy, p->pmz);
         FMM_LAUNCH_CHECK(c, "permute_particles");
         ctx_free(c, mm);
     }

@@ -216,3 +216,39 @@ def test_bad_arguments(fmm):
     bad[3] = np.nan
     with pytest.raises(fmm.FmmError):
         fmm.fmm_plan_create(w.x, w.y, w.z, w.px, w.py, bad, w.q, order_n=2, leaf_size=8, theta=0.5)
+
+
+# ---------------------------------------------------------------------------------------------
+# FMM_KERNEL_SOURCE_MOMENTUM: near field stretched along each source's own momentum (G6 alternative,
+# SURVEY.md 8(f) rank 2).  Same bars as the default kernel.
+# ---------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("N,targets", [(4096, None), (3001, 500)])
+def test_direct_source_momentum_matches_oracle(fmm, N, targets):
+    w = workloads.config(4, N=N)                      # gamma = 100, 2 % spread: the two readings differ most here
+    tg = None if targets is None else np.sort(np.random.default_rng(5).choice(N, targets, replace=False)).astype(np.int64)
+    E, B = to_np(fmm.fmm_direct(*w.arrays(), w.q, flags=fmm.FMM_KERNEL_SOURCE_MOMENTUM, targets=tg))
+    Eo, Bo = oracle.direct(*w.arrays(), w.q, source_momentum=True, targets=tg)
+    assert_close(E, Eo, "direct E (source momentum)")
+    assert_close(B, Bo, "direct B (source momentum)")
+    Em, _ = oracle.direct(*w.arrays(), w.q, targets=tg)
+    assert oracle.err2(Eo, Em) > 1e-4                 # ... and it is a different kernel
+
+
+@pytest.mark.parametrize("case", [c for c in CASES if c[0] in ("config1", "config2_ragged", "config4_small", "paper_cube_n2",
+                                                              "single_leaf")], ids=lambda c: c[0])
+def test_fmm_source_momentum_matches_serial_oracle(fmm, case):
+    _, w, n, N0, theta = case
+    plan = fmm.fmm_plan_create(*w.arrays(), w.q, order_n=n, leaf_size=N0, theta=theta,
+                               flags=fmm.FMM_TREE_KD | fmm.FMM_KERNEL_SOURCE_MOMENTUM)
+    st = plan.stats()
+    E, B = to_np(plan.eval())
+    ex = plan.export()
+    op = oracle.Plan(*w.arrays(), w.q, order_n=n, leaf_size=N0, theta=theta, gamma_bar_value=st["gamma_bar"],
+                     source_momentum=True)
+    p2p, m2l = op.lists()                              # the kernel mode does not touch tree or lists
+    assert np.array_equal(ex["perm"], op.perm())
+    assert np.array_equal(ex["p2p_src"], p2p[:, 1]) and np.array_equal(ex["m2l_src"], m2l[:, 1])
+    Eo, Bo = op.eval()
+    assert_close(E, Eo, "FMM E (source momentum)")
+    assert_close(B, Bo, "FMM B (source momentum)")
+    plan.close()
