@@ -61,7 +61,7 @@ __device__ __forceinline__ void stage_tile(double2 *tile, int count, const doubl
 // (4 LDS.128 per source), and the accumulate-FMAs of the NT targets that share a source weight are adjacent.
 template <int NT, bool SM>
 __device__ __forceinline__ void tile_interact(const double2 *tile, int count, const double (&xt)[NT], const double (&yt)[NT],
-                                              const double (&zt)[NT], double g2, double (&ex)[NT], double (&ey)[NT], double (&ez)[NT],
+                                              const double (&zt)[NT], double gb, double (&ex)[NT], double (&ey)[NT], double (&ez)[NT],
                                               double (&bx)[NT], double (&by)[NT], double (&bz)[NT])
 {
 #pragma unroll 2
@@ -79,8 +79,10 @@ __device__ __forceinline__ void tile_interact(const double2 *tile, int count, co
                 D = fma(dz, dz, D);
                 double pd = fma(pyz.y, dz, fma(pyz.x, dy, d.y * dx));
                 D = fma(pd, pd, D);
-            } else {   // eq. (3.2): D = dx^2 + dy^2 + gamma_bar^2 dz^2
-                D = fma(g2 * dz, dz, D);
+            } else {   // eq. (3.2): D = dx^2 + dy^2 + (gamma_bar dz)^2; squaring the scaled difference keeps the
+                       // DFMA at two register operands (full FP64 issue rate)
+                const double sz = gb * dz;
+                D = fma(sz, sz, D);
             }
             double w = inv_r3(D);
             gx[k] = w * dx; gy[k] = w * dy; gz[k] = w * dz;
@@ -102,7 +104,7 @@ __device__ __forceinline__ void tile_interact(const double2 *tile, int count, co
 // thread; the source leaves of the CSR row are staged tile by tile.
 // ---------------------------------------------------------------------------------------
 template <int NT, bool SM>
-__global__ void __launch_bounds__(256) p2p_kernel(int N, double g2, const int32_t *__restrict__ order, const int32_t *__restrict__ off,
+__global__ void __launch_bounds__(256) p2p_kernel(int N, double gb, const int32_t *__restrict__ order, const int32_t *__restrict__ off,
                                                   const int32_t *__restrict__ src, const int32_t *__restrict__ node_lo,
                                                   const int32_t *__restrict__ node_hi, const double *__restrict__ tx,
                                                   const double *__restrict__ ty, const double *__restrict__ tz,
@@ -132,7 +134,7 @@ __global__ void __launch_bounds__(256) p2p_kernel(int N, double g2, const int32_
                 __syncthreads();
                 stage_tile<SM>(tile, count, tx, ty, tz, w0, w1, w2, w3, pmx, pmy, pmz, j0);
                 __syncthreads();
-                tile_interact<NT, SM>(tile, count, xt, yt, zt, g2, ex, ey, ez, bx, by, bz);
+                tile_interact<NT, SM>(tile, count, xt, yt, zt, gb, ex, ey, ez, bx, by, bz);
             }
         }
 #pragma unroll
@@ -179,7 +181,7 @@ int pairs_p2p(fmm_plan *p)
     p2p_shape(p->leaves, maxleaf, &nt, &threads);
     const bool sm = (p->flags & FMM_KERNEL_SOURCE_MOMENTUM) != 0;
 #define P2P_LAUNCH(NT, SM)                                                                                                               \
-    p2p_kernel<NT, SM><<<(unsigned)p->leaves, threads, 0, c->stream>>>((int)p->N, p->gamma_bar * p->gamma_bar, p->p2p_order, p->p2p_off, \
+    p2p_kernel<NT, SM><<<(unsigned)p->leaves, threads, 0, c->stream>>>((int)p->N, p->gamma_bar, p->p2p_order, p->p2p_off, \
                                                                        p->p2p_src, p->node_lo, p->node_hi, p->tx, p->ty, p->tz, p->w0,   \
                                                                        p->w1, p->w2, p->w3, p->pmx, p->pmy, p->pmz, p->near_)
     switch (nt) {
@@ -201,7 +203,7 @@ int pairs_p2p(fmm_plan *p)
 #define DIRECT_THREADS 128
 #define DIRECT_TARGETS (DIRECT_NT * DIRECT_THREADS)
 template <bool SM>
-__global__ void __launch_bounds__(DIRECT_THREADS) direct_kernel(int64_t N, double g2, int64_t nt, const int64_t *__restrict__ tidx,
+__global__ void __launch_bounds__(DIRECT_THREADS) direct_kernel(int64_t N, double gb, int64_t nt, const int64_t *__restrict__ tidx,
                                                                 int64_t chunk, const double *__restrict__ x, const double *__restrict__ y,
                                                                 const double *__restrict__ z, const double *__restrict__ w0,
                                                                 const double *__restrict__ w1, const double *__restrict__ w2,
@@ -226,7 +228,7 @@ __global__ void __launch_bounds__(DIRECT_THREADS) direct_kernel(int64_t N, doubl
         __syncthreads();
         stage_tile<SM>(tile, count, x, y, z, w0, w1, w2, w3, px, py, pz, j0);
         __syncthreads();
-        tile_interact<DIRECT_NT, SM>(tile, count, xt, yt, zt, g2, ex, ey, ez, bx, by, bz);
+        tile_interact<DIRECT_NT, SM>(tile, count, xt, yt, zt, gb, ex, ey, ez, bx, by, bz);
     }
 #pragma unroll
     for (int k = 0; k < DIRECT_NT; ++k) {
@@ -272,9 +274,9 @@ int pairs_direct(fmm_ctx *c, int64_t N, const double *x, const double *y, const 
     if (!part) return FMM_ENOMEM;
     dim3 grid((unsigned)tblocks, (unsigned)splits);
     if (px)
-        direct_kernel<true><<<grid, DIRECT_THREADS, 0, c->stream>>>(N, gamma_bar * gamma_bar, nt, tidx, chunk, x, y, z, w0, w1, w2, w3, px, py, pz, part);
+        direct_kernel<true><<<grid, DIRECT_THREADS, 0, c->stream>>>(N, gamma_bar, nt, tidx, chunk, x, y, z, w0, w1, w2, w3, px, py, pz, part);
     else
-        direct_kernel<false><<<grid, DIRECT_THREADS, 0, c->stream>>>(N, gamma_bar * gamma_bar, nt, tidx, chunk, x, y, z, w0, w1, w2, w3, px, py, pz, part);
+        direct_kernel<false><<<grid, DIRECT_THREADS, 0, c->stream>>>(N, gamma_bar, nt, tidx, chunk, x, y, z, w0, w1, w2, w3, px, py, pz, part);
     FMM_LAUNCH_CHECK(c, "direct_kernel");
     double cE = 1.0, cB = 1.0;
     if (!raw) {
