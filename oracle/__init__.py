@@ -57,6 +57,8 @@ def lib():
         _lib.orc_plan_create.restype = C.c_void_p
         _lib.orc_plan_create.argtypes = [C.c_int64] + [_dp] * 7 + [C.c_double, C.c_int, C.c_int,
                                                                     C.c_double, C.c_double, C.c_int, C.c_int]
+        _lib.orc_plan_create_given_order.restype = C.c_void_p
+        _lib.orc_plan_create_given_order.argtypes = list(_lib.orc_plan_create.argtypes[:13]) + [C.c_int, _i64p]
         _lib.orc_plan_destroy.argtypes = [C.c_void_p]
         _lib.orc_plan_sizes.argtypes = [C.c_void_p, _i64p]
         _lib.orc_plan_gamma_bar.restype = C.c_double
@@ -131,13 +133,23 @@ class Plan:
     """O2: tree + interaction lists, then upward / eval (serial FMM of Alg 5.12)."""
 
     def __init__(self, x, y, z, px, py, pz, q=None, *, order_n, leaf_size, theta,
-                 gamma_bar_value=None, tree_mode=TREE_KD, raw=False, source_momentum=False):
+                 gamma_bar_value=None, tree_mode=TREE_KD, raw=False, source_momentum=False, given_order=None):
+        """given_order: particle order (tree position -> particle index) to build the tree over instead of sorting
+        (refit of an existing partition); tree_mode is then ignored."""
         arrs = [_d(a) for a in (x, y, z, px, py, pz)]
         self.N = len(arrs[0][0])
         qa, qp, qs = _charges(q, self.N)
         gb = -1.0 if gamma_bar_value is None else float(gamma_bar_value)
-        self._h = lib().orc_plan_create(self.N, *[p for _, p in arrs], qp, qs, int(order_n),
-                                        int(leaf_size), float(theta), gb, int(tree_mode), int(bool(raw)) | (2 if source_momentum else 0))
+        flags = int(bool(raw)) | (2 if source_momentum else 0)
+        if given_order is None:
+            self._h = lib().orc_plan_create(self.N, *[p for _, p in arrs], qp, qs, int(order_n),
+                                            int(leaf_size), float(theta), gb, int(tree_mode), flags)
+        else:
+            go = np.ascontiguousarray(given_order, dtype=np.int64)
+            if go.shape != (self.N,) or not np.array_equal(np.sort(go), np.arange(self.N)):
+                raise ValueError("given_order must be a permutation of range(N)")
+            self._h = lib().orc_plan_create_given_order(self.N, *[p for _, p in arrs], qp, qs, int(order_n),
+                                                        int(leaf_size), float(theta), gb, flags, go.ctypes.data_as(_i64p))
         if not self._h:
             raise ValueError("orc_plan_create: invalid arguments")
         s = np.empty(6, dtype=np.int64)

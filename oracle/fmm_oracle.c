@@ -411,11 +411,41 @@ static int cmp_pair(const void *pa, const void *pb)
 }
 
 /* Plan ------------------------------------------------------------------------ */
+static orc_plan_t *plan_create(int64_t N, const double *x, const double *y, const double *z,
+                               const double *px, const double *py, const double *pz,
+                               const double *q, double q_scalar,
+                               int n, int N0, double theta, double gamma_bar,
+                               int tree_mode, int raw, const int64_t *given_perm);
+
 orc_plan_t *orc_plan_create(int64_t N, const double *x, const double *y, const double *z,
                             const double *px, const double *py, const double *pz,
                             const double *q, double q_scalar,
                             int n, int N0, double theta, double gamma_bar,
                             int tree_mode, int raw)
+{
+    if (tree_mode != ORC_TREE_KD && tree_mode != ORC_TREE_MORTON_MEDIAN)
+        return NULL;
+    return plan_create(N, x, y, z, px, py, pz, q, q_scalar, n, N0, theta, gamma_bar, tree_mode, raw, NULL);
+}
+
+/* Cluster tree over a GIVEN particle order (refit of an existing partition): node ranges are the
+ * closed-form ranges of T-2 over perm, bounding boxes are tight (T-4), lists come from the same traversal.  Any
+ * partition into contiguous ranges is a valid cluster tree for Alg 5.11 (PAPER.md:253 only asks for a partition);
+ * the admissibility condition is evaluated on the actual bounding boxes. */
+orc_plan_t *orc_plan_create_given_order(int64_t N, const double *x, const double *y, const double *z,
+                                        const double *px, const double *py, const double *pz,
+                                        const double *q, double q_scalar,
+                                        int n, int N0, double theta, double gamma_bar, int raw, const int64_t *perm)
+{
+    if (!perm) return NULL;
+    return plan_create(N, x, y, z, px, py, pz, q, q_scalar, n, N0, theta, gamma_bar, ORC_TREE_GIVEN, raw, perm);
+}
+
+static orc_plan_t *plan_create(int64_t N, const double *x, const double *y, const double *z,
+                               const double *px, const double *py, const double *pz,
+                               const double *q, double q_scalar,
+                               int n, int N0, double theta, double gamma_bar,
+                               int tree_mode, int raw, const int64_t *given_perm)
 {
     if (N < 1 || n < 1 || n > 31 || N0 < 1 || !(theta > 0.0))
         return NULL;
@@ -465,7 +495,7 @@ orc_plan_t *orc_plan_create(int64_t N, const double *x, const double *y, const d
     }
     p->perm = (int64_t *)malloc(sizeof(int64_t) * (size_t)N);
     for (int64_t j = 0; j < N; ++j)
-        p->perm[j] = j;
+        p->perm[j] = given_perm ? given_perm[j] : j;
     p->lo = (int64_t *)calloc((size_t)p->nodes + 1, sizeof(int64_t));
     p->hi = (int64_t *)calloc((size_t)p->nodes + 1, sizeof(int64_t));
     p->bbox = (double *)calloc(6 * ((size_t)p->nodes + 1), sizeof(double));

@@ -34,6 +34,7 @@ extern "C" {
 
 #define ORC_TREE_KD            0  /* Alg 5.2, reading T-3   */
 #define ORC_TREE_MORTON_MEDIAN 1  /* DESIGN.md reading T-3' (north_star's Morton order)  */
+#define ORC_TREE_GIVEN         2  /* particle order supplied by the caller (orc_plan_create_given_order) */
 
 /* flags word passed as `raw`: */
 #define ORC_RAW_SUMS               1  /* no SI prefactors                                                  */
@@ -66,6 +67,12 @@ orc_plan_t *orc_plan_create(int64_t N, const double *x, const double *y, const d
                             const double *q, double q_scalar,
                             int n, int N0, double theta, double gamma_bar,
                             int tree_mode, int raw);
+/* Same, over a particle order supplied by the caller (perm[N]: tree position -> particle index, a permutation):
+ * closed-form node ranges (T-2) over that order, tight boxes, same traversal.  Refit of an existing partition. */
+orc_plan_t *orc_plan_create_given_order(int64_t N, const double *x, const double *y, const double *z,
+                                        const double *px, const double *py, const double *pz,
+                                        const double *q, double q_scalar,
+                                        int n, int N0, double theta, double gamma_bar, int raw, const int64_t *perm);
 void orc_plan_destroy(orc_plan_t *);
 
 /* sizes: out[0]=kappa out[1]=nodes out[2]=leaves out[3]=P out[4]=len(p2p) out[5]=len(m2l) */

@@ -337,3 +337,56 @@ def test_paper_shaped_input_identical_momenta():
     assert oracle.err2(B, Bexp) < 1e-12
     Ed, Bd = oracle.direct(*w.arrays(), q=w.q)
     assert oracle.err2(E, Ed) < 5e-3
+
+
+# ---------------------------------------------------------------------------------------------
+# Tree over a given particle order (refit of an existing partition)
+# ---------------------------------------------------------------------------------------------
+def test_given_order_equal_to_kd_order_reproduces_the_kd_plan():
+    """Fed the KD plan's own permutation, the given-order plan is the KD plan: same ranges, boxes, lists, fields."""
+    w = small(N=3000)
+    a = plan_of(w, theta=0.5)
+    b = oracle.Plan(*w.arrays(), w.q, order_n=4, leaf_size=64, theta=0.5, gamma_bar_value=a.gamma_bar, given_order=a.perm())
+    assert np.array_equal(a.perm(), b.perm())
+    for u, v in zip(a.node_arrays(), b.node_arrays()):
+        assert np.array_equal(u, v)
+    for u, v in zip(a.lists(), b.lists()):
+        assert np.array_equal(u, v)
+    Ea, Ba = a.eval()
+    Eb, Bb = b.eval()
+    assert np.array_equal(Ea, Eb) and np.array_equal(Ba, Bb)
+
+
+def test_given_order_after_a_drift_is_a_valid_tree_with_the_same_accuracy():
+    """Particles drift (a tracker step); the OLD order is kept.  The plan is still a partition with tight boxes, every
+    leaf pair is covered exactly once (P10), and the FMM error against the direct sum stays at the KD tree's level."""
+    w = small(N=4096)
+    old = plan_of(w, theta=0.5)
+    rng = np.random.default_rng(3)
+    x2 = w.x + 2e-5 * rng.standard_normal(w.N)       # 2 % of sigma_x
+    y2 = w.y + 2e-5 * rng.standard_normal(w.N)
+    z2 = w.z + 2e-6 * rng.standard_normal(w.N)
+    args = (x2, y2, z2, w.px, w.py, w.pz)
+    p = oracle.Plan(*args, w.q, order_n=4, leaf_size=64, theta=0.5, given_order=old.perm())
+    assert np.array_equal(p.perm(), old.perm())
+    lo, hi, bb = p.node_arrays()
+    lo0, hi0, _ = old.node_arrays()
+    assert np.array_equal(lo, lo0) and np.array_equal(hi, hi0)           # T-2 ranges depend on (N, N0) only
+    perm = p.perm()
+    for i in (1, 2, 37, p.nodes):                                         # tight boxes (T-4)
+        m = perm[lo[i - 1]:hi[i - 1]]
+        assert np.array_equal(bb[i - 1], [x2[m].min(), y2[m].min(), z2[m].min(), x2[m].max(), y2[m].max(), z2[m].max()])
+    p2p, m2l = p.lists()
+    Lf = p.leaves
+    cover = np.zeros((Lf, Lf), dtype=np.int32)
+    for t, s in np.concatenate([p2p, m2l]):
+        lt, ls = int(np.log2(t)), int(np.log2(s))
+        wt, ws = Lf >> lt, Lf >> ls
+        cover[(t - (1 << lt)) * wt:(t - (1 << lt) + 1) * wt, (s - (1 << ls)) * ws:(s - (1 << ls) + 1) * ws] += 1
+    assert np.all(cover == 1)
+    Ed, Bd = oracle.direct(*args, w.q, gamma_bar_value=p.gamma_bar)
+    E, B = p.eval()
+    fresh = oracle.Plan(*args, w.q, order_n=4, leaf_size=64, theta=0.5, gamma_bar_value=p.gamma_bar)
+    Ef, _ = fresh.eval()
+    e_refit, e_fresh = oracle.err2(E, Ed), oracle.err2(Ef, Ed)
+    assert e_refit < 3 * e_fresh and e_refit < 5e-3, (e_refit, e_fresh)
