@@ -135,6 +135,14 @@ int fmm_plan_create(fmm_plan_t **out, const fmm_particles_t *particles, const fm
  * reusing the workspace where sizes allow. */
 int fmm_plan_update(fmm_plan_t *plan, const fmm_particles_t *particles);
 
+/* Refit for time stepping (the paper leaves the tracker outside): same N and
+ * parameters, particles have moved a little.  The particle ORDER of the last fmm_plan_create / fmm_plan_update is kept
+ * (no sort): the new positions / momenta / charges are gathered through it, gamma_bar, the tight bounding boxes and both
+ * interaction lists are rebuilt on the new boxes.  Any partition into contiguous ranges is a valid cluster tree for
+ * Alg 5.11 and the admissibility condition is evaluated on the actual boxes, so the result is a correct FMM of the same
+ * order of accuracy; it is no longer the median split of the NEW positions.  Synchronises the stream. */
+int fmm_plan_refit(fmm_plan_t *plan, const fmm_particles_t *particles);
+
 /* a4-a10: P2M, M2M, M2L, P2P, L2L, L2P, prefactors, scatter to caller order.  Enqueue only.
  * Ex..Bz: device arrays of length N, overwritten. */
 int fmm_eval(fmm_plan_t *plan, double *Ex, double *Ey, double *Ez, double *Bx, double *By, double *Bz);

@@ -63,7 +63,7 @@ class fmm_export_t(C.Structure):
                 ("M", C.c_void_p), ("L", C.c_void_p)]
 
 
-EXPORTED_SYMBOLS = ["fmm_plan_create", "fmm_plan_update", "fmm_eval", "fmm_direct", "fmm_field_host",
+EXPORTED_SYMBOLS = ["fmm_plan_create", "fmm_plan_update", "fmm_plan_refit", "fmm_eval", "fmm_direct", "fmm_field_host",
                     "fmm_plan_set_timing", "fmm_plan_stats", "fmm_plan_export", "fmm_plan_destroy",
                     "fmm_launch_count", "fmm_probe_fp64_peak", "fmm_strerror", "fmm_last_error", "fmm_version"]
 
@@ -89,6 +89,8 @@ def load_library():
                                     ALLOC_FN, FREE_FN, vp, vp]
     lib.fmm_plan_update.restype = C.c_int
     lib.fmm_plan_update.argtypes = [vp, C.POINTER(fmm_particles_t)]
+    lib.fmm_plan_refit.restype = C.c_int
+    lib.fmm_plan_refit.argtypes = [vp, C.POINTER(fmm_particles_t)]
     lib.fmm_eval.restype = C.c_int
     lib.fmm_eval.argtypes = [vp] + [vp] * 6
     lib.fmm_direct.restype = C.c_int
@@ -195,6 +197,9 @@ class Plan:
     def update(self, x, y, z, px, py, pz, q=None):
         return fmm_plan_update(self, x, y, z, px, py, pz, q)
 
+    def refit(self, x, y, z, px, py, pz, q=None):
+        return fmm_plan_refit(self, x, y, z, px, py, pz, q)
+
     def eval(self, out=None):
         return fmm_eval(self, out)
 
@@ -240,6 +245,15 @@ def fmm_plan_update(plan: Plan, x, y, z, px, py, pz, q=None):
     with torch.cuda.device(plan.device):
         parts, keep = _particles(x, y, z, px, py, pz, q, plan.device)
         _check(lib.fmm_plan_update(plan._h, C.byref(parts)), plan._h)
+        del keep
+
+
+def fmm_plan_refit(plan: Plan, x, y, z, px, py, pz, q=None):
+    """Keeps the particle order of the last build; new boxes and lists on the moved particles (no sort)."""
+    lib = load_library()
+    with torch.cuda.device(plan.device):
+        parts, keep = _particles(x, y, z, px, py, pz, q, plan.device)
+        _check(lib.fmm_plan_refit(plan._h, C.byref(parts)), plan._h)
         del keep
 
 

@@ -132,7 +132,7 @@ static int plan_alloc_fixed(fmm_plan *p)
     return FMM_OK;
 }
 
-static int plan_build(fmm_plan *p, const fmm_particles_t *in)
+static int plan_build(fmm_plan *p, const fmm_particles_t *in, bool refit = false)
 {
     fmm_ctx *c = &p->ctx;
     FMM_CUDA(c, cudaEventRecord(p->ev_plan[0], c->stream));
@@ -142,7 +142,7 @@ static int plan_build(fmm_plan *p, const fmm_particles_t *in)
         FMM_TRY(tree_gamma_bar(c, p->N, in->px, in->py, in->pz, &p->gamma_bar));
         if (!isfinite(p->gamma_bar)) return FMM_ENONFINITE;
     }
-    FMM_TRY(tree_build(p, in));
+    FMM_TRY(refit ? tree_refit(p, in) : tree_build(p, in));
     FMM_CUDA(c, cudaEventRecord(p->ev_plan[1], c->stream));
     FMM_TRY(dtt_build_lists(p));
     FMM_CUDA(c, cudaEventRecord(p->ev_plan[2], c->stream));
@@ -211,6 +211,12 @@ extern "C" int fmm_plan_update(fmm_plan_t *p, const fmm_particles_t *in)
 {
     if (!p || check_particles(in) != FMM_OK || in->N != p->N) return FMM_EINVAL;
     return plan_build(p, in);
+}
+
+extern "C" int fmm_plan_refit(fmm_plan_t *p, const fmm_particles_t *in)
+{
+    if (!p || check_particles(in) != FMM_OK || in->N != p->N) return FMM_EINVAL;
+    return plan_build(p, in, true);
 }
 
 extern "C" int fmm_plan_set_timing(fmm_plan_t *p, int on)

@@ -92,6 +92,8 @@ struct fmm_plan {
 int tree_gamma_bar(fmm_ctx *c, int64_t N, const double *px, const double *py, const double *pz,
                    double *gamma_bar_out /* host */);
 int tree_build(fmm_plan *p, const fmm_particles_t *in);
+int tree_boxes(fmm_plan *p);
+int tree_refit(fmm_plan *p, const fmm_particles_t *in);  // keeps the particle order of the last build
 // ---- kernels_dtt.cu -----------------------------------------------------------------
 int dtt_build_lists(fmm_plan *p);
 // ---- kernels_interp.cu --------------------------------------------------------------

@@ -290,7 +290,7 @@ __global__ void permute_particles(int N, const uint32_t *__restrict__ order, con
     int k = blockIdx.x * blockDim.x + threadIdx.x;
     if (k >= N) return;
     uint32_t j = order[k];
-    perm[k] = (int32_t)j;
+    if (perm) perm[k] = (int32_t)j;
     tx[k] = x[j];
     ty[k] = y[j];
     tz[k] = z[j];
@@ -458,9 +458,30 @@ int tree_build(fmm_plan *p, const fmm_particles_t *in)
     }
     ctx_free(c, keys); ctx_free(c, tkeys); ctx_free(c, tvals); ctx_free(c, lists);
 
-    leaf_bbox<<<(unsigned)((p->leaves * 32 + T - 1) / T), T, 0, st>>>((int)p->leaves, p->node_lo, p->node_hi, p->tx, p->ty, p->tz, p->bbox);
+    return tree_boxes(p);
+}
+
+// a2 on the particles as they sit in tree order
+int tree_boxes(fmm_plan *p)
+{
+    fmm_ctx *c = &p->ctx;
+    const int T = 256;
+    leaf_bbox<<<(unsigned)((p->leaves * 32 + T - 1) / T), T, 0, c->stream>>>((int)p->leaves, p->node_lo, p->node_hi, p->tx, p->ty, p->tz, p->bbox);
     FMM_LAUNCH_CHECK(c, "leaf_bbox");
-    upper_bbox_and_geometry<<<1, 1024, 0, st>>>(p->kappa, (int)p->nodes, p->node_lo, p->node_hi, p->gamma_bar, p->bbox, p->node_geo);
+    upper_bbox_and_geometry<<<1, 1024, 0, c->stream>>>(p->kappa, (int)p->nodes, p->node_lo, p->node_hi, p->gamma_bar, p->bbox, p->node_geo);
     FMM_LAUNCH_CHECK(c, "upper_bbox_and_geometry");
     return FMM_OK;
+}
+
+// Refit: the particle order of the last build is kept; the new positions / momenta are
+// gathered through it and only the bounding boxes are recomputed.  Node ranges (T-2) depend on (N, N0) alone.
+int tree_refit(fmm_plan *p, const fmm_particles_t *in)
+{
+    fmm_ctx *c = &p->ctx;
+    const int N = (int)p->N, T = 256;
+    permute_particles<<<(N + T - 1) / T, T, 0, c->stream>>>(N, reinterpret_cast<const uint32_t *>(p->perm), in->x, in->y, in->z, in->px,
+                                                            in->py, in->pz, in->q, in->q_scalar, NULL, p->tx, p->ty, p->tz, p->w0, p->w1,
+                                                            p->w2, p->w3, p->pmx, p->pmy, p->pmz);
+    FMM_LAUNCH_CHECK(c, "permute_particles");
+    return tree_boxes(p);
 }

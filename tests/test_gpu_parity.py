@@ -252,3 +252,40 @@ def test_fmm_source_momentum_matches_serial_oracle(fmm, case):
     assert_close(E, Eo, "FMM E (source momentum)")
     assert_close(B, Bo, "FMM B (source momentum)")
     plan.close()
+
+
+# ---------------------------------------------------------------------------------------------
+# fmm_plan_refit: the particle order of the last build is kept
+# ---------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("sm", [False, True], ids=["mean_gamma", "source_momentum"])
+def test_refit_matches_oracle_over_the_same_order(fmm, sm):
+    w = workloads.config(2, N=20011)
+    flags = fmm.FMM_TREE_KD | (fmm.FMM_KERNEL_SOURCE_MOMENTUM if sm else 0)
+    plan = fmm.fmm_plan_create(*w.arrays(), w.q, order_n=4, leaf_size=128, theta=0.5, flags=flags)
+    perm0 = plan.export()["perm"].copy()
+    rng = np.random.default_rng(17)
+    x2 = w.x + 3e-5 * rng.standard_normal(w.N)
+    y2 = w.y + 3e-5 * rng.standard_normal(w.N)
+    z2 = w.z + 3e-6 * rng.standard_normal(w.N)
+    pz2 = w.pz * (1.0 + 1e-3 * rng.standard_normal(w.N))
+    args = (x2, y2, z2, w.px, w.py, pz2)
+    plan.refit(*args, w.q)
+    st = plan.stats()
+    ex = plan.export()
+    assert np.array_equal(ex["perm"], perm0), "refit must keep the particle order"
+    op = oracle.Plan(*args, w.q, order_n=4, leaf_size=128, theta=0.5, gamma_bar_value=st["gamma_bar"], given_order=perm0,
+                     source_momentum=sm)
+    assert abs(st["gamma_bar"] - oracle.gamma_bar(w.px, w.py, pz2)) <= 1e-13 * st["gamma_bar"]
+    lo, hi, bb = op.node_arrays()
+    assert np.array_equal(ex["bbox"].view(np.uint64), bb.view(np.uint64)), "bounding boxes differ"
+    p2p, m2l = op.lists()
+    assert np.array_equal(ex["p2p_src"], p2p[:, 1]) and np.array_equal(ex["m2l_src"], m2l[:, 1])
+    E, B = to_np(plan.eval())
+    Eo, Bo = op.eval()
+    assert_close(E, Eo, "refit E")
+    assert_close(B, Bo, "refit B")
+    # a full update afterwards re-sorts: back to the KD tree of the new positions
+    plan.update(*args, w.q)
+    ok = oracle.Plan(*args, w.q, order_n=4, leaf_size=128, theta=0.5, gamma_bar_value=plan.stats()["gamma_bar"], source_momentum=sm)
+    assert np.array_equal(plan.export()["perm"], ok.perm())
+    plan.close()
