@@ -125,7 +125,6 @@ static int plan_alloc_fixed(fmm_plan *p)
     ALLOC(p2p_off, int32_t, nodes1 + 1); ALLOC(m2l_off, int32_t, nodes1 + 1);
     ALLOC(p2p_order, int32_t, nodes1); ALLOC(m2l_order, int32_t, nodes1);
     ALLOC(M, double, 4 * (size_t)p->P * nodes1);
-    ALLOC(MZ, double, 4 * (size_t)p->P * nodes1);
     ALLOC(L, double, 6 * (size_t)p->P * nodes1);
     ALLOC(near_, double, 6 * N);
 #undef ALLOC

@@ -78,7 +78,6 @@ struct fmm_plan {
     // expansions
     double *M;              // [nodes+1][P][4]
     double *L;              // [nodes+1][P][6]
-    double *MZ;             // [nodes+1][P][4] (m0, m1, m2, 0) x relative z proxy coordinate, filled by pairs_m2l
     double *near_;          // [6][N] tree order, P2P result
     // timing
     int timing;

@@ -315,8 +315,8 @@ struct m2l_cfg {
 #define M2L_MINB 2
 #endif
     static constexpr int MINB = (THREADS + 32 <= 400) ? M2L_MINB : 1;
-    // pipeline depth: as many stages of (M tile + MZ tile + proxy coordinates) as fit 227 KB, at most 3
-    static constexpr int STAGE_BYTES = 64 * P + 3 * 16 * 8;
+    // pipeline depth: as many stages of (M tile + proxy coordinates) as fit 227 KB, at most 3
+    static constexpr int STAGE_BYTES = 32 * P + 3 * 16 * 8;
     static constexpr int FIT = (227 * 1024 - 64) / STAGE_BYTES;
     static constexpr int STAGES = FIT >= 3 ? 3 : (FIT >= 2 ? 2 : 1);
 };
@@ -364,9 +364,12 @@ __device__ __forceinline__ void mbar_arrive(uint64_t *bar)
 // Per-node tables for M2L, filled once per evaluation:
 //   xi[node][g][k]  proxy points per axis (reading I-3), row stride M2L_XI_STRIDE.  Row 2 (z) holds the points
 //                   RELATIVE to the box centre z0 = (a_z + b_z)/2, and z0 itself sits in xi[node][2][15].
-//   MZ[node][nu][4] = (m0, m1, m2, 0) * zrel_{nu3}: with it  sum_nu m_k w dz = (zt - z0) sum_nu m_k w - sum_nu MZ_k w,
-//                   so the innermost loop needs no dz and all of its accumulate-FMAs share the operand w.
+//                   xi[node][2][14] = h_z = (b_z - a_z)/2, so that zrel_k = h_z c_k up to one rounding of the proxy point.
+// With z relative to the source box centre,  sum_nu m_k w dz = (zt - z0) sum_nu m_k w - h_z sum_nu m_k (c_{nu3} w):
+// the innermost loop needs no dz array; the Chebyshev points c_k are compile-time-indexed constant-bank operands
+// (m2l_cheb_c), so the extra product u = c_k w costs no register and vanishes for c_k = +-1 and 0.
 #define M2L_XI_STRIDE 16
+__constant__ double m2l_cheb_c[FMM_MAX_ORDER + 2][M2L_XI_STRIDE];  // [n1][k] = cos(k pi / (n1 - 1)) (reading I-1)
 #define M2L_XI_BYTES (3 * M2L_XI_STRIDE * 8)
 __global__ void m2l_proxy_points(int nodes, int n1, cheb13 ch, const double *__restrict__ bbox, double *__restrict__ xi)
 {
@@ -382,23 +385,11 @@ __global__ void m2l_proxy_points(int nodes, int n1, cheb13 ch, const double *__r
             if (g == 2) v = __dsub_rn(v, mid);
         } else if (g == 2 && k == M2L_XI_STRIDE - 1) {
             v = mid;
+        } else if (g == 2 && k == M2L_XI_STRIDE - 2) {
+            v = __dmul_rn(__dsub_rn(bs[3 + g], bs[g]), 0.5);
         }
     }
     xi[q] = v;
-}
-
-__global__ void m2l_moment_z(int64_t count, int P, int n1, const double *__restrict__ xi, const double *__restrict__ M, double *__restrict__ MZ)
-{
-    int64_t q = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;  // (node, nu)
-    if (q >= count) return;
-    int64_t node = q / P;
-    int nu = (int)(q - node * P);
-    const double zr = xi[(size_t)node * 3 * M2L_XI_STRIDE + 2 * M2L_XI_STRIDE + nu % n1];
-    const double2 *m = reinterpret_cast<const double2 *>(M + 4 * q);
-    double2 m01 = m[0], m23 = m[1];
-    double2 *o = reinterpret_cast<double2 *>(MZ + 4 * q);
-    o[0] = make_double2(m01.x * zr, m01.y * zr);
-    o[1] = make_double2(m23.x * zr, 0.0);
 }
 
 // Shared memory of one block: m2l_cfg::STAGES stages, each = the source node's moments (P x 4 doubles, one contiguous
@@ -409,15 +400,14 @@ __global__ void m2l_moment_z(int64_t count, int P, int n1, const double *__restr
 template <int N1>
 __global__ void __launch_bounds__(m2l_cfg<N1>::THREADS + 32, m2l_cfg<N1>::MINB) m2l_kernel(double g2, const int32_t *__restrict__ order,
                                                                                       const int32_t *__restrict__ off, const int32_t *__restrict__ src,
-                                                                                      const double *__restrict__ xi, const double *__restrict__ M,
-                                                                                      const double *__restrict__ MZ, double *__restrict__ L)
+                                                                                      const double *__restrict__ xi, const double *__restrict__ M, double *__restrict__ L)
 {
     constexpr int P = m2l_cfg<N1>::P;
     constexpr int THREADS = m2l_cfg<N1>::THREADS;
     constexpr int WARPS = THREADS / 32;
     constexpr int S = m2l_cfg<N1>::STAGES;
     constexpr uint32_t TILE_BYTES = 32u * P;
-    constexpr uint32_t STAGE_BYTES = 2 * TILE_BYTES + M2L_XI_BYTES;
+    constexpr uint32_t STAGE_BYTES = TILE_BYTES + M2L_XI_BYTES;
     extern __shared__ __align__(128) unsigned char m2l_smem_raw[];
     uint64_t *full = reinterpret_cast<uint64_t *>(m2l_smem_raw + S * STAGE_BYTES);
     uint64_t *empty = full + S;
@@ -444,8 +434,7 @@ __global__ void __launch_bounds__(m2l_cfg<N1>::THREADS + 32, m2l_cfg<N1>::MINB) 
         unsigned char *dst = m2l_smem_raw + (size_t)st * STAGE_BYTES;
         mbar_expect_tx(&full[st], STAGE_BYTES);
         bulk_g2s(dst, M + 4 * (size_t)P * sn, TILE_BYTES, &full[st]);
-        bulk_g2s(dst + TILE_BYTES, MZ + 4 * (size_t)P * sn, TILE_BYTES, &full[st]);
-        bulk_g2s(dst + 2 * TILE_BYTES, xi + (size_t)sn * 3 * M2L_XI_STRIDE, M2L_XI_BYTES, &full[st]);
+        bulk_g2s(dst + TILE_BYTES, xi + (size_t)sn * 3 * M2L_XI_STRIDE, M2L_XI_BYTES, &full[st]);
     };
     if (threadIdx.x >= THREADS) {  // producer warp: one lane keeps the stages filled, then the warp retires
         if (threadIdx.x == THREADS)
@@ -461,7 +450,6 @@ __global__ void __launch_bounds__(m2l_cfg<N1>::THREADS + 32, m2l_cfg<N1>::MINB) 
     for (int mu0 = 0; mu0 < P; mu0 += NT * THREADS) {
         // the thread's NT target proxy points; z = centre + relative part, as the oracle's xi (mid + half c_k)
         double xt[NT], yt[NT], zt[NT], ex[NT], ey[NT], ez[NT], bx[NT], by[NT], bz[NT];
-        double S0[NT], S1[NT], S2[NT];  // sum over all sources of MZ_k w (subtracted once, after the last source)
 #pragma unroll
         for (int k = 0; k < NT; ++k) {
             const int mu = mu0 + k * THREADS + threadIdx.x;
@@ -470,15 +458,15 @@ __global__ void __launch_bounds__(m2l_cfg<N1>::THREADS + 32, m2l_cfg<N1>::MINB) 
             xt[k] = xt3[a];
             yt[k] = xt3[M2L_XI_STRIDE + b];
             zt[k] = __dadd_rn(xt3[2 * M2L_XI_STRIDE + M2L_XI_STRIDE - 1], xt3[2 * M2L_XI_STRIDE + c3]);
-            ex[k] = ey[k] = ez[k] = bx[k] = by[k] = bz[k] = S0[k] = S1[k] = S2[k] = 0.0;
+            ex[k] = ey[k] = ez[k] = bx[k] = by[k] = bz[k] = 0.0;
         }
         for (int e = 0; e < ne; ++e, ++i) {
             const int st = i % S;
             mbar_wait(&full[st], (uint32_t)((i / S) & 1));
             const double2 *Ms = reinterpret_cast<const double2 *>(m2l_smem_raw + (size_t)st * STAGE_BYTES);
-            const double2 *Zs = reinterpret_cast<const double2 *>(m2l_smem_raw + (size_t)st * STAGE_BYTES + TILE_BYTES);
-            const double *xs = reinterpret_cast<const double *>(m2l_smem_raw + (size_t)st * STAGE_BYTES + 2 * TILE_BYTES);
+            const double *xs = reinterpret_cast<const double *>(m2l_smem_raw + (size_t)st * STAGE_BYTES + TILE_BYTES);
             double ztr[NT], gz2[NT][N1];
+            double S0[NT], S1[NT], S2[NT];  // sum over this source of m_k (c_{nu3} w)
 #pragma unroll
             for (int k = 0; k < NT; ++k) {
                 ztr[k] = zt[k] - xs[2 * M2L_XI_STRIDE + M2L_XI_STRIDE - 1];  // target z relative to the source box centre
@@ -487,6 +475,7 @@ __global__ void __launch_bounds__(m2l_cfg<N1>::THREADS + 32, m2l_cfg<N1>::MINB) 
                     const double dz = ztr[k] - xs[2 * M2L_XI_STRIDE + c];
                     gz2[k][c] = (g2 * dz) * dz;
                 }
+                S0[k] = S1[k] = S2[k] = 0.0;
             }
             for (int a2 = 0; a2 < N1; ++a2) {
                 double dx[NT], dx2[NT];
@@ -498,7 +487,6 @@ __global__ void __launch_bounds__(m2l_cfg<N1>::THREADS + 32, m2l_cfg<N1>::MINB) 
 #pragma unroll 1
                 for (int b2 = 0; b2 < N1; ++b2) {
                     const double2 *row = Ms + 2 * ((a2 * N1 + b2) * N1);
-                    const double2 *rowz = Zs + 2 * ((a2 * N1 + b2) * N1);
                     double dy[NT], s2[NT], A0[NT], A1[NT], A2[NT], A3[NT];
 #pragma unroll
                     for (int k = 0; k < NT; ++k) {
@@ -509,8 +497,6 @@ __global__ void __launch_bounds__(m2l_cfg<N1>::THREADS + 32, m2l_cfg<N1>::MINB) 
 #pragma unroll
                     for (int c2 = 0; c2 < N1; ++c2) {
                         const double2 m01 = row[2 * c2], m23 = row[2 * c2 + 1];
-                        const double2 z01 = rowz[2 * c2];
-                        const double z2 = rowz[2 * c2 + 1].x;
 #pragma unroll
                         for (int k = 0; k < NT; ++k) {
                             const double w = inv_r3(s2[k] + gz2[k][c2]);
@@ -518,14 +504,17 @@ __global__ void __launch_bounds__(m2l_cfg<N1>::THREADS + 32, m2l_cfg<N1>::MINB) 
                             A1[k] = fma(m01.y, w, A1[k]);
                             A2[k] = fma(m23.x, w, A2[k]);
                             A3[k] = fma(m23.y, w, A3[k]);
-                            S0[k] = fma(z01.x, w, S0[k]);
-                            S1[k] = fma(z01.y, w, S1[k]);
-                            S2[k] = fma(z2, w, S2[k]);
+                            if (c2 == 0 || c2 == N1 - 1 || 2 * c2 != N1 - 1) {  // c_k = 0 at the middle point of an even order
+                                const double u = (c2 == 0) ? w : (c2 == N1 - 1) ? -w : w * m2l_cheb_c[N1][c2];
+                                S0[k] = fma(m01.x, u, S0[k]);
+                                S1[k] = fma(m01.y, u, S1[k]);
+                                S2[k] = fma(m23.x, u, S2[k]);
+                            }
                         }
                     }
 #pragma unroll
                     for (int k = 0; k < NT; ++k) {
-                        // sum m_k w dz = ztr sum m_k w - sum MZ_k w:  E_z += Z0,  B_x += Z2,  B_y -= Z1
+                        // sum m_k w dz = ztr sum m_k w - h_z sum m_k c w:  E_z += Z0,  B_x += Z2,  B_y -= Z1
                         ex[k] = fma(A0[k], dx[k], ex[k]);
                         ey[k] = fma(A0[k], dy[k], ey[k]);
                         ez[k] = fma(A0[k], ztr[k], ez[k]);
@@ -533,6 +522,15 @@ __global__ void __launch_bounds__(m2l_cfg<N1>::THREADS + 32, m2l_cfg<N1>::MINB) 
                         by[k] = fma(A3[k], dx[k], fma(-A1[k], ztr[k], by[k]));
                         bz[k] = fma(A1[k], dy[k], fma(-A2[k], dx[k], bz[k]));
                     }
+                }
+            }
+            {
+                const double hz = xs[2 * M2L_XI_STRIDE + M2L_XI_STRIDE - 2];
+#pragma unroll
+                for (int k = 0; k < NT; ++k) {
+                    ez[k] = fma(-hz, S0[k], ez[k]);
+                    bx[k] = fma(-hz, S2[k], bx[k]);
+                    by[k] = fma(hz, S1[k], by[k]);
                 }
             }
             __syncwarp();
@@ -543,7 +541,7 @@ __global__ void __launch_bounds__(m2l_cfg<N1>::THREADS + 32, m2l_cfg<N1>::MINB) 
             const int mu = mu0 + k * THREADS + threadIdx.x;
             if (mu < P) {
                 double *o = Lt + 6 * (size_t)mu;
-                o[0] = ex[k]; o[1] = ey[k]; o[2] = ez[k] - S0[k]; o[3] = bx[k] - S2[k]; o[4] = by[k] + S1[k]; o[5] = bz[k];
+                o[0] = ex[k]; o[1] = ey[k]; o[2] = ez[k]; o[3] = bx[k]; o[4] = by[k]; o[5] = bz[k];
             }
         }
     }
@@ -553,19 +551,37 @@ template <int N1>
 static int launch_m2l(fmm_plan *p)
 {
     fmm_ctx *c = &p->ctx;
-    const size_t smem = m2l_cfg<N1>::STAGES * ((size_t)64 * m2l_cfg<N1>::P + M2L_XI_BYTES) + 2 * m2l_cfg<N1>::STAGES * sizeof(uint64_t);
+    const size_t smem = m2l_cfg<N1>::STAGES * ((size_t)32 * m2l_cfg<N1>::P + M2L_XI_BYTES) + 2 * m2l_cfg<N1>::STAGES * sizeof(uint64_t);
     if (smem > 48 * 1024)
         FMM_CUDA(c, cudaFuncSetAttribute((const void *)m2l_kernel<N1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     // the default carveout leaves room for one block only; ask for enough shared memory for every resident block
     FMM_CUDA(c, cudaFuncSetAttribute((const void *)m2l_kernel<N1>, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared));
     m2l_kernel<N1><<<(unsigned)p->nodes, m2l_cfg<N1>::THREADS + 32, smem, c->stream>>>(p->gamma_bar * p->gamma_bar, p->m2l_order, p->m2l_off,
-                                                                               p->m2l_src, p->node_xi, p->M, p->MZ, p->L);
+                                                                               p->m2l_src, p->node_xi, p->M, p->L);
     FMM_LAUNCH_CHECK(c, "m2l_kernel");
+    return FMM_OK;
+}
+
+static int m2l_upload_cheb(fmm_ctx *c)
+{
+    static std::atomic<int> done{0};
+    if (done.load(std::memory_order_acquire)) return FMM_OK;
+    double tab[FMM_MAX_ORDER + 2][M2L_XI_STRIDE];
+    memset(tab, 0, sizeof(tab));
+    for (int n1 = 2; n1 <= FMM_MAX_ORDER + 1; ++n1) {
+        const int n = n1 - 1;
+        for (int k = 0; k <= n; ++k) tab[n1][k] = sin(FMM_PI * (double)(n - 2 * k) / (double)(2 * n));  // I-1
+        tab[n1][0] = 1.0;
+        tab[n1][n] = -1.0;
+    }
+    FMM_CUDA(c, cudaMemcpyToSymbol(m2l_cheb_c, tab, sizeof(tab)));  // identical bytes from every caller
+    done.store(1, std::memory_order_release);
     return FMM_OK;
 }
 
 int pairs_m2l(fmm_plan *p)
 {
+    FMM_TRY(m2l_upload_cheb(&p->ctx));
     cheb13 ch;
     memset(&ch, 0, sizeof(ch));
     for (int k = 0; k <= p->n; ++k) ch.c[k] = sin(FMM_PI * (double)(p->n - 2 * k) / (double)(2 * p->n));  // I-1
@@ -576,9 +592,6 @@ int pairs_m2l(fmm_plan *p)
         int count = (int)(p->nodes + 1) * 3 * M2L_XI_STRIDE;
         m2l_proxy_points<<<(count + 255) / 256, 256, 0, c->stream>>>((int)p->nodes, p->n1, ch, p->bbox, p->node_xi);
         FMM_LAUNCH_CHECK(c, "m2l_proxy_points");
-        int64_t cnt = (p->nodes + 1) * (int64_t)p->P;
-        m2l_moment_z<<<(unsigned)((cnt + 255) / 256), 256, 0, c->stream>>>(cnt, p->P, p->n1, p->node_xi, p->M, p->MZ);
-        FMM_LAUNCH_CHECK(c, "m2l_moment_z");
     }
     switch (p->n1) {
         case 2: return launch_m2l<2>(p);
