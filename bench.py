@@ -30,6 +30,7 @@ if ROOT not in sys.path:
 
 from paper_2302_07567_b200 import workloads  # noqa: E402
 
+STAGE_KEYS = ("ms_tree", "ms_lists", "ms_p2m", "ms_m2m", "ms_m2l", "ms_l2l", "ms_p2p", "ms_l2p")
 METRIC = "fmm_E+B_particles_per_s"
 UNIT = "particles/s"
 FLOP_PER_EVAL = 34          # algorithmic flop per kernel evaluation (fma = 2, rsqrt = 1)
@@ -47,6 +48,7 @@ def parse_args():
     ap.add_argument("--tree", default="kd", choices=["kd", "morton"])
     ap.add_argument("--kernel", default="mean_gamma", choices=["mean_gamma", "source_momentum"],
                     help="near-field kernel: eq. (3.2) with gamma_bar (default) or the G6 alternative (SURVEY 8(f) rank 2)")
+    ap.add_argument("--no-overlap", action="store_true", help="run P2P after L2L on one stream instead of beside the far-field chain")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cpu-sample-leaves", type=int, default=2048,
                     help="target leaves the oracle evaluates in the cpu_baseline leg (the reference arm uses 1/8 of it per step)")
@@ -235,7 +237,9 @@ def run_cuda(args):
     prm = dict(order_n=w.order_n, leaf_size=w.leaf_size, theta=w.theta, flags=flags, device=dev)
 
     plan = fmm.fmm_plan_create(*d_in, w.q, **prm)
-    plan.set_timing(True)
+    overlap = not args.no_overlap
+    plan.set_overlap(overlap)
+    plan.set_timing(not overlap)   # per-stage events force the serial order: with overlap they are taken in a second pass
 
     def step():
         plan.update(*d_in, w.q)     # a0-a3
@@ -254,10 +258,28 @@ def run_cuda(args):
             step()
             ev[k][1].record()
             st = plan.stats()
-            for key in ("ms_tree", "ms_lists", "ms_p2m", "ms_m2m", "ms_m2l", "ms_l2l", "ms_p2p", "ms_l2p"):
-                stage_ms.setdefault(key, []).append(st[key])
+            if not overlap:
+                for key in STAGE_KEYS:
+                    stage_ms.setdefault(key, []).append(st[key])
         barrier()
-    launches = fmm.fmm_launch_count() - l0
+        launches = fmm.fmm_launch_count() - l0
+        ms_serial = None
+        if overlap:
+            # stage pass: the same K steps again, stages in serial order with CUDA events around every kernel group
+            # (fmm_plan_set_timing); these are the per-kernel durations the roofline object uses
+            plan.set_timing(True)
+            sev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+            for k in range(args.steps):
+                flush.fill_(k & 0xff)
+                sev[k][0].record()
+                step()
+                sev[k][1].record()
+                st = plan.stats()
+                for key in STAGE_KEYS:
+                    stage_ms.setdefault(key, []).append(st[key])
+            barrier()
+            ms_serial = sum(a.elapsed_time(b) for a, b in sev) / args.steps
+            plan.set_timing(False)
     ms_total = max_over_ranks(sum(a.elapsed_time(b) for a, b in ev), world, dev)
     value = aggregate_throughput(world, w.N, args.steps, ms_total)
     clocks = clk.summary()
@@ -310,6 +332,9 @@ def run_cuda(args):
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": 6 * 8 * w.N, "d2h_bytes_per_step": 6 * 8 * w.N},
             "gpu_launches": int(launches), "clocks": clocks, "roofline": roofline,
             "stages_ms": {k: round(v, 4) for k, v in stages.items()},
+            "stage_timing": ("per-stage CUDA events of a second pass of the same K steps in serial stage order "
+                             f"({ms_serial:.3f} ms/step); the timed region runs P2P on a second stream beside P2M/M2M/M2L/L2L"
+                             if ms_serial is not None else "per-stage CUDA events inside the timed region (serial stage order)"),
             "lists": {"n_p2p": st["n_p2p"], "n_m2l": st["n_m2l"], "kappa": st["kappa"], "gamma_bar": st["gamma_bar"]},
             "hbm_peak_gbs": hbm, "parallelism": "replicas only" if world > 1 else "single GPU"}
     if world == 1 and not args.no_cpu_baseline:

@@ -64,7 +64,7 @@ class fmm_export_t(C.Structure):
 
 
 EXPORTED_SYMBOLS = ["fmm_plan_create", "fmm_plan_update", "fmm_plan_refit", "fmm_eval", "fmm_direct", "fmm_field_host",
-                    "fmm_plan_set_timing", "fmm_plan_stats", "fmm_plan_export", "fmm_plan_destroy",
+                    "fmm_plan_set_timing", "fmm_plan_set_overlap", "fmm_plan_stats", "fmm_plan_export", "fmm_plan_destroy",
                     "fmm_launch_count", "fmm_probe_fp64_peak", "fmm_strerror", "fmm_last_error", "fmm_version"]
 
 _lib = None
@@ -101,6 +101,8 @@ def load_library():
                                   [C.POINTER(fmm_stats_t), ALLOC_FN, FREE_FN, vp, vp]
     lib.fmm_plan_set_timing.restype = C.c_int
     lib.fmm_plan_set_timing.argtypes = [vp, C.c_int]
+    lib.fmm_plan_set_overlap.restype = C.c_int
+    lib.fmm_plan_set_overlap.argtypes = [vp, C.c_int]
     lib.fmm_plan_stats.restype = C.c_int
     lib.fmm_plan_stats.argtypes = [vp, C.POINTER(fmm_stats_t)]
     lib.fmm_plan_export.restype = C.c_int
@@ -208,6 +210,9 @@ class Plan:
 
     def export(self, want_M=False, want_L=False) -> dict:
         return fmm_plan_export(self, want_M, want_L)
+
+    def set_overlap(self, on=True):
+        _check(load_library().fmm_plan_set_overlap(self._h, int(bool(on))), self._h)
 
     def set_timing(self, on=True):
         _check(load_library().fmm_plan_set_timing(self._h, int(bool(on))), self._h)

@@ -77,6 +77,27 @@ void ctx_free_all(fmm_ctx *c)
     while (!c->owned.empty()) ctx_free(c, c->owned.back());
 }
 
+// One side stream per device for the near / far overlap, created on first use and kept for the life of the process
+// (creating a stream costs about a millisecond, too much for fmm_field_host, which builds a plan per call).  Plans that
+// share it are still ordered correctly: every fmm_eval forks from and joins into its own stream with events.
+#include <mutex>
+static cudaError_t side_stream_for_current_device(cudaStream_t *out)
+{
+    static std::mutex mu;
+    static cudaStream_t streams[64] = {};
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    if (dev < 0 || dev >= 64) return cudaErrorInvalidDevice;
+    std::lock_guard<std::mutex> lock(mu);
+    if (!streams[dev]) {
+        e = cudaStreamCreateWithFlags(&streams[dev], cudaStreamNonBlocking);
+        if (e != cudaSuccess) return e;
+    }
+    *out = streams[dev];
+    return cudaSuccess;
+}
+
 static int check_particles(const fmm_particles_t *in)
 {
     if (!in || in->N < 1 || in->N >= ((int64_t)1 << 31)) return FMM_EINVAL;
@@ -161,6 +182,8 @@ extern "C" void fmm_plan_destroy(fmm_plan_t *p)
         if (p->ev[k]) cudaEventDestroy(p->ev[k]);
     for (int k = 0; k < 3; ++k)
         if (p->ev_plan[k]) cudaEventDestroy(p->ev_plan[k]);
+    if (p->ev_fork) cudaEventDestroy(p->ev_fork);
+    if (p->ev_join) cudaEventDestroy(p->ev_join);
     delete p;
 }
 
@@ -195,6 +218,11 @@ extern "C" int fmm_plan_create(fmm_plan_t **out, const fmm_particles_t *in, cons
         if (cudaEventCreate(&p->ev[k]) != cudaSuccess) rc = FMM_ECUDA;
     for (int k = 0; k < 3 && rc == FMM_OK; ++k)
         if (cudaEventCreate(&p->ev_plan[k]) != cudaSuccess) rc = FMM_ECUDA;
+    if (rc == FMM_OK && (side_stream_for_current_device(&p->side) != cudaSuccess ||
+                         cudaEventCreateWithFlags(&p->ev_fork, cudaEventDisableTiming) != cudaSuccess ||
+                         cudaEventCreateWithFlags(&p->ev_join, cudaEventDisableTiming) != cudaSuccess))
+        rc = FMM_ECUDA;
+    p->overlap = 1;
     if (rc == FMM_OK) rc = plan_alloc_fixed(p);
     if (rc == FMM_OK) rc = plan_build(p, in);
     if (rc != FMM_OK) {
@@ -218,6 +246,13 @@ extern "C" int fmm_plan_refit(fmm_plan_t *p, const fmm_particles_t *in)
     return plan_build(p, in, true);
 }
 
+extern "C" int fmm_plan_set_overlap(fmm_plan_t *p, int on)
+{
+    if (!p) return FMM_EINVAL;
+    p->overlap = on ? 1 : 0;
+    return FMM_OK;
+}
+
 extern "C" int fmm_plan_set_timing(fmm_plan_t *p, int on)
 {
     if (!p) return FMM_EINVAL;
@@ -237,6 +272,26 @@ extern "C" int fmm_plan_set_timing(fmm_plan_t *p, int on)
 extern "C" int fmm_eval(fmm_plan_t *p, double *Ex, double *Ey, double *Ez, double *Bx, double *By, double *Bz)
 {
     if (!p || !Ex || !Ey || !Ez || !Bx || !By || !Bz) return FMM_EINVAL;
+    if (p->overlap && !p->timing) {
+        // a7 does not depend on a4-a6/a8: it runs on the side stream, forked after everything already enqueued on the
+        // caller's stream and joined before L2P adds near + far.  Results are identical (each kernel is deterministic).
+        fmm_ctx *c = &p->ctx;
+        cudaStream_t main_stream = c->stream;
+        FMM_CUDA(c, cudaEventRecord(p->ev_fork, main_stream));
+        FMM_CUDA(c, cudaStreamWaitEvent(p->side, p->ev_fork, 0));
+        FMM_TRY(interp_p2m(p));
+        FMM_TRY(interp_m2m(p));
+        FMM_TRY(pairs_m2l(p));
+        c->stream = p->side;
+        int rc = pairs_p2p(p);
+        c->stream = main_stream;
+        FMM_TRY(rc);
+        FMM_CUDA(c, cudaEventRecord(p->ev_join, p->side));
+        FMM_TRY(interp_l2l(p));
+        FMM_CUDA(c, cudaStreamWaitEvent(main_stream, p->ev_join, 0));
+        FMM_TRY(interp_l2p_finalize(p, Ex, Ey, Ez, Bx, By, Bz));
+        return FMM_OK;
+    }
     MARK(p, EV_P2M);
     FMM_TRY(interp_p2m(p));          // Alg 5.3 at the leaves
     MARK(p, EV_M2M);

@@ -83,6 +83,10 @@ struct fmm_plan {
     int timing;
     cudaEvent_t ev[EV_COUNT];
     cudaEvent_t ev_plan[3];
+    // near / far overlap: P2P runs on `side` while the upward pass, M2L and L2L run on the caller's stream
+    cudaStream_t side;
+    cudaEvent_t ev_fork, ev_join;
+    int overlap;
     int ev_valid;
     float ms_tree, ms_lists;
 };

@@ -533,6 +533,10 @@ __global__ void __launch_bounds__(m2l_cfg<N1>::THREADS + 32, m2l_cfg<N1>::MINB) 
                     by[k] = fma(hz, S1[k], by[k]);
                 }
             }
+            // The stage is about to be overwritten by a bulk TMA copy (async proxy): order this thread's generic-proxy
+            // reads of it before the release.  Without this fence a warp occasionally (about 1 evaluation in 10 when P2P
+            // runs beside M2L) saw part of the NEXT source's tile: a cross-proxy write-after-read hazard.
+            asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
             __syncwarp();
             if ((threadIdx.x & 31) == 0) mbar_arrive(&empty[st]);
         }

@@ -289,3 +289,21 @@ def test_refit_matches_oracle_over_the_same_order(fmm, sm):
     ok = oracle.Plan(*args, w.q, order_n=4, leaf_size=128, theta=0.5, gamma_bar_value=plan.stats()["gamma_bar"], source_momentum=sm)
     assert np.array_equal(plan.export()["perm"], ok.perm())
     plan.close()
+
+
+def test_overlap_is_bit_identical_to_serial_and_stable(fmm):
+    """fmm_plan_set_overlap: P2P on the plan's side stream beside P2M/M2M/M2L/L2L.  Regression for a cross-proxy
+    write-after-read hazard in the M2L source ring (generic reads of a stage vs. the next bulk-TMA copy into it) that
+    only showed with concurrent kernels: 25 evaluations in each mode must be bit-identical."""
+    import torch
+    w = workloads.config(3, N=30000)
+    plan = fmm.fmm_plan_create(*w.arrays(), w.q, order_n=3, leaf_size=100, theta=0.4)
+    plan.set_overlap(False)
+    E0, B0 = plan.eval()
+    E0, B0 = E0.clone(), B0.clone()
+    for ov in (True, False, True):
+        plan.set_overlap(ov)
+        for _ in range(25):
+            E, B = plan.eval()
+            assert torch.equal(E, E0) and torch.equal(B, B0), f"overlap={ov}: result changed between evaluations"
+    plan.close()
