@@ -173,28 +173,100 @@ __global__ void kd_mark_left(int N, int level, const int8_t *__restrict__ axis, 
     left[part] = (i < mid) ? 1 : 0;
 }
 
-__global__ void kd_gather_flags(int N, const uint8_t *__restrict__ left, const uint32_t *__restrict__ lists /* [4][N] */,
-                                int32_t *__restrict__ f /* [4N] */)
+// Number of "left" flags inside a subtree of `s` members that is `r` levels above the level being split: after r
+// balanced halvings (T-2) the parts have q+1 (m of them) or q members, q = s >> r, m = s - (q << r); a part of size
+// c sends ceil(c/2) members left.
+__host__ __device__ __forceinline__ int kd_lefts(int s, int r)
 {
-    int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= 4ll * N) return;
-    f[i] = left[lists[i]];
+    int q = s >> r, m = s - (q << r);
+    return m * ((q + 2) >> 1) + ((1 << r) - m) * ((q + 1) >> 1);
 }
 
-// stable partition of every node segment of the four lists: left members first
-__global__ void kd_partition(int N, int level, const uint8_t *__restrict__ left, const int32_t *__restrict__ scan /* [4N] */,
-                             const uint32_t *__restrict__ lists, uint32_t *__restrict__ out)
+// position i of a list -> its node [lo, hi) at `level` and the number of left flags in the nodes before it
+__device__ __forceinline__ void kd_node_of(int N, int level, int i, int &lo, int &hi, int &lefts_before)
 {
-    int64_t g = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (g >= 4ll * N) return;
-    int li = (int)(g / N), i = (int)(g - (int64_t)li * N);
-    int node, lo, hi;
-    node_at_level(N, level, i, node, lo, hi);
-    int mid = lo + (hi - lo + 1) / 2;
-    uint32_t part = lists[g];
-    int nleft_before = scan[g] - scan[(int64_t)li * N + lo];
-    int dest = left[part] ? (lo + nleft_before) : (mid + (i - lo - nleft_before));
-    out[(int64_t)li * N + dest] = part;
+    lo = 0;
+    hi = N;
+    lefts_before = 0;
+    for (int l = 0; l < level; ++l) {
+        int mid = lo + (hi - lo + 1) / 2;
+        if (i < mid) {
+            hi = mid;
+        } else {
+            lefts_before += kd_lefts(mid - lo, level - l - 1);
+            lo = mid;
+        }
+    }
+}
+
+#define KD_TILE_ITEMS 8
+#define KD_TILE (256 * KD_TILE_ITEMS)
+
+// left flags of the four lists, counted per tile of KD_TILE consecutive entries (no flag array is stored)
+__global__ void __launch_bounds__(256) kd_tile_counts(int64_t n4, const uint8_t *__restrict__ left, const uint32_t *__restrict__ lists,
+                                                      int32_t *__restrict__ sums)
+{
+    __shared__ int sm[8];
+    int64_t base = (int64_t)blockIdx.x * KD_TILE + (int64_t)threadIdx.x * KD_TILE_ITEMS;
+    int s = 0;
+#pragma unroll
+    for (int k = 0; k < KD_TILE_ITEMS; ++k)
+        if (base + k < n4) s += left[lists[base + k]];
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) s += __shfl_down_sync(0xffffffffu, s, o);
+    if ((threadIdx.x & 31) == 0) sm[threadIdx.x >> 5] = s;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        int t = 0;
+        for (int k = 0; k < 8; ++k) t += sm[k];
+        sums[blockIdx.x] = t;
+    }
+}
+
+// stable partition of every node segment of the four lists: left members first.  The number of left flags before
+// entry g is tile_base[tile] + the scan inside the tile; the number before the node's start is closed-form (kd_lefts).
+__global__ void __launch_bounds__(256) kd_partition(int N, int level, const uint8_t *__restrict__ left, const int32_t *__restrict__ tile_base,
+                                                    const uint32_t *__restrict__ lists, uint32_t *__restrict__ out)
+{
+    __shared__ int sm[8];
+    const int64_t n4 = 4ll * N;
+    const int64_t base = (int64_t)blockIdx.x * KD_TILE + (int64_t)threadIdx.x * KD_TILE_ITEMS;
+    uint32_t part[KD_TILE_ITEMS];
+    int flag[KD_TILE_ITEMS], s = 0;
+#pragma unroll
+    for (int k = 0; k < KD_TILE_ITEMS; ++k) {
+        part[k] = (base + k < n4) ? lists[base + k] : 0u;
+        flag[k] = (base + k < n4) ? (int)left[part[k]] : 0;
+        s += flag[k];
+    }
+    // exclusive scan of s over the block
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    int inc = s;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        int t = __shfl_up_sync(0xffffffffu, inc, o);
+        if (lane >= o) inc += t;
+    }
+    if (lane == 31) sm[warp] = inc;
+    __syncthreads();
+    int wbase = 0;
+    for (int k = 0; k < warp; ++k) wbase += sm[k];
+    int before = tile_base[blockIdx.x] + wbase + inc - s;  // left flags before entry `base`, over all four lists
+    const int lefts_per_list = kd_lefts(N, level);
+#pragma unroll
+    for (int k = 0; k < KD_TILE_ITEMS; ++k) {
+        const int64_t g = base + k;
+        if (g < n4) {
+            const int li = (int)(g / N), i = (int)(g - (int64_t)li * N);
+            int lo, hi, lb;
+            kd_node_of(N, level, i, lo, hi, lb);
+            const int mid = lo + (hi - lo + 1) / 2;
+            const int nleft_before = before - li * lefts_per_list - lb;  // within the node, before entry i
+            const int dest = flag[k] ? (lo + nleft_before) : (mid + (i - lo - nleft_before));
+            out[(int64_t)li * N + dest] = part[k];
+        }
+        before += flag[k];
+    }
 }
 
 // ---------------------------------------------------------------------------------------
@@ -405,7 +477,8 @@ int tree_build(fmm_plan *p, const fmm_particles_t *in)
 
     if ((p->flags & FMM_TREE_MASK) == FMM_TREE_KD) {
         uint32_t *lists2 = (uint32_t *)ctx_alloc(c, sizeof(uint32_t) * 4 * (size_t)N);
-        int32_t *scan = (int32_t *)ctx_alloc(c, sizeof(int32_t) * 4 * (size_t)N);
+        const int ntiles = (int)((4ll * N + KD_TILE - 1) / KD_TILE);
+        int32_t *scan = (int32_t *)ctx_alloc(c, sizeof(int32_t) * (size_t)ntiles);  // left flags per tile, then their exclusive scan
         uint8_t *left = (uint8_t *)ctx_alloc(c, (size_t)N);
         int8_t *axis = (int8_t *)ctx_alloc(c, (size_t)((p->leaves > 1) ? p->leaves : 1));
         if (!lists2 || !scan || !left || !axis) return FMM_ENOMEM;
@@ -420,7 +493,6 @@ int tree_build(fmm_plan *p, const fmm_particles_t *in)
         kd_iota<<<gN, T, 0, st>>>(N, lists + 3 * (size_t)N);
         FMM_LAUNCH_CHECK(c, "kd_iota");
         uint32_t *cur = lists, *nxt = lists2;
-        const int g4 = (int)((4ll * N + T - 1) / T);
         for (int level = 0; level < p->kappa; ++level) {
             int nn = 1 << level;
             kd_choose_axis<<<(nn + T - 1) / T, T, 0, st>>>(N, level, in->x, in->y, in->z, cur, cur + N, cur + 2 * (size_t)N,
@@ -428,10 +500,10 @@ int tree_build(fmm_plan *p, const fmm_particles_t *in)
             FMM_LAUNCH_CHECK(c, "kd_choose_axis");
             kd_mark_left<<<gN, T, 0, st>>>(N, level, axis, cur, cur + N, cur + 2 * (size_t)N, left);
             FMM_LAUNCH_CHECK(c, "kd_mark_left");
-            kd_gather_flags<<<g4, T, 0, st>>>(N, left, cur, scan);
-            FMM_LAUNCH_CHECK(c, "kd_gather_flags");
-            FMM_TRY(scan_exclusive_i32(c, scan, scan, 4ll * N));
-            kd_partition<<<g4, T, 0, st>>>(N, level, left, scan, cur, nxt);
+            kd_tile_counts<<<ntiles, 256, 0, st>>>(4ll * N, left, cur, scan);
+            FMM_LAUNCH_CHECK(c, "kd_tile_counts");
+            FMM_TRY(scan_exclusive_i32(c, scan, scan, ntiles));
+            kd_partition<<<ntiles, 256, 0, st>>>(N, level, left, scan, cur, nxt);
             FMM_LAUNCH_CHECK(c, "kd_partition");
             uint32_t *t = cur; cur = nxt; nxt = t;
         }
