@@ -568,7 +568,11 @@ static int launch_m2l(fmm_plan *p)
 
 static int m2l_upload_cheb(fmm_ctx *c)
 {
-    static std::atomic<int> done{0};
+    static std::atomic<int> done_on[64];  // __constant__ memory is per device
+    int dev = 0;
+    FMM_CUDA(c, cudaGetDevice(&dev));
+    if (dev < 0 || dev >= 64) return FMM_EINVAL;
+    std::atomic<int> &done = done_on[dev];
     if (done.load(std::memory_order_acquire)) return FMM_OK;
     double tab[FMM_MAX_ORDER + 2][M2L_XI_STRIDE];
     memset(tab, 0, sizeof(tab));
