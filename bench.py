@@ -48,9 +48,9 @@ def parse_args():
     ap.add_argument("--tree", default="kd", choices=["kd", "morton"])
     ap.add_argument("--kernel", default="mean_gamma", choices=["mean_gamma", "source_momentum"],
                     help="near-field kernel: eq. (3.2) with gamma_bar (default) or the G6 alternative (SURVEY 8(f) rank 2)")
-    ap.add_argument("--no-overlap", action="store_true", help="run P2P after L2L on one stream instead of beside the far-field chain")
+    ap.add_argument("--overlap", action="store_true", help="run P2P on a second stream beside the far-field chain (fmm_plan_set_overlap)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--cpu-sample-leaves", type=int, default=2048,
+    ap.add_argument("--cpu-sample-leaves", type=int, default=4096,
                     help="target leaves the oracle evaluates in the cpu_baseline leg (the reference arm uses 1/8 of it per step)")
     return ap.parse_args()
 
@@ -237,7 +237,7 @@ def run_cuda(args):
     prm = dict(order_n=w.order_n, leaf_size=w.leaf_size, theta=w.theta, flags=flags, device=dev)
 
     plan = fmm.fmm_plan_create(*d_in, w.q, **prm)
-    overlap = not args.no_overlap
+    overlap = args.overlap
     plan.set_overlap(overlap)
     plan.set_timing(not overlap)   # per-stage events force the serial order: with overlap they are taken in a second pass
 

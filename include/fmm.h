@@ -169,10 +169,12 @@ int fmm_field_host(const fmm_particles_t *particles_host, const fmm_params_t *pa
  * fmm_plan_stats synchronises on the last one. */
 int fmm_plan_set_timing(fmm_plan_t *plan, int on);
 
-/* on != 0 (default): fmm_eval runs P2P (a7) on a second stream of the plan, concurrently with P2M, M2M, M2L and L2L on
+/* on != 0 (default is 0): fmm_eval runs P2P (a7) on a second stream of the plan, concurrently with P2M, M2M, M2L and L2L on
  * the caller's stream (a7 is independent of a4-a6, a8; PAPER.md:562-566 runs them as separate kernels too); the second
  * stream is forked from and joined into the caller's stream with events, so the call still behaves as work enqueued on
- * `cuda_stream`.  Results are bit-identical either way.  Stage timing (fmm_plan_set_timing) forces the serial order. */
+ * `cuda_stream`.  Results are bit-identical either way.  Stage timing (fmm_plan_set_timing) forces the serial order.
+ * Measured on B200: 2 % faster at N = 2^20, n = 6 (the small upward / downward kernels hide behind P2P), but P2P itself
+ * runs up to 45 % slower whenever other grids are resident beside it, so this is opt-in for far-field-heavy settings. */
 int fmm_plan_set_overlap(fmm_plan_t *plan, int on);
 int fmm_plan_stats(fmm_plan_t *plan, fmm_stats_t *stats);
 int fmm_plan_export(fmm_plan_t *plan, fmm_export_t *out);  /* synchronises the stream */

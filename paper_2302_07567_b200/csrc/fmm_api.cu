@@ -222,7 +222,7 @@ extern "C" int fmm_plan_create(fmm_plan_t **out, const fmm_particles_t *in, cons
                          cudaEventCreateWithFlags(&p->ev_fork, cudaEventDisableTiming) != cudaSuccess ||
                          cudaEventCreateWithFlags(&p->ev_join, cudaEventDisableTiming) != cudaSuccess))
         rc = FMM_ECUDA;
-    p->overlap = 1;
+    p->overlap = 0;  // opt-in (fmm_plan_set_overlap): +2 % at the headline workload, but up to -45 % when P2P dominates
     if (rc == FMM_OK) rc = plan_alloc_fixed(p);
     if (rc == FMM_OK) rc = plan_build(p, in);
     if (rc != FMM_OK) {

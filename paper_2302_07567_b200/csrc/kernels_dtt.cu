@@ -90,7 +90,7 @@ __global__ void csr_from_sorted(const uint64_t *__restrict__ keys, int64_t n, in
 
 // LPT block order: targets by descending work (number of source clusters x their sizes)
 __global__ void list_work_keys(int first, int count, const int32_t *__restrict__ off, const int32_t *__restrict__ src,
-                               const int32_t *__restrict__ node_lo, const int32_t *__restrict__ node_hi, int by_size, int work_shift,
+                               const int32_t *__restrict__ node_lo, const int32_t *__restrict__ node_hi, int by_size,
                                uint64_t *__restrict__ keys, uint32_t *__restrict__ vals, unsigned long long *__restrict__ total)
 {
     int k = blockIdx.x * blockDim.x + threadIdx.x;
@@ -104,9 +104,15 @@ __global__ void list_work_keys(int first, int count, const int32_t *__restrict__
     } else {
         work = (unsigned long long)(off[t + 1] - off[t]);
     }
-    // block order only needs a coarse, deterministic ranking: 16-bit keys (2 radix passes), work in units of 2^shift
-    unsigned long long wq = work >> work_shift;
-    if (wq > 0xffffull) wq = 0xffffull;
+    // block order only needs a coarse, deterministic ranking: a 16-bit monotone code of the work (6-bit exponent,
+    // 10-bit mantissa: 0.1 % resolution over the whole 64-bit range), so the sort takes 2 radix passes
+    unsigned long long wq = 0;
+    if (work > 0) {
+        int e = 63 - __clzll((long long)work);
+        unsigned long long mant = (e >= 10) ? (work >> (e - 10)) : (work << (10 - e));  // 1.xxxxxxxxxx
+        wq = ((unsigned long long)e << 10) | (mant & 0x3ffull);
+        wq += 1;  // keep 0 for "no work"
+    }
     keys[k] = 0xffffull - wq;  // ascending sort of this = descending work
     vals[k] = (uint32_t)t;
 }
@@ -117,7 +123,7 @@ __global__ void copy_u32_to_i32(int n, const uint32_t *__restrict__ a, int32_t *
     if (k < n) b[k] = (int32_t)a[k];
 }
 
-static int make_order(fmm_plan *p, int first, int count, const int32_t *off, const int32_t *src, int by_size, int work_shift,
+static int make_order(fmm_plan *p, int first, int count, const int32_t *off, const int32_t *src, int by_size,
                       int32_t *order_out, unsigned long long *total_dev)
 {
     fmm_ctx *c = &p->ctx;
@@ -126,7 +132,7 @@ static int make_order(fmm_plan *p, int first, int count, const int32_t *off, con
     uint32_t *vals = (uint32_t *)ctx_alloc(c, sizeof(uint32_t) * count);
     uint32_t *tvals = (uint32_t *)ctx_alloc(c, sizeof(uint32_t) * count);
     if (!keys || !tkeys || !vals || !tvals) return FMM_ENOMEM;
-    list_work_keys<<<(count + 255) / 256, 256, 0, c->stream>>>(first, count, off, src, p->node_lo, p->node_hi, by_size, work_shift, keys, vals, total_dev);
+    list_work_keys<<<(count + 255) / 256, 256, 0, c->stream>>>(first, count, off, src, p->node_lo, p->node_hi, by_size, keys, vals, total_dev);
     FMM_LAUNCH_CHECK(c, "list_work_keys");
     FMM_TRY(sort_pairs_u64(c, keys, vals, tkeys, tvals, count, 0, 16));
     copy_u32_to_i32<<<(count + 255) / 256, 256, 0, c->stream>>>(count, vals, order_out);
@@ -194,11 +200,8 @@ int dtt_build_lists(fmm_plan *p)
 
     // block orders (descending work) and evaluation counts
     FMM_CUDA(c, cudaMemsetAsync(total_dev, 0, sizeof(unsigned long long), st));
-    int64_t maxleaf = (p->N + p->leaves - 1) / p->leaves;
-    int p2p_shift = 0;  // a row of 64 full leaf pairs still fits 16 bits; longer rows saturate (they are issued first anyway)
-    while (((maxleaf * maxleaf * 64) >> p2p_shift) > 0xffff) ++p2p_shift;
-    FMM_TRY(make_order(p, (int)p->leaves, (int)p->leaves, p->p2p_off, p->p2p_src, 1, p2p_shift, p->p2p_order, total_dev));
-    FMM_TRY(make_order(p, 1, (int)p->nodes, p->m2l_off, p->m2l_src, 0, 0, p->m2l_order, total_dev));
+    FMM_TRY(make_order(p, (int)p->leaves, (int)p->leaves, p->p2p_off, p->p2p_src, 1, p->p2p_order, total_dev));
+    FMM_TRY(make_order(p, 1, (int)p->nodes, p->m2l_off, p->m2l_src, 0, p->m2l_order, total_dev));
     unsigned long long total_h = 0;
     FMM_CUDA(c, cudaMemcpyAsync(&total_h, total_dev, sizeof(total_h), cudaMemcpyDeviceToHost, st));
     FMM_CUDA(c, cudaStreamSynchronize(st));
