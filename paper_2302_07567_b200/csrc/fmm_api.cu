@@ -147,7 +147,6 @@ static int plan_alloc_fixed(fmm_plan *p)
     ALLOC(p2p_order, int32_t, nodes1); ALLOC(m2l_order, int32_t, nodes1);
     ALLOC(M, double, 4 * (size_t)p->P * nodes1);
     ALLOC(L, double, 6 * (size_t)p->P * nodes1);
-    ALLOC(near_, double, 6 * N);
 #undef ALLOC
     return FMM_OK;
 }
@@ -165,6 +164,7 @@ static int plan_build(fmm_plan *p, const fmm_particles_t *in, bool refit = false
     FMM_TRY(refit ? tree_refit(p, in) : tree_build(p, in));
     FMM_CUDA(c, cudaEventRecord(p->ev_plan[1], c->stream));
     FMM_TRY(dtt_build_lists(p));
+    FMM_TRY(pairs_p2p_prepare(p));
     FMM_CUDA(c, cudaEventRecord(p->ev_plan[2], c->stream));
     FMM_CUDA(c, cudaStreamSynchronize(c->stream));
     FMM_CUDA(c, cudaEventElapsedTime(&p->ms_tree, p->ev_plan[0], p->ev_plan[1]));

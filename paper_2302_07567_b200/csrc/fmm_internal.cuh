@@ -73,12 +73,15 @@ struct fmm_plan {
     int32_t *p2p_off, *p2p_src, *m2l_off, *m2l_src;
     int64_t n_p2p, n_m2l, cap_p2p, cap_m2l;
     int64_t p2p_pairs, m2l_pairs;
+    int64_t p2p_max_row;    // largest number of particle pairs in one target leaf's row
+    int p2p_split;          // P2P row split K: block (t, k) sums chunk k of t's row into near_[k]; L2P adds the K partials in order
+    int64_t near_cap;       // doubles allocated for near_
     int32_t *p2p_order, *m2l_order;  // target ids sorted by descending work (LPT block order)
     int32_t n_p2p_targets, n_m2l_targets;
     // expansions
     double *M;              // [nodes+1][P][4]
     double *L;              // [nodes+1][P][6]
-    double *near_;          // [6][N] tree order, P2P result
+    double *near_;          // [p2p_split][6][N] tree order, P2P partial results
     // timing
     int timing;
     cudaEvent_t ev[EV_COUNT];
@@ -106,6 +109,7 @@ int interp_l2l(fmm_plan *p);
 int interp_l2p_finalize(fmm_plan *p, double *Ex, double *Ey, double *Ez, double *Bx, double *By, double *Bz);
 // ---- kernels_pairs.cu ---------------------------------------------------------------
 int pairs_p2p(fmm_plan *p);
+int pairs_p2p_prepare(fmm_plan *p);
 int pairs_m2l(fmm_plan *p);
 int pairs_direct(fmm_ctx *c, int64_t N, const double *x, const double *y, const double *z,
                  const double *w0, const double *w1, const double *w2, const double *w3,

@@ -101,6 +101,7 @@ __global__ void list_work_keys(int first, int count, const int32_t *__restrict__
         unsigned long long nt = (unsigned long long)(node_hi[t] - node_lo[t]);
         for (int e = off[t]; e < off[t + 1]; ++e) work += nt * (unsigned long long)(node_hi[src[e]] - node_lo[src[e]]);
         atomicAdd(total, work);
+        atomicMax(total + 1, work);
     } else {
         work = (unsigned long long)(off[t + 1] - off[t]);
     }
@@ -147,7 +148,7 @@ int dtt_build_lists(fmm_plan *p)
     cudaStream_t st = c->stream;
     const int key_shift = p->kappa + 2;  // node ids < 2^(kappa+1)
     const int nsteps = 2 * p->kappa + 1;
-    dtt_counters *cnt = (dtt_counters *)ctx_alloc(c, sizeof(dtt_counters) + sizeof(unsigned long long));
+    dtt_counters *cnt = (dtt_counters *)ctx_alloc(c, sizeof(dtt_counters) + 2 * sizeof(unsigned long long));
     if (!cnt) return FMM_ENOMEM;
     unsigned long long *total_dev = (unsigned long long *)(cnt + 1);
     dtt_counters h;
@@ -199,13 +200,14 @@ int dtt_build_lists(fmm_plan *p)
     ctx_free(c, tkeys); ctx_free(c, kp2p); ctx_free(c, km2l);
 
     // block orders (descending work) and evaluation counts
-    FMM_CUDA(c, cudaMemsetAsync(total_dev, 0, sizeof(unsigned long long), st));
+    FMM_CUDA(c, cudaMemsetAsync(total_dev, 0, 2 * sizeof(unsigned long long), st));
     FMM_TRY(make_order(p, (int)p->leaves, (int)p->leaves, p->p2p_off, p->p2p_src, 1, p->p2p_order, total_dev));
     FMM_TRY(make_order(p, 1, (int)p->nodes, p->m2l_off, p->m2l_src, 0, p->m2l_order, total_dev));
-    unsigned long long total_h = 0;
-    FMM_CUDA(c, cudaMemcpyAsync(&total_h, total_dev, sizeof(total_h), cudaMemcpyDeviceToHost, st));
+    unsigned long long total_h2[2] = {0, 0};
+    FMM_CUDA(c, cudaMemcpyAsync(total_h2, total_dev, sizeof(total_h2), cudaMemcpyDeviceToHost, st));
     FMM_CUDA(c, cudaStreamSynchronize(st));
-    p->p2p_pairs = (int64_t)total_h;
+    p->p2p_pairs = (int64_t)total_h2[0];
+    p->p2p_max_row = (int64_t)total_h2[1];
     p->m2l_pairs = p->n_m2l * (int64_t)p->P * (int64_t)p->P;
     ctx_free(c, cnt);
     return FMM_OK;

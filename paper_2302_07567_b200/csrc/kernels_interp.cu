@@ -289,7 +289,7 @@ __global__ void __launch_bounds__(L2P_THREADS) l2p_kernel(int n, cheb_t ch, int 
                                                           const int32_t *__restrict__ node_hi, const double *__restrict__ bbox,
                                                           const double *__restrict__ tx, const double *__restrict__ ty,
                                                           const double *__restrict__ tz, const double *__restrict__ L,
-                                                          const double *__restrict__ near_, const int32_t *__restrict__ perm,
+                                                          const double *__restrict__ near_, int K, const int32_t *__restrict__ perm,
                                                           double cE, double cB, double *__restrict__ Ex, double *__restrict__ Ey,
                                                           double *__restrict__ Ez, double *__restrict__ Bx, double *__restrict__ By,
                                                           double *__restrict__ Bz)
@@ -330,12 +330,19 @@ __global__ void __launch_bounds__(L2P_THREADS) l2p_kernel(int n, cheb_t ch, int 
         }
         int i = perm[k];
         // fixed order: near + far, then the prefactors of eq. (3.1)
-        Ex[i] = cE * (near_[k] + fx[0]);
-        Ey[i] = cE * (near_[(size_t)N + k] + fx[1]);
-        Ez[i] = cE * (near_[2 * (size_t)N + k] + fx[2]);
-        Bx[i] = cB * (near_[3 * (size_t)N + k] + fx[3]);
-        By[i] = cB * (near_[4 * (size_t)N + k] + fx[4]);
-        Bz[i] = cB * (near_[5 * (size_t)N + k] + fx[5]);
+        double nr[6];  // near field: the K row chunks of P2P, added in chunk order
+#pragma unroll
+        for (int f = 0; f < 6; ++f) nr[f] = near_[f * (size_t)N + k];
+        if (K > 1)
+            for (int kc = 1; kc < K; ++kc)
+#pragma unroll
+                for (int f = 0; f < 6; ++f) nr[f] += near_[((size_t)kc * 6 + f) * (size_t)N + k];
+        Ex[i] = cE * (nr[0] + fx[0]);
+        Ey[i] = cE * (nr[1] + fx[1]);
+        Ez[i] = cE * (nr[2] + fx[2]);
+        Bx[i] = cB * (nr[3] + fx[3]);
+        By[i] = cB * (nr[4] + fx[4]);
+        Bz[i] = cB * (nr[5] + fx[5]);
     }
 }
 
@@ -418,7 +425,7 @@ int interp_l2p_finalize(fmm_plan *p, double *Ex, double *Ey, double *Ez, double 
     size_t smem = sizeof(double) * (6 * (size_t)p->P + 3 * (size_t)p->n1 * L2P_THREADS);
     FMM_TRY(set_smem(c, (const void *)l2p_kernel, smem));
     l2p_kernel<<<(unsigned)p->leaves, L2P_THREADS, smem, c->stream>>>(p->n, ch, (int)p->leaves, (int)p->N, p->node_lo, p->node_hi, p->bbox,
-                                                                      p->tx, p->ty, p->tz, p->L, p->near_, p->perm, cE, cB, Ex, Ey, Ez,
+                                                                      p->tx, p->ty, p->tz, p->L, p->near_, p->p2p_split, p->perm, cE, cB, Ex, Ey, Ez,
                                                                       Bx, By, Bz);
     FMM_LAUNCH_CHECK(c, "l2p_kernel");
     return FMM_OK;

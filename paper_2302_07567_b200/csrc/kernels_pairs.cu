@@ -103,7 +103,7 @@ __device__ __forceinline__ void tile_interact(const double2 *tile, int count, co
 // a7: P2P.  One block per target leaf (blocks issued in descending-work order); NT target particles per
 // thread; the source leaves of the CSR row are staged tile by tile.
 // ---------------------------------------------------------------------------------------
-template <int NT, bool SM>
+template <int NT, bool SM, bool SPLIT>
 __global__ void __launch_bounds__(256) p2p_kernel(int N, double gb, const int32_t *__restrict__ order, const int32_t *__restrict__ off,
                                                   const int32_t *__restrict__ src, const int32_t *__restrict__ node_lo,
                                                   const int32_t *__restrict__ node_hi, const double *__restrict__ tx,
@@ -111,12 +111,14 @@ __global__ void __launch_bounds__(256) p2p_kernel(int N, double gb, const int32_
                                                   const double *__restrict__ w0, const double *__restrict__ w1,
                                                   const double *__restrict__ w2, const double *__restrict__ w3,
                                                   const double *__restrict__ pmx, const double *__restrict__ pmy,
-                                                  const double *__restrict__ pmz, double *__restrict__ near_)
+                                                  const double *__restrict__ pmz, int K, double *__restrict__ near_)
 {
     __shared__ double2 tile[(SM ? 5 : 4) * PAIR_TILE];
-    const int t = order[blockIdx.x];
+    // block (t, k): chunk k of the K contiguous chunks of target t's row; its sums go to partial buffer k
+    const int t = SPLIT ? order[blockIdx.x / K] : order[blockIdx.x], kc = SPLIT ? blockIdx.x % K : 0;
     const int tlo = node_lo[t], thi = node_hi[t];
-    const int e0 = off[t], e1 = off[t + 1];
+    const int r0 = off[t], rl = off[t + 1] - r0;
+    const int e0 = SPLIT ? r0 + (int)(((int64_t)rl * kc) / K) : r0, e1 = SPLIT ? r0 + (int)(((int64_t)rl * (kc + 1)) / K) : r0 + rl;
     for (int i0 = tlo; i0 < thi; i0 += NT * blockDim.x) {
         double xt[NT], yt[NT], zt[NT], ex[NT], ey[NT], ez[NT], bx[NT], by[NT], bz[NT];
 #pragma unroll
@@ -141,20 +143,20 @@ __global__ void __launch_bounds__(256) p2p_kernel(int N, double gb, const int32_
         for (int k = 0; k < NT; ++k) {
             int i = i0 + k * blockDim.x + threadIdx.x;
             if (i < thi) {
-                near_[i] = ex[k];
-                near_[(size_t)N + i] = ey[k];
-                near_[2 * (size_t)N + i] = ez[k];
-                near_[3 * (size_t)N + i] = bx[k];
-                near_[4 * (size_t)N + i] = by[k];
-                near_[5 * (size_t)N + i] = bz[k];
+                double *o = near_ + (SPLIT ? (size_t)kc * 6 * (size_t)N : (size_t)0) + i;
+                o[0] = ex[k];
+                o[(size_t)N] = ey[k];
+                o[2 * (size_t)N] = ez[k];
+                o[3 * (size_t)N] = bx[k];
+                o[4 * (size_t)N] = by[k];
+                o[5 * (size_t)N] = bz[k];
             }
         }
     }
 }
 
-// Targets per thread: the largest NT <= 4 that still leaves >= 8 warps per SM in flight, among those the one that
-// wastes the fewest lanes (a leaf of 78 particles fills 3 x 32 slots at NT = 3 but only 78 of 128 at NT = 4).
-static void p2p_shape(int64_t leaves, int maxleaf, int *nt_out, int *threads_out)
+// Targets per thread: the NT <= 4 that wastes the fewest lanes, ties to the larger NT (a leaf of 78 particles fills 3 x 32 slots at NT = 3 but only 78 of 128 at NT = 4).
+static void p2p_shape(int64_t leaves, int maxleaf, int64_t pairs, int64_t max_row, int *nt_out, int *threads_out, int *split_out)
 {
     int best_nt = 1, best_threads = 32;
     double best_score = -1.0;
@@ -164,26 +166,57 @@ static void p2p_shape(int64_t leaves, int maxleaf, int *nt_out, int *threads_out
         if (threads > 256) threads = 256;
         int passes = (maxleaf + nt * threads - 1) / (nt * threads);
         double eff = (double)maxleaf / ((double)passes * nt * threads);
-        double warps = (double)leaves * (threads / 32);
-        double fill = warps >= 8.0 * FMM_SM_COUNT ? 1.0 : warps / (8.0 * FMM_SM_COUNT);
-        double score = eff * fill * (1.0 + 0.02 * nt);  // ties: more targets per thread
+        double score = eff * (1.0 + 0.02 * nt);  // ties: more targets per thread (the row split K restores the block count)
         if (score > best_score) { best_score = score; best_nt = nt; best_threads = threads; }
     }
     *nt_out = best_nt;
     *threads_out = best_threads;
+    // Row split K: (a) enough warps in flight when there are few leaves, (b) no single row longer than a quarter of an
+    // SM's fair share of the whole near field (the tail leaves of a Gaussian bunch have rows of several hundred leaves).
+    double warps = (double)leaves * (best_threads / 32);
+    int k_fill = (int)((8.0 * FMM_SM_COUNT + warps - 1) / warps);
+    double fair = (double)pairs / (4.0 * FMM_SM_COUNT);
+    int k_bal = (fair > 0.0) ? (int)((double)max_row / fair + 0.999) : 1;
+    int K = k_fill > k_bal ? k_fill : k_bal;
+    if (K > 8) K = 8;
+    if (K < 1) K = 1;
+    *split_out = K;
+}
+
+int pairs_p2p_prepare(fmm_plan *p)  // after the lists: choose the row split and size the partial buffers
+{
+    fmm_ctx *c = &p->ctx;
+    int maxleaf = (int)((p->N + p->leaves - 1) / p->leaves);
+    int nt, threads, K;
+    p2p_shape(p->leaves, maxleaf, p->p2p_pairs, p->p2p_max_row, &nt, &threads, &K);
+    p->p2p_split = K;
+    int64_t need = (int64_t)K * 6 * p->N;
+    if (need > p->near_cap) {
+        if (p->near_) ctx_free(c, p->near_);
+        p->near_ = (double *)ctx_alloc(c, sizeof(double) * (size_t)need);
+        if (!p->near_) return FMM_ENOMEM;
+        p->near_cap = need;
+    }
+    return FMM_OK;
 }
 
 int pairs_p2p(fmm_plan *p)
 {
     fmm_ctx *c = &p->ctx;
     int maxleaf = (int)((p->N + p->leaves - 1) / p->leaves);
-    int nt, threads;
-    p2p_shape(p->leaves, maxleaf, &nt, &threads);
+    int nt, threads, K;
+    p2p_shape(p->leaves, maxleaf, p->p2p_pairs, p->p2p_max_row, &nt, &threads, &K);
+    K = p->p2p_split;
     const bool sm = (p->flags & FMM_KERNEL_SOURCE_MOMENTUM) != 0;
 #define P2P_LAUNCH(NT, SM)                                                                                                               \
-    p2p_kernel<NT, SM><<<(unsigned)p->leaves, threads, 0, c->stream>>>((int)p->N, p->gamma_bar, p->p2p_order, p->p2p_off, \
+    if (K > 1)                                                                                                                           \
+        p2p_kernel<NT, SM, true><<<(unsigned)(p->leaves * K), threads, 0, c->stream>>>((int)p->N, p->gamma_bar, p->p2p_order, p->p2p_off, \
                                                                        p->p2p_src, p->node_lo, p->node_hi, p->tx, p->ty, p->tz, p->w0,   \
-                                                                       p->w1, p->w2, p->w3, p->pmx, p->pmy, p->pmz, p->near_)
+                                                                       p->w1, p->w2, p->w3, p->pmx, p->pmy, p->pmz, K, p->near_);        \
+    else                                                                                                                                 \
+    p2p_kernel<NT, SM, false><<<(unsigned)(p->leaves * K), threads, 0, c->stream>>>((int)p->N, p->gamma_bar, p->p2p_order, p->p2p_off, \
+                                                                       p->p2p_src, p->node_lo, p->node_hi, p->tx, p->ty, p->tz, p->w0,   \
+                                                                       p->w1, p->w2, p->w3, p->pmx, p->pmy, p->pmz, K, p->near_)
     switch (nt) {
         case 1: if (sm) P2P_LAUNCH(1, true); else P2P_LAUNCH(1, false); break;
         case 2: if (sm) P2P_LAUNCH(2, true); else P2P_LAUNCH(2, false); break;
