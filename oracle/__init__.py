@@ -71,6 +71,10 @@ def lib():
         _lib.orc_eval.restype = C.c_int
         _lib.orc_eval.argtypes = [C.c_void_p, C.c_int64, _i64p, C.c_int] + [_dp] * 7
         _lib.orc_m2l_raw.argtypes = [C.c_void_p, _dp]
+        _lib.orc_treecode_sizes.argtypes = [C.c_void_p, _i64p]
+        _lib.orc_treecode_lists.argtypes = [C.c_void_p, _i32p, _i32p, _i32p, _i32p]
+        _lib.orc_eval_treecode.restype = C.c_int
+        _lib.orc_eval_treecode.argtypes = [C.c_void_p] + [_dp] * 6
         _lib.orc_num_threads.restype = C.c_int
     return _lib
 
@@ -200,6 +204,21 @@ class Plan:
         L = np.empty((self.nodes, self.P, 6))
         lib().orc_m2l_raw(self._h, L.ctypes.data_as(_dp))
         return L
+
+    def treecode_lists(self):
+        """(pp[npp,2], pc[npc,2]) as (target leaf, source) heap ids sorted by (target, source)."""
+        s = np.empty(2, dtype=np.int64)
+        lib().orc_treecode_sizes(self._h, s.ctypes.data_as(_i64p))
+        a = [np.empty(int(s[0]), dtype=np.int32), np.empty(int(s[0]), dtype=np.int32),
+             np.empty(int(s[1]), dtype=np.int32), np.empty(int(s[1]), dtype=np.int32)]
+        lib().orc_treecode_lists(self._h, *[v.ctypes.data_as(_i32p) for v in a])
+        return np.stack(a[:2], axis=1), np.stack(a[2:], axis=1)
+
+    def eval_treecode(self):
+        """Treecode variant (particle-cluster): (E[N,3], B[N,3]) in caller order."""
+        out = [np.empty(self.N) for _ in range(6)]
+        lib().orc_eval_treecode(self._h, *[o.ctypes.data_as(_dp) for o in out])
+        return np.stack(out[:3], axis=1), np.stack(out[3:], axis=1)
 
     def eval(self, leaves=None, part="all", want_L=False):
         """Returns (E[N,3], B[N,3]) in caller order (rows of unselected leaves are NaN)."""

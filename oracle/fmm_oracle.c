@@ -37,6 +37,8 @@ struct orc_plan {
     double *bbox;         /* [nodes+1][6] ax ay az bx by bz */
     int64_t np2p, nm2l, cap_p2p, cap_m2l;
     int32_t *p2p, *m2l;   /* pairs (t,s) interleaved */
+    int64_t ntcpp, ntcpc, cap_tcpp, cap_tcpc;
+    int32_t *tcpp, *tcpc; /* treecode lists: (target leaf, source leaf) and (target leaf, source cluster) */
     double *M;            /* [nodes+1][P][4] */
     int have_M;
     double cheb[64];
@@ -515,7 +517,7 @@ void orc_plan_destroy(orc_plan_t *p)
 {
     if (!p) return;
     free(p->x); free(p->y); free(p->z); free(p->w); free(p->pm); free(p->perm);
-    free(p->lo); free(p->hi); free(p->bbox); free(p->p2p); free(p->m2l); free(p->M);
+    free(p->lo); free(p->hi); free(p->bbox); free(p->p2p); free(p->m2l); free(p->tcpp); free(p->tcpc); free(p->M);
     free(p);
 }
 
@@ -793,6 +795,94 @@ void orc_m2l_raw(orc_plan_t *p, double *L_raw)
     m2l_all(p, NULL, L);
     memcpy(L_raw, &L[P6], sizeof(double) * P6 * (size_t)p->nodes);
     free(L);
+}
+
+/* Treecode variant (particle-cluster, Fig. 1a, ref [16]) -------------------------
+ * The traversal is Alg 9.1 with the target held at a leaf: for every target leaf t, dualtraverse(t, root).  With a
+ * leaf target Alg 9.1 never splits the target, so: both leaves -> direct sum (PP list); admissible (Alg 5.8) ->
+ * particle-cluster interaction (PC list): the target PARTICLES evaluate the kernel at the source's proxy points,
+ *   E_i += sum_nu gamma_{s,nu} g(x_i, xi_{s,nu}),  B_i += sum_nu p_{s,nu} x g(x_i, xi_{s,nu})   (eq. (2.5) with the
+ * target side not interpolated); otherwise the source is split.  Needs P2M / M2M only; no L2L / L2P. */
+static void treecode_lists(orc_plan_t *p)
+{
+    if (p->tcpp || p->tcpc) return;
+    /* reuse dualtraversefillitl with temporarily swapped list buffers */
+    int32_t *sp2p = p->p2p, *sm2l = p->m2l;
+    int64_t np2p = p->np2p, nm2l = p->nm2l, cp2p = p->cap_p2p, cm2l = p->cap_m2l;
+    p->p2p = NULL; p->m2l = NULL; p->np2p = p->nm2l = p->cap_p2p = p->cap_m2l = 0;
+    for (int64_t t = p->leaves; t <= p->nodes; ++t)
+        dualtraversefillitl(p, t, 1);
+    qsort(p->p2p, (size_t)p->np2p, 2 * sizeof(int32_t), cmp_pair);
+    qsort(p->m2l, (size_t)p->nm2l, 2 * sizeof(int32_t), cmp_pair);
+    p->tcpp = p->p2p; p->ntcpp = p->np2p; p->cap_tcpp = p->cap_p2p;
+    p->tcpc = p->m2l; p->ntcpc = p->nm2l; p->cap_tcpc = p->cap_m2l;
+    if (!p->tcpp) p->tcpp = (int32_t *)malloc(8);
+    if (!p->tcpc) p->tcpc = (int32_t *)malloc(8);
+    p->p2p = sp2p; p->m2l = sm2l; p->np2p = np2p; p->nm2l = nm2l; p->cap_p2p = cp2p; p->cap_m2l = cm2l;
+}
+
+void orc_treecode_sizes(orc_plan_t *p, int64_t *out /* [2]: len(pp), len(pc) */)
+{
+    treecode_lists(p);
+    out[0] = p->ntcpp;
+    out[1] = p->ntcpc;
+}
+
+void orc_treecode_lists(orc_plan_t *p, int32_t *pp_t, int32_t *pp_s, int32_t *pc_t, int32_t *pc_s)
+{
+    treecode_lists(p);
+    for (int64_t k = 0; k < p->ntcpp; ++k) { pp_t[k] = p->tcpp[2 * k]; pp_s[k] = p->tcpp[2 * k + 1]; }
+    for (int64_t k = 0; k < p->ntcpc; ++k) { pc_t[k] = p->tcpc[2 * k]; pc_s[k] = p->tcpc[2 * k + 1]; }
+}
+
+/* particle-cluster interaction of target leaf t with source cluster s (far field with the mean gamma_bar, eq. (3.2)) */
+static void pc(const orc_plan_t *p, int64_t t, int64_t s, double *far /* [N][6] tree order */)
+{
+    int n1 = p->n1;
+    double g2 = p->gamma_bar * p->gamma_bar;
+    double xs[192];
+    proxy_points(p, s, xs);
+    const double *Ms = &p->M[4 * (size_t)p->P * s];
+    for (int64_t ki = p->lo[t]; ki < p->hi[t]; ++ki) {
+        int64_t i = p->perm[ki];
+        double *acc = &far[6 * ki];
+        for (int a2 = 0; a2 < n1; ++a2)
+            for (int b2 = 0; b2 < n1; ++b2)
+                for (int c2 = 0; c2 < n1; ++c2)
+                    accumulate(p->x[i] - xs[a2], p->y[i] - xs[64 + b2], p->z[i] - xs[128 + c2], g2,
+                               &Ms[4 * ((a2 * n1 + b2) * n1 + c2)], acc);
+    }
+}
+
+int orc_eval_treecode(orc_plan_t *p, double *Ex, double *Ey, double *Ez, double *Bx, double *By, double *Bz)
+{
+    int64_t N = p->N;
+    treecode_lists(p);
+    upward(p);
+    double *near = (double *)calloc(6 * (size_t)N, sizeof(double));
+    double *far = (double *)calloc(6 * (size_t)N, sizeof(double));
+    int64_t *offp = (int64_t *)malloc(sizeof(int64_t) * ((size_t)p->nodes + 2));
+    int64_t *offc = (int64_t *)malloc(sizeof(int64_t) * ((size_t)p->nodes + 2));
+    csr_offsets(p->tcpp, p->ntcpp, p->nodes, offp);
+    csr_offsets(p->tcpc, p->ntcpc, p->nodes, offc);
+#pragma omp parallel for schedule(dynamic, 1)
+    for (int64_t t = p->leaves; t <= p->nodes; ++t) {
+        for (int64_t k = offp[t]; k < offp[t + 1]; ++k) p2p(p, t, p->tcpp[2 * k + 1], near);
+        for (int64_t k = offc[t]; k < offc[t + 1]; ++k) pc(p, t, p->tcpc[2 * k + 1], far);
+    }
+    double cE, cB;
+    prefactors(p->raw, &cE, &cB);
+    for (int64_t k = 0; k < N; ++k) {
+        int64_t i = p->perm[k];
+        Ex[i] = cE * (near[6 * k + 0] + far[6 * k + 0]); /* fixed order: near + far */
+        Ey[i] = cE * (near[6 * k + 1] + far[6 * k + 1]);
+        Ez[i] = cE * (near[6 * k + 2] + far[6 * k + 2]);
+        Bx[i] = cB * (near[6 * k + 3] + far[6 * k + 3]);
+        By[i] = cB * (near[6 * k + 4] + far[6 * k + 4]);
+        Bz[i] = cB * (near[6 * k + 5] + far[6 * k + 5]);
+    }
+    free(near); free(far); free(offp); free(offc);
+    return 0;
 }
 
 /* Alg 5.12 after subdivide. */

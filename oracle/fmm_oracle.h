@@ -101,6 +101,13 @@ int orc_eval(orc_plan_t *, int64_t nsel, const int64_t *sel, int part /*0 all,1 
              double *Ex, double *Ey, double *Ez, double *Bx, double *By, double *Bz,
              double *L_out);
 
+/* Treecode variant (particle-cluster; Fig. 1a): Alg 9.1 started at (t, root) for
+ * every target leaf t -> PP list (leaf, leaf: direct sum) and PC list (leaf, admissible cluster: the leaf's particles
+ * evaluate the kernel at the cluster's proxy points with its moments).  Lists sorted by (target, source). */
+void orc_treecode_sizes(orc_plan_t *, int64_t *out /* [2]: len(pp), len(pc) */);
+void orc_treecode_lists(orc_plan_t *, int32_t *pp_t, int32_t *pp_s, int32_t *pc_t, int32_t *pc_s);
+int  orc_eval_treecode(orc_plan_t *, double *Ex, double *Ey, double *Ez, double *Bx, double *By, double *Bz);
+
 /* M2L sums only (before any L2L): L_raw[nodes][P][6]. Pin P8 (Lemma 1). */
 void orc_m2l_raw(orc_plan_t *, double *L_raw);
 

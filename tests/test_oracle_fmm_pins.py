@@ -390,3 +390,88 @@ def test_given_order_after_a_drift_is_a_valid_tree_with_the_same_accuracy():
     Ef, _ = fresh.eval()
     e_refit, e_fresh = oracle.err2(E, Ed), oracle.err2(Ef, Ed)
     assert e_refit < 3 * e_fresh and e_refit < 5e-3, (e_refit, e_fresh)
+
+
+# ---------------------------------------------------------------------------------------------
+# Treecode variant (particle-cluster; Fig. 1a)
+# ---------------------------------------------------------------------------------------------
+def _leaf_span(i, Lf):
+    lvl = int(np.log2(i)); width = Lf >> lvl
+    first = (i - (1 << lvl)) * width
+    return first, first + width
+
+
+@pytest.mark.parametrize("theta", [0.3, 0.5])
+def test_treecode_lists_cover_every_source_leaf_once_per_target_leaf(theta):
+    w = small(N=4096)
+    p = plan_of(w, theta=theta)
+    pp, pc = p.treecode_lists()
+    Lf = p.leaves
+    cover = np.zeros((Lf, Lf), dtype=np.int32)
+    assert np.all(pp >= Lf) and np.all(pc[:, 0] >= Lf)           # targets are leaves; PP sources are leaves
+    for t, s in np.concatenate([pp, pc]):
+        s0, s1 = _leaf_span(s, Lf)
+        cover[t - Lf, s0:s1] += 1
+    assert np.all(cover == 1)
+    assert len(pc) > 0 or theta < 0.5                            # (theta = 0.3 leaves no admissible cluster at this size)
+    lo, hi, bb = p.node_arrays()                                 # every PC pair satisfies Alg 5.8, no PP pair was tested
+    s = np.array([1.0, 1.0, p.gamma_bar])
+    for t, c in pc[:: max(1, len(pc) // 200)]:
+        bt, bc = bb[t - 1], bb[c - 1]
+        rt = np.linalg.norm(s * (bt[3:] - bt[:3]) * 0.5); rc = np.linalg.norm(s * (bc[3:] - bc[:3]) * 0.5)
+        d = np.linalg.norm(s * ((bt[:3] + bt[3:]) * 0.5 - (bc[:3] + bc[3:]) * 0.5))
+        assert max(rt, rc) < theta * d * (1 + 1e-12)
+
+
+def test_treecode_equals_numpy_restatement_and_direct_without_clusters():
+    """PC interaction restated in numpy from the exported moments, boxes and Chebyshev points; with a tiny theta the
+    PC list is empty and the treecode is the direct sum."""
+    w = small(N=600)
+    p = oracle.Plan(*w.arrays(), w.q, order_n=3, leaf_size=40, theta=0.5, raw=True)
+    pp, pc = p.treecode_lists()
+    M = p.upward()
+    lo, hi, bb = p.node_arrays()
+    perm = p.perm()
+    c = oracle.cheb_nodes(3)
+    g2 = p.gamma_bar ** 2
+    X = np.stack([w.x, w.y, w.z], axis=1)
+    gam = np.sqrt(1 + w.px ** 2 + w.py ** 2 + w.pz ** 2)
+    W = np.stack([w.q * gam, w.q * w.px, w.q * w.py, w.q * w.pz], axis=1)
+    E = np.zeros((w.N, 3)); B = np.zeros((w.N, 3))
+
+    def add(tidx, src_x, src_w):
+        d = X[tidx][:, None, :] - src_x[None, :, :]
+        D = d[..., 0] ** 2 + d[..., 1] ** 2 + g2 * d[..., 2] ** 2
+        wgt = np.where(D > 0, 1.0 / np.where(D > 0, D, 1.0) ** 1.5, 0.0)
+        g = wgt[..., None] * d
+        E[tidx] += np.einsum("ts,tsk->tk", src_w[None, :, 0] * np.ones_like(wgt), g)
+        B[tidx] += np.einsum("tsk->tk", np.cross(np.broadcast_to(src_w[None, :, 1:], g.shape), g))
+    for t, s in pp:
+        add(perm[lo[t - 1]:hi[t - 1]], X[perm[lo[s - 1]:hi[s - 1]]], W[perm[lo[s - 1]:hi[s - 1]]])
+    for t, s in pc:
+        b = bb[s - 1]
+        ax = [(b[k] + b[3 + k]) * 0.5 + (b[3 + k] - b[k]) * 0.5 * c for k in range(3)]
+        xi = np.stack(np.meshgrid(*ax, indexing="ij"), axis=-1).reshape(-1, 3)      # nu = (nu1 (n+1) + nu2)(n+1) + nu3
+        add(perm[lo[t - 1]:hi[t - 1]], xi, M[s - 1])
+    Et, Bt = p.eval_treecode()
+    assert len(pc) > 0
+    assert oracle.err2(Et, E) < 1e-13 and oracle.err2(Bt, B) < 1e-13
+    q = oracle.Plan(*w.arrays(), w.q, order_n=3, leaf_size=40, theta=0.01, raw=True)
+    assert len(q.treecode_lists()[1]) == 0
+    Ed, Bd = oracle.direct(*w.arrays(), w.q, raw=True)
+    Eq, Bq = q.eval_treecode()
+    assert oracle.err2(Eq, Ed) < 1e-13 and oracle.err2(Bq, Bd) < 1e-13
+
+
+def test_treecode_converges_and_is_at_least_as_accurate_as_the_fmm():
+    w = small(N=4096)
+    Ed, _ = oracle.direct(*w.arrays(), w.q)
+    errs = []
+    for n in (2, 4, 6):
+        p = oracle.Plan(*w.arrays(), w.q, order_n=n, leaf_size=64, theta=0.5)
+        Et, _ = p.eval_treecode()
+        Ef, _ = p.eval()
+        et, ef = oracle.err2(Et, Ed), oracle.err2(Ef, Ed)
+        errs.append(et)
+        assert et < 1.5 * ef, (n, et, ef)        # only the source side is interpolated
+    assert errs[0] > errs[1] > errs[2] and errs[2] < 1e-3
