@@ -48,6 +48,8 @@ def parse_args():
     ap.add_argument("--tree", default="kd", choices=["kd", "morton"])
     ap.add_argument("--kernel", default="mean_gamma", choices=["mean_gamma", "source_momentum"],
                     help="near-field kernel: eq. (3.2) with gamma_bar (default) or the G6 alternative (SURVEY 8(f) rank 2)")
+    ap.add_argument("--method", default="fmm", choices=["fmm", "treecode"],
+                    help="Alg 5.12 (default) or the particle-cluster treecode variant (SURVEY 8(f) rank 3)")
     ap.add_argument("--overlap", action="store_true", help="run P2P on a second stream beside the far-field chain (fmm_plan_set_overlap)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cpu-sample-leaves", type=int, default=4096,
@@ -231,6 +233,8 @@ def run_cuda(args):
     flags = fmm.FMM_TREE_KD if args.tree == "kd" else fmm.FMM_TREE_MORTON_MEDIAN
     if args.kernel == "source_momentum":
         flags |= fmm.FMM_KERNEL_SOURCE_MOMENTUM
+    if args.method == "treecode":
+        flags |= fmm.FMM_METHOD_TREECODE
     d_in = [torch.as_tensor(a).to(dev) for a in w.arrays()]
     out = torch.empty((6, w.N), dtype=torch.float64, device=dev)
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
@@ -328,7 +332,7 @@ def run_cuda(args):
     hbm = float(peaks.get("hbm_gbs", 6650.0))
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": ms_total / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-            "dtype": "f64", "data": "synthetic", "config": dict(workload_config(w, args.tree), kernel=args.kernel),
+            "dtype": "f64", "data": "synthetic", "config": dict(workload_config(w, args.tree), kernel=args.kernel, method=args.method),
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": 6 * 8 * w.N, "d2h_bytes_per_step": 6 * 8 * w.N},
             "gpu_launches": int(launches), "clocks": clocks, "roofline": roofline,
             "stages_ms": {k: round(v, 4) for k, v in stages.items()},

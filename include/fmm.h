@@ -61,6 +61,12 @@ extern "C" {
                                           D = |d|^2 + (p_j . d)^2, the exact field of a uniformly moving
                                           charge; the far field (M2L) keeps eq. (3.2) with gamma_bar      */
 
+#define FMM_METHOD_FMM      0u      /* Alg 5.12: dual tree traversal, M2L, L2L, L2P (default)              */
+#define FMM_METHOD_TREECODE 16u     /* particle-cluster variant (Fig. 1a): Alg 9.1
+                                       with the target held at a leaf; admissible clusters act on the target PARTICLES
+                                       through their proxy points (no M2L / L2L / L2P).  In the statistics and the export
+                                       the "m2l" list is then the particle-cluster list (target leaf, source cluster). */
+
 #define FMM_OK          0
 #define FMM_EINVAL     -1           /* bad argument: N < 1, order out of range, leaf_size < 1,
                                        theta <= 0 or non-finite, NULL pointer                    */
@@ -88,7 +94,7 @@ typedef struct {
     double theta;                   /* admissibility parameter eta > 0 (eq. (4.3)) */
     double gamma_bar;               /* <= 0: computed from the mean momentum;
                                        > 0: use this value                                       */
-    uint32_t flags;                 /* FMM_TREE_* | FMM_RAW_SUMS | FMM_KERNEL_*                  */
+    uint32_t flags;                 /* FMM_TREE_* | FMM_RAW_SUMS | FMM_KERNEL_* | FMM_METHOD_* */
 } fmm_params_t;
 
 /* Per-stage device times are CUDA-event times of the last fmm_plan_create/_update (tree, lists)

@@ -25,6 +25,8 @@ FMM_TREE_MORTON_MEDIAN = 1
 FMM_RAW_SUMS = 4
 FMM_KERNEL_MEAN_GAMMA = 0
 FMM_KERNEL_SOURCE_MOMENTUM = 8
+FMM_METHOD_FMM = 0
+FMM_METHOD_TREECODE = 16
 
 _dp = C.POINTER(C.c_double)
 _i64p = C.POINTER(C.c_int64)

@@ -272,6 +272,22 @@ extern "C" int fmm_plan_set_timing(fmm_plan_t *p, int on)
 extern "C" int fmm_eval(fmm_plan_t *p, double *Ex, double *Ey, double *Ez, double *Bx, double *By, double *Bz)
 {
     if (!p || !Ex || !Ey || !Ez || !Bx || !By || !Bz) return FMM_EINVAL;
+    if (p->flags & FMM_METHOD_TREECODE) {  // P2M, M2M, particle-cluster + P2P, finalise (no M2L / L2L / far L2P)
+        MARK(p, EV_P2M);
+        FMM_TRY(interp_p2m(p));
+        MARK(p, EV_M2M);
+        FMM_TRY(interp_m2m(p));
+        MARK(p, EV_M2L);
+        FMM_TRY(pairs_pc(p));
+        MARK(p, EV_L2L);
+        MARK(p, EV_P2P);
+        FMM_TRY(pairs_p2p(p));
+        MARK(p, EV_L2P);
+        FMM_TRY(interp_l2p_finalize(p, Ex, Ey, Ez, Bx, By, Bz));
+        MARK(p, EV_END);
+        if (p->timing) p->ev_valid = 1;
+        return FMM_OK;
+    }
     if (p->overlap && !p->timing) {
         // a7 does not depend on a4-a6/a8: it runs on the side stream, forked after everything already enqueued on the
         // caller's stream and joined before L2P adds near + far.  Results are identical (each kernel is deterministic).

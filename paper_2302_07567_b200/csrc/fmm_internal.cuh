@@ -106,11 +106,12 @@ int dtt_build_lists(fmm_plan *p);
 int interp_p2m(fmm_plan *p);
 int interp_m2m(fmm_plan *p);
 int interp_l2l(fmm_plan *p);
-int interp_l2p_finalize(fmm_plan *p, double *Ex, double *Ey, double *Ez, double *Bx, double *By, double *Bz);
+int interp_l2p_finalize(fmm_plan *p, /* treecode: no far interpolation, near_ has one more partial */ double *Ex, double *Ey, double *Ez, double *Bx, double *By, double *Bz);
 // ---- kernels_pairs.cu ---------------------------------------------------------------
 int pairs_p2p(fmm_plan *p);
 int pairs_p2p_prepare(fmm_plan *p);
 int pairs_m2l(fmm_plan *p);
+int pairs_pc(fmm_plan *p);   // treecode: particle-cluster sums
 int pairs_direct(fmm_ctx *c, int64_t N, const double *x, const double *y, const double *z,
                  const double *w0, const double *w1, const double *w2, const double *w3,
                  const double *px, const double *py, const double *pz /* non-NULL: source-momentum kernel */,

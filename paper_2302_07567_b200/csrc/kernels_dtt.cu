@@ -15,14 +15,18 @@ struct dtt_counters {           // device
     unsigned int n_front[72];   // frontier sizes per step (at most 2*kappa+2 steps)
 };
 
-__global__ void dtt_init(dtt_counters *cnt, uint64_t *front0)
+__global__ void dtt_init(dtt_counters *cnt, uint64_t *front0, int treecode_leaves)
 {
-    if (threadIdx.x == 0 && blockIdx.x == 0) {
+    // FMM: the traversal starts at (root, root).  Treecode (FMM_METHOD_TREECODE): at (t, root) for every leaf t, so
+    // the target is never split and the "m2l" list becomes the particle-cluster list.
+    int k0 = blockIdx.x * blockDim.x + threadIdx.x;
+    if (k0 == 0) {
         cnt->n_p2p = cnt->n_m2l = cnt->overflow = cnt->pad = 0;
         for (int k = 0; k < 72; ++k) cnt->n_front[k] = 0;
-        cnt->n_front[0] = 1;
-        front0[0] = (1ull << 32) | 1ull;  // (root, root)
+        cnt->n_front[0] = treecode_leaves > 0 ? (unsigned)treecode_leaves : 1u;
+        if (treecode_leaves <= 0) front0[0] = (1ull << 32) | 1ull;  // (root, root)
     }
+    if (k0 < treecode_leaves) front0[k0] = ((uint64_t)(treecode_leaves + k0) << 32) | 1ull;  // (leaf, root)
 }
 
 __global__ void __launch_bounds__(256) dtt_step(int step, int leaves, double gamma_bar, double theta2,
@@ -162,7 +166,8 @@ int dtt_build_lists(fmm_plan *p)
         kp2p = (uint64_t *)ctx_alloc(c, sizeof(uint64_t) * cap);
         km2l = (uint64_t *)ctx_alloc(c, sizeof(uint64_t) * cap);
         if (!f0 || !f1 || !kp2p || !km2l) return FMM_ENOMEM;
-        dtt_init<<<1, 32, 0, st>>>(cnt, f0);
+        const int tc_leaves = (p->flags & FMM_METHOD_TREECODE) ? (int)p->leaves : 0;
+        dtt_init<<<tc_leaves > 0 ? (tc_leaves + 255) / 256 : 1, 256, 0, st>>>(cnt, f0, tc_leaves);
         FMM_LAUNCH_CHECK(c, "dtt_init");
         uint64_t *fin = f0, *fout = f1;
         for (int step = 0; step < nsteps; ++step) {
@@ -208,7 +213,8 @@ int dtt_build_lists(fmm_plan *p)
     FMM_CUDA(c, cudaStreamSynchronize(st));
     p->p2p_pairs = (int64_t)total_h2[0];
     p->p2p_max_row = (int64_t)total_h2[1];
-    p->m2l_pairs = p->n_m2l * (int64_t)p->P * (int64_t)p->P;
+    p->m2l_pairs = (p->flags & FMM_METHOD_TREECODE) ? p->n_m2l * (int64_t)p->P * ((p->N + p->leaves - 1) / p->leaves)  // particle-proxy pairs (full leaves)
+                                                    : p->n_m2l * (int64_t)p->P * (int64_t)p->P;
     ctx_free(c, cnt);
     return FMM_OK;
 }

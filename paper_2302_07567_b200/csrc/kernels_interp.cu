@@ -289,7 +289,7 @@ __global__ void __launch_bounds__(L2P_THREADS) l2p_kernel(int n, cheb_t ch, int 
                                                           const int32_t *__restrict__ node_hi, const double *__restrict__ bbox,
                                                           const double *__restrict__ tx, const double *__restrict__ ty,
                                                           const double *__restrict__ tz, const double *__restrict__ L,
-                                                          const double *__restrict__ near_, int K, const int32_t *__restrict__ perm,
+                                                          const double *__restrict__ near_, int K, int skip_far, const int32_t *__restrict__ perm,
                                                           double cE, double cB, double *__restrict__ Ex, double *__restrict__ Ey,
                                                           double *__restrict__ Ez, double *__restrict__ Bx, double *__restrict__ By,
                                                           double *__restrict__ Bz)
@@ -302,7 +302,8 @@ __global__ void __launch_bounds__(L2P_THREADS) l2p_kernel(int n, cheb_t ch, int 
     int lo = node_lo[node], hi = node_hi[node];
     const double *bb = bbox + 6 * (int64_t)node;
     const double *Ln = L + (int64_t)P6 * node;
-    for (int e = threadIdx.x; e < P6; e += L2P_THREADS) Ls[e] = Ln[e];
+    if (!skip_far)
+        for (int e = threadIdx.x; e < P6; e += L2P_THREADS) Ls[e] = Ln[e];
     __syncthreads();
     for (int k = lo + threadIdx.x; k < hi; k += L2P_THREADS) {
         double *lx = bas + threadIdx.x, *ly = lx + n1 * L2P_THREADS, *lz = ly + n1 * L2P_THREADS;
@@ -310,7 +311,7 @@ __global__ void __launch_bounds__(L2P_THREADS) l2p_kernel(int n, cheb_t ch, int 
         basis_1d(n, ch, bb[1], bb[4], ty[k], ly, L2P_THREADS);
         basis_1d(n, ch, bb[2], bb[5], tz[k], lz, L2P_THREADS);
         double fx[6] = {0, 0, 0, 0, 0, 0};
-        for (int a = 0; a < n1; ++a) {
+        for (int a = 0; a < (skip_far ? 0 : n1); ++a) {
             double fy[6] = {0, 0, 0, 0, 0, 0};
             for (int b = 0; b < n1; ++b) {
                 double fz[6] = {0, 0, 0, 0, 0, 0};
@@ -425,7 +426,8 @@ int interp_l2p_finalize(fmm_plan *p, double *Ex, double *Ey, double *Ez, double 
     size_t smem = sizeof(double) * (6 * (size_t)p->P + 3 * (size_t)p->n1 * L2P_THREADS);
     FMM_TRY(set_smem(c, (const void *)l2p_kernel, smem));
     l2p_kernel<<<(unsigned)p->leaves, L2P_THREADS, smem, c->stream>>>(p->n, ch, (int)p->leaves, (int)p->N, p->node_lo, p->node_hi, p->bbox,
-                                                                      p->tx, p->ty, p->tz, p->L, p->near_, p->p2p_split, p->perm, cE, cB, Ex, Ey, Ez,
+                                                                      p->tx, p->ty, p->tz, p->L, p->near_, p->p2p_split + ((p->flags & FMM_METHOD_TREECODE) ? 1 : 0),
+                                                                      (p->flags & FMM_METHOD_TREECODE) ? 1 : 0, p->perm, cE, cB, Ex, Ey, Ez,
                                                                       Bx, By, Bz);
     FMM_LAUNCH_CHECK(c, "l2p_kernel");
     return FMM_OK;

@@ -190,7 +190,7 @@ int pairs_p2p_prepare(fmm_plan *p)  // after the lists: choose the row split and
     int nt, threads, K;
     p2p_shape(p->leaves, maxleaf, p->p2p_pairs, p->p2p_max_row, &nt, &threads, &K);
     p->p2p_split = K;
-    int64_t need = (int64_t)K * 6 * p->N;
+    int64_t need = (int64_t)(K + ((p->flags & FMM_METHOD_TREECODE) ? 1 : 0)) * 6 * p->N;  // treecode: + the particle-cluster sums
     if (need > p->near_cap) {
         if (p->near_) ctx_free(c, p->near_);
         p->near_ = (double *)ctx_alloc(c, sizeof(double) * (size_t)need);
@@ -599,6 +599,71 @@ static int launch_m2l(fmm_plan *p)
     return FMM_OK;
 }
 
+// ---------------------------------------------------------------------------------------
+// Treecode variant (FMM_METHOD_TREECODE): particle-cluster interaction.  One block per target leaf, NT target
+// particles per thread as in P2P; the "source particles" of a cluster are its (n+1)^3 proxy points with the moments
+// M as weights (eq. (2.5) with the target side not interpolated; mean-gamma kernel of eq. (3.2)).  The sums go to
+// partial buffer `slot` of near_, which L2P adds to the P2P partials in a fixed order.
+// ---------------------------------------------------------------------------------------
+template <int NT>
+__global__ void __launch_bounds__(256) pc_kernel(int N, int n1, double gb, const int32_t *__restrict__ order, const int32_t *__restrict__ off,
+                                                 const int32_t *__restrict__ src, const int32_t *__restrict__ node_lo,
+                                                 const int32_t *__restrict__ node_hi, const double *__restrict__ tx,
+                                                 const double *__restrict__ ty, const double *__restrict__ tz,
+                                                 const double *__restrict__ xi, const double *__restrict__ M, int slot, int leaves,
+                                                 double *__restrict__ near_)
+{
+    __shared__ double2 tile[4 * PAIR_TILE];
+    const int t = order[blockIdx.x];
+    if (t < leaves) return;  // only leaves are targets
+    const int tlo = node_lo[t], thi = node_hi[t];
+    const int e0 = off[t], e1 = off[t + 1];
+    const int P = n1 * n1 * n1;
+    for (int i0 = tlo; i0 < thi; i0 += NT * blockDim.x) {
+        double xt[NT], yt[NT], zt[NT], ex[NT], ey[NT], ez[NT], bx[NT], by[NT], bz[NT];
+#pragma unroll
+        for (int k = 0; k < NT; ++k) {
+            int i = i0 + k * blockDim.x + threadIdx.x;
+            bool live = i < thi;
+            xt[k] = live ? tx[i] : 0.0; yt[k] = live ? ty[i] : 0.0; zt[k] = live ? tz[i] : 0.0;
+            ex[k] = ey[k] = ez[k] = bx[k] = by[k] = bz[k] = 0.0;
+        }
+        for (int e = e0; e < e1; ++e) {
+            const int s = src[e];
+            const double *xs = xi + (size_t)s * 3 * M2L_XI_STRIDE;
+            const double z0 = xs[2 * M2L_XI_STRIDE + M2L_XI_STRIDE - 1];
+            const double2 *Ms = reinterpret_cast<const double2 *>(M + 4 * (size_t)P * s);
+            for (int j0 = 0; j0 < P; j0 += PAIR_TILE) {
+                const int count = min(PAIR_TILE, P - j0);
+                __syncthreads();
+                for (int j = threadIdx.x; j < count; j += blockDim.x) {  // proxy nu = (a n1 + b) n1 + c as a source particle
+                    const int nu = j0 + j, a = nu / (n1 * n1), b = (nu / n1) % n1, c = nu % n1;
+                    const double2 m01 = Ms[2 * nu], m23 = Ms[2 * nu + 1];
+                    tile[4 * j + 0] = make_double2(xs[a], xs[M2L_XI_STRIDE + b]);
+                    tile[4 * j + 1] = make_double2(__dadd_rn(z0, xs[2 * M2L_XI_STRIDE + c]), m01.x);
+                    tile[4 * j + 2] = make_double2(m01.y, m23.x);
+                    tile[4 * j + 3] = make_double2(m23.y, 0.0);
+                }
+                __syncthreads();
+                tile_interact<NT, false>(tile, count, xt, yt, zt, gb, ex, ey, ez, bx, by, bz);
+            }
+        }
+#pragma unroll
+        for (int k = 0; k < NT; ++k) {
+            int i = i0 + k * blockDim.x + threadIdx.x;
+            if (i < thi) {
+                double *o = near_ + (size_t)slot * 6 * (size_t)N + i;
+                o[0] = ex[k];
+                o[(size_t)N] = ey[k];
+                o[2 * (size_t)N] = ez[k];
+                o[3 * (size_t)N] = bx[k];
+                o[4 * (size_t)N] = by[k];
+                o[5 * (size_t)N] = bz[k];
+            }
+        }
+    }
+}
+
 static int m2l_upload_cheb(fmm_ctx *c)
 {
     static std::atomic<int> done_on[64];  // __constant__ memory is per device
@@ -649,4 +714,33 @@ int pairs_m2l(fmm_plan *p)
         case 13: return launch_m2l<13>(p);
     }
     return FMM_EINVAL;
+}
+
+int pairs_pc(fmm_plan *p)  // treecode: particle-cluster sums into partial buffer p2p_split
+{
+    fmm_ctx *c = &p->ctx;
+    cheb13 ch;
+    memset(&ch, 0, sizeof(ch));
+    for (int k = 0; k <= p->n; ++k) ch.c[k] = sin(FMM_PI * (double)(p->n - 2 * k) / (double)(2 * p->n));  // I-1
+    ch.c[0] = 1.0;
+    ch.c[p->n] = -1.0;
+    int count = (int)(p->nodes + 1) * 3 * M2L_XI_STRIDE;
+    m2l_proxy_points<<<(count + 255) / 256, 256, 0, c->stream>>>((int)p->nodes, p->n1, ch, p->bbox, p->node_xi);
+    FMM_LAUNCH_CHECK(c, "m2l_proxy_points");
+    int maxleaf = (int)((p->N + p->leaves - 1) / p->leaves);
+    int nt, threads, K;
+    p2p_shape(p->leaves, maxleaf, p->p2p_pairs, p->p2p_max_row, &nt, &threads, &K);
+#define PC_LAUNCH(NT)                                                                                                            \
+    pc_kernel<NT><<<(unsigned)p->nodes, threads, 0, c->stream>>>((int)p->N, p->n1, p->gamma_bar, p->m2l_order, p->m2l_off, p->m2l_src, \
+                                                                 p->node_lo, p->node_hi, p->tx, p->ty, p->tz, p->node_xi, p->M,  \
+                                                                 p->p2p_split, (int)p->leaves, p->near_)
+    switch (nt) {
+        case 1: PC_LAUNCH(1); break;
+        case 2: PC_LAUNCH(2); break;
+        case 3: PC_LAUNCH(3); break;
+        default: PC_LAUNCH(4); break;
+    }
+#undef PC_LAUNCH
+    FMM_LAUNCH_CHECK(c, "pc_kernel");
+    return FMM_OK;
 }

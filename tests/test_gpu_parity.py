@@ -307,3 +307,46 @@ def test_overlap_is_bit_identical_to_serial_and_stable(fmm):
             E, B = plan.eval()
             assert torch.equal(E, E0) and torch.equal(B, B0), f"overlap={ov}: result changed between evaluations"
     plan.close()
+
+
+# ---------------------------------------------------------------------------------------------
+# FMM_METHOD_TREECODE: particle-cluster variant (Fig. 1a)
+# ---------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("case", [c for c in CASES if c[0] in ("config1", "config2_ragged", "config3_small_n3", "config4_small",
+                                                              "paper_cube_n2", "order8", "single_leaf", "three_particles")],
+                         ids=lambda c: c[0])
+def test_treecode_matches_oracle(fmm, case):
+    _, w, n, N0, theta = case
+    plan = fmm.fmm_plan_create(*w.arrays(), w.q, order_n=n, leaf_size=N0, theta=theta,
+                               flags=fmm.FMM_TREE_KD | fmm.FMM_METHOD_TREECODE)
+    st = plan.stats()
+    ex = plan.export()
+    op = oracle.Plan(*w.arrays(), w.q, order_n=n, leaf_size=N0, theta=theta, gamma_bar_value=st["gamma_bar"])
+    assert np.array_equal(ex["perm"], op.perm())
+    pp, pc = op.treecode_lists()
+    assert st["n_p2p"] == len(pp) and st["n_m2l"] == len(pc)
+    for name, ref in (("p2p", pp), ("m2l", pc)):          # "m2l" slots carry the particle-cluster list in this mode
+        off, src = ex[name + "_off"], ex[name + "_src"]
+        tgt = np.repeat(np.arange(1, st["nodes"] + 1, dtype=np.int32), np.diff(off))
+        assert np.array_equal(tgt, ref[:, 0]) and np.array_equal(src, ref[:, 1]), f"{name} list differs"
+    E, B = to_np(plan.eval())
+    Eo, Bo = op.eval_treecode()
+    assert_close(E, Eo, "treecode E")
+    assert_close(B, Bo, "treecode B")
+    E2, B2 = to_np(plan.eval())
+    assert np.array_equal(E, E2) and np.array_equal(B, B2)
+    plan.close()
+
+
+def test_treecode_cross_checks_the_fmm(fmm):
+    """Two independently structured approximations of the same sum agree at the level of their error against it."""
+    w = workloads.config(2, N=30000)
+    kw = dict(order_n=6, leaf_size=128, theta=0.5)
+    a = fmm.fmm_plan_create(*w.arrays(), w.q, **kw)
+    b = fmm.fmm_plan_create(*w.arrays(), w.q, flags=fmm.FMM_METHOD_TREECODE, **kw)
+    Ea, _ = to_np(a.eval())
+    Eb, _ = to_np(b.eval())
+    Ed, _ = to_np(fmm.fmm_direct(*w.arrays(), w.q, gamma_bar=a.stats()["gamma_bar"]))
+    ea, eb = oracle.err2(Ea, Ed), oracle.err2(Eb, Ed)
+    assert eb < 1.5 * ea and oracle.err2(Ea, Eb) < 2 * ea, (ea, eb)
+    a.close(); b.close()
