@@ -171,12 +171,13 @@ __device__ __forceinline__ void transfer_matrices(int n, const cheb_t &ch, const
 // ---------------------------------------------------------------------------------------
 #define XFER_THREADS 256
 
-__global__ void __launch_bounds__(XFER_THREADS) m2m_kernel(int n, cheb_t ch, int first, const int32_t *__restrict__ node_lo,
+template <int N1>
+__global__ void __launch_bounds__(XFER_THREADS) m2m_kernel(cheb_t ch, int first, const int32_t *__restrict__ node_lo,
                                                            const int32_t *__restrict__ node_hi, const double *__restrict__ bbox,
                                                            double *__restrict__ M)
 {
     extern __shared__ double sm[];
-    const int n1 = n + 1, P = n1 * n1 * n1, P4 = 4 * P;
+    constexpr int n = N1 - 1, n1 = N1, P = n1 * n1 * n1, P4 = 4 * P;  // compile-time order: index arithmetic without integer division
     double *T = sm;                   // [3][n1][n1]
     double *A = sm + 3 * n1 * n1;     // [P][4]
     double *B = A + P4;               // [P][4]
@@ -237,12 +238,13 @@ __global__ void __launch_bounds__(XFER_THREADS) m2m_kernel(int n, cheb_t ch, int
 // a8: L2L for one level.  One block per child S' (parent S = S'/2):
 //   L_S'[a',b',c'] += sum_{a,b,c} Tx[a][a'] Ty[b][b'] Tz[c][c'] L_S[a,b,c]
 // ---------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(XFER_THREADS) l2l_kernel(int n, cheb_t ch, int first, const int32_t *__restrict__ node_lo,
+template <int N1>
+__global__ void __launch_bounds__(XFER_THREADS) l2l_kernel(cheb_t ch, int first, const int32_t *__restrict__ node_lo,
                                                            const int32_t *__restrict__ node_hi, const double *__restrict__ bbox,
                                                            double *__restrict__ L)
 {
     extern __shared__ double sm[];
-    const int n1 = n + 1, P = n1 * n1 * n1, P6 = 6 * P;
+    constexpr int n = N1 - 1, n1 = N1, P = n1 * n1 * n1, P6 = 6 * P;
     double *T = sm;
     double *A = sm + 3 * n1 * n1;  // [P][6]
     double *B = A + P6;
@@ -285,7 +287,8 @@ __global__ void __launch_bounds__(XFER_THREADS) l2l_kernel(int n, cheb_t ch, int
 // ---------------------------------------------------------------------------------------
 #define L2P_THREADS 128
 
-__global__ void __launch_bounds__(L2P_THREADS) l2p_kernel(int n, cheb_t ch, int leaves, int N, const int32_t *__restrict__ node_lo,
+template <int N1>
+__global__ void __launch_bounds__(L2P_THREADS) l2p_kernel(cheb_t ch, int leaves, int N, const int32_t *__restrict__ node_lo,
                                                           const int32_t *__restrict__ node_hi, const double *__restrict__ bbox,
                                                           const double *__restrict__ tx, const double *__restrict__ ty,
                                                           const double *__restrict__ tz, const double *__restrict__ L,
@@ -295,7 +298,7 @@ __global__ void __launch_bounds__(L2P_THREADS) l2p_kernel(int n, cheb_t ch, int 
                                                           double *__restrict__ Bz)
 {
     extern __shared__ double sm[];
-    const int n1 = n + 1, P = n1 * n1 * n1, P6 = 6 * P;
+    constexpr int n = N1 - 1, n1 = N1, P = n1 * n1 * n1, P6 = 6 * P;
     double *Ls = sm;                 // [P][6]
     double *bas = sm + P6;           // [3][n1][L2P_THREADS]
     int node = leaves + blockIdx.x;
@@ -386,15 +389,32 @@ int interp_p2m(fmm_plan *p)
     return FMM_EINVAL;
 }
 
+// kernels templated on N1 = n + 1: dispatch on the plan's order
+#include <type_traits>
+template <typename F>
+static int dispatch_n1(int n1, F &&f)
+{
+    switch (n1) {
+#define INTERP_CASE(K) case K: return f(std::integral_constant<int, K>{});
+        INTERP_CASE(2) INTERP_CASE(3) INTERP_CASE(4) INTERP_CASE(5) INTERP_CASE(6) INTERP_CASE(7) INTERP_CASE(8)
+        INTERP_CASE(9) INTERP_CASE(10) INTERP_CASE(11) INTERP_CASE(12) INTERP_CASE(13)
+#undef INTERP_CASE
+    }
+    return FMM_EINVAL;
+}
+
 int interp_m2m(fmm_plan *p)
 {
     fmm_ctx *c = &p->ctx;
     cheb_t ch = host_cheb(p->n);
     size_t smem = sizeof(double) * (3 * (size_t)p->n1 * p->n1 + 8 * (size_t)p->P);
-    FMM_TRY(set_smem(c, (const void *)m2m_kernel, smem));
+    FMM_TRY(dispatch_n1(p->n1, [&](auto k) { return set_smem(c, (const void *)m2m_kernel<decltype(k)::value>, smem); }));
     for (int level = p->kappa - 1; level >= 0; --level) {
         int first = 1 << level;
-        m2m_kernel<<<first, XFER_THREADS, smem, c->stream>>>(p->n, ch, first, p->node_lo, p->node_hi, p->bbox, p->M);
+        FMM_TRY(dispatch_n1(p->n1, [&](auto k) {
+            m2m_kernel<decltype(k)::value><<<first, XFER_THREADS, smem, c->stream>>>(ch, first, p->node_lo, p->node_hi, p->bbox, p->M);
+            return FMM_OK;
+        }));
         FMM_LAUNCH_CHECK(c, "m2m_kernel");
     }
     return FMM_OK;
@@ -405,10 +425,13 @@ int interp_l2l(fmm_plan *p)
     fmm_ctx *c = &p->ctx;
     cheb_t ch = host_cheb(p->n);
     size_t smem = sizeof(double) * (3 * (size_t)p->n1 * p->n1 + 12 * (size_t)p->P);
-    FMM_TRY(set_smem(c, (const void *)l2l_kernel, smem));
+    FMM_TRY(dispatch_n1(p->n1, [&](auto k) { return set_smem(c, (const void *)l2l_kernel<decltype(k)::value>, smem); }));
     for (int level = 1; level <= p->kappa; ++level) {
         int first = 1 << level;
-        l2l_kernel<<<first, XFER_THREADS, smem, c->stream>>>(p->n, ch, first, p->node_lo, p->node_hi, p->bbox, p->L);
+        FMM_TRY(dispatch_n1(p->n1, [&](auto k) {
+            l2l_kernel<decltype(k)::value><<<first, XFER_THREADS, smem, c->stream>>>(ch, first, p->node_lo, p->node_hi, p->bbox, p->L);
+            return FMM_OK;
+        }));
         FMM_LAUNCH_CHECK(c, "l2l_kernel");
     }
     return FMM_OK;
@@ -424,11 +447,15 @@ int interp_l2p_finalize(fmm_plan *p, double *Ex, double *Ey, double *Ez, double 
         cB = 1.0 / (4.0 * FMM_PI * FMM_EPS0 * FMM_C0);
     }
     size_t smem = sizeof(double) * (6 * (size_t)p->P + 3 * (size_t)p->n1 * L2P_THREADS);
-    FMM_TRY(set_smem(c, (const void *)l2p_kernel, smem));
-    l2p_kernel<<<(unsigned)p->leaves, L2P_THREADS, smem, c->stream>>>(p->n, ch, (int)p->leaves, (int)p->N, p->node_lo, p->node_hi, p->bbox,
-                                                                      p->tx, p->ty, p->tz, p->L, p->near_, p->p2p_split + ((p->flags & FMM_METHOD_TREECODE) ? 1 : 0),
-                                                                      (p->flags & FMM_METHOD_TREECODE) ? 1 : 0, p->perm, cE, cB, Ex, Ey, Ez,
-                                                                      Bx, By, Bz);
+    FMM_TRY(dispatch_n1(p->n1, [&](auto k) { return set_smem(c, (const void *)l2p_kernel<decltype(k)::value>, smem); }));
+    const int nparts = p->p2p_split + ((p->flags & FMM_METHOD_TREECODE) ? 1 : 0);
+    const int skip_far = (p->flags & FMM_METHOD_TREECODE) ? 1 : 0;
+    FMM_TRY(dispatch_n1(p->n1, [&](auto k) {
+        l2p_kernel<decltype(k)::value><<<(unsigned)p->leaves, L2P_THREADS, smem, c->stream>>>(
+            ch, (int)p->leaves, (int)p->N, p->node_lo, p->node_hi, p->bbox, p->tx, p->ty, p->tz, p->L, p->near_, nparts, skip_far, p->perm,
+            cE, cB, Ex, Ey, Ez, Bx, By, Bz);
+        return FMM_OK;
+    }));
     FMM_LAUNCH_CHECK(c, "l2p_kernel");
     return FMM_OK;
 }
