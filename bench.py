@@ -78,7 +78,14 @@ def oracle_step(w, tree, sample_leaves):
     op.upward()
     t2 = time.perf_counter()
     S = max(1, min(sample_leaves, op.leaves))
-    sel = (op.leaves + (np.arange(S) * op.leaves) // S).astype(np.int64)
+    # the sample is 8 evenly spaced runs of contiguous leaves (whole sub-trees): the M2L work of their ancestor chains
+    # then scales with the sample like the leaf work does (single evenly spaced leaves would pull in almost every
+    # upper-level node and overstate the extrapolated time)
+    runs = min(8, S)
+    per = S // runs
+    S = per * runs
+    starts = (np.arange(runs) * op.leaves) // runs
+    sel = (op.leaves + (starts[:, None] + np.arange(per)[None, :]).ravel()).astype(np.int64)
     op.eval(leaves=sel)
     t3 = time.perf_counter()
     full = (t1 - t0) + (t2 - t1) + (t3 - t2) * (op.leaves / S)
