@@ -337,12 +337,28 @@ def run_cuda(args):
                 "p2p": {"evals": evals["p2p"], "ms": stages["p2p"], "tflops": ach["p2p"], "frac": ach["p2p"] / nominal},
                 "m2l": {"evals": evals["m2l"], "ms": stages["m2l"], "tflops": ach["m2l"], "frac": ach["m2l"] / nominal}}
     hbm = float(peaks.get("hbm_gbs", 6650.0))
+    # HBM-side rooflines of the tree / interpolation stages (north_star): ALGORITHMIC bytes (every array a
+    # stage must read or write once) over the stage's CUDA-event time, against the measured copy bandwidth.  These stages are
+    # launch- and latency-bound at N = 2^20 (a few MB to a few hundred MB per stage), so the fractions are small by nature.
+    Pn = (w.order_n + 1) ** 3
+    nodes, leaves_n = st["nodes"], st["leaves"]
+    stage_bytes = {
+        "tree": 128 * w.N,                                              # read x, p (48 B) + write tree-ordered x, weights, perm (60 B) + slack
+        "lists": 8 * (st["n_p2p"] + st["n_m2l"]) * 3,                   # 64-bit pair keys: emit, sort, CSR
+        "p2m": 56 * w.N + 32 * Pn * leaves_n,
+        "m2m": 32 * Pn * ((nodes - 1) + (nodes - leaves_n)),             # read every child once, write every parent once
+        "l2l": 48 * Pn * (nodes - 1) * 2 + 48 * Pn * (nodes - leaves_n),  # read parent + child, write child
+        "l2p": 48 * Pn * leaves_n + (24 + 48 * st.get("p2p_split", 1) + 4 + 48) * w.N,
+    }
+    stage_roof = {k: {"bytes": int(b), "gbs": round(b / (stages[k] * 1e-3) / 1e9, 1), "frac_of_hbm_peak": round(b / (stages[k] * 1e-3) / 1e9 / hbm, 4)}
+                  for k, b in stage_bytes.items() if stages.get(k, 0) > 0}
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": ms_total / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f64", "data": "synthetic", "config": dict(workload_config(w, args.tree), kernel=args.kernel, method=args.method),
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": 6 * 8 * w.N, "d2h_bytes_per_step": 6 * 8 * w.N},
             "gpu_launches": int(launches), "clocks": clocks, "roofline": roofline,
             "stages_ms": {k: round(v, 4) for k, v in stages.items()},
+            "stages_hbm": stage_roof,
             "stage_timing": ("per-stage CUDA events of a second pass of the same K steps in serial stage order "
                              f"({ms_serial:.3f} ms/step); the timed region runs P2P on a second stream beside P2M/M2M/M2L/L2L"
                              if ms_serial is not None else "per-stage CUDA events inside the timed region (serial stage order)"),
