@@ -352,6 +352,12 @@ struct m2l_cfg {
     static constexpr int STAGE_BYTES = 32 * P + 3 * 16 * 8;
     static constexpr int FIT = (227 * 1024 - 64) / STAGE_BYTES;
     static constexpr int STAGES = FIT >= 3 ? 3 : (FIT >= 2 ? 2 : 1);
+    // Helper warp: WARPS consumer warps with WARPS % 4 == 3 (11 at n = 6) cannot be spread evenly over the four SM
+    // sub-partitions.  One more consumer warp takes, for source e, the target group e mod (WARPS + 1) off its owner
+    // (nothing when that is WARPS), so all WARPS + 1 warps do the same (WARPS / (WARPS + 1)) share of the work.
+    static constexpr bool HELP = (NT == 1) && (BATCHES == 1) && ((THREADS / 32) % 4 == 3);
+    static constexpr int CWARPS = THREADS / 32 + (HELP ? 1 : 0);       // consumer warps
+    static constexpr int BLOCK = 32 * CWARPS + (HELP ? 0 : 32);        // + a producer warp (with a helper, the helper also refills the ring)
 };
 
 struct cheb13 {
@@ -389,6 +395,20 @@ __device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity)
         : "memory");
 }
 
+__device__ __forceinline__ bool mbar_test(uint64_t *bar, uint32_t parity)  // non-blocking
+{
+    uint32_t ok;
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "mbarrier.test_wait.parity.shared::cta.b64 p, [%1], %2;\n"
+        "selp.u32 %0, 1, 0, p;\n"
+        "}\n"
+        : "=r"(ok)
+        : "r"(smem_u32(bar)), "r"(parity)
+        : "memory");
+    return ok != 0;
+}
 __device__ __forceinline__ void mbar_arrive(uint64_t *bar)
 {
     asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
@@ -430,156 +450,196 @@ __global__ void m2l_proxy_points(int nodes, int n1, cheb13 ch, const double *__r
 // stage's `full` mbarrier.  There is no block-wide barrier in the source loop: every warp walks the CSR row at its
 // own pace, waits on full[stage], and releases the stage on empty[stage] (one arrival per warp); an extra producer
 // warp refills a stage as soon as all consumer warps have left it, so warps may drift up to STAGES-1 sources apart.
+// one source node (stage in shared memory) acting on one target proxy point per thread
+struct m2l_no_poll {
+    __device__ __forceinline__ void operator()() const {}
+};
+template <int N1, typename Poll>
+__device__ __forceinline__ void m2l_source(const double2 *__restrict__ Ms, const double *__restrict__ xs, double g2, double xt, double yt,
+                                           double zt, double &ex, double &ey, double &ez, double &bx, double &by, double &bz, Poll poll)
+{
+    const double ztr = zt - xs[2 * M2L_XI_STRIDE + M2L_XI_STRIDE - 1];  // target z relative to the source box centre
+    double gz2[N1];
+#pragma unroll
+    for (int c = 0; c < N1; ++c) {
+        const double dz = ztr - xs[2 * M2L_XI_STRIDE + c];
+        gz2[c] = (g2 * dz) * dz;
+    }
+    double S0 = 0, S1 = 0, S2 = 0;  // sum over this source of m_k (c_{nu3} w)
+    for (int a2 = 0; a2 < N1; ++a2) {
+        poll();  // (helper warp: refill a released stage; nothing for the other warps)
+        const double dx = xt - xs[a2];
+        const double dx2 = dx * dx;
+#pragma unroll 1
+        for (int b2 = 0; b2 < N1; ++b2) {
+            const double2 *row = Ms + 2 * ((a2 * N1 + b2) * N1);
+            const double dy = yt - xs[M2L_XI_STRIDE + b2];
+            const double s2 = fma(dy, dy, dx2);
+            double A0 = 0, A1 = 0, A2 = 0, A3 = 0;
+#pragma unroll
+            for (int c2 = 0; c2 < N1; ++c2) {
+                const double2 m01 = row[2 * c2], m23 = row[2 * c2 + 1];
+                const double w = inv_r3(s2 + gz2[c2]);
+                A0 = fma(m01.x, w, A0);
+                A1 = fma(m01.y, w, A1);
+                A2 = fma(m23.x, w, A2);
+                A3 = fma(m23.y, w, A3);
+                if (c2 == 0 || c2 == N1 - 1 || 2 * c2 != N1 - 1) {  // c_k = 0 at the middle point of an even order
+                    const double u = (c2 == 0) ? w : (c2 == N1 - 1) ? -w : w * m2l_cheb_c[N1][c2];
+                    S0 = fma(m01.x, u, S0);
+                    S1 = fma(m01.y, u, S1);
+                    S2 = fma(m23.x, u, S2);
+                }
+            }
+            // sum m_k w dz = ztr sum m_k w - h_z sum m_k c w:  E_z += Z0,  B_x += Z2,  B_y -= Z1
+            ex = fma(A0, dx, ex);
+            ey = fma(A0, dy, ey);
+            ez = fma(A0, ztr, ez);
+            bx = fma(-A3, dy, fma(A2, ztr, bx));
+            by = fma(A3, dx, fma(-A1, ztr, by));
+            bz = fma(A1, dy, fma(-A2, dx, bz));
+        }
+    }
+    const double hz = xs[2 * M2L_XI_STRIDE + M2L_XI_STRIDE - 2];
+    ez = fma(-hz, S0, ez);
+    bx = fma(-hz, S2, bx);
+    by = fma(hz, S1, by);
+}
+
 template <int N1>
-__global__ void __launch_bounds__(m2l_cfg<N1>::THREADS + 32, m2l_cfg<N1>::MINB) m2l_kernel(double g2, const int32_t *__restrict__ order,
-                                                                                      const int32_t *__restrict__ off, const int32_t *__restrict__ src,
-                                                                                      const double *__restrict__ xi, const double *__restrict__ M, double *__restrict__ L)
+__global__ void __launch_bounds__(m2l_cfg<N1>::BLOCK, m2l_cfg<N1>::MINB) m2l_kernel(double g2, const int32_t *__restrict__ order,
+                                                                                  const int32_t *__restrict__ off, const int32_t *__restrict__ src,
+                                                                                  const double *__restrict__ xi, const double *__restrict__ M, double *__restrict__ L)
 {
     constexpr int P = m2l_cfg<N1>::P;
-    constexpr int THREADS = m2l_cfg<N1>::THREADS;
+    constexpr int THREADS = m2l_cfg<N1>::THREADS;   // threads that own target proxy points
     constexpr int WARPS = THREADS / 32;
+    constexpr bool HELP = m2l_cfg<N1>::HELP;
+    constexpr int CWARPS = m2l_cfg<N1>::CWARPS;
+    constexpr int CTHREADS = 32 * CWARPS;
     constexpr int S = m2l_cfg<N1>::STAGES;
     constexpr uint32_t TILE_BYTES = 32u * P;
     constexpr uint32_t STAGE_BYTES = TILE_BYTES + M2L_XI_BYTES;
     extern __shared__ __align__(128) unsigned char m2l_smem_raw[];
     uint64_t *full = reinterpret_cast<uint64_t *>(m2l_smem_raw + S * STAGE_BYTES);
     uint64_t *empty = full + S;
+    double *hacc = reinterpret_cast<double *>(m2l_smem_raw + S * STAGE_BYTES + 2 * S * sizeof(uint64_t));  // [THREADS][6], HELP only
     const int t = order[blockIdx.x];
     const int e0 = off[t], e1 = off[t + 1];
     double *Lt = L + 6 * (size_t)P * t;
     if (e0 == e1) {  // no far-field sources: the local expansion starts at zero (L2L adds into it)
-        for (int k = threadIdx.x; k < 6 * P; k += THREADS + 32) Lt[k] = 0.0;
+        for (int k = threadIdx.x; k < 6 * P; k += m2l_cfg<N1>::BLOCK) Lt[k] = 0.0;
         return;
     }
     if (threadIdx.x == 0) {
         for (int k = 0; k < S; ++k) {
             mbar_init(&full[k], 1);
-            mbar_init(&empty[k], WARPS);
+            mbar_init(&empty[k], CWARPS);
         }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     __syncthreads();
     const int ne = e1 - e0;
     const int total = m2l_cfg<N1>::BATCHES * ne;  // loads in the order they are consumed
-    auto issue = [&](int q) {                     // thread 0 only
-        const int st = q % S;
-        const int sn = src[e0 + q % ne];
-        unsigned char *dst = m2l_smem_raw + (size_t)st * STAGE_BYTES;
-        mbar_expect_tx(&full[st], STAGE_BYTES);
-        bulk_g2s(dst, M + 4 * (size_t)P * sn, TILE_BYTES, &full[st]);
-        bulk_g2s(dst + TILE_BYTES, xi + (size_t)sn * 3 * M2L_XI_STRIDE, M2L_XI_BYTES, &full[st]);
-    };
-    if (threadIdx.x >= THREADS) {  // producer warp: one lane keeps the stages filled, then the warp retires
-        if (threadIdx.x == THREADS)
+    if (!HELP && threadIdx.x >= CTHREADS) {  // producer warp: one lane keeps the stages filled, then the warp retires
+        if (threadIdx.x == CTHREADS)
             for (int q = 0; q < total; ++q) {
-                if (q >= S) mbar_wait(&empty[q % S], (uint32_t)((q / S - 1) & 1));  // all consumer warps left that stage
-                issue(q);
+                const int st = q % S;
+                if (q >= S) mbar_wait(&empty[st], (uint32_t)((q / S - 1) & 1));  // all consumer warps left that stage
+                const int sn = src[e0 + q % ne];
+                unsigned char *dst = m2l_smem_raw + (size_t)st * STAGE_BYTES;
+                mbar_expect_tx(&full[st], STAGE_BYTES);
+                bulk_g2s(dst, M + 4 * (size_t)P * sn, TILE_BYTES, &full[st]);
+                bulk_g2s(dst + TILE_BYTES, xi + (size_t)sn * 3 * M2L_XI_STRIDE, M2L_XI_BYTES, &full[st]);
             }
         return;
     }
     const double *xt3 = xi + (size_t)t * 3 * M2L_XI_STRIDE;
-    int i = 0;  // consumed loads so far
-    constexpr int NT = m2l_cfg<N1>::NT;
-    for (int mu0 = 0; mu0 < P; mu0 += NT * THREADS) {
-        // the thread's NT target proxy points; z = centre + relative part, as the oracle's xi (mid + half c_k)
-        double xt[NT], yt[NT], zt[NT], ex[NT], ey[NT], ez[NT], bx[NT], by[NT], bz[NT];
-#pragma unroll
-        for (int k = 0; k < NT; ++k) {
-            const int mu = mu0 + k * THREADS + threadIdx.x;
-            const bool live = mu < P;
-            const int a = live ? mu / (N1 * N1) : 0, b = live ? (mu / N1) % N1 : 0, c3 = live ? mu % N1 : 0;
-            xt[k] = xt3[a];
-            yt[k] = xt3[M2L_XI_STRIDE + b];
-            zt[k] = __dadd_rn(xt3[2 * M2L_XI_STRIDE + M2L_XI_STRIDE - 1], xt3[2 * M2L_XI_STRIDE + c3]);
-            ex[k] = ey[k] = ez[k] = bx[k] = by[k] = bz[k] = 0.0;
+    const int wi = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    // release of a stage: order this thread's generic-proxy reads before the next bulk copy into it (async proxy);
+    // without the fence a warp occasionally saw part of the NEXT source's tile (cross-proxy write-after-read hazard)
+    auto release = [&](int st) {
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+        __syncwarp();
+        if (lane == 0) mbar_arrive(&empty[st]);
+    };
+    auto target_point = [&](int mu, double &xt, double &yt, double &zt) {  // z = centre + relative part (mid + half c_k)
+        const bool live = mu < P;
+        const int a = live ? mu / (N1 * N1) : 0, b = live ? (mu / N1) % N1 : 0, c3 = live ? mu % N1 : 0;
+        xt = xt3[a];
+        yt = xt3[M2L_XI_STRIDE + b];
+        zt = __dadd_rn(xt3[2 * M2L_XI_STRIDE + M2L_XI_STRIDE - 1], xt3[2 * M2L_XI_STRIDE + c3]);
+    };
+    if (HELP && wi == WARPS) {
+        // helper warp: for source e it works for target group e mod CWARPS (sums kept in hacc), and its lane 0 keeps the
+        // ring filled: it polls the `empty` barriers between slices of its own work and only blocks when the next
+        // source it needs itself has not been requested yet
+        for (int k = lane; k < 6 * THREADS; k += 32) hacc[k] = 0.0;
+        int q = 0;  // loads issued so far (lane 0)
+        auto issue = [&]() {
+            const int st = q % S;
+            const int sn = src[e0 + q];
+            unsigned char *dst = m2l_smem_raw + (size_t)st * STAGE_BYTES;
+            mbar_expect_tx(&full[st], STAGE_BYTES);
+            bulk_g2s(dst, M + 4 * (size_t)P * sn, TILE_BYTES, &full[st]);
+            bulk_g2s(dst + TILE_BYTES, xi + (size_t)sn * 3 * M2L_XI_STRIDE, M2L_XI_BYTES, &full[st]);
+            ++q;
+        };
+        auto poll = [&]() {
+            if (lane == 0 && q < ne && (q < S || mbar_test(&empty[q % S], (uint32_t)((q / S - 1) & 1)))) issue();
+        };
+        if (lane == 0)
+            while (q < ne && q < S) issue();
+        __syncwarp();
+        for (int e = 0; e < ne; ++e) {
+            const int st = e % S, g = e % CWARPS;
+            if (lane == 0)
+                while (q <= e) {  // source e itself must be on its way before anybody can wait for it
+                    if (q >= S) mbar_wait(&empty[q % S], (uint32_t)((q / S - 1) & 1));
+                    issue();
+                }
+            __syncwarp();
+            mbar_wait(&full[st], (uint32_t)((e / S) & 1));  // (also when idle: see the note at the other consumer loop)
+            if (g < WARPS) {
+                double xt, yt, zt, ex = 0, ey = 0, ez = 0, bx = 0, by = 0, bz = 0;
+                target_point(g * 32 + lane, xt, yt, zt);
+                m2l_source<N1>(reinterpret_cast<const double2 *>(m2l_smem_raw + (size_t)st * STAGE_BYTES),
+                               reinterpret_cast<const double *>(m2l_smem_raw + (size_t)st * STAGE_BYTES + TILE_BYTES), g2, xt, yt, zt, ex,
+                               ey, ez, bx, by, bz, poll);
+                double *h = hacc + 6 * (g * 32 + lane);
+                h[0] += ex; h[1] += ey; h[2] += ez; h[3] += bx; h[4] += by; h[5] += bz;
+            }
+            release(st);
+            poll();
         }
+        asm volatile("bar.sync 1, %0;" ::"n"(CTHREADS) : "memory");  // hacc complete (consumer warps only)
+        return;
+    }
+    int i = 0;  // consumed loads so far
+    for (int mu0 = 0; mu0 < P; mu0 += THREADS) {
+        const int mu = mu0 + threadIdx.x;
+        double xt, yt, zt, ex = 0, ey = 0, ez = 0, bx = 0, by = 0, bz = 0;
+        target_point(mu, xt, yt, zt);
         for (int e = 0; e < ne; ++e, ++i) {
             const int st = i % S;
+            // every warp waits for the stage even when it skips the source: arrivals on `empty` are anonymous, and an
+            // early second arrival would complete the PREVIOUS phase while a slower warp is still reading the stage
             mbar_wait(&full[st], (uint32_t)((i / S) & 1));
-            const double2 *Ms = reinterpret_cast<const double2 *>(m2l_smem_raw + (size_t)st * STAGE_BYTES);
-            const double *xs = reinterpret_cast<const double *>(m2l_smem_raw + (size_t)st * STAGE_BYTES + TILE_BYTES);
-            double ztr[NT], gz2[NT][N1];
-            double S0[NT], S1[NT], S2[NT];  // sum over this source of m_k (c_{nu3} w)
-#pragma unroll
-            for (int k = 0; k < NT; ++k) {
-                ztr[k] = zt[k] - xs[2 * M2L_XI_STRIDE + M2L_XI_STRIDE - 1];  // target z relative to the source box centre
-#pragma unroll
-                for (int c = 0; c < N1; ++c) {
-                    const double dz = ztr[k] - xs[2 * M2L_XI_STRIDE + c];
-                    gz2[k][c] = (g2 * dz) * dz;
-                }
-                S0[k] = S1[k] = S2[k] = 0.0;
+            if (!(HELP && (e % CWARPS) == wi)) {  // (with a helper: the helper takes this group's source e)
+                m2l_source<N1>(reinterpret_cast<const double2 *>(m2l_smem_raw + (size_t)st * STAGE_BYTES),
+                               reinterpret_cast<const double *>(m2l_smem_raw + (size_t)st * STAGE_BYTES + TILE_BYTES), g2, xt, yt, zt, ex,
+                               ey, ez, bx, by, bz, m2l_no_poll());
             }
-            for (int a2 = 0; a2 < N1; ++a2) {
-                double dx[NT], dx2[NT];
-#pragma unroll
-                for (int k = 0; k < NT; ++k) {
-                    dx[k] = xt[k] - xs[a2];
-                    dx2[k] = dx[k] * dx[k];
-                }
-#pragma unroll 1
-                for (int b2 = 0; b2 < N1; ++b2) {
-                    const double2 *row = Ms + 2 * ((a2 * N1 + b2) * N1);
-                    double dy[NT], s2[NT], A0[NT], A1[NT], A2[NT], A3[NT];
-#pragma unroll
-                    for (int k = 0; k < NT; ++k) {
-                        dy[k] = yt[k] - xs[M2L_XI_STRIDE + b2];
-                        s2[k] = fma(dy[k], dy[k], dx2[k]);
-                        A0[k] = A1[k] = A2[k] = A3[k] = 0.0;
-                    }
-#pragma unroll
-                    for (int c2 = 0; c2 < N1; ++c2) {
-                        const double2 m01 = row[2 * c2], m23 = row[2 * c2 + 1];
-#pragma unroll
-                        for (int k = 0; k < NT; ++k) {
-                            const double w = inv_r3(s2[k] + gz2[k][c2]);
-                            A0[k] = fma(m01.x, w, A0[k]);
-                            A1[k] = fma(m01.y, w, A1[k]);
-                            A2[k] = fma(m23.x, w, A2[k]);
-                            A3[k] = fma(m23.y, w, A3[k]);
-                            if (c2 == 0 || c2 == N1 - 1 || 2 * c2 != N1 - 1) {  // c_k = 0 at the middle point of an even order
-                                const double u = (c2 == 0) ? w : (c2 == N1 - 1) ? -w : w * m2l_cheb_c[N1][c2];
-                                S0[k] = fma(m01.x, u, S0[k]);
-                                S1[k] = fma(m01.y, u, S1[k]);
-                                S2[k] = fma(m23.x, u, S2[k]);
-                            }
-                        }
-                    }
-#pragma unroll
-                    for (int k = 0; k < NT; ++k) {
-                        // sum m_k w dz = ztr sum m_k w - h_z sum m_k c w:  E_z += Z0,  B_x += Z2,  B_y -= Z1
-                        ex[k] = fma(A0[k], dx[k], ex[k]);
-                        ey[k] = fma(A0[k], dy[k], ey[k]);
-                        ez[k] = fma(A0[k], ztr[k], ez[k]);
-                        bx[k] = fma(-A3[k], dy[k], fma(A2[k], ztr[k], bx[k]));
-                        by[k] = fma(A3[k], dx[k], fma(-A1[k], ztr[k], by[k]));
-                        bz[k] = fma(A1[k], dy[k], fma(-A2[k], dx[k], bz[k]));
-                    }
-                }
-            }
-            {
-                const double hz = xs[2 * M2L_XI_STRIDE + M2L_XI_STRIDE - 2];
-#pragma unroll
-                for (int k = 0; k < NT; ++k) {
-                    ez[k] = fma(-hz, S0[k], ez[k]);
-                    bx[k] = fma(-hz, S2[k], bx[k]);
-                    by[k] = fma(hz, S1[k], by[k]);
-                }
-            }
-            // The stage is about to be overwritten by a bulk TMA copy (async proxy): order this thread's generic-proxy
-            // reads of it before the release.  Without this fence a warp occasionally (about 1 evaluation in 10 when P2P
-            // runs beside M2L) saw part of the NEXT source's tile: a cross-proxy write-after-read hazard.
-            asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-            __syncwarp();
-            if ((threadIdx.x & 31) == 0) mbar_arrive(&empty[st]);
+            release(st);
         }
-#pragma unroll
-        for (int k = 0; k < NT; ++k) {
-            const int mu = mu0 + k * THREADS + threadIdx.x;
-            if (mu < P) {
-                double *o = Lt + 6 * (size_t)mu;
-                o[0] = ex[k]; o[1] = ey[k]; o[2] = ez[k]; o[3] = bx[k]; o[4] = by[k]; o[5] = bz[k];
-            }
+        if (HELP) {  // own sums + the helper's, in this fixed order
+            asm volatile("bar.sync 1, %0;" ::"n"(CTHREADS) : "memory");
+            const double *h = hacc + 6 * threadIdx.x;
+            ex += h[0]; ey += h[1]; ez += h[2]; bx += h[3]; by += h[4]; bz += h[5];
+        }
+        if (mu < P) {
+            double *o = Lt + 6 * (size_t)mu;
+            o[0] = ex; o[1] = ey; o[2] = ez; o[3] = bx; o[4] = by; o[5] = bz;
         }
     }
 }
@@ -588,12 +648,13 @@ template <int N1>
 static int launch_m2l(fmm_plan *p)
 {
     fmm_ctx *c = &p->ctx;
-    const size_t smem = m2l_cfg<N1>::STAGES * ((size_t)32 * m2l_cfg<N1>::P + M2L_XI_BYTES) + 2 * m2l_cfg<N1>::STAGES * sizeof(uint64_t);
+    const size_t smem = m2l_cfg<N1>::STAGES * ((size_t)32 * m2l_cfg<N1>::P + M2L_XI_BYTES) + 2 * m2l_cfg<N1>::STAGES * sizeof(uint64_t) +
+                        (m2l_cfg<N1>::HELP ? sizeof(double) * 6 * m2l_cfg<N1>::THREADS : 0);
     if (smem > 48 * 1024)
         FMM_CUDA(c, cudaFuncSetAttribute((const void *)m2l_kernel<N1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     // the default carveout leaves room for one block only; ask for enough shared memory for every resident block
     FMM_CUDA(c, cudaFuncSetAttribute((const void *)m2l_kernel<N1>, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared));
-    m2l_kernel<N1><<<(unsigned)p->nodes, m2l_cfg<N1>::THREADS + 32, smem, c->stream>>>(p->gamma_bar * p->gamma_bar, p->m2l_order, p->m2l_off,
+    m2l_kernel<N1><<<(unsigned)p->nodes, m2l_cfg<N1>::BLOCK, smem, c->stream>>>(p->gamma_bar * p->gamma_bar, p->m2l_order, p->m2l_off,
                                                                                p->m2l_src, p->node_xi, p->M, p->L);
     FMM_LAUNCH_CHECK(c, "m2l_kernel");
     return FMM_OK;

@@ -296,17 +296,20 @@ def test_overlap_is_bit_identical_to_serial_and_stable(fmm):
     write-after-read hazard in the M2L source ring (generic reads of a stage vs. the next bulk-TMA copy into it) that
     only showed with concurrent kernels: 25 evaluations in each mode must be bit-identical."""
     import torch
-    w = workloads.config(3, N=30000)
-    plan = fmm.fmm_plan_create(*w.arrays(), w.q, order_n=3, leaf_size=100, theta=0.4)
-    plan.set_overlap(False)
-    E0, B0 = plan.eval()
-    E0, B0 = E0.clone(), B0.clone()
-    for ov in (True, False, True):
-        plan.set_overlap(ov)
-        for _ in range(25):
-            E, B = plan.eval()
-            assert torch.equal(E, E0) and torch.equal(B, B0), f"overlap={ov}: result changed between evaluations"
-    plan.close()
+    # n = 3: two consumer warps + producer warp; n = 5 and n = 6: 7 / 11 consumer warps + the helper warp that also
+    # refills the ring (anonymous `empty` arrivals: every warp must wait for a stage before releasing it)
+    for cfg, N, n, N0, theta in ((3, 30000, 3, 100, 0.4), (2, 20000, 5, 128, 0.5), (3, 40000, 6, 256, 0.5)):
+        w = workloads.config(cfg, N=N)
+        plan = fmm.fmm_plan_create(*w.arrays(), w.q, order_n=n, leaf_size=N0, theta=theta)
+        plan.set_overlap(False)
+        E0, B0 = plan.eval()
+        E0, B0 = E0.clone(), B0.clone()
+        for ov in (True, False, True):
+            plan.set_overlap(ov)
+            for _ in range(25):
+                E, B = plan.eval()
+                assert torch.equal(E, E0) and torch.equal(B, B0), f"n={n} overlap={ov}: result changed between evaluations"
+        plan.close()
 
 
 # ---------------------------------------------------------------------------------------------
