@@ -339,7 +339,7 @@ struct m2l_cfg {
 #define M2L_NT 1
 #endif
     static constexpr int NT = M2L_NT;                      // target proxy points per thread
-    static constexpr int BATCHES = (P + 1024 * NT - 1) / (1024 * NT);
+    static constexpr int BATCHES = (P + 992 * NT - 1) / (992 * NT);  // 992 + the 32 producer threads = 1024 per block
     static constexpr int PER = (P + BATCHES - 1) / BATCHES;
     static constexpr int THREADS = (((PER + NT - 1) / NT + 31) / 32) * 32;
     // two resident blocks per SM while 2 x THREADS x 88 registers fit the register file (the dependent

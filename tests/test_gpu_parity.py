@@ -59,6 +59,8 @@ def small_cases():
     yield "paper_cube_n2", w, 2, 27, 0.5
     w = workloads.config(2, N=3000)           # n = 8: P = 729, M2L threads = 736 (one block per SM)
     yield "order8", w, 8, 200, 0.5
+    w = workloads.config(2, N=2000)           # n = 9: P = 1000 = two batches of 500 (1024 threads would leave no room for the producer warp)
+    yield "order9", w, 9, 150, 0.5
     w = workloads.config(3, N=2500)           # n = 10: P = 1331 > 1024 -> two proxy batches per target node, 2 pipeline stages
     yield "order10_batches", w, 10, 300, 0.5
     w = workloads.config(1, N=1500)           # n = 12 (FMM_MAX_ORDER): P = 2197, three batches, single-stage pipeline
