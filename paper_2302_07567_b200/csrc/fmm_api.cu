@@ -165,6 +165,7 @@ static int plan_build(fmm_plan *p, const fmm_particles_t *in, bool refit = false
     FMM_CUDA(c, cudaEventRecord(p->ev_plan[1], c->stream));
     FMM_TRY(dtt_build_lists(p));
     FMM_TRY(pairs_p2p_prepare(p));
+    FMM_TRY(pairs_m2l_prepare(p));
     FMM_CUDA(c, cudaEventRecord(p->ev_plan[2], c->stream));
     FMM_CUDA(c, cudaStreamSynchronize(c->stream));
     FMM_CUDA(c, cudaEventElapsedTime(&p->ms_tree, p->ev_plan[0], p->ev_plan[1]));

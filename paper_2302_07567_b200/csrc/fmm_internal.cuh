@@ -76,6 +76,9 @@ struct fmm_plan {
     int64_t p2p_max_row;    // largest number of particle pairs in one target leaf's row
     int p2p_split;          // P2P row split K: block (t, k) sums chunk k of t's row into near_[k]; L2P adds the K partials in order
     int64_t near_cap;       // doubles allocated for near_
+    int m2l_split;          // M2L row split (small trees): chunk kc > 0 of a row goes to Lpart[kc-1], combined into L in order
+    double *Lpart;          // [m2l_split-1][nodes+2][P][6]
+    int64_t lpart_cap;
     int32_t *p2p_order, *m2l_order;  // target ids sorted by descending work (LPT block order)
     int32_t n_p2p_targets, n_m2l_targets;
     // expansions
@@ -110,6 +113,7 @@ int interp_l2p_finalize(fmm_plan *p, /* treecode: no far interpolation, near_ ha
 // ---- kernels_pairs.cu ---------------------------------------------------------------
 int pairs_p2p(fmm_plan *p);
 int pairs_p2p_prepare(fmm_plan *p);
+int pairs_m2l_prepare(fmm_plan *p);
 int pairs_m2l(fmm_plan *p);
 int pairs_pc(fmm_plan *p);   // treecode: particle-cluster sums
 int pairs_direct(fmm_ctx *c, int64_t N, const double *x, const double *y, const double *z,

@@ -183,6 +183,30 @@ static void p2p_shape(int64_t leaves, int maxleaf, int64_t pairs, int64_t max_ro
     *split_out = K;
 }
 
+int pairs_m2l_prepare(fmm_plan *p)  // after the lists: M2L row split for small trees
+{
+    fmm_ctx *c = &p->ctx;
+    int K = 1;
+    if (!(p->flags & FMM_METHOD_TREECODE) && p->n_m2l > 0) {
+        // two resident blocks per SM; aim at four waves of blocks.  Only trees with few nodes need it, and the partial
+        // buffers stay below 256 MB.
+        int64_t want = 4 * 2 * FMM_SM_COUNT;
+        K = (int)((want + p->nodes - 1) / p->nodes);
+        if (K > 4) K = 4;
+        if (K < 1) K = 1;
+        while (K > 1 && (int64_t)(K - 1) * 48 * p->P * (p->nodes + 2) > ((int64_t)256 << 20)) --K;
+    }
+    p->m2l_split = K;
+    int64_t need = (int64_t)(K - 1) * 6 * p->P * (p->nodes + 2);
+    if (need > p->lpart_cap) {
+        if (p->Lpart) ctx_free(c, p->Lpart);
+        p->Lpart = (double *)ctx_alloc(c, sizeof(double) * (size_t)need);
+        if (!p->Lpart) return FMM_ENOMEM;
+        p->lpart_cap = need;
+    }
+    return FMM_OK;
+}
+
 int pairs_p2p_prepare(fmm_plan *p)  // after the lists: choose the row split and size the partial buffers
 {
     fmm_ctx *c = &p->ctx;
@@ -506,10 +530,11 @@ __device__ __forceinline__ void m2l_source(const double2 *__restrict__ Ms, const
     by = fma(hz, S1, by);
 }
 
-template <int N1>
+template <int N1, bool SPLIT>
 __global__ void __launch_bounds__(m2l_cfg<N1>::BLOCK, m2l_cfg<N1>::MINB) m2l_kernel(double g2, const int32_t *__restrict__ order,
                                                                                   const int32_t *__restrict__ off, const int32_t *__restrict__ src,
-                                                                                  const double *__restrict__ xi, const double *__restrict__ M, double *__restrict__ L)
+                                                                                  const double *__restrict__ xi, const double *__restrict__ M, double *__restrict__ L,
+                                                                                  int K, double *__restrict__ Lpart, size_t lstride)
 {
     constexpr int P = m2l_cfg<N1>::P;
     constexpr int THREADS = m2l_cfg<N1>::THREADS;   // threads that own target proxy points
@@ -524,9 +549,12 @@ __global__ void __launch_bounds__(m2l_cfg<N1>::BLOCK, m2l_cfg<N1>::MINB) m2l_ker
     uint64_t *full = reinterpret_cast<uint64_t *>(m2l_smem_raw + S * STAGE_BYTES);
     uint64_t *empty = full + S;
     double *hacc = reinterpret_cast<double *>(m2l_smem_raw + S * STAGE_BYTES + 2 * S * sizeof(uint64_t));  // [THREADS][6], HELP only
-    const int t = order[blockIdx.x];
-    const int e0 = off[t], e1 = off[t + 1];
-    double *Lt = L + 6 * (size_t)P * t;
+    // block (t, kc): chunk kc of the K contiguous chunks of target t's row (K > 1 only for small trees, to fill the GPU);
+    // chunk 0 writes L, chunk kc > 0 the partial buffer kc - 1, added to L in chunk order by m2l_combine
+    const int t = SPLIT ? order[blockIdx.x / K] : order[blockIdx.x], kc = SPLIT ? blockIdx.x % K : 0;
+    const int r0 = off[t], rl = off[t + 1] - r0;
+    const int e0 = SPLIT ? r0 + (int)(((int64_t)rl * kc) / K) : r0, e1 = SPLIT ? r0 + (int)(((int64_t)rl * (kc + 1)) / K) : r0 + rl;
+    double *Lt = ((!SPLIT || kc == 0) ? L : Lpart + (size_t)(kc - 1) * lstride) + 6 * (size_t)P * t;
     if (e0 == e1) {  // no far-field sources: the local expansion starts at zero (L2L adds into it)
         for (int k = threadIdx.x; k < 6 * P; k += m2l_cfg<N1>::BLOCK) Lt[k] = 0.0;
         return;
@@ -644,6 +672,16 @@ __global__ void __launch_bounds__(m2l_cfg<N1>::BLOCK, m2l_cfg<N1>::MINB) m2l_ker
     }
 }
 
+// L += partial buffers of the row chunks 1 .. K-1, in chunk order
+__global__ void m2l_combine(size_t count, int K, size_t lstride, const double *__restrict__ Lpart, double *__restrict__ L)
+{
+    size_t k = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= count) return;
+    double v = L[k];
+    for (int kc = 1; kc < K; ++kc) v += Lpart[(size_t)(kc - 1) * lstride + k];
+    L[k] = v;
+}
+
 template <int N1>
 static int launch_m2l(fmm_plan *p)
 {
@@ -651,12 +689,27 @@ static int launch_m2l(fmm_plan *p)
     const size_t smem = m2l_cfg<N1>::STAGES * ((size_t)32 * m2l_cfg<N1>::P + M2L_XI_BYTES) + 2 * m2l_cfg<N1>::STAGES * sizeof(uint64_t) +
                         (m2l_cfg<N1>::HELP ? sizeof(double) * 6 * m2l_cfg<N1>::THREADS : 0);
     if (smem > 48 * 1024)
-        FMM_CUDA(c, cudaFuncSetAttribute((const void *)m2l_kernel<N1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    {
+        FMM_CUDA(c, cudaFuncSetAttribute((const void *)m2l_kernel<N1, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        FMM_CUDA(c, cudaFuncSetAttribute((const void *)m2l_kernel<N1, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    }
     // the default carveout leaves room for one block only; ask for enough shared memory for every resident block
-    FMM_CUDA(c, cudaFuncSetAttribute((const void *)m2l_kernel<N1>, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared));
-    m2l_kernel<N1><<<(unsigned)p->nodes, m2l_cfg<N1>::BLOCK, smem, c->stream>>>(p->gamma_bar * p->gamma_bar, p->m2l_order, p->m2l_off,
-                                                                               p->m2l_src, p->node_xi, p->M, p->L);
+    FMM_CUDA(c, cudaFuncSetAttribute((const void *)m2l_kernel<N1, false>, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared));
+    FMM_CUDA(c, cudaFuncSetAttribute((const void *)m2l_kernel<N1, true>, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared));
+    const int K = p->m2l_split;
+    const size_t lstride = 6 * (size_t)m2l_cfg<N1>::P * (size_t)(p->nodes + 2);
+    if (K > 1)
+        m2l_kernel<N1, true><<<(unsigned)(p->nodes * K), m2l_cfg<N1>::BLOCK, smem, c->stream>>>(p->gamma_bar * p->gamma_bar, p->m2l_order, p->m2l_off,
+                                                                                               p->m2l_src, p->node_xi, p->M, p->L, K, p->Lpart, lstride);
+    else
+        m2l_kernel<N1, false><<<(unsigned)p->nodes, m2l_cfg<N1>::BLOCK, smem, c->stream>>>(p->gamma_bar * p->gamma_bar, p->m2l_order, p->m2l_off,
+                                                                                          p->m2l_src, p->node_xi, p->M, p->L, K, p->Lpart, lstride);
     FMM_LAUNCH_CHECK(c, "m2l_kernel");
+    if (K > 1) {
+        const size_t count = 6 * (size_t)m2l_cfg<N1>::P * (size_t)(p->nodes + 1);
+        m2l_combine<<<(unsigned)((count + 255) / 256), 256, 0, c->stream>>>(count, K, lstride, p->Lpart, p->L);
+        FMM_LAUNCH_CHECK(c, "m2l_combine");
+    }
     return FMM_OK;
 }
 
