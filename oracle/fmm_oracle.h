@@ -19,7 +19,11 @@
  * moving charge, Coulomb limit, B = beta x E / c0, symmetry, Theorem 1 polynomial
  * reproduction, moment conservation, M2M == P2M at the parent, Lemma 1, empty far
  * list => FMM == direct, brute-force coverage of the leaf x leaf matrix, tree
- * invariants, convergence in n and eta.  The ABSOLUTE FMM-vs-direct error values
+ * invariants, convergence in n and eta; the traversal's split rule (Alg 5.11: target iff
+ * diam(S_t) > diam(S_s), ties split the source) by a plain-Python restatement of Alg 5.11 whose
+ * lists must equal these exactly, incl. mirror-symmetric inputs with bit-identical radii and a
+ * hand-worked example; Alg 5.1's first-maximiser rule by two- and three-way non-zero ties
+ * (tests/test_oracle_traversal_pins.py).  The ABSOLUTE FMM-vs-direct error values
  * are "parity unpinned" by the paper (Fig. 2 is an image): only their trend is pinned.
  *
  * All pointers are HOST pointers.  Arrays are caller-owned unless stated.
