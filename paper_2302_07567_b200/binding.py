@@ -188,15 +188,48 @@ def _stream_ptr():
     return C.c_void_p(torch.cuda.current_stream().cuda_stream)
 
 
+class _on_plan_stream:
+    """Run a block on the plan's stream: the plan stream first waits for the caller's current stream (inputs the
+    caller has just produced), and on exit the caller's stream waits for the plan stream (outputs).  Workspace and
+    outputs allocated inside belong to the plan stream's pool; ``keep`` tensors are recorded on the caller's stream."""
+
+    def __init__(self, plan):
+        self.plan = plan
+
+    def __enter__(self):
+        self.caller = torch.cuda.current_stream(self.plan.device)
+        self.same = self.caller == self.plan.stream
+        if not self.same:
+            self.plan.stream.wait_stream(self.caller)
+        self.ctx = torch.cuda.stream(self.plan.stream)
+        self.ctx.__enter__()
+        return self
+
+    def hand_over(self, *tensors):
+        if not self.same:
+            for t in tensors:
+                t.record_stream(self.caller)
+
+    def __exit__(self, *exc):
+        self.ctx.__exit__(*exc)
+        if not self.same:
+            self.caller.wait_stream(self.plan.stream)
+        return False
+
+
 # ---- the C calls --------------------------------------------------------------------------------
 class Plan:
     """Handle of an fmm_plan_t (tree + interaction lists).  Create with ``fmm_plan_create``."""
 
-    def __init__(self, handle, allocator, N, device):
+    def __init__(self, handle, allocator, N, device, stream):
         self._h = handle
         self._alloc = allocator
         self.N = N
         self.device = device
+        # The library enqueues everything on the stream given to fmm_plan_create and frees scratch right after
+        # enqueueing (stream-ordered).  Torch's caching allocator is per stream, so every later call runs under
+        # this stream (``_on_plan_stream``) and the caller's current stream is ordered with it on both sides.
+        self.stream = stream
 
     def update(self, x, y, z, px, py, pz, q=None):
         return fmm_plan_update(self, x, y, z, px, py, pz, q)
@@ -243,13 +276,14 @@ def fmm_plan_create(x, y, z, px, py, pz, q=None, *, order_n, leaf_size, theta, g
         rc = lib.fmm_plan_create(C.byref(h), C.byref(parts), C.byref(prm), alloc.alloc_cb, alloc.free_cb, None,
                                  _stream_ptr())
         _check(rc)
+        stream = torch.cuda.current_stream(device)
         del keep
-    return Plan(h, alloc, parts.N, device)
+    return Plan(h, alloc, parts.N, device, stream)
 
 
 def fmm_plan_update(plan: Plan, x, y, z, px, py, pz, q=None):
     lib = load_library()
-    with torch.cuda.device(plan.device):
+    with torch.cuda.device(plan.device), _on_plan_stream(plan):
         parts, keep = _particles(x, y, z, px, py, pz, q, plan.device)
         _check(lib.fmm_plan_update(plan._h, C.byref(parts)), plan._h)
         del keep
@@ -258,7 +292,7 @@ def fmm_plan_update(plan: Plan, x, y, z, px, py, pz, q=None):
 def fmm_plan_refit(plan: Plan, x, y, z, px, py, pz, q=None):
     """Keeps the particle order of the last build; new boxes and lists on the moved particles (no sort)."""
     lib = load_library()
-    with torch.cuda.device(plan.device):
+    with torch.cuda.device(plan.device), _on_plan_stream(plan):
         parts, keep = _particles(x, y, z, px, py, pz, q, plan.device)
         _check(lib.fmm_plan_refit(plan._h, C.byref(parts)), plan._h)
         del keep
@@ -267,9 +301,10 @@ def fmm_plan_refit(plan: Plan, x, y, z, px, py, pz, q=None):
 def fmm_eval(plan: Plan, out=None):
     """a4-a10.  Returns (E[3,N], B[3,N]) device tensors in caller order (rows x, y, z).  Enqueue only."""
     lib = load_library()
-    with torch.cuda.device(plan.device):
+    with torch.cuda.device(plan.device), _on_plan_stream(plan) as s:
         if out is None:
             out = torch.empty((6, plan.N), dtype=torch.float64, device=plan.device)
+            s.hand_over(out)
         ptrs = [C.c_void_p(out[k].data_ptr()) for k in range(6)]
         _check(lib.fmm_eval(plan._h, *ptrs), plan._h)
     return out[:3], out[3:]
@@ -298,7 +333,8 @@ def fmm_plan_export(plan: Plan, want_M=False, want_L=False) -> dict:
     e = fmm_export_t()
     for k, v in out.items():
         setattr(e, k, v.ctypes.data if v.size else None)
-    _check(load_library().fmm_plan_export(plan._h, C.byref(e)), plan._h)
+    with torch.cuda.device(plan.device), _on_plan_stream(plan):
+        _check(load_library().fmm_plan_export(plan._h, C.byref(e)), plan._h)
     return out
 
 

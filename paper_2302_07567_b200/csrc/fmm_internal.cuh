@@ -71,9 +71,18 @@ struct fmm_plan {
     double *node_xi;        // [nodes+1][3][16] : proxy points per axis (I-3), filled by pairs_m2l
     // interaction lists, CSR by target node id (offset arrays indexed by node id, length nodes+2)
     int32_t *p2p_off, *p2p_src, *m2l_off, *m2l_src;
+    // mutual near field (kernels_dtt.cu "p2p_mates"): per P2P entry, dst >= 0: the target's block owns the pair and writes the
+    // reaction on the source leaf to partial segment dst; dst = -1: one-sided; dst = -2: the mate's block does the work and
+    // recv >= 0 is the segment holding the sums for this entry's target particles.  NULL with FMM_KERNEL_SOURCE_MOMENTUM.
+    int32_t *p2p_dst, *p2p_recv;
+    int64_t p2p_react;      // particles in all reaction segments
+    double *react;          // [6][p2p_react] reaction sums (E, B components as planes), rewritten by every fmm_eval
+    int64_t react_cap;
+    int react_used;         // the last pairs_p2p ran the mutual kernel (L2P then subtracts the reaction segments)
     int64_t n_p2p, n_m2l, cap_p2p, cap_m2l;
     int64_t p2p_pairs, m2l_pairs;
-    int64_t p2p_max_row;    // largest number of particle pairs in one target leaf's row
+    int64_t p2p_work;       // block work of the whole P2P list in one-sided pair units (an owned mutual pair counts 34/25, a pair the mate owns 0)
+    int64_t p2p_max_row;    // heaviest target leaf row, same units
     int p2p_split;          // P2P row split K: block (t, k) sums chunk k of t's row into near_[k]; L2P adds the K partials in order
     int64_t near_cap;       // doubles allocated for near_
     int m2l_split;          // M2L row split (small trees): chunk kc > 0 of a row goes to Lpart[kc-1], combined into L in order

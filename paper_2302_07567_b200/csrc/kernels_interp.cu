@@ -293,6 +293,8 @@ __global__ void __launch_bounds__(L2P_THREADS) l2p_kernel(cheb_t ch, int leaves,
                                                           const double *__restrict__ tx, const double *__restrict__ ty,
                                                           const double *__restrict__ tz, const double *__restrict__ L,
                                                           const double *__restrict__ near_, int K, int skip_far, const int32_t *__restrict__ perm,
+                                                          const int32_t *__restrict__ p2p_off, const int32_t *__restrict__ p2p_recv,
+                                                          const double *__restrict__ react, size_t rstride,
                                                           double cE, double cB, double *__restrict__ Ex, double *__restrict__ Ey,
                                                           double *__restrict__ Ez, double *__restrict__ Bx, double *__restrict__ By,
                                                           double *__restrict__ Bz)
@@ -341,6 +343,15 @@ __global__ void __launch_bounds__(L2P_THREADS) l2p_kernel(cheb_t ch, int leaves,
             for (int kc = 1; kc < K; ++kc)
 #pragma unroll
                 for (int f = 0; f < 6; ++f) nr[f] += near_[((size_t)kc * 6 + f) * (size_t)N + k];
+        if (p2p_recv) {  // mutual near field: the pairs a neighbour's block evaluated, g(x_j, x_i) = -g(x_i, x_j), in list order
+            for (int e = p2p_off[node]; e < p2p_off[node + 1]; ++e) {
+                const int r = p2p_recv[e];
+                if (r < 0) continue;
+                const double *rp = react + (size_t)r + (size_t)(k - lo);
+#pragma unroll
+                for (int f = 0; f < 6; ++f) nr[f] -= rp[f * rstride];
+            }
+        }
         Ex[i] = cE * (nr[0] + fx[0]);
         Ey[i] = cE * (nr[1] + fx[1]);
         Ez[i] = cE * (nr[2] + fx[2]);
@@ -453,7 +464,7 @@ int interp_l2p_finalize(fmm_plan *p, double *Ex, double *Ey, double *Ez, double 
     FMM_TRY(dispatch_n1(p->n1, [&](auto k) {
         l2p_kernel<decltype(k)::value><<<(unsigned)p->leaves, L2P_THREADS, smem, c->stream>>>(
             ch, (int)p->leaves, (int)p->N, p->node_lo, p->node_hi, p->bbox, p->tx, p->ty, p->tz, p->L, p->near_, nparts, skip_far, p->perm,
-            cE, cB, Ex, Ey, Ez, Bx, By, Bz);
+            p->p2p_off, p->react_used ? p->p2p_recv : NULL, p->react, (size_t)(p->react_cap > 0 ? p->react_cap : 1), cE, cB, Ex, Ey, Ez, Bx, By, Bz);
         return FMM_OK;
     }));
     FMM_LAUNCH_CHECK(c, "l2p_kernel");

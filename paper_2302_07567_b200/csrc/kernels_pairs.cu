@@ -155,12 +155,231 @@ __global__ void __launch_bounds__(256) p2p_kernel(int N, double gb, const int32_
     }
 }
 
+
+// ---------------------------------------------------------------------------------------
+// a7, mutual form (mean-gamma kernel only).  g(x_j, x_i) = -g(x_i, x_j) for the kernel of eq. (3.2), so for a pair of
+// leaves {t, s} that sits in the P2P list in both directions the owner's block evaluates D^{-3/2} once per particle
+// pair and forms both sums: 34 FP64 instructions per particle pair = 17 per kernel evaluation instead of 25.
+//   * targets: NT particles per thread in registers (positions, their own source weights, six sums), as in p2p_kernel;
+//   * sources: the owned source leaves of the row are streamed through a shared-memory tile (structure of arrays) in
+//     batches of 32; at step k of a batch lane l works on source (l + k) mod 32, so every lane reads its own source
+//     (conflict-free LDS.64) and every target / source pair of the batch is visited once in 32 steps;
+//   * reaction: the six sums of a source travel with it from lane to lane (SHFL, one rotation per step) and are back in
+//     the source's home lane after 32 steps holding the contribution of this warp's 32 NT targets; the warps of the
+//     block are then added in warp order (shared memory) and the result is stored to the partial segment of the
+//     entry (s, t), which L2P subtracts from s's own sums in list order.  One writer per segment, fixed orders: no atomics.
+// Entries without a mate (and t's own leaf) go through the one-sided loop.  Dead lanes / padded sources carry zero
+// weights (they add exact zeros) and their own results are dropped.
+// ---------------------------------------------------------------------------------------
+#define MUT_TILE 256
+
+template <int NT>
+struct mut_targets {
+    double x[NT], y[NT], z[NT], q0[NT], q1[NT], q2[NT], q3[NT];
+    double ex[NT], ey[NT], ez[NT], bx[NT], by[NT], bz[NT];
+};
+
+struct mut_tile {
+    double x[MUT_TILE], y[MUT_TILE], z[MUT_TILE], m0[MUT_TILE], m1[MUT_TILE], m2[MUT_TILE], m3[MUT_TILE];
+    int dst[MUT_TILE];
+};
+
+template <int NT>
+__device__ __forceinline__ void mut_pair_terms(const mut_targets<NT> &T, double gb, double xs, double ys, double zs,
+                                               double (&gx)[NT], double (&gy)[NT], double (&gz)[NT])
+{
+#pragma unroll
+    for (int k = 0; k < NT; ++k) {
+        const double dx = T.x[k] - xs, dy = T.y[k] - ys, dz = T.z[k] - zs;
+        double D = dx * dx;
+        D = fma(dy, dy, D);
+        const double sz = gb * dz;
+        D = fma(sz, sz, D);
+        const double w = inv_r3(D);
+        gx[k] = w * dx; gy[k] = w * dy; gz[k] = w * dz;
+    }
+}
+
+template <int NT>
+__device__ __forceinline__ void mut_target_sums(mut_targets<NT> &T, double m0, double m1, double m2, double m3,
+                                                const double (&gx)[NT], const double (&gy)[NT], const double (&gz)[NT])
+{
+#pragma unroll
+    for (int k = 0; k < NT; ++k) { T.ex[k] = fma(m0, gx[k], T.ex[k]); T.ey[k] = fma(m0, gy[k], T.ey[k]); T.ez[k] = fma(m0, gz[k], T.ez[k]); }
+#pragma unroll
+    for (int k = 0; k < NT; ++k) { T.bx[k] = fma(m2, gz[k], T.bx[k]); T.bz[k] = fma(-m2, gx[k], T.bz[k]); }
+#pragma unroll
+    for (int k = 0; k < NT; ++k) { T.by[k] = fma(m3, gx[k], T.by[k]); T.bx[k] = fma(-m3, gy[k], T.bx[k]); }
+#pragma unroll
+    for (int k = 0; k < NT; ++k) { T.bz[k] = fma(m1, gy[k], T.bz[k]); T.by[k] = fma(-m1, gz[k], T.by[k]); }
+}
+
+// `cnt` staged sources (a multiple of 32), both directions
+template <int NT, int W>
+__device__ __forceinline__ void mut_process_mutual(mut_targets<NT> &T, const mut_tile &S, int cnt, double gb, double *red,
+                                                   double *__restrict__ react, size_t rstride)
+{
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    for (int b0 = 0; b0 < cnt; b0 += 32) {
+        double rex = 0, rey = 0, rez = 0, rbx = 0, rby = 0, rbz = 0;  // sum_i q_i (x) g(x_i, x_j) for the source travelling through this lane
+#pragma unroll 1
+        for (int k2 = 0; k2 < 32; ++k2) {
+            const int j = b0 + ((lane + k2) & 31);
+            const double xs = S.x[j], ys = S.y[j], zs = S.z[j], m0 = S.m0[j], m1 = S.m1[j], m2 = S.m2[j], m3 = S.m3[j];
+            double gx[NT], gy[NT], gz[NT];
+            mut_pair_terms<NT>(T, gb, xs, ys, zs, gx, gy, gz);
+            mut_target_sums<NT>(T, m0, m1, m2, m3, gx, gy, gz);
+#pragma unroll
+            for (int k = 0; k < NT; ++k) {
+                rex = fma(T.q0[k], gx[k], rex); rey = fma(T.q0[k], gy[k], rey); rez = fma(T.q0[k], gz[k], rez);
+                rbx = fma(T.q2[k], gz[k], rbx); rbz = fma(-T.q2[k], gx[k], rbz);
+                rby = fma(T.q3[k], gx[k], rby); rbx = fma(-T.q3[k], gy[k], rbx);
+                rbz = fma(T.q1[k], gy[k], rbz); rby = fma(-T.q1[k], gz[k], rby);
+            }
+            const int from = (lane + 1) & 31;  // the source this lane takes next was with lane + 1
+            rex = __shfl_sync(0xffffffffu, rex, from); rey = __shfl_sync(0xffffffffu, rey, from); rez = __shfl_sync(0xffffffffu, rez, from);
+            rbx = __shfl_sync(0xffffffffu, rbx, from); rby = __shfl_sync(0xffffffffu, rby, from); rbz = __shfl_sync(0xffffffffu, rbz, from);
+        }
+        // lane l now holds the sums for source b0 + l over this warp's targets
+        if (W == 1) {
+            const int d = S.dst[b0 + lane];
+            if (d >= 0) {
+                react[d] = rex; react[rstride + d] = rey; react[2 * rstride + d] = rez;
+                react[3 * rstride + d] = rbx; react[4 * rstride + d] = rby; react[5 * rstride + d] = rbz;
+            }
+        } else {
+            double *r = red + (size_t)warp * 192 + lane;
+            r[0] = rex; r[32] = rey; r[64] = rez; r[96] = rbx; r[128] = rby; r[160] = rbz;
+            __syncthreads();
+            for (int q = threadIdx.x; q < 192; q += 32 * W) {
+                const int d = S.dst[b0 + (q & 31)];
+                double v = red[q];
+#pragma unroll
+                for (int w = 1; w < W; ++w) v += red[(size_t)w * 192 + q];  // warp order
+                if (d >= 0) react[(size_t)(q >> 5) * rstride + d] = v;
+            }
+            __syncthreads();
+        }
+    }
+}
+
+// `cnt` staged sources acting on the targets only (broadcast reads)
+template <int NT>
+__device__ __forceinline__ void mut_process_onesided(mut_targets<NT> &T, const mut_tile &S, int cnt, double gb)
+{
+#pragma unroll 2
+    for (int j = 0; j < cnt; ++j) {
+        double gx[NT], gy[NT], gz[NT];
+        mut_pair_terms<NT>(T, gb, S.x[j], S.y[j], S.z[j], gx, gy, gz);
+        mut_target_sums<NT>(T, S.m0[j], S.m1[j], S.m2[j], S.m3[j], gx, gy, gz);
+    }
+}
+
+// resident warps per SM the register budget is sized for: 216 registers at NT = 4 schedule the four dependency chains of a
+// step with the fewest stalls (profiles/r02_p2p_mutual.md), the smaller shapes fit more warps
+template <int NT, int W>
+struct mut_cfg {
+    static constexpr int WARPS = (NT == 4) ? 8 : (NT == 3) ? 12 : (NT == 2) ? 16 : 32;
+    static constexpr int MINB = (WARPS / W) > 0 ? (WARPS / W) : 1;
+};
+
+template <int NT, int W, bool SPLIT>
+__global__ void __launch_bounds__(32 * W, mut_cfg<NT, W>::MINB) p2p_mutual_kernel(int N, double gb, const int32_t *__restrict__ order, const int32_t *__restrict__ off,
+                                                         const int32_t *__restrict__ src, const int32_t *__restrict__ dst,
+                                                         const int32_t *__restrict__ node_lo, const int32_t *__restrict__ node_hi,
+                                                         const double *__restrict__ tx, const double *__restrict__ ty,
+                                                         const double *__restrict__ tz, const double *__restrict__ w0,
+                                                         const double *__restrict__ w1, const double *__restrict__ w2,
+                                                         const double *__restrict__ w3, int K, double *__restrict__ near_,
+                                                         double *__restrict__ react, size_t rstride)
+{
+    __shared__ mut_tile S;
+    __shared__ double mut_red[W > 1 ? W * 192 : 1];  // [W][6][32]
+    const int t = SPLIT ? order[blockIdx.x / K] : order[blockIdx.x], kc = SPLIT ? blockIdx.x % K : 0;
+    const int tlo = node_lo[t], thi = node_hi[t];
+    const int r0 = off[t], rl = off[t + 1] - r0;
+    const int e0 = SPLIT ? r0 + (int)(((int64_t)rl * kc) / K) : r0, e1 = SPLIT ? r0 + (int)(((int64_t)rl * (kc + 1)) / K) : r0 + rl;
+    mut_targets<NT> T;
+#pragma unroll
+    for (int k = 0; k < NT; ++k) {
+        const int i = tlo + k * blockDim.x + threadIdx.x;
+        const bool live = i < thi;
+        T.x[k] = live ? tx[i] : 0.0; T.y[k] = live ? ty[i] : 0.0; T.z[k] = live ? tz[i] : 0.0;
+        T.q0[k] = live ? w0[i] : 0.0; T.q1[k] = live ? w1[i] : 0.0; T.q2[k] = live ? w2[i] : 0.0; T.q3[k] = live ? w3[i] : 0.0;
+        T.ex[k] = T.ey[k] = T.ez[k] = T.bx[k] = T.by[k] = T.bz[k] = 0.0;
+    }
+    // the row is walked twice: first the owned mutual entries (pass 0), then the one-sided ones (pass 1); the sources of a
+    // pass form one stream that fills the tile across entry boundaries, so only the last tile of a pass is ragged
+    for (int pass = 0; pass < 2; ++pass) {
+        int fill = 0;
+        for (int e = e0; e <= e1; ++e) {
+            int slo = 0, shi = 0, d = -1;
+            const bool flush = (e == e1);
+            if (!flush) {
+                d = dst[e];
+                if (pass == 0 ? (d < 0) : (d != -1)) continue;
+                const int s = src[e];
+                slo = node_lo[s]; shi = node_hi[s];
+            }
+            int j0 = slo;
+            while (j0 < shi || (flush && fill > 0)) {
+                if (!flush) {
+                    const int n = min(shi - j0, MUT_TILE - fill);
+                    for (int j = threadIdx.x; j < n; j += blockDim.x) {
+                        const int a = fill + j, g = j0 + j;
+                        S.x[a] = tx[g]; S.y[a] = ty[g]; S.z[a] = tz[g];
+                        S.m0[a] = w0[g]; S.m1[a] = w1[g]; S.m2[a] = w2[g]; S.m3[a] = w3[g];
+                        S.dst[a] = d + (g - slo);
+                    }
+                    fill += n; j0 += n;
+                    if (fill < MUT_TILE) break;  // (this entry is exhausted)
+                } else if (pass == 0) {
+                    const int padded = (fill + 31) & ~31;  // dead sources: zero weights, nowhere to store
+                    for (int a = fill + threadIdx.x; a < padded; a += blockDim.x) {
+                        S.x[a] = S.y[a] = S.z[a] = S.m0[a] = S.m1[a] = S.m2[a] = S.m3[a] = 0.0;
+                        S.dst[a] = -1;
+                    }
+                    fill = padded;
+                }
+                __syncthreads();
+                if (pass == 0) mut_process_mutual<NT, W>(T, S, fill, gb, mut_red, react, rstride);
+                else mut_process_onesided<NT>(T, S, fill, gb);
+                __syncthreads();
+                fill = 0;
+            }
+        }
+    }
+#pragma unroll
+    for (int k = 0; k < NT; ++k) {
+        const int i = tlo + k * blockDim.x + threadIdx.x;
+        if (i < thi) {
+            double *o = near_ + (SPLIT ? (size_t)kc * 6 * (size_t)N : (size_t)0) + i;
+            o[0] = T.ex[k];
+            o[(size_t)N] = T.ey[k];
+            o[2 * (size_t)N] = T.ez[k];
+            o[3 * (size_t)N] = T.bx[k];
+            o[4 * (size_t)N] = T.by[k];
+            o[5 * (size_t)N] = T.bz[k];
+        }
+    }
+}
+
 // Targets per thread: the NT <= 4 that wastes the fewest lanes, ties to the larger NT (a leaf of 78 particles fills 3 x 32 slots at NT = 3 but only 78 of 128 at NT = 4).
-static void p2p_shape(int64_t leaves, int maxleaf, int64_t pairs, int64_t max_row, int *nt_out, int *threads_out, int *split_out)
+// Mutual kernel (mutual != 0): a whole leaf in one pass, the fewest warps W with NT <= 4, then the smallest NT; the travelling
+// reaction sums cost the same per step whatever NT is, so NT is kept high (NT < 4 only with W <= 3).
+static void p2p_shape(int64_t leaves, int maxleaf, int64_t pairs, int64_t max_row, int *nt_out, int *threads_out, int *split_out,
+                      int mutual = 0)
 {
     int best_nt = 1, best_threads = 32;
     double best_score = -1.0;
-    for (int nt = 1; nt <= 4; ++nt) {
+    if (mutual && maxleaf <= 1024) {
+        const int W = (maxleaf + 127) / 128 > 0 ? (maxleaf + 127) / 128 : 1;
+        best_threads = 32 * W;
+        best_nt = (maxleaf + best_threads - 1) / best_threads;
+        if (best_nt < 1) best_nt = 1;
+        best_score = 1.0;
+    }
+    for (int nt = 1; nt <= 4 && best_score < 0.0; ++nt) {
         int per = (maxleaf + nt - 1) / nt;
         int threads = ((per + 31) / 32) * 32;
         if (threads > 256) threads = 256;
@@ -207,13 +426,24 @@ int pairs_m2l_prepare(fmm_plan *p)  // after the lists: M2L row split for small 
     return FMM_OK;
 }
 
+// the mutual kernel keeps a whole target leaf in one pass of NT x blockDim registers
+static bool p2p_use_mutual(const fmm_plan *p, int maxleaf) { return p->p2p_dst != NULL && maxleaf <= 1024; }
+
 int pairs_p2p_prepare(fmm_plan *p)  // after the lists: choose the row split and size the partial buffers
 {
     fmm_ctx *c = &p->ctx;
     int maxleaf = (int)((p->N + p->leaves - 1) / p->leaves);
     int nt, threads, K;
-    p2p_shape(p->leaves, maxleaf, p->p2p_pairs, p->p2p_max_row, &nt, &threads, &K);
+    p2p_shape(p->leaves, maxleaf, p->p2p_work, p->p2p_max_row, &nt, &threads, &K, p2p_use_mutual(p, maxleaf));
     p->p2p_split = K;
+    if (p2p_use_mutual(p, maxleaf) && p->p2p_react > p->react_cap) {
+        if (p->p2p_react >= ((int64_t)1 << 31)) return FMM_EOVERFLOW;
+        if (p->react) ctx_free(c, p->react);
+        p->react_cap = 0;
+        p->react = (double *)ctx_alloc(c, sizeof(double) * 6 * (size_t)p->p2p_react);
+        if (!p->react) return FMM_ENOMEM;
+        p->react_cap = p->p2p_react;
+    }
     int64_t need = (int64_t)(K + ((p->flags & FMM_METHOD_TREECODE) ? 1 : 0)) * 6 * p->N;  // treecode: + the particle-cluster sums
     if (need > p->near_cap) {
         if (p->near_) ctx_free(c, p->near_);
@@ -229,9 +459,39 @@ int pairs_p2p(fmm_plan *p)
     fmm_ctx *c = &p->ctx;
     int maxleaf = (int)((p->N + p->leaves - 1) / p->leaves);
     int nt, threads, K;
-    p2p_shape(p->leaves, maxleaf, p->p2p_pairs, p->p2p_max_row, &nt, &threads, &K);
+    p2p_shape(p->leaves, maxleaf, p->p2p_work, p->p2p_max_row, &nt, &threads, &K, p2p_use_mutual(p, maxleaf));
     K = p->p2p_split;
     const bool sm = (p->flags & FMM_KERNEL_SOURCE_MOMENTUM) != 0;
+    p->react_used = p2p_use_mutual(p, maxleaf) ? 1 : 0;
+    if (p->react_used) {
+        const size_t rstride = (size_t)(p->react_cap > 0 ? p->react_cap : 1);
+#define MUT_LAUNCH(NT, W)                                                                                                                 \
+    if (K > 1)                                                                                                                            \
+        p2p_mutual_kernel<NT, W, true><<<(unsigned)(p->leaves * K), 32 * W, 0, c->stream>>>(                                              \
+            (int)p->N, p->gamma_bar, p->p2p_order, p->p2p_off, p->p2p_src, p->p2p_dst, p->node_lo, p->node_hi, p->tx, p->ty, p->tz, p->w0, \
+            p->w1, p->w2, p->w3, K, p->near_, p->react, rstride);                                                                         \
+    else                                                                                                                                  \
+        p2p_mutual_kernel<NT, W, false><<<(unsigned)p->leaves, 32 * W, 0, c->stream>>>(                                                   \
+            (int)p->N, p->gamma_bar, p->p2p_order, p->p2p_off, p->p2p_src, p->p2p_dst, p->node_lo, p->node_hi, p->tx, p->ty, p->tz, p->w0, \
+            p->w1, p->w2, p->w3, K, p->near_, p->react, rstride)
+        const int W = threads / 32;
+        if (nt == 1) { MUT_LAUNCH(1, 1); }
+        else if (nt == 2) { MUT_LAUNCH(2, 1); }
+        else if (nt == 3 && W == 1) { MUT_LAUNCH(3, 1); }
+        else if (nt == 3 && W == 2) { MUT_LAUNCH(3, 2); }
+        else if (nt == 3) { MUT_LAUNCH(3, 3); }
+        else if (W == 1) { MUT_LAUNCH(4, 1); }
+        else if (W == 2) { MUT_LAUNCH(4, 2); }
+        else if (W == 3) { MUT_LAUNCH(4, 3); }
+        else if (W == 4) { MUT_LAUNCH(4, 4); }
+        else if (W == 5) { MUT_LAUNCH(4, 5); }
+        else if (W == 6) { MUT_LAUNCH(4, 6); }
+        else if (W == 7) { MUT_LAUNCH(4, 7); }
+        else { MUT_LAUNCH(4, 8); }
+#undef MUT_LAUNCH
+        FMM_LAUNCH_CHECK(c, "p2p_mutual_kernel");
+        return FMM_OK;
+    }
 #define P2P_LAUNCH(NT, SM)                                                                                                               \
     if (K > 1)                                                                                                                           \
         p2p_kernel<NT, SM, true><<<(unsigned)(p->leaves * K), threads, 0, c->stream>>>((int)p->N, p->gamma_bar, p->p2p_order, p->p2p_off, \
@@ -843,7 +1103,7 @@ int pairs_pc(fmm_plan *p)  // treecode: particle-cluster sums into partial buffe
     FMM_LAUNCH_CHECK(c, "m2l_proxy_points");
     int maxleaf = (int)((p->N + p->leaves - 1) / p->leaves);
     int nt, threads, K;
-    p2p_shape(p->leaves, maxleaf, p->p2p_pairs, p->p2p_max_row, &nt, &threads, &K);
+    p2p_shape(p->leaves, maxleaf, p->p2p_work, p->p2p_max_row, &nt, &threads, &K);
 #define PC_LAUNCH(NT)                                                                                                            \
     pc_kernel<NT><<<(unsigned)p->nodes, threads, 0, c->stream>>>((int)p->N, p->n1, p->gamma_bar, p->m2l_order, p->m2l_off, p->m2l_src, \
                                                                  p->node_lo, p->node_hi, p->tx, p->ty, p->tz, p->node_xi, p->M,  \

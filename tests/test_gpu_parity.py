@@ -355,3 +355,82 @@ def test_treecode_cross_checks_the_fmm(fmm):
     ea, eb = oracle.err2(Ea, Ed), oracle.err2(Eb, Ed)
     assert eb < 1.5 * ea and oracle.err2(Ea, Eb) < 2 * ea, (ea, eb)
     a.close(); b.close()
+
+
+# ---------------------------------------------------------------------------------------------
+# mutual near field: one block evaluates a pair of leaves for both directions; entries whose reverse pair is
+# missing from the list (after a radius tie in Alg 5.11, reading D-3) must take the one-sided path
+# ---------------------------------------------------------------------------------------------
+def _mirrored_bunch(N_half, seed):
+    rng = np.random.default_rng(seed)
+    x = rng.uniform(0.01, 4.0, N_half)
+    y = rng.uniform(-0.5, 0.5, N_half)
+    z = rng.uniform(-0.05, 0.05, N_half)
+    X = np.concatenate([x, -x]); Y = np.concatenate([y, y]); Z = np.concatenate([z, z])
+    N = 2 * N_half
+    px, py = 1e-2 * rng.standard_normal(N), 1e-2 * rng.standard_normal(N)
+    pz = 3.0 * (1.0 + 0.05 * rng.standard_normal(N))
+    q = rng.uniform(0.5, 2.0, N)
+    return X, Y, Z, px, py, pz, q
+
+
+@pytest.mark.parametrize("theta,seed,N_half,N0", [(0.5, 7, 512, 16), (0.3, 7, 1024, 8), (0.5, 3, 2048, 32), (0.5, 9, 1024, 8)])
+def test_mutual_near_field_handles_one_sided_entries(fmm, theta, seed, N_half, N0):
+    X, Y, Z, px, py, pz, q = _mirrored_bunch(N_half, seed)
+    plan = fmm.fmm_plan_create(X, Y, Z, px, py, pz, q, order_n=3, leaf_size=N0, theta=theta, flags=fmm.FMM_RAW_SUMS)
+    st = plan.stats()
+    ex = plan.export()
+    op = oracle.Plan(X, Y, Z, px, py, pz, q, order_n=3, leaf_size=N0, theta=theta, gamma_bar_value=st["gamma_bar"], raw=True)
+    p2p, _ = op.lists()
+    tgt = np.repeat(np.arange(1, st["nodes"] + 1, dtype=np.int32), np.diff(ex["p2p_off"]))
+    assert np.array_equal(tgt, p2p[:, 0]) and np.array_equal(ex["p2p_src"], p2p[:, 1])
+    pairs = set(map(tuple, p2p))
+    mateless = sum((s, t) not in pairs for t, s in pairs)
+    if (theta, seed) != (0.5, 9):
+        assert mateless > 0, "this input is meant to contain entries without a reverse pair"
+    E, B = to_np(plan.eval())
+    Eo, Bo = op.eval()
+    assert_close(E, Eo, f"mutual near field E ({mateless} one-sided entries)")
+    assert_close(B, Bo, f"mutual near field B ({mateless} one-sided entries)")
+    plan.close()
+
+
+@pytest.mark.parametrize("N,N0,n", [(5000, 300, 2), (7001, 700, 2), (2500, 1000, 3), (1300, 1300, 2), (20000, 33, 2)])
+def test_mutual_near_field_leaf_shapes(fmm, N, N0, n):
+    """Leaves of 157 / 438 / 625 / 1300 (one leaf, more than 1024 particles: one-sided kernel) / 20 particles: every
+    (targets per thread, warps per block) shape of the near-field kernels, ragged last tiles, many entries per tile."""
+    w = workloads.config(2, N=N)
+    plan = fmm.fmm_plan_create(*w.arrays(), w.q, order_n=n, leaf_size=N0, theta=0.5)
+    st = plan.stats()
+    E, B = to_np(plan.eval())
+    Eo, Bo = oracle.Plan(*w.arrays(), w.q, order_n=n, leaf_size=N0, theta=0.5, gamma_bar_value=st["gamma_bar"]).eval()
+    assert_close(E, Eo, "E")
+    assert_close(B, Bo, "B")
+    plan.close()
+
+
+def test_plan_on_one_stream_evaluated_under_another(fmm):
+    """the library works on the stream given at fmm_plan_create and frees scratch right after enqueueing; the
+    binding must therefore run every later call on that stream, whatever torch's current stream is."""
+    import torch
+    w = workloads.config(2, N=15000)
+    dev = torch.device("cuda", 0)
+    ref_plan = fmm.fmm_plan_create(*w.arrays(), w.q, order_n=4, leaf_size=64, theta=0.5)
+    Eref, Bref = to_np(ref_plan.eval())
+    ref_plan.close()
+    sa, sb = torch.cuda.Stream(dev), torch.cuda.Stream(dev)
+    with torch.cuda.stream(sa):
+        plan = fmm.fmm_plan_create(*w.arrays(), w.q, order_n=4, leaf_size=64, theta=0.5)
+    assert plan.stream == sa
+    d_in = [torch.as_tensor(a).to(dev) for a in w.arrays()]
+    junk = []
+    with torch.cuda.stream(sb):
+        for _ in range(3):
+            plan.update(*d_in, w.q)
+            junk.append(torch.full((1 << 22,), 7.0, device=dev))   # allocator pressure on stream B's pool
+            E, B = plan.eval()
+            E2 = E * 1.0                                          # consumer on stream B right after the call
+        sb.synchronize()
+    assert np.array_equal(E2.cpu().numpy().T, Eref)
+    assert np.array_equal(to_np((E, B))[1], Bref)
+    plan.close()
