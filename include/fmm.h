@@ -20,14 +20,27 @@
  *              are read-only and need not outlive the call that takes them.
  *   Workspace  every byte of device workspace is obtained through the caller's allocator
  *              (fmm_alloc_fn / fmm_free_fn, e.g. PyTorch's caching allocator).  If both are
- *              NULL the library uses cudaMalloc / cudaFree.  A plan frees its workspace in
- *              fmm_plan_destroy.
+ *              NULL the library uses cudaMallocAsync / cudaFreeAsync on `cuda_stream`.  The
+ *              allocator must be STREAM-ORDERED on `cuda_stream`: the library hands scratch
+ *              back (free_) right after enqueueing the kernels that use it, while they may
+ *              still be pending, so a block may be handed out again only to work that is
+ *              enqueued on the same stream (PyTorch's allocator behaves like this for the
+ *              stream that was current at allocation; the Python binding therefore runs every
+ *              call of a plan under the stream the plan was created on).  A plan frees its
+ *              remaining workspace in fmm_plan_destroy.
  *   Stream     all work is enqueued on `cuda_stream` (a cudaStream_t passed as void*; NULL =
  *              the legacy default stream).  fmm_plan_create / fmm_plan_update synchronise the
  *              stream internally (the interaction-list lengths must be read back to size the
  *              lists); fmm_eval and fmm_direct only enqueue and return.
- *   Errors     0 on success, a negative FMM_E* code otherwise; no exceptions, no exit(), no
- *              global state.  Outputs are unspecified after an error.
+ *   Errors     0 on success, a negative FMM_E* code otherwise; no exceptions, no exit().
+ *              Outputs are unspecified after an error.  A plan whose fmm_plan_update /
+ *              fmm_plan_refit failed is marked invalid: fmm_eval returns FMM_EINVAL for it
+ *              until a later update / refit succeeds (or destroy it).
+ *   Globals    the library keeps three process-wide items, none of which carries results from
+ *              one call to another: the launch counter behind fmm_launch_count, one side
+ *              stream per device (fmm_plan_set_overlap), and a per-device flag that the table
+ *              of Chebyshev points has been uploaded to constant memory.  Plans are otherwise
+ *              independent; one plan must not be used from two threads at once.
  *   Order      outputs are in the caller's particle order.
  *   Units      SI; eps0 = 8.8541878128e-12 F/m, c0 = 299792458 m/s (CODATA 2018), unless
  *              FMM_RAW_SUMS is set (then the bare sums without prefactors are returned).
@@ -72,7 +85,8 @@ extern "C" {
                                        theta <= 0 or non-finite, NULL pointer                    */
 #define FMM_ENOMEM     -2           /* the allocator returned NULL                               */
 #define FMM_ECUDA      -3           /* a CUDA call failed; text in fmm_last_error                */
-#define FMM_ENONFINITE -4           /* gamma_bar came out non-finite (NaN / Inf in the momenta)  */
+#define FMM_ENONFINITE -4           /* NaN or Inf among x, y, z, px, py, pz, q (one fused scan in
+                                       step a0), or the caller's gamma_bar is not finite          */
 #define FMM_EOVERFLOW  -5           /* an interaction list exceeds 2^31-1 entries                */
 
 typedef struct fmm_plan fmm_plan_t; /* opaque; owns its device workspace                          */

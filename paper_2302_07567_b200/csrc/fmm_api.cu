@@ -112,7 +112,7 @@ extern "C" const char *fmm_strerror(int code)
         case FMM_EINVAL: return "invalid argument";
         case FMM_ENOMEM: return "device allocator returned NULL";
         case FMM_ECUDA: return "CUDA error";
-        case FMM_ENONFINITE: return "gamma_bar is not finite (NaN/Inf in the momenta)";
+        case FMM_ENONFINITE: return "NaN or Inf among the positions, momenta or charges";
         case FMM_EOVERFLOW: return "interaction list exceeds 2^31-1 entries";
     }
     return "unknown error code";
@@ -140,6 +140,7 @@ static int plan_alloc_fixed(fmm_plan *p)
         ALLOC(pmx, double, N); ALLOC(pmy, double, N); ALLOC(pmz, double, N);
     }
     ALLOC(perm, int32_t, N);
+    ALLOC(hdr, fmm_hdr, 1);
     ALLOC(node_lo, int32_t, nodes1); ALLOC(node_hi, int32_t, nodes1);
     ALLOC(bbox, double, 6 * nodes1); ALLOC(node_geo, double, 4 * nodes1);
     ALLOC(node_xi, double, 48 * nodes1);
@@ -154,16 +155,12 @@ static int plan_alloc_fixed(fmm_plan *p)
 static int plan_build(fmm_plan *p, const fmm_particles_t *in, bool refit = false)
 {
     fmm_ctx *c = &p->ctx;
+    p->valid = 0;  // a build that fails part-way leaves lists that must not be used (fmm_eval then returns FMM_EINVAL)
     FMM_CUDA(c, cudaEventRecord(p->ev_plan[0], c->stream));
-    if (p->gamma_bar_param > 0.0) {
-        p->gamma_bar = p->gamma_bar_param;
-    } else {
-        FMM_TRY(tree_gamma_bar(c, p->N, in->px, in->py, in->pz, &p->gamma_bar));
-        if (!isfinite(p->gamma_bar)) return FMM_ENONFINITE;
-    }
+    FMM_TRY(tree_scan_inputs(p, in));  // a0: gamma_bar, coordinate ranges, input check -> p->hdr (device)
     FMM_TRY(refit ? tree_refit(p, in) : tree_build(p, in));
     FMM_CUDA(c, cudaEventRecord(p->ev_plan[1], c->stream));
-    FMM_TRY(dtt_build_lists(p));
+    FMM_TRY(dtt_build_lists(p));       // (reads gamma_bar and the input check back together with the list lengths)
     FMM_TRY(pairs_p2p_prepare(p));
     FMM_TRY(pairs_m2l_prepare(p));
     FMM_CUDA(c, cudaEventRecord(p->ev_plan[2], c->stream));
@@ -171,6 +168,7 @@ static int plan_build(fmm_plan *p, const fmm_particles_t *in, bool refit = false
     FMM_CUDA(c, cudaEventElapsedTime(&p->ms_tree, p->ev_plan[0], p->ev_plan[1]));
     FMM_CUDA(c, cudaEventElapsedTime(&p->ms_lists, p->ev_plan[1], p->ev_plan[2]));
     p->ev_valid = 0;
+    p->valid = 1;
     return FMM_OK;
 }
 
@@ -273,6 +271,10 @@ extern "C" int fmm_plan_set_timing(fmm_plan_t *p, int on)
 extern "C" int fmm_eval(fmm_plan_t *p, double *Ex, double *Ey, double *Ez, double *Bx, double *By, double *Bz)
 {
     if (!p || !Ex || !Ey || !Ez || !Bx || !By || !Bz) return FMM_EINVAL;
+    if (!p->valid) {
+        snprintf(p->ctx.err, sizeof(p->ctx.err), "the last fmm_plan_update / fmm_plan_refit of this plan failed: its lists are not usable");
+        return FMM_EINVAL;
+    }
     if (p->flags & FMM_METHOD_TREECODE) {  // P2M, M2M, particle-cluster + P2P, finalise (no M2L / L2L / far L2P)
         MARK(p, EV_P2M);
         FMM_TRY(interp_p2m(p));

@@ -50,6 +50,16 @@ int ctx_cuda_fail(fmm_ctx *c, cudaError_t e, const char *what);
         if (rc__ != FMM_OK) return rc__; \
     } while (0)
 
+// Device-resident scalars of one plan build (step a0), read by every kernel that needs them, so that the build
+// never waits for the host between a0 and the traversal.
+struct fmm_hdr {
+    double gamma_bar;        // sqrt(1 + pbar.pbar), or the caller's value
+    double g2;               // gamma_bar * gamma_bar (one rounding), the stretch of eq. (3.2)
+    double mm[6];            // min x, y, z / max x, y, z of the positions
+    unsigned int nonfinite;  // number of NaN / Inf values among x, y, z, px, py, pz, q (saturating) + 1 if gamma_bar is not finite
+    unsigned int pad;
+};
+
 enum { EV_P2M = 0, EV_M2M, EV_M2L, EV_L2L, EV_P2P, EV_L2P, EV_END, EV_COUNT };
 
 struct fmm_plan {
@@ -58,6 +68,8 @@ struct fmm_plan {
     int n, n1, P, N0, kappa;
     int64_t nodes, leaves;
     double theta, gamma_bar, gamma_bar_param;
+    fmm_hdr *hdr;           // device
+    int valid;              // 0 after a failed build: fmm_eval refuses the plan until an update / refit succeeds
     uint32_t flags;
     // particles in tree order (SoA), source weights w0 = q gamma, w1..3 = q p
     double *tx, *ty, *tz, *w0, *w1, *w2, *w3;
@@ -108,7 +120,8 @@ struct fmm_plan {
 
 // ---- kernels_tree.cu ----------------------------------------------------------------
 int tree_gamma_bar(fmm_ctx *c, int64_t N, const double *px, const double *py, const double *pz,
-                   double *gamma_bar_out /* host */);
+                   double *gamma_bar_out /* host */);  // plan-less calls (fmm_direct): synchronises
+int tree_scan_inputs(fmm_plan *p, const fmm_particles_t *in);  // a0 into p->hdr, enqueue only
 int tree_build(fmm_plan *p, const fmm_particles_t *in);
 int tree_boxes(fmm_plan *p);
 int tree_refit(fmm_plan *p, const fmm_particles_t *in);  // keeps the particle order of the last build

@@ -29,7 +29,7 @@ __global__ void dtt_init(dtt_counters *cnt, uint64_t *front0, int treecode_leave
     if (k0 < treecode_leaves) front0[k0] = ((uint64_t)(treecode_leaves + k0) << 32) | 1ull;  // (leaf, root)
 }
 
-__global__ void __launch_bounds__(256) dtt_step(int step, int leaves, double gamma_bar, double theta2,
+__global__ void __launch_bounds__(256) dtt_step(int step, int leaves, const fmm_hdr *__restrict__ hdr, double theta2,
                                                 const int32_t *__restrict__ node_lo, const int32_t *__restrict__ node_hi,
                                                 const double *__restrict__ geo, const uint64_t *__restrict__ front_in,
                                                 uint64_t *__restrict__ front_out, unsigned int cap_front,
@@ -37,6 +37,8 @@ __global__ void __launch_bounds__(256) dtt_step(int step, int leaves, double gam
                                                 uint64_t *__restrict__ m2l, unsigned int cap_m2l,
                                                 int key_shift, dtt_counters *cnt)
 {
+    if (hdr->nonfinite) return;  // NaN / Inf in the inputs: no lists (FMM_ENONFINITE after the read-back)
+    const double gamma_bar = hdr->gamma_bar;
     unsigned int nin = cnt->n_front[step];
     if (nin > cap_front) nin = cap_front;
     for (unsigned int k = blockIdx.x * blockDim.x + threadIdx.x; k < nin; k += gridDim.x * blockDim.x) {
@@ -231,14 +233,22 @@ int dtt_build_lists(fmm_plan *p)
         FMM_LAUNCH_CHECK(c, "dtt_init");
         uint64_t *fin = f0, *fout = f1;
         for (int step = 0; step < nsteps; ++step) {
-            dtt_step<<<2 * FMM_SM_COUNT, 256, 0, st>>>(step, (int)p->leaves, p->gamma_bar, p->theta * p->theta, p->node_lo, p->node_hi,
+            dtt_step<<<2 * FMM_SM_COUNT, 256, 0, st>>>(step, (int)p->leaves, p->hdr, p->theta * p->theta, p->node_lo, p->node_hi,
                                                        p->node_geo, fin, fout, (unsigned)cap, kp2p, (unsigned)cap, km2l, (unsigned)cap,
                                                        key_shift, cnt);
             FMM_LAUNCH_CHECK(c, "dtt_step");
             uint64_t *t = fin; fin = fout; fout = t;
         }
+        fmm_hdr hh;
         FMM_CUDA(c, cudaMemcpyAsync(&h, cnt, sizeof(h), cudaMemcpyDeviceToHost, st));
-        FMM_CUDA(c, cudaStreamSynchronize(st));
+        FMM_CUDA(c, cudaMemcpyAsync(&hh, p->hdr, sizeof(hh), cudaMemcpyDeviceToHost, st));
+        FMM_CUDA(c, cudaStreamSynchronize(st));  // the one host wait of a build: list lengths, gamma_bar, the input check
+        p->gamma_bar = hh.gamma_bar;
+        if (hh.nonfinite) {
+            ctx_free(c, f0); ctx_free(c, f1); ctx_free(c, kp2p); ctx_free(c, km2l); ctx_free(c, cnt);
+            snprintf(c->err, sizeof(c->err), "%u non-finite values among the positions, momenta and charges (or gamma_bar is not finite)", hh.nonfinite);
+            return FMM_ENONFINITE;
+        }
         ctx_free(c, f0); ctx_free(c, f1);
         if (!h.overflow) break;
         ctx_free(c, kp2p); ctx_free(c, km2l);

@@ -109,6 +109,119 @@ int tree_gamma_bar(fmm_ctx *c, int64_t N, const double *px, const double *py, co
 }
 
 // ---------------------------------------------------------------------------------------
+// a0 for a plan: one pass over the inputs gives the momentum sums (same fixed grid and reduction tree as above), the
+// coordinate ranges (Morton keys, sort keys) and the number of non-finite input values (FMM_ENONFINITE); the result
+// stays on the device (fmm_hdr).
+// ---------------------------------------------------------------------------------------
+#define A0_STRIDE 10  // per block: 3 momentum sums, 3 minima, 3 maxima, non-finite count
+
+__global__ void __launch_bounds__(RED_THREADS) a0_scan_partial(int64_t N, const double *__restrict__ x, const double *__restrict__ y,
+                                                               const double *__restrict__ z, const double *__restrict__ px,
+                                                               const double *__restrict__ py, const double *__restrict__ pz,
+                                                               const double *__restrict__ q, double *__restrict__ partial)
+{
+    __shared__ double sm[8];
+    __shared__ double smm[6][8];
+    __shared__ int sbad[8];
+    double sx = 0.0, sy = 0.0, sz = 0.0;
+    double lo[3] = {INFINITY, INFINITY, INFINITY}, hi[3] = {-INFINITY, -INFINITY, -INFINITY};
+    int bad = 0;
+    for (int64_t j = (int64_t)blockIdx.x * RED_THREADS + threadIdx.x; j < N; j += (int64_t)RED_BLOCKS * RED_THREADS) {
+        const double ax = px[j], ay = py[j], az = pz[j], vx = x[j], vy = y[j], vz = z[j];
+        sx += ax; sy += ay; sz += az;
+        lo[0] = fmin(lo[0], vx); hi[0] = fmax(hi[0], vx);
+        lo[1] = fmin(lo[1], vy); hi[1] = fmax(hi[1], vy);
+        lo[2] = fmin(lo[2], vz); hi[2] = fmax(hi[2], vz);
+        bad += !isfinite(ax) + !isfinite(ay) + !isfinite(az) + !isfinite(vx) + !isfinite(vy) + !isfinite(vz);
+        if (q) bad += !isfinite(q[j]);
+    }
+    sx = block_sum_256(sx, sm);
+    sy = block_sum_256(sy, sm);
+    sz = block_sum_256(sz, sm);
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+#pragma unroll
+    for (int k = 0; k < 3; ++k) {
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+            lo[k] = fmin(lo[k], __shfl_down_sync(0xffffffffu, lo[k], o));
+            hi[k] = fmax(hi[k], __shfl_down_sync(0xffffffffu, hi[k], o));
+        }
+        if (lane == 0) { smm[k][warp] = lo[k]; smm[3 + k][warp] = hi[k]; }
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) bad += __shfl_down_sync(0xffffffffu, bad, o);
+    if (lane == 0) sbad[warp] = bad;
+    __syncthreads();
+    double *out = partial + (size_t)A0_STRIDE * blockIdx.x;
+    if (threadIdx.x == 0) {
+        out[0] = sx; out[1] = sy; out[2] = sz;
+        int b = 0;
+        for (int w = 0; w < 8; ++w) b += sbad[w];
+        out[9] = (double)b;
+    }
+    if (threadIdx.x < 6) {
+        double v = smm[threadIdx.x][0];
+        for (int w = 1; w < 8; ++w) v = (threadIdx.x < 3) ? fmin(v, smm[threadIdx.x][w]) : fmax(v, smm[threadIdx.x][w]);
+        out[3 + threadIdx.x] = v;
+    }
+}
+
+// one warp: lane l adds the blocks l, l + 32, ... in order, then the lanes are added by a fixed shuffle tree
+__global__ void a0_scan_final(int64_t N, double gamma_bar_param, const double *__restrict__ partial, fmm_hdr *__restrict__ hdr)
+{
+    const int lane = threadIdx.x;
+    double s[3] = {0.0, 0.0, 0.0}, lo[3] = {INFINITY, INFINITY, INFINITY}, hi[3] = {-INFINITY, -INFINITY, -INFINITY}, bad = 0.0;
+    for (int b = lane; b < RED_BLOCKS; b += 32) {
+        const double *pb = partial + (size_t)A0_STRIDE * b;
+#pragma unroll
+        for (int k = 0; k < 3; ++k) {
+            s[k] += pb[k];
+            lo[k] = fmin(lo[k], pb[3 + k]);
+            hi[k] = fmax(hi[k], pb[6 + k]);
+        }
+        bad += pb[9];
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+#pragma unroll
+        for (int k = 0; k < 3; ++k) {
+            s[k] += __shfl_down_sync(0xffffffffu, s[k], o);
+            lo[k] = fmin(lo[k], __shfl_down_sync(0xffffffffu, lo[k], o));
+            hi[k] = fmax(hi[k], __shfl_down_sync(0xffffffffu, hi[k], o));
+        }
+        bad += __shfl_down_sync(0xffffffffu, bad, o);
+    }
+    if (lane == 0) {
+        double gb = gamma_bar_param;
+        if (!(gb > 0.0)) {
+            const double mx = s[0] / (double)N, my = s[1] / (double)N, mz = s[2] / (double)N;
+            gb = sqrt(1.0 + (mx * mx + my * my + mz * mz));  // gamma_bar^2 = 1 + pbar.pbar
+        }
+        hdr->gamma_bar = gb;
+        hdr->g2 = __dmul_rn(gb, gb);
+#pragma unroll
+        for (int k = 0; k < 3; ++k) { hdr->mm[k] = lo[k]; hdr->mm[3 + k] = hi[k]; }
+        unsigned int nb = bad > 4.0e9 ? 4000000000u : (unsigned int)bad;
+        if (!isfinite(gb)) nb += 1u;
+        hdr->nonfinite = nb;
+        hdr->pad = 0;
+    }
+}
+
+int tree_scan_inputs(fmm_plan *p, const fmm_particles_t *in)
+{
+    fmm_ctx *c = &p->ctx;
+    double *partial = (double *)ctx_alloc(c, sizeof(double) * A0_STRIDE * RED_BLOCKS);
+    if (!partial) return FMM_ENOMEM;
+    a0_scan_partial<<<RED_BLOCKS, RED_THREADS, 0, c->stream>>>(p->N, in->x, in->y, in->z, in->px, in->py, in->pz, in->q, partial);
+    FMM_LAUNCH_CHECK(c, "a0_scan_partial");
+    a0_scan_final<<<1, 32, 0, c->stream>>>(p->N, p->gamma_bar_param, partial, p->hdr);
+    FMM_LAUNCH_CHECK(c, "a0_scan_final");
+    ctx_free(c, partial);
+    return FMM_OK;
+}
+
+// ---------------------------------------------------------------------------------------
 // a1, mode KD
 // ---------------------------------------------------------------------------------------
 // total order of doubles as unsigned keys; -0.0 == +0.0 (the oracle compares with <, so they tie)
@@ -137,10 +250,11 @@ __global__ void kd_iota(int N, uint32_t *__restrict__ v)
 // are sorted by coordinate inside every node segment, so the bounding box is read off the segment ends.
 __global__ void kd_choose_axis(int N, int level, const double *__restrict__ x, const double *__restrict__ y, const double *__restrict__ z,
                                const uint32_t *__restrict__ LX, const uint32_t *__restrict__ LY, const uint32_t *__restrict__ LZ,
-                               double gamma_bar, int8_t *__restrict__ axis /* [2^level] */)
+                               const fmm_hdr *__restrict__ hdr, int8_t *__restrict__ axis /* [2^level] */)
 {
     int k = blockIdx.x * blockDim.x + threadIdx.x;
     if (k >= (1 << level)) return;
+    const double gamma_bar = hdr->gamma_bar;
     int lo = 0, hi = N;
     for (int b = level - 1; b >= 0; --b) {
         int mid = lo + (hi - lo + 1) / 2;
@@ -272,43 +386,6 @@ __global__ void __launch_bounds__(256) kd_partition(int N, int level, const uint
 // ---------------------------------------------------------------------------------------
 // a1', mode MORTON_MEDIAN (DESIGN T-3')
 // ---------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(RED_THREADS) minmax_partial(int64_t N, const double *__restrict__ x, const double *__restrict__ y,
-                                                              const double *__restrict__ z, double *__restrict__ partial /* [RED_BLOCKS][6] */)
-{
-    __shared__ double sm[6][8];
-    double lo[3] = {INFINITY, INFINITY, INFINITY}, hi[3] = {-INFINITY, -INFINITY, -INFINITY};
-    for (int64_t j = (int64_t)blockIdx.x * RED_THREADS + threadIdx.x; j < N; j += (int64_t)RED_BLOCKS * RED_THREADS) {
-        lo[0] = fmin(lo[0], x[j]); hi[0] = fmax(hi[0], x[j]);
-        lo[1] = fmin(lo[1], y[j]); hi[1] = fmax(hi[1], y[j]);
-        lo[2] = fmin(lo[2], z[j]); hi[2] = fmax(hi[2], z[j]);
-    }
-    int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-#pragma unroll
-    for (int k = 0; k < 3; ++k) {
-#pragma unroll
-        for (int o = 16; o > 0; o >>= 1) {
-            lo[k] = fmin(lo[k], __shfl_down_sync(0xffffffffu, lo[k], o));
-            hi[k] = fmax(hi[k], __shfl_down_sync(0xffffffffu, hi[k], o));
-        }
-        if (lane == 0) { sm[k][warp] = lo[k]; sm[3 + k][warp] = hi[k]; }
-    }
-    __syncthreads();
-    if (threadIdx.x < 6) {
-        double v = sm[threadIdx.x][0];
-        for (int w = 1; w < 8; ++w) v = (threadIdx.x < 3) ? fmin(v, sm[threadIdx.x][w]) : fmax(v, sm[threadIdx.x][w]);
-        partial[6 * blockIdx.x + threadIdx.x] = v;
-    }
-}
-
-__global__ void minmax_final(const double *__restrict__ partial, double *__restrict__ out /* [6] */)
-{
-    if (threadIdx.x >= 6) return;
-    double v = partial[threadIdx.x];
-    for (int b = 1; b < RED_BLOCKS; ++b)
-        v = (threadIdx.x < 3) ? fmin(v, partial[6 * b + threadIdx.x]) : fmax(v, partial[6 * b + threadIdx.x]);
-    out[threadIdx.x] = v;
-}
-
 __device__ __forceinline__ uint64_t spread3(uint64_t v)  // 21 bits -> every third bit
 {
     v &= 0x1fffffull;
@@ -321,11 +398,13 @@ __device__ __forceinline__ uint64_t spread3(uint64_t v)  // 21 bits -> every thi
 }
 
 __global__ void morton_keys(int N, const double *__restrict__ x, const double *__restrict__ y, const double *__restrict__ z,
-                            const double *__restrict__ mm /* [6] min xyz, max xyz of the raw coordinates */, double gamma_bar,
+                            const fmm_hdr *__restrict__ hdr /* min xyz, max xyz of the raw coordinates, gamma_bar */,
                             uint64_t *__restrict__ keys, uint32_t *__restrict__ vals)
 {
     int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= N) return;
+    const double *mm = hdr->mm;
+    const double gamma_bar = hdr->gamma_bar;
     // u = s o x; s > 0 so min/max commute with the scaling (every operation rounded separately)
     double s[3] = {1.0, 1.0, gamma_bar};
     double lo[3], L = 0.0;
@@ -420,9 +499,10 @@ __global__ void leaf_bbox(int leaves, const int32_t *__restrict__ node_lo, const
 // squared radius (Alg 5.6) and the box centre (Alg 5.7) of every node, each
 // product and sum rounded separately (reading D-2) so that the traversal is bit-reproducible.
 __global__ void __launch_bounds__(1024) upper_bbox_and_geometry(int kappa, int nodes, const int32_t *__restrict__ node_lo,
-                                                                const int32_t *__restrict__ node_hi, double gamma_bar,
+                                                                const int32_t *__restrict__ node_hi, const fmm_hdr *__restrict__ hdr,
                                                                 double *__restrict__ bbox, double *__restrict__ geo)
 {
+    const double gamma_bar = hdr->gamma_bar;
     for (int level = kappa - 1; level >= 0; --level) {
         int first = 1 << level;
         for (int i = first + threadIdx.x; i < 2 * first; i += blockDim.x) {
@@ -496,7 +576,7 @@ int tree_build(fmm_plan *p, const fmm_particles_t *in)
         for (int level = 0; level < p->kappa; ++level) {
             int nn = 1 << level;
             kd_choose_axis<<<(nn + T - 1) / T, T, 0, st>>>(N, level, in->x, in->y, in->z, cur, cur + N, cur + 2 * (size_t)N,
-                                                           p->gamma_bar, axis);
+                                                           p->hdr, axis);
             FMM_LAUNCH_CHECK(c, "kd_choose_axis");
             kd_mark_left<<<gN, T, 0, st>>>(N, level, axis, cur, cur + N, cur + 2 * (size_t)N, left);
             FMM_LAUNCH_CHECK(c, "kd_mark_left");
@@ -513,20 +593,13 @@ int tree_build(fmm_plan *p, const fmm_particles_t *in)
         FMM_LAUNCH_CHECK(c, "permute_particles");
         ctx_free(c, lists2); ctx_free(c, scan); ctx_free(c, left); ctx_free(c, axis);
     } else {
-        double *mm = (double *)ctx_alloc(c, sizeof(double) * (6 * RED_BLOCKS + 6));
-        if (!mm) return FMM_ENOMEM;
-        minmax_partial<<<RED_BLOCKS, RED_THREADS, 0, st>>>(N, in->x, in->y, in->z, mm);
-        FMM_LAUNCH_CHECK(c, "minmax_partial");
-        minmax_final<<<1, 32, 0, st>>>(mm, mm + 6 * RED_BLOCKS);
-        FMM_LAUNCH_CHECK(c, "minmax_final");
-        morton_keys<<<gN, T, 0, st>>>(N, in->x, in->y, in->z, mm + 6 * RED_BLOCKS, p->gamma_bar, keys, lists);
+        morton_keys<<<gN, T, 0, st>>>(N, in->x, in->y, in->z, p->hdr, keys, lists);
         FMM_LAUNCH_CHECK(c, "morton_keys");
         FMM_TRY(sort_pairs_u64(c, keys, lists, tkeys, tvals, N, 0, 64));
         order = lists;
         permute_particles<<<gN, T, 0, st>>>(N, order, in->x, in->y, in->z, in->px, in->py, in->pz, in->q, in->q_scalar,
                                             p->perm, p->tx, p->ty, p->tz, p->w0, p->w1, p->w2, p->w3, p->pmx, p->pmy, p->pmz);
         FMM_LAUNCH_CHECK(c, "permute_particles");
-        ctx_free(c, mm);
     }
     ctx_free(c, keys); ctx_free(c, tkeys); ctx_free(c, tvals); ctx_free(c, lists);
 
@@ -540,7 +613,7 @@ int tree_boxes(fmm_plan *p)
     const int T = 256;
     leaf_bbox<<<(unsigned)((p->leaves * 32 + T - 1) / T), T, 0, c->stream>>>((int)p->leaves, p->node_lo, p->node_hi, p->tx, p->ty, p->tz, p->bbox);
     FMM_LAUNCH_CHECK(c, "leaf_bbox");
-    upper_bbox_and_geometry<<<1, 1024, 0, c->stream>>>(p->kappa, (int)p->nodes, p->node_lo, p->node_hi, p->gamma_bar, p->bbox, p->node_geo);
+    upper_bbox_and_geometry<<<1, 1024, 0, c->stream>>>(p->kappa, (int)p->nodes, p->node_lo, p->node_hi, p->hdr, p->bbox, p->node_geo);
     FMM_LAUNCH_CHECK(c, "upper_bbox_and_geometry");
     return FMM_OK;
 }

@@ -220,6 +220,38 @@ def test_bad_arguments(fmm):
         fmm.fmm_plan_create(w.x, w.y, w.z, w.px, w.py, bad, w.q, order_n=2, leaf_size=8, theta=0.5)
 
 
+def test_non_finite_inputs_are_refused(fmm):
+    """FMM_ENONFINITE (include/fmm.h): one fused scan in step a0 finds NaN / Inf in x, y, z, px, py, pz or q, also when
+    gamma_bar is given; a plan whose update failed refuses fmm_eval until an update succeeds."""
+    w = workloads.config(1, N=5000)
+    base = dict(order_n=2, leaf_size=40, theta=0.5)
+    names = ["x", "y", "z", "px", "py", "pz"]
+    for k, name in enumerate(names):
+        for val in (np.nan, np.inf, -np.inf):
+            arrs = [a.copy() for a in w.arrays()]
+            arrs[k][(17 * k + 3) % w.N] = val
+            for gb in (0.0, 10.0):
+                with pytest.raises(fmm.FmmError, match="-4"):
+                    fmm.fmm_plan_create(*arrs, w.q, gamma_bar=gb, **base)
+    q = np.full(w.N, workloads.ELECTRON_CHARGE)
+    q[-1] = np.nan
+    with pytest.raises(fmm.FmmError, match="-4"):
+        fmm.fmm_plan_create(*w.arrays(), q, **base)
+    # a failed update invalidates the plan, a good one revives it
+    plan = fmm.fmm_plan_create(*w.arrays(), w.q, **base)
+    E0, B0 = to_np(plan.eval())
+    arrs = [a.copy() for a in w.arrays()]
+    arrs[0][5] = np.inf
+    with pytest.raises(fmm.FmmError, match="-4"):
+        plan.update(*arrs, w.q)
+    with pytest.raises(fmm.FmmError, match="-1"):
+        plan.eval()
+    plan.update(*w.arrays(), w.q)
+    E1, B1 = to_np(plan.eval())
+    assert np.array_equal(E0, E1) and np.array_equal(B0, B1)
+    plan.close()
+
+
 # ---------------------------------------------------------------------------------------------
 # FMM_KERNEL_SOURCE_MOMENTUM: near field stretched along each source's own momentum (DESIGN.md G6 alternative,
 # SURVEY.md 8(f) rank 2).  Same bars as the default kernel.
