@@ -29,9 +29,11 @@
  *              call of a plan under the stream the plan was created on).  A plan frees its
  *              remaining workspace in fmm_plan_destroy.
  *   Stream     all work is enqueued on `cuda_stream` (a cudaStream_t passed as void*; NULL =
- *              the legacy default stream).  fmm_plan_create / fmm_plan_update synchronise the
- *              stream internally (the interaction-list lengths must be read back to size the
- *              lists); fmm_eval and fmm_direct only enqueue and return.
+ *              the legacy default stream).  fmm_plan_create / fmm_plan_update / fmm_plan_refit
+ *              wait for the stream ONCE, after the traversal (the interaction-list lengths
+ *              must be read back to size the lists; gamma_bar and the input check come with
+ *              them), and return with the rest of the build enqueued; the inputs are no
+ *              longer read after that wait.  fmm_eval and fmm_direct only enqueue and return.
  *   Errors     0 on success, a negative FMM_E* code otherwise; no exceptions, no exit().
  *              Outputs are unspecified after an error.  A plan whose fmm_plan_update /
  *              fmm_plan_refit failed is marked invalid: fmm_eval returns FMM_EINVAL for it
@@ -147,7 +149,7 @@ typedef struct {
 } fmm_export_t;
 
 /* a0-a3: mean momentum -> gamma_bar, tree order, bounding boxes, dual tree traversal, CSR lists.
- * Synchronises the stream.  *out is NULL on error. */
+ * Waits for the stream once (see "Stream" above).  *out is NULL on error. */
 int fmm_plan_create(fmm_plan_t **out, const fmm_particles_t *particles, const fmm_params_t *params,
                     fmm_alloc_fn alloc, fmm_free_fn free_, void *user, void *cuda_stream);
 
@@ -160,7 +162,7 @@ int fmm_plan_update(fmm_plan_t *plan, const fmm_particles_t *particles);
  * (no sort): the new positions / momenta / charges are gathered through it, gamma_bar, the tight bounding boxes and both
  * interaction lists are rebuilt on the new boxes.  Any partition into contiguous ranges is a valid cluster tree for
  * Alg 5.11 and the admissibility condition is evaluated on the actual boxes, so the result is a correct FMM of the same
- * order of accuracy; it is no longer the median split of the NEW positions.  Synchronises the stream. */
+ * order of accuracy; it is no longer the median split of the NEW positions.  Waits for the stream once. */
 int fmm_plan_refit(fmm_plan_t *plan, const fmm_particles_t *particles);
 
 /* a4-a10: P2M, M2M, M2L, P2P, L2L, L2P, prefactors, scatter to caller order.  Enqueue only.

@@ -20,6 +20,9 @@ static void ctx_init(fmm_ctx *c, fmm_alloc_fn alloc, fmm_free_fn free_, void *us
     c->stream = (cudaStream_t)stream;
     c->err[0] = 0;
     c->bytes = 0;
+    c->arena = NULL;
+    c->arena_cap = c->arena_top = c->arena_need = 0;
+    c->arena_on = 0;
 }
 
 static void ctx_set_error(fmm_ctx *c, const char *msg)
@@ -37,6 +40,42 @@ int ctx_cuda_fail(fmm_ctx *c, cudaError_t e, const char *what)
 }
 
 void *ctx_alloc(fmm_ctx *c, size_t bytes)
+{
+    if (c->arena_on) {
+        const size_t need = ((bytes ? bytes : 8) + 255) & ~(size_t)255;
+        c->arena_need += need;
+        if (c->arena_top + need <= c->arena_cap) {
+            void *p = c->arena + c->arena_top;
+            c->arena_marks.push_back(c->arena_top);
+            c->arena_live.push_back(1);
+            c->arena_top += need;
+            return p;
+        }
+    }
+    return ctx_alloc_keep(c, bytes);
+}
+
+int ctx_arena_begin(fmm_ctx *c, size_t estimate)
+{
+    size_t want = estimate > c->arena_need + c->arena_need / 8 ? estimate : c->arena_need + c->arena_need / 8;  // what the last build asked for
+    if (want > c->arena_cap) {
+        if (c->arena) ctx_free_keep(c, c->arena);
+        c->arena = NULL;
+        c->arena_cap = 0;
+        c->arena = (char *)ctx_alloc_keep(c, want);
+        if (!c->arena) return FMM_ENOMEM;
+        c->arena_cap = want;
+    }
+    c->arena_top = c->arena_need = 0;
+    c->arena_marks.clear();
+    c->arena_live.clear();
+    c->arena_on = 1;
+    return FMM_OK;
+}
+
+void ctx_arena_end(fmm_ctx *c) { c->arena_on = 0; }
+
+void *ctx_alloc_keep(fmm_ctx *c, size_t bytes)
 {
     if (bytes == 0) bytes = 8;
     void *p = NULL;
@@ -60,6 +99,24 @@ void *ctx_alloc(fmm_ctx *c, size_t bytes)
 void ctx_free(fmm_ctx *c, void *p)
 {
     if (!p) return;
+    if (c->arena && (char *)p >= c->arena && (char *)p < c->arena + c->arena_cap) {
+        // arena block: its space comes back once it is the newest live block (together with everything freed below it)
+        const size_t at = (size_t)((char *)p - c->arena);
+        for (size_t k = c->arena_marks.size(); k-- > 0;)
+            if (c->arena_marks[k] == at) { c->arena_live[k] = 0; break; }
+        while (!c->arena_marks.empty() && !c->arena_live.back()) {
+            c->arena_top = c->arena_marks.back();
+            c->arena_marks.pop_back();
+            c->arena_live.pop_back();
+        }
+        return;
+    }
+    ctx_free_keep(c, p);
+}
+
+void ctx_free_keep(fmm_ctx *c, void *p)
+{
+    if (!p) return;
     for (size_t k = c->owned.size(); k-- > 0;) {
         if (c->owned[k] == p) {
             c->bytes -= (int64_t)c->owned_bytes[k];
@@ -74,7 +131,9 @@ void ctx_free(fmm_ctx *c, void *p)
 
 void ctx_free_all(fmm_ctx *c)
 {
-    while (!c->owned.empty()) ctx_free(c, c->owned.back());
+    while (!c->owned.empty()) ctx_free_keep(c, c->owned.back());
+    c->arena = NULL;
+    c->arena_cap = 0;
 }
 
 // One side stream per device for the near / far overlap, created on first use and kept for the life of the process
@@ -156,17 +215,21 @@ static int plan_build(fmm_plan *p, const fmm_particles_t *in, bool refit = false
 {
     fmm_ctx *c = &p->ctx;
     p->valid = 0;  // a build that fails part-way leaves lists that must not be used (fmm_eval then returns FMM_EINVAL)
+    // scratch of the whole build from one arena block: sort keys and index lists of the tree (about 100 N bytes), frontier
+    // and pair buffers of the traversal; sized from the last build once there was one
+    const size_t estimate = (size_t)120 * (size_t)p->N + (size_t)64 * (size_t)(p->list_cap > 0 ? p->list_cap : p->leaves * 128) +
+                            (size_t)64 * (size_t)p->nodes + ((size_t)4 << 20);
+    FMM_TRY(ctx_arena_begin(c, estimate));
+    struct arena_guard { fmm_ctx *c; ~arena_guard() { ctx_arena_end(c); } } guard{c};
     FMM_CUDA(c, cudaEventRecord(p->ev_plan[0], c->stream));
     FMM_TRY(tree_scan_inputs(p, in));  // a0: gamma_bar, coordinate ranges, input check -> p->hdr (device)
     FMM_TRY(refit ? tree_refit(p, in) : tree_build(p, in));
     FMM_CUDA(c, cudaEventRecord(p->ev_plan[1], c->stream));
     FMM_TRY(dtt_build_lists(p));       // (reads gamma_bar and the input check back together with the list lengths)
+    FMM_CUDA(c, cudaEventRecord(p->ev_plan[2], c->stream));
     FMM_TRY(pairs_p2p_prepare(p));
     FMM_TRY(pairs_m2l_prepare(p));
-    FMM_CUDA(c, cudaEventRecord(p->ev_plan[2], c->stream));
-    FMM_CUDA(c, cudaStreamSynchronize(c->stream));
-    FMM_CUDA(c, cudaEventElapsedTime(&p->ms_tree, p->ev_plan[0], p->ev_plan[1]));
-    FMM_CUDA(c, cudaEventElapsedTime(&p->ms_lists, p->ev_plan[1], p->ev_plan[2]));
+    p->plan_ms_pending = 1;  // (read in fmm_plan_stats: the tail of the build is enqueue-only)
     p->ev_valid = 0;
     p->valid = 1;
     return FMM_OK;
@@ -346,6 +409,13 @@ extern "C" int fmm_plan_stats(fmm_plan_t *p, fmm_stats_t *s)
     s->gamma_bar = p->gamma_bar;
     s->theta = p->theta;
     s->flags = p->flags;
+    if (p->plan_ms_pending) {
+        fmm_ctx *c = &p->ctx;
+        FMM_CUDA(c, cudaEventSynchronize(p->ev_plan[2]));
+        FMM_CUDA(c, cudaEventElapsedTime(&p->ms_tree, p->ev_plan[0], p->ev_plan[1]));
+        FMM_CUDA(c, cudaEventElapsedTime(&p->ms_lists, p->ev_plan[1], p->ev_plan[2]));
+        p->plan_ms_pending = 0;
+    }
     s->ms_tree = p->ms_tree;
     s->ms_lists = p->ms_lists;
     s->workspace_bytes = p->ctx.bytes;

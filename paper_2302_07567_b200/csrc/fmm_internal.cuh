@@ -27,10 +27,22 @@ struct fmm_ctx {  // allocator + stream + error text, shared by plans and plan-l
     int64_t bytes;
     std::vector<void *> owned;
     std::vector<size_t> owned_bytes;
+    // Scratch arena of a plan: one block from the caller's allocator that serves every temporary of a build (bump
+    // pointer, reset per build), so that a build costs no allocator calls in steady state (each call through the Python
+    // binding is a callback into torch, ~10 us of host time with the GPU idle).  Stream-ordered like everything else.
+    char *arena;
+    size_t arena_cap, arena_top, arena_need;
+    int arena_on;
+    std::vector<size_t> arena_marks;  // start offsets of the arena blocks handed out, for last-in-first-out reuse
+    std::vector<char> arena_live;
 };
 
-void *ctx_alloc(fmm_ctx *c, size_t bytes);  // NULL on failure (err set)
+void *ctx_alloc(fmm_ctx *c, size_t bytes);       // NULL on failure (err set); from the arena while a build is running
+void *ctx_alloc_keep(fmm_ctx *c, size_t bytes);  // always from the caller's allocator (buffers that outlive the build)
 void ctx_free(fmm_ctx *c, void *p);
+void ctx_free_keep(fmm_ctx *c, void *p);
+int ctx_arena_begin(fmm_ctx *c, size_t estimate);
+void ctx_arena_end(fmm_ctx *c);
 void ctx_free_all(fmm_ctx *c);
 int ctx_cuda_fail(fmm_ctx *c, cudaError_t e, const char *what);
 #define FMM_CUDA(c, call)                                                  \
@@ -87,14 +99,15 @@ struct fmm_plan {
     // reaction on the source leaf to partial segment dst; dst = -1: one-sided; dst = -2: the mate's block does the work and
     // recv >= 0 is the segment holding the sums for this entry's target particles.  NULL with FMM_KERNEL_SOURCE_MOMENTUM.
     int32_t *p2p_dst, *p2p_recv;
-    int64_t p2p_react;      // particles in all reaction segments
+    int p2p_mutual;         // the lists of the last build carry pair ownership (dst / recv) that the near-field kernel may use
+    int64_t list_cap;       // entries allocated for p2p_src, m2l_src, p2p_dst, p2p_recv
+    int64_t p2p_react;      // upper bound of the particles in all reaction segments
     double *react;          // [6][p2p_react] reaction sums (E, B components as planes), rewritten by every fmm_eval
     int64_t react_cap;
     int react_used;         // the last pairs_p2p ran the mutual kernel (L2P then subtracts the reaction segments)
     int64_t n_p2p, n_m2l, cap_p2p, cap_m2l;
     int64_t p2p_pairs, m2l_pairs;
-    int64_t p2p_work;       // block work of the whole P2P list in one-sided pair units (an owned mutual pair counts 34/25, a pair the mate owns 0)
-    int64_t p2p_max_row;    // heaviest target leaf row, same units
+    int64_t p2p_max_row;    // particle pairs of the heaviest target leaf row
     int p2p_split;          // P2P row split K: block (t, k) sums chunk k of t's row into near_[k]; L2P adds the K partials in order
     int64_t near_cap;       // doubles allocated for near_
     int m2l_split;          // M2L row split (small trees): chunk kc > 0 of a row goes to Lpart[kc-1], combined into L in order
@@ -115,6 +128,7 @@ struct fmm_plan {
     cudaEvent_t ev_fork, ev_join;
     int overlap;
     int ev_valid;
+    int plan_ms_pending;    // ms_tree / ms_lists of the last build have not been read from ev_plan yet
     float ms_tree, ms_lists;
 };
 

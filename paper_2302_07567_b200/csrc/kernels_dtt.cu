@@ -1,99 +1,283 @@
 // kernels_dtt.cu -- step a3: dual tree traversal (Alg 9.1; same logic as Alg 5.11,
 // PAPER.md:400-435) with the stretched admissibility condition of Alg 5.6-5.8 (PAPER.md:337-366,
-// eq. (4.3)), emitting the two interaction lists, then sorting them by
-// (target, source) into CSR form (readings D-4, G20).
+// eq. (4.3)), emitting the two interaction lists in CSR form sorted by
+// (target, source) (readings D-4, G20).
 //
-// The recursion is run level-synchronously: a frontier of (target, source) node pairs is
-// classified by one kernel per step (P2P / M2L / split), children are appended to the next frontier
-// through INTEGER atomic counters (order inside a frontier is irrelevant: the lists are sorted
-// afterwards, so the result is unique and bit-reproducible).  No host round trip until the final
-// list lengths are read back.
+// The recursion runs in two kernels: one block expands the pair (root, root) breadth-first (classify every pair of
+// the frontier as P2P / M2L / split, block barrier, next frontier) until the frontier holds a few thousand pairs;
+// then every such pair is walked depth-first by one warp with a stack in shared memory.  Pairs are emitted through INTEGER
+// atomic counters and count into their target's row length.  The order of emission is irrelevant: rows are laid out
+// from the scanned row lengths and then sorted by source, so the lists are unique and bit-reproducible.  One host
+// wait per build, at its very end (list lengths, gamma_bar, the input check).
 #include "fmm_internal.cuh"
+
+#include <cooperative_groups.h>
+namespace cg = cooperative_groups;
 
 struct dtt_counters {           // device
     unsigned int n_p2p, n_m2l, overflow, pad;
     unsigned int n_front[72];   // frontier sizes per step (at most 2*kappa+2 steps)
+    unsigned long long evals;   // particle pairs of the whole P2P list
+    unsigned long long max_row; // particle pairs of the heaviest target leaf
 };
 
-__global__ void dtt_init(dtt_counters *cnt, uint64_t *front0, int treecode_leaves)
+struct dtt_args {
+    int nsteps, leaves, key_shift, treecode_leaves;
+    double theta2;
+    const fmm_hdr *hdr;
+    const int32_t *node_lo, *node_hi;
+    const double *geo;
+    uint64_t *front0, *front1, *p2p, *m2l;
+    unsigned int cap;
+    int32_t *rows;              // [2][rows_len] row lengths: P2P by target leaf id, then M2L by target node id
+    int32_t *row_work;          // [leaves] sum of the source leaf sizes of a target leaf's row
+    int rows_len;
+    dtt_counters *cnt;
+};
+
+#define DTT_ROOTS 4096   // breadth-first until the frontier holds this many pairs, then one depth-first walk per pair
+
+// one pair of Alg 9.1: 0 = nothing (empty cluster), 1 = P2P, 2 = M2L, 3 = split the target, 4 = split the source
+__device__ __forceinline__ int dtt_decide(const dtt_args &a, double gamma_bar, int i, int j, int *nj_out)
 {
-    // FMM: the traversal starts at (root, root).  Treecode (FMM_METHOD_TREECODE): at (t, root) for every leaf t, so
-    // the target is never split and the "m2l" list becomes the particle-cluster list.
-    int k0 = blockIdx.x * blockDim.x + threadIdx.x;
-    if (k0 == 0) {
+    const int ni = a.node_hi[i] - a.node_lo[i], nj = a.node_hi[j] - a.node_lo[j];
+    *nj_out = nj;
+    if (ni <= 0 || nj <= 0) return 0;
+    const bool leaf_i = i >= a.leaves, leaf_j = j >= a.leaves;
+    if (leaf_i && leaf_j) return 1;  // D-1: leaf-leaf -> P2P, no admissibility test
+    // D-2: Alg 5.6-5.8 squared; every product and sum rounded separately, in this order
+    const double *gi = a.geo + 4 * (int64_t)i, *gj = a.geo + 4 * (int64_t)j;
+    const double ri = gi[0], rj = gj[0];
+    const double ex = __dmul_rn(1.0, __dsub_rn(gi[1], gj[1]));
+    const double ey = __dmul_rn(1.0, __dsub_rn(gi[2], gj[2]));
+    const double ez = __dmul_rn(gamma_bar, __dsub_rn(gi[3], gj[3]));
+    const double d2 = __dadd_rn(__dadd_rn(__dmul_rn(ex, ex), __dmul_rn(ey, ey)), __dmul_rn(ez, ez));
+    const double rmax = (ri > rj) ? ri : rj;
+    if (rmax < __dmul_rn(a.theta2, d2)) return 2;  // admissible -> M2L
+    // D-3: which side to split
+    return (leaf_i ? false : (leaf_j ? true : (ri > rj))) ? 3 : 4;
+}
+
+// slot in a pair buffer: one atomic per group of threads that arrive together (the counter is a single hot address)
+__device__ __forceinline__ unsigned int dtt_slot(unsigned int *counter)
+{
+    cg::coalesced_group g = cg::coalesced_threads();
+    unsigned int base = 0;
+    if (g.thread_rank() == 0) base = atomicAdd(counter, (unsigned int)g.size());
+    return g.shfl(base, 0) + g.thread_rank();
+}
+
+__device__ __forceinline__ void dtt_emit(const dtt_args &a, int kind, int i, int j, int nj)
+{
+    dtt_counters *cnt = a.cnt;
+    if (kind == 1) {
+        const unsigned int pos = dtt_slot(&cnt->n_p2p);
+        if (pos < a.cap) a.p2p[pos] = ((uint64_t)i << a.key_shift) | (uint64_t)j; else cnt->overflow = 1;
+        atomicAdd(&a.rows[i], 1);
+        atomicAdd(&a.row_work[i - a.leaves], nj);
+    } else {
+        const unsigned int pos = dtt_slot(&cnt->n_m2l);
+        if (pos < a.cap) a.m2l[pos] = ((uint64_t)i << a.key_shift) | (uint64_t)j; else cnt->overflow = 1;
+        atomicAdd(&a.rows[a.rows_len + i], 1);
+    }
+}
+
+// Top of the traversal by ONE block (block barriers between the steps): resets the counters and the row lengths, seeds the
+// frontier -- FMM: (root, root); treecode (FMM_METHOD_TREECODE): (t, root) for every leaf t, so the target is never split
+// and the "m2l" list becomes the particle-cluster list -- and expands it breadth-first until it holds DTT_ROOTS pairs.
+__global__ void __launch_bounds__(1024) dtt_top(dtt_args a)
+{
+    __shared__ unsigned int n_in, n_out;
+    dtt_counters *cnt = a.cnt;
+    const int tid = threadIdx.x, nth = blockDim.x;
+    if (tid == 0) {
         cnt->n_p2p = cnt->n_m2l = cnt->overflow = cnt->pad = 0;
-        for (int k = 0; k < 72; ++k) cnt->n_front[k] = 0;
-        cnt->n_front[0] = treecode_leaves > 0 ? (unsigned)treecode_leaves : 1u;
-        if (treecode_leaves <= 0) front0[0] = (1ull << 32) | 1ull;  // (root, root)
+        cnt->evals = cnt->max_row = 0ull;
+        n_in = a.treecode_leaves > 0 ? (unsigned)a.treecode_leaves : 1u;
+        if (a.treecode_leaves <= 0) a.front0[0] = (1ull << 32) | 1ull;
+        n_out = 0;
     }
-    if (k0 < treecode_leaves) front0[k0] = ((uint64_t)(treecode_leaves + k0) << 32) | 1ull;  // (leaf, root)
-}
-
-__global__ void __launch_bounds__(256) dtt_step(int step, int leaves, const fmm_hdr *__restrict__ hdr, double theta2,
-                                                const int32_t *__restrict__ node_lo, const int32_t *__restrict__ node_hi,
-                                                const double *__restrict__ geo, const uint64_t *__restrict__ front_in,
-                                                uint64_t *__restrict__ front_out, unsigned int cap_front,
-                                                uint64_t *__restrict__ p2p, unsigned int cap_p2p,
-                                                uint64_t *__restrict__ m2l, unsigned int cap_m2l,
-                                                int key_shift, dtt_counters *cnt)
-{
-    if (hdr->nonfinite) return;  // NaN / Inf in the inputs: no lists (FMM_ENONFINITE after the read-back)
-    const double gamma_bar = hdr->gamma_bar;
-    unsigned int nin = cnt->n_front[step];
-    if (nin > cap_front) nin = cap_front;
-    for (unsigned int k = blockIdx.x * blockDim.x + threadIdx.x; k < nin; k += gridDim.x * blockDim.x) {
-        uint64_t pr = front_in[k];
-        int i = (int)(pr >> 32), j = (int)(pr & 0xffffffffu);  // i = target, j = source
-        if (node_hi[i] <= node_lo[i] || node_hi[j] <= node_lo[j]) continue;  // empty cluster
-        bool leaf_i = i >= leaves, leaf_j = j >= leaves;
-        if (leaf_i && leaf_j) {  // D-1: leaf-leaf -> P2P, no admissibility test
-            unsigned int pos = atomicAdd(&cnt->n_p2p, 1u);
-            if (pos < cap_p2p) p2p[pos] = ((uint64_t)i << key_shift) | (uint64_t)j; else cnt->overflow = 1;
-            continue;
-        }
-        // D-2: Alg 5.6-5.8 squared; every product and sum rounded separately, in this order
-        const double *gi = geo + 4 * (int64_t)i, *gj = geo + 4 * (int64_t)j;
-        double ri = gi[0], rj = gj[0];
-        double ex = __dmul_rn(1.0, __dsub_rn(gi[1], gj[1]));
-        double ey = __dmul_rn(1.0, __dsub_rn(gi[2], gj[2]));
-        double ez = __dmul_rn(gamma_bar, __dsub_rn(gi[3], gj[3]));
-        double d2 = __dadd_rn(__dadd_rn(__dmul_rn(ex, ex), __dmul_rn(ey, ey)), __dmul_rn(ez, ez));
-        double rmax = (ri > rj) ? ri : rj;
-        if (rmax < __dmul_rn(theta2, d2)) {  // admissible -> M2L
-            unsigned int pos = atomicAdd(&cnt->n_m2l, 1u);
-            if (pos < cap_m2l) m2l[pos] = ((uint64_t)i << key_shift) | (uint64_t)j; else cnt->overflow = 1;
-            continue;
-        }
-        // D-3: which side to split
-        bool split_target = leaf_i ? false : (leaf_j ? true : (ri > rj));
-        unsigned int pos = atomicAdd(&cnt->n_front[step + 1], 2u);
-        if (pos + 1 < cap_front) {
-            if (split_target) {
-                front_out[pos] = ((uint64_t)(2 * i) << 32) | (uint64_t)j;
-                front_out[pos + 1] = ((uint64_t)(2 * i + 1) << 32) | (uint64_t)j;
-            } else {
-                front_out[pos] = ((uint64_t)i << 32) | (uint64_t)(2 * j);
-                front_out[pos + 1] = ((uint64_t)i << 32) | (uint64_t)(2 * j + 1);
+    for (int k = tid; k < 72; k += nth) cnt->n_front[k] = 0;
+    for (int k = tid; k < a.treecode_leaves; k += nth) a.front0[k] = ((uint64_t)(a.treecode_leaves + k) << 32) | 1ull;
+    for (int k = tid; k < 2 * a.rows_len; k += nth) a.rows[k] = 0;
+    for (int k = tid; k < a.leaves; k += nth) a.row_work[k] = 0;
+    __threadfence();
+    __syncthreads();
+    int step = 0;
+    if (!a.hdr->nonfinite) {  // NaN / Inf in the inputs: no lists (FMM_ENONFINITE after the read-back)
+        const double gamma_bar = a.hdr->gamma_bar;
+        for (; step < a.nsteps; ++step) {
+            const unsigned int nin = n_in;
+            if (nin == 0 || nin >= DTT_ROOTS || nin > a.cap) break;
+            const uint64_t *front_in = (step & 1) ? a.front1 : a.front0;
+            uint64_t *front_out = (step & 1) ? a.front0 : a.front1;
+            for (unsigned int k = tid; k < nin; k += nth) {
+                const uint64_t pr = front_in[k];
+                const int i = (int)(pr >> 32), j = (int)(pr & 0xffffffffu);  // i = target, j = source
+                int nj;
+                const int kind = dtt_decide(a, gamma_bar, i, j, &nj);
+                if (kind == 1 || kind == 2) dtt_emit(a, kind, i, j, nj);
+                if (kind >= 3) {
+                    const unsigned int pos = atomicAdd(&n_out, 2u);
+                    if (pos + 1 < a.cap) {
+                        front_out[pos] = (kind == 3) ? (((uint64_t)(2 * i) << 32) | (uint64_t)j) : (((uint64_t)i << 32) | (uint64_t)(2 * j));
+                        front_out[pos + 1] = (kind == 3) ? (((uint64_t)(2 * i + 1) << 32) | (uint64_t)j) : (((uint64_t)i << 32) | (uint64_t)(2 * j + 1));
+                    } else {
+                        cnt->overflow = 1;
+                    }
+                }
             }
-        } else {
-            cnt->overflow = 1;
+            __syncthreads();
+            if (tid == 0) { n_in = n_out; n_out = 0; }
+            __syncthreads();
+        }
+    }
+    if (tid == 0) {  // what is left for the walks: n_front[0] pairs in buffer (n_front[1] & 1)
+        cnt->n_front[0] = a.hdr->nonfinite ? 0u : (n_in > a.cap ? a.cap : n_in);
+        cnt->n_front[1] = (unsigned)step;
+    }
+}
+
+// Rest of the traversal: every pair the top left over is the root of a walk by one WARP.  The warp keeps a stack of pairs
+// in shared memory, takes up to 32 pairs off its top per round (one per lane), classifies them and pushes the children of
+// the pairs that split: depth-first in blocks of 32, so the stack stays short while all lanes have work.  A stack that
+// would overflow hands the children to a global buffer instead, which a second launch walks the same way.
+#define DTT_WALK_WARPS 4
+#define DTT_WSTACK 512
+__global__ void __launch_bounds__(32 * DTT_WALK_WARPS) dtt_walk(dtt_args a, int pass)
+{
+    __shared__ uint64_t stk_all[DTT_WALK_WARPS][DTT_WSTACK];
+    dtt_counters *cnt = a.cnt;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    uint64_t *stk = stk_all[warp];
+    // pass 0: roots left by dtt_top in buffer (n_front[1] & 1), spill into the other buffer counted by n_front[2];
+    // pass 1: walks that spill; anything it would spill again is reported as an overflow (larger buffers, new traversal)
+    const int rb = (int)(cnt->n_front[1] & 1) ^ pass;
+    const unsigned int nroots = pass == 0 ? cnt->n_front[0] : (cnt->n_front[2] > a.cap ? a.cap : cnt->n_front[2]);
+    const uint64_t *roots = rb ? a.front1 : a.front0;
+    uint64_t *spill = rb ? a.front0 : a.front1;
+    if (nroots == 0) return;
+    const double gamma_bar = a.hdr->gamma_bar;
+    const unsigned int lt = (1u << lane) - 1u;
+    for (unsigned int r = blockIdx.x * DTT_WALK_WARPS + warp; r < nroots; r += gridDim.x * DTT_WALK_WARPS) {
+        int top = 1;
+        if (lane == 0) stk[0] = roots[r];
+        __syncwarp();
+        while (top > 0) {
+            const int take = top < 32 ? top : 32;
+            top -= take;
+            const uint64_t pr = lane < take ? stk[top + lane] : 0ull;
+            __syncwarp();
+            const int i = (int)(pr >> 32), j = (int)(pr & 0xffffffffu);  // i = target, j = source
+            int kind = 0, nj = 0;
+            if (lane < take) kind = dtt_decide(a, gamma_bar, i, j, &nj);
+            if (kind == 1 || kind == 2) dtt_emit(a, kind, i, j, nj);
+            const unsigned int splits = __ballot_sync(0xffffffffu, kind >= 3);
+            const int nsplit = __popc(splits);
+            if (kind >= 3) {
+                const uint64_t c0 = (kind == 3) ? (((uint64_t)(2 * i) << 32) | (uint64_t)j) : (((uint64_t)i << 32) | (uint64_t)(2 * j));
+                const uint64_t c1 = (kind == 3) ? (((uint64_t)(2 * i + 1) << 32) | (uint64_t)j) : (((uint64_t)i << 32) | (uint64_t)(2 * j + 1));
+                if (top + 2 * nsplit <= DTT_WSTACK) {
+                    const int at = top + 2 * __popc(splits & lt);
+                    stk[at] = c0;
+                    stk[at + 1] = c1;
+                } else {  // (warp-uniform condition)
+                    const unsigned int pos = atomicAdd(&cnt->n_front[2 + pass], 2u);
+                    if (pass == 0 && pos + 1 < a.cap) { spill[pos] = c0; spill[pos + 1] = c1; }
+                    else cnt->overflow = 1;
+                }
+            }
+            if (top + 2 * nsplit <= DTT_WSTACK) top += 2 * nsplit;
+            __syncwarp();
         }
     }
 }
 
-// sorted keys (target << shift | source) -> CSR: off[t] = first position with target >= t
-__global__ void csr_from_sorted(const uint64_t *__restrict__ keys, int64_t n, int key_shift, int nodes,
-                                int32_t *__restrict__ off /* [nodes+2] */, int32_t *__restrict__ src, int32_t *__restrict__ tgt /* or NULL */)
+// particle pairs of the P2P list and of its heaviest row (the near-field kernels choose their row split from these)
+__global__ void __launch_bounds__(256) dtt_totals(dtt_args a)
 {
-    int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (k > n) return;
-    uint64_t mask = (1ull << key_shift) - 1ull;
-    int t_prev = (k == 0) ? -1 : (int)(keys[k - 1] >> key_shift);
-    int t_cur = (k == n) ? nodes + 1 : (int)(keys[k] >> key_shift);
-    for (int t = t_prev + 1; t <= t_cur; ++t) off[t] = (int32_t)k;
-    if (k < n) {
-        src[k] = (int32_t)(keys[k] & mask);
-        if (tgt) tgt[k] = t_cur;
+    const int gtid = blockIdx.x * blockDim.x + threadIdx.x, gsize = gridDim.x * blockDim.x;
+    unsigned long long sum = 0, mx = 0;
+    for (int k = gtid; k < a.leaves; k += gsize) {
+        const int t = a.leaves + k;
+        const unsigned long long w = (unsigned long long)(a.node_hi[t] - a.node_lo[t]) * (unsigned long long)a.row_work[k];
+        sum += w;
+        mx = w > mx ? w : mx;
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        sum += __shfl_down_sync(0xffffffffu, sum, o);
+        const unsigned long long m2 = __shfl_down_sync(0xffffffffu, mx, o);
+        mx = m2 > mx ? m2 : mx;
+    }
+    if ((threadIdx.x & 31) == 0 && sum) {
+        atomicAdd(&a.cnt->evals, sum);
+        atomicMax(&a.cnt->max_row, mx);
+    }
+}
+
+// rows of both lists from the scanned row lengths: offsets, then every emitted pair takes a slot of its target's row
+__global__ void csr_offsets(int rows_len, const int32_t *__restrict__ scan /* [2 rows_len] */, int32_t *__restrict__ p2p_off,
+                            int32_t *__restrict__ m2l_off)
+{
+    int k = blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= rows_len) return;
+    p2p_off[k] = scan[k];
+    m2l_off[k] = scan[rows_len + k] - scan[rows_len];
+}
+
+__global__ void csr_fill(const dtt_counters *__restrict__ cnt, const uint64_t *__restrict__ kp2p, const uint64_t *__restrict__ km2l, int key_shift,
+                         int rows_len, const int32_t *__restrict__ p2p_off, const int32_t *__restrict__ m2l_off,
+                         int32_t *__restrict__ rows /* remaining slots per row, counted down */, int32_t *__restrict__ p2p_tmp,
+                         int32_t *__restrict__ m2l_tmp)
+{
+    if (cnt->overflow) return;  // (the host enlarges the buffers and runs the traversal again)
+    const int64_t n_p2p = cnt->n_p2p, n_all = n_p2p + (int64_t)cnt->n_m2l;
+    const uint64_t mask = (1ull << key_shift) - 1ull;
+    for (int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; k < n_all; k += (int64_t)gridDim.x * blockDim.x) {
+        if (k < n_p2p) {
+            const uint64_t key = kp2p[k];
+            const int t = (int)(key >> key_shift);
+            const int slot = atomicSub(&rows[t], 1) - 1;
+            p2p_tmp[p2p_off[t] + slot] = (int32_t)(key & mask);
+        } else {
+            const uint64_t key = km2l[k - n_p2p];
+            const int t = (int)(key >> key_shift);
+            const int slot = atomicSub(&rows[rows_len + t], 1) - 1;
+            m2l_tmp[m2l_off[t] + slot] = (int32_t)(key & mask);
+        }
+    }
+}
+
+// One block per row: ascending source ids (the sources of a row are distinct, so the rank of an entry is the number of
+// smaller ones).  Rows are short (tens of entries with the KD tree, at most a few thousand with MORTON_MEDIAN).
+#define ROWSORT_THREADS 64
+__global__ void __launch_bounds__(ROWSORT_THREADS) csr_sort_rows(const dtt_counters *__restrict__ cnt, int first_p2p, int n_rows_p2p, int first_m2l, const int32_t *__restrict__ p2p_off,
+                                                                 const int32_t *__restrict__ m2l_off, const int32_t *__restrict__ p2p_tmp,
+                                                                 const int32_t *__restrict__ m2l_tmp, int32_t *__restrict__ p2p_src,
+                                                                 int32_t *__restrict__ m2l_src, int32_t *__restrict__ p2p_tgt)
+{
+    __shared__ int32_t sm[1024];
+    if (cnt->overflow) return;
+    const bool is_p2p = (int)blockIdx.x < n_rows_p2p;
+    const int t = is_p2p ? first_p2p + blockIdx.x : first_m2l + (blockIdx.x - n_rows_p2p);
+    const int32_t *off = is_p2p ? p2p_off : m2l_off;
+    const int a = off[t], m = off[t + 1] - a;
+    if (m <= 0) return;
+    const int32_t *in = (is_p2p ? p2p_tmp : m2l_tmp) + a;
+    int32_t *out = (is_p2p ? p2p_src : m2l_src) + a;
+    const bool staged = m <= 1024;
+    if (staged) {
+        for (int k = threadIdx.x; k < m; k += ROWSORT_THREADS) sm[k] = in[k];
+        __syncthreads();
+    }
+    const int32_t *row = staged ? sm : in;
+    for (int k = threadIdx.x; k < m; k += ROWSORT_THREADS) {
+        const int32_t v = row[k];
+        int rank = 0;
+        for (int q = 0; q < m; ++q) rank += row[q] < v;
+        out[rank] = v;
+        if (is_p2p && p2p_tgt) p2p_tgt[a + rank] = t;
     }
 }
 
@@ -113,74 +297,70 @@ __device__ __forceinline__ int p2p_pair_owner(int t, int s)
     return ((lo + hi) & 1) ? hi : lo;
 }
 
-__global__ void p2p_mates(int64_t n, const int32_t *__restrict__ off, const int32_t *__restrict__ src, const int32_t *__restrict__ tgt,
-                          const int32_t *__restrict__ node_lo, const int32_t *__restrict__ node_hi, int32_t *__restrict__ mate,
-                          int32_t *__restrict__ len)
+__global__ void p2p_mates(const dtt_counters *__restrict__ cnt, int64_t cap, const int32_t *__restrict__ off, const int32_t *__restrict__ src,
+                          const int32_t *__restrict__ tgt, const int32_t *__restrict__ node_lo, const int32_t *__restrict__ node_hi,
+                          int32_t *__restrict__ mate, int32_t *__restrict__ len /* [cap], zero beyond the list */)
 {
-    int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (e >= n) return;
-    const int t = tgt[e], s = src[e];
-    int m = -1;
-    if (s != t) {  // row s is sorted by source: binary search for t
-        int a = off[s], b = off[s + 1];
-        while (a < b) {
-            int mid = (a + b) >> 1;
-            int v = src[mid];
-            if (v < t) a = mid + 1; else b = mid;
+    const int64_t n = cnt->overflow ? 0 : (int64_t)cnt->n_p2p;
+    for (int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; e < cap; e += (int64_t)gridDim.x * blockDim.x) {
+        if (e >= n) { len[e] = 0; continue; }
+        const int t = tgt[e], s = src[e];
+        int m = -1;
+        if (s != t) {  // row s is sorted by source: binary search for t
+            int a = off[s], b = off[s + 1];
+            while (a < b) {
+                int mid = (a + b) >> 1;
+                int v = src[mid];
+                if (v < t) a = mid + 1; else b = mid;
+            }
+            if (a < off[s + 1] && src[a] == t) m = a;
         }
-        if (a < off[s + 1] && src[a] == t) m = a;
+        mate[e] = m;
+        len[e] = (m >= 0 && p2p_pair_owner(t, s) != t) ? (node_hi[t] - node_lo[t]) : 0;  // non-empty clusters only reach the list
     }
-    mate[e] = m;
-    len[e] = (m >= 0 && p2p_pair_owner(t, s) != t) ? (node_hi[t] - node_lo[t]) : 0;  // non-empty clusters only reach the list
 }
 
-__global__ void p2p_segments(int64_t n, const int32_t *__restrict__ src, const int32_t *__restrict__ tgt, const int32_t *__restrict__ mate,
-                             const int32_t *__restrict__ len, const int32_t *__restrict__ scan, int32_t *__restrict__ dst,
-                             int32_t *__restrict__ recv, unsigned long long *__restrict__ total /* [2] = reaction particles */)
+__global__ void p2p_segments(const dtt_counters *__restrict__ cnt, const int32_t *__restrict__ mate, const int32_t *__restrict__ len,
+                             const int32_t *__restrict__ scan, int32_t *__restrict__ dst, int32_t *__restrict__ recv)
 {
-    int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (e >= n) return;
-    const int m = mate[e];
-    recv[e] = len[e] > 0 ? scan[e] : -1;
-    dst[e] = (m < 0) ? -1 : (len[e] > 0 ? -2 : scan[m]);
-    if (e == n - 1) total[2] = (unsigned long long)scan[e] + (unsigned long long)len[e];
+    const int64_t n = cnt->overflow ? 0 : (int64_t)cnt->n_p2p;
+    for (int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; e < n; e += (int64_t)gridDim.x * blockDim.x) {
+        const int m = mate[e];
+        recv[e] = len[e] > 0 ? scan[e] : -1;
+        dst[e] = (m < 0) ? -1 : (len[e] > 0 ? -2 : scan[m]);
+    }
 }
 
-// LPT block order: targets by descending work (number of source clusters x their sizes)
-__global__ void list_work_keys(int first, int count, const int32_t *__restrict__ off, const int32_t *__restrict__ src,
+// LPT block order: targets by descending work.  The order only needs a coarse, deterministic ranking: an 8-bit monotone
+// code of the work (5-bit exponent, 3-bit mantissa), so the sort is a single radix pass.
+__global__ void list_work_keys(const dtt_counters *__restrict__ cnt, int first, int count, const int32_t *__restrict__ off, const int32_t *__restrict__ src,
                                const int32_t *__restrict__ node_lo, const int32_t *__restrict__ node_hi, int by_size,
                                const int32_t *__restrict__ dst /* P2P entry kinds, or NULL */,
-                               uint64_t *__restrict__ keys, uint32_t *__restrict__ vals, unsigned long long *__restrict__ total)
+                               uint64_t *__restrict__ keys, uint32_t *__restrict__ vals)
 {
     int k = blockIdx.x * blockDim.x + threadIdx.x;
     if (k >= count) return;
     int t = first + k;
     unsigned long long work = 0;
-    if (by_size) {
-        unsigned long long nt = (unsigned long long)(node_hi[t] - node_lo[t]), evals = 0;
-        for (int e = off[t]; e < off[t + 1]; ++e) {
-            const unsigned long long pairs = nt * (unsigned long long)(node_hi[src[e]] - node_lo[src[e]]);
-            evals += pairs;
-            // block work in FP64 instructions per particle pair: 25 one-sided, 34 for an owned mutual pair, 0 if the mate owns it
-            work += pairs * (unsigned long long)(!dst ? 25 : (dst[e] >= 0 ? 34 : (dst[e] == -1 ? 25 : 0)));
-        }
-        work /= 25;
-        atomicAdd(total, evals);      // kernel evaluations of the whole list (the algorithmic count)
-        atomicMax(total + 1, work);   // heaviest row, in one-sided pair units
-        atomicAdd(total + 3, work);
+    if (cnt->overflow) {
+        work = 0;
+    } else if (by_size) {
+        // block work in FP64 instructions per particle pair: 25 one-sided, 34 for an owned mutual pair, 0 if the mate owns it
+        for (int e = off[t]; e < off[t + 1]; ++e)
+            work += (unsigned long long)(node_hi[src[e]] - node_lo[src[e]]) * (unsigned long long)(!dst ? 25 : (dst[e] >= 0 ? 34 : (dst[e] == -1 ? 25 : 0)));
     } else {
         work = (unsigned long long)(off[t + 1] - off[t]);
     }
-    // block order only needs a coarse, deterministic ranking: a 16-bit monotone code of the work (6-bit exponent,
-    // 10-bit mantissa: 0.1 % resolution over the whole 64-bit range), so the sort takes 2 radix passes
-    unsigned long long wq = 0;
+    unsigned int wq = 0;
     if (work > 0) {
         int e = 63 - __clzll((long long)work);
-        unsigned long long mant = (e >= 10) ? (work >> (e - 10)) : (work << (10 - e));  // 1.xxxxxxxxxx
-        wq = ((unsigned long long)e << 10) | (mant & 0x3ffull);
+        if (e > 30) e = 30;
+        unsigned long long mant = (e >= 3) ? (work >> (e - 3)) : (work << (3 - e));  // 1.xxx
+        if (mant > 15) mant = 15;
+        wq = ((unsigned int)e << 3) | (unsigned int)(mant & 7ull);
         wq += 1;  // keep 0 for "no work"
     }
-    keys[k] = 0xffffull - wq;  // ascending sort of this = descending work
+    keys[k] = 0xffull - (unsigned long long)wq;  // ascending sort of this = descending work
     vals[k] = (uint32_t)t;
 }
 
@@ -190,8 +370,8 @@ __global__ void copy_u32_to_i32(int n, const uint32_t *__restrict__ a, int32_t *
     if (k < n) b[k] = (int32_t)a[k];
 }
 
-static int make_order(fmm_plan *p, int first, int count, const int32_t *off, const int32_t *src, int by_size, const int32_t *dst,
-                      int32_t *order_out, unsigned long long *total_dev)
+static int make_order(fmm_plan *p, const dtt_counters *cnt, int first, int count, const int32_t *off, const int32_t *src, int by_size,
+                      const int32_t *dst, int32_t *order_out)
 {
     fmm_ctx *c = &p->ctx;
     uint64_t *keys = (uint64_t *)ctx_alloc(c, sizeof(uint64_t) * count);
@@ -199,13 +379,22 @@ static int make_order(fmm_plan *p, int first, int count, const int32_t *off, con
     uint32_t *vals = (uint32_t *)ctx_alloc(c, sizeof(uint32_t) * count);
     uint32_t *tvals = (uint32_t *)ctx_alloc(c, sizeof(uint32_t) * count);
     if (!keys || !tkeys || !vals || !tvals) return FMM_ENOMEM;
-    list_work_keys<<<(count + 255) / 256, 256, 0, c->stream>>>(first, count, off, src, p->node_lo, p->node_hi, by_size, dst, keys, vals, total_dev);
+    list_work_keys<<<(count + 255) / 256, 256, 0, c->stream>>>(cnt, first, count, off, src, p->node_lo, p->node_hi, by_size, dst, keys, vals);
     FMM_LAUNCH_CHECK(c, "list_work_keys");
-    FMM_TRY(sort_pairs_u64(c, keys, vals, tkeys, tvals, count, 0, 16));
+    FMM_TRY(sort_pairs_u64(c, keys, vals, tkeys, tvals, count, 0, 8));
     copy_u32_to_i32<<<(count + 255) / 256, 256, 0, c->stream>>>(count, vals, order_out);
     FMM_LAUNCH_CHECK(c, "copy_u32_to_i32");
     ctx_free(c, keys); ctx_free(c, tkeys); ctx_free(c, vals); ctx_free(c, tvals);
     return FMM_OK;
+}
+
+// (re)size one of the plan's list buffers; they keep their capacity from build to build
+static int ensure_list(fmm_ctx *c, int32_t **buf, int64_t have, int64_t want)
+{
+    if (*buf && have >= want) return FMM_OK;
+    if (*buf) ctx_free(c, *buf);
+    *buf = (int32_t *)ctx_alloc_keep(c, sizeof(int32_t) * (size_t)want);
+    return *buf ? FMM_OK : FMM_ENOMEM;
 }
 
 int dtt_build_lists(fmm_plan *p)
@@ -214,103 +403,107 @@ int dtt_build_lists(fmm_plan *p)
     cudaStream_t st = c->stream;
     const int key_shift = p->kappa + 2;  // node ids < 2^(kappa+1)
     const int nsteps = 2 * p->kappa + 1;
-    dtt_counters *cnt = (dtt_counters *)ctx_alloc(c, sizeof(dtt_counters) + 4 * sizeof(unsigned long long));
-    if (!cnt) return FMM_ENOMEM;
-    unsigned long long *total_dev = (unsigned long long *)(cnt + 1);
+    const int rows_len = (int)p->nodes + 2;
+    const int64_t maxleaf = (p->N + p->leaves - 1) / p->leaves;
+    // the mean-gamma kernel is antisymmetric in the pair, the source-momentum kernel (D depends on p_j) is not
+    const bool mutual = !(p->flags & FMM_KERNEL_SOURCE_MOMENTUM) && maxleaf <= 1024;
     dtt_counters h;
-    int64_t cap = p->leaves * 128;  // first guess; doubled until nothing overflows
+    fmm_hdr hh;
+    int64_t cap = p->leaves * 128;  // first guess; enlarged until nothing overflows, and kept by the plan
     if (cap < 4096) cap = 4096;
-    uint64_t *f0 = NULL, *f1 = NULL, *kp2p = NULL, *km2l = NULL;
+    if (cap < p->list_cap) cap = p->list_cap;
     for (int attempt = 0;; ++attempt) {
         if (cap >= ((int64_t)1 << 31)) return FMM_EOVERFLOW;
-        f0 = (uint64_t *)ctx_alloc(c, sizeof(uint64_t) * cap);
-        f1 = (uint64_t *)ctx_alloc(c, sizeof(uint64_t) * cap);
-        kp2p = (uint64_t *)ctx_alloc(c, sizeof(uint64_t) * cap);
-        km2l = (uint64_t *)ctx_alloc(c, sizeof(uint64_t) * cap);
-        if (!f0 || !f1 || !kp2p || !km2l) return FMM_ENOMEM;
-        const int tc_leaves = (p->flags & FMM_METHOD_TREECODE) ? (int)p->leaves : 0;
-        dtt_init<<<tc_leaves > 0 ? (tc_leaves + 255) / 256 : 1, 256, 0, st>>>(cnt, f0, tc_leaves);
-        FMM_LAUNCH_CHECK(c, "dtt_init");
-        uint64_t *fin = f0, *fout = f1;
-        for (int step = 0; step < nsteps; ++step) {
-            dtt_step<<<2 * FMM_SM_COUNT, 256, 0, st>>>(step, (int)p->leaves, p->hdr, p->theta * p->theta, p->node_lo, p->node_hi,
-                                                       p->node_geo, fin, fout, (unsigned)cap, kp2p, (unsigned)cap, km2l, (unsigned)cap,
-                                                       key_shift, cnt);
-            FMM_LAUNCH_CHECK(c, "dtt_step");
-            uint64_t *t = fin; fin = fout; fout = t;
+        // the lists themselves (kept by the plan) ...
+        const int64_t have = p->list_cap;
+        FMM_TRY(ensure_list(c, &p->p2p_src, have, cap));
+        FMM_TRY(ensure_list(c, &p->m2l_src, have, cap));
+        if (mutual) {
+            FMM_TRY(ensure_list(c, &p->p2p_dst, have, cap));
+            FMM_TRY(ensure_list(c, &p->p2p_recv, have, cap));
         }
-        fmm_hdr hh;
+        p->list_cap = cap;
+        // ... and the scratch of this build (arena)
+        dtt_counters *cnt = (dtt_counters *)ctx_alloc(c, sizeof(dtt_counters));
+        int32_t *rows = (int32_t *)ctx_alloc(c, sizeof(int32_t) * 2 * (size_t)rows_len);
+        int32_t *row_work = (int32_t *)ctx_alloc(c, sizeof(int32_t) * (size_t)p->leaves);
+        int32_t *scan = (int32_t *)ctx_alloc(c, sizeof(int32_t) * 2 * (size_t)rows_len);
+        uint64_t *f0 = (uint64_t *)ctx_alloc(c, sizeof(uint64_t) * cap);
+        uint64_t *f1 = (uint64_t *)ctx_alloc(c, sizeof(uint64_t) * cap);
+        uint64_t *kp2p = (uint64_t *)ctx_alloc(c, sizeof(uint64_t) * cap);
+        uint64_t *km2l = (uint64_t *)ctx_alloc(c, sizeof(uint64_t) * cap);
+        int32_t *p2p_tmp = (int32_t *)ctx_alloc(c, sizeof(int32_t) * cap);
+        int32_t *m2l_tmp = (int32_t *)ctx_alloc(c, sizeof(int32_t) * cap);
+        if (!cnt || !rows || !row_work || !scan || !f0 || !f1 || !kp2p || !km2l || !p2p_tmp || !m2l_tmp) return FMM_ENOMEM;
+        int32_t *tgt = NULL, *mate = NULL, *len = NULL, *seg = NULL;
+        if (mutual) {
+            tgt = (int32_t *)ctx_alloc(c, sizeof(int32_t) * cap);
+            mate = (int32_t *)ctx_alloc(c, sizeof(int32_t) * cap);
+            len = (int32_t *)ctx_alloc(c, sizeof(int32_t) * cap);
+            seg = (int32_t *)ctx_alloc(c, sizeof(int32_t) * cap);
+            if (!tgt || !mate || !len || !seg) return FMM_ENOMEM;
+        }
+        dtt_args a;
+        a.nsteps = nsteps; a.leaves = (int)p->leaves; a.key_shift = key_shift;
+        a.treecode_leaves = (p->flags & FMM_METHOD_TREECODE) ? (int)p->leaves : 0;
+        a.theta2 = p->theta * p->theta;
+        a.hdr = p->hdr; a.node_lo = p->node_lo; a.node_hi = p->node_hi; a.geo = p->node_geo;
+        a.front0 = f0; a.front1 = f1; a.p2p = kp2p; a.m2l = km2l; a.cap = (unsigned)cap;
+        a.rows = rows; a.row_work = row_work; a.rows_len = rows_len; a.cnt = cnt;
+        dtt_top<<<1, 1024, 0, st>>>(a);
+        FMM_LAUNCH_CHECK(c, "dtt_top");
+        dtt_walk<<<DTT_ROOTS / DTT_WALK_WARPS, 32 * DTT_WALK_WARPS, 0, st>>>(a, 0);
+        FMM_LAUNCH_CHECK(c, "dtt_walk");
+        dtt_walk<<<2 * FMM_SM_COUNT, 32 * DTT_WALK_WARPS, 0, st>>>(a, 1);  // (walks that spilled: normally none)
+        FMM_LAUNCH_CHECK(c, "dtt_walk");
+        dtt_totals<<<(unsigned)((p->leaves + 255) / 256 < 2 * FMM_SM_COUNT ? (p->leaves + 255) / 256 : 2 * FMM_SM_COUNT), 256, 0, st>>>(a);
+        FMM_LAUNCH_CHECK(c, "dtt_totals");
+        // rows -> CSR without waiting for the host (the list lengths are read on the device; every kernel below does
+        // nothing if the traversal overflowed its buffers): offsets from the scanned row lengths, entries dealt to their
+        // rows, rows sorted by source, then pair ownership and the reaction segments, then the block orders
+        FMM_TRY(scan_exclusive_i32(c, rows, scan, 2 * (int64_t)rows_len));
+        csr_offsets<<<(rows_len + 255) / 256, 256, 0, st>>>(rows_len, scan, p->p2p_off, p->m2l_off);
+        FMM_LAUNCH_CHECK(c, "csr_offsets");
+        csr_fill<<<4 * FMM_SM_COUNT, 256, 0, st>>>(cnt, kp2p, km2l, key_shift, rows_len, p->p2p_off, p->m2l_off, rows, p2p_tmp, m2l_tmp);
+        FMM_LAUNCH_CHECK(c, "csr_fill");
+        csr_sort_rows<<<(unsigned)(p->leaves + p->nodes), ROWSORT_THREADS, 0, st>>>(cnt, (int)p->leaves, (int)p->leaves, 1, p->p2p_off, p->m2l_off,
+                                                                                   p2p_tmp, m2l_tmp, p->p2p_src, p->m2l_src, tgt);
+        FMM_LAUNCH_CHECK(c, "csr_sort_rows");
+        if (mutual) {
+            p2p_mates<<<4 * FMM_SM_COUNT, 256, 0, st>>>(cnt, cap, p->p2p_off, p->p2p_src, tgt, p->node_lo, p->node_hi, mate, len);
+            FMM_LAUNCH_CHECK(c, "p2p_mates");
+            FMM_TRY(scan_exclusive_i32(c, len, seg, cap));  // segment starts, in particles
+            p2p_segments<<<4 * FMM_SM_COUNT, 256, 0, st>>>(cnt, mate, len, seg, p->p2p_dst, p->p2p_recv);
+            FMM_LAUNCH_CHECK(c, "p2p_segments");
+        }
+        FMM_TRY(make_order(p, cnt, (int)p->leaves, (int)p->leaves, p->p2p_off, p->p2p_src, 1, mutual ? p->p2p_dst : NULL, p->p2p_order));
+        FMM_TRY(make_order(p, cnt, 1, (int)p->nodes, p->m2l_off, p->m2l_src, 0, NULL, p->m2l_order));
         FMM_CUDA(c, cudaMemcpyAsync(&h, cnt, sizeof(h), cudaMemcpyDeviceToHost, st));
         FMM_CUDA(c, cudaMemcpyAsync(&hh, p->hdr, sizeof(hh), cudaMemcpyDeviceToHost, st));
         FMM_CUDA(c, cudaStreamSynchronize(st));  // the one host wait of a build: list lengths, gamma_bar, the input check
+        ctx_free(c, seg); ctx_free(c, len); ctx_free(c, mate); ctx_free(c, tgt);
+        ctx_free(c, m2l_tmp); ctx_free(c, p2p_tmp); ctx_free(c, km2l); ctx_free(c, kp2p); ctx_free(c, f1); ctx_free(c, f0);
+        ctx_free(c, scan); ctx_free(c, row_work); ctx_free(c, rows); ctx_free(c, cnt);
         p->gamma_bar = hh.gamma_bar;
         if (hh.nonfinite) {
-            ctx_free(c, f0); ctx_free(c, f1); ctx_free(c, kp2p); ctx_free(c, km2l); ctx_free(c, cnt);
             snprintf(c->err, sizeof(c->err), "%u non-finite values among the positions, momenta and charges (or gamma_bar is not finite)", hh.nonfinite);
             return FMM_ENONFINITE;
         }
-        ctx_free(c, f0); ctx_free(c, f1);
         if (!h.overflow) break;
-        ctx_free(c, kp2p); ctx_free(c, km2l);
-        cap *= 4;
+        int64_t need = (int64_t)h.n_p2p;  // the counters kept counting past the capacity: they say how much was needed so far
+        if ((int64_t)h.n_m2l > need) need = h.n_m2l;
+        if ((int64_t)h.n_front[0] > need) need = h.n_front[0];
+        if ((int64_t)h.n_front[2] > need) need = h.n_front[2];
+        cap = (need + need / 8 > 2 * cap) ? need + need / 8 : 2 * cap;
     }
     p->n_p2p = h.n_p2p;
     p->n_m2l = h.n_m2l;
-
-    // sort by (target, source), then CSR
-    int64_t nmax = (p->n_p2p > p->n_m2l) ? p->n_p2p : p->n_m2l;
-    uint64_t *tkeys = (uint64_t *)ctx_alloc(c, sizeof(uint64_t) * (nmax > 0 ? nmax : 1));
-    if (!tkeys) return FMM_ENOMEM;
-    if (p->p2p_src) ctx_free(c, p->p2p_src);
-    if (p->m2l_src) ctx_free(c, p->m2l_src);
-    if (p->p2p_dst) ctx_free(c, p->p2p_dst);
-    if (p->p2p_recv) ctx_free(c, p->p2p_recv);
-    p->p2p_dst = p->p2p_recv = NULL;
-    p->p2p_src = (int32_t *)ctx_alloc(c, sizeof(int32_t) * (p->n_p2p > 0 ? p->n_p2p : 1));
-    p->m2l_src = (int32_t *)ctx_alloc(c, sizeof(int32_t) * (p->n_m2l > 0 ? p->n_m2l : 1));
-    if (!p->p2p_src || !p->m2l_src) return FMM_ENOMEM;
-    // the mean-gamma kernel is antisymmetric in the pair, the source-momentum kernel (D depends on p_j) is not
-    const bool mutual = !(p->flags & FMM_KERNEL_SOURCE_MOMENTUM) && p->n_p2p > 0;
-    int32_t *tgt = NULL, *mate = NULL, *len = NULL, *seg = NULL;
-    if (mutual) {
-        p->p2p_dst = (int32_t *)ctx_alloc(c, sizeof(int32_t) * p->n_p2p);
-        p->p2p_recv = (int32_t *)ctx_alloc(c, sizeof(int32_t) * p->n_p2p);
-        tgt = (int32_t *)ctx_alloc(c, sizeof(int32_t) * p->n_p2p);
-        mate = (int32_t *)ctx_alloc(c, sizeof(int32_t) * p->n_p2p);
-        len = (int32_t *)ctx_alloc(c, sizeof(int32_t) * p->n_p2p);
-        seg = (int32_t *)ctx_alloc(c, sizeof(int32_t) * p->n_p2p);
-        if (!p->p2p_dst || !p->p2p_recv || !tgt || !mate || !len || !seg) return FMM_ENOMEM;
-    }
-    FMM_TRY(sort_pairs_u64(c, kp2p, NULL, tkeys, NULL, p->n_p2p, 0, 2 * key_shift));
-    FMM_TRY(sort_pairs_u64(c, km2l, NULL, tkeys, NULL, p->n_m2l, 0, 2 * key_shift));
-    csr_from_sorted<<<(unsigned)((p->n_p2p + 256) / 256), 256, 0, st>>>(kp2p, p->n_p2p, key_shift, (int)p->nodes, p->p2p_off, p->p2p_src, tgt);
-    FMM_LAUNCH_CHECK(c, "csr_from_sorted");
-    csr_from_sorted<<<(unsigned)((p->n_m2l + 256) / 256), 256, 0, st>>>(km2l, p->n_m2l, key_shift, (int)p->nodes, p->m2l_off, p->m2l_src, NULL);
-    FMM_LAUNCH_CHECK(c, "csr_from_sorted");
-    ctx_free(c, tkeys); ctx_free(c, kp2p); ctx_free(c, km2l);
-    FMM_CUDA(c, cudaMemsetAsync(total_dev, 0, 4 * sizeof(unsigned long long), st));
-    if (mutual) {  // pair ownership and the reaction segments
-        const unsigned g = (unsigned)((p->n_p2p + 255) / 256);
-        p2p_mates<<<g, 256, 0, st>>>(p->n_p2p, p->p2p_off, p->p2p_src, tgt, p->node_lo, p->node_hi, mate, len);
-        FMM_LAUNCH_CHECK(c, "p2p_mates");
-        FMM_TRY(scan_exclusive_i32(c, len, seg, p->n_p2p));  // segment starts, in particles
-        p2p_segments<<<g, 256, 0, st>>>(p->n_p2p, p->p2p_src, tgt, mate, len, seg, p->p2p_dst, p->p2p_recv, total_dev);
-        FMM_LAUNCH_CHECK(c, "p2p_segments");
-        ctx_free(c, tgt); ctx_free(c, mate); ctx_free(c, len); ctx_free(c, seg);
-    }
-
-    // block orders (descending work) and evaluation counts
-    FMM_TRY(make_order(p, (int)p->leaves, (int)p->leaves, p->p2p_off, p->p2p_src, 1, p->p2p_dst, p->p2p_order, total_dev));
-    FMM_TRY(make_order(p, 1, (int)p->nodes, p->m2l_off, p->m2l_src, 0, NULL, p->m2l_order, total_dev));
-    unsigned long long total_h2[4] = {0, 0, 0, 0};
-    FMM_CUDA(c, cudaMemcpyAsync(total_h2, total_dev, sizeof(total_h2), cudaMemcpyDeviceToHost, st));
-    FMM_CUDA(c, cudaStreamSynchronize(st));
-    p->p2p_pairs = (int64_t)total_h2[0];
-    p->p2p_max_row = (int64_t)total_h2[1];
-    p->p2p_react = (int64_t)total_h2[2];
-    p->p2p_work = (int64_t)total_h2[3];
+    p->p2p_pairs = (int64_t)h.evals;
+    p->p2p_max_row = (int64_t)h.max_row;
     p->m2l_pairs = (p->flags & FMM_METHOD_TREECODE) ? p->n_m2l * (int64_t)p->P * ((p->N + p->leaves - 1) / p->leaves)  // particle-proxy pairs (full leaves)
                                                     : p->n_m2l * (int64_t)p->P * (int64_t)p->P;
-    ctx_free(c, cnt);
+    // the reaction segments hold at most one leaf per pair of mated entries (segment offsets are 32-bit)
+    p->p2p_mutual = (mutual && p->n_p2p > 0 && (p->n_p2p / 2) * maxleaf < ((int64_t)1 << 31)) ? 1 : 0;
+    p->p2p_react = p->p2p_mutual ? (p->n_p2p / 2) * maxleaf : 0;
     return FMM_OK;
 }

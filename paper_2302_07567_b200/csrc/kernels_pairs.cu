@@ -419,7 +419,7 @@ int pairs_m2l_prepare(fmm_plan *p)  // after the lists: M2L row split for small 
     int64_t need = (int64_t)(K - 1) * 6 * p->P * (p->nodes + 2);
     if (need > p->lpart_cap) {
         if (p->Lpart) ctx_free(c, p->Lpart);
-        p->Lpart = (double *)ctx_alloc(c, sizeof(double) * (size_t)need);
+        p->Lpart = (double *)ctx_alloc_keep(c, sizeof(double) * (size_t)need);
         if (!p->Lpart) return FMM_ENOMEM;
         p->lpart_cap = need;
     }
@@ -427,27 +427,27 @@ int pairs_m2l_prepare(fmm_plan *p)  // after the lists: M2L row split for small 
 }
 
 // the mutual kernel keeps a whole target leaf in one pass of NT x blockDim registers
-static bool p2p_use_mutual(const fmm_plan *p, int maxleaf) { return p->p2p_dst != NULL && maxleaf <= 1024; }
+static bool p2p_use_mutual(const fmm_plan *p, int maxleaf) { return p->p2p_mutual && p->p2p_dst != NULL && maxleaf <= 1024; }
 
 int pairs_p2p_prepare(fmm_plan *p)  // after the lists: choose the row split and size the partial buffers
 {
     fmm_ctx *c = &p->ctx;
     int maxleaf = (int)((p->N + p->leaves - 1) / p->leaves);
     int nt, threads, K;
-    p2p_shape(p->leaves, maxleaf, p->p2p_work, p->p2p_max_row, &nt, &threads, &K, p2p_use_mutual(p, maxleaf));
+    p2p_shape(p->leaves, maxleaf, p->p2p_pairs, p->p2p_max_row, &nt, &threads, &K, p2p_use_mutual(p, maxleaf));
     p->p2p_split = K;
     if (p2p_use_mutual(p, maxleaf) && p->p2p_react > p->react_cap) {
         if (p->p2p_react >= ((int64_t)1 << 31)) return FMM_EOVERFLOW;
         if (p->react) ctx_free(c, p->react);
         p->react_cap = 0;
-        p->react = (double *)ctx_alloc(c, sizeof(double) * 6 * (size_t)p->p2p_react);
+        p->react = (double *)ctx_alloc_keep(c, sizeof(double) * 6 * (size_t)p->p2p_react);
         if (!p->react) return FMM_ENOMEM;
         p->react_cap = p->p2p_react;
     }
     int64_t need = (int64_t)(K + ((p->flags & FMM_METHOD_TREECODE) ? 1 : 0)) * 6 * p->N;  // treecode: + the particle-cluster sums
     if (need > p->near_cap) {
         if (p->near_) ctx_free(c, p->near_);
-        p->near_ = (double *)ctx_alloc(c, sizeof(double) * (size_t)need);
+        p->near_ = (double *)ctx_alloc_keep(c, sizeof(double) * (size_t)need);
         if (!p->near_) return FMM_ENOMEM;
         p->near_cap = need;
     }
@@ -459,7 +459,7 @@ int pairs_p2p(fmm_plan *p)
     fmm_ctx *c = &p->ctx;
     int maxleaf = (int)((p->N + p->leaves - 1) / p->leaves);
     int nt, threads, K;
-    p2p_shape(p->leaves, maxleaf, p->p2p_work, p->p2p_max_row, &nt, &threads, &K, p2p_use_mutual(p, maxleaf));
+    p2p_shape(p->leaves, maxleaf, p->p2p_pairs, p->p2p_max_row, &nt, &threads, &K, p2p_use_mutual(p, maxleaf));
     K = p->p2p_split;
     const bool sm = (p->flags & FMM_KERNEL_SOURCE_MOMENTUM) != 0;
     p->react_used = p2p_use_mutual(p, maxleaf) ? 1 : 0;
@@ -1103,7 +1103,7 @@ int pairs_pc(fmm_plan *p)  // treecode: particle-cluster sums into partial buffe
     FMM_LAUNCH_CHECK(c, "m2l_proxy_points");
     int maxleaf = (int)((p->N + p->leaves - 1) / p->leaves);
     int nt, threads, K;
-    p2p_shape(p->leaves, maxleaf, p->p2p_work, p->p2p_max_row, &nt, &threads, &K);
+    p2p_shape(p->leaves, maxleaf, p->p2p_pairs, p->p2p_max_row, &nt, &threads, &K);
 #define PC_LAUNCH(NT)                                                                                                            \
     pc_kernel<NT><<<(unsigned)p->nodes, threads, 0, c->stream>>>((int)p->N, p->n1, p->gamma_bar, p->m2l_order, p->m2l_off, p->m2l_src, \
                                                                  p->node_lo, p->node_hi, p->tx, p->ty, p->tz, p->node_xi, p->M,  \
