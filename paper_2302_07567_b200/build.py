@@ -16,7 +16,7 @@ from pathlib import Path
 HERE = Path(__file__).resolve().parent
 CSRC = HERE / "csrc"
 LIB = HERE / "libfmm_b200.so"
-SOURCES = ["fmm_api.cu", "sort.cu", "kernels_tree.cu", "kernels_dtt.cu", "kernels_interp.cu", "kernels_pairs.cu"]
+SOURCES = ["fmm_api.cu", "sort.cu", "kernels_tree.cu", "kernels_kd.cu", "kernels_dtt.cu", "kernels_interp.cu", "kernels_pairs.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC", "-Xptxas", "-v"]
 

@@ -221,12 +221,20 @@ static int plan_build(fmm_plan *p, const fmm_particles_t *in, bool refit = false
                             (size_t)64 * (size_t)p->nodes + ((size_t)4 << 20);
     FMM_TRY(ctx_arena_begin(c, estimate));
     struct arena_guard { fmm_ctx *c; ~arena_guard() { ctx_arena_end(c); } } guard{c};
-    FMM_CUDA(c, cudaEventRecord(p->ev_plan[0], c->stream));
-    FMM_TRY(tree_scan_inputs(p, in));  // a0: gamma_bar, coordinate ranges, input check -> p->hdr (device)
-    FMM_TRY(refit ? tree_refit(p, in) : tree_build(p, in));
-    FMM_CUDA(c, cudaEventRecord(p->ev_plan[1], c->stream));
-    FMM_TRY(dtt_build_lists(p));       // (reads gamma_bar and the input check back together with the list lengths)
-    FMM_CUDA(c, cudaEventRecord(p->ev_plan[2], c->stream));
+    for (int round = 0; round < 2; ++round) {
+        if (round == 1) {  // the quantised sort keys of the KD build were not enough (kernels_kd.cu): once more with exact keys
+            p->kd_exact = 1;
+            ctx_arena_end(c);
+            FMM_TRY(ctx_arena_begin(c, estimate + (size_t)48 * (size_t)p->N));
+        }
+        FMM_CUDA(c, cudaEventRecord(p->ev_plan[0], c->stream));
+        FMM_TRY(tree_scan_inputs(p, in));  // a0: gamma_bar, coordinate ranges, input check -> p->hdr (device)
+        FMM_TRY(refit ? tree_refit(p, in) : tree_build(p, in));
+        FMM_CUDA(c, cudaEventRecord(p->ev_plan[1], c->stream));
+        FMM_TRY(dtt_build_lists(p));       // (reads gamma_bar and the input check back together with the list lengths)
+        FMM_CUDA(c, cudaEventRecord(p->ev_plan[2], c->stream));
+        if (!p->kd_retry) break;
+    }
     FMM_TRY(pairs_p2p_prepare(p));
     FMM_TRY(pairs_m2l_prepare(p));
     p->plan_ms_pending = 1;  // (read in fmm_plan_stats: the tail of the build is enqueue-only)

@@ -69,7 +69,7 @@ struct fmm_hdr {
     double g2;               // gamma_bar * gamma_bar (one rounding), the stretch of eq. (3.2)
     double mm[6];            // min x, y, z / max x, y, z of the positions
     unsigned int nonfinite;  // number of NaN / Inf values among x, y, z, px, py, pz, q (saturating) + 1 if gamma_bar is not finite
-    unsigned int pad;
+    unsigned int kd_fallback; // the quantised sort keys of the KD build left a long run out of order: rebuild with exact keys
 };
 
 enum { EV_P2M = 0, EV_M2M, EV_M2L, EV_L2L, EV_P2P, EV_L2P, EV_END, EV_COUNT };
@@ -81,6 +81,8 @@ struct fmm_plan {
     int64_t nodes, leaves;
     double theta, gamma_bar, gamma_bar_param;
     fmm_hdr *hdr;           // device
+    int kd_exact;           // KD build with the exact 64-bit sort keys (set once the quantised keys were not enough)
+    int kd_retry;           // the last build asked for that
     int valid;              // 0 after a failed build: fmm_eval refuses the plan until an update / refit succeeds
     uint32_t flags;
     // particles in tree order (SoA), source weights w0 = q gamma, w1..3 = q p
@@ -137,6 +139,7 @@ int tree_gamma_bar(fmm_ctx *c, int64_t N, const double *px, const double *py, co
                    double *gamma_bar_out /* host */);  // plan-less calls (fmm_direct): synchronises
 int tree_scan_inputs(fmm_plan *p, const fmm_particles_t *in);  // a0 into p->hdr, enqueue only
 int tree_build(fmm_plan *p, const fmm_particles_t *in);
+int kd_build_order(fmm_plan *p, const fmm_particles_t *in, uint32_t **order_out);  // kernels_kd.cu
 int tree_boxes(fmm_plan *p);
 int tree_refit(fmm_plan *p, const fmm_particles_t *in);  // keeps the particle order of the last build
 // ---- kernels_dtt.cu -----------------------------------------------------------------
@@ -166,6 +169,7 @@ int sort_pairs_u64(fmm_ctx *c, uint64_t *keys, uint32_t *vals, uint64_t *tmp_key
                    int64_t n, int bit_lo, int bit_hi);
 int sort_pairs_u64_batched(fmm_ctx *c, uint64_t *keys, uint32_t *vals, uint64_t *tmp_keys, uint32_t *tmp_vals,
                            int64_t n, int batch, int bit_lo, int bit_hi);  // `batch` segments of length n, back to back
+int sort_pairs_u32_batched(fmm_ctx *c, uint32_t *keys, uint32_t *vals, uint32_t *tmp_keys, uint32_t *tmp_vals, int64_t n, int batch);
 int scan_exclusive_i32(fmm_ctx *c, const int32_t *in, int32_t *out, int64_t n);  // out may alias in
 
 #ifdef __CUDACC__

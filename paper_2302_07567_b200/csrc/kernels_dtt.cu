@@ -485,6 +485,8 @@ int dtt_build_lists(fmm_plan *p)
         ctx_free(c, m2l_tmp); ctx_free(c, p2p_tmp); ctx_free(c, km2l); ctx_free(c, kp2p); ctx_free(c, f1); ctx_free(c, f0);
         ctx_free(c, scan); ctx_free(c, row_work); ctx_free(c, rows); ctx_free(c, cnt);
         p->gamma_bar = hh.gamma_bar;
+        p->kd_retry = (hh.kd_fallback && !p->kd_exact) ? 1 : 0;
+        if (p->kd_retry) return FMM_OK;  // (plan_build runs the whole build again with exact sort keys)
         if (hh.nonfinite) {
             snprintf(c->err, sizeof(c->err), "%u non-finite values among the positions, momenta and charges (or gamma_bar is not finite)", hh.nonfinite);
             return FMM_ENONFINITE;

@@ -1,0 +1,506 @@
+// kernels_kd.cu -- step a1, mode KD: the particle order of the balanced cluster tree of Alg 5.1 / 5.2
+// (App. B) on the array tree of section 8.
+//
+// Exactly the paper's tree (readings T-1 .. T-3, G7 - G9): every node splits at the median rank along the axis of
+// largest stretched extent, members ranked by (coordinate, original index), the first ceil(size/2) go left, ties of
+// the axis choice to the first maximiser, ascending original index inside a leaf.  Built without recursion:
+//   1. three index lists LX, LY, LZ sorted by (coordinate, index) and the index-ordered list LI.  The sort key is a
+//      monotone 32-bit quantisation of the coordinate (4 radix passes instead of 8 on the 64-bit pattern); runs of
+//      equal keys are then put into exact (coordinate, index) order by kd_find_runs / kd_fix_runs, which report the (pathological)
+//      inputs they cannot repair locally so that the build falls back to the exact 64-bit keys;
+//   2. per level: mark the left members in a bit mask (the first ceil(size/2) entries of the node's segment in the list
+//      of its split axis; the node's box is read off the segment ends of the three sorted lists), then split every
+//      segment of all four lists stably (left members first).  One kernel each: the running count of a node that spans
+//      several tiles is looked up from the tiles before it (every tile publishes its count before it looks back, so
+//      nothing waits on a chain), node ranges are closed-form (T-2);
+//   3. once a node holds at most KD_LOCAL particles one block finishes all its remaining levels in shared memory.
+// Integer / compare work only: HBM-, L2- and launch-latency-bound.
+#include "fmm_internal.cuh"
+
+#define KD_TILE 2048     // list entries per block of the level kernels (256 threads x 8)
+#define KD_LOCAL 4096    // nodes of at most this many particles are finished by one block
+#define KDL_THREADS 512
+#define KDL_ITEMS 8      // KDL_THREADS x KDL_ITEMS = KD_LOCAL
+
+// node [lo, hi) at `level` that contains list position pos (T-2: the left child gets ceil(size / 2))
+__device__ __forceinline__ void kd_range_of(int N, int level, int pos, int &lo, int &hi)
+{
+    lo = 0;
+    hi = N;
+    for (int l = 0; l < level; ++l) {
+        const int mid = lo + (hi - lo + 1) / 2;
+        if (pos < mid) hi = mid; else lo = mid;
+    }
+}
+
+// Alg 5.1: split axis = first maximiser of s_k (b_k - a_k) (reading G9).  The lists are sorted by
+// coordinate inside every node segment, so the bounding box is read off the segment ends.
+__device__ __forceinline__ int kd_axis(double gamma_bar, double x0, double x1, double y0, double y1, double z0, double z1)
+{
+    const double ex = __dmul_rn(1.0, __dsub_rn(x1, x0));
+    const double ey = __dmul_rn(1.0, __dsub_rn(y1, y0));
+    const double ez = __dmul_rn(gamma_bar, __dsub_rn(z1, z0));
+    int a = 0;
+    double best = ex;
+    if (ey > best) { best = ey; a = 1; }
+    if (ez > best) { best = ez; a = 2; }
+    return a;
+}
+
+// ---------------------------------------------------------------------------------------
+// sort keys
+// ---------------------------------------------------------------------------------------
+// total order of doubles as unsigned keys; -0.0 == +0.0 (the oracle compares with <, so they tie)
+__device__ __forceinline__ uint64_t sortable_key(double v)
+{
+    v = v + 0.0;  // -0.0 -> +0.0
+    uint64_t b = (uint64_t)__double_as_longlong(v);
+    return (b >> 63) ? ~b : (b | 0x8000000000000000ull);
+}
+
+__global__ void kd_keys64(int N, const double *__restrict__ x, const double *__restrict__ y, const double *__restrict__ z,
+                          uint64_t *__restrict__ keys /* [3 N] */, uint32_t *__restrict__ lists /* [4 N] */)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= N) return;
+    keys[i] = sortable_key(x[i]);
+    keys[(size_t)N + i] = sortable_key(y[i]);
+    keys[2 * (size_t)N + i] = sortable_key(z[i]);
+#pragma unroll
+    for (int a = 0; a < 4; ++a) lists[(size_t)a * N + i] = (uint32_t)i;
+}
+
+// q = min(floor((c - lo) * 2^32 / (hi - lo)), 2^32 - 1): every step is monotone in c, so c1 <= c2 implies q1 <= q2
+__global__ void kd_keys32(int N, const double *__restrict__ x, const double *__restrict__ y, const double *__restrict__ z,
+                          const fmm_hdr *__restrict__ hdr, uint32_t *__restrict__ keys /* [3 N] */, uint32_t *__restrict__ lists /* [4 N] */)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= N) return;
+    const double c[3] = {x[i], y[i], z[i]};
+#pragma unroll
+    for (int a = 0; a < 3; ++a) {
+        const double lo = hdr->mm[a], ext = hdr->mm[3 + a] - lo;
+        const double scale = (ext > 0.0) ? 4294967296.0 / ext : 0.0;
+        double f = floor((c[a] - lo) * scale);
+        f = fmin(f, 4294967295.0);
+        keys[(size_t)a * N + i] = (f > 0.0) ? (uint32_t)f : 0u;  // (NaN / negative -> 0; non-finite inputs are refused later)
+        lists[(size_t)a * N + i] = (uint32_t)i;
+    }
+    lists[3 * (size_t)N + i] = (uint32_t)i;
+}
+
+// After the stable sort by the quantised key a run of equal keys is in index order; the tree wants (coordinate, index).
+// kd_find_runs (read-only): the thread at the FIRST out-of-order position of a run records the run; kd_fix_runs: one thread
+// per recorded run puts it in order (insertion sort on the indices, at most KD_RUN entries).  Longer runs that are out of
+// order raise hdr->kd_fallback (the build is redone with exact keys).
+#define KD_RUN 64
+__global__ void kd_find_runs(int N, const double *__restrict__ x, const double *__restrict__ y, const double *__restrict__ z,
+                             const uint32_t *__restrict__ keys /* [3 N] sorted */, const uint32_t *__restrict__ lists,
+                             fmm_hdr *__restrict__ hdr, unsigned int *__restrict__ nruns, uint2 *__restrict__ runs /* (axis N + head, end) */)
+{
+    const int64_t g = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (g >= 3 * (int64_t)N) return;
+    const int a = (int)(g / N), j = (int)(g - (int64_t)a * N);
+    if (j == 0) return;
+    const uint32_t *K = keys + (size_t)a * N;
+    const uint32_t *V = lists + (size_t)a * N;
+    const double *coord = (a == 0) ? x : (a == 1) ? y : z;
+    const uint32_t q = K[j];
+    if (K[j - 1] != q) return;
+    if (!(coord[V[j]] < coord[V[j - 1]])) return;  // in order here
+    // first violation of its run?  walk back to the head of the run
+    int h = j - 1;
+    while (h > 0 && K[h - 1] == q) {
+        if (j - h > KD_RUN) { hdr->kd_fallback = 1; return; }
+        if (coord[V[h]] < coord[V[h - 1]]) return;  // an earlier violation: that thread records the run
+        --h;
+    }
+    int e = j + 1;
+    while (e < N && K[e] == q) {
+        if (e - h > KD_RUN) { hdr->kd_fallback = 1; return; }
+        ++e;
+    }
+    const unsigned int slot = atomicAdd(nruns, 1u);
+    runs[slot] = make_uint2((unsigned int)a * (unsigned int)N + (unsigned int)h, (unsigned int)a * (unsigned int)N + (unsigned int)e);
+}
+
+__global__ void kd_fix_runs(int N, const double *__restrict__ x, const double *__restrict__ y, const double *__restrict__ z,
+                            const unsigned int *__restrict__ nruns, const uint2 *__restrict__ runs, uint32_t *__restrict__ lists)
+{
+    const unsigned int n = *nruns;
+    for (unsigned int r = blockIdx.x * blockDim.x + threadIdx.x; r < n; r += gridDim.x * blockDim.x) {
+        const uint2 run = runs[r];
+        const int a = (int)(run.x / (unsigned int)N);
+        const double *coord = (a == 0) ? x : (a == 1) ? y : z;
+        uint32_t *V = lists;
+        for (unsigned int k = run.x + 1; k < run.y; ++k) {  // [head, k) is in (coordinate, index) order; equals keep ascending index
+            const uint32_t v = V[k];
+            const double cv = coord[v];
+            unsigned int m = k;
+            while (m > run.x && cv < coord[V[m - 1]]) { V[m] = V[m - 1]; --m; }
+            V[m] = v;
+        }
+    }
+}
+
+// ---------------------------------------------------------------------------------------
+// one level on the whole lists (nodes larger than KD_LOCAL: a tile of KD_TILE entries meets at most two nodes)
+// ---------------------------------------------------------------------------------------
+// Alg 5.2 (readings G7, G8): in the list of the split axis the first ceil(size/2) members of the
+// node (ranked by (coordinate, index)) go to the left child: their bits are set.
+__global__ void __launch_bounds__(256) kd_mark(int N, int level, const double *__restrict__ x, const double *__restrict__ y,
+                                               const double *__restrict__ z, const uint32_t *__restrict__ lists,
+                                               const fmm_hdr *__restrict__ hdr, uint32_t *__restrict__ bits)
+{
+    __shared__ int s_lo[2], s_hi[2], s_axis[2];
+    const int start = blockIdx.x * KD_TILE, end = min(N, start + KD_TILE);
+    if (threadIdx.x < 2) {
+        int lo, hi;
+        kd_range_of(N, level, threadIdx.x == 0 ? start : end - 1, lo, hi);
+        const uint32_t *LX = lists, *LY = lists + N, *LZ = lists + 2 * (size_t)N;
+        s_lo[threadIdx.x] = lo;
+        s_hi[threadIdx.x] = hi;
+        s_axis[threadIdx.x] = kd_axis(hdr->gamma_bar, x[LX[lo]], x[LX[hi - 1]], y[LY[lo]], y[LY[hi - 1]], z[LZ[lo]], z[LZ[hi - 1]]);
+    }
+    __syncthreads();
+    for (int i = start + threadIdx.x; i < end; i += 256) {
+        const int k = (i >= s_hi[0]) ? 1 : 0;
+        const int lo = s_lo[k], hi = s_hi[k];
+        const int mid = lo + (hi - lo + 1) / 2;
+        if (i < mid) {
+            const uint32_t p = lists[(size_t)s_axis[k] * N + i];
+            atomicOr(&bits[p >> 5], 1u << (p & 31));
+        }
+    }
+}
+
+__device__ __forceinline__ int kd_block_scan_256(int v, int *total, int *sm /* [8] */)
+{
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    int inc = v;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        const int t = __shfl_up_sync(0xffffffffu, inc, o);
+        if (lane >= o) inc += t;
+    }
+    __syncthreads();
+    if (lane == 31) sm[warp] = inc;
+    __syncthreads();
+    int wb = 0, tot = 0;
+#pragma unroll
+    for (int w = 0; w < 8; ++w) {
+        const int t = sm[w];
+        if (w < warp) wb += t;
+        tot += t;
+    }
+    *total = tot;
+    return wb + inc - v;
+}
+
+// stable split of every node segment of the four lists: left members first.  Tiles are taken in ticket order, publish the
+// number of left members of their last node, and a tile whose first node began earlier adds up the tiles before it.
+__global__ void __launch_bounds__(256) kd_split(int N, int level, int tiles_per_list, const uint32_t *__restrict__ bits,
+                                                const uint32_t *__restrict__ cur, uint32_t *__restrict__ nxt,
+                                                unsigned int *pub /* [4 tiles_per_list] */, unsigned int *ticket)
+{
+    __shared__ int sm[8];
+    __shared__ unsigned int s_tile;
+    if (threadIdx.x == 0) s_tile = atomicAdd(ticket, 1u);
+    __syncthreads();
+    const int tile = (int)s_tile;
+    const int li = tile / tiles_per_list, t = tile - li * tiles_per_list;
+    const int start = t * KD_TILE, end = min(N, start + KD_TILE);
+    int loA, hiA, hiB;
+    kd_range_of(N, level, start, loA, hiA);
+    hiB = hiA;
+    if (hiA < end) {
+        int lo2;
+        kd_range_of(N, level, hiA, lo2, hiB);
+    }
+    const uint32_t *L = cur + (size_t)li * N;
+    uint32_t *O = nxt + (size_t)li * N;
+    const int i0 = start + threadIdx.x * 8;
+    uint32_t part[8];
+    unsigned int flags = 0;
+    int s = 0, sA = 0;
+#pragma unroll
+    for (int k = 0; k < 8; ++k) {
+        const int i = i0 + k;
+        part[k] = (i < end) ? L[i] : 0u;
+        const unsigned int f = (i < end) ? ((__ldg(&bits[part[k] >> 5]) >> (part[k] & 31)) & 1u) : 0u;
+        flags |= f << k;
+        s += (int)f;
+        sA += (int)(f && i < hiA);
+    }
+    int total, cA;
+    const int ex = kd_block_scan_256(s, &total, sm);
+    kd_block_scan_256(sA, &cA, sm);
+    const unsigned int tag = (unsigned int)(level + 1) << 16;
+    if (threadIdx.x == 0) {
+        __threadfence();
+        atomicExch(&pub[tile], tag | (unsigned int)((hiA < end) ? total - cA : total));
+    }
+    // left members of node A in the tiles before this one
+    int carry = 0;
+    if (loA < start) {
+        const int nback = (start - loA + KD_TILE - 1) / KD_TILE;
+        int mine = 0;
+        for (int j = threadIdx.x + 1; j <= nback; j += 256) {
+            unsigned int w;
+            do { w = *((volatile unsigned int *)&pub[tile - j]); } while ((w & 0xffff0000u) != tag);
+            mine += (int)(w & 0xffffu);
+        }
+        kd_block_scan_256(mine, &carry, sm);
+    }
+    int running = ex;
+#pragma unroll
+    for (int k = 0; k < 8; ++k) {
+        const int i = i0 + k;
+        if (i < end) {
+            const bool inA = i < hiA;
+            const int lo = inA ? loA : hiA, hi = inA ? hiA : hiB;
+            const int mid = lo + (hi - lo + 1) / 2;
+            const int before = inA ? carry + running : running - cA;  // left members of the node before entry i
+            const unsigned int f = (flags >> k) & 1u;
+            O[f ? (lo + before) : (mid + (i - lo - before))] = part[k];
+            running += (int)f;
+        }
+    }
+}
+
+// ---------------------------------------------------------------------------------------
+// all remaining levels of one node of at most KD_LOCAL particles in one block
+// ---------------------------------------------------------------------------------------
+// The node's members are renamed 0 .. m-1 by ascending original index (their order in LI); the three sorted lists and LI
+// become arrays of 16-bit local names in shared memory, the left flags a byte array.  Output: the node's part of the
+// final particle order (leaves in heap order, ascending index inside, reading T-3).
+struct kdl_smem {
+    uint32_t ids[KD_LOCAL];          // local name -> particle
+    uint16_t L[2][4][KD_LOCAL];      // ping-pong: LX, LY, LZ, LI in local names
+    uint16_t F[KD_LOCAL + 8];        // exclusive scan of the flags along one list
+    uint8_t flag[KD_LOCAL];
+    uint8_t axis[KD_LOCAL];          // split axis per sub-node of the current level
+    int scan[KDL_THREADS / 32];
+};
+
+__device__ __forceinline__ int kdl_block_scan(int v, int *total, int *sm)
+{
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    int inc = v;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        const int t = __shfl_up_sync(0xffffffffu, inc, o);
+        if (lane >= o) inc += t;
+    }
+    __syncthreads();
+    if (lane == 31) sm[warp] = inc;
+    __syncthreads();
+    int wb = 0, tot = 0;
+#pragma unroll
+    for (int w = 0; w < KDL_THREADS / 32; ++w) {
+        const int t = sm[w];
+        if (w < warp) wb += t;
+        tot += t;
+    }
+    *total = tot;
+    return wb + inc - v;
+}
+
+// sub-node of [lo, hi) `depth` levels further down that contains position pos; k = its index among the 2^depth sub-nodes
+__device__ __forceinline__ void kdl_sub_of(int lo, int hi, int depth, int pos, int &slo, int &shi, int &k)
+{
+    slo = lo;
+    shi = hi;
+    k = 0;
+    for (int l = 0; l < depth; ++l) {
+        const int mid = slo + (shi - slo + 1) / 2;
+        k <<= 1;
+        if (pos < mid) shi = mid; else { slo = mid; k |= 1; }
+    }
+}
+
+__global__ void __launch_bounds__(KDL_THREADS) kd_local(int N, int level0, int kappa, const double *__restrict__ x, const double *__restrict__ y,
+                                                        const double *__restrict__ z, const fmm_hdr *__restrict__ hdr,
+                                                        const uint32_t *__restrict__ lists, uint32_t *__restrict__ order)
+{
+    extern __shared__ __align__(16) unsigned char kdl_raw[];
+    kdl_smem &S = *reinterpret_cast<kdl_smem *>(kdl_raw);
+    int lo = 0, hi = N;
+    for (int b = level0 - 1; b >= 0; --b) {  // node blockIdx.x of level0
+        const int mid = lo + (hi - lo + 1) / 2;
+        if ((blockIdx.x >> b) & 1) lo = mid; else hi = mid;
+    }
+    const int m = hi - lo;
+    if (m <= 0) return;
+    const double gamma_bar = hdr->gamma_bar;
+    for (int r = threadIdx.x; r < m; r += KDL_THREADS) {
+        S.ids[r] = lists[3 * (size_t)N + lo + r];
+        S.L[0][3][r] = (uint16_t)r;
+    }
+    __syncthreads();
+    for (int q = threadIdx.x; q < 3 * m; q += KDL_THREADS) {  // local name of a particle = its rank in the (ascending) ids
+        const int a = q / m, i = q - a * m;
+        const uint32_t p = lists[(size_t)a * N + lo + i];
+        int b0 = 0, b1 = m;
+        while (b0 < b1) {
+            const int mid = (b0 + b1) >> 1;
+            if (S.ids[mid] < p) b0 = mid + 1; else b1 = mid;
+        }
+        S.L[0][a][i] = (uint16_t)b0;
+    }
+    __syncthreads();
+    int cb = 0;
+    for (int level = level0; level < kappa; ++level) {
+        const int depth = level - level0, nsub = 1 << depth;
+        uint16_t(*Lc)[KD_LOCAL] = S.L[cb];
+        uint16_t(*Ln)[KD_LOCAL] = S.L[cb ^ 1];
+        // split axis of every sub-node (Alg 5.1) from the ends of its segments
+        for (int k = threadIdx.x; k < nsub; k += KDL_THREADS) {
+            int slo = lo, shi = hi;
+            for (int b = depth - 1; b >= 0; --b) {
+                const int mid = slo + (shi - slo + 1) / 2;
+                if ((k >> b) & 1) slo = mid; else shi = mid;
+            }
+            int ax = 0;
+            if (shi > slo) {
+                const int a0 = slo - lo, a1 = shi - 1 - lo;
+                ax = kd_axis(gamma_bar, x[S.ids[Lc[0][a0]]], x[S.ids[Lc[0][a1]]], y[S.ids[Lc[1][a0]]], y[S.ids[Lc[1][a1]]],
+                             z[S.ids[Lc[2][a0]]], z[S.ids[Lc[2][a1]]]);
+            }
+            S.axis[k] = (uint8_t)ax;
+        }
+        __syncthreads();
+        // this thread's positions: KDL_ITEMS consecutive entries; their sub-nodes are the same in all four lists
+        const int i0 = threadIdx.x * KDL_ITEMS;
+        int slo[KDL_ITEMS], smid[KDL_ITEMS];
+#pragma unroll
+        for (int k = 0; k < KDL_ITEMS; ++k) {
+            const int i = i0 + k;
+            slo[k] = smid[k] = 0;
+            if (i < m) {
+                int a, b, sk;
+                kdl_sub_of(lo, hi, depth, lo + i, a, b, sk);
+                slo[k] = a - lo;
+                smid[k] = a - lo + (b - a + 1) / 2;
+                S.flag[Lc[S.axis[sk]][i]] = (uint8_t)(i < smid[k]);  // Alg 5.2: the first ceil(size/2) along the split axis go left
+            }
+        }
+        __syncthreads();
+        for (int a = 0; a < 4; ++a) {
+            uint16_t r[KDL_ITEMS];
+            unsigned int fl = 0;
+            int s = 0;
+#pragma unroll
+            for (int k = 0; k < KDL_ITEMS; ++k) {
+                const int i = i0 + k;
+                r[k] = (i < m) ? Lc[a][i] : (uint16_t)0;
+                const unsigned int f = (i < m) ? S.flag[r[k]] : 0u;
+                fl |= f << k;
+                s += (int)f;
+            }
+            int total;
+            int run = kdl_block_scan(s, &total, S.scan);
+#pragma unroll
+            for (int k = 0; k < KDL_ITEMS; ++k) {
+                if (i0 + k < m) S.F[i0 + k] = (uint16_t)run;
+                run += (int)((fl >> k) & 1u);
+            }
+            __syncthreads();
+#pragma unroll
+            for (int k = 0; k < KDL_ITEMS; ++k) {
+                const int i = i0 + k;
+                if (i < m) {
+                    const int before = (int)S.F[i] - (int)S.F[slo[k]];  // left members of the sub-node before entry i
+                    const unsigned int f = (fl >> k) & 1u;
+                    Ln[a][f ? (slo[k] + before) : (smid[k] + (i - slo[k] - before))] = r[k];
+                }
+            }
+            __syncthreads();
+        }
+        cb ^= 1;
+    }
+    for (int i = threadIdx.x; i < m; i += KDL_THREADS) order[lo + i] = S.ids[S.L[cb][3][i]];
+}
+
+// ---------------------------------------------------------------------------------------
+// host: particle order of the KD tree into `order` ([N], scratch from the arena)
+// ---------------------------------------------------------------------------------------
+int kd_build_order(fmm_plan *p, const fmm_particles_t *in, uint32_t **order_out)
+{
+    fmm_ctx *c = &p->ctx;
+    cudaStream_t st = c->stream;
+    const int N = (int)p->N, T = 256, gN = (N + T - 1) / T;
+    uint32_t *lists = (uint32_t *)ctx_alloc(c, sizeof(uint32_t) * 4 * (size_t)N);  // LX, LY, LZ, LI
+    uint32_t *lists2 = (uint32_t *)ctx_alloc(c, sizeof(uint32_t) * 4 * (size_t)N);
+    if (!lists || !lists2) return FMM_ENOMEM;
+    if (p->kappa == 0) {  // the root is a leaf: index order
+        uint32_t *k32 = (uint32_t *)ctx_alloc(c, sizeof(uint32_t) * 3 * (size_t)N);
+        if (!k32) return FMM_ENOMEM;
+        kd_keys32<<<gN, T, 0, st>>>(N, in->x, in->y, in->z, p->hdr, k32, lists);
+        FMM_LAUNCH_CHECK(c, "kd_keys32");
+        *order_out = lists + 3 * (size_t)N;
+        return FMM_OK;
+    }
+    if (p->kd_exact) {  // exact 64-bit keys: 8 radix passes
+        uint64_t *keys = (uint64_t *)ctx_alloc(c, sizeof(uint64_t) * 3 * (size_t)N);
+        uint64_t *tkeys = (uint64_t *)ctx_alloc(c, sizeof(uint64_t) * 3 * (size_t)N);
+        if (!keys || !tkeys) return FMM_ENOMEM;
+        kd_keys64<<<gN, T, 0, st>>>(N, in->x, in->y, in->z, keys, lists);
+        FMM_LAUNCH_CHECK(c, "kd_keys64");
+        FMM_TRY(sort_pairs_u64_batched(c, keys, lists, tkeys, lists2, N, 3, 0, 64));
+        ctx_free(c, tkeys);
+        ctx_free(c, keys);
+    } else {
+        uint32_t *k32 = (uint32_t *)ctx_alloc(c, sizeof(uint32_t) * 3 * (size_t)N);
+        uint32_t *t32 = (uint32_t *)ctx_alloc(c, sizeof(uint32_t) * 3 * (size_t)N);
+        if (!k32 || !t32) return FMM_ENOMEM;
+        kd_keys32<<<gN, T, 0, st>>>(N, in->x, in->y, in->z, p->hdr, k32, lists);
+        FMM_LAUNCH_CHECK(c, "kd_keys32");
+        FMM_TRY(sort_pairs_u32_batched(c, k32, lists, t32, lists2, N, 3));
+        // (3 N <= 2^32 - 1: positions axis N + j fit 32 bits because sort_pairs_u32_batched requires 3 N < 2^31)
+        unsigned int *nruns = (unsigned int *)ctx_alloc(c, sizeof(unsigned int) * 2 + sizeof(uint2) * (3 * (size_t)N / 2 + 2));
+        if (!nruns) return FMM_ENOMEM;
+        uint2 *runs = reinterpret_cast<uint2 *>(nruns + 2);
+        FMM_CUDA(c, cudaMemsetAsync(nruns, 0, sizeof(unsigned int) * 2, st));
+        kd_find_runs<<<(unsigned)((3 * (int64_t)N + T - 1) / T), T, 0, st>>>(N, in->x, in->y, in->z, k32, lists, p->hdr, nruns, runs);
+        FMM_LAUNCH_CHECK(c, "kd_find_runs");
+        kd_fix_runs<<<FMM_SM_COUNT, 128, 0, st>>>(N, in->x, in->y, in->z, nruns, runs, lists);
+        FMM_LAUNCH_CHECK(c, "kd_fix_runs");
+        ctx_free(c, nruns);
+        ctx_free(c, t32);
+        ctx_free(c, k32);
+    }
+    // levels on the whole lists while a node holds more than KD_LOCAL particles ...
+    int level0 = 0;
+    while (level0 < p->kappa && (((int64_t)N + ((int64_t)1 << level0) - 1) >> level0) > KD_LOCAL) ++level0;
+    uint32_t *cur = lists, *nxt = lists2;
+    if (level0 > 0) {
+        const int tiles = (N + KD_TILE - 1) / KD_TILE;
+        const size_t nbits = ((size_t)N + 31) / 32;
+        uint32_t *bits = (uint32_t *)ctx_alloc(c, sizeof(uint32_t) * nbits);
+        unsigned int *pub = (unsigned int *)ctx_alloc(c, sizeof(unsigned int) * (4 * (size_t)tiles + 64));
+        if (!bits || !pub) return FMM_ENOMEM;
+        unsigned int *ticket = pub + 4 * (size_t)tiles;  // one counter per level
+        FMM_CUDA(c, cudaMemsetAsync(pub, 0, sizeof(unsigned int) * (4 * (size_t)tiles + 64), st));
+        for (int level = 0; level < level0; ++level) {
+            FMM_CUDA(c, cudaMemsetAsync(bits, 0, sizeof(uint32_t) * nbits, st));
+            kd_mark<<<tiles, 256, 0, st>>>(N, level, in->x, in->y, in->z, cur, p->hdr, bits);
+            FMM_LAUNCH_CHECK(c, "kd_mark");
+            kd_split<<<4 * tiles, 256, 0, st>>>(N, level, tiles, bits, cur, nxt, pub, ticket + level);
+            FMM_LAUNCH_CHECK(c, "kd_split");
+            uint32_t *t = cur; cur = nxt; nxt = t;
+        }
+    }
+    // ... then one block per node for the rest
+    if (level0 < p->kappa) {
+        const size_t smem = sizeof(kdl_smem);
+        FMM_CUDA(c, cudaFuncSetAttribute((const void *)kd_local, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        uint32_t *order = nxt;  // (the other list buffer is free now)
+        kd_local<<<1u << level0, KDL_THREADS, smem, st>>>(N, level0, p->kappa, in->x, in->y, in->z, p->hdr, cur, order);
+        FMM_LAUNCH_CHECK(c, "kd_local");
+        *order_out = order;
+    } else {
+        *order_out = cur + 3 * (size_t)N;  // the index-ordered list: leaves in heap order, ascending index inside (T-3)
+    }
+    return FMM_OK;
+}

@@ -1,8 +1,7 @@
 // kernels_tree.cu -- steps a0-a2 of the hot path:
 //   a0  mean momentum -> gamma_bar, source weights q gamma, q p
-//   a1  particle order of the balanced cluster tree: mode KD = Alg 5.1/5.2 (PAPER.md:255-289,
-//       App. B) on the array tree of section 8;
-//       mode MORTON_MEDIAN = 63-bit Morton order of the stretched coordinates (DESIGN T-3')
+//   a1  particle order of the balanced cluster tree: mode KD = Alg 5.1/5.2 in kernels_kd.cu;
+//       mode MORTON_MEDIAN = 63-bit Morton order of the stretched coordinates (DESIGN T-3') here
 //   a2  tight bounding boxes, stretched radii and centres (Alg 5.6/5.7)
 // Everything here is integer / compare / min-max work: HBM- and launch-latency-bound.
 #include "fmm_internal.cuh"
@@ -204,7 +203,7 @@ __global__ void a0_scan_final(int64_t N, double gamma_bar_param, const double *_
         unsigned int nb = bad > 4.0e9 ? 4000000000u : (unsigned int)bad;
         if (!isfinite(gb)) nb += 1u;
         hdr->nonfinite = nb;
-        hdr->pad = 0;
+        hdr->kd_fallback = 0;
     }
 }
 
@@ -219,168 +218,6 @@ int tree_scan_inputs(fmm_plan *p, const fmm_particles_t *in)
     FMM_LAUNCH_CHECK(c, "a0_scan_final");
     ctx_free(c, partial);
     return FMM_OK;
-}
-
-// ---------------------------------------------------------------------------------------
-// a1, mode KD
-// ---------------------------------------------------------------------------------------
-// total order of doubles as unsigned keys; -0.0 == +0.0 (the oracle compares with <, so they tie)
-__device__ __forceinline__ uint64_t sortable_key(double v)
-{
-    v = v + 0.0;  // -0.0 -> +0.0
-    uint64_t b = (uint64_t)__double_as_longlong(v);
-    return (b >> 63) ? ~b : (b | 0x8000000000000000ull);
-}
-
-__global__ void kd_make_keys(int N, const double *__restrict__ coord, uint64_t *__restrict__ keys, uint32_t *__restrict__ vals)
-{
-    int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= N) return;
-    keys[i] = sortable_key(coord[i]);
-    vals[i] = (uint32_t)i;
-}
-
-__global__ void kd_iota(int N, uint32_t *__restrict__ v)
-{
-    int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i < N) v[i] = (uint32_t)i;
-}
-
-// Alg 5.1: split axis = first maximiser of s_k (b_k - a_k) (reading G9).  The lists
-// are sorted by coordinate inside every node segment, so the bounding box is read off the segment ends.
-__global__ void kd_choose_axis(int N, int level, const double *__restrict__ x, const double *__restrict__ y, const double *__restrict__ z,
-                               const uint32_t *__restrict__ LX, const uint32_t *__restrict__ LY, const uint32_t *__restrict__ LZ,
-                               const fmm_hdr *__restrict__ hdr, int8_t *__restrict__ axis /* [2^level] */)
-{
-    int k = blockIdx.x * blockDim.x + threadIdx.x;
-    if (k >= (1 << level)) return;
-    const double gamma_bar = hdr->gamma_bar;
-    int lo = 0, hi = N;
-    for (int b = level - 1; b >= 0; --b) {
-        int mid = lo + (hi - lo + 1) / 2;
-        if ((k >> b) & 1) lo = mid; else hi = mid;
-    }
-    int a = 0;
-    if (hi > lo) {
-        double ex = __dmul_rn(1.0, __dsub_rn(x[LX[hi - 1]], x[LX[lo]]));
-        double ey = __dmul_rn(1.0, __dsub_rn(y[LY[hi - 1]], y[LY[lo]]));
-        double ez = __dmul_rn(gamma_bar, __dsub_rn(z[LZ[hi - 1]], z[LZ[lo]]));
-        double best = ex;
-        if (ey > best) { best = ey; a = 1; }
-        if (ez > best) { best = ez; a = 2; }
-    }
-    axis[k] = (int8_t)a;
-}
-
-// Alg 5.2 (readings G7, G8): in the list of the chosen axis the first ceil(size/2)
-// members of the node (ranked by (coordinate, index)) go to the left child.
-__global__ void kd_mark_left(int N, int level, const int8_t *__restrict__ axis, const uint32_t *__restrict__ LX,
-                             const uint32_t *__restrict__ LY, const uint32_t *__restrict__ LZ, uint8_t *__restrict__ left)
-{
-    int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= N) return;
-    int node, lo, hi;
-    node_at_level(N, level, i, node, lo, hi);
-    int a = axis[node - (1 << level)];
-    int mid = lo + (hi - lo + 1) / 2;
-    uint32_t part = (a == 0) ? LX[i] : (a == 1) ? LY[i] : LZ[i];
-    left[part] = (i < mid) ? 1 : 0;
-}
-
-// Number of "left" flags inside a subtree of `s` members that is `r` levels above the level being split: after r
-// balanced halvings (T-2) the parts have q+1 (m of them) or q members, q = s >> r, m = s - (q << r); a part of size
-// c sends ceil(c/2) members left.
-__host__ __device__ __forceinline__ int kd_lefts(int s, int r)
-{
-    int q = s >> r, m = s - (q << r);
-    return m * ((q + 2) >> 1) + ((1 << r) - m) * ((q + 1) >> 1);
-}
-
-// position i of a list -> its node [lo, hi) at `level` and the number of left flags in the nodes before it
-__device__ __forceinline__ void kd_node_of(int N, int level, int i, int &lo, int &hi, int &lefts_before)
-{
-    lo = 0;
-    hi = N;
-    lefts_before = 0;
-    for (int l = 0; l < level; ++l) {
-        int mid = lo + (hi - lo + 1) / 2;
-        if (i < mid) {
-            hi = mid;
-        } else {
-            lefts_before += kd_lefts(mid - lo, level - l - 1);
-            lo = mid;
-        }
-    }
-}
-
-#define KD_TILE_ITEMS 8
-#define KD_TILE (256 * KD_TILE_ITEMS)
-
-// left flags of the four lists, counted per tile of KD_TILE consecutive entries (no flag array is stored)
-__global__ void __launch_bounds__(256) kd_tile_counts(int64_t n4, const uint8_t *__restrict__ left, const uint32_t *__restrict__ lists,
-                                                      int32_t *__restrict__ sums)
-{
-    __shared__ int sm[8];
-    int64_t base = (int64_t)blockIdx.x * KD_TILE + (int64_t)threadIdx.x * KD_TILE_ITEMS;
-    int s = 0;
-#pragma unroll
-    for (int k = 0; k < KD_TILE_ITEMS; ++k)
-        if (base + k < n4) s += left[lists[base + k]];
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) s += __shfl_down_sync(0xffffffffu, s, o);
-    if ((threadIdx.x & 31) == 0) sm[threadIdx.x >> 5] = s;
-    __syncthreads();
-    if (threadIdx.x == 0) {
-        int t = 0;
-        for (int k = 0; k < 8; ++k) t += sm[k];
-        sums[blockIdx.x] = t;
-    }
-}
-
-// stable partition of every node segment of the four lists: left members first.  The number of left flags before
-// entry g is tile_base[tile] + the scan inside the tile; the number before the node's start is closed-form (kd_lefts).
-__global__ void __launch_bounds__(256) kd_partition(int N, int level, const uint8_t *__restrict__ left, const int32_t *__restrict__ tile_base,
-                                                    const uint32_t *__restrict__ lists, uint32_t *__restrict__ out)
-{
-    __shared__ int sm[8];
-    const int64_t n4 = 4ll * N;
-    const int64_t base = (int64_t)blockIdx.x * KD_TILE + (int64_t)threadIdx.x * KD_TILE_ITEMS;
-    uint32_t part[KD_TILE_ITEMS];
-    int flag[KD_TILE_ITEMS], s = 0;
-#pragma unroll
-    for (int k = 0; k < KD_TILE_ITEMS; ++k) {
-        part[k] = (base + k < n4) ? lists[base + k] : 0u;
-        flag[k] = (base + k < n4) ? (int)left[part[k]] : 0;
-        s += flag[k];
-    }
-    // exclusive scan of s over the block
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    int inc = s;
-#pragma unroll
-    for (int o = 1; o < 32; o <<= 1) {
-        int t = __shfl_up_sync(0xffffffffu, inc, o);
-        if (lane >= o) inc += t;
-    }
-    if (lane == 31) sm[warp] = inc;
-    __syncthreads();
-    int wbase = 0;
-    for (int k = 0; k < warp; ++k) wbase += sm[k];
-    int before = tile_base[blockIdx.x] + wbase + inc - s;  // left flags before entry `base`, over all four lists
-    const int lefts_per_list = kd_lefts(N, level);
-#pragma unroll
-    for (int k = 0; k < KD_TILE_ITEMS; ++k) {
-        const int64_t g = base + k;
-        if (g < n4) {
-            const int li = (int)(g / N), i = (int)(g - (int64_t)li * N);
-            int lo, hi, lb;
-            kd_node_of(N, level, i, lo, hi, lb);
-            const int mid = lo + (hi - lo + 1) / 2;
-            const int nleft_before = before - li * lefts_per_list - lb;  // within the node, before entry i
-            const int dest = flag[k] ? (lo + nleft_before) : (mid + (i - lo - nleft_before));
-            out[(int64_t)li * N + dest] = part[k];
-        }
-        before += flag[k];
-    }
 }
 
 // ---------------------------------------------------------------------------------------
@@ -547,63 +384,23 @@ int tree_build(fmm_plan *p, const fmm_particles_t *in)
     node_ranges_kernel<<<(unsigned)((p->nodes + T - 1) / T), T, 0, st>>>(N, p->kappa, (int)p->nodes, p->node_lo, p->node_hi);
     FMM_LAUNCH_CHECK(c, "node_ranges_kernel");
 
-    const int nsort = ((p->flags & FMM_TREE_MASK) == FMM_TREE_KD) ? 3 : 1;  // KD: the three axes are sorted in one batch
-    uint64_t *keys = (uint64_t *)ctx_alloc(c, sizeof(uint64_t) * N * nsort);
-    uint64_t *tkeys = (uint64_t *)ctx_alloc(c, sizeof(uint64_t) * N * nsort);
-    uint32_t *tvals = (uint32_t *)ctx_alloc(c, sizeof(uint32_t) * N * nsort);
-    uint32_t *lists = (uint32_t *)ctx_alloc(c, sizeof(uint32_t) * 4 * (size_t)N);  // LX, LY, LZ, LI
-    if (!keys || !tkeys || !tvals || !lists) return FMM_ENOMEM;
-    const uint32_t *order = NULL;
-
+    uint32_t *order = NULL;
     if ((p->flags & FMM_TREE_MASK) == FMM_TREE_KD) {
-        uint32_t *lists2 = (uint32_t *)ctx_alloc(c, sizeof(uint32_t) * 4 * (size_t)N);
-        const int ntiles = (int)((4ll * N + KD_TILE - 1) / KD_TILE);
-        int32_t *scan = (int32_t *)ctx_alloc(c, sizeof(int32_t) * (size_t)ntiles);  // left flags per tile, then their exclusive scan
-        uint8_t *left = (uint8_t *)ctx_alloc(c, (size_t)N);
-        int8_t *axis = (int8_t *)ctx_alloc(c, (size_t)((p->leaves > 1) ? p->leaves : 1));
-        if (!lists2 || !scan || !left || !axis) return FMM_ENOMEM;
-        if (p->kappa > 0) {
-            const double *coord[3] = {in->x, in->y, in->z};
-            for (int a = 0; a < 3; ++a) {
-                kd_make_keys<<<gN, T, 0, st>>>(N, coord[a], keys + (size_t)a * N, lists + (size_t)a * N);
-                FMM_LAUNCH_CHECK(c, "kd_make_keys");
-            }
-            FMM_TRY(sort_pairs_u64_batched(c, keys, lists, tkeys, tvals, N, 3, 0, 64));
-        }
-        kd_iota<<<gN, T, 0, st>>>(N, lists + 3 * (size_t)N);
-        FMM_LAUNCH_CHECK(c, "kd_iota");
-        uint32_t *cur = lists, *nxt = lists2;
-        for (int level = 0; level < p->kappa; ++level) {
-            int nn = 1 << level;
-            kd_choose_axis<<<(nn + T - 1) / T, T, 0, st>>>(N, level, in->x, in->y, in->z, cur, cur + N, cur + 2 * (size_t)N,
-                                                           p->hdr, axis);
-            FMM_LAUNCH_CHECK(c, "kd_choose_axis");
-            kd_mark_left<<<gN, T, 0, st>>>(N, level, axis, cur, cur + N, cur + 2 * (size_t)N, left);
-            FMM_LAUNCH_CHECK(c, "kd_mark_left");
-            kd_tile_counts<<<ntiles, 256, 0, st>>>(4ll * N, left, cur, scan);
-            FMM_LAUNCH_CHECK(c, "kd_tile_counts");
-            FMM_TRY(scan_exclusive_i32(c, scan, scan, ntiles));
-            kd_partition<<<ntiles, 256, 0, st>>>(N, level, left, scan, cur, nxt);
-            FMM_LAUNCH_CHECK(c, "kd_partition");
-            uint32_t *t = cur; cur = nxt; nxt = t;
-        }
-        order = cur + 3 * (size_t)N;  // the index-ordered list: leaves in heap order, ascending index inside (T-3)
-        permute_particles<<<gN, T, 0, st>>>(N, order, in->x, in->y, in->z, in->px, in->py, in->pz, in->q, in->q_scalar,
-                                            p->perm, p->tx, p->ty, p->tz, p->w0, p->w1, p->w2, p->w3, p->pmx, p->pmy, p->pmz);
-        FMM_LAUNCH_CHECK(c, "permute_particles");
-        ctx_free(c, lists2); ctx_free(c, scan); ctx_free(c, left); ctx_free(c, axis);
+        FMM_TRY(kd_build_order(p, in, &order));  // kernels_kd.cu
     } else {
-        morton_keys<<<gN, T, 0, st>>>(N, in->x, in->y, in->z, p->hdr, keys, lists);
+        uint64_t *keys = (uint64_t *)ctx_alloc(c, sizeof(uint64_t) * N);
+        uint64_t *tkeys = (uint64_t *)ctx_alloc(c, sizeof(uint64_t) * N);
+        uint32_t *tvals = (uint32_t *)ctx_alloc(c, sizeof(uint32_t) * N);
+        order = (uint32_t *)ctx_alloc(c, sizeof(uint32_t) * (size_t)N);
+        if (!keys || !tkeys || !tvals || !order) return FMM_ENOMEM;
+        morton_keys<<<gN, T, 0, st>>>(N, in->x, in->y, in->z, p->hdr, keys, order);
         FMM_LAUNCH_CHECK(c, "morton_keys");
-        FMM_TRY(sort_pairs_u64(c, keys, lists, tkeys, tvals, N, 0, 64));
-        order = lists;
-        permute_particles<<<gN, T, 0, st>>>(N, order, in->x, in->y, in->z, in->px, in->py, in->pz, in->q, in->q_scalar,
-                                            p->perm, p->tx, p->ty, p->tz, p->w0, p->w1, p->w2, p->w3, p->pmx, p->pmy, p->pmz);
-        FMM_LAUNCH_CHECK(c, "permute_particles");
+        FMM_TRY(sort_pairs_u64(c, keys, order, tkeys, tvals, N, 0, 64));
     }
-    ctx_free(c, keys); ctx_free(c, tkeys); ctx_free(c, tvals); ctx_free(c, lists);
-
-    return tree_boxes(p);
+    permute_particles<<<gN, T, 0, st>>>(N, order, in->x, in->y, in->z, in->px, in->py, in->pz, in->q, in->q_scalar,
+                                        p->perm, p->tx, p->ty, p->tz, p->w0, p->w1, p->w2, p->w3, p->pmx, p->pmy, p->pmz);
+    FMM_LAUNCH_CHECK(c, "permute_particles");
+    return tree_boxes(p);  // (the scratch goes back with the arena of the build)
 }
 
 // a2 on the particles as they sit in tree order

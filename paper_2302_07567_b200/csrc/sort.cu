@@ -243,3 +243,135 @@ int sort_pairs_u64_batched(fmm_ctx *c, uint64_t *keys, uint32_t *vals, uint64_t 
     ctx_free(c, table);
     return FMM_OK;
 }
+
+// ----------------------------------------------------------------------------------------
+// radix sort of (u32 key, u32 value) pairs, 8 bits per pass, for the KD build (quantised coordinates).  Same ranking
+// as above (stable); the scatter first reorders the tile in shared memory so that the keys of one digit leave the
+// block as one contiguous run (coalesced stores instead of one sector per key).
+// ----------------------------------------------------------------------------------------
+#define RS32_ROUNDS 16
+#define RS32_TILE (RS_THREADS * RS32_ROUNDS)  // 4096 keys per block
+
+__global__ void __launch_bounds__(RS_THREADS) rs32_histogram(const uint32_t *__restrict__ keys, int64_t n, int shift,
+                                                             int32_t *__restrict__ table, int nblocks)
+{
+    __shared__ int cnt[RS_RADIX];
+    cnt[threadIdx.x] = 0;
+    __syncthreads();
+    keys += (int64_t)blockIdx.y * n;
+    table += (int64_t)blockIdx.y * RS_RADIX * nblocks;
+    const int64_t base = (int64_t)blockIdx.x * RS32_TILE;
+#pragma unroll
+    for (int r = 0; r < RS32_ROUNDS; ++r) {
+        const int64_t i = base + (int64_t)r * RS_THREADS + threadIdx.x;
+        if (i < n) atomicAdd(&cnt[(keys[i] >> shift) & 0xffu], 1);
+    }
+    __syncthreads();
+    table[(int64_t)threadIdx.x * nblocks + blockIdx.x] = cnt[threadIdx.x];
+}
+
+__global__ void __launch_bounds__(RS_THREADS) rs32_scatter(const uint32_t *__restrict__ keys, const uint32_t *__restrict__ vals,
+                                                           uint32_t *__restrict__ okeys, uint32_t *__restrict__ ovals, int64_t n, int shift,
+                                                           const int32_t *__restrict__ table, int nblocks)
+{
+    __shared__ int cnt[RS_WARPS][RS_RADIX];  // per-warp running digit counts, then per-warp bases inside the tile
+    __shared__ int dbase[RS_RADIX];          // first tile position of a digit
+    __shared__ int gbase[RS_RADIX];          // global position of a digit's first key of this block
+    __shared__ uint32_t skey[RS32_TILE], sval[RS32_TILE];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    for (int k = threadIdx.x; k < RS_WARPS * RS_RADIX; k += RS_THREADS) (&cnt[0][0])[k] = 0;
+    __syncthreads();
+    const int64_t seg = (int64_t)blockIdx.y * n;
+    keys += seg; okeys += seg; vals += seg; ovals += seg;
+    table += (int64_t)blockIdx.y * RS_RADIX * nblocks;
+    const int64_t tile0 = (int64_t)blockIdx.x * RS32_TILE;
+    const int64_t wbase = tile0 + (int64_t)warp * (RS32_TILE / RS_WARPS);
+    const int live = (int)((n - tile0 < RS32_TILE) ? (n - tile0) : RS32_TILE);
+    uint32_t key[RS32_ROUNDS];
+    int rank[RS32_ROUNDS];
+    const unsigned lt = (1u << lane) - 1u;
+#pragma unroll
+    for (int r = 0; r < RS32_ROUNDS; ++r) {  // warp w walks its contiguous chunk in rounds of 32: (warp, round, lane) order == input order
+        const int64_t i = wbase + r * 32 + lane;
+        const bool ok = i < n;
+        key[r] = ok ? keys[i] : 0xffffffffu;
+        const int d = ok ? (int)((key[r] >> shift) & 0xffu) : 256;  // 256: out of range, matches only other tails
+        const unsigned m = __match_any_sync(0xffffffffu, d);
+        const int leader = __ffs(m) - 1;
+        int prior = 0;
+        if (ok && lane == leader) {
+            prior = cnt[warp][d];
+            cnt[warp][d] = prior + __popc(m);
+        }
+        prior = __shfl_sync(0xffffffffu, prior, leader);
+        rank[r] = prior + __popc(m & lt);
+        __syncwarp();
+    }
+    __syncthreads();
+    {  // digit d = threadIdx.x: exclusive prefix over warps, then over digits
+        const int d = threadIdx.x;
+        int run = 0;
+#pragma unroll
+        for (int w = 0; w < RS_WARPS; ++w) {
+            const int t = cnt[w][d];
+            cnt[w][d] = run;
+            run += t;
+        }
+        // exclusive scan of the digit totals over the block (256 threads)
+        int inc = run;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const int t = __shfl_up_sync(0xffffffffu, inc, o);
+            if (lane >= o) inc += t;
+        }
+        __shared__ int wsum[RS_WARPS];
+        if (lane == 31) wsum[warp] = inc;
+        __syncthreads();
+        int wb = 0;
+        for (int w = 0; w < warp; ++w) wb += wsum[w];
+        dbase[d] = wb + inc - run;
+        gbase[d] = table[(int64_t)d * nblocks + blockIdx.x] - (int)seg;
+    }
+    __syncthreads();
+#pragma unroll
+    for (int r = 0; r < RS32_ROUNDS; ++r) {
+        const int64_t i = wbase + r * 32 + lane;
+        if (i < n) {
+            const int d = (int)((key[r] >> shift) & 0xffu);
+            const int pos = dbase[d] + cnt[warp][d] + rank[r];
+            skey[pos] = key[r];
+            sval[pos] = vals[i];
+        }
+    }
+    __syncthreads();
+    for (int q = threadIdx.x; q < live; q += RS_THREADS) {
+        const uint32_t k = skey[q];
+        const int d = (int)((k >> shift) & 0xffu);
+        const int64_t pos = (int64_t)gbase[d] + (q - dbase[d]);
+        okeys[pos] = k;
+        ovals[pos] = sval[q];
+    }
+}
+
+// `batch` independent sorts of length n laid out back to back on all 32 key bits; the result ends in keys / vals
+int sort_pairs_u32_batched(fmm_ctx *c, uint32_t *keys, uint32_t *vals, uint32_t *tmp_keys, uint32_t *tmp_vals, int64_t n, int batch)
+{
+    if (n <= 1 || batch < 1) return FMM_OK;
+    if (n * batch >= (int64_t)1 << 31) return FMM_EOVERFLOW;
+    const int nblocks = (int)((n + RS32_TILE - 1) / RS32_TILE);
+    const int64_t tlen = (int64_t)RS_RADIX * nblocks * batch;
+    int32_t *table = (int32_t *)ctx_alloc(c, sizeof(int32_t) * tlen);
+    if (!table) return FMM_ENOMEM;
+    uint32_t *ki = keys, *ko = tmp_keys, *vi = vals, *vo = tmp_vals;
+    for (int shift = 0; shift < 32; shift += 8) {  // (an even number of passes: the result is back in keys / vals)
+        rs32_histogram<<<dim3(nblocks, batch), RS_THREADS, 0, c->stream>>>(ki, n, shift, table, nblocks);
+        FMM_LAUNCH_CHECK(c, "rs32_histogram");
+        FMM_TRY(scan_exclusive_i32(c, table, table, tlen));
+        rs32_scatter<<<dim3(nblocks, batch), RS_THREADS, 0, c->stream>>>(ki, vi, ko, vo, n, shift, table, nblocks);
+        FMM_LAUNCH_CHECK(c, "rs32_scatter");
+        uint32_t *tk = ki; ki = ko; ko = tk;
+        uint32_t *tv = vi; vi = vo; vo = tv;
+    }
+    ctx_free(c, table);
+    return FMM_OK;
+}

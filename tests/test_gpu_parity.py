@@ -466,3 +466,36 @@ def test_plan_on_one_stream_evaluated_under_another(fmm):
     assert np.array_equal(E2.cpu().numpy().T, Eref)
     assert np.array_equal(to_np((E, B))[1], Bref)
     plan.close()
+
+
+@pytest.mark.parametrize("kind", ["short_runs", "long_run", "all_equal_axis", "duplicates"])
+def test_kd_sort_key_ties(fmm, kind):
+    """The KD build sorts by a 32-bit quantisation of the coordinates and repairs runs of equal keys afterwards
+    (kernels_kd.cu): runs of up to 64 entries in place, longer ones by a rebuild with exact keys.  The particle order must be
+    the oracle's (coordinate, index) order in every case."""
+    rng = np.random.default_rng(42)
+    N = 6000
+    y = rng.normal(0, 1e-3, N)
+    z = rng.normal(0, 1e-4, N)
+    if kind == "short_runs":      # 300 clusters of 20 points 1e-13 apart: 20 entries per sort key, out of order
+        x = np.repeat(rng.uniform(-1, 1, 300), 20) + 1e-13 * rng.standard_normal(N)
+    elif kind == "long_run":      # one tight cluster and two far outliers: thousands of entries per sort key
+        x = 1e-9 * rng.random(N)
+        x[7], x[4000] = -1e3, 1e3
+    elif kind == "all_equal_axis":
+        x = np.full(N, 0.25)
+    else:                          # exact duplicates: ties go to the index
+        x = np.repeat(rng.uniform(-1, 1, N // 4), 4)
+        rng.shuffle(x)
+    px, py, pz = np.zeros(N), np.zeros(N), np.full(N, 5.0)
+    plan = fmm.fmm_plan_create(x, y, z, px, py, pz, 1.0, order_n=2, leaf_size=40, theta=0.5)
+    st = plan.stats()
+    ex = plan.export()
+    op = oracle.Plan(x, y, z, px, py, pz, 1.0, order_n=2, leaf_size=40, theta=0.5, gamma_bar_value=st["gamma_bar"])
+    assert np.array_equal(ex["perm"], op.perm()), "permutation differs"
+    _, _, bb = op.node_arrays()
+    assert np.array_equal(ex["bbox"].view(np.uint64), bb.view(np.uint64))
+    E, B = to_np(plan.eval())
+    Eo, Bo = op.eval()
+    assert_close(E, Eo, "E")
+    plan.close()
