@@ -153,14 +153,20 @@ __global__ void __launch_bounds__(256) kd_mark(int N, int level, const double *_
                                                const fmm_hdr *__restrict__ hdr, uint32_t *__restrict__ bits)
 {
     __shared__ int s_lo[2], s_hi[2], s_axis[2];
+    __shared__ double s_ext[2][6];
     const int start = blockIdx.x * KD_TILE, end = min(N, start + KD_TILE);
-    if (threadIdx.x < 2) {
+    if (threadIdx.x < 12) {  // the (at most two) nodes of this tile: six segment ends each, fetched by twelve threads at once
+        const int k = threadIdx.x / 6, e = threadIdx.x - 6 * k, a = e >> 1;
         int lo, hi;
-        kd_range_of(N, level, threadIdx.x == 0 ? start : end - 1, lo, hi);
-        const uint32_t *LX = lists, *LY = lists + N, *LZ = lists + 2 * (size_t)N;
-        s_lo[threadIdx.x] = lo;
-        s_hi[threadIdx.x] = hi;
-        s_axis[threadIdx.x] = kd_axis(hdr->gamma_bar, x[LX[lo]], x[LX[hi - 1]], y[LY[lo]], y[LY[hi - 1]], z[LZ[lo]], z[LZ[hi - 1]]);
+        kd_range_of(N, level, k == 0 ? start : end - 1, lo, hi);
+        const double *coord = (a == 0) ? x : (a == 1) ? y : z;
+        s_ext[k][e] = coord[lists[(size_t)a * N + ((e & 1) ? hi - 1 : lo)]];
+        if (e == 0) { s_lo[k] = lo; s_hi[k] = hi; }
+    }
+    __syncthreads();
+    if (threadIdx.x < 2) {
+        const double *v = s_ext[threadIdx.x];
+        s_axis[threadIdx.x] = kd_axis(hdr->gamma_bar, v[0], v[1], v[2], v[3], v[4], v[5]);
     }
     __syncthreads();
     for (int i = start + threadIdx.x; i < end; i += 256) {
@@ -197,18 +203,16 @@ __device__ __forceinline__ int kd_block_scan_256(int v, int *total, int *sm /* [
     return wb + inc - v;
 }
 
-// stable split of every node segment of the four lists: left members first.  Tiles are taken in ticket order, publish the
-// number of left members of their last node, and a tile whose first node began earlier adds up the tiles before it.
-__global__ void __launch_bounds__(256) kd_split(int N, int level, int tiles_per_list, const uint32_t *__restrict__ bits,
-                                                const uint32_t *__restrict__ cur, uint32_t *__restrict__ nxt,
-                                                unsigned int *pub /* [4 tiles_per_list] */, unsigned int *ticket)
+// stable split of every node segment of the four lists: left members first.  A tile publishes the number of left members
+// of its last node, and a tile whose first node began earlier adds up the tiles before it.
+__global__ void __launch_bounds__(256, 6) kd_split(int N, int level, int tiles_per_list, const uint32_t *__restrict__ bits,
+                                                   const uint32_t *__restrict__ cur, uint32_t *__restrict__ nxt,
+                                                   unsigned int *pub /* [4 tiles_per_list] */)
 {
     __shared__ int sm[8];
-    __shared__ unsigned int s_tile;
-    if (threadIdx.x == 0) s_tile = atomicAdd(ticket, 1u);
-    __syncthreads();
-    const int tile = (int)s_tile;
-    const int li = tile / tiles_per_list, t = tile - li * tiles_per_list;
+    // tile = block index: a tile only waits for tiles with smaller indices, and blocks of a 1-D grid start in index
+    // order, so the tiles it waits for are running or done (the assumption of every single-pass look-back scan)
+    const int li = blockIdx.y, t = blockIdx.x, tile = li * tiles_per_list + t;
     const int start = t * KD_TILE, end = min(N, start + KD_TILE);
     int loA, hiA, hiB;
     kd_range_of(N, level, start, loA, hiA);
@@ -232,14 +236,11 @@ __global__ void __launch_bounds__(256) kd_split(int N, int level, int tiles_per_
         s += (int)f;
         sA += (int)(f && i < hiA);
     }
-    int total, cA;
-    const int ex = kd_block_scan_256(s, &total, sm);
-    kd_block_scan_256(sA, &cA, sm);
+    int both;  // one scan for both counts: left members in the low half, those of node A in the high half (each <= 2048)
+    const int ex = kd_block_scan_256(s | (sA << 16), &both, sm) & 0xffff;
+    const int total = both & 0xffff, cA = both >> 16;
     const unsigned int tag = (unsigned int)(level + 1) << 16;
-    if (threadIdx.x == 0) {
-        __threadfence();
-        atomicExch(&pub[tile], tag | (unsigned int)((hiA < end) ? total - cA : total));
-    }
+    if (threadIdx.x == 0) atomicExch(&pub[tile], tag | (unsigned int)((hiA < end) ? total - cA : total));
     // left members of node A in the tiles before this one
     int carry = 0;
     if (loA < start) {
@@ -274,7 +275,7 @@ __global__ void __launch_bounds__(256) kd_split(int N, int level, int tiles_per_
 // The node's members are renamed 0 .. m-1 by ascending original index (their order in LI); the three sorted lists and LI
 // become arrays of 16-bit local names in shared memory, the left flags a byte array.  Output: the node's part of the
 // final particle order (leaves in heap order, ascending index inside, reading T-3).
-struct kdl_smem {
+struct __align__(16) kdl_smem {
     uint32_t ids[KD_LOCAL];          // local name -> particle
     uint16_t L[2][4][KD_LOCAL];      // ping-pong: LX, LY, LZ, LI in local names
     uint16_t F[KD_LOCAL + 8];        // exclusive scan of the flags along one list
@@ -321,7 +322,8 @@ __device__ __forceinline__ void kdl_sub_of(int lo, int hi, int depth, int pos, i
 
 __global__ void __launch_bounds__(KDL_THREADS) kd_local(int N, int level0, int kappa, const double *__restrict__ x, const double *__restrict__ y,
                                                         const double *__restrict__ z, const fmm_hdr *__restrict__ hdr,
-                                                        const uint32_t *__restrict__ lists, uint32_t *__restrict__ order)
+                                                        const uint32_t *__restrict__ lists, uint16_t *names /* [N] scratch */,
+                                                        uint32_t *__restrict__ order)
 {
     extern __shared__ __align__(16) unsigned char kdl_raw[];
     kdl_smem &S = *reinterpret_cast<kdl_smem *>(kdl_raw);
@@ -333,20 +335,18 @@ __global__ void __launch_bounds__(KDL_THREADS) kd_local(int N, int level0, int k
     const int m = hi - lo;
     if (m <= 0) return;
     const double gamma_bar = hdr->gamma_bar;
+    // local name of a particle = its rank in the node's (ascending) part of LI; the map particle -> name goes through a
+    // global scratch array (written and read by this block only; read past L1, which may hold a neighbour's stale line)
     for (int r = threadIdx.x; r < m; r += KDL_THREADS) {
-        S.ids[r] = lists[3 * (size_t)N + lo + r];
+        const uint32_t p = lists[3 * (size_t)N + lo + r];
+        S.ids[r] = p;
         S.L[0][3][r] = (uint16_t)r;
+        names[p] = (uint16_t)r;
     }
     __syncthreads();
-    for (int q = threadIdx.x; q < 3 * m; q += KDL_THREADS) {  // local name of a particle = its rank in the (ascending) ids
+    for (int q = threadIdx.x; q < 3 * m; q += KDL_THREADS) {
         const int a = q / m, i = q - a * m;
-        const uint32_t p = lists[(size_t)a * N + lo + i];
-        int b0 = 0, b1 = m;
-        while (b0 < b1) {
-            const int mid = (b0 + b1) >> 1;
-            if (S.ids[mid] < p) b0 = mid + 1; else b1 = mid;
-        }
-        S.L[0][a][i] = (uint16_t)b0;
+        S.L[0][a][i] = __ldcg(&names[lists[(size_t)a * N + lo + i]]);
     }
     __syncthreads();
     int cb = 0;
@@ -373,27 +373,37 @@ __global__ void __launch_bounds__(KDL_THREADS) kd_local(int N, int level0, int k
         // this thread's positions: KDL_ITEMS consecutive entries; their sub-nodes are the same in all four lists
         const int i0 = threadIdx.x * KDL_ITEMS;
         int slo[KDL_ITEMS], smid[KDL_ITEMS];
+        {
+            union { uint4 v; uint16_t h[KDL_ITEMS]; } n3[3];  // the thread's entries of LX, LY, LZ (three LDS.128)
 #pragma unroll
-        for (int k = 0; k < KDL_ITEMS; ++k) {
-            const int i = i0 + k;
-            slo[k] = smid[k] = 0;
-            if (i < m) {
-                int a, b, sk;
-                kdl_sub_of(lo, hi, depth, lo + i, a, b, sk);
-                slo[k] = a - lo;
-                smid[k] = a - lo + (b - a + 1) / 2;
-                S.flag[Lc[S.axis[sk]][i]] = (uint8_t)(i < smid[k]);  // Alg 5.2: the first ceil(size/2) along the split axis go left
+            for (int a = 0; a < 3; ++a) n3[a].v = *reinterpret_cast<const uint4 *>(&Lc[a][i0]);
+#pragma unroll
+            for (int k = 0; k < KDL_ITEMS; ++k) {
+                const int i = i0 + k;
+                slo[k] = smid[k] = 0;
+                if (i < m) {
+                    int a, b, sk;
+                    kdl_sub_of(lo, hi, depth, lo + i, a, b, sk);
+                    slo[k] = a - lo;
+                    smid[k] = a - lo + (b - a + 1) / 2;
+                    const int ax = S.axis[sk];
+                    const uint16_t name = (ax == 0) ? n3[0].h[k] : (ax == 1) ? n3[1].h[k] : n3[2].h[k];
+                    S.flag[name] = (uint8_t)(i < smid[k]);  // Alg 5.2: the first ceil(size/2) along the split axis go left
+                }
             }
         }
         __syncthreads();
         for (int a = 0; a < 4; ++a) {
+            // the thread's KDL_ITEMS = 8 consecutive 16-bit names are one 16-byte word: LDS.128 / STS.128 without bank conflicts
+            union { uint4 v; uint16_t h[KDL_ITEMS]; } rr, ff;
+            rr.v = *reinterpret_cast<const uint4 *>(&Lc[a][i0]);
             uint16_t r[KDL_ITEMS];
             unsigned int fl = 0;
             int s = 0;
 #pragma unroll
             for (int k = 0; k < KDL_ITEMS; ++k) {
                 const int i = i0 + k;
-                r[k] = (i < m) ? Lc[a][i] : (uint16_t)0;
+                r[k] = (i < m) ? rr.h[k] : (uint16_t)0;
                 const unsigned int f = (i < m) ? S.flag[r[k]] : 0u;
                 fl |= f << k;
                 s += (int)f;
@@ -402,15 +412,16 @@ __global__ void __launch_bounds__(KDL_THREADS) kd_local(int N, int level0, int k
             int run = kdl_block_scan(s, &total, S.scan);
 #pragma unroll
             for (int k = 0; k < KDL_ITEMS; ++k) {
-                if (i0 + k < m) S.F[i0 + k] = (uint16_t)run;
+                ff.h[k] = (uint16_t)run;
                 run += (int)((fl >> k) & 1u);
             }
+            *reinterpret_cast<uint4 *>(&S.F[i0]) = ff.v;  // (entries beyond m are never read)
             __syncthreads();
 #pragma unroll
             for (int k = 0; k < KDL_ITEMS; ++k) {
                 const int i = i0 + k;
                 if (i < m) {
-                    const int before = (int)S.F[i] - (int)S.F[slo[k]];  // left members of the sub-node before entry i
+                    const int before = (int)ff.h[k] - (int)S.F[slo[k]];  // left members of the sub-node before entry i
                     const unsigned int f = (fl >> k) & 1u;
                     Ln[a][f ? (slo[k] + before) : (smid[k] + (i - slo[k] - before))] = r[k];
                 }
@@ -478,15 +489,14 @@ int kd_build_order(fmm_plan *p, const fmm_particles_t *in, uint32_t **order_out)
         const int tiles = (N + KD_TILE - 1) / KD_TILE;
         const size_t nbits = ((size_t)N + 31) / 32;
         uint32_t *bits = (uint32_t *)ctx_alloc(c, sizeof(uint32_t) * nbits);
-        unsigned int *pub = (unsigned int *)ctx_alloc(c, sizeof(unsigned int) * (4 * (size_t)tiles + 64));
+        unsigned int *pub = (unsigned int *)ctx_alloc(c, sizeof(unsigned int) * 4 * (size_t)tiles);
         if (!bits || !pub) return FMM_ENOMEM;
-        unsigned int *ticket = pub + 4 * (size_t)tiles;  // one counter per level
-        FMM_CUDA(c, cudaMemsetAsync(pub, 0, sizeof(unsigned int) * (4 * (size_t)tiles + 64), st));
+        FMM_CUDA(c, cudaMemsetAsync(pub, 0, sizeof(unsigned int) * 4 * (size_t)tiles, st));
         for (int level = 0; level < level0; ++level) {
             FMM_CUDA(c, cudaMemsetAsync(bits, 0, sizeof(uint32_t) * nbits, st));
             kd_mark<<<tiles, 256, 0, st>>>(N, level, in->x, in->y, in->z, cur, p->hdr, bits);
             FMM_LAUNCH_CHECK(c, "kd_mark");
-            kd_split<<<4 * tiles, 256, 0, st>>>(N, level, tiles, bits, cur, nxt, pub, ticket + level);
+            kd_split<<<dim3(tiles, 4), 256, 0, st>>>(N, level, tiles, bits, cur, nxt, pub);
             FMM_LAUNCH_CHECK(c, "kd_split");
             uint32_t *t = cur; cur = nxt; nxt = t;
         }
@@ -495,8 +505,9 @@ int kd_build_order(fmm_plan *p, const fmm_particles_t *in, uint32_t **order_out)
     if (level0 < p->kappa) {
         const size_t smem = sizeof(kdl_smem);
         FMM_CUDA(c, cudaFuncSetAttribute((const void *)kd_local, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        uint32_t *order = nxt;  // (the other list buffer is free now)
-        kd_local<<<1u << level0, KDL_THREADS, smem, st>>>(N, level0, p->kappa, in->x, in->y, in->z, p->hdr, cur, order);
+        uint32_t *order = nxt;  // (the other list buffer is free now: [0, N) takes the order, the rest the name map)
+        uint16_t *names = reinterpret_cast<uint16_t *>(nxt + (size_t)N);
+        kd_local<<<1u << level0, KDL_THREADS, smem, st>>>(N, level0, p->kappa, in->x, in->y, in->z, p->hdr, cur, names, order);
         FMM_LAUNCH_CHECK(c, "kd_local");
         *order_out = order;
     } else {

@@ -332,44 +332,60 @@ __global__ void leaf_bbox(int leaves, const int32_t *__restrict__ node_lo, const
     }
 }
 
-// one block: parents = union of the non-empty children, level by level upward; then the stretched
-// squared radius (Alg 5.6) and the box centre (Alg 5.7) of every node, each
-// product and sum rounded separately (reading D-2) so that the traversal is bit-reproducible.
-__global__ void __launch_bounds__(1024) upper_bbox_and_geometry(int kappa, int nodes, const int32_t *__restrict__ node_lo,
-                                                                const int32_t *__restrict__ node_hi, const fmm_hdr *__restrict__ hdr,
-                                                                double *__restrict__ bbox, double *__restrict__ geo)
+// Parents = union of the non-empty children (an empty cluster has a zero box and takes part in nothing).  One warp takes
+// 32 consecutive nodes of level `lc` and forms their ancestors on up to five levels with shuffles (min / max are exact and
+// order-free), so the whole upward pass is ceil(kappa / 5) small launches instead of kappa block barriers.
+__global__ void __launch_bounds__(256) bbox_up_warp(int lc, int steps, const int32_t *__restrict__ node_lo, const int32_t *__restrict__ node_hi,
+                                                    double *__restrict__ bbox)
 {
-    const double gamma_bar = hdr->gamma_bar;
-    for (int level = kappa - 1; level >= 0; --level) {
-        int first = 1 << level;
-        for (int i = first + threadIdx.x; i < 2 * first; i += blockDim.x) {
-            int c0 = 2 * i, c1 = 2 * i + 1;
-            bool e0 = node_hi[c0] <= node_lo[c0], e1 = node_hi[c1] <= node_lo[c1];
-            double *bb = bbox + 6 * (int64_t)i;
-            const double *b0 = bbox + 6 * (int64_t)c0, *b1 = bbox + 6 * (int64_t)c1;
-            for (int k = 0; k < 3; ++k) {
-                double lo, hi;
-                if (e0 && e1) { lo = 0.0; hi = 0.0; }
-                else if (e1) { lo = b0[k]; hi = b0[3 + k]; }
-                else if (e0) { lo = b1[k]; hi = b1[3 + k]; }
-                else { lo = fmin(b0[k], b1[k]); hi = fmax(b0[3 + k], b1[3 + k]); }
-                bb[k] = lo;
-                bb[3 + k] = hi;
+    const int w = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
+    const int first = 1 << lc, count = 1 << lc;
+    const int k = w * 32 + lane;
+    if (w * 32 >= count) return;
+    const bool live = k < count;
+    const int node = first + (live ? k : 0);
+    bool empty = !live || node_hi[node] <= node_lo[node];
+    double b[6];
+#pragma unroll
+    for (int q = 0; q < 6; ++q) b[q] = empty ? 0.0 : bbox[6 * (int64_t)node + q];
+    for (int s = 1; s <= steps; ++s) {
+        const int o = 1 << (s - 1);
+        const bool e2 = __shfl_down_sync(0xffffffffu, empty, o);
+        double c[6];
+#pragma unroll
+        for (int q = 0; q < 6; ++q) c[q] = __shfl_down_sync(0xffffffffu, b[q], o);
+        if ((lane & ((1 << s) - 1)) == 0) {  // this lane holds the left child, lane + o the right one
+#pragma unroll
+            for (int q = 0; q < 3; ++q) {
+                b[q] = empty ? c[q] : (e2 ? b[q] : fmin(b[q], c[q]));
+                b[3 + q] = empty ? c[3 + q] : (e2 ? b[3 + q] : fmax(b[3 + q], c[3 + q]));
+            }
+            empty = empty && e2;
+            if (live) {
+                double *bb = bbox + 6 * (int64_t)(node >> s);
+#pragma unroll
+                for (int q = 0; q < 6; ++q) bb[q] = empty ? 0.0 : b[q];
             }
         }
-        __syncthreads();
     }
-    for (int i = 1 + threadIdx.x; i <= nodes; i += blockDim.x) {
-        const double *bb = bbox + 6 * (int64_t)i;
-        double hx = __dmul_rn(__dsub_rn(bb[3], bb[0]), 0.5), hy = __dmul_rn(__dsub_rn(bb[4], bb[1]), 0.5),
-               hz = __dmul_rn(__dsub_rn(bb[5], bb[2]), 0.5);
-        double ex = __dmul_rn(1.0, hx), ey = __dmul_rn(1.0, hy), ez = __dmul_rn(gamma_bar, hz);
-        double *g = geo + 4 * (int64_t)i;
-        g[0] = __dadd_rn(__dadd_rn(__dmul_rn(ex, ex), __dmul_rn(ey, ey)), __dmul_rn(ez, ez));
-        g[1] = __dmul_rn(__dadd_rn(bb[0], bb[3]), 0.5);
-        g[2] = __dmul_rn(__dadd_rn(bb[1], bb[4]), 0.5);
-        g[3] = __dmul_rn(__dadd_rn(bb[2], bb[5]), 0.5);
-    }
+}
+
+// the stretched squared radius (Alg 5.6) and the box centre (Alg 5.7) of every node, each product
+// and sum rounded separately (reading D-2) so that the traversal is bit-reproducible
+__global__ void node_geometry(int nodes, const fmm_hdr *__restrict__ hdr, const double *__restrict__ bbox, double *__restrict__ geo)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x + 1;
+    if (i > nodes) return;
+    const double gamma_bar = hdr->gamma_bar;
+    const double *bb = bbox + 6 * (int64_t)i;
+    double hx = __dmul_rn(__dsub_rn(bb[3], bb[0]), 0.5), hy = __dmul_rn(__dsub_rn(bb[4], bb[1]), 0.5),
+           hz = __dmul_rn(__dsub_rn(bb[5], bb[2]), 0.5);
+    double ex = __dmul_rn(1.0, hx), ey = __dmul_rn(1.0, hy), ez = __dmul_rn(gamma_bar, hz);
+    double *g = geo + 4 * (int64_t)i;
+    g[0] = __dadd_rn(__dadd_rn(__dmul_rn(ex, ex), __dmul_rn(ey, ey)), __dmul_rn(ez, ez));
+    g[1] = __dmul_rn(__dadd_rn(bb[0], bb[3]), 0.5);
+    g[2] = __dmul_rn(__dadd_rn(bb[1], bb[4]), 0.5);
+    g[3] = __dmul_rn(__dadd_rn(bb[2], bb[5]), 0.5);
 }
 
 // ---------------------------------------------------------------------------------------
@@ -410,8 +426,14 @@ int tree_boxes(fmm_plan *p)
     const int T = 256;
     leaf_bbox<<<(unsigned)((p->leaves * 32 + T - 1) / T), T, 0, c->stream>>>((int)p->leaves, p->node_lo, p->node_hi, p->tx, p->ty, p->tz, p->bbox);
     FMM_LAUNCH_CHECK(c, "leaf_bbox");
-    upper_bbox_and_geometry<<<1, 1024, 0, c->stream>>>(p->kappa, (int)p->nodes, p->node_lo, p->node_hi, p->hdr, p->bbox, p->node_geo);
-    FMM_LAUNCH_CHECK(c, "upper_bbox_and_geometry");
+    for (int lc = p->kappa; lc > 0; lc -= 5) {
+        const int steps = lc < 5 ? lc : 5;
+        const int64_t threads = (int64_t)1 << lc;
+        bbox_up_warp<<<(unsigned)((threads + T - 1) / T), T, 0, c->stream>>>(lc, steps, p->node_lo, p->node_hi, p->bbox);
+        FMM_LAUNCH_CHECK(c, "bbox_up_warp");
+    }
+    node_geometry<<<(unsigned)((p->nodes + T - 1) / T), T, 0, c->stream>>>((int)p->nodes, p->hdr, p->bbox, p->node_geo);
+    FMM_LAUNCH_CHECK(c, "node_geometry");
     return FMM_OK;
 }
 

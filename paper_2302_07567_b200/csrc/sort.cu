@@ -125,6 +125,21 @@ int scan_exclusive_i32(fmm_ctx *c, const int32_t *in, int32_t *out, int64_t n) {
 // ----------------------------------------------------------------------------------------
 #define RS_THREADS 256
 #define RS_WARPS 8
+
+// lanes of the warp whose 8-bit digit equals this lane's (dead lanes match only dead lanes).  Eight ballots instead of
+// MATCH.ANY: the match instruction walks the distinct values of the warp one by one (about 300 cycles per call with
+// random digits, measured in profiles/r02_tree.md), the ballots are single-issue.
+__device__ __forceinline__ unsigned digit_peers(int d, bool ok)
+{
+    unsigned m = __ballot_sync(0xffffffffu, ok);
+    m = ok ? m : ~m;
+#pragma unroll
+    for (int b = 0; b < 8; ++b) {
+        const unsigned bal = __ballot_sync(0xffffffffu, (d >> b) & 1);
+        m &= ((d >> b) & 1) ? bal : ~bal;
+    }
+    return m;
+}
 #define RS_ROUNDS 8                       // keys per thread
 #define RS_TILE (RS_THREADS * RS_ROUNDS)  // 2048 keys per block
 #define RS_RADIX 256
@@ -172,8 +187,8 @@ __global__ void __launch_bounds__(RS_THREADS) rs_scatter(const uint64_t *__restr
         int64_t i = wbase + r * 32 + lane;
         bool ok = i < n;
         key[r] = ok ? keys[i] : ~0ull;
-        int d = ok ? (int)((key[r] >> shift) & 0xff) : 256;  // 256: out of range, matches only other tails
-        unsigned m = __match_any_sync(0xffffffffu, d);
+        int d = ok ? (int)((key[r] >> shift) & 0xff) : 0;
+        unsigned m = digit_peers(d, ok);
         int leader = __ffs(m) - 1;
         int prior = 0;
         if (ok && lane == leader) {
@@ -261,10 +276,16 @@ __global__ void __launch_bounds__(RS_THREADS) rs32_histogram(const uint32_t *__r
     keys += (int64_t)blockIdx.y * n;
     table += (int64_t)blockIdx.y * RS_RADIX * nblocks;
     const int64_t base = (int64_t)blockIdx.x * RS32_TILE;
+    uint32_t k[RS32_ROUNDS];
+#pragma unroll
+    for (int r = 0; r < RS32_ROUNDS; ++r) {  // all loads first: one memory round trip per thread
+        const int64_t i = base + (int64_t)r * RS_THREADS + threadIdx.x;
+        k[r] = (i < n) ? keys[i] : 0u;
+    }
 #pragma unroll
     for (int r = 0; r < RS32_ROUNDS; ++r) {
         const int64_t i = base + (int64_t)r * RS_THREADS + threadIdx.x;
-        if (i < n) atomicAdd(&cnt[(keys[i] >> shift) & 0xffu], 1);
+        if (i < n) atomicAdd(&cnt[(k[r] >> shift) & 0xffu], 1);
     }
     __syncthreads();
     table[(int64_t)threadIdx.x * nblocks + blockIdx.x] = cnt[threadIdx.x];
@@ -295,8 +316,8 @@ __global__ void __launch_bounds__(RS_THREADS) rs32_scatter(const uint32_t *__res
         const int64_t i = wbase + r * 32 + lane;
         const bool ok = i < n;
         key[r] = ok ? keys[i] : 0xffffffffu;
-        const int d = ok ? (int)((key[r] >> shift) & 0xffu) : 256;  // 256: out of range, matches only other tails
-        const unsigned m = __match_any_sync(0xffffffffu, d);
+        const int d = ok ? (int)((key[r] >> shift) & 0xffu) : 0;
+        const unsigned m = digit_peers(d, ok);
         const int leader = __ffs(m) - 1;
         int prior = 0;
         if (ok && lane == leader) {
