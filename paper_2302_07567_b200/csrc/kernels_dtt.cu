@@ -23,6 +23,7 @@ struct dtt_counters {           // device
 
 struct dtt_args {
     int nsteps, leaves, key_shift, treecode_leaves;
+    unsigned int roots;         // breadth-first until the frontier holds this many pairs, then one depth-first walk per pair
     double theta2;
     const fmm_hdr *hdr;
     const int32_t *node_lo, *node_hi;
@@ -35,7 +36,6 @@ struct dtt_args {
     dtt_counters *cnt;
 };
 
-#define DTT_ROOTS 4096   // breadth-first until the frontier holds this many pairs, then one depth-first walk per pair
 
 // one pair of Alg 9.1: 0 = nothing (empty cluster), 1 = P2P, 2 = M2L, 3 = split the target, 4 = split the source
 __device__ __forceinline__ int dtt_decide(const dtt_args &a, double gamma_bar, int i, int j, int *nj_out)
@@ -84,7 +84,7 @@ __device__ __forceinline__ void dtt_emit(const dtt_args &a, int kind, int i, int
 
 // Top of the traversal by ONE block (block barriers between the steps): resets the counters and the row lengths, seeds the
 // frontier -- FMM: (root, root); treecode (FMM_METHOD_TREECODE): (t, root) for every leaf t, so the target is never split
-// and the "m2l" list becomes the particle-cluster list -- and expands it breadth-first until it holds DTT_ROOTS pairs.
+// and the "m2l" list becomes the particle-cluster list -- and expands it breadth-first until it holds a.roots pairs.
 __global__ void __launch_bounds__(1024) dtt_top(dtt_args a)
 {
     __shared__ unsigned int n_in, n_out;
@@ -108,7 +108,7 @@ __global__ void __launch_bounds__(1024) dtt_top(dtt_args a)
         const double gamma_bar = a.hdr->gamma_bar;
         for (; step < a.nsteps; ++step) {
             const unsigned int nin = n_in;
-            if (nin == 0 || nin >= DTT_ROOTS || nin > a.cap) break;
+            if (nin == 0 || nin >= a.roots || nin > a.cap) break;
             const uint64_t *front_in = (step & 1) ? a.front1 : a.front0;
             uint64_t *front_out = (step & 1) ? a.front0 : a.front1;
             for (unsigned int k = tid; k < nin; k += nth) {
@@ -159,7 +159,12 @@ __global__ void __launch_bounds__(32 * DTT_WALK_WARPS) dtt_walk(dtt_args a, int 
     if (nroots == 0) return;
     const double gamma_bar = a.hdr->gamma_bar;
     const unsigned int lt = (1u << lane) - 1u;
-    for (unsigned int r = blockIdx.x * DTT_WALK_WARPS + warp; r < nroots; r += gridDim.x * DTT_WALK_WARPS) {
+    // the sub-trees differ a lot in size: warps take the next root from a counter instead of a fixed share
+    for (;;) {
+        unsigned int r = 0;
+        if (lane == 0) r = atomicAdd(&cnt->n_front[4 + pass], 1u);
+        r = __shfl_sync(0xffffffffu, r, 0);
+        if (r >= nroots) break;
         int top = 1;
         if (lane == 0) stk[0] = roots[r];
         __syncwarp();
@@ -447,12 +452,13 @@ int dtt_build_lists(fmm_plan *p)
         a.nsteps = nsteps; a.leaves = (int)p->leaves; a.key_shift = key_shift;
         a.treecode_leaves = (p->flags & FMM_METHOD_TREECODE) ? (int)p->leaves : 0;
         a.theta2 = p->theta * p->theta;
+        a.roots = (unsigned int)(p->leaves / 4 < 4096 ? 4096 : (p->leaves / 4 > 65536 ? 65536 : p->leaves / 4));
         a.hdr = p->hdr; a.node_lo = p->node_lo; a.node_hi = p->node_hi; a.geo = p->node_geo;
         a.front0 = f0; a.front1 = f1; a.p2p = kp2p; a.m2l = km2l; a.cap = (unsigned)cap;
         a.rows = rows; a.row_work = row_work; a.rows_len = rows_len; a.cnt = cnt;
         dtt_top<<<1, 1024, 0, st>>>(a);
         FMM_LAUNCH_CHECK(c, "dtt_top");
-        dtt_walk<<<DTT_ROOTS / DTT_WALK_WARPS, 32 * DTT_WALK_WARPS, 0, st>>>(a, 0);
+        dtt_walk<<<12 * FMM_SM_COUNT, 32 * DTT_WALK_WARPS, 0, st>>>(a, 0);
         FMM_LAUNCH_CHECK(c, "dtt_walk");
         dtt_walk<<<2 * FMM_SM_COUNT, 32 * DTT_WALK_WARPS, 0, st>>>(a, 1);  // (walks that spilled: normally none)
         FMM_LAUNCH_CHECK(c, "dtt_walk");

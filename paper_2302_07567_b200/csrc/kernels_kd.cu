@@ -23,14 +23,17 @@
 #define KDL_ITEMS 8      // KDL_THREADS x KDL_ITEMS = KD_LOCAL
 
 // node [lo, hi) at `level` that contains list position pos (T-2: the left child gets ceil(size / 2))
-__device__ __forceinline__ void kd_range_of(int N, int level, int pos, int &lo, int &hi)
+__device__ __forceinline__ int kd_range_of(int N, int level, int pos, int &lo, int &hi)  // returns the node's index in its level
 {
     lo = 0;
     hi = N;
+    int k = 0;
     for (int l = 0; l < level; ++l) {
         const int mid = lo + (hi - lo + 1) / 2;
-        if (pos < mid) hi = mid; else lo = mid;
+        k <<= 1;
+        if (pos < mid) hi = mid; else { lo = mid; k |= 1; }
     }
+    return k;
 }
 
 // Alg 5.1: split axis = first maximiser of s_k (b_k - a_k) (reading G9).  The lists are sorted by
@@ -150,23 +153,26 @@ __global__ void kd_fix_runs(int N, const double *__restrict__ x, const double *_
 // node (ranked by (coordinate, index)) go to the left child: their bits are set.
 __global__ void __launch_bounds__(256) kd_mark(int N, int level, const double *__restrict__ x, const double *__restrict__ y,
                                                const double *__restrict__ z, const uint32_t *__restrict__ lists,
-                                               const fmm_hdr *__restrict__ hdr, uint32_t *__restrict__ bits)
+                                               const fmm_hdr *__restrict__ hdr, uint32_t *__restrict__ bits,
+                                               uint8_t *__restrict__ node_axis /* [2^level] */)
 {
-    __shared__ int s_lo[2], s_hi[2], s_axis[2];
+    __shared__ int s_lo[2], s_hi[2], s_axis[2], s_node[2];
     __shared__ double s_ext[2][6];
     const int start = blockIdx.x * KD_TILE, end = min(N, start + KD_TILE);
+    if (start >= N) return;
     if (threadIdx.x < 12) {  // the (at most two) nodes of this tile: six segment ends each, fetched by twelve threads at once
         const int k = threadIdx.x / 6, e = threadIdx.x - 6 * k, a = e >> 1;
         int lo, hi;
-        kd_range_of(N, level, k == 0 ? start : end - 1, lo, hi);
+        const int node = kd_range_of(N, level, k == 0 ? start : end - 1, lo, hi);
         const double *coord = (a == 0) ? x : (a == 1) ? y : z;
         s_ext[k][e] = coord[lists[(size_t)a * N + ((e & 1) ? hi - 1 : lo)]];
-        if (e == 0) { s_lo[k] = lo; s_hi[k] = hi; }
+        if (e == 0) { s_lo[k] = lo; s_hi[k] = hi; s_node[k] = node; }
     }
     __syncthreads();
     if (threadIdx.x < 2) {
         const double *v = s_ext[threadIdx.x];
         s_axis[threadIdx.x] = kd_axis(hdr->gamma_bar, v[0], v[1], v[2], v[3], v[4], v[5]);
+        node_axis[s_node[threadIdx.x]] = (uint8_t)s_axis[threadIdx.x];  // (every tile of a node writes the same value)
     }
     __syncthreads();
     for (int i = start + threadIdx.x; i < end; i += 256) {
@@ -203,35 +209,67 @@ __device__ __forceinline__ int kd_block_scan_256(int v, int *total, int *sm /* [
     return wb + inc - v;
 }
 
-// stable split of every node segment of the four lists: left members first.  A tile publishes the number of left members
-// of its last node, and a tile whose first node began earlier adds up the tiles before it.
+// stable split of every node segment of the four lists: left members first.  Single pass with a decoupled look-back: a
+// tile publishes the number of left members of its last node (as a final running count if that node starts inside the
+// tile), a tile whose first node began earlier walks back over the published words until it meets a running count, and
+// then publishes its own.  In the list of a node's split axis the left members are simply the first ceil(size/2)
+// entries: no look-up in the bit mask there.
+#define KD_PUB_AGG 1ull
+#define KD_PUB_RUN 2ull
+__device__ __forceinline__ unsigned long long kd_pub_word(int level, unsigned long long status, int value)
+{
+    return ((unsigned long long)(level + 1) << 40) | (status << 32) | (unsigned long long)(unsigned int)value;
+}
+
 __global__ void __launch_bounds__(256, 6) kd_split(int N, int level, int tiles_per_list, const uint32_t *__restrict__ bits,
-                                                   const uint32_t *__restrict__ cur, uint32_t *__restrict__ nxt,
-                                                   unsigned int *pub /* [4 tiles_per_list] */)
+                                                   const uint8_t *__restrict__ node_axis, const uint32_t *__restrict__ cur,
+                                                   uint32_t *__restrict__ nxt, unsigned long long *pub /* [4 tiles_per_list] */)
 {
     __shared__ int sm[8];
+    __shared__ int s_carry;
+    __shared__ uint32_t stage[KD_TILE];
     // tile = block index: a tile only waits for tiles with smaller indices, and blocks of a 1-D grid start in index
-    // order, so the tiles it waits for are running or done (the assumption of every single-pass look-back scan)
+    // order, so the tiles it waits for are running or done (the assumption of every single-pass look-back scan).
+    // The tiles of list li are shifted by sh entries so that a thread's eight entries are two aligned 16-byte words.
     const int li = blockIdx.y, t = blockIdx.x, tile = li * tiles_per_list + t;
-    const int start = t * KD_TILE, end = min(N, start + KD_TILE);
+    const int sh = (int)(((size_t)li * (size_t)N) & 3);
+    const int start = max(0, t * KD_TILE - sh), end = min(N, (t + 1) * KD_TILE - sh);
+    if (start >= end) {  // (only the last tile of a list can be empty)
+        if (threadIdx.x == 0) atomicExch(&pub[tile], kd_pub_word(level, KD_PUB_RUN, 0));
+        return;
+    }
     int loA, hiA, hiB;
-    kd_range_of(N, level, start, loA, hiA);
+    const int nodeA = kd_range_of(N, level, start, loA, hiA);
     hiB = hiA;
     if (hiA < end) {
         int lo2;
         kd_range_of(N, level, hiA, lo2, hiB);
     }
+    const int midA = loA + (hiA - loA + 1) / 2, midB = hiA + (hiB - hiA + 1) / 2;
+    const bool axisA = node_axis[nodeA] == li, axisB = (hiA < end) && node_axis[nodeA + 1] == li;
     const uint32_t *L = cur + (size_t)li * N;
     uint32_t *O = nxt + (size_t)li * N;
-    const int i0 = start + threadIdx.x * 8;
+    const int i0 = t * KD_TILE - sh + threadIdx.x * 8;
     uint32_t part[8];
+    if (i0 >= 0 && i0 + 8 <= N) {
+        const uint4 v0 = *reinterpret_cast<const uint4 *>(L + i0), v1 = *reinterpret_cast<const uint4 *>(L + i0 + 4);
+        part[0] = v0.x; part[1] = v0.y; part[2] = v0.z; part[3] = v0.w;
+        part[4] = v1.x; part[5] = v1.y; part[6] = v1.z; part[7] = v1.w;
+    } else {
+#pragma unroll
+        for (int k = 0; k < 8; ++k) part[k] = (i0 + k >= 0 && i0 + k < N) ? L[i0 + k] : 0u;
+    }
     unsigned int flags = 0;
     int s = 0, sA = 0;
 #pragma unroll
     for (int k = 0; k < 8; ++k) {
         const int i = i0 + k;
-        part[k] = (i < end) ? L[i] : 0u;
-        const unsigned int f = (i < end) ? ((__ldg(&bits[part[k] >> 5]) >> (part[k] & 31)) & 1u) : 0u;
+        unsigned int f = 0;
+        if (i >= start && i < end) {
+            const bool inA = i < hiA;
+            if (inA ? axisA : axisB) f = (unsigned int)(i < (inA ? midA : midB));
+            else f = (__ldg(&bits[part[k] >> 5]) >> (part[k] & 31)) & 1u;
+        }
         flags |= f << k;
         s += (int)f;
         sA += (int)(f && i < hiA);
@@ -239,33 +277,60 @@ __global__ void __launch_bounds__(256, 6) kd_split(int N, int level, int tiles_p
     int both;  // one scan for both counts: left members in the low half, those of node A in the high half (each <= 2048)
     const int ex = kd_block_scan_256(s | (sA << 16), &both, sm) & 0xffff;
     const int total = both & 0xffff, cA = both >> 16;
-    const unsigned int tag = (unsigned int)(level + 1) << 16;
-    if (threadIdx.x == 0) atomicExch(&pub[tile], tag | (unsigned int)((hiA < end) ? total - cA : total));
-    // left members of node A in the tiles before this one
-    int carry = 0;
-    if (loA < start) {
-        const int nback = (start - loA + KD_TILE - 1) / KD_TILE;
-        int mine = 0;
-        for (int j = threadIdx.x + 1; j <= nback; j += 256) {
-            unsigned int w;
-            do { w = *((volatile unsigned int *)&pub[tile - j]); } while ((w & 0xffff0000u) != tag);
-            mine += (int)(w & 0xffffu);
-        }
-        kd_block_scan_256(mine, &carry, sm);
+    const bool hasB = hiA < end, startsA = loA >= start;
+    if (threadIdx.x == 0) {
+        if (hasB) atomicExch(&pub[tile], kd_pub_word(level, KD_PUB_RUN, total - cA));          // node B starts here
+        else atomicExch(&pub[tile], kd_pub_word(level, startsA ? KD_PUB_RUN : KD_PUB_AGG, total));
     }
-    int running = ex;
+    // The tile's entries leave in four runs: left / right members of node A, then of node B.  They are collected in
+    // shared memory first so that every run is written with coalesced stores.
+    const int endA = min(end, hiA);
+    const int nAL = cA, nAR = (endA - start) - cA, nBL = total - cA;
+    {
+        int running = ex;
 #pragma unroll
-    for (int k = 0; k < 8; ++k) {
-        const int i = i0 + k;
-        if (i < end) {
-            const bool inA = i < hiA;
-            const int lo = inA ? loA : hiA, hi = inA ? hiA : hiB;
-            const int mid = lo + (hi - lo + 1) / 2;
-            const int before = inA ? carry + running : running - cA;  // left members of the node before entry i
-            const unsigned int f = (flags >> k) & 1u;
-            O[f ? (lo + before) : (mid + (i - lo - before))] = part[k];
-            running += (int)f;
+        for (int k = 0; k < 8; ++k) {
+            const int i = i0 + k;
+            if (i >= start && i < end) {
+                const unsigned int f = (flags >> k) & 1u;
+                int slot;
+                if (i < hiA) slot = f ? running : nAL + (i - start - running);
+                else slot = nAL + nAR + (f ? (running - cA) : nBL + (i - hiA - (running - cA)));
+                stage[slot] = part[k];
+                running += (int)f;
+            }
         }
+    }
+    // left members of node A in the tiles before this one: warp 0 walks back, 32 tiles per round, to the nearest running count
+    if (!startsA && threadIdx.x < 32) {
+        const int lane = threadIdx.x;
+        const unsigned long long tag = (unsigned long long)(level + 1);
+        int carry = 0;
+        for (int j = tile - 1;; j -= 32) {
+            unsigned long long w = kd_pub_word(level, KD_PUB_RUN, 0);  // (lanes that would leave the list: nothing before it)
+            if (j - lane >= li * tiles_per_list) {
+                do { w = *((volatile unsigned long long *)&pub[j - lane]); } while ((w >> 40) != tag);
+            }
+            const unsigned int runs = __ballot_sync(0xffffffffu, ((w >> 32) & 0xffull) == KD_PUB_RUN);
+            const int stop = runs ? __ffs(runs) - 1 : 32;  // the nearest tile whose count is final
+            int v = (lane <= stop) ? (int)(unsigned int)w : 0;
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+            carry += v;
+            if (runs) break;
+        }
+        if (lane == 0) {
+            s_carry = carry;
+            if (!hasB) atomicExch(&pub[tile], kd_pub_word(level, KD_PUB_RUN, carry + total));  // node A goes on: its running count
+        }
+    }
+    __syncthreads();
+    const int carry = startsA ? 0 : s_carry;
+    const int gAL = loA + carry, gAR = midA + (start - loA - carry), gBL = hiA, gBR = midB;
+    const int b1 = nAL, b2 = nAL + nAR, b3 = nAL + nAR + nBL, cnt = end - start;
+    for (int q = threadIdx.x; q < cnt; q += 256) {
+        const int dest = (q < b1) ? gAL + q : (q < b2) ? gAR + (q - b1) : (q < b3) ? gBL + (q - b2) : gBR + (q - b3);
+        O[dest] = stage[q];
     }
 }
 
@@ -486,17 +551,18 @@ int kd_build_order(fmm_plan *p, const fmm_particles_t *in, uint32_t **order_out)
     while (level0 < p->kappa && (((int64_t)N + ((int64_t)1 << level0) - 1) >> level0) > KD_LOCAL) ++level0;
     uint32_t *cur = lists, *nxt = lists2;
     if (level0 > 0) {
-        const int tiles = (N + KD_TILE - 1) / KD_TILE;
+        const int tiles = (N + 3 + KD_TILE - 1) / KD_TILE;  // (tiles of a list are shifted by up to three entries, see kd_split)
         const size_t nbits = ((size_t)N + 31) / 32;
         uint32_t *bits = (uint32_t *)ctx_alloc(c, sizeof(uint32_t) * nbits);
-        unsigned int *pub = (unsigned int *)ctx_alloc(c, sizeof(unsigned int) * 4 * (size_t)tiles);
-        if (!bits || !pub) return FMM_ENOMEM;
-        FMM_CUDA(c, cudaMemsetAsync(pub, 0, sizeof(unsigned int) * 4 * (size_t)tiles, st));
+        unsigned long long *pub = (unsigned long long *)ctx_alloc(c, sizeof(unsigned long long) * 4 * (size_t)tiles);
+        uint8_t *node_axis = (uint8_t *)ctx_alloc(c, (size_t)1 << level0);
+        if (!bits || !pub || !node_axis) return FMM_ENOMEM;
+        FMM_CUDA(c, cudaMemsetAsync(pub, 0, sizeof(unsigned long long) * 4 * (size_t)tiles, st));
         for (int level = 0; level < level0; ++level) {
             FMM_CUDA(c, cudaMemsetAsync(bits, 0, sizeof(uint32_t) * nbits, st));
-            kd_mark<<<tiles, 256, 0, st>>>(N, level, in->x, in->y, in->z, cur, p->hdr, bits);
+            kd_mark<<<tiles, 256, 0, st>>>(N, level, in->x, in->y, in->z, cur, p->hdr, bits, node_axis);
             FMM_LAUNCH_CHECK(c, "kd_mark");
-            kd_split<<<dim3(tiles, 4), 256, 0, st>>>(N, level, tiles, bits, cur, nxt, pub);
+            kd_split<<<dim3(tiles, 4), 256, 0, st>>>(N, level, tiles, bits, node_axis, cur, nxt, pub);
             FMM_LAUNCH_CHECK(c, "kd_split");
             uint32_t *t = cur; cur = nxt; nxt = t;
         }
