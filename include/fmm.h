@@ -128,6 +128,10 @@ typedef struct {
     float ms_lists;                         /* a3: traversal, sort, CSR                            */
     float ms_p2m, ms_m2m, ms_m2l, ms_l2l, ms_p2p, ms_l2p;  /* a4-a10 (l2p includes finalise)      */
     int64_t workspace_bytes;                /* device bytes currently held by the plan            */
+    int32_t p2p_split, m2l_split;           /* row chunks per target of the near / far pair kernels (partial sums added in order) */
+    int32_t p2p_mutual;                     /* 1: the near field evaluates every mated pair of leaves once for both directions   */
+    int32_t reserved;
+    int64_t react_particles;                /* particles in the reaction segments of the mutual near field (6 doubles each)       */
 } fmm_stats_t;
 
 /* Copies of the plan's integer structures and (optionally) expansions, for bit-exact
@@ -204,11 +208,6 @@ void fmm_plan_destroy(fmm_plan_t *plan);
 
 /* Number of kernel launches the library has enqueued in this process (bench.py's gpu_launches). */
 int64_t fmm_launch_count(void);
-
-/* Diagnostic: sustained rate of dependent-free DFMA chains on the FP64 pipe, in TFLOP/s (2 flop per
- * DFMA), best of 3 timed launches of ~1.2e12 flop.  The roofline denominator bench.py quotes beside
- * the nominal 148 SM x 64 lanes x 2 x clock.  Synchronises the stream. */
-int fmm_probe_fp64_peak(double *tflops, double *ms, void *cuda_stream);
 
 const char *fmm_strerror(int code);
 const char *fmm_last_error(const fmm_plan_t *plan);  /* plan may be NULL: last error of a plan-less call */

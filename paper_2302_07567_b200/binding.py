@@ -53,7 +53,9 @@ class fmm_stats_t(C.Structure):
                 ("gamma_bar", C.c_double), ("theta", C.c_double), ("flags", C.c_uint32),
                 ("timing_valid", C.c_int32), ("ms_tree", C.c_float), ("ms_lists", C.c_float),
                 ("ms_p2m", C.c_float), ("ms_m2m", C.c_float), ("ms_m2l", C.c_float), ("ms_l2l", C.c_float),
-                ("ms_p2p", C.c_float), ("ms_l2p", C.c_float), ("workspace_bytes", C.c_int64)]
+                ("ms_p2p", C.c_float), ("ms_l2p", C.c_float), ("workspace_bytes", C.c_int64),
+                ("p2p_split", C.c_int32), ("m2l_split", C.c_int32), ("p2p_mutual", C.c_int32), ("reserved", C.c_int32),
+                ("react_particles", C.c_int64)]
 
     def as_dict(self) -> dict:
         return {k: getattr(self, k) for k, _ in self._fields_}
@@ -67,7 +69,7 @@ class fmm_export_t(C.Structure):
 
 EXPORTED_SYMBOLS = ["fmm_plan_create", "fmm_plan_update", "fmm_plan_refit", "fmm_eval", "fmm_direct", "fmm_field_host",
                     "fmm_plan_set_timing", "fmm_plan_set_overlap", "fmm_plan_stats", "fmm_plan_export", "fmm_plan_destroy",
-                    "fmm_launch_count", "fmm_probe_fp64_peak", "fmm_strerror", "fmm_last_error", "fmm_version"]
+                    "fmm_launch_count", "fmm_strerror", "fmm_last_error", "fmm_version"]
 
 _lib = None
 
@@ -112,8 +114,6 @@ def load_library():
     lib.fmm_plan_destroy.restype = None
     lib.fmm_plan_destroy.argtypes = [vp]
     lib.fmm_launch_count.restype = C.c_int64
-    lib.fmm_probe_fp64_peak.restype = C.c_int
-    lib.fmm_probe_fp64_peak.argtypes = [_dp, _dp, vp]
     lib.fmm_strerror.restype = C.c_char_p
     lib.fmm_strerror.argtypes = [C.c_int]
     lib.fmm_last_error.restype = C.c_char_p
@@ -401,11 +401,3 @@ def fmm_field_host(x, y, z, px, py, pz, q=None, *, order_n, leaf_size, theta, ga
 
 def fmm_launch_count() -> int:
     return int(load_library().fmm_launch_count())
-
-
-def fmm_probe_fp64_peak() -> float:
-    """Sustained DFMA rate of the device in TFLOP/s (diagnostic; roofline denominator)."""
-    _require_cuda()
-    t, ms = C.c_double(), C.c_double()
-    _check(load_library().fmm_probe_fp64_peak(C.byref(t), C.byref(ms), _stream_ptr()))
-    return float(t.value)

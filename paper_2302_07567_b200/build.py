@@ -16,6 +16,7 @@ from pathlib import Path
 HERE = Path(__file__).resolve().parent
 CSRC = HERE / "csrc"
 LIB = HERE / "libfmm_b200.so"
+PROBE_LIB = HERE / "libfmm_probe.so"   # FP64 pipe micro-benchmarks for bench.py (measurement tooling, not the boundary)
 SOURCES = ["fmm_api.cu", "sort.cu", "kernels_tree.cu", "kernels_kd.cu", "kernels_dtt.cu", "kernels_interp.cu", "kernels_pairs.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC", "-Xptxas", "-v"]
@@ -62,5 +63,21 @@ def build_library(force: bool = False, verbose: bool = False) -> Path:
     return LIB
 
 
+def build_probe(force: bool = False) -> Path:
+    """libfmm_probe.so from csrc/probe_fp64.cu (see the header comment of that file)."""
+    src = CSRC / "probe_fp64.cu"
+    if not force and PROBE_LIB.exists() and PROBE_LIB.stat().st_mtime >= src.stat().st_mtime:
+        return PROBE_LIB
+    tmp = PROBE_LIB.with_suffix(f".tmp{os.getpid()}.so")
+    cmd = [_nvcc(), "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17", "-Xcompiler", "-fPIC",
+           "-shared", str(src), "-o", str(tmp)]
+    r = subprocess.run(cmd, capture_output=True, text=True)
+    if r.returncode != 0:
+        raise RuntimeError(f"nvcc failed on probe_fp64.cu:\n{r.stderr}")
+    os.replace(tmp, PROBE_LIB)
+    return PROBE_LIB
+
+
 if __name__ == "__main__":
     build_library(force="--force" in sys.argv, verbose=True)
+    build_probe(force="--force" in sys.argv)

@@ -427,6 +427,10 @@ extern "C" int fmm_plan_stats(fmm_plan_t *p, fmm_stats_t *s)
     s->ms_tree = p->ms_tree;
     s->ms_lists = p->ms_lists;
     s->workspace_bytes = p->ctx.bytes;
+    s->p2p_split = p->p2p_split;
+    s->m2l_split = p->m2l_split;
+    s->p2p_mutual = (p->p2p_mutual && p->p2p_dst != NULL) ? 1 : 0;
+    s->react_particles = s->p2p_mutual ? p->p2p_react : 0;
     if (p->timing && p->ev_valid) {
         fmm_ctx *c = &p->ctx;
         FMM_CUDA(c, cudaEventSynchronize(p->ev[EV_END]));
@@ -550,56 +554,4 @@ extern "C" int fmm_field_host(const fmm_particles_t *h, const fmm_params_t *prm,
     cudaStreamSynchronize(c->stream);
     ctx_free_all(c);
     return rc;
-}
-
-// ---------------------------------------------------------------------------------------
-// diagnostic: sustained DFMA rate of the FP64 pipe (the denominator of the P2P / M2L roofline)
-// ---------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(256) dfma_chain_kernel(int iters, double a, double b, double *out)
-{
-    double v[8];
-#pragma unroll
-    for (int k = 0; k < 8; ++k) v[k] = (double)(threadIdx.x + k) * 1e-3;
-    for (int it = 0; it < iters; ++it) {
-#pragma unroll
-        for (int u = 0; u < 4; ++u)
-#pragma unroll
-            for (int k = 0; k < 8; ++k) v[k] = fma(v[k], a, b);
-    }
-    double s = 0.0;
-#pragma unroll
-    for (int k = 0; k < 8; ++k) s += v[k];
-    if (s == 123.456) out[0] = s;  // keeps the chain alive without a store in practice
-}
-
-extern "C" int fmm_probe_fp64_peak(double *tflops, double *ms_out, void *cuda_stream)
-{
-    if (!tflops) return FMM_EINVAL;
-    fmm_ctx ctx;
-    ctx_init(&ctx, NULL, NULL, NULL, cuda_stream);
-    fmm_ctx *c = &ctx;
-    double *out = (double *)ctx_alloc(c, 64);
-    if (!out) return FMM_ENOMEM;
-    cudaEvent_t e0, e1;
-    FMM_CUDA(c, cudaEventCreate(&e0));
-    FMM_CUDA(c, cudaEventCreate(&e1));
-    const int blocks = FMM_SM_COUNT * 8, iters = 20000;
-    float best = 1e30f;
-    for (int rep = 0; rep < 4; ++rep) {
-        FMM_CUDA(c, cudaEventRecord(e0, c->stream));
-        dfma_chain_kernel<<<blocks, 256, 0, c->stream>>>(iters, 0.999999, 1e-9, out);
-        FMM_LAUNCH_CHECK(c, "dfma_chain_kernel");
-        FMM_CUDA(c, cudaEventRecord(e1, c->stream));
-        FMM_CUDA(c, cudaEventSynchronize(e1));
-        float ms = 0;
-        FMM_CUDA(c, cudaEventElapsedTime(&ms, e0, e1));
-        if (rep > 0 && ms < best) best = ms;
-    }
-    cudaEventDestroy(e0);
-    cudaEventDestroy(e1);
-    ctx_free_all(c);
-    double flop = 2.0 * 32.0 * (double)iters * 256.0 * (double)blocks;
-    *tflops = flop / ((double)best * 1e-3) / 1e12;
-    if (ms_out) *ms_out = best;
-    return FMM_OK;
 }

@@ -248,17 +248,21 @@ __device__ __forceinline__ void mut_process_mutual(mut_targets<NT> &T, const mut
                 react[3 * rstride + d] = rbx; react[4 * rstride + d] = rby; react[5 * rstride + d] = rbz;
             }
         } else {
-            double *r = red + (size_t)warp * 192 + lane;
-            r[0] = rex; r[32] = rey; r[64] = rez; r[96] = rbx; r[128] = rby; r[160] = rbz;
-            __syncthreads();
-            for (int q = threadIdx.x; q < 192; q += 32 * W) {
-                const int d = S.dst[b0 + (q & 31)];
+            double *r = red + (size_t)warp * (6 * MUT_TILE) + b0 + lane;
+            r[0] = rex; r[MUT_TILE] = rey; r[2 * MUT_TILE] = rez; r[3 * MUT_TILE] = rbx; r[4 * MUT_TILE] = rby; r[5 * MUT_TILE] = rbz;
+        }
+    }
+    if (W > 1) {  // once per tile: the warps' sums are added in warp order and stored (the caller's barrier follows)
+        __syncthreads();
+        for (int q = threadIdx.x; q < 6 * MUT_TILE; q += 32 * W) {
+            const int j = q & (MUT_TILE - 1);
+            if (j < cnt) {
+                const int d = S.dst[j];
                 double v = red[q];
 #pragma unroll
-                for (int w = 1; w < W; ++w) v += red[(size_t)w * 192 + q];  // warp order
-                if (d >= 0) react[(size_t)(q >> 5) * rstride + d] = v;
+                for (int w = 1; w < W; ++w) v += red[(size_t)w * (6 * MUT_TILE) + q];
+                if (d >= 0) react[(size_t)(q / MUT_TILE) * rstride + d] = v;
             }
-            __syncthreads();
         }
     }
 }
@@ -279,7 +283,7 @@ __device__ __forceinline__ void mut_process_onesided(mut_targets<NT> &T, const m
 // step with the fewest stalls (profiles/r02_p2p_mutual.md), the smaller shapes fit more warps
 template <int NT, int W>
 struct mut_cfg {
-    static constexpr int WARPS = (NT == 4) ? 8 : (NT == 3) ? 12 : (NT == 2) ? 16 : 32;
+    static constexpr int WARPS = (NT == 4) ? 8 : (NT == 3) ? ((W == 8) ? 8 : 12) : (NT == 2) ? 16 : 32;
     static constexpr int MINB = (WARPS / W) > 0 ? (WARPS / W) : 1;
 };
 
@@ -294,7 +298,7 @@ __global__ void __launch_bounds__(32 * W, mut_cfg<NT, W>::MINB) p2p_mutual_kerne
                                                          double *__restrict__ react, size_t rstride)
 {
     __shared__ mut_tile S;
-    __shared__ double mut_red[W > 1 ? W * 192 : 1];  // [W][6][32]
+    extern __shared__ double mut_red[];  // [W][6][MUT_TILE] reaction sums of the current tile, per warp (W > 1)
     const int t = SPLIT ? order[blockIdx.x / K] : order[blockIdx.x], kc = SPLIT ? blockIdx.x % K : 0;
     const int tlo = node_lo[t], thi = node_hi[t];
     const int r0 = off[t], rl = off[t + 1] - r0;
@@ -365,15 +369,18 @@ __global__ void __launch_bounds__(32 * W, mut_cfg<NT, W>::MINB) p2p_mutual_kerne
 }
 
 // Targets per thread: the NT <= 4 that wastes the fewest lanes, ties to the larger NT (a leaf of 78 particles fills 3 x 32 slots at NT = 3 but only 78 of 128 at NT = 4).
-// Mutual kernel (mutual != 0): a whole leaf in one pass, the fewest warps W with NT <= 4, then the smallest NT; the travelling
-// reaction sums cost the same per step whatever NT is, so NT is kept high (NT < 4 only with W <= 3).
+// Mutual kernel (mutual != 0): a whole leaf in one pass, the fewest warps W in {1, 2, 4, 8} with NT <= 4, then the smallest NT;
+// the travelling reaction sums cost the same per step whatever NT is, so NT is kept high (NT >= 3 whenever W > 1).
 static void p2p_shape(int64_t leaves, int maxleaf, int64_t pairs, int64_t max_row, int *nt_out, int *threads_out, int *split_out,
                       int mutual = 0)
 {
     int best_nt = 1, best_threads = 32;
     double best_score = -1.0;
     if (mutual && maxleaf <= 1024) {
-        const int W = (maxleaf + 127) / 128 > 0 ? (maxleaf + 127) / 128 : 1;
+        // W a power of two: the resident warps of an SM then split evenly over its four sub-partitions (three warps per
+        // block left one sub-partition with 3 of 9 warps: 46 % instead of 60 % of peak at leaves of 312, profiles/r02_bench_configs.md)
+        int W = 1;
+        while (32 * 4 * W < maxleaf) W *= 2;
         best_threads = 32 * W;
         best_nt = (maxleaf + best_threads - 1) / best_threads;
         if (best_nt < 1) best_nt = 1;
@@ -466,12 +473,17 @@ int pairs_p2p(fmm_plan *p)
     if (p->react_used) {
         const size_t rstride = (size_t)(p->react_cap > 0 ? p->react_cap : 1);
 #define MUT_LAUNCH(NT, W)                                                                                                                 \
+    const size_t red_bytes = (W > 1) ? sizeof(double) * 6 * MUT_TILE * W : 0;                                                             \
+    if (red_bytes + sizeof(mut_tile) > 48 * 1024) {                                                                                       \
+        FMM_CUDA(c, cudaFuncSetAttribute((const void *)p2p_mutual_kernel<NT, W, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)red_bytes));  \
+        FMM_CUDA(c, cudaFuncSetAttribute((const void *)p2p_mutual_kernel<NT, W, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)red_bytes)); \
+    }                                                                                                                                     \
     if (K > 1)                                                                                                                            \
-        p2p_mutual_kernel<NT, W, true><<<(unsigned)(p->leaves * K), 32 * W, 0, c->stream>>>(                                              \
+        p2p_mutual_kernel<NT, W, true><<<(unsigned)(p->leaves * K), 32 * W, red_bytes, c->stream>>>(                                      \
             (int)p->N, p->gamma_bar, p->p2p_order, p->p2p_off, p->p2p_src, p->p2p_dst, p->node_lo, p->node_hi, p->tx, p->ty, p->tz, p->w0, \
             p->w1, p->w2, p->w3, K, p->near_, p->react, rstride);                                                                         \
     else                                                                                                                                  \
-        p2p_mutual_kernel<NT, W, false><<<(unsigned)p->leaves, 32 * W, 0, c->stream>>>(                                                   \
+        p2p_mutual_kernel<NT, W, false><<<(unsigned)p->leaves, 32 * W, red_bytes, c->stream>>>(                                           \
             (int)p->N, p->gamma_bar, p->p2p_order, p->p2p_off, p->p2p_src, p->p2p_dst, p->node_lo, p->node_hi, p->tx, p->ty, p->tz, p->w0, \
             p->w1, p->w2, p->w3, K, p->near_, p->react, rstride)
         const int W = threads / 32;
@@ -479,14 +491,11 @@ int pairs_p2p(fmm_plan *p)
         else if (nt == 2) { MUT_LAUNCH(2, 1); }
         else if (nt == 3 && W == 1) { MUT_LAUNCH(3, 1); }
         else if (nt == 3 && W == 2) { MUT_LAUNCH(3, 2); }
-        else if (nt == 3) { MUT_LAUNCH(3, 3); }
+        else if (nt == 3 && W == 4) { MUT_LAUNCH(3, 4); }
+        else if (nt == 3) { MUT_LAUNCH(3, 8); }
         else if (W == 1) { MUT_LAUNCH(4, 1); }
         else if (W == 2) { MUT_LAUNCH(4, 2); }
-        else if (W == 3) { MUT_LAUNCH(4, 3); }
         else if (W == 4) { MUT_LAUNCH(4, 4); }
-        else if (W == 5) { MUT_LAUNCH(4, 5); }
-        else if (W == 6) { MUT_LAUNCH(4, 6); }
-        else if (W == 7) { MUT_LAUNCH(4, 7); }
         else { MUT_LAUNCH(4, 8); }
 #undef MUT_LAUNCH
         FMM_LAUNCH_CHECK(c, "p2p_mutual_kernel");
