@@ -203,6 +203,7 @@ static int plan_alloc_fixed(fmm_plan *p)
     ALLOC(node_lo, int32_t, nodes1); ALLOC(node_hi, int32_t, nodes1);
     ALLOC(bbox, double, 6 * nodes1); ALLOC(node_geo, double, 4 * nodes1);
     ALLOC(node_xi, double, 48 * nodes1);
+    ALLOC(node_T, double, (size_t)((3 * p->n1 * p->n1 + 1) & ~1) * nodes1);
     ALLOC(p2p_off, int32_t, nodes1 + 1); ALLOC(m2l_off, int32_t, nodes1 + 1);
     ALLOC(p2p_order, int32_t, nodes1); ALLOC(m2l_order, int32_t, nodes1);
     ALLOC(M, double, 4 * (size_t)p->P * nodes1);

@@ -94,6 +94,7 @@ struct fmm_plan {
     int32_t *node_hi;
     double *bbox;           // [nodes+1][6]
     double *node_geo;       // [nodes+1][4] : r^2 (Alg 5.6 squared), cx, cy, cz (box centres)
+    double *node_T;         // [nodes+2][3 (n+1)^2 rounded up to even] 1-D transfer matrices child <- parent, filled per build
     double *node_xi;        // [nodes+1][3][16] : proxy points per axis (I-3), filled by pairs_m2l
     // interaction lists, CSR by target node id (offset arrays indexed by node id, length nodes+2)
     int32_t *p2p_off, *p2p_src, *m2l_off, *m2l_src;
@@ -145,6 +146,7 @@ int tree_refit(fmm_plan *p, const fmm_particles_t *in);  // keeps the particle o
 // ---- kernels_dtt.cu -----------------------------------------------------------------
 int dtt_build_lists(fmm_plan *p);
 // ---- kernels_interp.cu --------------------------------------------------------------
+int interp_transfer_tables(fmm_plan *p);  // after the boxes of a build
 int interp_p2m(fmm_plan *p);
 int interp_m2m(fmm_plan *p);
 int interp_l2l(fmm_plan *p);

@@ -47,7 +47,8 @@ __device__ __forceinline__ void basis_1d(int n, const cheb_t &ch, double a, doub
     if (hit >= 0) {
         for (int k = 0; k <= n; ++k) out[k * stride] = (k == hit) ? 1.0 : 0.0;
     } else {
-        for (int k = 0; k <= n; ++k) out[k * stride] = out[k * stride] / S;
+        const double rS = 1.0 / S;  // (one division; l_k = t_k / S to one more rounding)
+        for (int k = 0; k <= n; ++k) out[k * stride] = out[k * stride] * rS;
     }
 }
 
@@ -71,7 +72,7 @@ struct p2m_cfg {
 };
 
 template <int N1>
-__global__ void __launch_bounds__(P2M_THREADS) p2m_kernel(cheb_t ch, int leaves, const int32_t *__restrict__ node_lo,
+__global__ void __launch_bounds__(P2M_THREADS, (N1 <= 7) ? 3 : 1) p2m_kernel(cheb_t ch, int leaves, const int32_t *__restrict__ node_lo,
                                                           const int32_t *__restrict__ node_hi, const double *__restrict__ bbox,
                                                           const double *__restrict__ tx, const double *__restrict__ ty,
                                                           const double *__restrict__ tz, const double *__restrict__ w0,
@@ -154,15 +155,35 @@ __global__ void __launch_bounds__(P2M_THREADS) p2m_kernel(cheb_t ch, int leaves,
 // ---------------------------------------------------------------------------------------
 // 1-D transfer matrices T_g[k][k'] = l_{S,k}(xi_{S',k'}) on the three axes (S = parent, S' = child)
 // ---------------------------------------------------------------------------------------
-__device__ __forceinline__ void transfer_matrices(int n, const cheb_t &ch, const double *bS, const double *bC, double *T /* [3][n1][n1] */)
+// T of every child node C (parent S = C / 2), stride XFER_T per node, computed once per plan build (the boxes do not change
+// between evaluations): M2M and L2L then only load 3 (n+1)^2 doubles instead of running 3 (n+1) barycentric evaluations
+// with their divisions at the head of every level's dependency chain.
+__global__ void transfer_tables_kernel(int n, cheb_t ch, int nodes, int stride, const int32_t *__restrict__ node_lo,
+                                       const int32_t *__restrict__ node_hi, const double *__restrict__ bbox, double *__restrict__ tab)
 {
     const int n1 = n + 1;
-    for (int t = threadIdx.x; t < 3 * n1; t += blockDim.x) {
-        int g = t / n1, kc = t - g * n1;
-        double mid = __dmul_rn(__dadd_rn(bC[g], bC[3 + g]), 0.5), half = __dmul_rn(__dsub_rn(bC[3 + g], bC[g]), 0.5);
-        double xi = node_point(mid, half, ch.c[kc]);
-        basis_1d(n, ch, bS[g], bS[3 + g], xi, T + (size_t)g * n1 * n1 + kc, n1);  // column kc
-    }
+    const int q = blockIdx.x * blockDim.x + threadIdx.x;  // (child, axis, column)
+    const int C = 2 + q / (3 * n1);
+    if (C > nodes) return;
+    if (node_hi[C] <= node_lo[C]) return;
+    const int r = q - (C - 2) * 3 * n1, g = r / n1, kc = r - g * n1;
+    const double *bS = bbox + 6 * (int64_t)(C >> 1), *bC = bbox + 6 * (int64_t)C;
+    const double mid = __dmul_rn(__dadd_rn(bC[g], bC[3 + g]), 0.5), half = __dmul_rn(__dsub_rn(bC[3 + g], bC[g]), 0.5);
+    const double xi = node_point(mid, half, ch.c[kc]);
+    basis_1d(n, ch, bS[g], bS[3 + g], xi, tab + (size_t)C * stride + (size_t)g * n1 * n1 + kc, n1);  // column kc
+}
+
+int interp_transfer_tables(fmm_plan *p)
+{
+    fmm_ctx *c = &p->ctx;
+    if (p->nodes < 2) return FMM_OK;
+    const cheb_t ch = host_cheb(p->n);
+    const int stride = (3 * p->n1 * p->n1 + 1) & ~1;
+    const int64_t count = (int64_t)(p->nodes - 1) * 3 * p->n1;
+    transfer_tables_kernel<<<(unsigned)((count + 127) / 128), 128, 0, c->stream>>>(p->n, ch, (int)p->nodes, stride, p->node_lo, p->node_hi, p->bbox,
+                                                                                 p->node_T);
+    FMM_LAUNCH_CHECK(c, "transfer_tables_kernel");
+    return FMM_OK;
 }
 
 // ---------------------------------------------------------------------------------------
@@ -172,15 +193,15 @@ __device__ __forceinline__ void transfer_matrices(int n, const cheb_t &ch, const
 #define XFER_THREADS 256
 
 template <int N1>
-__global__ void __launch_bounds__(XFER_THREADS) m2m_kernel(cheb_t ch, int first, const int32_t *__restrict__ node_lo,
-                                                           const int32_t *__restrict__ node_hi, const double *__restrict__ bbox,
+__global__ void __launch_bounds__(XFER_THREADS) m2m_kernel(int first, const int32_t *__restrict__ node_lo,
+                                                           const int32_t *__restrict__ node_hi, const double *__restrict__ tab,
                                                            double *__restrict__ M)
 {
-    extern __shared__ double sm[];
-    constexpr int n = N1 - 1, n1 = N1, P = n1 * n1 * n1, P4 = 4 * P;  // compile-time order: index arithmetic without integer division
-    double *T = sm;                   // [3][n1][n1]
-    double *A = sm + 3 * n1 * n1;     // [P][4]
-    double *B = A + P4;               // [P][4]
+    extern __shared__ __align__(16) double sm[];
+    constexpr int n1 = N1, P = n1 * n1 * n1, P4 = 4 * P, TS = (3 * n1 * n1 + 1) & ~1;  // compile-time order: index arithmetic without integer division
+    double *T = sm;                              // [3][n1][n1]
+    double *A = sm + TS;                         // [P][4], 16-byte aligned
+    double *B = A + P4;                          // [P][4]
     int S = first + blockIdx.x;
     double *MS = M + (int64_t)P4 * S;
     // parent accumulators live in registers across the two children: element e = threadIdx.x + k*blockDim
@@ -193,25 +214,41 @@ __global__ void __launch_bounds__(XFER_THREADS) m2m_kernel(cheb_t ch, int first,
             int C = 2 * S + child;
             if (node_hi[C] <= node_lo[C]) continue;  // uniform per block
             __syncthreads();
-            transfer_matrices(n, ch, bbox + 6 * (int64_t)S, bbox + 6 * (int64_t)C, T);
+            for (int e = threadIdx.x; e < 3 * n1 * n1; e += XFER_THREADS) T[e] = tab[(size_t)C * TS + e];
             const double *MC = M + (int64_t)P4 * C;
             for (int e = threadIdx.x; e < P4; e += XFER_THREADS) A[e] = MC[e];
             __syncthreads();
             const double *Tx = T, *Ty = T + n1 * n1, *Tz = T + 2 * n1 * n1;
-            // z: B[a',b',c] = sum_c' Tz[c][c'] A[a',b',c']
-            for (int e = threadIdx.x; e < P4; e += XFER_THREADS) {
-                int f = e & 3, nu = e >> 2, c3 = nu % n1, ab = nu / n1;
-                double s = 0.0;
-                for (int k = 0; k < n1; ++k) s = fma(Tz[c3 * n1 + k], A[4 * (ab * n1 + k) + f], s);
-                B[e] = s;
+            // z: B[a',b',c] = sum_c' Tz[c][c'] A[a',b',c']   (a thread takes a proxy point with its four moments: the moments
+            // come as two 16-byte words, a matrix entry is loaded once for four products)
+            for (int nu = threadIdx.x; nu < P; nu += XFER_THREADS) {
+                const int c3 = nu % n1, ab = nu / n1;
+                double s0 = 0.0, s1 = 0.0, s2 = 0.0, s3 = 0.0;
+#pragma unroll
+                for (int k = 0; k < n1; ++k) {
+                    const double t = Tz[c3 * n1 + k];
+                    const double2 v01 = *reinterpret_cast<const double2 *>(&A[4 * (ab * n1 + k)]);
+                    const double2 v23 = *reinterpret_cast<const double2 *>(&A[4 * (ab * n1 + k) + 2]);
+                    s0 = fma(t, v01.x, s0); s1 = fma(t, v01.y, s1); s2 = fma(t, v23.x, s2); s3 = fma(t, v23.y, s3);
+                }
+                *reinterpret_cast<double2 *>(&B[4 * nu]) = make_double2(s0, s1);
+                *reinterpret_cast<double2 *>(&B[4 * nu + 2]) = make_double2(s2, s3);
             }
             __syncthreads();
             // y: A[a',b,c] = sum_b' Ty[b][b'] B[a',b',c]
-            for (int e = threadIdx.x; e < P4; e += XFER_THREADS) {
-                int f = e & 3, nu = e >> 2, c3 = nu % n1, b = (nu / n1) % n1, a = nu / (n1 * n1);
-                double s = 0.0;
-                for (int k = 0; k < n1; ++k) s = fma(Ty[b * n1 + k], B[4 * ((a * n1 + k) * n1 + c3) + f], s);
-                A[e] = s;
+            for (int nu = threadIdx.x; nu < P; nu += XFER_THREADS) {
+                const int c3 = nu % n1, b = (nu / n1) % n1, a = nu / (n1 * n1);
+                double s0 = 0.0, s1 = 0.0, s2 = 0.0, s3 = 0.0;
+#pragma unroll
+                for (int k = 0; k < n1; ++k) {
+                    const double t = Ty[b * n1 + k];
+                    const int q = 4 * ((a * n1 + k) * n1 + c3);
+                    const double2 v01 = *reinterpret_cast<const double2 *>(&B[q]);
+                    const double2 v23 = *reinterpret_cast<const double2 *>(&B[q + 2]);
+                    s0 = fma(t, v01.x, s0); s1 = fma(t, v01.y, s1); s2 = fma(t, v23.x, s2); s3 = fma(t, v23.y, s3);
+                }
+                *reinterpret_cast<double2 *>(&A[4 * nu]) = make_double2(s0, s1);
+                *reinterpret_cast<double2 *>(&A[4 * nu + 2]) = make_double2(s2, s3);
             }
             __syncthreads();
             // x: out[a,b,c] = sum_a' Tx[a][a'] A[a',b,c]
@@ -239,37 +276,54 @@ __global__ void __launch_bounds__(XFER_THREADS) m2m_kernel(cheb_t ch, int first,
 //   L_S'[a',b',c'] += sum_{a,b,c} Tx[a][a'] Ty[b][b'] Tz[c][c'] L_S[a,b,c]
 // ---------------------------------------------------------------------------------------
 template <int N1>
-__global__ void __launch_bounds__(XFER_THREADS) l2l_kernel(cheb_t ch, int first, const int32_t *__restrict__ node_lo,
-                                                           const int32_t *__restrict__ node_hi, const double *__restrict__ bbox,
+__global__ void __launch_bounds__(XFER_THREADS) l2l_kernel(int first, const int32_t *__restrict__ node_lo,
+                                                           const int32_t *__restrict__ node_hi, const double *__restrict__ tab,
                                                            double *__restrict__ L)
 {
-    extern __shared__ double sm[];
-    constexpr int n = N1 - 1, n1 = N1, P = n1 * n1 * n1, P6 = 6 * P;
+    extern __shared__ __align__(16) double sm[];
+    constexpr int n1 = N1, P = n1 * n1 * n1, P6 = 6 * P, TS = (3 * n1 * n1 + 1) & ~1;
     double *T = sm;
-    double *A = sm + 3 * n1 * n1;  // [P][6]
+    double *A = sm + TS;  // [P][6], 16-byte aligned
     double *B = A + P6;
     int C = first + blockIdx.x, S = C >> 1;
     if (node_hi[C] <= node_lo[C]) return;
-    transfer_matrices(n, ch, bbox + 6 * (int64_t)S, bbox + 6 * (int64_t)C, T);
+    for (int e = threadIdx.x; e < 3 * n1 * n1; e += XFER_THREADS) T[e] = tab[(size_t)C * TS + e];
     const double *LS = L + (int64_t)P6 * S;
     double *LC = L + (int64_t)P6 * C;
     for (int e = threadIdx.x; e < P6; e += XFER_THREADS) A[e] = LS[e];
     __syncthreads();
     const double *Tx = T, *Ty = T + n1 * n1, *Tz = T + 2 * n1 * n1;
-    // z: B[a,b,c'] = sum_c Tz[c][c'] A[a,b,c]
-    for (int e = threadIdx.x; e < P6; e += XFER_THREADS) {
-        int f = e % 6, nu = e / 6, c3 = nu % n1, ab = nu / n1;
-        double s = 0.0;
-        for (int k = 0; k < n1; ++k) s = fma(Tz[k * n1 + c3], A[6 * (ab * n1 + k) + f], s);
-        B[e] = s;
+    // z: B[a,b,c'] = sum_c Tz[c][c'] A[a,b,c]   (a thread takes a proxy point with its six field components: three 16-byte
+    // words per term, a matrix entry is loaded once for six products)
+    for (int nu = threadIdx.x; nu < P; nu += XFER_THREADS) {
+        const int c3 = nu % n1, ab = nu / n1;
+        double s[6] = {0, 0, 0, 0, 0, 0};
+#pragma unroll
+        for (int k = 0; k < n1; ++k) {
+            const double t = Tz[k * n1 + c3];
+            const double2 *v = reinterpret_cast<const double2 *>(&A[6 * (ab * n1 + k)]);
+            const double2 v0 = v[0], v1 = v[1], v2 = v[2];
+            s[0] = fma(t, v0.x, s[0]); s[1] = fma(t, v0.y, s[1]); s[2] = fma(t, v1.x, s[2]);
+            s[3] = fma(t, v1.y, s[3]); s[4] = fma(t, v2.x, s[4]); s[5] = fma(t, v2.y, s[5]);
+        }
+        double2 *o = reinterpret_cast<double2 *>(&B[6 * nu]);
+        o[0] = make_double2(s[0], s[1]); o[1] = make_double2(s[2], s[3]); o[2] = make_double2(s[4], s[5]);
     }
     __syncthreads();
     // y: A[a,b',c'] = sum_b Ty[b][b'] B[a,b,c']
-    for (int e = threadIdx.x; e < P6; e += XFER_THREADS) {
-        int f = e % 6, nu = e / 6, c3 = nu % n1, b = (nu / n1) % n1, a = nu / (n1 * n1);
-        double s = 0.0;
-        for (int k = 0; k < n1; ++k) s = fma(Ty[k * n1 + b], B[6 * ((a * n1 + k) * n1 + c3) + f], s);
-        A[e] = s;
+    for (int nu = threadIdx.x; nu < P; nu += XFER_THREADS) {
+        const int c3 = nu % n1, b = (nu / n1) % n1, a = nu / (n1 * n1);
+        double s[6] = {0, 0, 0, 0, 0, 0};
+#pragma unroll
+        for (int k = 0; k < n1; ++k) {
+            const double t = Ty[k * n1 + b];
+            const double2 *v = reinterpret_cast<const double2 *>(&B[6 * ((a * n1 + k) * n1 + c3)]);
+            const double2 v0 = v[0], v1 = v[1], v2 = v[2];
+            s[0] = fma(t, v0.x, s[0]); s[1] = fma(t, v0.y, s[1]); s[2] = fma(t, v1.x, s[2]);
+            s[3] = fma(t, v1.y, s[3]); s[4] = fma(t, v2.x, s[4]); s[5] = fma(t, v2.y, s[5]);
+        }
+        double2 *o = reinterpret_cast<double2 *>(&A[6 * nu]);
+        o[0] = make_double2(s[0], s[1]); o[1] = make_double2(s[2], s[3]); o[2] = make_double2(s[4], s[5]);
     }
     __syncthreads();
     // x: L_S'[a',b',c'] += sum_a Tx[a][a'] A[a,b',c']
@@ -286,6 +340,7 @@ __global__ void __launch_bounds__(XFER_THREADS) l2l_kernel(cheb_t ch, int first,
 // per particle; the leaf's local fields sit in shared memory and are read as broadcasts.
 // ---------------------------------------------------------------------------------------
 #define L2P_THREADS 128
+#define L2P_SEGS 256
 
 template <int N1>
 __global__ void __launch_bounds__(L2P_THREADS) l2p_kernel(cheb_t ch, int leaves, int N, const int32_t *__restrict__ node_lo,
@@ -299,7 +354,9 @@ __global__ void __launch_bounds__(L2P_THREADS) l2p_kernel(cheb_t ch, int leaves,
                                                           double *__restrict__ Ez, double *__restrict__ Bx, double *__restrict__ By,
                                                           double *__restrict__ Bz)
 {
-    extern __shared__ double sm[];
+    extern __shared__ __align__(16) double sm[];
+    __shared__ int seg[L2P_SEGS];    // reaction segments of this leaf's row, in list order
+    __shared__ int nseg_s;
     constexpr int n = N1 - 1, n1 = N1, P = n1 * n1 * n1, P6 = 6 * P;
     double *Ls = sm;                 // [P][6]
     double *bas = sm + P6;           // [3][n1][L2P_THREADS]
@@ -309,7 +366,23 @@ __global__ void __launch_bounds__(L2P_THREADS) l2p_kernel(cheb_t ch, int leaves,
     const double *Ln = L + (int64_t)P6 * node;
     if (!skip_far)
         for (int e = threadIdx.x; e < P6; e += L2P_THREADS) Ls[e] = Ln[e];
+    // mutual near field: the segments holding the pairs a neighbour's block evaluated (g(x_j, x_i) = -g(x_i, x_j)); warp 0
+    // compacts the row's valid entries in list order, so that the gather below runs on independent loads
+    const int row0 = p2p_recv ? p2p_off[node] : 0, rowlen = p2p_recv ? p2p_off[node + 1] - row0 : 0;
+    if (threadIdx.x < 32) {
+        int count = 0;
+        for (int e0 = 0; e0 < rowlen; e0 += 32) {
+            const int e = e0 + threadIdx.x;
+            const int r = (e < rowlen) ? p2p_recv[row0 + e] : -1;
+            const unsigned int m = __ballot_sync(0xffffffffu, r >= 0);
+            const int at = count + __popc(m & ((1u << threadIdx.x) - 1u));
+            if (r >= 0 && at < L2P_SEGS) seg[at] = r;
+            count += __popc(m);
+        }
+        if (threadIdx.x == 0) nseg_s = count;
+    }
     __syncthreads();
+    const int nseg = nseg_s;  // (> L2P_SEGS: the row is walked entry by entry instead)
     for (int k = lo + threadIdx.x; k < hi; k += L2P_THREADS) {
         double *lx = bas + threadIdx.x, *ly = lx + n1 * L2P_THREADS, *lz = ly + n1 * L2P_THREADS;
         basis_1d(n, ch, bb[0], bb[3], tx[k], lx, L2P_THREADS);
@@ -323,8 +396,10 @@ __global__ void __launch_bounds__(L2P_THREADS) l2p_kernel(cheb_t ch, int leaves,
                 const double *row = Ls + 6 * (size_t)((a * n1 + b) * n1);
                 for (int c3 = 0; c3 < n1; ++c3) {
                     double l = lz[c3 * L2P_THREADS];
-#pragma unroll
-                    for (int f = 0; f < 6; ++f) fz[f] = fma(l, row[6 * c3 + f], fz[f]);
+                    const double2 *v = reinterpret_cast<const double2 *>(row + 6 * c3);  // (three 16-byte broadcasts)
+                    const double2 v0 = v[0], v1 = v[1], v2 = v[2];
+                    fz[0] = fma(l, v0.x, fz[0]); fz[1] = fma(l, v0.y, fz[1]); fz[2] = fma(l, v1.x, fz[2]);
+                    fz[3] = fma(l, v1.y, fz[3]); fz[4] = fma(l, v2.x, fz[4]); fz[5] = fma(l, v2.y, fz[5]);
                 }
                 double l = ly[b * L2P_THREADS];
 #pragma unroll
@@ -343,8 +418,15 @@ __global__ void __launch_bounds__(L2P_THREADS) l2p_kernel(cheb_t ch, int leaves,
             for (int kc = 1; kc < K; ++kc)
 #pragma unroll
                 for (int f = 0; f < 6; ++f) nr[f] += near_[((size_t)kc * 6 + f) * (size_t)N + k];
-        if (p2p_recv) {  // mutual near field: the pairs a neighbour's block evaluated, g(x_j, x_i) = -g(x_i, x_j), in list order
-            for (int e = p2p_off[node]; e < p2p_off[node + 1]; ++e) {
+        if (nseg <= L2P_SEGS) {
+#pragma unroll 4
+            for (int q = 0; q < nseg; ++q) {
+                const double *rp = react + (size_t)seg[q] + (size_t)(k - lo);
+#pragma unroll
+                for (int f = 0; f < 6; ++f) nr[f] -= rp[f * rstride];
+            }
+        } else {
+            for (int e = row0; e < row0 + rowlen; ++e) {
                 const int r = p2p_recv[e];
                 if (r < 0) continue;
                 const double *rp = react + (size_t)r + (size_t)(k - lo);
@@ -417,13 +499,12 @@ static int dispatch_n1(int n1, F &&f)
 int interp_m2m(fmm_plan *p)
 {
     fmm_ctx *c = &p->ctx;
-    cheb_t ch = host_cheb(p->n);
-    size_t smem = sizeof(double) * (3 * (size_t)p->n1 * p->n1 + 8 * (size_t)p->P);
+    size_t smem = sizeof(double) * (3 * (size_t)p->n1 * p->n1 + 1 + 8 * (size_t)p->P);
     FMM_TRY(dispatch_n1(p->n1, [&](auto k) { return set_smem(c, (const void *)m2m_kernel<decltype(k)::value>, smem); }));
     for (int level = p->kappa - 1; level >= 0; --level) {
         int first = 1 << level;
         FMM_TRY(dispatch_n1(p->n1, [&](auto k) {
-            m2m_kernel<decltype(k)::value><<<first, XFER_THREADS, smem, c->stream>>>(ch, first, p->node_lo, p->node_hi, p->bbox, p->M);
+            m2m_kernel<decltype(k)::value><<<first, XFER_THREADS, smem, c->stream>>>(first, p->node_lo, p->node_hi, p->node_T, p->M);
             return FMM_OK;
         }));
         FMM_LAUNCH_CHECK(c, "m2m_kernel");
@@ -434,13 +515,12 @@ int interp_m2m(fmm_plan *p)
 int interp_l2l(fmm_plan *p)
 {
     fmm_ctx *c = &p->ctx;
-    cheb_t ch = host_cheb(p->n);
-    size_t smem = sizeof(double) * (3 * (size_t)p->n1 * p->n1 + 12 * (size_t)p->P);
+    size_t smem = sizeof(double) * (3 * (size_t)p->n1 * p->n1 + 1 + 12 * (size_t)p->P);
     FMM_TRY(dispatch_n1(p->n1, [&](auto k) { return set_smem(c, (const void *)l2l_kernel<decltype(k)::value>, smem); }));
     for (int level = 1; level <= p->kappa; ++level) {
         int first = 1 << level;
         FMM_TRY(dispatch_n1(p->n1, [&](auto k) {
-            l2l_kernel<decltype(k)::value><<<first, XFER_THREADS, smem, c->stream>>>(ch, first, p->node_lo, p->node_hi, p->bbox, p->L);
+            l2l_kernel<decltype(k)::value><<<first, XFER_THREADS, smem, c->stream>>>(first, p->node_lo, p->node_hi, p->node_T, p->L);
             return FMM_OK;
         }));
         FMM_LAUNCH_CHECK(c, "l2l_kernel");

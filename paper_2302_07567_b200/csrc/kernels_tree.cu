@@ -434,6 +434,7 @@ int tree_boxes(fmm_plan *p)
     }
     node_geometry<<<(unsigned)((p->nodes + T - 1) / T), T, 0, c->stream>>>((int)p->nodes, p->hdr, p->bbox, p->node_geo);
     FMM_LAUNCH_CHECK(c, "node_geometry");
+    FMM_TRY(interp_transfer_tables(p));  // M2M / L2L matrices of the new boxes (kernels_interp.cu)
     return FMM_OK;
 }
 
