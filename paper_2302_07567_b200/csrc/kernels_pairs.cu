@@ -215,7 +215,7 @@ __device__ __forceinline__ void mut_target_sums(mut_targets<NT> &T, double m0, d
 }
 
 // `cnt` staged sources (a multiple of 32), both directions
-template <int NT, int W>
+template <int NT, int W, bool ACCUM = false>  // ACCUM: add to the segment instead of overwriting it (all-pairs kernel)
 __device__ __forceinline__ void mut_process_mutual(mut_targets<NT> &T, const mut_tile &S, int cnt, double gb, double *red,
                                                    double *__restrict__ react, size_t rstride)
 {
@@ -244,8 +244,9 @@ __device__ __forceinline__ void mut_process_mutual(mut_targets<NT> &T, const mut
         if (W == 1) {
             const int d = S.dst[b0 + lane];
             if (d >= 0) {
-                react[d] = rex; react[rstride + d] = rey; react[2 * rstride + d] = rez;
-                react[3 * rstride + d] = rbx; react[4 * rstride + d] = rby; react[5 * rstride + d] = rbz;
+                const double r6[6] = {rex, rey, rez, rbx, rby, rbz};
+#pragma unroll
+                for (int f = 0; f < 6; ++f) react[f * rstride + d] = ACCUM ? react[f * rstride + d] + r6[f] : r6[f];
             }
         } else {
             double *r = red + (size_t)warp * (6 * MUT_TILE) + b0 + lane;
@@ -261,7 +262,10 @@ __device__ __forceinline__ void mut_process_mutual(mut_targets<NT> &T, const mut
                 double v = red[q];
 #pragma unroll
                 for (int w = 1; w < W; ++w) v += red[(size_t)w * (6 * MUT_TILE) + q];
-                if (d >= 0) react[(size_t)(q / MUT_TILE) * rstride + d] = v;
+                if (d >= 0) {
+                    double *o = react + (size_t)(q / MUT_TILE) * rstride + d;
+                    *o = ACCUM ? *o + v : v;
+                }
             }
         }
     }
@@ -580,12 +584,126 @@ __global__ void direct_reduce(int64_t nt, int splits, const double *__restrict__
     Bx[k] = cB * a[3]; By[k] = cB * a[4]; Bz[k] = cB * a[5];
 }
 
+// ---------------------------------------------------------------------------------------
+// a11, mutual form (all targets, mean-gamma kernel): the particles are cut into tiles of 256 and the tiles into super-tiles of
+// G; block (a, b), a <= b, lets every tile I of super-tile a act on every tile J of super-tile b and back (J >= I on the
+// diagonal, I == J one-sided) with the same inner loops as the mutual near field.  The sums of the targets of I go to
+// tpart[block][I], the reaction on J is added to rpart[block][J] in the fixed order of the I loop (one block owns the
+// segment: no atomics); direct_mutual_reduce adds a particle's partials over the blocks of its row and column.
+// ---------------------------------------------------------------------------------------
+#define DM_NT 4
+#define DM_W 2
+__global__ void __launch_bounds__(32 * DM_W, mut_cfg<DM_NT, DM_W>::MINB) direct_mutual_kernel(
+    int64_t N, double gb, int G, int S, const double *__restrict__ x, const double *__restrict__ y, const double *__restrict__ z,
+    const double *__restrict__ w0, const double *__restrict__ w1, const double *__restrict__ w2, const double *__restrict__ w3,
+    double *__restrict__ tpart, double *__restrict__ rpart /* [blocks][6][G * 256] each */)
+{
+    __shared__ mut_tile St;
+    __shared__ double red[DM_W * 6 * MUT_TILE];
+    // block -> (a, b), a <= b: row a holds S - a blocks
+    int a = 0, rem = blockIdx.x;
+    while (rem >= S - a) { rem -= S - a; ++a; }
+    const int b = a + rem;
+    const size_t plane = (size_t)G * MUT_TILE;
+    double *tp = tpart + (size_t)blockIdx.x * 6 * plane, *rp = rpart + (size_t)blockIdx.x * 6 * plane;
+    for (int il = 0; il < G; ++il) {
+        const int64_t i0 = ((int64_t)a * G + il) * MUT_TILE;
+        mut_targets<DM_NT> T;
+#pragma unroll
+        for (int k = 0; k < DM_NT; ++k) {
+            const int64_t i = i0 + k * (32 * DM_W) + threadIdx.x;
+            const bool live = i < N;
+            T.x[k] = live ? x[i] : 0.0; T.y[k] = live ? y[i] : 0.0; T.z[k] = live ? z[i] : 0.0;
+            T.q0[k] = live ? w0[i] : 0.0; T.q1[k] = live ? w1[i] : 0.0; T.q2[k] = live ? w2[i] : 0.0; T.q3[k] = live ? w3[i] : 0.0;
+            T.ex[k] = T.ey[k] = T.ez[k] = T.bx[k] = T.by[k] = T.bz[k] = 0.0;
+        }
+        if (i0 < N) {
+            for (int jl = (a == b ? il : 0); jl < G; ++jl) {
+                const int64_t j0 = ((int64_t)b * G + jl) * MUT_TILE;
+                if (j0 >= N) break;
+                __syncthreads();
+                for (int j = threadIdx.x; j < MUT_TILE; j += 32 * DM_W) {  // (dead sources: zero weights)
+                    const int64_t g = j0 + j;
+                    const bool live = g < N;
+                    St.x[j] = live ? x[g] : 0.0; St.y[j] = live ? y[g] : 0.0; St.z[j] = live ? z[g] : 0.0;
+                    St.m0[j] = live ? w0[g] : 0.0; St.m1[j] = live ? w1[g] : 0.0; St.m2[j] = live ? w2[g] : 0.0; St.m3[j] = live ? w3[g] : 0.0;
+                    St.dst[j] = jl * MUT_TILE + j;
+                }
+                __syncthreads();
+                // the reaction segment of J is written by the first tile I that meets it (il == 0) and added to afterwards
+                if (a == b && il == jl) mut_process_onesided<DM_NT>(T, St, MUT_TILE, gb);
+                else if (il == 0) mut_process_mutual<DM_NT, DM_W, false>(T, St, MUT_TILE, gb, red, rp, plane);
+                else mut_process_mutual<DM_NT, DM_W, true>(T, St, MUT_TILE, gb, red, rp, plane);
+            }
+        }
+#pragma unroll
+        for (int k = 0; k < DM_NT; ++k) {
+            const int q = il * MUT_TILE + k * (32 * DM_W) + threadIdx.x;
+            tp[q] = T.ex[k]; tp[plane + q] = T.ey[k]; tp[2 * plane + q] = T.ez[k];
+            tp[3 * plane + q] = T.bx[k]; tp[4 * plane + q] = T.by[k]; tp[5 * plane + q] = T.bz[k];
+        }
+    }
+}
+
+__global__ void direct_mutual_reduce(int64_t N, int G, int S, const double *__restrict__ tpart, const double *__restrict__ rpart, double cE,
+                                     double cB, double *__restrict__ Ex, double *__restrict__ Ey, double *__restrict__ Ez,
+                                     double *__restrict__ Bx, double *__restrict__ By, double *__restrict__ Bz)
+{
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= N) return;
+    const size_t plane = (size_t)G * MUT_TILE;
+    const int s = (int)(i / (int64_t)plane);
+    const size_t q = (size_t)(i - (int64_t)s * (int64_t)plane);
+    auto block_of = [&](int a, int b) { return (size_t)a * S - (size_t)a * (a - 1) / 2 + (size_t)(b - a); };
+    double acc[6] = {0, 0, 0, 0, 0, 0};
+    for (int b = s; b < S; ++b) {  // this particle as a target: blocks (s, b)
+        const double *p = tpart + block_of(s, b) * 6 * plane + q;
+#pragma unroll
+        for (int f = 0; f < 6; ++f) acc[f] += p[f * plane];
+    }
+    // ... and as a source: the reaction sums of blocks (c, s), g(x_j, x_i) = -g(x_i, x_j).  On the diagonal block the first tile
+    // of the super-tile receives nothing (its segment is never written): tiles J > I only.
+    for (int c = 0; c <= s; ++c) {
+        if (c == s && q < MUT_TILE) continue;
+        const double *p = rpart + block_of(c, s) * 6 * plane + q;
+#pragma unroll
+        for (int f = 0; f < 6; ++f) acc[f] -= p[f * plane];
+    }
+    Ex[i] = cE * acc[0]; Ey[i] = cE * acc[1]; Ez[i] = cE * acc[2];
+    Bx[i] = cB * acc[3]; By[i] = cB * acc[4]; Bz[i] = cB * acc[5];
+}
+
 int pairs_direct(fmm_ctx *c, int64_t N, const double *x, const double *y, const double *z,
                  const double *w0, const double *w1, const double *w2, const double *w3,
                  const double *px, const double *py, const double *pz,
                  double gamma_bar, int raw, int64_t nt, const int64_t *tidx,
                  double *Ex, double *Ey, double *Ez, double *Bx, double *By, double *Bz)
 {
+    double cE = 1.0, cB = 1.0;
+    if (!raw) {
+        cE = 1.0 / (4.0 * FMM_PI * FMM_EPS0);
+        cB = 1.0 / (4.0 * FMM_PI * FMM_EPS0 * FMM_C0);
+    }
+    if (!px && !tidx && nt == N && N >= 8 * MUT_TILE) {  // all targets, kernel of eq. (3.2): every pair once for both directions
+        const int64_t tiles = (N + MUT_TILE - 1) / MUT_TILE;
+        int G = (int)(tiles / 64);
+        if (G < 1) G = 1;
+        if (G > 32) G = 32;
+        const int S = (int)((tiles + G - 1) / G);
+        const int64_t blocks = (int64_t)S * (S + 1) / 2;
+        const size_t bytes = sizeof(double) * 6 * (size_t)G * MUT_TILE * (size_t)blocks;
+        if (2 * bytes <= ((size_t)8 << 30) && blocks < ((int64_t)1 << 31)) {
+            double *tp = (double *)ctx_alloc(c, bytes), *rp = (double *)ctx_alloc(c, bytes);
+            if (!tp || !rp) return FMM_ENOMEM;
+            direct_mutual_kernel<<<(unsigned)blocks, 32 * DM_W, 0, c->stream>>>(N, gamma_bar, G, S, x, y, z, w0, w1, w2, w3, tp, rp);
+            FMM_LAUNCH_CHECK(c, "direct_mutual_kernel");
+            direct_mutual_reduce<<<(unsigned)((N + 255) / 256), 256, 0, c->stream>>>(N, G, S, tp, rp, cE, cB, Ex, Ey, Ez, Bx, By, Bz);
+            FMM_LAUNCH_CHECK(c, "direct_mutual_reduce");
+            ctx_free(c, rp);
+            ctx_free(c, tp);
+            return FMM_OK;
+        }
+    }
     int64_t tblocks = (nt + DIRECT_TARGETS - 1) / DIRECT_TARGETS;
     // enough blocks for ~8 waves of 148 SMs x 4 resident blocks, source slices in whole tiles
     int64_t want = 8 * 4 * FMM_SM_COUNT;
@@ -604,11 +722,6 @@ int pairs_direct(fmm_ctx *c, int64_t N, const double *x, const double *y, const 
     else
         direct_kernel<false><<<grid, DIRECT_THREADS, 0, c->stream>>>(N, gamma_bar, nt, tidx, chunk, x, y, z, w0, w1, w2, w3, px, py, pz, part);
     FMM_LAUNCH_CHECK(c, "direct_kernel");
-    double cE = 1.0, cB = 1.0;
-    if (!raw) {
-        cE = 1.0 / (4.0 * FMM_PI * FMM_EPS0);
-        cB = 1.0 / (4.0 * FMM_PI * FMM_EPS0 * FMM_C0);
-    }
     direct_reduce<<<(unsigned)((nt + 255) / 256), 256, 0, c->stream>>>(nt, (int)splits, part, cE, cB, Ex, Ey, Ez, Bx, By, Bz);
     FMM_LAUNCH_CHECK(c, "direct_reduce");
     ctx_free(c, part);

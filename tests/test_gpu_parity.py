@@ -499,3 +499,23 @@ def test_kd_sort_key_ties(fmm, kind):
     Eo, Bo = op.eval()
     assert_close(E, Eo, "E")
     plan.close()
+
+
+@pytest.mark.parametrize("N", [2048, 5003, 70001])
+def test_direct_all_targets_mutual_form(fmm, N):
+    """fmm_direct with all N targets evaluates every particle pair once for both directions (tiles of 256 in super-tiles,
+    kernels_pairs.cu direct_mutual_kernel): ragged last tile, ragged last super-tile, first / diagonal / off-diagonal blocks.
+    Compared with the oracle's direct sum on a seeded sample of targets."""
+    w = workloads.config(4, N=N)
+    q = np.random.default_rng(17).uniform(0.5, 2.0, N) * workloads.ELECTRON_CHARGE
+    gb = oracle.gamma_bar(w.px, w.py, w.pz)
+    E, B = to_np(fmm.fmm_direct(*w.arrays(), q, gamma_bar=gb))
+    idx = np.sort(np.random.default_rng(18).choice(N, size=min(N, 1500), replace=False)).astype(np.int64)
+    idx[:4] = [0, 255, 256, N - 1][: len(idx[:4])]
+    Eo, Bo = oracle.direct(*w.arrays(), q, gamma_bar_value=gb, targets=idx)
+    assert_close(E[idx], Eo, "direct (mutual form) E")
+    assert_close(B[idx], Bo, "direct (mutual form) B")
+    # and identical to the one-sided kernel (targets given explicitly) up to summation order
+    E1, B1 = to_np(fmm.fmm_direct(*w.arrays(), q, gamma_bar=gb, targets=idx))
+    assert_close(E[idx], E1, "mutual vs one-sided direct E")
+    assert_close(B[idx], B1, "mutual vs one-sided direct B")
