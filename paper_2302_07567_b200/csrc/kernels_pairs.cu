@@ -686,7 +686,7 @@ int pairs_direct(fmm_ctx *c, int64_t N, const double *x, const double *y, const 
     }
     if (!px && !tidx && nt == N && N >= 8 * MUT_TILE) {  // all targets, kernel of eq. (3.2): every pair once for both directions
         const int64_t tiles = (N + MUT_TILE - 1) / MUT_TILE;
-        int G = (int)(tiles / 64);
+        int G = (int)(tiles / 128);  // (about 8,000 blocks: enough to level the half-size diagonal blocks out)
         if (G < 1) G = 1;
         if (G > 32) G = 32;
         const int S = (int)((tiles + G - 1) / G);
