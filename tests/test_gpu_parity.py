@@ -519,3 +519,25 @@ def test_direct_all_targets_mutual_form(fmm, N):
     E1, B1 = to_np(fmm.fmm_direct(*w.arrays(), q, gamma_bar=gb, targets=idx))
     assert_close(E[idx], E1, "mutual vs one-sided direct E")
     assert_close(B[idx], B1, "mutual vs one-sided direct B")
+
+
+@pytest.mark.parametrize("shift,axis,tol", [(1.0, 2, 1e-12), (1.0, 0, 1e-12), (100.0, 2, 1e-10), (100.0, 0, 1e-10)])
+def test_displaced_bunch(fmm, shift, axis, tol):
+    """positions far from the origin (a lab-frame offset of metres for a millimetre bunch).  The fields depend on
+    differences only, but the M2L z trick works with box-centre-relative proxy offsets whose rounding grows with |z0|
+    (DESIGN.md section 9): 1e-12 holds for |offset| / extent up to about 1e3, at 1e5 the documented bound is 1e-10."""
+    w = workloads.config(2, N=20000)
+    pos = [w.x.copy(), w.y.copy(), w.z.copy()]
+    pos[axis] += shift
+    plan = fmm.fmm_plan_create(*pos, w.px, w.py, w.pz, w.q, order_n=5, leaf_size=128, theta=0.5)
+    st = plan.stats()
+    E, B = to_np(plan.eval())
+    ex = plan.export()
+    op = oracle.Plan(*pos, w.px, w.py, w.pz, w.q, order_n=5, leaf_size=128, theta=0.5, gamma_bar_value=st["gamma_bar"])
+    assert np.array_equal(ex["perm"], op.perm())
+    p2p, m2l = op.lists()
+    assert np.array_equal(ex["p2p_src"], p2p[:, 1]) and np.array_equal(ex["m2l_src"], m2l[:, 1])
+    Eo, Bo = op.eval()
+    assert_close(E, Eo, f"E, bunch displaced by {shift} m along axis {axis}", tol)
+    assert_close(B, Bo, f"B, bunch displaced by {shift} m along axis {axis}", tol)
+    plan.close()
