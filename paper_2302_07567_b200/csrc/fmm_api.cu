@@ -203,6 +203,8 @@ static int plan_alloc_fixed(fmm_plan *p)
     ALLOC(node_lo, int32_t, nodes1); ALLOC(node_hi, int32_t, nodes1);
     ALLOC(bbox, double, 6 * nodes1); ALLOC(node_geo, double, 4 * nodes1);
     ALLOC(node_xi, double, 48 * nodes1);
+    ALLOC(xfer_sync, int, 2 * nodes1);
+    if (cudaMemsetAsync(p->xfer_sync, 0, sizeof(int) * 2 * nodes1, c->stream) != cudaSuccess) return FMM_ECUDA;
     ALLOC(node_T, double, (size_t)((3 * p->n1 * p->n1 + 1) & ~1) * nodes1);
     ALLOC(p2p_off, int32_t, nodes1 + 1); ALLOC(m2l_off, int32_t, nodes1 + 1);
     ALLOC(p2p_order, int32_t, nodes1); ALLOC(m2l_order, int32_t, nodes1);

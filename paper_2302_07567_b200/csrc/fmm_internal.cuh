@@ -95,6 +95,8 @@ struct fmm_plan {
     double *bbox;           // [nodes+1][6]
     double *node_geo;       // [nodes+1][4] : r^2 (Alg 5.6 squared), cx, cy, cz (box centres)
     double *node_T;         // [nodes+2][3 (n+1)^2 rounded up to even] 1-D transfer matrices child <- parent, filled per build
+    int *xfer_sync;         // [2][nodes+2] M2M arrival counters (zero between evaluations), L2L stamps
+    int xfer_stamp;         // stamp of the last L2L launch
     double *node_xi;        // [nodes+1][3][16] : proxy points per axis (I-3), filled by pairs_m2l
     // interaction lists, CSR by target node id (offset arrays indexed by node id, length nodes+2)
     int32_t *p2p_off, *p2p_src, *m2l_off, *m2l_src;

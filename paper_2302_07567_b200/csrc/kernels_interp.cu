@@ -192,17 +192,22 @@ int interp_transfer_tables(fmm_plan *p)
 // ---------------------------------------------------------------------------------------
 #define XFER_THREADS 256
 
+// The whole upward pass is ONE launch: a block starts at a parent of two leaves; when a node is finished the block counts
+// itself into the node's parent, and the second of the two siblings to arrive (both children are then complete) goes on with
+// the parent.  No grid barrier, no launch per level: the dependency chain of the kappa levels costs a few microseconds per
+// level.  The result does not depend on which sibling arrives last (child 0 is always added before child 1).
 template <int N1>
 __global__ void __launch_bounds__(XFER_THREADS) m2m_kernel(int first, const int32_t *__restrict__ node_lo,
                                                            const int32_t *__restrict__ node_hi, const double *__restrict__ tab,
-                                                           double *__restrict__ M)
+                                                           double *M, int *arrive /* [nodes + 2], zero between evaluations */)
 {
     extern __shared__ __align__(16) double sm[];
+    __shared__ int s_prev;
     constexpr int n1 = N1, P = n1 * n1 * n1, P4 = 4 * P, TS = (3 * n1 * n1 + 1) & ~1;  // compile-time order: index arithmetic without integer division
     double *T = sm;                              // [3][n1][n1]
     double *A = sm + TS;                         // [P][4], 16-byte aligned
     double *B = A + P4;                          // [P][4]
-    int S = first + blockIdx.x;
+    for (int S = first + blockIdx.x; S >= 1; S >>= 1) {
     double *MS = M + (int64_t)P4 * S;
     // parent accumulators live in registers across the two children: element e = threadIdx.x + k*blockDim
     for (int e0 = 0; e0 < P4; e0 += XFER_THREADS * 8) {
@@ -216,7 +221,7 @@ __global__ void __launch_bounds__(XFER_THREADS) m2m_kernel(int first, const int3
             __syncthreads();
             for (int e = threadIdx.x; e < 3 * n1 * n1; e += XFER_THREADS) T[e] = tab[(size_t)C * TS + e];
             const double *MC = M + (int64_t)P4 * C;
-            for (int e = threadIdx.x; e < P4; e += XFER_THREADS) A[e] = MC[e];
+            for (int e = threadIdx.x; e < P4; e += XFER_THREADS) A[e] = __ldcg(MC + e);  // (written by another block of this launch: past L1)
             __syncthreads();
             const double *Tx = T, *Ty = T + n1 * n1, *Tz = T + 2 * n1 * n1;
             // z: B[a',b',c] = sum_c' Tz[c][c'] A[a',b',c']   (a thread takes a proxy point with its four moments: the moments
@@ -269,16 +274,32 @@ __global__ void __launch_bounds__(XFER_THREADS) m2m_kernel(int first, const int3
             if (e < P4) MS[e] = acc[k8];
         }
     }
+    // node S is complete: make it visible, then count into the parent; the first sibling to arrive stops here
+    if (S == 1) break;
+    __threadfence();
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        const int prev = atomicAdd(&arrive[S >> 1], 1);
+        if (prev == 1) arrive[S >> 1] = 0;  // (both are here: leave the counter clean for the next evaluation)
+        __threadfence();
+        s_prev = prev;
+    }
+    __syncthreads();
+    if (s_prev == 0) break;
+    }
 }
 
 // ---------------------------------------------------------------------------------------
 // a8: L2L for one level.  One block per child S' (parent S = S'/2):
 //   L_S'[a',b',c'] += sum_{a,b,c} Tx[a][a'] Ty[b][b'] Tz[c][c'] L_S[a,b,c]
 // ---------------------------------------------------------------------------------------
+// The whole downward pass is ONE launch over the nodes 2 .. nodes in heap order: a block waits until its parent carries this
+// evaluation's stamp, adds the parent's field and stamps its own node.  A block only ever waits for a block with a smaller
+// index, and the blocks of a 1-D grid start in index order, so the block it waits for is running or done.
 template <int N1>
-__global__ void __launch_bounds__(XFER_THREADS) l2l_kernel(int first, const int32_t *__restrict__ node_lo,
+__global__ void __launch_bounds__(XFER_THREADS) l2l_kernel(int first, int leaves, int stamp, const int32_t *__restrict__ node_lo,
                                                            const int32_t *__restrict__ node_hi, const double *__restrict__ tab,
-                                                           double *__restrict__ L)
+                                                           double *L, int *ready /* [nodes + 2] */)
 {
     extern __shared__ __align__(16) double sm[];
     constexpr int n1 = N1, P = n1 * n1 * n1, P6 = 6 * P, TS = (3 * n1 * n1 + 1) & ~1;
@@ -286,11 +307,18 @@ __global__ void __launch_bounds__(XFER_THREADS) l2l_kernel(int first, const int3
     double *A = sm + TS;  // [P][6], 16-byte aligned
     double *B = A + P6;
     int C = first + blockIdx.x, S = C >> 1;
-    if (node_hi[C] <= node_lo[C]) return;
+    if (node_hi[C] <= node_lo[C]) return;  // (its descendants are empty too: nobody waits for it)
     for (int e = threadIdx.x; e < 3 * n1 * n1; e += XFER_THREADS) T[e] = tab[(size_t)C * TS + e];
+    if (S > 1) {
+        if (threadIdx.x == 0) {
+            while (*((volatile int *)&ready[S]) != stamp) {}
+            __threadfence();
+        }
+        __syncthreads();
+    }
     const double *LS = L + (int64_t)P6 * S;
     double *LC = L + (int64_t)P6 * C;
-    for (int e = threadIdx.x; e < P6; e += XFER_THREADS) A[e] = LS[e];
+    for (int e = threadIdx.x; e < P6; e += XFER_THREADS) A[e] = __ldcg(LS + e);  // (written by another block of this launch: past L1)
     __syncthreads();
     const double *Tx = T, *Ty = T + n1 * n1, *Tz = T + 2 * n1 * n1;
     // z: B[a,b,c'] = sum_c Tz[c][c'] A[a,b,c]   (a thread takes a proxy point with its six field components: three 16-byte
@@ -332,6 +360,11 @@ __global__ void __launch_bounds__(XFER_THREADS) l2l_kernel(int first, const int3
         double s = 0.0;
         for (int k = 0; k < n1; ++k) s = fma(Tx[k * n1 + a], A[6 * (k * n1 * n1 + bc) + f], s);
         LC[e] += s;
+    }
+    if (C < leaves) {  // an inner node: its children wait for this stamp
+        __threadfence();
+        __syncthreads();
+        if (threadIdx.x == 0) *((volatile int *)&ready[C]) = stamp;
     }
 }
 
@@ -499,32 +532,32 @@ static int dispatch_n1(int n1, F &&f)
 int interp_m2m(fmm_plan *p)
 {
     fmm_ctx *c = &p->ctx;
+    if (p->kappa < 1) return FMM_OK;
     size_t smem = sizeof(double) * (3 * (size_t)p->n1 * p->n1 + 1 + 8 * (size_t)p->P);
     FMM_TRY(dispatch_n1(p->n1, [&](auto k) { return set_smem(c, (const void *)m2m_kernel<decltype(k)::value>, smem); }));
-    for (int level = p->kappa - 1; level >= 0; --level) {
-        int first = 1 << level;
-        FMM_TRY(dispatch_n1(p->n1, [&](auto k) {
-            m2m_kernel<decltype(k)::value><<<first, XFER_THREADS, smem, c->stream>>>(first, p->node_lo, p->node_hi, p->node_T, p->M);
-            return FMM_OK;
-        }));
-        FMM_LAUNCH_CHECK(c, "m2m_kernel");
-    }
+    const int first = 1 << (p->kappa - 1);  // one block per parent of two leaves; it climbs as long as it is the second to arrive
+    FMM_TRY(dispatch_n1(p->n1, [&](auto k) {
+        m2m_kernel<decltype(k)::value><<<first, XFER_THREADS, smem, c->stream>>>(first, p->node_lo, p->node_hi, p->node_T, p->M, p->xfer_sync);
+        return FMM_OK;
+    }));
+    FMM_LAUNCH_CHECK(c, "m2m_kernel");
     return FMM_OK;
 }
 
 int interp_l2l(fmm_plan *p)
 {
     fmm_ctx *c = &p->ctx;
+    if (p->kappa < 1) return FMM_OK;
     size_t smem = sizeof(double) * (3 * (size_t)p->n1 * p->n1 + 1 + 12 * (size_t)p->P);
     FMM_TRY(dispatch_n1(p->n1, [&](auto k) { return set_smem(c, (const void *)l2l_kernel<decltype(k)::value>, smem); }));
-    for (int level = 1; level <= p->kappa; ++level) {
-        int first = 1 << level;
-        FMM_TRY(dispatch_n1(p->n1, [&](auto k) {
-            l2l_kernel<decltype(k)::value><<<first, XFER_THREADS, smem, c->stream>>>(first, p->node_lo, p->node_hi, p->node_T, p->L);
-            return FMM_OK;
-        }));
-        FMM_LAUNCH_CHECK(c, "l2l_kernel");
-    }
+    p->xfer_stamp = (p->xfer_stamp >= (1 << 30)) ? 1 : p->xfer_stamp + 1;
+    int *ready = p->xfer_sync + (p->nodes + 2);
+    FMM_TRY(dispatch_n1(p->n1, [&](auto k) {
+        l2l_kernel<decltype(k)::value><<<(unsigned)(p->nodes - 1), XFER_THREADS, smem, c->stream>>>(2, (int)p->leaves, p->xfer_stamp, p->node_lo, p->node_hi,
+                                                                                                   p->node_T, p->L, ready);
+        return FMM_OK;
+    }));
+    FMM_LAUNCH_CHECK(c, "l2l_kernel");
     return FMM_OK;
 }
 
