@@ -479,7 +479,8 @@ __global__ void __launch_bounds__(L2P_THREADS) l2p_kernel(cheb_t ch, int leaves,
 // ---------------------------------------------------------------------------------------
 static int set_smem(fmm_ctx *c, const void *fn, size_t bytes)
 {
-    if (bytes > 48 * 1024) FMM_CUDA(c, cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes));
+    // (dynamic + static shared memory count against the 48 KB default: opt in a little below it)
+    if (bytes > 40 * 1024) FMM_CUDA(c, cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes));
     return FMM_OK;
 }
 

@@ -541,3 +541,17 @@ def test_displaced_bunch(fmm, shift, axis, tol):
     assert_close(E, Eo, f"E, bunch displaced by {shift} m along axis {axis}", tol)
     assert_close(B, Bo, f"B, bunch displaced by {shift} m along axis {axis}", tol)
     plan.close()
+
+
+@pytest.mark.parametrize("n", [7, 11])
+def test_orders_at_the_shared_memory_opt_in_boundary(fmm, n):
+    """n = 7: the L2P kernel needs exactly 48 KB of dynamic shared memory beside 1 KB of static (the default limit counts
+    both); n = 11 sits between the other cases of the order sweep."""
+    w = workloads.config(3, N=4000)
+    plan = fmm.fmm_plan_create(*w.arrays(), w.q, order_n=n, leaf_size=256, theta=0.5)
+    st = plan.stats()
+    E, B = to_np(plan.eval())
+    Eo, Bo = oracle.Plan(*w.arrays(), w.q, order_n=n, leaf_size=256, theta=0.5, gamma_bar_value=st["gamma_bar"]).eval()
+    assert_close(E, Eo, "E")
+    assert_close(B, Bo, "B")
+    plan.close()
