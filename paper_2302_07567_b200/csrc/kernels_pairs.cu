@@ -404,7 +404,10 @@ static void p2p_shape(int64_t leaves, int maxleaf, int64_t pairs, int64_t max_ro
     // Row split K: (a) enough warps in flight when there are few leaves, (b) no single row longer than a quarter of an
     // SM's fair share of the whole near field (the tail leaves of a Gaussian bunch have rows of several hundred leaves).
     double warps = (double)leaves * (best_threads / 32);
-    int k_fill = (int)((8.0 * FMM_SM_COUNT + warps - 1) / warps);
+    // four waves of resident warps: with few leaves (N = 65,536: 512 one-warp blocks) the last wave otherwise runs a third
+    // empty (P2P 48 % -> 62 % of peak there, profiles/r02_bench_configs.md)
+    const double K_FILL_WAVES = 4.0;
+    int k_fill = (int)((K_FILL_WAVES * 8.0 * FMM_SM_COUNT + warps - 1) / warps);
     double fair = (double)pairs / (4.0 * FMM_SM_COUNT);
     int k_bal = (fair > 0.0) ? (int)((double)max_row / fair + 0.999) : 1;
     int K = k_fill > k_bal ? k_fill : k_bal;
@@ -422,7 +425,7 @@ int pairs_m2l_prepare(fmm_plan *p)  // after the lists: M2L row split for small 
         // buffers stay below 256 MB.
         int64_t want = 4 * 2 * FMM_SM_COUNT;
         K = (int)((want + p->nodes - 1) / p->nodes);
-        if (K > 4) K = 4;
+        if (K > 8) K = 8;
         if (K < 1) K = 1;
         while (K > 1 && (int64_t)(K - 1) * 48 * p->P * (p->nodes + 2) > ((int64_t)256 << 20)) --K;
     }
