@@ -382,7 +382,7 @@ static void p2p_shape(int64_t leaves, int maxleaf, int64_t pairs, int64_t max_ro
     double best_score = -1.0;
     if (mutual && maxleaf <= 1024) {
         // W a power of two: the resident warps of an SM then split evenly over its four sub-partitions (three warps per
-        // block left one sub-partition with 3 of 9 warps: 46 % instead of 60 % of peak at leaves of 312, profiles/r02_bench_configs.md)
+        // block left one sub-partition with 3 of 9 warps: 46 % instead of 59 % of peak at leaves of 312, profiles/r02_sweep_paper.md)
         int W = 1;
         while (32 * 4 * W < maxleaf) W *= 2;
         best_threads = 32 * W;
