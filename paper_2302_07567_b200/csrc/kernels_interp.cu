@@ -397,8 +397,22 @@ __global__ void __launch_bounds__(L2P_THREADS) l2p_kernel(cheb_t ch, int leaves,
     int lo = node_lo[node], hi = node_hi[node];
     const double *bb = bbox + 6 * (int64_t)node;
     const double *Ln = L + (int64_t)P6 * node;
-    if (!skip_far)
-        for (int e = threadIdx.x; e < P6; e += L2P_THREADS) Ls[e] = Ln[e];
+    if (!skip_far) {  // the leaf's local field: all loads of a thread first (one memory round trip), 16-byte words
+        constexpr int W2 = P6 / 2, PER = (W2 + L2P_THREADS - 1) / L2P_THREADS;  // (6 P doubles: an even number)
+        const double2 *src2 = reinterpret_cast<const double2 *>(Ln);
+        double2 *dst2 = reinterpret_cast<double2 *>(Ls);
+        double2 v[PER];
+#pragma unroll
+        for (int k = 0; k < PER; ++k) {
+            const int e = threadIdx.x + k * L2P_THREADS;
+            if (e < W2) v[k] = src2[e];
+        }
+#pragma unroll
+        for (int k = 0; k < PER; ++k) {
+            const int e = threadIdx.x + k * L2P_THREADS;
+            if (e < W2) dst2[e] = v[k];
+        }
+    }
     // mutual near field: the segments holding the pairs a neighbour's block evaluated (g(x_j, x_i) = -g(x_i, x_j)); warp 0
     // compacts the row's valid entries in list order, so that the gather below runs on independent loads
     const int row0 = p2p_recv ? p2p_off[node] : 0, rowlen = p2p_recv ? p2p_off[node + 1] - row0 : 0;
@@ -452,7 +466,7 @@ __global__ void __launch_bounds__(L2P_THREADS) l2p_kernel(cheb_t ch, int leaves,
 #pragma unroll
                 for (int f = 0; f < 6; ++f) nr[f] += near_[((size_t)kc * 6 + f) * (size_t)N + k];
         if (nseg <= L2P_SEGS) {
-#pragma unroll 4
+#pragma unroll 8
             for (int q = 0; q < nseg; ++q) {
                 const double *rp = react + (size_t)seg[q] + (size_t)(k - lo);
 #pragma unroll
