@@ -220,7 +220,7 @@ static int plan_build(fmm_plan *p, const fmm_particles_t *in, bool refit = false
     p->valid = 0;  // a build that fails part-way leaves lists that must not be used (fmm_eval then returns FMM_EINVAL)
     // scratch of the whole build from one arena block: sort keys and index lists of the tree (about 100 N bytes), frontier
     // and pair buffers of the traversal; sized from the last build once there was one
-    const size_t estimate = (size_t)120 * (size_t)p->N + (size_t)64 * (size_t)(p->list_cap > 0 ? p->list_cap : p->leaves * 128) +
+    const size_t estimate = (size_t)(p->N >= ((int64_t)1 << 21) ? 184 : 120) * (size_t)p->N + (size_t)64 * (size_t)(p->list_cap > 0 ? p->list_cap : p->leaves * 128) +
                             (size_t)64 * (size_t)p->nodes + ((size_t)4 << 20);
     FMM_TRY(ctx_arena_begin(c, estimate));
     struct arena_guard { fmm_ctx *c; ~arena_guard() { ctx_arena_end(c); } } guard{c};
