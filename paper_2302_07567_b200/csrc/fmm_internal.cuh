@@ -81,6 +81,7 @@ struct fmm_plan {
     int64_t nodes, leaves;
     double theta, gamma_bar, gamma_bar_param;
     fmm_hdr *hdr;           // device
+    int ranges_done;        // node_lo / node_hi are filled (they depend on N and N0 only)
     int kd_exact;           // KD build with the exact 64-bit sort keys (set once the quantised keys were not enough)
     int kd_retry;           // the last build asked for that
     int valid;              // 0 after a failed build: fmm_eval refuses the plan until an update / refit succeeds

@@ -369,6 +369,51 @@ __global__ void list_work_keys(const dtt_counters *__restrict__ cnt, int first, 
     vals[k] = (uint32_t)t;
 }
 
+// The same order by ONE block (counting sort on the 8-bit code) for small lists (up to LIST_ORDER_SMALL targets; slower than the sort beyond): five launches less per
+// list.  Targets of equal code come out in arbitrary order: the order only schedules blocks, it never enters the arithmetic.
+#define LIST_ORDER_SMALL 1024
+__global__ void __launch_bounds__(1024) list_order_small(const dtt_counters *__restrict__ cnt, int first, int count, const int32_t *__restrict__ off,
+                                                         const int32_t *__restrict__ src, const int32_t *__restrict__ node_lo,
+                                                         const int32_t *__restrict__ node_hi, int by_size, const int32_t *__restrict__ dst,
+                                                         int32_t *__restrict__ order)
+{
+    __shared__ int hist[256], cursor[256];
+    for (int k = threadIdx.x; k < 256; k += blockDim.x) hist[k] = 0;
+    __syncthreads();
+    const bool bad = cnt->overflow != 0;
+    auto code = [&](int t) -> int {
+        unsigned long long work = 0;
+        if (bad) {
+            work = 0;
+        } else if (by_size) {
+            for (int e = off[t]; e < off[t + 1]; ++e)
+                work += (unsigned long long)(node_hi[src[e]] - node_lo[src[e]]) * (unsigned long long)(!dst ? 25 : (dst[e] >= 0 ? 34 : (dst[e] == -1 ? 25 : 0)));
+        } else {
+            work = (unsigned long long)(off[t + 1] - off[t]);
+        }
+        unsigned int wq = 0;
+        if (work > 0) {
+            int e = 63 - __clzll((long long)work);
+            if (e > 30) e = 30;
+            unsigned long long mant = (e >= 3) ? (work >> (e - 3)) : (work << (3 - e));
+            if (mant > 15) mant = 15;
+            wq = (((unsigned int)e << 3) | (unsigned int)(mant & 7ull)) + 1;
+        }
+        return 255 - (int)wq;  // ascending code = descending work
+    };
+    for (int k = threadIdx.x; k < count; k += blockDim.x) atomicAdd(&hist[code(first + k)], 1);
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        int run = 0;
+        for (int d = 0; d < 256; ++d) { cursor[d] = run; run += hist[d]; }
+    }
+    __syncthreads();
+    for (int k = threadIdx.x; k < count; k += blockDim.x) {
+        const int t = first + k;
+        order[atomicAdd(&cursor[code(t)], 1)] = t;
+    }
+}
+
 __global__ void copy_u32_to_i32(int n, const uint32_t *__restrict__ a, int32_t *__restrict__ b)
 {
     int k = blockIdx.x * blockDim.x + threadIdx.x;
@@ -379,6 +424,11 @@ static int make_order(fmm_plan *p, const dtt_counters *cnt, int first, int count
                       const int32_t *dst, int32_t *order_out)
 {
     fmm_ctx *c = &p->ctx;
+    if (count <= LIST_ORDER_SMALL) {
+        list_order_small<<<1, 1024, 0, c->stream>>>(cnt, first, count, off, src, p->node_lo, p->node_hi, by_size, dst, order_out);
+        FMM_LAUNCH_CHECK(c, "list_order_small");
+        return FMM_OK;
+    }
     uint64_t *keys = (uint64_t *)ctx_alloc(c, sizeof(uint64_t) * count);
     uint64_t *tkeys = (uint64_t *)ctx_alloc(c, sizeof(uint64_t) * count);
     uint32_t *vals = (uint32_t *)ctx_alloc(c, sizeof(uint32_t) * count);

@@ -147,6 +147,45 @@ __global__ void kd_fix_runs(int N, const double *__restrict__ x, const double *_
 }
 
 // ---------------------------------------------------------------------------------------
+// small bunches (N <= KD_LOCAL): the three sorts in one launch, one block per axis, bitonic network in shared memory on the
+// exact (coordinate key, index) pairs -- the 4-pass radix sort is 16 launches, which at N = 4,096 is most of the tree time
+// ---------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(1024) kd_sort_small(int N, int npow2, const double *__restrict__ x, const double *__restrict__ y,
+                                                      const double *__restrict__ z, uint32_t *__restrict__ lists /* [4 N] */)
+{
+    extern __shared__ __align__(16) unsigned char kss_raw[];
+    uint64_t *key = reinterpret_cast<uint64_t *>(kss_raw);          // [npow2]
+    uint32_t *val = reinterpret_cast<uint32_t *>(key + npow2);      // [npow2]
+    const int a = blockIdx.x;
+    const double *coord = (a == 0) ? x : (a == 1) ? y : z;
+    for (int i = threadIdx.x; i < npow2; i += blockDim.x) {
+        key[i] = (i < N) ? sortable_key(coord[i]) : ~0ull;  // padding sorts last (index beyond every particle)
+        val[i] = (uint32_t)i;
+    }
+    if (a == 0)
+        for (int i = threadIdx.x; i < N; i += blockDim.x) lists[3 * (size_t)N + i] = (uint32_t)i;
+    __syncthreads();
+    for (int k = 2; k <= npow2; k <<= 1) {
+        for (int j = k >> 1; j > 0; j >>= 1) {
+            for (int i = threadIdx.x; i < npow2; i += blockDim.x) {
+                const int l = i ^ j;
+                if (l > i) {
+                    const uint64_t ki = key[i], kl = key[l];
+                    const uint32_t vi = val[i], vl = val[l];
+                    const bool greater = (ki > kl) || (ki == kl && vi > vl);  // (coordinate, index): a total order
+                    if (greater == ((i & k) == 0)) {
+                        key[i] = kl; key[l] = ki;
+                        val[i] = vl; val[l] = vi;
+                    }
+                }
+            }
+            __syncthreads();
+        }
+    }
+    for (int i = threadIdx.x; i < N; i += blockDim.x) lists[(size_t)a * N + i] = val[i];
+}
+
+// ---------------------------------------------------------------------------------------
 // one level on the whole lists (nodes larger than KD_LOCAL: a tile of KD_TILE entries meets at most two nodes)
 // ---------------------------------------------------------------------------------------
 // Alg 5.2 (readings G7, G8): in the list of the split axis the first ceil(size/2) members of the
@@ -517,7 +556,14 @@ int kd_build_order(fmm_plan *p, const fmm_particles_t *in, uint32_t **order_out)
         *order_out = lists + 3 * (size_t)N;
         return FMM_OK;
     }
-    if (p->kd_exact) {  // exact 64-bit keys: 8 radix passes
+    if (N <= KD_LOCAL) {  // one launch for the three sorts
+        int npow2 = 1;
+        while (npow2 < N) npow2 <<= 1;
+        const size_t smem = (size_t)npow2 * 12;
+        if (smem > 40 * 1024) FMM_CUDA(c, cudaFuncSetAttribute((const void *)kd_sort_small, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        kd_sort_small<<<3, 1024, smem, st>>>(N, npow2, in->x, in->y, in->z, lists);
+        FMM_LAUNCH_CHECK(c, "kd_sort_small");
+    } else if (p->kd_exact) {  // exact 64-bit keys: 8 radix passes
         uint64_t *keys = (uint64_t *)ctx_alloc(c, sizeof(uint64_t) * 3 * (size_t)N);
         uint64_t *tkeys = (uint64_t *)ctx_alloc(c, sizeof(uint64_t) * 3 * (size_t)N);
         if (!keys || !tkeys) return FMM_ENOMEM;

@@ -456,8 +456,11 @@ int tree_build(fmm_plan *p, const fmm_particles_t *in)
     const int T = 256;
     const int gN = (N + T - 1) / T;
 
-    node_ranges_kernel<<<(unsigned)((p->nodes + T - 1) / T), T, 0, st>>>(N, p->kappa, (int)p->nodes, p->node_lo, p->node_hi);
-    FMM_LAUNCH_CHECK(c, "node_ranges_kernel");
+    if (!p->ranges_done) {  // closed-form ranges (T-2): they depend on (N, N0) only
+        node_ranges_kernel<<<(unsigned)((p->nodes + T - 1) / T), T, 0, st>>>(N, p->kappa, (int)p->nodes, p->node_lo, p->node_hi);
+        FMM_LAUNCH_CHECK(c, "node_ranges_kernel");
+        p->ranges_done = 1;
+    }
 
     uint32_t *order = NULL;
     if ((p->flags & FMM_TREE_MASK) == FMM_TREE_KD) {
