@@ -180,17 +180,16 @@ int scan_exclusive_i32(fmm_ctx *c, const int32_t *in, int32_t *out, int64_t n); 
 #ifdef __CUDACC__
 // ---- device helpers -------------------------------------------------------------------
 
-// w = D^{-3/2} for D > 0, and 0 for D == 0 (reading G17: a coincident pair contributes nothing,
-// which also removes i == j).  One MUFU.RSQ64H seed y0 (relative error ~2^-20) and one cubic
-// correction of y0^3:  D y0^2 = 1 - e  =>  D^{-3/2} = y0^3 (1-e)^{-3/2} = y0^3 (1 + 3/2 e + 15/8 e^2 + O(e^3)),
-// truncation 35/16 e^3 < 1e-17 relative.  6 FP64 instructions.  Subnormal D is flushed to 0 by the seed.
+// w = D^{-3/2}.  Reading G17 (a coincident pair contributes nothing, which also removes i == j) is met without a test: every
+// D is built as FMM_TINY_D + dx^2 + ..., so a coincident pair gets the finite w = 1e300 and g = w d = 0 exactly, while
+// D + 1e-200 == D for every D > 1e-184 (distances above 1e-92 in the caller's unit).  One MUFU.RSQ64H seed y0 (relative error
+// ~2^-20) and one cubic correction of y0^3:  D y0^2 = 1 - e  =>  D^{-3/2} = y0^3 (1-e)^{-3/2} = y0^3 (1 + 3/2 e + 15/8 e^2 + O(e^3)),
+// truncation 35/16 e^3 < 1e-17 relative.  6 FP64 instructions, no integer ones.
+#define FMM_TINY_D 1e-200
 __device__ __forceinline__ double inv_r3(double D)
 {
     double y0;
     asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y0) : "d"(D));
-    int hi = __double2hiint(y0);
-    hi = (hi == 0x7ff00000) ? 0 : hi;          // D == 0 -> seed +inf -> 0 (integer pipe, no FP64 slot)
-    y0 = __hiloint2double(hi, 0);
     double t = y0 * y0;
     double e = fma(-D, t, 1.0);
     double c = y0 * t;
@@ -208,7 +207,7 @@ __device__ __forceinline__ void pair_accumulate(double xt, double yt, double zt,
                                                 double &bx, double &by, double &bz)
 {
     double dx = xt - xs, dy = yt - ys, dz = zt - zs;
-    double D = dx * dx;
+    double D = fma(dx, dx, FMM_TINY_D);
     D = fma(dy, dy, D);
     D = fma(g2 * dz, dz, D);
     double w = inv_r3(D);

@@ -73,7 +73,7 @@ __device__ __forceinline__ void tile_interact(const double2 *tile, int count, co
 #pragma unroll
         for (int k = 0; k < NT; ++k) {
             double dx = xt[k] - a.x, dy = yt[k] - a.y, dz = zt[k] - b.x;
-            double D = dx * dx;
+            double D = fma(dx, dx, FMM_TINY_D);  // (> 0 also for a coincident pair: see inv_r3)
             D = fma(dy, dy, D);
             if (SM) {  // D = |d|^2 + (p_j . d)^2 (G6 alternative)
                 D = fma(dz, dz, D);
@@ -191,7 +191,7 @@ __device__ __forceinline__ void mut_pair_terms(const mut_targets<NT> &T, double 
 #pragma unroll
     for (int k = 0; k < NT; ++k) {
         const double dx = T.x[k] - xs, dy = T.y[k] - ys, dz = T.z[k] - zs;
-        double D = dx * dx;
+        double D = fma(dx, dx, FMM_TINY_D);  // (> 0 also for a coincident pair: see inv_r3)
         D = fma(dy, dy, D);
         const double sz = gb * dz;
         D = fma(sz, sz, D);
@@ -878,7 +878,7 @@ __device__ __forceinline__ void m2l_source(const double2 *__restrict__ Ms, const
     for (int a2 = 0; a2 < N1; ++a2) {
         poll();  // (helper warp: refill a released stage; nothing for the other warps)
         const double dx = xt - xs[a2];
-        const double dx2 = dx * dx;
+        const double dx2 = fma(dx, dx, FMM_TINY_D);  // (keeps D > 0 should two proxy points coincide: see inv_r3)
 #pragma unroll 1
         for (int b2 = 0; b2 < N1; ++b2) {
             const double2 *row = Ms + 2 * ((a2 * N1 + b2) * N1);

@@ -68,7 +68,7 @@ __global__ void __launch_bounds__(PROBE_THREADS) probe_kernel(int iters, double 
 #pragma unroll
             for (int k = 0; k < 4; ++k) {
                 const double dx = x[k] - xs, dy = y[k] - ys, dz = in[k] - zs;
-                double D = dx * dx;
+                double D = fma(dx, dx, 1e-200);
                 D = fma(dy, dy, D);
                 const double sz = a * dz;
                 D = fma(sz, sz, D);
