@@ -448,16 +448,19 @@ int pairs_p2p_prepare(fmm_plan *p)  // after the lists: choose the row split and
     fmm_ctx *c = &p->ctx;
     int maxleaf = (int)((p->N + p->leaves - 1) / p->leaves);
     int nt, threads, K;
-    p2p_shape(p->leaves, maxleaf, p->p2p_pairs, p->p2p_max_row, &nt, &threads, &K, p2p_use_mutual(p, maxleaf));
-    p->p2p_split = K;
     if (p2p_use_mutual(p, maxleaf) && p->p2p_react > p->react_cap) {
-        if (p->p2p_react >= ((int64_t)1 << 31)) return FMM_EOVERFLOW;
         if (p->react) ctx_free(c, p->react);
         p->react_cap = 0;
         p->react = (double *)ctx_alloc_keep(c, sizeof(double) * 6 * (size_t)p->p2p_react);
-        if (!p->react) return FMM_ENOMEM;
-        p->react_cap = p->p2p_react;
+        if (p->react) {
+            p->react_cap = p->p2p_react;
+        } else {  // no room for the reaction segments (48 bytes per particle of half the list): the one-sided kernel needs none
+            p->p2p_mutual = 0;
+            c->err[0] = 0;
+        }
     }
+    p2p_shape(p->leaves, maxleaf, p->p2p_pairs, p->p2p_max_row, &nt, &threads, &K, p2p_use_mutual(p, maxleaf));
+    p->p2p_split = K;
     int64_t need = (int64_t)(K + ((p->flags & FMM_METHOD_TREECODE) ? 1 : 0)) * 6 * p->N;  // treecode: + the particle-cluster sums
     if (need > p->near_cap) {
         if (p->near_) ctx_free(c, p->near_);

@@ -555,3 +555,29 @@ def test_orders_at_the_shared_memory_opt_in_boundary(fmm, n):
     assert_close(E, Eo, "E")
     assert_close(B, Bo, "B")
     plan.close()
+
+
+def test_one_sided_fallback_when_the_reaction_segments_do_not_fit(fmm, monkeypatch):
+    """The mutual near field needs 48 bytes per particle of half the P2P list; if the allocator refuses that block the plan
+    falls back to the one-sided kernel (same fields up to summation order) instead of failing."""
+    w = workloads.config(2, N=20000)
+    kw = dict(order_n=3, leaf_size=64, theta=0.5)
+    plan = fmm.fmm_plan_create(*w.arrays(), w.q, **kw)
+    st = plan.stats()
+    assert st["p2p_mutual"] == 1 and st["react_particles"] > 0
+    E0, B0 = to_np(plan.eval())
+    plan.close()
+    refused = 48 * st["react_particles"]
+    orig = fmm._TorchAllocator._alloc
+
+    def picky(self, nbytes, user):
+        return None if int(nbytes) == refused else orig(self, nbytes, user)
+
+    monkeypatch.setattr(fmm._TorchAllocator, "_alloc", picky)
+    plan = fmm.fmm_plan_create(*w.arrays(), w.q, **kw)
+    st1 = plan.stats()
+    assert st1["p2p_mutual"] == 0 and st1["n_p2p"] == st["n_p2p"]
+    E1, B1 = to_np(plan.eval())
+    assert_close(E1, E0, "one-sided fallback E")
+    assert_close(B1, B0, "one-sided fallback B")
+    plan.close()
