@@ -11,6 +11,8 @@
 // wait per build, at its very end (list lengths, gamma_bar, the input check).
 #include "fmm_internal.cuh"
 
+#include <stdlib.h>
+
 #include <cooperative_groups.h>
 namespace cg = cooperative_groups;
 
@@ -144,7 +146,7 @@ __global__ void __launch_bounds__(1024) dtt_top(dtt_args a)
 // would overflow hands the children to a global buffer instead, which a second launch walks the same way.
 #define DTT_WALK_WARPS 4
 #define DTT_WSTACK 512
-__global__ void __launch_bounds__(32 * DTT_WALK_WARPS) dtt_walk(dtt_args a, int pass)
+__global__ void __launch_bounds__(32 * DTT_WALK_WARPS) dtt_walk(dtt_args a, int pass, int wstack /* <= DTT_WSTACK */)
 {
     __shared__ uint64_t stk_all[DTT_WALK_WARPS][DTT_WSTACK];
     dtt_counters *cnt = a.cnt;
@@ -182,7 +184,7 @@ __global__ void __launch_bounds__(32 * DTT_WALK_WARPS) dtt_walk(dtt_args a, int 
             if (kind >= 3) {
                 const uint64_t c0 = (kind == 3) ? (((uint64_t)(2 * i) << 32) | (uint64_t)j) : (((uint64_t)i << 32) | (uint64_t)(2 * j));
                 const uint64_t c1 = (kind == 3) ? (((uint64_t)(2 * i + 1) << 32) | (uint64_t)j) : (((uint64_t)i << 32) | (uint64_t)(2 * j + 1));
-                if (top + 2 * nsplit <= DTT_WSTACK) {
+                if (top + 2 * nsplit <= wstack) {
                     const int at = top + 2 * __popc(splits & lt);
                     stk[at] = c0;
                     stk[at + 1] = c1;
@@ -192,7 +194,7 @@ __global__ void __launch_bounds__(32 * DTT_WALK_WARPS) dtt_walk(dtt_args a, int 
                     else cnt->overflow = 1;
                 }
             }
-            if (top + 2 * nsplit <= DTT_WSTACK) top += 2 * nsplit;
+            if (top + 2 * nsplit <= wstack) top += 2 * nsplit;
             __syncwarp();
         }
     }
@@ -508,9 +510,13 @@ int dtt_build_lists(fmm_plan *p)
         a.rows = rows; a.row_work = row_work; a.rows_len = rows_len; a.cnt = cnt;
         dtt_top<<<1, 1024, 0, st>>>(a);
         FMM_LAUNCH_CHECK(c, "dtt_top");
-        dtt_walk<<<12 * FMM_SM_COUNT, 32 * DTT_WALK_WARPS, 0, st>>>(a, 0);
+        // (FMM_TEST_WALK_STACK shrinks the walk's stack so that the tests reach the spill path)
+        const char *ws = getenv("FMM_TEST_WALK_STACK");
+        int wstack = ws ? atoi(ws) : DTT_WSTACK;
+        if (wstack < 64 || wstack > DTT_WSTACK) wstack = DTT_WSTACK;
+        dtt_walk<<<12 * FMM_SM_COUNT, 32 * DTT_WALK_WARPS, 0, st>>>(a, 0, wstack);
         FMM_LAUNCH_CHECK(c, "dtt_walk");
-        dtt_walk<<<2 * FMM_SM_COUNT, 32 * DTT_WALK_WARPS, 0, st>>>(a, 1);  // (walks that spilled: normally none)
+        dtt_walk<<<2 * FMM_SM_COUNT, 32 * DTT_WALK_WARPS, 0, st>>>(a, 1, DTT_WSTACK);  // (walks that spilled: normally none)
         FMM_LAUNCH_CHECK(c, "dtt_walk");
         dtt_totals<<<(unsigned)((p->leaves + 255) / 256 < 2 * FMM_SM_COUNT ? (p->leaves + 255) / 256 : 2 * FMM_SM_COUNT), 256, 0, st>>>(a);
         FMM_LAUNCH_CHECK(c, "dtt_totals");

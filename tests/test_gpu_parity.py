@@ -581,3 +581,18 @@ def test_one_sided_fallback_when_the_reaction_segments_do_not_fit(fmm, monkeypat
     assert_close(E1, E0, "one-sided fallback E")
     assert_close(B1, B0, "one-sided fallback B")
     plan.close()
+
+
+def test_traversal_spill_path(fmm, monkeypatch):
+    """The warp walks of the traversal keep their pairs in a 512-entry stack and hand what does not fit to a second
+    launch; with the stack shrunk to 64 entries (FMM_TEST_WALK_STACK) many walks spill and the lists must still be the oracle's."""
+    monkeypatch.setenv("FMM_TEST_WALK_STACK", "64")
+    w = workloads.config(2, N=60000)
+    plan = fmm.fmm_plan_create(*w.arrays(), w.q, order_n=2, leaf_size=8, theta=0.5)
+    st = plan.stats()
+    ex = plan.export()
+    op = oracle.Plan(*w.arrays(), w.q, order_n=2, leaf_size=8, theta=0.5, gamma_bar_value=st["gamma_bar"])
+    p2p, m2l = op.lists()
+    assert st["n_p2p"] == len(p2p) and st["n_m2l"] == len(m2l)
+    assert np.array_equal(ex["p2p_src"], p2p[:, 1]) and np.array_equal(ex["m2l_src"], m2l[:, 1])
+    plan.close()
