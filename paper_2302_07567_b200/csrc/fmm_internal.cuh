@@ -198,37 +198,4 @@ __device__ __forceinline__ double inv_r3(double D)
     return fma(c, pe, c);
 }
 
-// One source (x, y, z, m0..m3) acting on one target: eq. (3.1)-(3.2) without prefactors,
-// E += m0 g, B += (m1,m2,m3) x g.  25 FP64 instructions.
-__device__ __forceinline__ void pair_accumulate(double xt, double yt, double zt, double g2,
-                                                double xs, double ys, double zs,
-                                                double m0, double m1, double m2, double m3,
-                                                double &ex, double &ey, double &ez,
-                                                double &bx, double &by, double &bz)
-{
-    double dx = xt - xs, dy = yt - ys, dz = zt - zs;
-    double D = fma(dx, dx, FMM_TINY_D);
-    D = fma(dy, dy, D);
-    D = fma(g2 * dz, dz, D);
-    double w = inv_r3(D);
-    double gx = w * dx, gy = w * dy, gz = w * dz;
-    ex = fma(m0, gx, ex);
-    ey = fma(m0, gy, ey);
-    ez = fma(m0, gz, ez);
-    bx = fma(m2, gz, bx);
-    bx = fma(-m3, gy, bx);
-    by = fma(m3, gx, by);
-    by = fma(-m1, gz, by);
-    bz = fma(m1, gy, bz);
-    bz = fma(-m2, gx, bz);
-}
-
-// Reference Chebyshev points of the second kind on [-1,1] (reading I-1): c_k = cos(k pi / n)
-// written as sin(pi (n - 2k) / (2n)) so that c_k = -c_{n-k}; c_0 = 1, c_n = -1 exactly.
-__device__ __forceinline__ double cheb_ref(int n, int k)
-{
-    if (k == 0) return 1.0;
-    if (k == n) return -1.0;
-    return sin(FMM_PI * (double)(n - 2 * k) / (double)(2 * n));
-}
 #endif

@@ -9,23 +9,6 @@
 // ---------------------------------------------------------------------------------------
 // closed-form node ranges (DESIGN T-2): root [0,N); left child gets ceil(size/2)
 // ---------------------------------------------------------------------------------------
-__host__ __device__ __forceinline__ void node_at_level(int N, int level, int pos, int &node, int &lo, int &hi)
-{
-    lo = 0;
-    hi = N;
-    node = 1;
-    for (int l = 0; l < level; ++l) {
-        int mid = lo + (hi - lo + 1) / 2;
-        if (pos < mid) {
-            hi = mid;
-            node = 2 * node;
-        } else {
-            lo = mid;
-            node = 2 * node + 1;
-        }
-    }
-}
-
 __global__ void node_ranges_kernel(int N, int kappa, int nodes, int32_t *__restrict__ node_lo, int32_t *__restrict__ node_hi)
 {
     int i = blockIdx.x * blockDim.x + threadIdx.x + 1;  // heap id

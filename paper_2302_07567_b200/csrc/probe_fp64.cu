@@ -9,7 +9,7 @@
 //             2  DFMA v_k = fma(x_0, y_k, v_k), x_0 shared by neighbours  (three sources, one repeated: operand reuse)
 //             3  DMUL / DADD alternating, two distinct register sources
 //             4  MUFU.RSQ64H (rsqrt.approx.ftz.f64)
-//             5  the one-sided near-field evaluation (25 FP64 instructions, fmm_internal.cuh pair_accumulate)
+//             5  the one-sided near-field evaluation (25 FP64 instructions, kernels_pairs.cu tile_interact)
 //             6  the mutual near-field evaluation of a pair (34 FP64 instructions)
 //     inst_per_s = thread-level instructions (patterns 5, 6: kernel evaluations) per second, best of 3 launches.
 #include <cuda_runtime.h>
