@@ -68,7 +68,7 @@ struct p2m_cfg {
     static constexpr int G0 = P2M_THREADS / COLS;
     static constexpr int G = G0 > 8 ? 8 : (G0 < 1 ? 1 : G0);
     static constexpr int P = N1 * N1 * N1;
-    static constexpr size_t SMEM = sizeof(double) * (3 * N1 * P2M_CHUNK + 4 * P2M_CHUNK + (G > 1 ? 4 * P : 0));
+    static constexpr size_t SMEM = sizeof(double) * (3 * N1 * P2M_CHUNK + 4 * P2M_CHUNK + (G > 1 ? G * 4 * P : 0));
 };
 
 template <int N1>
@@ -80,7 +80,7 @@ __global__ void __launch_bounds__(P2M_THREADS, (N1 <= 7) ? 3 : 1) p2m_kernel(che
                                                           const double *__restrict__ w3, double *__restrict__ M)
 {
     constexpr int COLS = p2m_cfg<N1>::COLS, G = p2m_cfg<N1>::G, P = p2m_cfg<N1>::P, n = N1 - 1;
-    extern __shared__ double sm[];
+    extern __shared__ __align__(16) double sm[];
     double *bas = sm;                                  // [3][P2M_CHUNK][N1]
     double *wts = sm + 3 * N1 * P2M_CHUNK;             // [P2M_CHUNK][4]
     double *red = wts + 4 * P2M_CHUNK;                 // [P][4] (only if G > 1)
@@ -136,19 +136,22 @@ __global__ void __launch_bounds__(P2M_THREADS, (N1 <= 7) ? 3 : 1) p2m_kernel(che
                 m[0] = acc[0][c]; m[1] = acc[1][c]; m[2] = acc[2][c]; m[3] = acc[3][c];
             }
     } else {
-        for (int g = 0; g < G; ++g) {  // group partial sums added in group order
-            __syncthreads();
-            if (grp == g)
-#pragma unroll
-                for (int c = 0; c < N1; ++c)
-#pragma unroll
-                    for (int k = 0; k < 4; ++k) {
-                        double *r = red + 4 * (col * N1 + c) + k;
-                        *r = (g == 0) ? acc[k][c] : (*r + acc[k][c]);
-                    }
-        }
+        // every group leaves its partial sums in its own slab; they are then added in group order (two barriers instead of G)
         __syncthreads();
-        for (int e = threadIdx.x; e < 4 * P; e += P2M_THREADS) Mn[e] = red[e];
+        if (active)
+#pragma unroll
+            for (int c = 0; c < N1; ++c) {
+                double *r = red + (size_t)grp * 4 * P + 4 * (col * N1 + c);
+                *reinterpret_cast<double2 *>(r) = make_double2(acc[0][c], acc[1][c]);
+                *reinterpret_cast<double2 *>(r + 2) = make_double2(acc[2][c], acc[3][c]);
+            }
+        __syncthreads();
+        for (int e = threadIdx.x; e < 4 * P; e += P2M_THREADS) {
+            double v = red[e];
+#pragma unroll
+            for (int g = 1; g < G; ++g) v += red[(size_t)g * 4 * P + e];
+            Mn[e] = v;
+        }
     }
 }
 
@@ -190,20 +193,26 @@ int interp_transfer_tables(fmm_plan *p)
 // a5: M2M for one level.  One block per parent; for each non-empty child three 1-D contractions:
 //   M_S[a,b,c] += sum_{a',b',c'} Tx[a][a'] Ty[b][b'] Tz[c][c'] M_S'[a',b',c']
 // ---------------------------------------------------------------------------------------
-#define XFER_THREADS 256
+// threads of a transfer block: one per proxy point (in whole warps) up to 512, so the two inner phases are one pass
+template <int N1>
+struct xfer_cfg {
+    static constexpr int P = N1 * N1 * N1;
+    static constexpr int THREADS = ((P + 31) / 32 * 32 <= 512) ? ((P + 31) / 32 * 32 < 64 ? 64 : (P + 31) / 32 * 32) : 512;
+};
 
 // The whole upward pass is ONE launch: a block starts at a parent of two leaves; when a node is finished the block counts
 // itself into the node's parent, and the second of the two siblings to arrive (both children are then complete) goes on with
 // the parent.  No grid barrier, no launch per level: the dependency chain of the kappa levels costs a few microseconds per
 // level.  The result does not depend on which sibling arrives last (child 0 is always added before child 1).
 template <int N1>
-__global__ void __launch_bounds__(XFER_THREADS) m2m_kernel(int first, const int32_t *__restrict__ node_lo,
+__global__ void __launch_bounds__(xfer_cfg<N1>::THREADS) m2m_kernel(int first, const int32_t *__restrict__ node_lo,
                                                            const int32_t *__restrict__ node_hi, const double *__restrict__ tab,
                                                            double *M, int *arrive /* [nodes + 2], zero between evaluations */)
 {
     extern __shared__ __align__(16) double sm[];
     __shared__ int s_prev;
     constexpr int n1 = N1, P = n1 * n1 * n1, P4 = 4 * P, TS = (3 * n1 * n1 + 1) & ~1;  // compile-time order: index arithmetic without integer division
+    constexpr int XFER_THREADS = xfer_cfg<N1>::THREADS;
     double *T = sm;                              // [3][n1][n1]
     double *A = sm + TS;                         // [P][4], 16-byte aligned
     double *B = A + P4;                          // [P][4]
@@ -297,12 +306,13 @@ __global__ void __launch_bounds__(XFER_THREADS) m2m_kernel(int first, const int3
 // evaluation's stamp, adds the parent's field and stamps its own node.  A block only ever waits for a block with a smaller
 // index, and the blocks of a 1-D grid start in index order, so the block it waits for is running or done.
 template <int N1>
-__global__ void __launch_bounds__(XFER_THREADS) l2l_kernel(int first, int leaves, int stamp, const int32_t *__restrict__ node_lo,
+__global__ void __launch_bounds__(xfer_cfg<N1>::THREADS) l2l_kernel(int first, int leaves, int stamp, const int32_t *__restrict__ node_lo,
                                                            const int32_t *__restrict__ node_hi, const double *__restrict__ tab,
                                                            double *L, int *ready /* [nodes + 2] */)
 {
     extern __shared__ __align__(16) double sm[];
     constexpr int n1 = N1, P = n1 * n1 * n1, P6 = 6 * P, TS = (3 * n1 * n1 + 1) & ~1;
+    constexpr int XFER_THREADS = xfer_cfg<N1>::THREADS;
     double *T = sm;
     double *A = sm + TS;  // [P][6], 16-byte aligned
     double *B = A + P6;
@@ -552,7 +562,7 @@ int interp_m2m(fmm_plan *p)
     FMM_TRY(dispatch_n1(p->n1, [&](auto k) { return set_smem(c, (const void *)m2m_kernel<decltype(k)::value>, smem); }));
     const int first = 1 << (p->kappa - 1);  // one block per parent of two leaves; it climbs as long as it is the second to arrive
     FMM_TRY(dispatch_n1(p->n1, [&](auto k) {
-        m2m_kernel<decltype(k)::value><<<first, XFER_THREADS, smem, c->stream>>>(first, p->node_lo, p->node_hi, p->node_T, p->M, p->xfer_sync);
+        m2m_kernel<decltype(k)::value><<<first, xfer_cfg<decltype(k)::value>::THREADS, smem, c->stream>>>(first, p->node_lo, p->node_hi, p->node_T, p->M, p->xfer_sync);
         return FMM_OK;
     }));
     FMM_LAUNCH_CHECK(c, "m2m_kernel");
@@ -568,7 +578,7 @@ int interp_l2l(fmm_plan *p)
     p->xfer_stamp = (p->xfer_stamp >= (1 << 30)) ? 1 : p->xfer_stamp + 1;
     int *ready = p->xfer_sync + (p->nodes + 2);
     FMM_TRY(dispatch_n1(p->n1, [&](auto k) {
-        l2l_kernel<decltype(k)::value><<<(unsigned)(p->nodes - 1), XFER_THREADS, smem, c->stream>>>(2, (int)p->leaves, p->xfer_stamp, p->node_lo, p->node_hi,
+        l2l_kernel<decltype(k)::value><<<(unsigned)(p->nodes - 1), xfer_cfg<decltype(k)::value>::THREADS, smem, c->stream>>>(2, (int)p->leaves, p->xfer_stamp, p->node_lo, p->node_hi,
                                                                                                    p->node_T, p->L, ready);
         return FMM_OK;
     }));
