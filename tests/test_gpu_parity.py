@@ -596,3 +596,42 @@ def test_traversal_spill_path(fmm, monkeypatch):
     assert st["n_p2p"] == len(p2p) and st["n_m2l"] == len(m2l)
     assert np.array_equal(ex["p2p_src"], p2p[:, 1]) and np.array_equal(ex["m2l_src"], m2l[:, 1])
     plan.close()
+
+
+@pytest.mark.parametrize("kind", ["coplanar_z", "coplanar_x", "collinear_z", "at_rest", "wide_theta", "gamma_1e4"])
+def test_degenerate_geometry_and_momenta(fmm, kind):
+    """Boxes with zero extent along one or two axes (their proxy points coincide there and every particle hits a node of the
+    barycentric form exactly), a bunch at rest (gamma_bar = 1: B = 0), theta = 0.9 (large boxes still admissible) and
+    gamma_bar = 1e4 (z extents stretched far beyond x and y): structures bit-exact, fields as everywhere else."""
+    w = workloads.config(3, N=6000)
+    theta = 0.5
+    if kind == "coplanar_z":
+        w.z[:] = 0.25
+    elif kind == "coplanar_x":
+        w.x[:] = -1.0
+    elif kind == "collinear_z":
+        w.x[:] = 0.0
+        w.y[:] = 3.0
+    elif kind == "at_rest":
+        w.px[:] = 0.0; w.py[:] = 0.0; w.pz[:] = 0.0
+    elif kind == "wide_theta":
+        theta = 0.9
+    elif kind == "gamma_1e4":
+        w.pz[:] = w.pz * (1e4 / np.sqrt(1.0 + np.mean(w.pz) ** 2))
+    plan = fmm.fmm_plan_create(*w.arrays(), w.q, order_n=4, leaf_size=50, theta=theta)
+    st, ex = plan.stats(), plan.export()
+    E, B = to_np(plan.eval())
+    op = oracle.Plan(*w.arrays(), w.q, order_n=4, leaf_size=50, theta=theta, gamma_bar_value=st["gamma_bar"])
+    assert np.array_equal(ex["perm"], op.perm())
+    p2p, m2l = op.lists()
+    assert np.array_equal(ex["p2p_src"], p2p[:, 1]) and np.array_equal(ex["m2l_src"], m2l[:, 1])
+    assert st["n_m2l"] > 0
+    Eo, Bo = op.eval()
+    assert np.isfinite(E).all() and np.isfinite(B).all()
+    assert_close(E, Eo, "E " + kind)
+    if kind == "at_rest":
+        assert st["gamma_bar"] == 1.0 and np.all(B == 0.0) and np.all(Bo == 0.0)
+    else:
+        assert_close(B, Bo, "B " + kind)
+    plan.close()
+    op.close()
