@@ -147,42 +147,88 @@ __global__ void kd_fix_runs(int N, const double *__restrict__ x, const double *_
 }
 
 // ---------------------------------------------------------------------------------------
-// small bunches (N <= KD_LOCAL): the three sorts in one launch, one block per axis, bitonic network in shared memory on the
-// exact (coordinate key, index) pairs -- the 4-pass radix sort is 16 launches, which at N = 4,096 is most of the tree time
+// small bunches (N <= KD_LOCAL): the three sorts in one launch, one block per axis, bitonic network on the exact
+// (coordinate key, index) pairs -- the 4-pass radix sort is 16 launches, which at N = 4,096 is most of the tree time.
+// A thread keeps four consecutive elements in registers: partner distances 1 and 2 are exchanged in registers, 4 .. 64
+// by warp shuffles (the partner thread is in the same warp), and only distances >= 128 go through shared memory with
+// block barriers (15 of the 78 stages at 4,096 elements).
 // ---------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(1024) kd_sort_small(int N, int npow2, const double *__restrict__ x, const double *__restrict__ y,
+__device__ __forceinline__ bool kss_greater(uint64_t ka, uint32_t va, uint64_t kb, uint32_t vb)  // (coordinate, index): a total order
+{
+    return ka > kb || (ka == kb && va > vb);
+}
+
+__global__ void __launch_bounds__(1024) kd_sort_small(int N, int npow2 /* >= 128 */, const double *__restrict__ x, const double *__restrict__ y,
                                                       const double *__restrict__ z, uint32_t *__restrict__ lists /* [4 N] */)
 {
     extern __shared__ __align__(16) unsigned char kss_raw[];
-    uint64_t *key = reinterpret_cast<uint64_t *>(kss_raw);          // [npow2]
-    uint32_t *val = reinterpret_cast<uint32_t *>(key + npow2);      // [npow2]
-    const int a = blockIdx.x;
+    uint64_t *skey = reinterpret_cast<uint64_t *>(kss_raw);          // [npow2]
+    uint32_t *sval = reinterpret_cast<uint32_t *>(skey + npow2);     // [npow2]
+    const int a = blockIdx.x, t = threadIdx.x;
+    const bool active = 4 * t < npow2;  // (whole warps: npow2 / 4 is a multiple of 32)
     const double *coord = (a == 0) ? x : (a == 1) ? y : z;
-    for (int i = threadIdx.x; i < npow2; i += blockDim.x) {
-        key[i] = (i < N) ? sortable_key(coord[i]) : ~0ull;  // padding sorts last (index beyond every particle)
-        val[i] = (uint32_t)i;
+    uint64_t key[4];
+    uint32_t val[4];
+#pragma unroll
+    for (int e = 0; e < 4; ++e) {
+        const int i = 4 * t + e;
+        key[e] = (i < N) ? sortable_key(coord[i]) : ~0ull;  // padding sorts last (index beyond every particle)
+        val[e] = (uint32_t)i;
     }
     if (a == 0)
-        for (int i = threadIdx.x; i < N; i += blockDim.x) lists[3 * (size_t)N + i] = (uint32_t)i;
-    __syncthreads();
+        for (int i = t; i < N; i += blockDim.x) lists[3 * (size_t)N + i] = (uint32_t)i;
     for (int k = 2; k <= npow2; k <<= 1) {
         for (int j = k >> 1; j > 0; j >>= 1) {
-            for (int i = threadIdx.x; i < npow2; i += blockDim.x) {
-                const int l = i ^ j;
-                if (l > i) {
-                    const uint64_t ki = key[i], kl = key[l];
-                    const uint32_t vi = val[i], vl = val[l];
-                    const bool greater = (ki > kl) || (ki == kl && vi > vl);  // (coordinate, index): a total order
-                    if (greater == ((i & k) == 0)) {
-                        key[i] = kl; key[l] = ki;
-                        val[i] = vl; val[l] = vi;
+            if (j >= 128) {  // the partner thread t ^ (j / 4) sits in another warp
+                if (active) {
+#pragma unroll
+                    for (int e = 0; e < 4; ++e) { skey[4 * t + e] = key[e]; sval[4 * t + e] = val[e]; }
+                }
+                __syncthreads();
+                if (active) {
+                    const int pt = t ^ (j >> 2);
+#pragma unroll
+                    for (int e = 0; e < 4; ++e) {
+                        const int i = 4 * t + e;
+                        const uint64_t pk = skey[4 * pt + e];
+                        const uint32_t pv = sval[4 * pt + e];
+                        const bool g = kss_greater(key[e], val[e], pk, pv);
+                        const bool want_min = ((i & j) == 0) == ((i & k) == 0);
+                        if (want_min == g) { key[e] = pk; val[e] = pv; }
                     }
                 }
+                __syncthreads();
+            } else if (j >= 4) {  // same warp: lane ^ (j / 4)
+                if (active) {
+#pragma unroll
+                    for (int e = 0; e < 4; ++e) {
+                        const int i = 4 * t + e;
+                        const uint64_t pk = __shfl_xor_sync(0xffffffffu, key[e], j >> 2);
+                        const uint32_t pv = __shfl_xor_sync(0xffffffffu, val[e], j >> 2);
+                        const bool g = kss_greater(key[e], val[e], pk, pv);
+                        const bool want_min = ((i & j) == 0) == ((i & k) == 0);
+                        if (want_min == g) { key[e] = pk; val[e] = pv; }
+                    }
+                }
+            } else {  // both elements in this thread's registers (k >= 4: one direction for the thread's four elements)
+                const bool asc = ((4 * t) & k) == 0;
+#define KSS_CX(E, F, UP)                                                     \
+    if (kss_greater(key[E], val[E], key[F], val[F]) == (UP)) {               \
+        const uint64_t tk = key[E]; key[E] = key[F]; key[F] = tk;            \
+        const uint32_t tv = val[E]; val[E] = val[F]; val[F] = tv;            \
+    }
+                if (j == 2) { KSS_CX(0, 2, asc) KSS_CX(1, 3, asc) }
+                else if (k > 2) { KSS_CX(0, 1, asc) KSS_CX(2, 3, asc) }
+                else { KSS_CX(0, 1, true) KSS_CX(2, 3, false) }
+#undef KSS_CX
             }
-            __syncthreads();
         }
     }
-    for (int i = threadIdx.x; i < N; i += blockDim.x) lists[(size_t)a * N + i] = val[i];
+#pragma unroll
+    for (int e = 0; e < 4; ++e) {
+        const int i = 4 * t + e;
+        if (i < N) lists[(size_t)a * N + i] = val[e];
+    }
 }
 
 // ---------------------------------------------------------------------------------------
@@ -557,7 +603,7 @@ int kd_build_order(fmm_plan *p, const fmm_particles_t *in, uint32_t **order_out)
         return FMM_OK;
     }
     if (N <= KD_LOCAL) {  // one launch for the three sorts
-        int npow2 = 1;
+        int npow2 = 128;  // (four elements per thread, whole warps)
         while (npow2 < N) npow2 <<= 1;
         const size_t smem = (size_t)npow2 * 12;
         if (smem > 40 * 1024) FMM_CUDA(c, cudaFuncSetAttribute((const void *)kd_sort_small, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
