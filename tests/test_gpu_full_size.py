@@ -8,6 +8,8 @@
     tolerance 1e-12 in both measures of DESIGN.md "Tolerances";
   * configs[3] (N = 4,194,304, 3e11 kernel evaluations) is compared on SAMPLED outputs the oracle computes
     one by one: the serial-FMM oracle evaluated on a seeded sample of 256 target leaves (65,536 particles);
+  * the paper's own workload (`PAPER.md:380`: N = 1.28e6 in a cube, n = 4, N0 = 125 -- bench.py --config 7; ragged leaves of
+    78 / 79 particles) is compared on every particle as well;
   * the direct sum on a seeded sample of target particles (the GPU's FMM-vs-direct error must equal the
     oracle's to 3 digits);
   * properties that hold at any size: bit-reproducibility, finite outputs.
@@ -119,3 +121,10 @@ def test_config4_full_gamma100(fmm):
     w = workloads.config(4)
     st, err = _run_full(fmm, w, n_leaf_sample=256, n_direct_sample=64, seed=41)
     assert st["kappa"] == 14 and err["E"] < 1e-3
+
+
+def test_paper_workload_full(fmm):
+    """SURVEY.md 8(f) rank 1, bench.py --config 7: N = 1,280,000 uniform cube, identical momenta gamma = 50, n = 4, N0 = (n+1)^3."""
+    w = workloads.paper_cube()
+    st, err = _run_full(fmm, w, n_leaf_sample=None, n_direct_sample=256, seed=71)
+    assert st["kappa"] == 14 and st["leaves"] == 16384 and err["E"] < 1e-2
