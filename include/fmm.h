@@ -28,6 +28,15 @@
  *              stream that was current at allocation; the Python binding therefore runs every
  *              call of a plan under the stream the plan was created on).  A plan frees its
  *              remaining workspace in fmm_plan_destroy.
+ *   Memory     a plan keeps about 110 N bytes of particle data, 80 P bytes per tree node for
+ *              the moments and local fields (P = (n+1)^3), the two lists (4 to 16 bytes per
+ *              entry) and, with the mean-gamma kernel, the reaction segments of the mutual
+ *              near field: 48 bytes x ceil(N / leaves) per PAIR of P2P entries (0.9 GB at
+ *              N = 2^20 with leaves of 256, 18 GB at N = 2.56e7 with leaves of 78; reported
+ *              as fmm_stats_t.react_particles).  If the allocator refuses that block the plan
+ *              falls back to the one-sided near field (same results to rounding, about 1.3x
+ *              the P2P time) instead of failing.  A build needs 120 to 230 N bytes of scratch
+ *              on top, returned before the call ends.
  *   Stream     all work is enqueued on `cuda_stream` (a cudaStream_t passed as void*; NULL =
  *              the legacy default stream).  fmm_plan_create / fmm_plan_update / fmm_plan_refit
  *              wait for the stream ONCE, after the traversal (the interaction-list lengths
@@ -42,7 +51,9 @@
  *              one call to another: the launch counter behind fmm_launch_count, one side
  *              stream per device (fmm_plan_set_overlap), and a per-device flag that the table
  *              of Chebyshev points has been uploaded to constant memory.  Plans are otherwise
- *              independent; one plan must not be used from two threads at once.
+ *              independent; one plan must not be used from two threads at once.  The only
+ *              environment variable read is FMM_TEST_WALK_STACK (a smaller traversal stack,
+ *              used by the tests to reach the spill path; results do not depend on it).
  *   Order      outputs are in the caller's particle order.
  *   Units      SI; eps0 = 8.8541878128e-12 F/m, c0 = 299792458 m/s (CODATA 2018), unless
  *              FMM_RAW_SUMS is set (then the bare sums without prefactors are returned).
