@@ -42,7 +42,12 @@
  *              wait for the stream ONCE, after the traversal (the interaction-list lengths
  *              must be read back to size the lists; gamma_bar and the input check come with
  *              them), and return with the rest of the build enqueued; the inputs are no
- *              longer read after that wait.  fmm_eval and fmm_direct only enqueue and return.
+ *              longer read after that wait.  The upward pass (P2M, M2M: Alg 5.3-5.5), which
+ *              depends on the tree and the particles only, is enqueued by the build behind
+ *              the copies it waits for, so that the device works on it while the host reads
+ *              the lengths and returns to the caller; fmm_eval reuses those moments (they are
+ *              recomputed inside fmm_eval only after fmm_plan_set_timing, so that the stage
+ *              timers bracket them).  fmm_eval and fmm_direct only enqueue and return.
  *   Errors     0 on success, a negative FMM_E* code otherwise; no exceptions, no exit().
  *              Outputs are unspecified after an error.  A plan whose fmm_plan_update /
  *              fmm_plan_refit failed is marked invalid: fmm_eval returns FMM_EINVAL for it

@@ -214,6 +214,21 @@ static int plan_alloc_fixed(fmm_plan *p)
     return FMM_OK;
 }
 
+// a4 + a5 (P2M, M2M): the moments depend on the tree and the particles only, so a build enqueues them itself, right behind
+// the copies its one host wait is for (kernels_dtt.cu): the GPU works on them while the host reads the list lengths, returns
+// to the caller and comes back with fmm_eval, instead of idling for that time.  fmm_eval finds them done.
+int plan_upward(fmm_plan *p)
+{
+    if (p->upward_done) return FMM_OK;
+    if (p->timing) FMM_CUDA(&p->ctx, cudaEventRecord(p->ev[EV_P2M], p->ctx.stream));
+    FMM_TRY(interp_p2m(p));          // Alg 5.3 at the leaves
+    if (p->timing) FMM_CUDA(&p->ctx, cudaEventRecord(p->ev[EV_M2M], p->ctx.stream));
+    FMM_TRY(interp_m2m(p));          // Alg 5.4, levels kappa-1 .. 0 (Alg 5.5)
+    if (p->timing) FMM_CUDA(&p->ctx, cudaEventRecord(p->ev[EV_UPEND], p->ctx.stream));
+    p->upward_done = 1;
+    return FMM_OK;
+}
+
 static int plan_build(fmm_plan *p, const fmm_particles_t *in, bool refit = false)
 {
     fmm_ctx *c = &p->ctx;
@@ -230,12 +245,13 @@ static int plan_build(fmm_plan *p, const fmm_particles_t *in, bool refit = false
             ctx_arena_end(c);
             FMM_TRY(ctx_arena_begin(c, estimate + (size_t)48 * (size_t)p->N));
         }
+        p->upward_done = 0;
         FMM_CUDA(c, cudaEventRecord(p->ev_plan[0], c->stream));
         FMM_TRY(tree_scan_inputs(p, in));  // a0: gamma_bar, coordinate ranges, input check -> p->hdr (device)
         FMM_TRY(refit ? tree_refit(p, in) : tree_build(p, in));
         FMM_CUDA(c, cudaEventRecord(p->ev_plan[1], c->stream));
-        FMM_TRY(dtt_build_lists(p));       // (reads gamma_bar and the input check back together with the list lengths)
-        FMM_CUDA(c, cudaEventRecord(p->ev_plan[2], c->stream));
+        FMM_TRY(dtt_build_lists(p));       // (reads gamma_bar and the input check back together with the list lengths; records
+                                           //  ev_plan[2] behind its last kernel and enqueues the upward pass before it waits)
         if (!p->kd_retry) break;
     }
     FMM_TRY(pairs_p2p_prepare(p));
@@ -331,6 +347,7 @@ extern "C" int fmm_plan_set_timing(fmm_plan_t *p, int on)
     if (!p) return FMM_EINVAL;
     p->timing = on ? 1 : 0;
     p->ev_valid = 0;
+    p->upward_done = 0;  // (the next fmm_eval runs the upward pass again, between its own events)
     return FMM_OK;
 }
 
@@ -350,10 +367,7 @@ extern "C" int fmm_eval(fmm_plan_t *p, double *Ex, double *Ey, double *Ez, doubl
         return FMM_EINVAL;
     }
     if (p->flags & FMM_METHOD_TREECODE) {  // P2M, M2M, particle-cluster + P2P, finalise (no M2L / L2L / far L2P)
-        MARK(p, EV_P2M);
-        FMM_TRY(interp_p2m(p));
-        MARK(p, EV_M2M);
-        FMM_TRY(interp_m2m(p));
+        FMM_TRY(plan_upward(p));
         MARK(p, EV_M2L);
         FMM_TRY(pairs_pc(p));
         MARK(p, EV_L2L);
@@ -372,8 +386,7 @@ extern "C" int fmm_eval(fmm_plan_t *p, double *Ex, double *Ey, double *Ez, doubl
         cudaStream_t main_stream = c->stream;
         FMM_CUDA(c, cudaEventRecord(p->ev_fork, main_stream));
         FMM_CUDA(c, cudaStreamWaitEvent(p->side, p->ev_fork, 0));
-        FMM_TRY(interp_p2m(p));
-        FMM_TRY(interp_m2m(p));
+        FMM_TRY(plan_upward(p));
         FMM_TRY(pairs_m2l(p));
         c->stream = p->side;
         int rc = pairs_p2p(p);
@@ -385,10 +398,7 @@ extern "C" int fmm_eval(fmm_plan_t *p, double *Ex, double *Ey, double *Ez, doubl
         FMM_TRY(interp_l2p_finalize(p, Ex, Ey, Ez, Bx, By, Bz));
         return FMM_OK;
     }
-    MARK(p, EV_P2M);
-    FMM_TRY(interp_p2m(p));          // Alg 5.3 at the leaves
-    MARK(p, EV_M2M);
-    FMM_TRY(interp_m2m(p));          // Alg 5.4, levels kappa-1 .. 0 (Alg 5.5)
+    FMM_TRY(plan_upward(p));         // Alg 5.3-5.5 (already enqueued by the build unless timing was switched on since)
     MARK(p, EV_M2L);
     FMM_TRY(pairs_m2l(p));           // Alg 5.9 over m2l_itl
     MARK(p, EV_L2L);
@@ -438,7 +448,7 @@ extern "C" int fmm_plan_stats(fmm_plan_t *p, fmm_stats_t *s)
         fmm_ctx *c = &p->ctx;
         FMM_CUDA(c, cudaEventSynchronize(p->ev[EV_END]));
         FMM_CUDA(c, cudaEventElapsedTime(&s->ms_p2m, p->ev[EV_P2M], p->ev[EV_M2M]));
-        FMM_CUDA(c, cudaEventElapsedTime(&s->ms_m2m, p->ev[EV_M2M], p->ev[EV_M2L]));
+        FMM_CUDA(c, cudaEventElapsedTime(&s->ms_m2m, p->ev[EV_M2M], p->ev[EV_UPEND]));
         FMM_CUDA(c, cudaEventElapsedTime(&s->ms_m2l, p->ev[EV_M2L], p->ev[EV_L2L]));
         FMM_CUDA(c, cudaEventElapsedTime(&s->ms_l2l, p->ev[EV_L2L], p->ev[EV_P2P]));
         FMM_CUDA(c, cudaEventElapsedTime(&s->ms_p2p, p->ev[EV_P2P], p->ev[EV_L2P]));

@@ -72,7 +72,7 @@ struct fmm_hdr {
     unsigned int kd_fallback; // the quantised sort keys of the KD build left a long run out of order: rebuild with exact keys
 };
 
-enum { EV_P2M = 0, EV_M2M, EV_M2L, EV_L2L, EV_P2P, EV_L2P, EV_END, EV_COUNT };
+enum { EV_P2M = 0, EV_M2M, EV_UPEND, EV_M2L, EV_L2L, EV_P2P, EV_L2P, EV_END, EV_COUNT };
 
 struct fmm_plan {
     fmm_ctx ctx;
@@ -134,6 +134,7 @@ struct fmm_plan {
     cudaEvent_t ev_fork, ev_join;
     int overlap;
     int ev_valid;
+    int upward_done;        // P2M + M2M of the current tree are enqueued already (plan_upward: at the end of a build, behind the host wait)
     int plan_ms_pending;    // ms_tree / ms_lists of the last build have not been read from ev_plan yet
     float ms_tree, ms_lists;
 };
@@ -150,6 +151,7 @@ int tree_refit(fmm_plan *p, const fmm_particles_t *in);  // keeps the particle o
 int dtt_build_lists(fmm_plan *p);
 // ---- kernels_interp.cu --------------------------------------------------------------
 int interp_transfer_tables(fmm_plan *p);  // after the boxes of a build
+int plan_upward(fmm_plan *p);  // a4 + a5 once per build (fmm_api.cu)
 int interp_p2m(fmm_plan *p);
 int interp_m2m(fmm_plan *p);
 int interp_l2l(fmm_plan *p);

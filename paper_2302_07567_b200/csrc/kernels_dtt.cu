@@ -542,7 +542,11 @@ int dtt_build_lists(fmm_plan *p)
         FMM_TRY(make_order(p, cnt, 1, (int)p->nodes, p->m2l_off, p->m2l_src, 0, NULL, p->m2l_order));
         FMM_CUDA(c, cudaMemcpyAsync(&h, cnt, sizeof(h), cudaMemcpyDeviceToHost, st));
         FMM_CUDA(c, cudaMemcpyAsync(&hh, p->hdr, sizeof(hh), cudaMemcpyDeviceToHost, st));
-        FMM_CUDA(c, cudaStreamSynchronize(st));  // the one host wait of a build: list lengths, gamma_bar, the input check
+        // the one host wait of a build (list lengths, gamma_bar, the input check) is on an event behind those copies; the
+        // upward pass is enqueued first, so that the GPU has work while the host reads them and returns to the caller
+        FMM_CUDA(c, cudaEventRecord(p->ev_plan[2], st));
+        FMM_TRY(plan_upward(p));
+        FMM_CUDA(c, cudaEventSynchronize(p->ev_plan[2]));
         ctx_free(c, seg); ctx_free(c, len); ctx_free(c, mate); ctx_free(c, tgt);
         ctx_free(c, m2l_tmp); ctx_free(c, p2p_tmp); ctx_free(c, km2l); ctx_free(c, kp2p); ctx_free(c, f1); ctx_free(c, f0);
         ctx_free(c, scan); ctx_free(c, row_work); ctx_free(c, rows); ctx_free(c, cnt);

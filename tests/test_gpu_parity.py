@@ -635,3 +635,39 @@ def test_degenerate_geometry_and_momenta(fmm, kind):
         assert_close(B, Bo, "B " + kind)
     plan.close()
     op.close()
+
+
+@pytest.mark.parametrize("method", ["fmm", "treecode"])
+def test_upward_pass_of_the_build_and_stage_timers(fmm, method):
+    """A build enqueues P2M + M2M itself, behind its one host wait, and fmm_eval reuses the moments:
+    repeated evaluations, evaluations with the stage timers switched on or off in between (which makes fmm_eval run the
+    upward pass again, between its own events) and an update under running timers all give the same bits, and the six
+    stage times are there whenever the timers were on for the evaluation."""
+    w = workloads.config(2, N=9000)
+    flags = fmm.FMM_TREE_KD | (fmm.FMM_METHOD_TREECODE if method == "treecode" else 0)
+    plan = fmm.fmm_plan_create(*w.arrays(), w.q, order_n=3, leaf_size=50, theta=0.5, flags=flags)
+    E0, B0 = to_np(plan.eval())
+    plan.set_timing(True)
+    E1, B1 = to_np(plan.eval())
+    st = plan.stats()
+    assert st["timing_valid"] == 1 and st["ms_p2m"] > 0 and st["ms_m2m"] > 0 and st["ms_l2p"] > 0
+    E2, B2 = to_np(plan.eval())      # moments of the evaluation before
+    plan.update(*w.arrays(), w.q)    # same particles: the build runs the upward pass under the timers
+    E3, B3 = to_np(plan.eval())
+    st = plan.stats()
+    assert st["timing_valid"] == 1 and st["ms_p2m"] > 0 and st["ms_m2m"] > 0 and st["ms_m2l"] > 0 and st["ms_p2p"] > 0
+    plan.set_timing(False)
+    E4, B4 = to_np(plan.eval())
+    for E, B in ((E1, B1), (E2, B2), (E3, B3), (E4, B4)):
+        assert np.array_equal(E, E0) and np.array_equal(B, B0)
+    w2 = workloads.config(2, N=9000)
+    w2.x[:] = w2.x * 1.5             # a different tree: the moments must be those of the new build
+    plan.update(*w2.arrays(), w2.q)
+    st = plan.stats()
+    E5, B5 = to_np(plan.eval())
+    op = oracle.Plan(*w2.arrays(), w2.q, order_n=3, leaf_size=50, theta=0.5, gamma_bar_value=st["gamma_bar"])
+    Eo, Bo = op.eval_treecode() if method == "treecode" else op.eval()
+    assert_close(E5, Eo, "E after update")
+    assert_close(B5, Bo, "B after update")
+    plan.close()
+    op.close()
