@@ -160,6 +160,7 @@ int interp_l2p_finalize(fmm_plan *p, /* treecode: no far interpolation, near_ ha
 int pairs_p2p(fmm_plan *p);
 int pairs_p2p_prepare(fmm_plan *p);
 int pairs_m2l_prepare(fmm_plan *p);
+int pairs_proxy_points(fmm_plan *p);  // after the boxes of a build (a2): per-axis proxy points of every node
 int pairs_m2l(fmm_plan *p);
 int pairs_pc(fmm_plan *p);   // treecode: particle-cluster sums
 int pairs_direct(fmm_ctx *c, int64_t N, const double *x, const double *y, const double *z,

@@ -826,7 +826,7 @@ __device__ __forceinline__ void mbar_arrive(uint64_t *bar)
     asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
 }
 
-// Per-node tables for M2L, filled once per evaluation:
+// Per-node tables for M2L, filled once per build (pairs_proxy_points):
 //   xi[node][g][k]  proxy points per axis (reading I-3), row stride M2L_XI_STRIDE.  Row 2 (z) holds the points
 //                   RELATIVE to the box centre z0 = (a_z + b_z)/2, and z0 itself sits in xi[node][2][15].
 //                   xi[node][2][14] = h_z = (b_z - a_z)/2, so that zrel_k = h_z c_k up to one rounding of the proxy point.
@@ -1187,20 +1187,24 @@ static int m2l_upload_cheb(fmm_ctx *c)
     return FMM_OK;
 }
 
-int pairs_m2l(fmm_plan *p)
+// proxy points of every node (m2l_proxy_points): part of a2, called by the build after the boxes
+int pairs_proxy_points(fmm_plan *p)
 {
-    FMM_TRY(m2l_upload_cheb(&p->ctx));
+    fmm_ctx *c = &p->ctx;
+    FMM_TRY(m2l_upload_cheb(c));
     cheb13 ch;
     memset(&ch, 0, sizeof(ch));
     for (int k = 0; k <= p->n; ++k) ch.c[k] = sin(FMM_PI * (double)(p->n - 2 * k) / (double)(2 * p->n));  // I-1
     ch.c[0] = 1.0;
     ch.c[p->n] = -1.0;
-    {
-        fmm_ctx *c = &p->ctx;
-        int count = (int)(p->nodes + 1) * 3 * M2L_XI_STRIDE;
-        m2l_proxy_points<<<(count + 255) / 256, 256, 0, c->stream>>>((int)p->nodes, p->n1, ch, p->bbox, p->node_xi);
-        FMM_LAUNCH_CHECK(c, "m2l_proxy_points");
-    }
+    int count = (int)(p->nodes + 1) * 3 * M2L_XI_STRIDE;
+    m2l_proxy_points<<<(count + 255) / 256, 256, 0, c->stream>>>((int)p->nodes, p->n1, ch, p->bbox, p->node_xi);
+    FMM_LAUNCH_CHECK(c, "m2l_proxy_points");
+    return FMM_OK;
+}
+
+int pairs_m2l(fmm_plan *p)
+{
     switch (p->n1) {
         case 2: return launch_m2l<2>(p);
         case 3: return launch_m2l<3>(p);
@@ -1221,14 +1225,6 @@ int pairs_m2l(fmm_plan *p)
 int pairs_pc(fmm_plan *p)  // treecode: particle-cluster sums into partial buffer p2p_split
 {
     fmm_ctx *c = &p->ctx;
-    cheb13 ch;
-    memset(&ch, 0, sizeof(ch));
-    for (int k = 0; k <= p->n; ++k) ch.c[k] = sin(FMM_PI * (double)(p->n - 2 * k) / (double)(2 * p->n));  // I-1
-    ch.c[0] = 1.0;
-    ch.c[p->n] = -1.0;
-    int count = (int)(p->nodes + 1) * 3 * M2L_XI_STRIDE;
-    m2l_proxy_points<<<(count + 255) / 256, 256, 0, c->stream>>>((int)p->nodes, p->n1, ch, p->bbox, p->node_xi);
-    FMM_LAUNCH_CHECK(c, "m2l_proxy_points");
     int maxleaf = (int)((p->N + p->leaves - 1) / p->leaves);
     int nt, threads, K;
     p2p_shape(p->leaves, maxleaf, p->p2p_pairs, p->p2p_max_row, &nt, &threads, &K);

@@ -478,6 +478,7 @@ int tree_boxes(fmm_plan *p)
     node_geometry<<<(unsigned)((p->nodes + T - 1) / T), T, 0, c->stream>>>((int)p->nodes, p->hdr, p->bbox, p->node_geo);
     FMM_LAUNCH_CHECK(c, "node_geometry");
     FMM_TRY(interp_transfer_tables(p));  // M2M / L2L matrices of the new boxes (kernels_interp.cu)
+    FMM_TRY(pairs_proxy_points(p));      // proxy points of the new boxes for M2L and the treecode (kernels_pairs.cu)
     return FMM_OK;
 }
 
