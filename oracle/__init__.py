@@ -66,6 +66,7 @@ def lib():
         _lib.orc_plan_perm.argtypes = [C.c_void_p, _i64p]
         _lib.orc_plan_nodes.argtypes = [C.c_void_p, _i64p, _i64p, _dp]
         _lib.orc_plan_lists.argtypes = [C.c_void_p, _i32p, _i32p, _i32p, _i32p]
+        _lib.orc_plan_leaf_flags.argtypes = [C.c_void_p, C.POINTER(C.c_int8)]
         _lib.orc_upward.argtypes = [C.c_void_p, _dp]
         _lib.orc_p2m_node.argtypes = [C.c_void_p, C.c_int64, _dp]
         _lib.orc_eval.restype = C.c_int
@@ -137,14 +138,17 @@ class Plan:
     """O2: tree + interaction lists, then upward / eval (serial FMM of Alg 5.12)."""
 
     def __init__(self, x, y, z, px, py, pz, q=None, *, order_n, leaf_size, theta,
-                 gamma_bar_value=None, tree_mode=TREE_KD, raw=False, source_momentum=False, given_order=None):
-        """given_order: particle order (tree position -> particle index) to build the tree over instead of sorting
+                 gamma_bar_value=None, tree_mode=TREE_KD, raw=False, source_momentum=False, given_order=None,
+                 stop_at_n0=False):
+        """stop_at_n0: Alg 5.2 as printed -- a cluster of at most N0 particles is a leaf wherever it is (leaves on two
+        levels, ORC_TREE_STOP_AT_N0); default: every node of level kappa is a leaf (reading T-1).
+        given_order: particle order (tree position -> particle index) to build the tree over instead of sorting
         (refit of an existing partition); tree_mode is then ignored."""
         arrs = [_d(a) for a in (x, y, z, px, py, pz)]
         self.N = len(arrs[0][0])
         qa, qp, qs = _charges(q, self.N)
         gb = -1.0 if gamma_bar_value is None else float(gamma_bar_value)
-        flags = int(bool(raw)) | (2 if source_momentum else 0)
+        flags = int(bool(raw)) | (2 if source_momentum else 0) | (4 if stop_at_n0 else 0)
         if given_order is None:
             self._h = lib().orc_plan_create(self.N, *[p for _, p in arrs], qp, qs, int(order_n),
                                             int(leaf_size), float(theta), gb, int(tree_mode), flags)
@@ -182,6 +186,16 @@ class Plan:
         lib().orc_plan_nodes(self._h, lo.ctypes.data_as(_i64p), hi.ctypes.data_as(_i64p),
                              bb.ctypes.data_as(_dp))
         return lo, hi, bb
+
+    def leaf_flags(self) -> np.ndarray:
+        """[nodes] int8, row i-1 is heap node i: 1 leaf, 0 has children, 2 unused slot (stop_at_n0 only)."""
+        f = np.empty(self.nodes, dtype=np.int8)
+        lib().orc_plan_leaf_flags(self._h, f.ctypes.data_as(C.POINTER(C.c_int8)))
+        return f
+
+    def leaf_ids(self) -> np.ndarray:
+        """heap ids of the leaves, ascending"""
+        return np.flatnonzero(self.leaf_flags() == 1).astype(np.int64) + 1
 
     def lists(self):
         """(p2p[np2p,2], m2l[nm2l,2]) as (target, source) heap ids sorted by (target, source)."""

@@ -34,6 +34,7 @@ struct orc_plan {
     double *pm;           /* [N][3] plain momenta px, py, pz, caller order (source-momentum near field) */
     int64_t *perm;        /* tree position -> caller index */
     int64_t *lo, *hi;     /* [nodes+1], heap index, half open */
+    signed char *leaf;    /* [nodes+1]: 1 leaf, 0 has children, 2 unused slot below a leaf of level kappa-1 */
     double *bbox;         /* [nodes+1][6] ax ay az bx by bz */
     int64_t np2p, nm2l, cap_p2p, cap_m2l;
     int32_t *p2p, *m2l;   /* pairs (t,s) interleaved */
@@ -262,11 +263,16 @@ static void subdivide(orc_plan_t *p, int64_t node, int64_t lo, int64_t hi, int l
     p->hi[node] = hi;
     double *bb = &p->bbox[6 * node];
     tight_bbox(p, lo, hi, bb);
-    if (level == p->kappa) { /* leaf: canonical order = ascending original index (T-3) */
+    /* T-1: every node of level kappa is a leaf.  ORC_TREE_STOP_AT_N0: Alg 5.2 as printed,
+     * "if |S| > N0 then split ... else children(S) = {}" -- a node of at most N0 particles is a leaf wherever it is
+     * (a node of level kappa never holds more than N0). */
+    if (level == p->kappa || ((p->raw & ORC_TREE_STOP_AT_N0) && hi - lo <= p->N0)) {
+        p->leaf[node] = 1; /* canonical order inside a leaf = ascending original index (T-3) */
         if (p->tree_mode == ORC_TREE_KD)
             qsort(p->perm + lo, (size_t)(hi - lo), sizeof(int64_t), cmp_idx);
         return;
     }
+    p->leaf[node] = 0;
     int64_t mid = lo + (hi - lo + 1) / 2; /* T-2: left child gets ceil(size/2) */
     if (p->tree_mode == ORC_TREE_KD && hi > lo) {
         /* Alg 5.1: k = argmax s_k (b_k - a_k); G9: first maximiser */
@@ -380,7 +386,7 @@ static void dualtraversefillitl(orc_plan_t *p, int64_t i, int64_t j)
 {
     if (p->hi[i] == p->lo[i] || p->hi[j] == p->lo[j])
         return; /* an empty cluster has nothing to receive or to send */
-    int leaf_i = (i >= p->leaves), leaf_j = (j >= p->leaves);
+    int leaf_i = (p->leaf[i] == 1), leaf_j = (p->leaf[j] == 1);
     if (leaf_i && leaf_j) {
         push_pair(&p->p2p, &p->np2p, &p->cap_p2p, i, j);
         return;
@@ -501,6 +507,8 @@ static orc_plan_t *plan_create(int64_t N, const double *x, const double *y, cons
     p->lo = (int64_t *)calloc((size_t)p->nodes + 1, sizeof(int64_t));
     p->hi = (int64_t *)calloc((size_t)p->nodes + 1, sizeof(int64_t));
     p->bbox = (double *)calloc(6 * ((size_t)p->nodes + 1), sizeof(double));
+    p->leaf = (signed char *)malloc((size_t)p->nodes + 1);
+    memset(p->leaf, 2, (size_t)p->nodes + 1); /* slots that subdivide never reaches stay unused */
     if (tree_mode == ORC_TREE_MORTON_MEDIAN)
         morton_order(p);
     subdivide(p, 1, 0, N, 0);
@@ -517,7 +525,7 @@ void orc_plan_destroy(orc_plan_t *p)
 {
     if (!p) return;
     free(p->x); free(p->y); free(p->z); free(p->w); free(p->pm); free(p->perm);
-    free(p->lo); free(p->hi); free(p->bbox); free(p->p2p); free(p->m2l); free(p->tcpp); free(p->tcpc); free(p->M);
+    free(p->lo); free(p->hi); free(p->leaf); free(p->bbox); free(p->p2p); free(p->m2l); free(p->tcpp); free(p->tcpc); free(p->M);
     free(p);
 }
 
@@ -545,6 +553,12 @@ void orc_plan_nodes(const orc_plan_t *p, int64_t *lo, int64_t *hi, double *bbox)
         hi[i - 1] = p->hi[i];
         memcpy(&bbox[6 * (i - 1)], &p->bbox[6 * i], 6 * sizeof(double));
     }
+}
+
+void orc_plan_leaf_flags(const orc_plan_t *p, int8_t *leaf)
+{
+    for (int64_t i = 1; i <= p->nodes; ++i)
+        leaf[i - 1] = (int8_t)p->leaf[i];
 }
 
 void orc_plan_lists(const orc_plan_t *p, int32_t *p2p_t, int32_t *p2p_s, int32_t *m2l_t, int32_t *m2l_s)
@@ -642,12 +656,13 @@ static void upward(orc_plan_t *p)
     size_t P4 = 4 * (size_t)p->P;
     p->M = (double *)calloc(P4 * ((size_t)p->nodes + 1), sizeof(double));
 #pragma omp parallel for schedule(dynamic, 1)
-    for (int64_t i = p->leaves; i <= p->nodes; ++i)
-        p2m_node(p, i, &p->M[P4 * i]);
+    for (int64_t i = 1; i <= p->nodes; ++i)
+        if (p->leaf[i] == 1) p2m_node(p, i, &p->M[P4 * i]); /* Alg 5.5: P2M where children(S) is empty */
     for (int level = p->kappa - 1; level >= 0; --level) {
         int64_t first = (int64_t)1 << level;
 #pragma omp parallel for schedule(dynamic, 1)
         for (int64_t i = first; i < 2 * first; ++i) {
+            if (p->leaf[i] != 0) continue; /* a leaf or an unused slot has no children */
             m2m(p, i, 2 * i, p->M);
             m2m(p, i, 2 * i + 1, p->M);
         }
@@ -810,8 +825,8 @@ static void treecode_lists(orc_plan_t *p)
     int32_t *sp2p = p->p2p, *sm2l = p->m2l;
     int64_t np2p = p->np2p, nm2l = p->nm2l, cp2p = p->cap_p2p, cm2l = p->cap_m2l;
     p->p2p = NULL; p->m2l = NULL; p->np2p = p->nm2l = p->cap_p2p = p->cap_m2l = 0;
-    for (int64_t t = p->leaves; t <= p->nodes; ++t)
-        dualtraversefillitl(p, t, 1);
+    for (int64_t t = 1; t <= p->nodes; ++t)
+        if (p->leaf[t] == 1) dualtraversefillitl(p, t, 1);
     qsort(p->p2p, (size_t)p->np2p, 2 * sizeof(int32_t), cmp_pair);
     qsort(p->m2l, (size_t)p->nm2l, 2 * sizeof(int32_t), cmp_pair);
     p->tcpp = p->p2p; p->ntcpp = p->np2p; p->cap_tcpp = p->cap_p2p;
@@ -866,7 +881,7 @@ int orc_eval_treecode(orc_plan_t *p, double *Ex, double *Ey, double *Ez, double 
     csr_offsets(p->tcpp, p->ntcpp, p->nodes, offp);
     csr_offsets(p->tcpc, p->ntcpc, p->nodes, offc);
 #pragma omp parallel for schedule(dynamic, 1)
-    for (int64_t t = p->leaves; t <= p->nodes; ++t) {
+    for (int64_t t = 1; t <= p->nodes; ++t) { /* (only leaves have rows) */
         for (int64_t k = offp[t]; k < offp[t + 1]; ++k) p2p(p, t, p->tcpp[2 * k + 1], near);
         for (int64_t k = offc[t]; k < offc[t + 1]; ++k) pc(p, t, p->tcpc[2 * k + 1], far);
     }
@@ -896,7 +911,7 @@ int orc_eval(orc_plan_t *p, int64_t nsel, const int64_t *sel, int part,
     if (nsel > 0) { /* only the chains root -> selected leaf */
         need = (char *)calloc((size_t)p->nodes + 1, 1);
         for (int64_t k = 0; k < nsel; ++k) {
-            if (sel[k] < p->leaves || sel[k] > p->nodes) {
+            if (sel[k] < 1 || sel[k] > p->nodes || p->leaf[sel[k]] != 1) {
                 free(need);
                 return -1;
             }
@@ -916,7 +931,7 @@ int orc_eval(orc_plan_t *p, int64_t nsel, const int64_t *sel, int part,
         int64_t *off = (int64_t *)malloc(sizeof(int64_t) * ((size_t)p->nodes + 2));
         csr_offsets(p->p2p, p->np2p, p->nodes, off);
 #pragma omp parallel for schedule(dynamic, 1)
-        for (int64_t t = p->leaves; t <= p->nodes; ++t) {
+        for (int64_t t = 1; t <= p->nodes; ++t) { /* (only leaves have rows) */
             if (need && !need[t]) continue;
             for (int64_t k = off[t]; k < off[t + 1]; ++k)
                 p2p(p, t, p->p2p[2 * k + 1], near);
@@ -929,12 +944,13 @@ int orc_eval(orc_plan_t *p, int64_t nsel, const int64_t *sel, int part,
 #pragma omp parallel for schedule(dynamic, 1)
             for (int64_t c = first; c < 2 * first; ++c) {
                 if (need && !need[c]) continue;
+                if (p->leaf[c] == 2) continue; /* unused slot: its parent is a leaf */
                 l2l(p, c, c / 2, L);
             }
         }
 #pragma omp parallel for schedule(dynamic, 1)
-        for (int64_t t = p->leaves; t <= p->nodes; ++t) {
-            if (need && !need[t]) continue;
+        for (int64_t t = 1; t <= p->nodes; ++t) {
+            if (p->leaf[t] != 1 || (need && !need[t])) continue;
             l2p(p, t, L, far);
         }
         if (L_out)
@@ -942,8 +958,8 @@ int orc_eval(orc_plan_t *p, int64_t nsel, const int64_t *sel, int part,
     }
     double cE, cB;
     prefactors(p->raw, &cE, &cB);
-    for (int64_t t = p->leaves; t <= p->nodes; ++t) {
-        if (need && !need[t]) continue;
+    for (int64_t t = 1; t <= p->nodes; ++t) {
+        if (p->leaf[t] != 1 || (need && !need[t])) continue;
         for (int64_t k = p->lo[t]; k < p->hi[t]; ++k) {
             int64_t i = p->perm[k];
             double v[6];

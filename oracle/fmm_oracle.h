@@ -45,6 +45,12 @@ extern "C" {
 #define ORC_KERNEL_SOURCE_MOMENTUM 2  /* near field (P2P, direct) stretched along the source's own momentum,
                                          D = |d|^2 + (p_j.d)^2 (alternative reading of Alg 5.10, G6);
                                          the far field keeps eq. (3.2) with gamma_bar                      */
+#define ORC_TREE_STOP_AT_N0        4  /* Alg 5.2 as printed: a cluster is split only while |S| > N0,
+                                         so a cluster of exactly N0 particles one level above kappa stays a leaf and the
+                                         tree is not balanced (leaves on levels kappa-1 and kappa).
+                                         It sits in the same array of section 8: the slots below such
+                                         a leaf are unused (range [0,0), zero box).  Default (flag clear): reading T-1,
+                                         every node of level kappa is a leaf.                              */
 
 typedef struct orc_plan orc_plan_t;
 
@@ -86,6 +92,9 @@ double orc_plan_gamma_bar(const orc_plan_t *);
 void orc_plan_perm(const orc_plan_t *, int64_t *perm);
 /* node i = 1..nodes (heap index): lo[i-1], hi[i-1] (half-open), bbox[(i-1)*6 + {ax,ay,az,bx,by,bz}] */
 void orc_plan_nodes(const orc_plan_t *, int64_t *lo, int64_t *hi, double *bbox);
+/* leaf[i-1] = 1 if heap node i is a leaf, 0 if it has children, 2 if the slot is unused (below a leaf of level
+ * kappa-1, ORC_TREE_STOP_AT_N0 only) */
+void orc_plan_leaf_flags(const orc_plan_t *, int8_t *leaf);
 /* lists sorted by (target, source); node ids are heap indices (root = 1). */
 void orc_plan_lists(const orc_plan_t *, int32_t *p2p_t, int32_t *p2p_s, int32_t *m2l_t, int32_t *m2l_s);
 
