@@ -84,6 +84,13 @@ extern "C" {
 #define FMM_TREE_MORTON_MEDIAN 1u   /* particle order = 63-bit Morton key of the stretched, cube-
                                        normalised coordinates, same closed-form ranges (DESIGN T-3') */
 #define FMM_TREE_MASK          1u
+#define FMM_TREE_STOP_AT_N0    32u  /* non-balanced tree: Alg 5.2 as printed
+                                       splits a cluster only while |S| > N0, so a cluster of exactly N0 particles on level
+                                       kappa-1 stays a leaf; leaves then sit on levels kappa-1 and kappa of the same array
+                                       tree and the two slots below such a leaf are unused.  It differs
+                                       from the default (every node of level kappa is a leaf) only when
+                                       floor(N / 2^(kappa-1)) == N0; either tree order.  In the export the unused slots
+                                       have the range [0, 0), a zero box and zero expansions.              */
 #define FMM_RAW_SUMS           4u   /* skip the prefactors of eq. (3.1)                          */
 #define FMM_KERNEL_MEAN_GAMMA      0u  /* eq. (3.2) with gamma_bar in near and far field (default)    */
 #define FMM_KERNEL_SOURCE_MOMENTUM 8u  /* alternative reading of Alg 5.10 (PAPER.md:393-394 write
@@ -146,7 +153,7 @@ typedef struct {
     int64_t workspace_bytes;                /* device bytes currently held by the plan            */
     int32_t p2p_split, m2l_split;           /* row chunks per target of the near / far pair kernels (partial sums added in order) */
     int32_t p2p_mutual;                     /* 1: the near field evaluates every mated pair of leaves once for both directions   */
-    int32_t reserved;
+    int32_t early_leaves;                   /* FMM_TREE_STOP_AT_N0: leaves on level kappa-1 (0 otherwise)                        */
     int64_t react_particles;                /* particles in the reaction segments of the mutual near field (6 doubles each)       */
 } fmm_stats_t;
 

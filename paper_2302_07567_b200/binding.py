@@ -22,6 +22,7 @@ LIB_PATH = HERE / "libfmm_b200.so"
 FMM_MAX_ORDER = 12
 FMM_TREE_KD = 0
 FMM_TREE_MORTON_MEDIAN = 1
+FMM_TREE_STOP_AT_N0 = 32
 FMM_RAW_SUMS = 4
 FMM_KERNEL_MEAN_GAMMA = 0
 FMM_KERNEL_SOURCE_MOMENTUM = 8
@@ -54,7 +55,7 @@ class fmm_stats_t(C.Structure):
                 ("timing_valid", C.c_int32), ("ms_tree", C.c_float), ("ms_lists", C.c_float),
                 ("ms_p2m", C.c_float), ("ms_m2m", C.c_float), ("ms_m2l", C.c_float), ("ms_l2l", C.c_float),
                 ("ms_p2p", C.c_float), ("ms_l2p", C.c_float), ("workspace_bytes", C.c_int64),
-                ("p2p_split", C.c_int32), ("m2l_split", C.c_int32), ("p2p_mutual", C.c_int32), ("reserved", C.c_int32),
+                ("p2p_split", C.c_int32), ("m2l_split", C.c_int32), ("p2p_mutual", C.c_int32), ("early_leaves", C.c_int32),
                 ("react_particles", C.c_int64)]
 
     def as_dict(self) -> dict:

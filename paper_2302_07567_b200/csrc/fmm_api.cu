@@ -4,6 +4,7 @@
 #include "fmm_internal.cuh"
 
 #include <math.h>
+#include <algorithm>
 #include <new>
 
 std::atomic<int64_t> g_fmm_launches{0};
@@ -302,6 +303,18 @@ extern "C" int fmm_plan_create(fmm_plan_t **out, const fmm_particles_t *in, cons
     p->kappa = kappa;
     p->leaves = (int64_t)1 << kappa;
     p->nodes = ((int64_t)2 << kappa) - 1;
+    p->stop_level = -1;
+    p->early_leaves = 0;
+    p->maxleaf = (int)((p->N + p->leaves - 1) / p->leaves);
+    if ((p->flags & FMM_TREE_STOP_AT_N0) && kappa >= 1) {
+        // sizes on level kappa-1 are floor or ceil of N / 2^(kappa-1) > N0: clusters of exactly N0 exist iff the floor is N0
+        const int64_t m = (int64_t)1 << (kappa - 1);
+        if (p->N / m == p->N0) {
+            p->stop_level = kappa - 1;
+            p->early_leaves = (int)(m - p->N % m);
+            p->maxleaf = p->N0;
+        }
+    }
     int rc = FMM_OK;
     for (int k = 0; k < EV_COUNT && rc == FMM_OK; ++k)
         if (cudaEventCreate(&p->ev[k]) != cudaSuccess) rc = FMM_ECUDA;
@@ -444,6 +457,7 @@ extern "C" int fmm_plan_stats(fmm_plan_t *p, fmm_stats_t *s)
     s->m2l_split = p->m2l_split;
     s->p2p_mutual = (p->p2p_mutual && p->p2p_dst != NULL) ? 1 : 0;
     s->react_particles = s->p2p_mutual ? p->p2p_react : 0;
+    s->early_leaves = p->early_leaves;
     if (p->timing && p->ev_valid) {
         fmm_ctx *c = &p->ctx;
         FMM_CUDA(c, cudaEventSynchronize(p->ev[EV_END]));
@@ -483,14 +497,57 @@ extern "C" int fmm_plan_export(fmm_plan_t *p, fmm_export_t *o)
         for (size_t k = 0; k < nodes; ++k) o->node_hi[k] = tmp[k];
     }
     if (o->bbox) FMM_CUDA(c, cudaMemcpy(o->bbox, p->bbox + 6, sizeof(double) * 6 * nodes, cudaMemcpyDeviceToHost));
-    if (o->p2p_off) FMM_CUDA(c, cudaMemcpy(o->p2p_off, p->p2p_off + 1, sizeof(int32_t) * (nodes + 1), cudaMemcpyDeviceToHost));
-    if (o->m2l_off) FMM_CUDA(c, cudaMemcpy(o->m2l_off, p->m2l_off + 1, sizeof(int32_t) * (nodes + 1), cudaMemcpyDeviceToHost));
-    if (o->p2p_src && p->n_p2p > 0)
-        FMM_CUDA(c, cudaMemcpy(o->p2p_src, p->p2p_src, sizeof(int32_t) * (size_t)p->n_p2p, cudaMemcpyDeviceToHost));
-    if (o->m2l_src && p->n_m2l > 0)
-        FMM_CUDA(c, cudaMemcpy(o->m2l_src, p->m2l_src, sizeof(int32_t) * (size_t)p->n_m2l, cudaMemcpyDeviceToHost));
     if (o->M) FMM_CUDA(c, cudaMemcpy(o->M, p->M + 4 * (size_t)p->P, sizeof(double) * 4 * (size_t)p->P * nodes, cudaMemcpyDeviceToHost));
     if (o->L) FMM_CUDA(c, cudaMemcpy(o->L, p->L + 6 * (size_t)p->P, sizeof(double) * 6 * (size_t)p->P * nodes, cudaMemcpyDeviceToHost));
+    if (p->stop_level < 0) {
+        if (o->p2p_off) FMM_CUDA(c, cudaMemcpy(o->p2p_off, p->p2p_off + 1, sizeof(int32_t) * (nodes + 1), cudaMemcpyDeviceToHost));
+        if (o->m2l_off) FMM_CUDA(c, cudaMemcpy(o->m2l_off, p->m2l_off + 1, sizeof(int32_t) * (nodes + 1), cudaMemcpyDeviceToHost));
+        if (o->p2p_src && p->n_p2p > 0)
+            FMM_CUDA(c, cudaMemcpy(o->p2p_src, p->p2p_src, sizeof(int32_t) * (size_t)p->n_p2p, cudaMemcpyDeviceToHost));
+        if (o->m2l_src && p->n_m2l > 0)
+            FMM_CUDA(c, cudaMemcpy(o->m2l_src, p->m2l_src, sizeof(int32_t) * (size_t)p->n_m2l, cudaMemcpyDeviceToHost));
+        return FMM_OK;
+    }
+    // FMM_TREE_STOP_AT_N0: inside the library a leaf S of level kappa-1 works through its slot 2S (fmm_internal.cuh).  The
+    // export shows the tree of Alg 5.2: S is the leaf, its two slots are unused (range [0, 0), zeros), and the lists name S.
+    std::vector<int32_t> lo(nodes + 1), hi(nodes + 1);
+    FMM_CUDA(c, cudaMemcpy(lo.data(), p->node_lo, sizeof(int32_t) * (nodes + 1), cudaMemcpyDeviceToHost));
+    FMM_CUDA(c, cudaMemcpy(hi.data(), p->node_hi, sizeof(int32_t) * (nodes + 1), cudaMemcpyDeviceToHost));
+    const size_t leaves = (size_t)p->leaves;
+    std::vector<char> early(nodes + 2, 0);  // early[S] for S on level kappa-1; early[2S] = early[2S+1] = 2: unused slot
+    for (size_t S = leaves / 2; S < leaves; ++S)
+        if (hi[S] - lo[S] <= p->N0) { early[S] = 1; early[2 * S] = early[2 * S + 1] = 2; }
+    for (size_t i = 1; i <= nodes; ++i) {
+        if (early[i] != 2) continue;
+        if (o->node_lo) o->node_lo[i - 1] = 0;
+        if (o->node_hi) o->node_hi[i - 1] = 0;
+        if (o->bbox) memset(o->bbox + 6 * (i - 1), 0, sizeof(double) * 6);
+        if (o->M) memset(o->M + 4 * (size_t)p->P * (i - 1), 0, sizeof(double) * 4 * (size_t)p->P);
+        if (o->L) memset(o->L + 6 * (size_t)p->P * (i - 1), 0, sizeof(double) * 6 * (size_t)p->P);
+    }
+    auto name_of = [&](int32_t id) -> int32_t { return early[(size_t)id] == 2 ? id / 2 : id; };  // (only the left slot 2S is ever named)
+    auto remap = [&](const int32_t *dev_off, const int32_t *dev_src, int64_t n, int32_t *out_off, int32_t *out_src) -> int {
+        if (!out_off && !out_src) return FMM_OK;
+        std::vector<int32_t> off(nodes + 2), src((size_t)(n > 0 ? n : 1)), row;
+        FMM_CUDA(c, cudaMemcpy(off.data(), dev_off, sizeof(int32_t) * (nodes + 2), cudaMemcpyDeviceToHost));
+        if (n > 0) FMM_CUDA(c, cudaMemcpy(src.data(), dev_src, sizeof(int32_t) * (size_t)n, cudaMemcpyDeviceToHost));
+        int32_t at = 0;
+        for (size_t t = 1; t <= nodes; ++t) {  // out_off[t - 1] = start of the row of node t, out_off[nodes] = length
+            if (out_off) out_off[t - 1] = at;
+            if (early[t] == 2) continue;  // unused slot
+            row.assign(src.begin() + off[t], src.begin() + off[t + 1]);
+            if (early[t] == 1)  // P2P (and the treecode's particle-cluster) rows of S are kept under its slot 2S
+                row.insert(row.end(), src.begin() + off[2 * t], src.begin() + off[2 * t + 1]);
+            for (auto &v : row) v = name_of(v);
+            std::sort(row.begin(), row.end());  // ascending source id in the new names (D-4)
+            if (out_src) memcpy(out_src + at, row.data(), sizeof(int32_t) * row.size());
+            at += (int32_t)row.size();
+        }
+        if (out_off) out_off[nodes] = at;
+        return FMM_OK;
+    };
+    FMM_TRY(remap(p->p2p_off, p->p2p_src, p->n_p2p, o->p2p_off, o->p2p_src));
+    FMM_TRY(remap(p->m2l_off, p->m2l_src, p->n_m2l, o->m2l_off, o->m2l_src));
     return FMM_OK;
 }
 

@@ -45,6 +45,13 @@ int ctx_arena_begin(fmm_ctx *c, size_t estimate);
 void ctx_arena_end(fmm_ctx *c);
 void ctx_free_all(fmm_ctx *c);
 int ctx_cuda_fail(fmm_ctx *c, cudaError_t e, const char *what);
+
+// T-2: position that separates the children of the cluster [lo, hi) of `level`: the left child gets ceil(size / 2);
+// a cluster of level stop_level with at most N0 particles is not split (FMM_TREE_STOP_AT_N0): everything stays left.
+__host__ __device__ __forceinline__ int fmm_split_mid(int lo, int hi, int level, int stop_level, int N0)
+{
+    return (level == stop_level && hi - lo <= N0) ? hi : lo + (hi - lo + 1) / 2;
+}
 #define FMM_CUDA(c, call)                                                  \
     do {                                                                   \
         cudaError_t e__ = (call);                                          \
@@ -79,6 +86,13 @@ struct fmm_plan {
     int64_t N;
     int n, n1, P, N0, kappa;
     int64_t nodes, leaves;
+    // FMM_TREE_STOP_AT_N0 (Alg 5.2 as printed): a cluster of level stop_level = kappa-1 that holds at most N0 particles is a
+    // leaf.  In this library such a leaf S keeps its two slots: slot 2S holds all its particles (same range, same box), slot
+    // 2S+1 is empty, so that every kernel that works on "the leaves" still works on level kappa; the transfer matrices between
+    // S and 2S are identities (equal boxes, exact-hit rule I-4), so M_S and L_2S are exact copies.  Only the traversal knows:
+    // it treats S as a leaf and names it 2S in the P2P list; fmm_plan_export translates back.  -1: no such cluster.
+    int stop_level, early_leaves;
+    int maxleaf;            // largest leaf: N0 with early leaves, else ceil(N / 2^kappa)
     double theta, gamma_bar, gamma_bar_param;
     fmm_hdr *hdr;           // device
     int ranges_done;        // node_lo / node_hi are filled (they depend on N and N0 only)

@@ -25,6 +25,7 @@ struct dtt_counters {           // device
 
 struct dtt_args {
     int nsteps, leaves, key_shift, treecode_leaves;
+    int early_first, N0;        // FMM_TREE_STOP_AT_N0: a node >= early_first (level kappa-1) with at most N0 particles is a leaf (else INT_MAX)
     unsigned int roots;         // breadth-first until the frontier holds this many pairs, then one depth-first walk per pair
     double theta2;
     const fmm_hdr *hdr;
@@ -45,7 +46,8 @@ __device__ __forceinline__ int dtt_decide(const dtt_args &a, double gamma_bar, i
     const int ni = a.node_hi[i] - a.node_lo[i], nj = a.node_hi[j] - a.node_lo[j];
     *nj_out = nj;
     if (ni <= 0 || nj <= 0) return 0;
-    const bool leaf_i = i >= a.leaves, leaf_j = j >= a.leaves;
+    // children(S) empty (Alg 5.2): level kappa, or a cluster of level kappa-1 that was not split (FMM_TREE_STOP_AT_N0)
+    const bool leaf_i = i >= a.leaves || (i >= a.early_first && ni <= a.N0), leaf_j = j >= a.leaves || (j >= a.early_first && nj <= a.N0);
     if (leaf_i && leaf_j) return 1;  // D-1: leaf-leaf -> P2P, no admissibility test
     // D-2: Alg 5.6-5.8 squared; every product and sum rounded separately, in this order
     const double *gi = a.geo + 4 * (int64_t)i, *gj = a.geo + 4 * (int64_t)j;
@@ -73,6 +75,9 @@ __device__ __forceinline__ void dtt_emit(const dtt_args &a, int kind, int i, int
 {
     dtt_counters *cnt = a.cnt;
     if (kind == 1) {
+        // a leaf S of level kappa-1 goes by the name of its slot 2S on level kappa, which holds the same particles (fmm_internal.cuh)
+        if (i < a.leaves) i *= 2;
+        if (j < a.leaves) j *= 2;
         const unsigned int pos = dtt_slot(&cnt->n_p2p);
         if (pos < a.cap) a.p2p[pos] = ((uint64_t)i << a.key_shift) | (uint64_t)j; else cnt->overflow = 1;
         atomicAdd(&a.rows[i], 1);
@@ -461,7 +466,7 @@ int dtt_build_lists(fmm_plan *p)
     const int key_shift = p->kappa + 2;  // node ids < 2^(kappa+1)
     const int nsteps = 2 * p->kappa + 1;
     const int rows_len = (int)p->nodes + 2;
-    const int64_t maxleaf = (p->N + p->leaves - 1) / p->leaves;
+    const int64_t maxleaf = p->maxleaf;
     // the mean-gamma kernel is antisymmetric in the pair, the source-momentum kernel (D depends on p_j) is not
     const bool mutual = !(p->flags & FMM_KERNEL_SOURCE_MOMENTUM) && maxleaf <= 1024;
     dtt_counters h;
@@ -502,6 +507,7 @@ int dtt_build_lists(fmm_plan *p)
         }
         dtt_args a;
         a.nsteps = nsteps; a.leaves = (int)p->leaves; a.key_shift = key_shift;
+        a.early_first = p->stop_level >= 0 ? (int)(p->leaves / 2) : 0x7fffffff; a.N0 = p->N0;
         a.treecode_leaves = (p->flags & FMM_METHOD_TREECODE) ? (int)p->leaves : 0;
         a.theta2 = p->theta * p->theta;
         a.roots = (unsigned int)(p->leaves / 4 < 4096 ? 4096 : (p->leaves / 4 > 65536 ? 65536 : p->leaves / 4));

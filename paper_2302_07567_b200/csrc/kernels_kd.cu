@@ -236,7 +236,7 @@ __global__ void __launch_bounds__(1024) kd_sort_small(int N, int npow2 /* >= 128
 // ---------------------------------------------------------------------------------------
 // Alg 5.2 (readings G7, G8): in the list of the split axis the first ceil(size/2) members of the
 // node (ranked by (coordinate, index)) go to the left child: their bits are set.
-__global__ void __launch_bounds__(256) kd_mark(int N, int level, const double *__restrict__ x, const double *__restrict__ y,
+__global__ void __launch_bounds__(256) kd_mark(int N, int level, int stop_level, int N0, const double *__restrict__ x, const double *__restrict__ y,
                                                const double *__restrict__ z, const uint32_t *__restrict__ lists,
                                                const fmm_hdr *__restrict__ hdr, uint32_t *__restrict__ bits,
                                                uint8_t *__restrict__ node_axis /* [2^level] */)
@@ -263,7 +263,7 @@ __global__ void __launch_bounds__(256) kd_mark(int N, int level, const double *_
     for (int i = start + threadIdx.x; i < end; i += 256) {
         const int k = (i >= s_hi[0]) ? 1 : 0;
         const int lo = s_lo[k], hi = s_hi[k];
-        const int mid = lo + (hi - lo + 1) / 2;
+        const int mid = fmm_split_mid(lo, hi, level, stop_level, N0);
         if (i < mid) {
             const uint32_t p = lists[(size_t)s_axis[k] * N + i];
             atomicOr(&bits[p >> 5], 1u << (p & 31));
@@ -306,7 +306,7 @@ __device__ __forceinline__ unsigned long long kd_pub_word(int level, unsigned lo
     return ((unsigned long long)(level + 1) << 40) | (status << 32) | (unsigned long long)(unsigned int)value;
 }
 
-__global__ void __launch_bounds__(256, 6) kd_split(int N, int level, int tiles_per_list, const uint32_t *__restrict__ bits,
+__global__ void __launch_bounds__(256, 6) kd_split(int N, int level, int stop_level, int N0, int tiles_per_list, const uint32_t *__restrict__ bits,
                                                    const uint8_t *__restrict__ node_axis, const uint32_t *__restrict__ cur,
                                                    uint32_t *__restrict__ nxt, unsigned long long *pub /* [4 tiles_per_list] */)
 {
@@ -330,7 +330,7 @@ __global__ void __launch_bounds__(256, 6) kd_split(int N, int level, int tiles_p
         int lo2;
         kd_range_of(N, level, hiA, lo2, hiB);
     }
-    const int midA = loA + (hiA - loA + 1) / 2, midB = hiA + (hiB - hiA + 1) / 2;
+    const int midA = fmm_split_mid(loA, hiA, level, stop_level, N0), midB = fmm_split_mid(hiA, hiB, level, stop_level, N0);
     const bool axisA = node_axis[nodeA] == li, axisB = (hiA < end) && node_axis[nodeA + 1] == li;
     const uint32_t *L = cur + (size_t)li * N;
     uint32_t *O = nxt + (size_t)li * N;
@@ -470,7 +470,7 @@ __device__ __forceinline__ void kdl_sub_of(int lo, int hi, int depth, int pos, i
     }
 }
 
-__global__ void __launch_bounds__(KDL_THREADS) kd_local(int N, int level0, int kappa, const double *__restrict__ x, const double *__restrict__ y,
+__global__ void __launch_bounds__(KDL_THREADS) kd_local(int N, int level0, int kappa, int stop_level, int N0, const double *__restrict__ x, const double *__restrict__ y,
                                                         const double *__restrict__ z, const fmm_hdr *__restrict__ hdr,
                                                         const uint32_t *__restrict__ lists, uint16_t *names /* [N] scratch */,
                                                         uint32_t *__restrict__ order)
@@ -535,7 +535,7 @@ __global__ void __launch_bounds__(KDL_THREADS) kd_local(int N, int level0, int k
                     int a, b, sk;
                     kdl_sub_of(lo, hi, depth, lo + i, a, b, sk);
                     slo[k] = a - lo;
-                    smid[k] = a - lo + (b - a + 1) / 2;
+                    smid[k] = fmm_split_mid(a, b, level, stop_level, N0) - lo;  // (a cluster that stays a leaf keeps its order)
                     const int ax = S.axis[sk];
                     const uint16_t name = (ax == 0) ? n3[0].h[k] : (ax == 1) ? n3[1].h[k] : n3[2].h[k];
                     S.flag[name] = (uint8_t)(i < smid[k]);  // Alg 5.2: the first ceil(size/2) along the split axis go left
@@ -652,9 +652,9 @@ int kd_build_order(fmm_plan *p, const fmm_particles_t *in, uint32_t **order_out)
         FMM_CUDA(c, cudaMemsetAsync(pub, 0, sizeof(unsigned long long) * 4 * (size_t)tiles, st));
         for (int level = 0; level < level0; ++level) {
             FMM_CUDA(c, cudaMemsetAsync(bits, 0, sizeof(uint32_t) * nbits, st));
-            kd_mark<<<tiles, 256, 0, st>>>(N, level, in->x, in->y, in->z, cur, p->hdr, bits, node_axis);
+            kd_mark<<<tiles, 256, 0, st>>>(N, level, p->stop_level, p->N0, in->x, in->y, in->z, cur, p->hdr, bits, node_axis);
             FMM_LAUNCH_CHECK(c, "kd_mark");
-            kd_split<<<dim3(tiles, 4), 256, 0, st>>>(N, level, tiles, bits, node_axis, cur, nxt, pub);
+            kd_split<<<dim3(tiles, 4), 256, 0, st>>>(N, level, p->stop_level, p->N0, tiles, bits, node_axis, cur, nxt, pub);
             FMM_LAUNCH_CHECK(c, "kd_split");
             uint32_t *t = cur; cur = nxt; nxt = t;
         }
@@ -665,7 +665,7 @@ int kd_build_order(fmm_plan *p, const fmm_particles_t *in, uint32_t **order_out)
         FMM_CUDA(c, cudaFuncSetAttribute((const void *)kd_local, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         uint32_t *order = nxt;  // (the other list buffer is free now: [0, N) takes the order, the rest the name map)
         uint16_t *names = reinterpret_cast<uint16_t *>(nxt + (size_t)N);
-        kd_local<<<1u << level0, KDL_THREADS, smem, st>>>(N, level0, p->kappa, in->x, in->y, in->z, p->hdr, cur, names, order);
+        kd_local<<<1u << level0, KDL_THREADS, smem, st>>>(N, level0, p->kappa, p->stop_level, p->N0, in->x, in->y, in->z, p->hdr, cur, names, order);
         FMM_LAUNCH_CHECK(c, "kd_local");
         *order_out = order;
     } else {

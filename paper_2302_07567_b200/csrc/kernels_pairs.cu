@@ -446,7 +446,7 @@ static bool p2p_use_mutual(const fmm_plan *p, int maxleaf) { return p->p2p_mutua
 int pairs_p2p_prepare(fmm_plan *p)  // after the lists: choose the row split and size the partial buffers
 {
     fmm_ctx *c = &p->ctx;
-    int maxleaf = (int)((p->N + p->leaves - 1) / p->leaves);
+    int maxleaf = p->maxleaf;
     int nt, threads, K;
     if (p2p_use_mutual(p, maxleaf) && p->p2p_react > p->react_cap) {
         if (p->react) ctx_free(c, p->react);
@@ -474,7 +474,7 @@ int pairs_p2p_prepare(fmm_plan *p)  // after the lists: choose the row split and
 int pairs_p2p(fmm_plan *p)
 {
     fmm_ctx *c = &p->ctx;
-    int maxleaf = (int)((p->N + p->leaves - 1) / p->leaves);
+    int maxleaf = p->maxleaf;
     int nt, threads, K;
     p2p_shape(p->leaves, maxleaf, p->p2p_pairs, p->p2p_max_row, &nt, &threads, &K, p2p_use_mutual(p, maxleaf));
     K = p->p2p_split;
@@ -1225,7 +1225,7 @@ int pairs_m2l(fmm_plan *p)
 int pairs_pc(fmm_plan *p)  // treecode: particle-cluster sums into partial buffer p2p_split
 {
     fmm_ctx *c = &p->ctx;
-    int maxleaf = (int)((p->N + p->leaves - 1) / p->leaves);
+    int maxleaf = p->maxleaf;
     int nt, threads, K;
     p2p_shape(p->leaves, maxleaf, p->p2p_pairs, p->p2p_max_row, &nt, &threads, &K);
 #define PC_LAUNCH(NT)                                                                                                            \

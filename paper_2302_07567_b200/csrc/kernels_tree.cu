@@ -9,14 +9,15 @@
 // ---------------------------------------------------------------------------------------
 // closed-form node ranges (DESIGN T-2): root [0,N); left child gets ceil(size/2)
 // ---------------------------------------------------------------------------------------
-__global__ void node_ranges_kernel(int N, int kappa, int nodes, int32_t *__restrict__ node_lo, int32_t *__restrict__ node_hi)
+__global__ void node_ranges_kernel(int N, int kappa, int nodes, int stop_level, int N0, int32_t *__restrict__ node_lo,
+                                   int32_t *__restrict__ node_hi)
 {
     int i = blockIdx.x * blockDim.x + threadIdx.x + 1;  // heap id
     if (i > nodes) return;
     int level = 31 - __clz(i);
     int lo = 0, hi = N;
     for (int b = level - 1; b >= 0; --b) {
-        int mid = lo + (hi - lo + 1) / 2;
+        int mid = fmm_split_mid(lo, hi, level - 1 - b, stop_level, N0);
         if ((i >> b) & 1) lo = mid; else hi = mid;
     }
     node_lo[i] = lo;
@@ -440,7 +441,7 @@ int tree_build(fmm_plan *p, const fmm_particles_t *in)
     const int gN = (N + T - 1) / T;
 
     if (!p->ranges_done) {  // closed-form ranges (T-2): they depend on (N, N0) only
-        node_ranges_kernel<<<(unsigned)((p->nodes + T - 1) / T), T, 0, st>>>(N, p->kappa, (int)p->nodes, p->node_lo, p->node_hi);
+        node_ranges_kernel<<<(unsigned)((p->nodes + T - 1) / T), T, 0, st>>>(N, p->kappa, (int)p->nodes, p->stop_level, p->N0, p->node_lo, p->node_hi);
         FMM_LAUNCH_CHECK(c, "node_ranges_kernel");
         p->ranges_done = 1;
     }
