@@ -67,6 +67,10 @@ def lib():
         _lib.orc_plan_nodes.argtypes = [C.c_void_p, _i64p, _i64p, _dp]
         _lib.orc_plan_lists.argtypes = [C.c_void_p, _i32p, _i32p, _i32p, _i32p]
         _lib.orc_plan_leaf_flags.argtypes = [C.c_void_p, C.POINTER(C.c_int8)]
+        _lib.orc_plan_set_lists.restype = C.c_int
+        _lib.orc_plan_set_lists.argtypes = [C.c_void_p, C.c_int64, _i32p, _i32p, C.c_int64, _i32p, _i32p]
+        _lib.orc_plan_eta_eff.restype = C.c_double
+        _lib.orc_plan_eta_eff.argtypes = [C.c_void_p]
         _lib.orc_upward.argtypes = [C.c_void_p, _dp]
         _lib.orc_p2m_node.argtypes = [C.c_void_p, C.c_int64, _dp]
         _lib.orc_eval.restype = C.c_int
@@ -203,6 +207,19 @@ class Plan:
              np.empty(self.n_m2l, dtype=np.int32), np.empty(self.n_m2l, dtype=np.int32)]
         lib().orc_plan_lists(self._h, *[v.ctypes.data_as(_i32p) for v in a])
         return np.stack(a[:2], axis=1), np.stack(a[2:], axis=1)
+
+    def set_lists(self, p2p, m2l):
+        """Replace both lists by (target, source) pairs kept from an earlier traversal (refit with list reuse)."""
+        a = [np.ascontiguousarray(np.asarray(v, dtype=np.int32).reshape(-1, 2)[:, k]) for v in (p2p, m2l) for k in (0, 1)]
+        rc = lib().orc_plan_set_lists(self._h, len(a[0]), a[0].ctypes.data_as(_i32p), a[1].ctypes.data_as(_i32p),
+                                      len(a[2]), a[2].ctypes.data_as(_i32p), a[3].ctypes.data_as(_i32p))
+        if rc != 0:
+            raise ValueError("orc_plan_set_lists: bad node id")
+        self.n_p2p, self.n_m2l = len(a[0]), len(a[2])
+
+    def eta_eff(self) -> float:
+        """max over the M2L list of max(diam S_t, diam S_s) / dist(S_t, S_s) with the plan's boxes (Alg 5.6-5.8)."""
+        return float(lib().orc_plan_eta_eff(self._h))
 
     def upward(self) -> np.ndarray:
         M = np.empty((self.nodes, self.P, 4))

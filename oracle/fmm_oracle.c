@@ -555,6 +555,38 @@ void orc_plan_nodes(const orc_plan_t *p, int64_t *lo, int64_t *hi, double *bbox)
     }
 }
 
+int orc_plan_set_lists(orc_plan_t *p, int64_t np2p, const int32_t *p2p_t, const int32_t *p2p_s,
+                       int64_t nm2l, const int32_t *m2l_t, const int32_t *m2l_s)
+{
+    for (int64_t k = 0; k < np2p; ++k) {
+        if (p2p_t[k] < 1 || p2p_t[k] > p->nodes || p2p_s[k] < 1 || p2p_s[k] > p->nodes) return -1;
+        if (p->leaf[p2p_t[k]] != 1 || p->leaf[p2p_s[k]] != 1) return -1;
+    }
+    for (int64_t k = 0; k < nm2l; ++k)
+        if (m2l_t[k] < 1 || m2l_t[k] > p->nodes || m2l_s[k] < 1 || m2l_s[k] > p->nodes ||
+            p->leaf[m2l_t[k]] == 2 || p->leaf[m2l_s[k]] == 2)
+            return -1;
+    p->np2p = p->nm2l = 0;
+    for (int64_t k = 0; k < np2p; ++k) push_pair(&p->p2p, &p->np2p, &p->cap_p2p, p2p_t[k], p2p_s[k]);
+    for (int64_t k = 0; k < nm2l; ++k) push_pair(&p->m2l, &p->nm2l, &p->cap_m2l, m2l_t[k], m2l_s[k]);
+    qsort(p->p2p, (size_t)p->np2p, 2 * sizeof(int32_t), cmp_pair);
+    qsort(p->m2l, (size_t)p->nm2l, 2 * sizeof(int32_t), cmp_pair);
+    return 0;
+}
+
+double orc_plan_eta_eff(const orc_plan_t *p)
+{
+    double worst = 0.0;
+    for (int64_t k = 0; k < p->nm2l; ++k) {
+        int64_t i = p->m2l[2 * k], j = p->m2l[2 * k + 1];
+        double ri = diam2(p, i), rj = diam2(p, j), d2 = dist2(p, i, j);
+        double ratio = ((ri > rj) ? ri : rj) / d2; /* Alg 5.8 squared: admissible iff ratio < theta^2 */
+        if (ratio != ratio) ratio = INFINITY;      /* two point clusters at one place */
+        if (ratio > worst) worst = ratio;
+    }
+    return sqrt(worst);
+}
+
 void orc_plan_leaf_flags(const orc_plan_t *p, int8_t *leaf)
 {
     for (int64_t i = 1; i <= p->nodes; ++i)

@@ -98,6 +98,15 @@ void orc_plan_leaf_flags(const orc_plan_t *, int8_t *leaf);
 /* lists sorted by (target, source); node ids are heap indices (root = 1). */
 void orc_plan_lists(const orc_plan_t *, int32_t *p2p_t, int32_t *p2p_s, int32_t *m2l_t, int32_t *m2l_s);
 
+/* Lists kept from an earlier traversal (refit with list reuse): replaces both lists of the plan
+ * by the caller's pairs (heap ids; every target / source of the P2P list must be a leaf of this plan), sorted by
+ * (target, source) here.  Alg 5.12 is then evaluated over them exactly as over its own.  Returns 0, or -1 for a bad id. */
+int orc_plan_set_lists(orc_plan_t *, int64_t np2p, const int32_t *p2p_t, const int32_t *p2p_s,
+                       int64_t nm2l, const int32_t *m2l_t, const int32_t *m2l_s);
+/* The largest max(diam S_t, diam S_s) / dist(S_t, S_s) (Alg 5.6-5.8) over the plan's M2L list, with
+ * the plan's boxes and gamma_bar: below theta for lists the plan's own traversal made (Alg 5.8); 0 for an empty list. */
+double orc_plan_eta_eff(const orc_plan_t *);
+
 /* Upward pass (Alg 5.5). M_out (may be NULL) receives [nodes][P][4] = (q*gamma, q*px, q*py, q*pz)
  * moments, node i at row i-1, proxy nu = (nu1*(n+1)+nu2)*(n+1)+nu3. */
 void orc_upward(orc_plan_t *, double *M_out);
