@@ -192,6 +192,17 @@ int fmm_plan_update(fmm_plan_t *plan, const fmm_particles_t *particles);
  * order of accuracy; it is no longer the median split of the NEW positions.  Waits for the stream once. */
 int fmm_plan_refit(fmm_plan_t *plan, const fmm_particles_t *particles);
 
+/* Refit that also keeps BOTH INTERACTION LISTS of the last build ("reuse lists while particles move
+ * little"): no sort and no traversal; gamma_bar, the source weights, the tight boxes and what hangs on them (transfer
+ * matrices, proxy points, moments) are recomputed.  The kept lists still cover every ordered pair of leaves exactly once
+ * (Alg 5.11 decides that on index ranges, which have not changed), so the result is a complete sum; what can degrade is the
+ * accuracy of a kept far pair whose boxes no longer meet eq. (4.3).  *eta_eff (HOST pointer, may be NULL)
+ * receives the largest max(diam S_t, diam S_s) / dist(S_t, S_s) (Alg 5.6-5.8 with the new gamma_bar) over the kept M2L list:
+ * eta_eff < theta means every kept far pair is still admissible; the caller rebuilds (fmm_plan_refit / fmm_plan_update) when
+ * it has grown past what it accepts (+inf if two clusters of a kept pair now share their centre; 0 with an empty M2L list).
+ * Needs a valid plan; FMM_EINVAL with FMM_METHOD_TREECODE.  Waits for the stream once; errors as fmm_plan_refit. */
+int fmm_plan_refit_keep_lists(fmm_plan_t *plan, const fmm_particles_t *particles, double *eta_eff);
+
 /* a4-a10: P2M, M2M, M2L, P2P, L2L, L2P, prefactors, scatter to caller order.  Enqueue only.
  * Ex..Bz: device arrays of length N, overwritten. */
 int fmm_eval(fmm_plan_t *plan, double *Ex, double *Ey, double *Ez, double *Bx, double *By, double *Bz);

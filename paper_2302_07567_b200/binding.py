@@ -68,7 +68,7 @@ class fmm_export_t(C.Structure):
                 ("M", C.c_void_p), ("L", C.c_void_p)]
 
 
-EXPORTED_SYMBOLS = ["fmm_plan_create", "fmm_plan_update", "fmm_plan_refit", "fmm_eval", "fmm_direct", "fmm_field_host",
+EXPORTED_SYMBOLS = ["fmm_plan_create", "fmm_plan_update", "fmm_plan_refit", "fmm_plan_refit_keep_lists", "fmm_eval", "fmm_direct", "fmm_field_host",
                     "fmm_plan_set_timing", "fmm_plan_set_overlap", "fmm_plan_stats", "fmm_plan_export", "fmm_plan_destroy",
                     "fmm_launch_count", "fmm_strerror", "fmm_last_error", "fmm_version"]
 
@@ -96,6 +96,8 @@ def load_library():
     lib.fmm_plan_update.argtypes = [vp, C.POINTER(fmm_particles_t)]
     lib.fmm_plan_refit.restype = C.c_int
     lib.fmm_plan_refit.argtypes = [vp, C.POINTER(fmm_particles_t)]
+    lib.fmm_plan_refit_keep_lists.restype = C.c_int
+    lib.fmm_plan_refit_keep_lists.argtypes = [vp, C.POINTER(fmm_particles_t), C.POINTER(C.c_double)]
     lib.fmm_eval.restype = C.c_int
     lib.fmm_eval.argtypes = [vp] + [vp] * 6
     lib.fmm_direct.restype = C.c_int
@@ -235,6 +237,10 @@ class Plan:
     def update(self, x, y, z, px, py, pz, q=None):
         return fmm_plan_update(self, x, y, z, px, py, pz, q)
 
+    def refit_keep_lists(self, x, y, z, px, py, pz, q=None) -> float:
+        """fmm_plan_refit_keep_lists: returns eta_eff, the largest admissibility ratio of the kept far pairs."""
+        return fmm_plan_refit_keep_lists(self, x, y, z, px, py, pz, q)
+
     def refit(self, x, y, z, px, py, pz, q=None):
         return fmm_plan_refit(self, x, y, z, px, py, pz, q)
 
@@ -297,6 +303,17 @@ def fmm_plan_refit(plan: Plan, x, y, z, px, py, pz, q=None):
         parts, keep = _particles(x, y, z, px, py, pz, q, plan.device)
         _check(lib.fmm_plan_refit(plan._h, C.byref(parts)), plan._h)
         del keep
+
+
+def fmm_plan_refit_keep_lists(plan: Plan, x, y, z, px, py, pz, q=None) -> float:
+    """Keeps the particle order AND both lists of the last build; new gamma_bar, boxes and moments.  Returns eta_eff."""
+    lib = load_library()
+    eta = C.c_double(0.0)
+    with torch.cuda.device(plan.device), _on_plan_stream(plan):
+        parts, keep = _particles(x, y, z, px, py, pz, q, plan.device)
+        _check(lib.fmm_plan_refit_keep_lists(plan._h, C.byref(parts), C.byref(eta)), plan._h)
+        del keep
+    return float(eta.value)
 
 
 def fmm_eval(plan: Plan, out=None):

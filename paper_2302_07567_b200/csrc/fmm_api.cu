@@ -230,9 +230,13 @@ int plan_upward(fmm_plan *p)
     return FMM_OK;
 }
 
-static int plan_build(fmm_plan *p, const fmm_particles_t *in, bool refit = false)
+static int plan_build(fmm_plan *p, const fmm_particles_t *in, bool refit = false, bool keep_lists = false, double *eta_eff = NULL)
 {
     fmm_ctx *c = &p->ctx;
+    if (keep_lists && !p->valid) {
+        snprintf(c->err, sizeof(c->err), "fmm_plan_refit_keep_lists: the plan has no valid lists to keep");
+        return FMM_EINVAL;
+    }
     p->valid = 0;  // a build that fails part-way leaves lists that must not be used (fmm_eval then returns FMM_EINVAL)
     // scratch of the whole build from one arena block: sort keys and index lists of the tree (about 100 N bytes), frontier
     // and pair buffers of the traversal; sized from the last build once there was one
@@ -251,6 +255,10 @@ static int plan_build(fmm_plan *p, const fmm_particles_t *in, bool refit = false
         FMM_TRY(tree_scan_inputs(p, in));  // a0: gamma_bar, coordinate ranges, input check -> p->hdr (device)
         FMM_TRY(refit ? tree_refit(p, in) : tree_build(p, in));
         FMM_CUDA(c, cudaEventRecord(p->ev_plan[1], c->stream));
+        if (keep_lists) {
+            FMM_TRY(dtt_keep_lists(p, eta_eff));
+            break;
+        }
         FMM_TRY(dtt_build_lists(p));       // (reads gamma_bar and the input check back together with the list lengths; records
                                            //  ev_plan[2] behind its last kernel and enqueues the upward pass before it waits)
         if (!p->kd_retry) break;
@@ -346,6 +354,13 @@ extern "C" int fmm_plan_refit(fmm_plan_t *p, const fmm_particles_t *in)
 {
     if (!p || check_particles(in) != FMM_OK || in->N != p->N) return FMM_EINVAL;
     return plan_build(p, in, true);
+}
+
+extern "C" int fmm_plan_refit_keep_lists(fmm_plan_t *p, const fmm_particles_t *in, double *eta_eff)
+{
+    if (!p || check_particles(in) != FMM_OK || in->N != p->N) return FMM_EINVAL;
+    if (p->flags & FMM_METHOD_TREECODE) return FMM_EINVAL;
+    return plan_build(p, in, true, true, eta_eff);
 }
 
 extern "C" int fmm_plan_set_overlap(fmm_plan_t *p, int on)

@@ -163,6 +163,7 @@ int tree_boxes(fmm_plan *p);
 int tree_refit(fmm_plan *p, const fmm_particles_t *in);  // keeps the particle order of the last build
 // ---- kernels_dtt.cu -----------------------------------------------------------------
 int dtt_build_lists(fmm_plan *p);
+int dtt_keep_lists(fmm_plan *p, double *eta_eff /* host */);  // refit without a traversal: checks the kept far pairs
 // ---- kernels_interp.cu --------------------------------------------------------------
 int interp_transfer_tables(fmm_plan *p);  // after the boxes of a build
 int plan_upward(fmm_plan *p);  // a4 + a5 once per build (fmm_api.cu)

@@ -459,6 +459,71 @@ static int ensure_list(fmm_ctx *c, int32_t **buf, int64_t have, int64_t want)
     return *buf ? FMM_OK : FMM_ENOMEM;
 }
 
+// Lists kept across a refit (fmm_plan_refit_keep_lists): the two lists still cover every pair of leaves exactly once --
+// that is a property of the tree's index ranges alone -- but the boxes have moved, so a kept far pair may no longer meet
+// eq. (4.3).  One pass over the M2L list with the new boxes: the largest max(r_t^2, r_s^2) / d^2 (Alg 5.6-5.8 squared, same
+// rounding order as the traversal), kept as the bit pattern of a non-negative double (monotone as an integer).
+__global__ void __launch_bounds__(256) m2l_ratio_max(int nodes, const fmm_hdr *__restrict__ hdr, const double *__restrict__ geo,
+                                                     const int32_t *__restrict__ m2l_off, const int32_t *__restrict__ m2l_src,
+                                                     unsigned long long *__restrict__ out)
+{
+    const double gamma_bar = hdr->gamma_bar;
+    double worst = 0.0;
+    for (int t = blockIdx.x * blockDim.x + threadIdx.x + 1; t <= nodes; t += gridDim.x * blockDim.x) {
+        const int a = m2l_off[t], b = m2l_off[t + 1];
+        if (b <= a) continue;
+        const double *gi = geo + 4 * (int64_t)t;
+        for (int k = a; k < b; ++k) {
+            const double *gj = geo + 4 * (int64_t)m2l_src[k];
+            const double ex = __dmul_rn(1.0, __dsub_rn(gi[1], gj[1]));
+            const double ey = __dmul_rn(1.0, __dsub_rn(gi[2], gj[2]));
+            const double ez = __dmul_rn(gamma_bar, __dsub_rn(gi[3], gj[3]));
+            const double d2 = __dadd_rn(__dadd_rn(__dmul_rn(ex, ex), __dmul_rn(ey, ey)), __dmul_rn(ez, ez));
+            const double rmax = (gi[0] > gj[0]) ? gi[0] : gj[0];
+            double ratio = __ddiv_rn(rmax, d2);  // (d2 = 0: +inf, or NaN for two point clusters at one place -> reported as +inf)
+            if (ratio != ratio) ratio = INFINITY;
+            worst = ratio > worst ? ratio : worst;
+        }
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        const double v = __shfl_xor_sync(0xffffffffu, worst, o);
+        worst = v > worst ? v : worst;
+    }
+    if ((threadIdx.x & 31) == 0 && worst > 0.0) atomicMax(out, (unsigned long long)__double_as_longlong(worst));
+}
+
+// a3 of a refit that keeps the lists: no traversal; the admissibility ratio of the kept far pairs and the build's one host wait
+int dtt_keep_lists(fmm_plan *p, double *eta_eff /* host */)
+{
+    fmm_ctx *c = &p->ctx;
+    cudaStream_t st = c->stream;
+    unsigned long long *slot = (unsigned long long *)ctx_alloc(c, sizeof(unsigned long long));
+    if (!slot) return FMM_ENOMEM;
+    FMM_CUDA(c, cudaMemsetAsync(slot, 0, sizeof(unsigned long long), st));
+    const int blocks = (int)((p->nodes + 255) / 256 < 4 * FMM_SM_COUNT ? (p->nodes + 255) / 256 : 4 * FMM_SM_COUNT);
+    m2l_ratio_max<<<blocks, 256, 0, st>>>((int)p->nodes, p->hdr, p->node_geo, p->m2l_off, p->m2l_src, slot);
+    FMM_LAUNCH_CHECK(c, "m2l_ratio_max");
+    unsigned long long bits = 0;
+    fmm_hdr hh;
+    FMM_CUDA(c, cudaMemcpyAsync(&bits, slot, sizeof(bits), cudaMemcpyDeviceToHost, st));
+    FMM_CUDA(c, cudaMemcpyAsync(&hh, p->hdr, sizeof(hh), cudaMemcpyDeviceToHost, st));
+    FMM_CUDA(c, cudaEventRecord(p->ev_plan[2], st));
+    FMM_TRY(plan_upward(p));  // (as in a build: the GPU works on the moments while the host waits)
+    FMM_CUDA(c, cudaEventSynchronize(p->ev_plan[2]));
+    ctx_free(c, slot);
+    p->gamma_bar = hh.gamma_bar;
+    p->kd_retry = 0;
+    if (hh.nonfinite) {
+        snprintf(c->err, sizeof(c->err), "%u non-finite values among the positions, momenta and charges (or gamma_bar is not finite)", hh.nonfinite);
+        return FMM_ENONFINITE;
+    }
+    double r2;
+    memcpy(&r2, &bits, sizeof(r2));
+    if (eta_eff) *eta_eff = sqrt(r2);
+    return FMM_OK;
+}
+
 int dtt_build_lists(fmm_plan *p)
 {
     fmm_ctx *c = &p->ctx;
