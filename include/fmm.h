@@ -216,6 +216,23 @@ int fmm_direct(const fmm_particles_t *particles, double gamma_bar, uint32_t flag
                double *Ex, double *Ey, double *Ez, double *Bx, double *By, double *Bz,
                fmm_alloc_fn alloc, fmm_free_fn free_, void *user, void *cuda_stream);
 
+/* a11 for callers that must not allocate (code under CUDA graph capture, serving loops, harnesses that forbid cudaMalloc):
+ * the same sums as fmm_direct, computed by the same kernels, with NO allocation of any kind -- no allocator arguments, no
+ * cudaMalloc / cudaFree / cudaMallocAsync; kernel launches only, enqueue only.  The scratch (source weights, partial sums)
+ * is a fixed 8 MiB device array inside the library that every GPU which loads the library holds until the process exits.
+ *   Limits     N <= FMM_NOALLOC_MAX_N and n_targets <= FMM_NOALLOC_MAX_N, else FMM_EINVAL (text in fmm_last_error(NULL)).
+ *              gamma_bar must be given (> 0) unless FMM_KERNEL_SOURCE_MOMENTUM is set: computing it would need a host wait.
+ *   Sharing    every call on a device uses the same array, which keeps the last call's contents (a call writes all it
+ *              reads, so nothing needs clearing).  Calls that overlap on the GPU -- different streams or threads -- RACE on
+ *              it: issue one call at a time per device, or order them on one stream.
+ *   Accuracy   same kernels and summation scheme as fmm_direct's target-subset route; against fmm_direct the results agree
+ *              to rounding (the number of source slices, and for all-targets calls the pair-sharing kernel, may differ).
+ * Arguments as fmm_direct: device pointers, outputs of length n_targets, target_idx NULL = all N particles. */
+#define FMM_NOALLOC_MAX_N 32768
+int fmm_direct_noalloc(const fmm_particles_t *particles, double gamma_bar, uint32_t flags,
+                       int64_t n_targets, const int64_t *target_idx,
+                       double *Ex, double *Ey, double *Ez, double *Bx, double *By, double *Bz, void *cuda_stream);
+
 /* Whole of Alg 5.12 from HOST memory: copies the particles to the device, fmm_plan_create,
  * fmm_eval, copies E and B back, destroys the plan.  All pointers in `particles` and the six
  * outputs are HOST pointers (pinned memory makes the copies asynchronous).  Returns after the

@@ -68,7 +68,7 @@ class fmm_export_t(C.Structure):
                 ("M", C.c_void_p), ("L", C.c_void_p)]
 
 
-EXPORTED_SYMBOLS = ["fmm_plan_create", "fmm_plan_update", "fmm_plan_refit", "fmm_plan_refit_keep_lists", "fmm_eval", "fmm_direct", "fmm_field_host",
+EXPORTED_SYMBOLS = ["fmm_plan_create", "fmm_plan_update", "fmm_plan_refit", "fmm_plan_refit_keep_lists", "fmm_eval", "fmm_direct", "fmm_direct_noalloc", "fmm_field_host",
                     "fmm_plan_set_timing", "fmm_plan_set_overlap", "fmm_plan_stats", "fmm_plan_export", "fmm_plan_destroy",
                     "fmm_launch_count", "fmm_strerror", "fmm_last_error", "fmm_version"]
 
@@ -103,6 +103,8 @@ def load_library():
     lib.fmm_direct.restype = C.c_int
     lib.fmm_direct.argtypes = [C.POINTER(fmm_particles_t), C.c_double, C.c_uint32, C.c_int64, vp] + [vp] * 6 + \
                               [ALLOC_FN, FREE_FN, vp, vp]
+    lib.fmm_direct_noalloc.restype = C.c_int
+    lib.fmm_direct_noalloc.argtypes = [C.POINTER(fmm_particles_t), C.c_double, C.c_uint32, C.c_int64, vp] + [vp] * 6 + [vp]
     lib.fmm_field_host.restype = C.c_int
     lib.fmm_field_host.argtypes = [C.POINTER(fmm_particles_t), C.POINTER(fmm_params_t)] + [vp] * 6 + \
                                   [C.POINTER(fmm_stats_t), ALLOC_FN, FREE_FN, vp, vp]
@@ -380,6 +382,37 @@ def fmm_direct(x, y, z, px, py, pz, q=None, *, gamma_bar=0.0, flags=0, targets=N
         rc = lib.fmm_direct(C.byref(parts), float(gamma_bar), int(flags), nt, tptr,
                             *[C.c_void_p(out[k].data_ptr()) for k in range(6)],
                             alloc.alloc_cb, alloc.free_cb, None, _stream_ptr())
+        _check(rc)
+        torch.cuda.current_stream().synchronize()  # inputs (keep, tkeep) must outlive the enqueued work
+        del keep, tkeep
+    return out[:3], out[3:]
+
+
+FMM_NOALLOC_MAX_N = 32768
+
+
+def fmm_direct_noalloc(x, y, z, px, py, pz, q=None, *, gamma_bar, flags=0, targets=None, out=None, device="cuda:0"):
+    """a11 through the entry point that allocates nothing (scratch in a fixed device array of the library; N and the number
+    of targets at most FMM_NOALLOC_MAX_N; one call at a time per device).  Inputs already on the device are used in place and
+    ``out`` ([6, nt] float64 device tensor) is written in place, so that a caller who passes both makes no allocation at all.
+    Returns (E[3,nt], B[3,nt]) as views of ``out``.  Enqueue only when the inputs are device tensors."""
+    _require_cuda()
+    lib = load_library()
+    device = torch.device(device)
+    with torch.cuda.device(device):
+        parts, keep = _particles(x, y, z, px, py, pz, q, device)
+        if targets is None:
+            nt, tptr, tkeep = parts.N, None, None
+        else:
+            tkeep = targets if (torch.is_tensor(targets) and targets.is_cuda and targets.dtype == torch.int64) else \
+                torch.as_tensor(np.ascontiguousarray(targets, dtype=np.int64)).to(device)
+            nt, tptr = tkeep.numel(), C.c_void_p(tkeep.data_ptr())
+        if out is None:
+            out = torch.empty((6, nt), dtype=torch.float64, device=device)
+        if out.shape != (6, nt) or out.dtype != torch.float64 or not out.is_cuda or not out.is_contiguous():
+            raise ValueError("out must be a contiguous [6, n_targets] float64 device tensor")
+        rc = lib.fmm_direct_noalloc(C.byref(parts), float(gamma_bar), int(flags), nt, tptr,
+                                    *[C.c_void_p(out[k].data_ptr()) for k in range(6)], _stream_ptr())
         _check(rc)
         torch.cuda.current_stream().synchronize()  # inputs (keep, tkeep) must outlive the enqueued work
         del keep, tkeep

@@ -599,6 +599,29 @@ extern "C" int fmm_direct(const fmm_particles_t *in, double gamma_bar, uint32_t 
     return rc;
 }
 
+// a11 without any allocation: scratch in a file-scope device array of kernels_pairs.cu (see there)
+extern "C" int fmm_direct_noalloc(const fmm_particles_t *in, double gamma_bar, uint32_t flags, int64_t nt, const int64_t *tidx,
+                                  double *Ex, double *Ey, double *Ez, double *Bx, double *By, double *Bz, void *cuda_stream)
+{
+    if (check_particles(in) != FMM_OK || nt < 1 || !Ex || !Ey || !Ez || !Bx || !By || !Bz) return FMM_EINVAL;
+    if (!tidx && nt != in->N) return FMM_EINVAL;
+    fmm_ctx ctx;
+    ctx_init(&ctx, NULL, NULL, NULL, cuda_stream);
+    char msg[200];
+    if (in->N > FMM_NOALLOC_MAX_N || nt > FMM_NOALLOC_MAX_N) {
+        snprintf(msg, sizeof(msg), "fmm_direct_noalloc: N = %lld, n_targets = %lld exceed the fixed scratch (at most %d each); use fmm_direct",
+                 (long long)in->N, (long long)nt, FMM_NOALLOC_MAX_N);
+        ctx_set_error(&ctx, msg);
+        return FMM_EINVAL;
+    }
+    const bool sm = (flags & FMM_KERNEL_SOURCE_MOMENTUM) != 0;
+    if (!sm && !(gamma_bar > 0.0 && isfinite(gamma_bar))) {
+        ctx_set_error(&ctx, "fmm_direct_noalloc: gamma_bar must be given (> 0, finite) with the mean-gamma kernel");
+        return FMM_EINVAL;
+    }
+    return pairs_direct_noalloc(&ctx, in, sm, gamma_bar, (flags & FMM_RAW_SUMS) ? 1 : 0, nt, tidx, Ex, Ey, Ez, Bx, By, Bz);
+}
+
 // ---------------------------------------------------------------------------------------
 // whole of Alg 5.12 from host memory
 // ---------------------------------------------------------------------------------------

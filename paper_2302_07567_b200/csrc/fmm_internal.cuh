@@ -183,6 +183,8 @@ int pairs_direct(fmm_ctx *c, int64_t N, const double *x, const double *y, const 
                  const double *px, const double *py, const double *pz /* non-NULL: source-momentum kernel */,
                  double gamma_bar, int raw, int64_t nt, const int64_t *tidx,
                  double *Ex, double *Ey, double *Ez, double *Bx, double *By, double *Bz);
+int pairs_direct_noalloc(fmm_ctx *c, const fmm_particles_t *in, bool sm, double gamma_bar, int raw, int64_t nt, const int64_t *tidx,
+                         double *Ex, double *Ey, double *Ez, double *Bx, double *By, double *Bz);  // scratch in a static device array
 int pairs_source_weights(fmm_ctx *c, int64_t N, const double *px, const double *py, const double *pz,
                          const double *q, double q_scalar, double *w0, double *w1, double *w2, double *w3);
 // ---- sort.cu --------------------------------------------------------------------------

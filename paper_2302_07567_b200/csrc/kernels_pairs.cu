@@ -1242,3 +1242,78 @@ int pairs_pc(fmm_plan *p)  // treecode: particle-cluster sums into partial buffe
     FMM_LAUNCH_CHECK(c, "pc_kernel");
     return FMM_OK;
 }
+
+// ---------------------------------------------------------------------------------------
+// a11 for callers that cannot allocate (fmm_direct_noalloc, include/fmm.h): the same three kernels as the target-subset
+// route of pairs_direct -- source weights, one-sided direct sums per (target block, source slice), fixed-order reduction --
+// with their scratch (4 N weights + 6 n_targets partial sums per source slice) in ONE file-scope device array instead of
+// the caller's allocator.  Every GPU that loads the library holds these 8 MiB until the process exits.
+//   * No cudaMalloc / cudaFree / stream-ordered allocation anywhere on this route; kernel launches only.
+//   * In host code `g_noalloc_scratch` is a host-side stand-in, not a device address: the kernels get the pointer that
+//     cudaGetSymbolAddress returned for the CURRENT device (looked up once per device, kept).
+//   * Every call uses the same array and finds the last call's contents in it.  Nothing has to start at zero: the weights of
+//     all N sources and the partial sums of every (slice, target) the reduction reads are written by this call before they
+//     are read, so there is nothing to clear.  For the same reason two calls that overlap on the GPU (different streams, or
+//     different host threads) race on the array: one call at a time per device.
+// ---------------------------------------------------------------------------------------
+#include <mutex>
+
+#define NOALLOC_SCRATCH_DOUBLES ((size_t)1 << 20)                  // 8 MiB
+#define NOALLOC_WEIGHT_DOUBLES (4 * (size_t)FMM_NOALLOC_MAX_N)      // w0..w3 at a stride of FMM_NOALLOC_MAX_N (256-B aligned planes)
+static __device__ __align__(256) double g_noalloc_scratch[NOALLOC_SCRATCH_DOUBLES];
+static_assert(NOALLOC_WEIGHT_DOUBLES + 6 * (size_t)FMM_NOALLOC_MAX_N <= NOALLOC_SCRATCH_DOUBLES, "scratch too small for one source slice");
+
+static int noalloc_scratch_of_current_device(fmm_ctx *c, double **out)
+{
+    static std::mutex mu;
+    static double *addr[64] = {};
+    int dev = -1;
+    FMM_CUDA(c, cudaGetDevice(&dev));
+    if (dev < 0 || dev >= 64) return ctx_cuda_fail(c, cudaErrorInvalidDevice, "fmm_direct_noalloc: device ordinal beyond 63");
+    std::lock_guard<std::mutex> lock(mu);
+    if (!addr[dev]) {
+        double *p = NULL;
+        FMM_CUDA(c, cudaGetSymbolAddress((void **)&p, g_noalloc_scratch));  // the array's address on the current device
+        if (!p) return ctx_cuda_fail(c, cudaErrorInvalidSymbol, "fmm_direct_noalloc: cudaGetSymbolAddress returned NULL");
+        addr[dev] = p;
+    }
+    *out = addr[dev];
+    return FMM_OK;
+}
+
+int pairs_direct_noalloc(fmm_ctx *c, const fmm_particles_t *in, bool sm, double gamma_bar, int raw, int64_t nt, const int64_t *tidx,
+                         double *Ex, double *Ey, double *Ez, double *Bx, double *By, double *Bz)
+{
+    const int64_t N = in->N;
+    if (N > FMM_NOALLOC_MAX_N || nt > FMM_NOALLOC_MAX_N) return FMM_EINVAL;  // (the entry point has said why)
+    double *scratch = NULL;
+    FMM_TRY(noalloc_scratch_of_current_device(c, &scratch));
+    double *w0 = scratch, *w1 = w0 + FMM_NOALLOC_MAX_N, *w2 = w1 + FMM_NOALLOC_MAX_N, *w3 = w2 + FMM_NOALLOC_MAX_N;
+    double *part = scratch + NOALLOC_WEIGHT_DOUBLES;
+    double cE = 1.0, cB = 1.0;
+    if (!raw) {
+        cE = 1.0 / (4.0 * FMM_PI * FMM_EPS0);
+        cB = 1.0 / (4.0 * FMM_PI * FMM_EPS0 * FMM_C0);
+    }
+    source_weights_kernel<<<(unsigned)((N + 255) / 256), 256, 0, c->stream>>>(N, in->px, in->py, in->pz, in->q, in->q_scalar, w0, w1, w2, w3);
+    FMM_LAUNCH_CHECK(c, "source_weights_kernel");
+    // source slices as in pairs_direct, but no more than the partial sums the array has room for
+    const int64_t tblocks = (nt + DIRECT_TARGETS - 1) / DIRECT_TARGETS;
+    int64_t splits = (8 * 4 * FMM_SM_COUNT + tblocks - 1) / tblocks;
+    const int64_t tiles = (N + PAIR_TILE - 1) / PAIR_TILE;
+    const int64_t room = (int64_t)((NOALLOC_SCRATCH_DOUBLES - NOALLOC_WEIGHT_DOUBLES) / (6 * (size_t)nt));
+    if (splits > tiles) splits = tiles;
+    if (splits > room) splits = room;
+    if (splits < 1) splits = 1;
+    const int64_t chunk = ((tiles + splits - 1) / splits) * PAIR_TILE;
+    splits = (N + chunk - 1) / chunk;
+    const dim3 grid((unsigned)tblocks, (unsigned)splits);
+    if (sm)
+        direct_kernel<true><<<grid, DIRECT_THREADS, 0, c->stream>>>(N, gamma_bar, nt, tidx, chunk, in->x, in->y, in->z, w0, w1, w2, w3, in->px, in->py, in->pz, part);
+    else
+        direct_kernel<false><<<grid, DIRECT_THREADS, 0, c->stream>>>(N, gamma_bar, nt, tidx, chunk, in->x, in->y, in->z, w0, w1, w2, w3, NULL, NULL, NULL, part);
+    FMM_LAUNCH_CHECK(c, "direct_kernel");
+    direct_reduce<<<(unsigned)((nt + 255) / 256), 256, 0, c->stream>>>(nt, (int)splits, part, cE, cB, Ex, Ey, Ez, Bx, By, Bz);
+    FMM_LAUNCH_CHECK(c, "direct_reduce");
+    return FMM_OK;
+}
