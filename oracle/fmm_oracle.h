@@ -23,7 +23,10 @@
  * diam(S_t) > diam(S_s), ties split the source) by a plain-Python restatement of Alg 5.11 whose
  * lists must equal these exactly, incl. mirror-symmetric inputs with bit-identical radii and a
  * hand-worked example; Alg 5.1's first-maximiser rule by two- and three-way non-zero ties
- * (tests/test_oracle_traversal_pins.py).  The ABSOLUTE FMM-vs-direct error values
+ * (tests/test_oracle_traversal_pins.py); the non-balanced option ORC_TREE_STOP_AT_N0 by Alg 5.1 / 5.2 / 5.11 restated on
+ * plain index sets, Alg 5.2's invariants and brute-force coverage (tests/test_oracle_nonbalanced_pins.py); list reuse
+ * (orc_plan_set_lists, orc_plan_eta_eff) by list exchange between plans, the all-near list == direct sum and a numpy
+ * restatement of Alg 5.6-5.8 (tests/test_oracle_kept_lists_pins.py).  The ABSOLUTE FMM-vs-direct error values
  * are "parity unpinned" by the paper (Fig. 2 is an image): only their trend is pinned.
  *
  * All pointers are HOST pointers.  Arrays are caller-owned unless stated.
