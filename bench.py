@@ -54,6 +54,9 @@ def parse_args():
     ap.add_argument("--method", default="fmm", choices=["fmm", "treecode"],
                     help="Alg 5.12 (default) or the particle-cluster treecode variant (SURVEY 8(f) rank 3)")
     ap.add_argument("--overlap", action="store_true", help="run P2P on a second stream beside the far-field chain (fmm_plan_set_overlap)")
+    ap.add_argument("--plan-step", default="update", choices=["update", "refit", "keep_lists"],
+                    help="what a timed step does before fmm_eval: fmm_plan_update (a0-a3, the default and the headline), fmm_plan_refit "
+                         "(order kept: a0, a2, a3) or fmm_plan_refit_keep_lists (order and lists kept: a0, a2); SURVEY.md 8(f) rank 4")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cpu-sample-leaves", type=int, default=0,
                     help="target leaves the oracle evaluates per step (0 = all of them: a whole, unscaled step)")
@@ -64,9 +67,12 @@ def parse_args():
 
 def workload_config(w, args):
     """The same dictionary on both arms (the driver compares them)."""
-    return {"workload": w.name, "N": w.N, "order_n": w.order_n, "leaf_size": w.leaf_size, "theta": w.theta,
-            "tree": args.tree, "seed": w.seed, "precision": "fp64", "kernel": args.kernel, "method": args.method,
-            "l2": "L2 flushed (256 MiB write) before every timed step; flush not timed"}
+    cfg = {"workload": w.name, "N": w.N, "order_n": w.order_n, "leaf_size": w.leaf_size, "theta": w.theta,
+           "tree": args.tree, "seed": w.seed, "precision": "fp64", "kernel": args.kernel, "method": args.method,
+           "l2": "L2 flushed (256 MiB write) before every timed step; flush not timed"}
+    if getattr(args, "plan_step", "update") != "update":
+        cfg["plan_step"] = args.plan_step   # (not the headline: the tree order / the lists of an earlier build are reused)
+    return cfg
 
 
 # ------------------------------------------------------------------------------------------------
@@ -328,8 +334,10 @@ def run_cuda(args):
     plan.set_overlap(overlap)
     plan.set_timing(not overlap)   # per-stage events force the serial order: with overlap they are taken in a second pass
 
+    plan_step = {"update": plan.update, "refit": plan.refit, "keep_lists": plan.refit_keep_lists}[args.plan_step]
+
     def step():
-        plan.update(*d_in, w.q)     # a0-a3
+        plan_step(*d_in, w.q)       # a0-a3 (refit: without the sort; keep_lists: without the sort and the traversal)
         plan.eval(out)              # a4-a10
 
     for _ in range(args.warmup):
