@@ -200,6 +200,9 @@ int fmm_plan_refit(fmm_plan_t *plan, const fmm_particles_t *particles);
  * receives the largest max(diam S_t, diam S_s) / dist(S_t, S_s) (Alg 5.6-5.8 with the new gamma_bar) over the kept M2L list:
  * eta_eff < theta means every kept far pair is still admissible; the caller rebuilds (fmm_plan_refit / fmm_plan_update) when
  * it has grown past what it accepts (+inf if two clusters of a kept pair now share their centre; 0 with an empty M2L list).
+ * Right after a traversal the largest ratio of the list sits just below theta, so any motion pushes it over: build the plan
+ * with a margin (say theta = 0.42) and keep the lists while eta_eff <= the eta whose accuracy is wanted (say 0.5).  Past 0.5 the
+ * boxes of a "far" pair may overlap (reading G11) and the error grows at once (measured: x5 at eta_eff = 0.506).
  * Needs a valid plan; FMM_EINVAL with FMM_METHOD_TREECODE.  Waits for the stream once; errors as fmm_plan_refit. */
 int fmm_plan_refit_keep_lists(fmm_plan_t *plan, const fmm_particles_t *particles, double *eta_eff);
 

@@ -126,3 +126,34 @@ def test_keep_lists_refusals(fmm):
     E1, B1 = to_np(plan.eval())
     assert np.array_equal(E0, E1) and np.array_equal(B0, B1)   # same particles, same lists: the same result bit for bit
     plan.close()
+
+
+def test_time_stepping_policy_keeps_the_accuracy_of_a_fresh_plan(fmm):
+    """The loop of README.md: lists built with a margin (theta = 0.42), kept while eta_eff <= 0.5 (the eta whose accuracy is
+    accepted), rebuilt otherwise.  After every step the error against the all-pairs sum of the moved particles must stay at
+    the level of a plan freshly built with theta = 0.5 on those particles, and the policy must have used both branches."""
+    w = workloads.config(2, N=20000)
+    build_theta, accept, kw = 0.42, 0.5, dict(order_n=5, leaf_size=100)
+    rng = np.random.default_rng(33)
+    x, y, z = w.x.copy(), w.y.copy(), w.z.copy()
+    vel = [rng.normal(0.0, 0.01 * a.std(), w.N) for a in (x, y, z)]       # a steady drift of 1 % of the bunch size per step
+    plan = fmm.fmm_plan_create(x, y, z, w.px, w.py, w.pz, w.q, theta=build_theta, **kw)
+    kept = rebuilt = 0
+    for step in range(10):
+        x, y, z = x + vel[0], y + vel[1], z + vel[2]
+        eta = plan.refit_keep_lists(x, y, z, w.px, w.py, w.pz, w.q)
+        if eta > accept:
+            plan.refit(x, y, z, w.px, w.py, w.pz, w.q)
+            rebuilt += 1
+        else:
+            kept += 1
+        E, B = to_np(plan.eval())
+        gb = plan.stats()["gamma_bar"]
+        Ed, Bd = to_np(fmm.fmm_direct(x, y, z, w.px, w.py, w.pz, w.q, gamma_bar=gb))
+        fresh = fmm.fmm_plan_create(x, y, z, w.px, w.py, w.pz, w.q, theta=accept, gamma_bar=gb, **kw)
+        Ef, Bf = to_np(fresh.eval())
+        fresh.close()
+        assert oracle.err2(E, Ed) <= 1.5 * oracle.err2(Ef, Ed), (step, eta, oracle.err2(E, Ed), oracle.err2(Ef, Ed))
+        assert oracle.err2(B, Bd) <= 1.5 * oracle.err2(Bf, Bd), (step, eta)
+    assert kept >= 2 and rebuilt >= 1, (kept, rebuilt)
+    plan.close()
