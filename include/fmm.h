@@ -57,8 +57,9 @@
  *              stream per device (fmm_plan_set_overlap), and a per-device flag that the table
  *              of Chebyshev points has been uploaded to constant memory.  Plans are otherwise
  *              independent; one plan must not be used from two threads at once.  The only
- *              environment variable read is FMM_TEST_WALK_STACK (a smaller traversal stack,
- *              used by the tests to reach the spill path; results do not depend on it).
+ *              environment variables read are FMM_TEST_WALK_STACK (a smaller traversal stack,
+ *              used by the tests to reach the spill path) and FMM_TEST_KD_SORT_LI (the KD build
+ *              takes its large-N route on small bunches); results do not depend on either.
  *   Order      outputs are in the caller's particle order.
  *   Units      SI; eps0 = 8.8541878128e-12 F/m, c0 = 299792458 m/s (CODATA 2018), unless
  *              FMM_RAW_SUMS is set (then the bare sums without prefactors are returned).

@@ -13,9 +13,14 @@
 //      segment of all four lists stably (left members first).  One kernel each: the running count of a node that spans
 //      several tiles is looked up from the tiles before it (every tile publishes its count before it looks back, so
 //      nothing waits on a chain), node ranges are closed-form (T-2);
-//   3. once a node holds at most KD_LOCAL particles one block finishes all its remaining levels in shared memory.
+//   3. once a node holds at most KD_LOCAL particles one block finishes all its remaining levels in shared memory.  The
+//      index-ordered list LI is only needed there (ascending index inside a leaf), and a node's part of LI is just the
+//      sorted ids of its members: the block sorts them itself (kdl_sort_ids), so the level kernels of step 2 split three
+//      lists, not four (all four only when the leaves are larger than KD_LOCAL and step 3 does not run).
 // Integer / compare work only: HBM-, L2- and launch-latency-bound.
 #include "fmm_internal.cuh"
+
+#include <stdlib.h>
 
 #define KD_TILE 2048     // list entries per block of the level kernels (256 threads x 8)
 #define KD_LOCAL 4096    // nodes of at most this many particles are finished by one block
@@ -470,7 +475,61 @@ __device__ __forceinline__ void kdl_sub_of(int lo, int hi, int depth, int pos, i
     }
 }
 
-__global__ void __launch_bounds__(KDL_THREADS) kd_local(int N, int level0, int kappa, int stop_level, int N0, const double *__restrict__ x, const double *__restrict__ y,
+// ascending sort of the block's m <= KD_LOCAL member ids: thread t holds elements 8 t .. 8 t + 7; a bitonic network with
+// partner distances 1, 2, 4 in registers, 8 .. 128 by warp shuffles (partner lane = lane ^ (j / 8)) and >= 256 through `buf`
+// (shared memory, block barriers).  Padding (0xffffffff) sorts last.  All KDL_THREADS threads call it.
+__device__ __forceinline__ void kdl_sort_ids(uint32_t (&v)[KDL_ITEMS], int npow2 /* >= 256, power of two */, uint32_t *buf)
+{
+    const int t = threadIdx.x;
+    const bool active = KDL_ITEMS * t < npow2;  // (whole warps: npow2 / 8 is a multiple of 32)
+    for (int k = 2; k <= npow2; k <<= 1) {
+        for (int j = k >> 1; j > 0; j >>= 1) {
+            if (j >= 32 * KDL_ITEMS) {  // the partner thread t ^ (j / 8) sits in another warp
+                if (active) {
+#pragma unroll
+                    for (int e = 0; e < KDL_ITEMS; ++e) buf[KDL_ITEMS * t + e] = v[e];
+                }
+                __syncthreads();
+                if (active) {
+                    const int pt = t ^ (j / KDL_ITEMS);
+#pragma unroll
+                    for (int e = 0; e < KDL_ITEMS; ++e) {
+                        const int i = KDL_ITEMS * t + e;
+                        const uint32_t pv = buf[KDL_ITEMS * pt + e];
+                        const bool want_min = ((i & j) == 0) == ((i & k) == 0);
+                        if (want_min == (v[e] > pv)) v[e] = pv;
+                    }
+                }
+                __syncthreads();
+            } else if (j >= KDL_ITEMS) {  // same warp
+                if (active) {
+#pragma unroll
+                    for (int e = 0; e < KDL_ITEMS; ++e) {
+                        const int i = KDL_ITEMS * t + e;
+                        const uint32_t pv = __shfl_xor_sync(0xffffffffu, v[e], j / KDL_ITEMS);
+                        const bool want_min = ((i & j) == 0) == ((i & k) == 0);
+                        if (want_min == (v[e] > pv)) v[e] = pv;
+                    }
+                }
+            } else {  // both elements in this thread's registers (compile-time register indices)
+                static_assert(KDL_ITEMS == 8, "kdl_sort_ids is written for eight elements per thread");
+                const int base = KDL_ITEMS * t;
+#define KDL_CX(E, F)                                             \
+    {                                                            \
+        const bool up = ((base + E) & k) == 0;                   \
+        const uint32_t a = v[E], b = v[F];                       \
+        if ((a > b) == up) { v[E] = b; v[F] = a; }               \
+    }
+                if (j == 4) { KDL_CX(0, 4) KDL_CX(1, 5) KDL_CX(2, 6) KDL_CX(3, 7) }
+                else if (j == 2) { KDL_CX(0, 2) KDL_CX(1, 3) KDL_CX(4, 6) KDL_CX(5, 7) }
+                else { KDL_CX(0, 1) KDL_CX(2, 3) KDL_CX(4, 5) KDL_CX(6, 7) }
+#undef KDL_CX
+            }
+        }
+    }
+}
+
+__global__ void __launch_bounds__(KDL_THREADS) kd_local(int N, int level0, int kappa, int stop_level, int N0, int li_global, const double *__restrict__ x, const double *__restrict__ y,
                                                         const double *__restrict__ z, const fmm_hdr *__restrict__ hdr,
                                                         const uint32_t *__restrict__ lists, uint16_t *names /* [N] scratch */,
                                                         uint32_t *__restrict__ order)
@@ -487,11 +546,27 @@ __global__ void __launch_bounds__(KDL_THREADS) kd_local(int N, int level0, int k
     const double gamma_bar = hdr->gamma_bar;
     // local name of a particle = its rank in the node's (ascending) part of LI; the map particle -> name goes through a
     // global scratch array (written and read by this block only; read past L1, which may hold a neighbour's stale line)
-    for (int r = threadIdx.x; r < m; r += KDL_THREADS) {
-        const uint32_t p = lists[3 * (size_t)N + lo + r];
-        S.ids[r] = p;
-        S.L[0][3][r] = (uint16_t)r;
-        names[p] = (uint16_t)r;
+    // (the node's part of LI = its member ids in ascending order: taken from the x list and sorted here)
+    {
+        int npow2 = 32 * KDL_ITEMS;
+        while (npow2 < m) npow2 <<= 1;
+        uint32_t v[KDL_ITEMS];
+#pragma unroll
+        for (int e = 0; e < KDL_ITEMS; ++e) {
+            const int i = KDL_ITEMS * threadIdx.x + e;
+            // li_global: the level kernels carried LI along (small bunches, where sorting here costs more than a fourth list there)
+            v[e] = (i < m) ? (li_global ? lists[3 * (size_t)N + lo + i] : lists[lo + i]) : 0xffffffffu;
+        }
+        if (!li_global) kdl_sort_ids(v, npow2, S.ids);
+#pragma unroll
+        for (int e = 0; e < KDL_ITEMS; ++e) {
+            const int r = KDL_ITEMS * threadIdx.x + e;
+            if (r < m) {
+                S.ids[r] = v[e];
+                S.L[0][3][r] = (uint16_t)r;
+                names[v[e]] = (uint16_t)r;
+            }
+        }
     }
     __syncthreads();
     for (int q = threadIdx.x; q < 3 * m; q += KDL_THREADS) {
@@ -641,6 +716,10 @@ int kd_build_order(fmm_plan *p, const fmm_particles_t *in, uint32_t **order_out)
     // levels on the whole lists while a node holds more than KD_LOCAL particles ...
     int level0 = 0;
     while (level0 < p->kappa && (((int64_t)N + ((int64_t)1 << level0) - 1) >> level0) > KD_LOCAL) ++level0;
+    // LI through the level kernels, or rebuilt by kd_local from its members (one shared-memory sort per block): the sort pays
+    // from about 2^19 particles on (N = 2^20: a0-a2 0.725 -> 0.710 ms, N = 2.56e7: 15.3 -> 14.4 ms; N = 65,536: +25 us)
+    // (FMM_TEST_KD_SORT_LI: the tests take the sorting route on small bunches too)
+    const int li_global = (level0 == p->kappa || level0 == 0 || (N < (1 << 19) && !getenv("FMM_TEST_KD_SORT_LI"))) ? 1 : 0;
     uint32_t *cur = lists, *nxt = lists2;
     if (level0 > 0) {
         const int tiles = (N + 3 + KD_TILE - 1) / KD_TILE;  // (tiles of a list are shifted by up to three entries, see kd_split)
@@ -654,7 +733,7 @@ int kd_build_order(fmm_plan *p, const fmm_particles_t *in, uint32_t **order_out)
             FMM_CUDA(c, cudaMemsetAsync(bits, 0, sizeof(uint32_t) * nbits, st));
             kd_mark<<<tiles, 256, 0, st>>>(N, level, p->stop_level, p->N0, in->x, in->y, in->z, cur, p->hdr, bits, node_axis);
             FMM_LAUNCH_CHECK(c, "kd_mark");
-            kd_split<<<dim3(tiles, 4), 256, 0, st>>>(N, level, p->stop_level, p->N0, tiles, bits, node_axis, cur, nxt, pub);
+            kd_split<<<dim3(tiles, li_global ? 4 : 3), 256, 0, st>>>(N, level, p->stop_level, p->N0, tiles, bits, node_axis, cur, nxt, pub);
             FMM_LAUNCH_CHECK(c, "kd_split");
             uint32_t *t = cur; cur = nxt; nxt = t;
         }
@@ -665,7 +744,7 @@ int kd_build_order(fmm_plan *p, const fmm_particles_t *in, uint32_t **order_out)
         FMM_CUDA(c, cudaFuncSetAttribute((const void *)kd_local, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         uint32_t *order = nxt;  // (the other list buffer is free now: [0, N) takes the order, the rest the name map)
         uint16_t *names = reinterpret_cast<uint16_t *>(nxt + (size_t)N);
-        kd_local<<<1u << level0, KDL_THREADS, smem, st>>>(N, level0, p->kappa, p->stop_level, p->N0, in->x, in->y, in->z, p->hdr, cur, names, order);
+        kd_local<<<1u << level0, KDL_THREADS, smem, st>>>(N, level0, p->kappa, p->stop_level, p->N0, li_global, in->x, in->y, in->z, p->hdr, cur, names, order);
         FMM_LAUNCH_CHECK(c, "kd_local");
         *order_out = order;
     } else {

@@ -598,6 +598,27 @@ def test_traversal_spill_path(fmm, monkeypatch):
     plan.close()
 
 
+@pytest.mark.parametrize("N,N0,stop", [(20011, 128, False), (65536, 128, False), (9000, 7, False), (40970, 640, True), (5000, 300, False),
+                                       (16402, 4100, True)])
+def test_kd_order_with_li_rebuilt_by_the_leaf_blocks(fmm, monkeypatch, N, N0, stop):
+    """From 2^19 particles on the level kernels of the KD build split three lists and kd_local rebuilds the index-ordered list
+    of its node by sorting the member ids in shared memory; FMM_TEST_KD_SORT_LI takes that route on small bunches (ragged node
+    sizes, nodes of 2,500 .. 4,096 particles, leaves of 7, the non-balanced option; the last case has leaves beyond KD_LOCAL and
+    must keep all four lists).  The particle order must be the oracle's either way."""
+    w = workloads.config(2, N=N)
+    flags = fmm.FMM_TREE_STOP_AT_N0 if stop else 0
+    ref = fmm.fmm_plan_create(*w.arrays(), w.q, order_n=2, leaf_size=N0, theta=0.5, flags=flags)
+    perm_ref = ref.export()["perm"]
+    gb = ref.stats()["gamma_bar"]
+    ref.close()
+    monkeypatch.setenv("FMM_TEST_KD_SORT_LI", "1")
+    plan = fmm.fmm_plan_create(*w.arrays(), w.q, order_n=2, leaf_size=N0, theta=0.5, flags=flags)
+    perm = plan.export()["perm"]
+    plan.close()
+    op = oracle.Plan(*w.arrays(), w.q, order_n=2, leaf_size=N0, theta=0.5, gamma_bar_value=gb, stop_at_n0=stop)
+    assert np.array_equal(perm, op.perm()) and np.array_equal(perm_ref, perm)
+
+
 @pytest.mark.parametrize("kind", ["coplanar_z", "coplanar_x", "collinear_z", "at_rest", "wide_theta", "gamma_1e4"])
 def test_degenerate_geometry_and_momenta(fmm, kind):
     """Boxes with zero extent along one or two axes (their proxy points coincide there and every particle hits a node of the
