@@ -184,12 +184,14 @@ struct mut_tile {
     int dst[MUT_TILE];
 };
 
-template <int NT>
+// NL <= NT: the first NL of the thread's NT target slots are worked on (a warp whose last slot holds no particle of a ragged
+// leaf runs the NL = NT - 1 instantiation, see p2p_mutual_kernel)
+template <int NT, int NL = NT>
 __device__ __forceinline__ void mut_pair_terms(const mut_targets<NT> &T, double gb, double xs, double ys, double zs,
                                                double (&gx)[NT], double (&gy)[NT], double (&gz)[NT])
 {
 #pragma unroll
-    for (int k = 0; k < NT; ++k) {
+    for (int k = 0; k < NL; ++k) {
         const double dx = T.x[k] - xs, dy = T.y[k] - ys, dz = T.z[k] - zs;
         double D = fma(dx, dx, FMM_TINY_D);  // (> 0 also for a coincident pair: see inv_r3)
         D = fma(dy, dy, D);
@@ -200,24 +202,24 @@ __device__ __forceinline__ void mut_pair_terms(const mut_targets<NT> &T, double 
     }
 }
 
-template <int NT>
+template <int NT, int NL = NT>
 __device__ __forceinline__ void mut_target_sums(mut_targets<NT> &T, double m0, double m1, double m2, double m3,
                                                 const double (&gx)[NT], const double (&gy)[NT], const double (&gz)[NT])
 {
 #pragma unroll
-    for (int k = 0; k < NT; ++k) { T.ex[k] = fma(m0, gx[k], T.ex[k]); T.ey[k] = fma(m0, gy[k], T.ey[k]); T.ez[k] = fma(m0, gz[k], T.ez[k]); }
+    for (int k = 0; k < NL; ++k) { T.ex[k] = fma(m0, gx[k], T.ex[k]); T.ey[k] = fma(m0, gy[k], T.ey[k]); T.ez[k] = fma(m0, gz[k], T.ez[k]); }
 #pragma unroll
-    for (int k = 0; k < NT; ++k) { T.bx[k] = fma(m2, gz[k], T.bx[k]); T.bz[k] = fma(-m2, gx[k], T.bz[k]); }
+    for (int k = 0; k < NL; ++k) { T.bx[k] = fma(m2, gz[k], T.bx[k]); T.bz[k] = fma(-m2, gx[k], T.bz[k]); }
 #pragma unroll
-    for (int k = 0; k < NT; ++k) { T.by[k] = fma(m3, gx[k], T.by[k]); T.bx[k] = fma(-m3, gy[k], T.bx[k]); }
+    for (int k = 0; k < NL; ++k) { T.by[k] = fma(m3, gx[k], T.by[k]); T.bx[k] = fma(-m3, gy[k], T.bx[k]); }
 #pragma unroll
-    for (int k = 0; k < NT; ++k) { T.bz[k] = fma(m1, gy[k], T.bz[k]); T.by[k] = fma(-m1, gz[k], T.by[k]); }
+    for (int k = 0; k < NL; ++k) { T.bz[k] = fma(m1, gy[k], T.bz[k]); T.by[k] = fma(-m1, gz[k], T.by[k]); }
 }
 
-// `cnt` staged sources (a multiple of 32), both directions
-template <int NT, int W, bool ACCUM = false>  // ACCUM: add to the segment instead of overwriting it (all-pairs kernel)
-__device__ __forceinline__ void mut_process_mutual(mut_targets<NT> &T, const mut_tile &S, int cnt, double gb, double *red,
-                                                   double *__restrict__ react, size_t rstride)
+// `cnt` staged sources (a multiple of 32), both directions: this warp's part (no block barrier in here) ...
+template <int NT, int NL, int W, bool ACCUM>  // ACCUM: add to the segment instead of overwriting it (all-pairs kernel)
+__device__ __forceinline__ void mut_batches(mut_targets<NT> &T, const mut_tile &S, int cnt, double gb, double *red,
+                                            double *__restrict__ react, size_t rstride)
 {
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     for (int b0 = 0; b0 < cnt; b0 += 32) {
@@ -227,10 +229,10 @@ __device__ __forceinline__ void mut_process_mutual(mut_targets<NT> &T, const mut
             const int j = b0 + ((lane + k2) & 31);
             const double xs = S.x[j], ys = S.y[j], zs = S.z[j], m0 = S.m0[j], m1 = S.m1[j], m2 = S.m2[j], m3 = S.m3[j];
             double gx[NT], gy[NT], gz[NT];
-            mut_pair_terms<NT>(T, gb, xs, ys, zs, gx, gy, gz);
-            mut_target_sums<NT>(T, m0, m1, m2, m3, gx, gy, gz);
+            mut_pair_terms<NT, NL>(T, gb, xs, ys, zs, gx, gy, gz);
+            mut_target_sums<NT, NL>(T, m0, m1, m2, m3, gx, gy, gz);
 #pragma unroll
-            for (int k = 0; k < NT; ++k) {
+            for (int k = 0; k < NL; ++k) {
                 rex = fma(T.q0[k], gx[k], rex); rey = fma(T.q0[k], gy[k], rey); rez = fma(T.q0[k], gz[k], rez);
                 rbx = fma(T.q2[k], gz[k], rbx); rbz = fma(-T.q2[k], gx[k], rbz);
                 rby = fma(T.q3[k], gx[k], rby); rbx = fma(-T.q3[k], gy[k], rbx);
@@ -253,7 +255,13 @@ __device__ __forceinline__ void mut_process_mutual(mut_targets<NT> &T, const mut
             r[0] = rex; r[MUT_TILE] = rey; r[2 * MUT_TILE] = rez; r[3 * MUT_TILE] = rbx; r[4 * MUT_TILE] = rby; r[5 * MUT_TILE] = rbz;
         }
     }
-    if (W > 1) {  // once per tile: the warps' sums are added in warp order and stored (the caller's barrier follows)
+}
+
+// ... and, once per tile, the warps' sums added in warp order and stored (W > 1; the caller's barrier follows)
+template <int W, bool ACCUM>
+__device__ __forceinline__ void mut_reduce_tile(const mut_tile &S, int cnt, double *red, double *__restrict__ react, size_t rstride)
+{
+    if (W > 1) {
         __syncthreads();
         for (int q = threadIdx.x; q < 6 * MUT_TILE; q += 32 * W) {
             const int j = q & (MUT_TILE - 1);
@@ -271,15 +279,23 @@ __device__ __forceinline__ void mut_process_mutual(mut_targets<NT> &T, const mut
     }
 }
 
+template <int NT, int W, bool ACCUM = false>
+__device__ __forceinline__ void mut_process_mutual(mut_targets<NT> &T, const mut_tile &S, int cnt, double gb, double *red,
+                                                   double *__restrict__ react, size_t rstride)
+{
+    mut_batches<NT, NT, W, ACCUM>(T, S, cnt, gb, red, react, rstride);
+    mut_reduce_tile<W, ACCUM>(S, cnt, red, react, rstride);
+}
+
 // `cnt` staged sources acting on the targets only (broadcast reads)
-template <int NT>
+template <int NT, int NL = NT>
 __device__ __forceinline__ void mut_process_onesided(mut_targets<NT> &T, const mut_tile &S, int cnt, double gb)
 {
 #pragma unroll 2
     for (int j = 0; j < cnt; ++j) {
         double gx[NT], gy[NT], gz[NT];
-        mut_pair_terms<NT>(T, gb, S.x[j], S.y[j], S.z[j], gx, gy, gz);
-        mut_target_sums<NT>(T, S.m0[j], S.m1[j], S.m2[j], S.m3[j], gx, gy, gz);
+        mut_pair_terms<NT, NL>(T, gb, S.x[j], S.y[j], S.z[j], gx, gy, gz);
+        mut_target_sums<NT, NL>(T, S.m0[j], S.m1[j], S.m2[j], S.m3[j], gx, gy, gz);
     }
 }
 
@@ -291,7 +307,15 @@ struct mut_cfg {
     static constexpr int MINB = (WARPS / W) > 0 ? (WARPS / W) : 1;
 };
 
-template <int NT, int W, bool SPLIT>
+// RAGGED (W > 1, leaves that leave at least one whole warp-slot of the block's 32 W NT target slots empty, e.g. 313 particles
+// in 4 x 32 x 3 slots): the warps whose last slot is empty run the NL = NT - 1 instantiation of the loops, and the slot
+// assignment is rotated by the block index.  Warp w of every block sits on SM sub-partition w mod 4, so without the rotation
+// the lighter warps would always share the same sub-partitions and the heavier ones would still set the pace; with it every
+// sub-partition sees the mix and the block's FP64 work drops from W NT to ceil(leaf / 32) warp-slots.
+// Used at W = 8 only (one block per SM, so every sub-partition holds exactly one longer and one shorter warp): leaves of 625,
+// n = 8 of the paper's grid, 37.9 -> 34.7 ms.  At W = 4 (three blocks per SM) the block barriers keep every block at the pace
+// of its longer warps and the second copy of the loops only costs instruction fetches: leaves of 313, 17.7 -> 18.1 ms, not used.
+template <int NT, int W, bool SPLIT, bool RAGGED = false>
 __global__ void __launch_bounds__(32 * W, mut_cfg<NT, W>::MINB) p2p_mutual_kernel(int N, double gb, const int32_t *__restrict__ order, const int32_t *__restrict__ off,
                                                          const int32_t *__restrict__ src, const int32_t *__restrict__ dst,
                                                          const int32_t *__restrict__ node_lo, const int32_t *__restrict__ node_hi,
@@ -308,9 +332,13 @@ __global__ void __launch_bounds__(32 * W, mut_cfg<NT, W>::MINB) p2p_mutual_kerne
     const int r0 = off[t], rl = off[t + 1] - r0;
     const int e0 = SPLIT ? r0 + (int)(((int64_t)rl * kc) / K) : r0, e1 = SPLIT ? r0 + (int)(((int64_t)rl * (kc + 1)) / K) : r0 + rl;
     mut_targets<NT> T;
+    // slot k of this thread holds target tlo + k blockDim + vt; vt = the thread index, rotated by whole warps when RAGGED
+    const int vt = RAGGED ? (int)((threadIdx.x + 32u * (blockIdx.x % W)) & (32u * W - 1u)) : (int)threadIdx.x;
+    bool short_warp = false;  // (warp-uniform) the warp's last slot holds no particle at all
+    if (RAGGED) short_warp = (NT > 1) && (tlo + (NT - 1) * (int)blockDim.x + (vt & ~31) >= thi);
 #pragma unroll
     for (int k = 0; k < NT; ++k) {
-        const int i = tlo + k * blockDim.x + threadIdx.x;
+        const int i = tlo + k * blockDim.x + vt;
         const bool live = i < thi;
         T.x[k] = live ? tx[i] : 0.0; T.y[k] = live ? ty[i] : 0.0; T.z[k] = live ? tz[i] : 0.0;
         T.q0[k] = live ? w0[i] : 0.0; T.q1[k] = live ? w1[i] : 0.0; T.q2[k] = live ? w2[i] : 0.0; T.q3[k] = live ? w3[i] : 0.0;
@@ -350,8 +378,14 @@ __global__ void __launch_bounds__(32 * W, mut_cfg<NT, W>::MINB) p2p_mutual_kerne
                     fill = padded;
                 }
                 __syncthreads();
-                if (pass == 0) mut_process_mutual<NT, W>(T, S, fill, gb, mut_red, react, rstride);
-                else mut_process_onesided<NT>(T, S, fill, gb);
+                if (pass == 0) {
+                    if (RAGGED && short_warp) mut_batches<NT, (NT > 1 ? NT - 1 : 1), W, false>(T, S, fill, gb, mut_red, react, rstride);
+                    else mut_batches<NT, NT, W, false>(T, S, fill, gb, mut_red, react, rstride);
+                    mut_reduce_tile<W, false>(S, fill, mut_red, react, rstride);  // (all warps meet at its barrier)
+                } else {
+                    if (RAGGED && short_warp) mut_process_onesided<NT, (NT > 1 ? NT - 1 : 1)>(T, S, fill, gb);
+                    else mut_process_onesided<NT>(T, S, fill, gb);
+                }
                 __syncthreads();
                 fill = 0;
             }
@@ -359,7 +393,7 @@ __global__ void __launch_bounds__(32 * W, mut_cfg<NT, W>::MINB) p2p_mutual_kerne
     }
 #pragma unroll
     for (int k = 0; k < NT; ++k) {
-        const int i = tlo + k * blockDim.x + threadIdx.x;
+        const int i = tlo + k * blockDim.x + vt;
         if (i < thi) {
             double *o = near_ + (SPLIT ? (size_t)kc * 6 * (size_t)N : (size_t)0) + i;
             o[0] = T.ex[k];
@@ -482,32 +516,40 @@ int pairs_p2p(fmm_plan *p)
     p->react_used = p2p_use_mutual(p, maxleaf) ? 1 : 0;
     if (p->react_used) {
         const size_t rstride = (size_t)(p->react_cap > 0 ? p->react_cap : 1);
-#define MUT_LAUNCH(NT, W)                                                                                                                 \
-    const size_t red_bytes = (W > 1) ? sizeof(double) * 6 * MUT_TILE * W : 0;                                                             \
-    if (red_bytes + sizeof(mut_tile) > 48 * 1024) {                                                                                       \
-        FMM_CUDA(c, cudaFuncSetAttribute((const void *)p2p_mutual_kernel<NT, W, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)red_bytes));  \
-        FMM_CUDA(c, cudaFuncSetAttribute((const void *)p2p_mutual_kernel<NT, W, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)red_bytes)); \
-    }                                                                                                                                     \
-    if (K > 1)                                                                                                                            \
-        p2p_mutual_kernel<NT, W, true><<<(unsigned)(p->leaves * K), 32 * W, red_bytes, c->stream>>>(                                      \
-            (int)p->N, p->gamma_bar, p->p2p_order, p->p2p_off, p->p2p_src, p->p2p_dst, p->node_lo, p->node_hi, p->tx, p->ty, p->tz, p->w0, \
-            p->w1, p->w2, p->w3, K, p->near_, p->react, rstride);                                                                         \
-    else                                                                                                                                  \
-        p2p_mutual_kernel<NT, W, false><<<(unsigned)p->leaves, 32 * W, red_bytes, c->stream>>>(                                           \
-            (int)p->N, p->gamma_bar, p->p2p_order, p->p2p_off, p->p2p_src, p->p2p_dst, p->node_lo, p->node_hi, p->tx, p->ty, p->tz, p->w0, \
-            p->w1, p->w2, p->w3, K, p->near_, p->react, rstride)
+#define MUT_LAUNCH_R(NT, W, R)                                                                                                            \
+    {                                                                                                                                     \
+        const size_t red_bytes = (W > 1) ? sizeof(double) * 6 * MUT_TILE * W : 0;                                                         \
+        if (red_bytes + sizeof(mut_tile) > 48 * 1024) {                                                                                   \
+            FMM_CUDA(c, cudaFuncSetAttribute((const void *)p2p_mutual_kernel<NT, W, true, R>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)red_bytes));  \
+            FMM_CUDA(c, cudaFuncSetAttribute((const void *)p2p_mutual_kernel<NT, W, false, R>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)red_bytes)); \
+        }                                                                                                                                 \
+        if (K > 1)                                                                                                                        \
+            p2p_mutual_kernel<NT, W, true, R><<<(unsigned)(p->leaves * K), 32 * W, red_bytes, c->stream>>>(                               \
+                (int)p->N, p->gamma_bar, p->p2p_order, p->p2p_off, p->p2p_src, p->p2p_dst, p->node_lo, p->node_hi, p->tx, p->ty, p->tz, p->w0, \
+                p->w1, p->w2, p->w3, K, p->near_, p->react, rstride);                                                                     \
+        else                                                                                                                              \
+            p2p_mutual_kernel<NT, W, false, R><<<(unsigned)p->leaves, 32 * W, red_bytes, c->stream>>>(                                    \
+                (int)p->N, p->gamma_bar, p->p2p_order, p->p2p_off, p->p2p_src, p->p2p_dst, p->node_lo, p->node_hi, p->tx, p->ty, p->tz, p->w0, \
+                p->w1, p->w2, p->w3, K, p->near_, p->react, rstride);                                                                     \
+    }
+#define MUT_LAUNCH(NT, W) MUT_LAUNCH_R(NT, W, false)
+// eight warps per block: the ragged variant when at least one whole warp-slot of the block stays empty
+#define MUT_LAUNCH_W(NT, W)                                                       \
+    if (32 * W * NT - maxleaf >= 32) MUT_LAUNCH_R(NT, W, true) else MUT_LAUNCH_R(NT, W, false)
         const int W = threads / 32;
         if (nt == 1) { MUT_LAUNCH(1, 1); }
         else if (nt == 2) { MUT_LAUNCH(2, 1); }
         else if (nt == 3 && W == 1) { MUT_LAUNCH(3, 1); }
         else if (nt == 3 && W == 2) { MUT_LAUNCH(3, 2); }
         else if (nt == 3 && W == 4) { MUT_LAUNCH(3, 4); }
-        else if (nt == 3) { MUT_LAUNCH(3, 8); }
+        else if (nt == 3) { MUT_LAUNCH_W(3, 8); }
         else if (W == 1) { MUT_LAUNCH(4, 1); }
         else if (W == 2) { MUT_LAUNCH(4, 2); }
         else if (W == 4) { MUT_LAUNCH(4, 4); }
-        else { MUT_LAUNCH(4, 8); }
+        else { MUT_LAUNCH_W(4, 8); }
 #undef MUT_LAUNCH
+#undef MUT_LAUNCH_W
+#undef MUT_LAUNCH_R
         FMM_LAUNCH_CHECK(c, "p2p_mutual_kernel");
         return FMM_OK;
     }

@@ -619,6 +619,27 @@ def test_kd_order_with_li_rebuilt_by_the_leaf_blocks(fmm, monkeypatch, N, N0, st
     assert np.array_equal(perm, op.perm()) and np.array_equal(perm_ref, perm)
 
 
+@pytest.mark.parametrize("N,N0,cube", [(10000, 729, True), (40000, 729, True), (5003, 640, False), (200000, 900, True), (9000, 1000, False),
+                                       (5008, 343, True)])
+def test_ragged_leaves_in_the_mutual_near_field(fmm, N, N0, cube):
+    """Leaves that leave whole warp-slots of an eight-warp near-field block empty (625 particles in 8 x 32 x 3 slots, 782 or 879
+    in 8 x 32 x 4, ...): the warps with an empty last slot run the shorter loops and the slot assignment rotates with the block
+    index (p2p_mutual_kernel, RAGGED); with and without the row split; the last case (313 in 4 x 32 x 3) keeps the plain kernel.
+    Fields against the oracle, and the same bits from one evaluation to the next."""
+    w = workloads.paper_cube(N=N, order_n=2) if cube else workloads.config(2, N=N)
+    plan = fmm.fmm_plan_create(*w.arrays(), w.q, order_n=2, leaf_size=N0, theta=0.5)
+    st = plan.stats()
+    assert st["p2p_mutual"] == 1
+    E, B = to_np(plan.eval())
+    E2, B2 = to_np(plan.eval())
+    assert np.array_equal(E, E2) and np.array_equal(B, B2)
+    op = oracle.Plan(*w.arrays(), w.q, order_n=2, leaf_size=N0, theta=0.5, gamma_bar_value=st["gamma_bar"])
+    Eo, Bo = op.eval()
+    assert_close(E, Eo, "ragged leaves E")
+    assert_close(B, Bo, "ragged leaves B")
+    plan.close()
+
+
 @pytest.mark.parametrize("kind", ["coplanar_z", "coplanar_x", "collinear_z", "at_rest", "wide_theta", "gamma_1e4"])
 def test_degenerate_geometry_and_momenta(fmm, kind):
     """Boxes with zero extent along one or two axes (their proxy points coincide there and every particle hits a node of the
