@@ -93,6 +93,7 @@ struct fmm_plan {
     // it treats S as a leaf and names it 2S in the P2P list; fmm_plan_export translates back.  -1: no such cluster.
     int stop_level, early_leaves;
     int maxleaf;            // largest leaf: N0 with early leaves, else ceil(N / 2^kappa)
+#define FMM_MUTUAL_MAX_LEAF 2048  // the mutual near field holds a leaf's targets in registers: 1024 per pass, at most two passes
     double theta, gamma_bar, gamma_bar_param;
     fmm_hdr *hdr;           // device
     int ranges_done;        // node_lo / node_hi are filled (they depend on N and N0 only)

@@ -315,7 +315,9 @@ struct mut_cfg {
 // Used at W = 8 only (one block per SM, so every sub-partition holds exactly one longer and one shorter warp): leaves of 625,
 // n = 8 of the paper's grid, 37.9 -> 34.7 ms.  At W = 4 (three blocks per SM) the block barriers keep every block at the pace
 // of its longer warps and the second copy of the loops only costs instruction fetches: leaves of 313, 17.7 -> 18.1 ms, not used.
-template <int NT, int W, bool SPLIT, bool RAGGED = false>
+// TP = 2 (leaves of 1025 .. 2048 particles, W = 8): the block walks its row twice, for the first 32 W NT targets and for the
+// rest; the second walk ADDS its reaction sums to the segments the first one wrote (the same thread owns the same words).
+template <int NT, int W, bool SPLIT, bool RAGGED = false, int TP = 1>
 __global__ void __launch_bounds__(32 * W, mut_cfg<NT, W>::MINB) p2p_mutual_kernel(int N, double gb, const int32_t *__restrict__ order, const int32_t *__restrict__ off,
                                                          const int32_t *__restrict__ src, const int32_t *__restrict__ dst,
                                                          const int32_t *__restrict__ node_lo, const int32_t *__restrict__ node_hi,
@@ -328,9 +330,13 @@ __global__ void __launch_bounds__(32 * W, mut_cfg<NT, W>::MINB) p2p_mutual_kerne
     __shared__ mut_tile S;
     extern __shared__ double mut_red[];  // [W][6][MUT_TILE] reaction sums of the current tile, per warp (W > 1)
     const int t = SPLIT ? order[blockIdx.x / K] : order[blockIdx.x], kc = SPLIT ? blockIdx.x % K : 0;
-    const int tlo = node_lo[t], thi = node_hi[t];
+    const int tlo0 = node_lo[t], thi0 = node_hi[t];
     const int r0 = off[t], rl = off[t + 1] - r0;
     const int e0 = SPLIT ? r0 + (int)(((int64_t)rl * kc) / K) : r0, e1 = SPLIT ? r0 + (int)(((int64_t)rl * (kc + 1)) / K) : r0 + rl;
+#pragma unroll 1
+    for (int tp = 0; tp < TP; ++tp) {
+    const int tlo = tlo0 + tp * (32 * W * NT), thi = (TP > 1 && tp + 1 < TP) ? min(thi0, tlo + 32 * W * NT) : thi0;
+    if (TP > 1 && tp > 0) __syncthreads();  // (the tile of the walk before is no longer read)
     mut_targets<NT> T;
     // slot k of this thread holds target tlo + k blockDim + vt; vt = the thread index, rotated by whole warps when RAGGED
     const int vt = RAGGED ? (int)((threadIdx.x + 32u * (blockIdx.x % W)) & (32u * W - 1u)) : (int)threadIdx.x;
@@ -381,7 +387,9 @@ __global__ void __launch_bounds__(32 * W, mut_cfg<NT, W>::MINB) p2p_mutual_kerne
                 if (pass == 0) {
                     if (RAGGED && short_warp) mut_batches<NT, (NT > 1 ? NT - 1 : 1), W, false>(T, S, fill, gb, mut_red, react, rstride);
                     else mut_batches<NT, NT, W, false>(T, S, fill, gb, mut_red, react, rstride);
-                    mut_reduce_tile<W, false>(S, fill, mut_red, react, rstride);  // (all warps meet at its barrier)
+                    // (all warps meet at its barrier; the second walk over the row adds to what the first one stored)
+                    if (TP > 1 && tp > 0) mut_reduce_tile<W, true>(S, fill, mut_red, react, rstride);
+                    else mut_reduce_tile<W, false>(S, fill, mut_red, react, rstride);
                 } else {
                     if (RAGGED && short_warp) mut_process_onesided<NT, (NT > 1 ? NT - 1 : 1)>(T, S, fill, gb);
                     else mut_process_onesided<NT>(T, S, fill, gb);
@@ -404,6 +412,7 @@ __global__ void __launch_bounds__(32 * W, mut_cfg<NT, W>::MINB) p2p_mutual_kerne
             o[5 * (size_t)N] = T.bz[k];
         }
     }
+    }  // tp
 }
 
 // Targets per thread: the NT <= 4 that wastes the fewest lanes, ties to the larger NT (a leaf of 78 particles fills 3 x 32 slots at NT = 3 but only 78 of 128 at NT = 4).
@@ -414,7 +423,9 @@ static void p2p_shape(int64_t leaves, int maxleaf, int64_t pairs, int64_t max_ro
 {
     int best_nt = 1, best_threads = 32;
     double best_score = -1.0;
-    if (mutual && maxleaf <= 1024) {
+    if (mutual && maxleaf <= FMM_MUTUAL_MAX_LEAF) {
+        // (leaves of more than 1024 particles: two target passes of eight warps, the shape is that of half a leaf)
+        if (maxleaf > 1024) maxleaf = (maxleaf + 1) / 2;
         // W a power of two: the resident warps of an SM then split evenly over its four sub-partitions (three warps per
         // block left one sub-partition with 3 of 9 warps: 46 % instead of 59 % of peak at leaves of 312, profiles/r02_sweep_paper.md)
         int W = 1;
@@ -475,7 +486,7 @@ int pairs_m2l_prepare(fmm_plan *p)  // after the lists: M2L row split for small 
 }
 
 // the mutual kernel keeps a whole target leaf in one pass of NT x blockDim registers
-static bool p2p_use_mutual(const fmm_plan *p, int maxleaf) { return p->p2p_mutual && p->p2p_dst != NULL && maxleaf <= 1024; }
+static bool p2p_use_mutual(const fmm_plan *p, int maxleaf) { return p->p2p_mutual && p->p2p_dst != NULL && maxleaf <= FMM_MUTUAL_MAX_LEAF; }
 
 int pairs_p2p_prepare(fmm_plan *p)  // after the lists: choose the row split and size the partial buffers
 {
@@ -516,26 +527,28 @@ int pairs_p2p(fmm_plan *p)
     p->react_used = p2p_use_mutual(p, maxleaf) ? 1 : 0;
     if (p->react_used) {
         const size_t rstride = (size_t)(p->react_cap > 0 ? p->react_cap : 1);
-#define MUT_LAUNCH_R(NT, W, R)                                                                                                            \
+#define MUT_LAUNCH_R(NT, W, R, TP)                                                                                                        \
     {                                                                                                                                     \
         const size_t red_bytes = (W > 1) ? sizeof(double) * 6 * MUT_TILE * W : 0;                                                         \
         if (red_bytes + sizeof(mut_tile) > 48 * 1024) {                                                                                   \
-            FMM_CUDA(c, cudaFuncSetAttribute((const void *)p2p_mutual_kernel<NT, W, true, R>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)red_bytes));  \
-            FMM_CUDA(c, cudaFuncSetAttribute((const void *)p2p_mutual_kernel<NT, W, false, R>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)red_bytes)); \
+            FMM_CUDA(c, cudaFuncSetAttribute((const void *)p2p_mutual_kernel<NT, W, true, R, TP>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)red_bytes));  \
+            FMM_CUDA(c, cudaFuncSetAttribute((const void *)p2p_mutual_kernel<NT, W, false, R, TP>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)red_bytes)); \
         }                                                                                                                                 \
         if (K > 1)                                                                                                                        \
-            p2p_mutual_kernel<NT, W, true, R><<<(unsigned)(p->leaves * K), 32 * W, red_bytes, c->stream>>>(                               \
+            p2p_mutual_kernel<NT, W, true, R, TP><<<(unsigned)(p->leaves * K), 32 * W, red_bytes, c->stream>>>(                           \
                 (int)p->N, p->gamma_bar, p->p2p_order, p->p2p_off, p->p2p_src, p->p2p_dst, p->node_lo, p->node_hi, p->tx, p->ty, p->tz, p->w0, \
                 p->w1, p->w2, p->w3, K, p->near_, p->react, rstride);                                                                     \
         else                                                                                                                              \
-            p2p_mutual_kernel<NT, W, false, R><<<(unsigned)p->leaves, 32 * W, red_bytes, c->stream>>>(                                    \
+            p2p_mutual_kernel<NT, W, false, R, TP><<<(unsigned)p->leaves, 32 * W, red_bytes, c->stream>>>(                                \
                 (int)p->N, p->gamma_bar, p->p2p_order, p->p2p_off, p->p2p_src, p->p2p_dst, p->node_lo, p->node_hi, p->tx, p->ty, p->tz, p->w0, \
                 p->w1, p->w2, p->w3, K, p->near_, p->react, rstride);                                                                     \
     }
-#define MUT_LAUNCH(NT, W) MUT_LAUNCH_R(NT, W, false)
-// eight warps per block: the ragged variant when at least one whole warp-slot of the block stays empty
+#define MUT_LAUNCH(NT, W) MUT_LAUNCH_R(NT, W, false, 1)
+// eight warps per block: two target passes for leaves of more than 1024 particles; else the ragged variant when at least one
+// whole warp-slot of the block stays empty
 #define MUT_LAUNCH_W(NT, W)                                                       \
-    if (32 * W * NT - maxleaf >= 32) MUT_LAUNCH_R(NT, W, true) else MUT_LAUNCH_R(NT, W, false)
+    if (maxleaf > 1024) MUT_LAUNCH_R(NT, W, true, 2)                              \
+    else if (32 * W * NT - maxleaf >= 32) MUT_LAUNCH_R(NT, W, true, 1) else MUT_LAUNCH_R(NT, W, false, 1)
         const int W = threads / 32;
         if (nt == 1) { MUT_LAUNCH(1, 1); }
         else if (nt == 2) { MUT_LAUNCH(2, 1); }
