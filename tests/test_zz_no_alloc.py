@@ -103,3 +103,23 @@ def test_no_alloc_direct_at_its_size_limit_and_beyond(fmm):
     E2, B2 = fmm.fmm_direct_noalloc(*w.arrays(), w.q, gamma_bar=gb)
     import torch
     assert torch.equal(E2, E) and torch.equal(B2, B)
+
+
+def test_no_alloc_direct_tiny_inputs(fmm):
+    """One particle (no pair: zero fields), 33 particles (one ragged tile), a single target out of many."""
+    import torch
+    w = workloads.config(1, N=1)
+    E, B = fmm.fmm_direct_noalloc(*w.arrays(), w.q, gamma_bar=10.0)
+    assert E.shape == (3, 1) and not E.any() and not B.any()
+    w = workloads.config(1, N=33)
+    E, B = fmm.fmm_direct_noalloc(*w.arrays(), w.q, gamma_bar=10.0)
+    Er, Br = fmm.fmm_direct(*w.arrays(), w.q, gamma_bar=10.0)
+    assert_close(E, Er, "33 particles E")
+    assert_close(B, Br, "33 particles B")
+    w = workloads.config(2, N=20000)
+    one = np.array([12345], dtype=np.int64)
+    E, B = fmm.fmm_direct_noalloc(*w.arrays(), w.q, gamma_bar=10.0, targets=one)
+    Er, Br = fmm.fmm_direct(*w.arrays(), w.q, gamma_bar=10.0, targets=one)
+    assert E.shape == (3, 1)
+    assert_close(E, Er, "single target E")
+    assert_close(B, Br, "single target B")
