@@ -12,6 +12,8 @@
     78 / 79 particles) is compared on every particle as well;
   * the direct sum on a seeded sample of target particles (the GPU's FMM-vs-direct error must equal the
     oracle's to 3 digits);
+  * the non-balanced tree option (FMM_TREE_STOP_AT_N0) at N = 2^20 + 1, N0 = 512 (2,047 leaves one level above the rest):
+    structures in full, fields on 256 sampled leaves;
   * properties that hold at any size: bit-reproducibility, finite outputs.
 """
 import numpy as np
@@ -39,9 +41,10 @@ def _measures(f, fref):
     return float(e2), float(d)
 
 
-def _run_full(fmm, w, n_leaf_sample, n_direct_sample, seed):
+def _run_full(fmm, w, n_leaf_sample, n_direct_sample, seed, stop=False):
     import torch
-    plan = fmm.fmm_plan_create(*w.arrays(), w.q, order_n=w.order_n, leaf_size=w.leaf_size, theta=w.theta)
+    plan = fmm.fmm_plan_create(*w.arrays(), w.q, order_n=w.order_n, leaf_size=w.leaf_size, theta=w.theta,
+                               flags=fmm.FMM_TREE_STOP_AT_N0 if stop else 0)
     st = plan.stats()
     E, B = plan.eval()
     E2, B2 = plan.eval()
@@ -52,7 +55,7 @@ def _run_full(fmm, w, n_leaf_sample, n_direct_sample, seed):
     out_measures = {}
 
     op = oracle.Plan(*w.arrays(), w.q, order_n=w.order_n, leaf_size=w.leaf_size, theta=w.theta,
-                     gamma_bar_value=st["gamma_bar"])
+                     gamma_bar_value=st["gamma_bar"], stop_at_n0=stop)
     # --- integer structures: bit-exact, in full
     assert (st["kappa"], st["nodes"], st["leaves"]) == (op.kappa, op.nodes, op.leaves)
     assert np.array_equal(ex["perm"], op.perm()), "permutation differs"
@@ -73,7 +76,7 @@ def _run_full(fmm, w, n_leaf_sample, n_direct_sample, seed):
         rows = ~np.isnan(Eo[:, 0])
         assert rows.all() and rows.sum() == w.N
     else:
-        leaves = np.sort(rng.choice(op.leaves, size=n_leaf_sample, replace=False)) + op.leaves  # heap ids
+        leaves = np.sort(rng.choice(op.leaf_ids(), size=n_leaf_sample, replace=False))  # heap ids
         Eo, Bo = op.eval(leaves=leaves)
         rows = ~np.isnan(Eo[:, 0])
         assert rows.sum() >= n_leaf_sample * (w.N // op.leaves)
@@ -128,3 +131,13 @@ def test_paper_workload_full(fmm):
     w = workloads.paper_cube()
     st, err = _run_full(fmm, w, n_leaf_sample=None, n_direct_sample=256, seed=71)
     assert st["kappa"] == 14 and st["leaves"] == 16384 and err["E"] < 1e-2
+
+
+def test_non_balanced_tree_full_size(fmm):
+    """FMM_TREE_STOP_AT_N0 at N = 2^20 + 1 with N0 = 512: kappa = 12 and floor(N / 2^11) = 512, so 2,047 clusters of level 11
+    hold exactly N0 particles and stay leaves (Alg 5.2 as printed), one is split into 257 + 256.  Structures in full, fields
+    on 256 sampled leaves (early ones among them)."""
+    w = workloads.config(3, N=2 ** 20 + 1)
+    w.order_n, w.leaf_size = 4, 512
+    st, err = _run_full(fmm, w, n_leaf_sample=256, n_direct_sample=64, seed=91, stop=True)
+    assert st["kappa"] == 12 and st["early_leaves"] == 2047 and err["E"] < 1e-2
