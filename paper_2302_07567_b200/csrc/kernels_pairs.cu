@@ -216,31 +216,50 @@ __device__ __forceinline__ void mut_target_sums(mut_targets<NT> &T, double m0, d
     for (int k = 0; k < NL; ++k) { T.bz[k] = fma(m1, gy[k], T.bz[k]); T.by[k] = fma(-m1, gz[k], T.by[k]); }
 }
 
+// one step of a batch: lane l works on source b0 + (l + k2) mod 32 with its first NL target slots, then the six reaction sums
+// move on to the lane that takes this source next
+template <int NT, int NL>
+__device__ __forceinline__ void mut_step(mut_targets<NT> &T, const mut_tile &S, int b0, int lane, int k2, double gb, double &rex,
+                                         double &rey, double &rez, double &rbx, double &rby, double &rbz)
+{
+    const int j = b0 + ((lane + k2) & 31);
+    const double xs = S.x[j], ys = S.y[j], zs = S.z[j], m0 = S.m0[j], m1 = S.m1[j], m2 = S.m2[j], m3 = S.m3[j];
+    double gx[NT], gy[NT], gz[NT];
+    mut_pair_terms<NT, NL>(T, gb, xs, ys, zs, gx, gy, gz);
+    mut_target_sums<NT, NL>(T, m0, m1, m2, m3, gx, gy, gz);
+#pragma unroll
+    for (int k = 0; k < NL; ++k) {
+        rex = fma(T.q0[k], gx[k], rex); rey = fma(T.q0[k], gy[k], rey); rez = fma(T.q0[k], gz[k], rez);
+        rbx = fma(T.q2[k], gz[k], rbx); rbz = fma(-T.q2[k], gx[k], rbz);
+        rby = fma(T.q3[k], gx[k], rby); rbx = fma(-T.q3[k], gy[k], rbx);
+        rbz = fma(T.q1[k], gy[k], rbz); rby = fma(-T.q1[k], gz[k], rby);
+    }
+    const int from = (lane + 1) & 31;  // the source this lane takes next was with lane + 1
+    rex = __shfl_sync(0xffffffffu, rex, from); rey = __shfl_sync(0xffffffffu, rey, from); rez = __shfl_sync(0xffffffffu, rez, from);
+    rbx = __shfl_sync(0xffffffffu, rbx, from); rby = __shfl_sync(0xffffffffu, rby, from); rbz = __shfl_sync(0xffffffffu, rbz, from);
+}
+
 // `cnt` staged sources (a multiple of 32), both directions: this warp's part (no block barrier in here) ...
-template <int NT, int NL, int W, bool ACCUM>  // ACCUM: add to the segment instead of overwriting it (all-pairs kernel)
+// HALF (W = 1): the last target slot holds the leaf's 1 .. 15 tail particles TWICE, in lanes l and l + MUT_HALF_OFF (odd), and is
+// worked on at the even steps only: lane l then meets the sources of l's parity, lane l + MUT_HALF_OFF the others, so every
+// (tail target, source) pair is still visited exactly once while the slot costs 16 steps of a batch instead of 32.
+#define MUT_HALF_OFF 17
+template <int NT, int NL, int W, bool ACCUM, bool HALF = false>  // ACCUM: add to the segment instead of overwriting it (all-pairs kernel)
 __device__ __forceinline__ void mut_batches(mut_targets<NT> &T, const mut_tile &S, int cnt, double gb, double *red,
                                             double *__restrict__ react, size_t rstride)
 {
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     for (int b0 = 0; b0 < cnt; b0 += 32) {
         double rex = 0, rey = 0, rez = 0, rbx = 0, rby = 0, rbz = 0;  // sum_i q_i (x) g(x_i, x_j) for the source travelling through this lane
+        if (HALF) {
 #pragma unroll 1
-        for (int k2 = 0; k2 < 32; ++k2) {
-            const int j = b0 + ((lane + k2) & 31);
-            const double xs = S.x[j], ys = S.y[j], zs = S.z[j], m0 = S.m0[j], m1 = S.m1[j], m2 = S.m2[j], m3 = S.m3[j];
-            double gx[NT], gy[NT], gz[NT];
-            mut_pair_terms<NT, NL>(T, gb, xs, ys, zs, gx, gy, gz);
-            mut_target_sums<NT, NL>(T, m0, m1, m2, m3, gx, gy, gz);
-#pragma unroll
-            for (int k = 0; k < NL; ++k) {
-                rex = fma(T.q0[k], gx[k], rex); rey = fma(T.q0[k], gy[k], rey); rez = fma(T.q0[k], gz[k], rez);
-                rbx = fma(T.q2[k], gz[k], rbx); rbz = fma(-T.q2[k], gx[k], rbz);
-                rby = fma(T.q3[k], gx[k], rby); rbx = fma(-T.q3[k], gy[k], rbx);
-                rbz = fma(T.q1[k], gy[k], rbz); rby = fma(-T.q1[k], gz[k], rby);
+            for (int k2 = 0; k2 < 32; k2 += 2) {
+                mut_step<NT, NL>(T, S, b0, lane, k2, gb, rex, rey, rez, rbx, rby, rbz);
+                mut_step<NT, (NL > 1 ? NL - 1 : 1)>(T, S, b0, lane, k2 + 1, gb, rex, rey, rez, rbx, rby, rbz);
             }
-            const int from = (lane + 1) & 31;  // the source this lane takes next was with lane + 1
-            rex = __shfl_sync(0xffffffffu, rex, from); rey = __shfl_sync(0xffffffffu, rey, from); rez = __shfl_sync(0xffffffffu, rez, from);
-            rbx = __shfl_sync(0xffffffffu, rbx, from); rby = __shfl_sync(0xffffffffu, rby, from); rbz = __shfl_sync(0xffffffffu, rbz, from);
+        } else {
+#pragma unroll 1
+            for (int k2 = 0; k2 < 32; ++k2) mut_step<NT, NL>(T, S, b0, lane, k2, gb, rex, rey, rez, rbx, rby, rbz);
         }
         // lane l now holds the sums for source b0 + l over this warp's targets
         if (W == 1) {
@@ -317,7 +336,8 @@ struct mut_cfg {
 // of its longer warps and the second copy of the loops only costs instruction fetches: leaves of 313, 17.7 -> 18.1 ms, not used.
 // TP = 2 (leaves of 1025 .. 2048 particles, W = 8): the block walks its row twice, for the first 32 W NT targets and for the
 // rest; the second walk ADDS its reaction sums to the segments the first one wrote (the same thread owns the same words).
-template <int NT, int W, bool SPLIT, bool RAGGED = false, int TP = 1>
+// HALF (W = 1, NT >= 2, leaves whose last slot holds at most 15 particles, e.g. 78 = 32 + 32 + 14): see mut_batches.
+template <int NT, int W, bool SPLIT, bool RAGGED = false, int TP = 1, bool HALF = false>
 __global__ void __launch_bounds__(32 * W, mut_cfg<NT, W>::MINB) p2p_mutual_kernel(int N, double gb, const int32_t *__restrict__ order, const int32_t *__restrict__ off,
                                                          const int32_t *__restrict__ src, const int32_t *__restrict__ dst,
                                                          const int32_t *__restrict__ node_lo, const int32_t *__restrict__ node_hi,
@@ -342,18 +362,27 @@ __global__ void __launch_bounds__(32 * W, mut_cfg<NT, W>::MINB) p2p_mutual_kerne
     const int vt = RAGGED ? (int)((threadIdx.x + 32u * (blockIdx.x % W)) & (32u * W - 1u)) : (int)threadIdx.x;
     bool short_warp = false;  // (warp-uniform) the warp's last slot holds no particle at all
     if (RAGGED) short_warp = (NT > 1) && (tlo + (NT - 1) * (int)blockDim.x + (vt & ~31) >= thi);
+    // HALF: the second copy of the tail particle l sits in lane l + MUT_HALF_OFF
+    const int tail = HALF ? max(0, thi - (tlo + (NT - 1) * 32)) : 0;  // (at most 15 by the choice of the shape)
+    const bool copy_b = HALF && (int)threadIdx.x >= MUT_HALF_OFF && (int)threadIdx.x - MUT_HALF_OFF < tail;
 #pragma unroll
     for (int k = 0; k < NT; ++k) {
-        const int i = tlo + k * blockDim.x + vt;
+        int i = tlo + k * blockDim.x + vt;
+        if (HALF && k == NT - 1 && copy_b) i -= MUT_HALF_OFF;
         const bool live = i < thi;
         T.x[k] = live ? tx[i] : 0.0; T.y[k] = live ? ty[i] : 0.0; T.z[k] = live ? tz[i] : 0.0;
         T.q0[k] = live ? w0[i] : 0.0; T.q1[k] = live ? w1[i] : 0.0; T.q2[k] = live ? w2[i] : 0.0; T.q3[k] = live ? w3[i] : 0.0;
         T.ex[k] = T.ey[k] = T.ez[k] = T.bx[k] = T.by[k] = T.bz[k] = 0.0;
     }
+    double keep[6] = {0, 0, 0, 0, 0, 0};  // HALF: the second copy's sums while the one-sided pass (all sources, every step) runs
     // the row is walked twice: first the owned mutual entries (pass 0), then the one-sided ones (pass 1); the sources of a
     // pass form one stream that fills the tile across entry boundaries, so only the last tile of a pass is ragged
     for (int pass = 0; pass < 2; ++pass) {
         int fill = 0;
+        if (HALF && pass == 1) {  // the one-sided loops visit every source in every lane: only the first copy may count them
+            keep[0] = T.ex[NT - 1]; keep[1] = T.ey[NT - 1]; keep[2] = T.ez[NT - 1];
+            keep[3] = T.bx[NT - 1]; keep[4] = T.by[NT - 1]; keep[5] = T.bz[NT - 1];
+        }
         for (int e = e0; e <= e1; ++e) {
             int slo = 0, shi = 0, d = -1;
             const bool flush = (e == e1);
@@ -386,7 +415,7 @@ __global__ void __launch_bounds__(32 * W, mut_cfg<NT, W>::MINB) p2p_mutual_kerne
                 __syncthreads();
                 if (pass == 0) {
                     if (RAGGED && short_warp) mut_batches<NT, (NT > 1 ? NT - 1 : 1), W, false>(T, S, fill, gb, mut_red, react, rstride);
-                    else mut_batches<NT, NT, W, false>(T, S, fill, gb, mut_red, react, rstride);
+                    else mut_batches<NT, NT, W, false, HALF>(T, S, fill, gb, mut_red, react, rstride);
                     // (all warps meet at its barrier; the second walk over the row adds to what the first one stored)
                     if (TP > 1 && tp > 0) mut_reduce_tile<W, true>(S, fill, mut_red, react, rstride);
                     else mut_reduce_tile<W, false>(S, fill, mut_red, react, rstride);
@@ -397,6 +426,15 @@ __global__ void __launch_bounds__(32 * W, mut_cfg<NT, W>::MINB) p2p_mutual_kerne
                 __syncthreads();
                 fill = 0;
             }
+        }
+    }
+    if (HALF) {  // the tail particle's sums = first copy (mutual + one-sided entries) + second copy (its share of the mutual ones)
+        double *s6[6] = {&T.ex[NT - 1], &T.ey[NT - 1], &T.ez[NT - 1], &T.bx[NT - 1], &T.by[NT - 1], &T.bz[NT - 1]};
+#pragma unroll
+        for (int f = 0; f < 6; ++f) {
+            const double mine = copy_b ? keep[f] : *s6[f];
+            const double other = __shfl_sync(0xffffffffu, mine, (threadIdx.x + MUT_HALF_OFF) & 31);
+            *s6[f] = ((int)threadIdx.x < tail) ? mine + other : mine;
         }
     }
 #pragma unroll
@@ -527,40 +565,44 @@ int pairs_p2p(fmm_plan *p)
     p->react_used = p2p_use_mutual(p, maxleaf) ? 1 : 0;
     if (p->react_used) {
         const size_t rstride = (size_t)(p->react_cap > 0 ? p->react_cap : 1);
-#define MUT_LAUNCH_R(NT, W, R, TP)                                                                                                        \
+#define MUT_LAUNCH_R(NT, W, R, TP, H)                                                                                                     \
     {                                                                                                                                     \
         const size_t red_bytes = (W > 1) ? sizeof(double) * 6 * MUT_TILE * W : 0;                                                         \
         if (red_bytes + sizeof(mut_tile) > 48 * 1024) {                                                                                   \
-            FMM_CUDA(c, cudaFuncSetAttribute((const void *)p2p_mutual_kernel<NT, W, true, R, TP>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)red_bytes));  \
-            FMM_CUDA(c, cudaFuncSetAttribute((const void *)p2p_mutual_kernel<NT, W, false, R, TP>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)red_bytes)); \
+            FMM_CUDA(c, cudaFuncSetAttribute((const void *)p2p_mutual_kernel<NT, W, true, R, TP, H>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)red_bytes));  \
+            FMM_CUDA(c, cudaFuncSetAttribute((const void *)p2p_mutual_kernel<NT, W, false, R, TP, H>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)red_bytes)); \
         }                                                                                                                                 \
         if (K > 1)                                                                                                                        \
-            p2p_mutual_kernel<NT, W, true, R, TP><<<(unsigned)(p->leaves * K), 32 * W, red_bytes, c->stream>>>(                           \
+            p2p_mutual_kernel<NT, W, true, R, TP, H><<<(unsigned)(p->leaves * K), 32 * W, red_bytes, c->stream>>>(                        \
                 (int)p->N, p->gamma_bar, p->p2p_order, p->p2p_off, p->p2p_src, p->p2p_dst, p->node_lo, p->node_hi, p->tx, p->ty, p->tz, p->w0, \
                 p->w1, p->w2, p->w3, K, p->near_, p->react, rstride);                                                                     \
         else                                                                                                                              \
-            p2p_mutual_kernel<NT, W, false, R, TP><<<(unsigned)p->leaves, 32 * W, red_bytes, c->stream>>>(                                \
+            p2p_mutual_kernel<NT, W, false, R, TP, H><<<(unsigned)p->leaves, 32 * W, red_bytes, c->stream>>>(                             \
                 (int)p->N, p->gamma_bar, p->p2p_order, p->p2p_off, p->p2p_src, p->p2p_dst, p->node_lo, p->node_hi, p->tx, p->ty, p->tz, p->w0, \
                 p->w1, p->w2, p->w3, K, p->near_, p->react, rstride);                                                                     \
     }
-#define MUT_LAUNCH(NT, W) MUT_LAUNCH_R(NT, W, false, 1)
+#define MUT_LAUNCH(NT, W) MUT_LAUNCH_R(NT, W, false, 1, false)
+// one warp per block: the last slot at half rate when it holds at most 15 particles of the largest leaf
+#define MUT_LAUNCH_1(NT)                                                          \
+    if (maxleaf - 32 * (NT - 1) <= 15) MUT_LAUNCH_R(NT, 1, false, 1, true) else MUT_LAUNCH_R(NT, 1, false, 1, false)
 // eight warps per block: two target passes for leaves of more than 1024 particles; else the ragged variant when at least one
 // whole warp-slot of the block stays empty
 #define MUT_LAUNCH_W(NT, W)                                                       \
-    if (maxleaf > 1024) MUT_LAUNCH_R(NT, W, true, 2)                              \
-    else if (32 * W * NT - maxleaf >= 32) MUT_LAUNCH_R(NT, W, true, 1) else MUT_LAUNCH_R(NT, W, false, 1)
+    if (maxleaf > 1024) MUT_LAUNCH_R(NT, W, true, 2, false)                       \
+    else if (32 * W * NT - maxleaf >= 32) MUT_LAUNCH_R(NT, W, true, 1, false) else MUT_LAUNCH_R(NT, W, false, 1, false)
         const int W = threads / 32;
         if (nt == 1) { MUT_LAUNCH(1, 1); }
-        else if (nt == 2) { MUT_LAUNCH(2, 1); }
-        else if (nt == 3 && W == 1) { MUT_LAUNCH(3, 1); }
+        else if (nt == 2) { MUT_LAUNCH_1(2); }
+        else if (nt == 3 && W == 1) { MUT_LAUNCH_1(3); }
         else if (nt == 3 && W == 2) { MUT_LAUNCH(3, 2); }
         else if (nt == 3 && W == 4) { MUT_LAUNCH(3, 4); }
         else if (nt == 3) { MUT_LAUNCH_W(3, 8); }
-        else if (W == 1) { MUT_LAUNCH(4, 1); }
+        else if (W == 1) { MUT_LAUNCH_1(4); }
         else if (W == 2) { MUT_LAUNCH(4, 2); }
         else if (W == 4) { MUT_LAUNCH(4, 4); }
         else { MUT_LAUNCH_W(4, 8); }
 #undef MUT_LAUNCH
+#undef MUT_LAUNCH_1
 #undef MUT_LAUNCH_W
 #undef MUT_LAUNCH_R
         FMM_LAUNCH_CHECK(c, "p2p_mutual_kernel");

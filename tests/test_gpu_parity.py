@@ -643,6 +643,34 @@ def test_ragged_leaves_in_the_mutual_near_field(fmm, N, N0, cube):
     plan.close()
 
 
+@pytest.mark.parametrize("N,N0,cfg", [(5000, 40, 1), (10000, 110, 2), (13000, 110, 3), (20011, 128, 2), (80000, 125, 0), (4200, 47, 1), (1100, 79, 4)])
+def test_half_rate_tail_slot_of_one_warp_leaves(fmm, N, N0, cfg):
+    """One-warp leaves whose last target slot holds at most 15 particles (39 / 40 = 32 + 8, 78 / 79 = 64 + 15, 101 / 102 = 96 + 6,
+    33 = 32 + 1, 69 = 64 + 5): the tail sits in two lanes of opposite parity and the slot is worked on at every second step of the
+    rotation (p2p_mutual_kernel, HALF).  Fields against the oracle, the same bits from one evaluation to the next, and against the
+    all-pairs sum when nothing is admissible (every pair of leaves then goes through the near field)."""
+    w = workloads.paper_cube(N=N, order_n=3) if cfg == 0 else workloads.config(cfg, N=N)
+    for theta in (0.5, 1e-3):
+        plan = fmm.fmm_plan_create(*w.arrays(), w.q, order_n=3, leaf_size=N0, theta=theta)
+        st = plan.stats()
+        assert st["p2p_mutual"] == 1
+        E, B = to_np(plan.eval())
+        E2, B2 = to_np(plan.eval())
+        assert np.array_equal(E, E2) and np.array_equal(B, B2)
+        if theta == 0.5:
+            op = oracle.Plan(*w.arrays(), w.q, order_n=3, leaf_size=N0, theta=theta, gamma_bar_value=st["gamma_bar"])
+            Eo, Bo = op.eval()
+        elif N <= 20011:
+            assert st["n_m2l"] == 0
+            Eo, Bo = oracle.direct(*w.arrays(), w.q, gamma_bar_value=st["gamma_bar"])
+        else:
+            plan.close()
+            continue
+        assert_close(E, Eo, f"half-rate tail E (theta {theta})")
+        assert_close(B, Bo, f"half-rate tail B (theta {theta})")
+        plan.close()
+
+
 @pytest.mark.parametrize("kind", ["coplanar_z", "coplanar_x", "collinear_z", "at_rest", "wide_theta", "gamma_1e4"])
 def test_degenerate_geometry_and_momenta(fmm, kind):
     """Boxes with zero extent along one or two axes (their proxy points coincide there and every particle hits a node of the
