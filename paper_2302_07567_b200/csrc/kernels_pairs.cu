@@ -355,21 +355,39 @@ __global__ void __launch_bounds__(32 * W, mut_cfg<NT, W>::MINB) p2p_mutual_kerne
     const int e0 = SPLIT ? r0 + (int)(((int64_t)rl * kc) / K) : r0, e1 = SPLIT ? r0 + (int)(((int64_t)rl * (kc + 1)) / K) : r0 + rl;
 #pragma unroll 1
     for (int tp = 0; tp < TP; ++tp) {
-    const int tlo = tlo0 + tp * (32 * W * NT), thi = (TP > 1 && tp + 1 < TP) ? min(thi0, tlo + 32 * W * NT) : thi0;
+    int tlo, thi;  // the targets of this walk over the row
+    if (TP > 1 && HALF) {  // (TP = 2) the two halves of the leaf
+        const int half = (thi0 - tlo0 + 1) / 2;
+        tlo = tlo0 + tp * half;
+        thi = (tp + 1 < TP) ? tlo0 + half : thi0;
+    } else {
+        tlo = tlo0 + tp * (32 * W * NT);
+        thi = (TP > 1 && tp + 1 < TP) ? min(thi0, tlo + 32 * W * NT) : thi0;
+    }
     if (TP > 1 && tp > 0) __syncthreads();  // (the tile of the walk before is no longer read)
     mut_targets<NT> T;
     // slot k of this thread holds target tlo + k blockDim + vt; vt = the thread index, rotated by whole warps when RAGGED
     const int vt = RAGGED ? (int)((threadIdx.x + 32u * (blockIdx.x % W)) & (32u * W - 1u)) : (int)threadIdx.x;
     bool short_warp = false;  // (warp-uniform) the warp's last slot holds no particle at all
     if (RAGGED) short_warp = (NT > 1) && (tlo + (NT - 1) * (int)blockDim.x + (vt & ~31) >= thi);
-    // HALF: the second copy of the tail particle l sits in lane l + MUT_HALF_OFF
-    const int tail = HALF ? max(0, thi - (tlo + (NT - 1) * 32)) : 0;  // (at most 15 by the choice of the shape)
-    const bool copy_b = HALF && (int)threadIdx.x >= MUT_HALF_OFF && (int)threadIdx.x - MUT_HALF_OFF < tail;
+    // HALF: every warp takes an equal, contiguous share [wlo, whi) of the targets (slot k of lane l = wlo + 32 k + l), so that all
+    // warps of the block have the same short last slot; the second copy of its tail particle l sits in lane l + MUT_HALF_OFF
+    const int lane = threadIdx.x & 31;
+    int wlo = tlo, whi = thi, tstride = blockDim.x, tpos = vt;
+    if (HALF) {
+        const int share = (max(thi - tlo, 0) + W - 1) / W;
+        wlo = min(thi, tlo + (int)(threadIdx.x >> 5) * share);
+        whi = min(thi, wlo + share);
+        tstride = 32;
+        tpos = lane;
+    }
+    const int tail = HALF ? max(0, whi - (wlo + (NT - 1) * 32)) : 0;  // (at most 15 by the choice of the shape)
+    const bool copy_b = HALF && lane >= MUT_HALF_OFF && lane - MUT_HALF_OFF < tail;
 #pragma unroll
     for (int k = 0; k < NT; ++k) {
-        int i = tlo + k * blockDim.x + vt;
+        int i = wlo + k * tstride + tpos;
         if (HALF && k == NT - 1 && copy_b) i -= MUT_HALF_OFF;
-        const bool live = i < thi;
+        const bool live = i < whi;
         T.x[k] = live ? tx[i] : 0.0; T.y[k] = live ? ty[i] : 0.0; T.z[k] = live ? tz[i] : 0.0;
         T.q0[k] = live ? w0[i] : 0.0; T.q1[k] = live ? w1[i] : 0.0; T.q2[k] = live ? w2[i] : 0.0; T.q3[k] = live ? w3[i] : 0.0;
         T.ex[k] = T.ey[k] = T.ez[k] = T.bx[k] = T.by[k] = T.bz[k] = 0.0;
@@ -433,14 +451,14 @@ __global__ void __launch_bounds__(32 * W, mut_cfg<NT, W>::MINB) p2p_mutual_kerne
 #pragma unroll
         for (int f = 0; f < 6; ++f) {
             const double mine = copy_b ? keep[f] : *s6[f];
-            const double other = __shfl_sync(0xffffffffu, mine, (threadIdx.x + MUT_HALF_OFF) & 31);
-            *s6[f] = ((int)threadIdx.x < tail) ? mine + other : mine;
+            const double other = __shfl_sync(0xffffffffu, mine, (lane + MUT_HALF_OFF) & 31);
+            *s6[f] = (lane < tail) ? mine + other : mine;
         }
     }
 #pragma unroll
     for (int k = 0; k < NT; ++k) {
-        const int i = tlo + k * blockDim.x + vt;
-        if (i < thi) {
+        const int i = wlo + k * tstride + tpos;
+        if (i < whi) {
             double *o = near_ + (SPLIT ? (size_t)kc * 6 * (size_t)N : (size_t)0) + i;
             o[0] = T.ex[k];
             o[(size_t)N] = T.ey[k];
@@ -588,21 +606,32 @@ int pairs_p2p(fmm_plan *p)
 // eight warps per block: two target passes for leaves of more than 1024 particles; else the ragged variant when at least one
 // whole warp-slot of the block stays empty
 #define MUT_LAUNCH_W(NT, W)                                                       \
-    if (maxleaf > 1024) MUT_LAUNCH_R(NT, W, true, 2, false)                       \
+    if (maxleaf > 1024) {                                                         \
+        if (MUT_HALF_OK(NT, W)) MUT_LAUNCH_R(NT, W, false, 2, true) else MUT_LAUNCH_R(NT, W, true, 2, false)            \
+    } else if (MUT_HALF_OK(NT, W)) MUT_LAUNCH_R(NT, W, false, 1, true)            \
     else if (32 * W * NT - maxleaf >= 32) MUT_LAUNCH_R(NT, W, true, 1, false) else MUT_LAUNCH_R(NT, W, false, 1, false)
+// two or four warps per block: the half-rate last slot when every warp's share of the largest leaf ends in 1 .. 15 particles
+#define MUT_LAUNCH_H(NT, W)                                                       \
+    if (MUT_HALF_OK(NT, W)) MUT_LAUNCH_R(NT, W, false, 1, true) else MUT_LAUNCH_R(NT, W, false, 1, false)
+// (the share of a warp: the largest leaf, or its larger half when the block walks its row twice, divided by the warps)
+#define MUT_SHARE(W) (((maxleaf > 1024 ? (maxleaf + 1) / 2 : maxleaf) + W - 1) / W)
+#define MUT_HALF_OK(NT, W) ((MUT_SHARE(W) + 31) / 32 == NT && MUT_SHARE(W) - 32 * (NT - 1) >= 1 && MUT_SHARE(W) - 32 * (NT - 1) <= 15)
         const int W = threads / 32;
         if (nt == 1) { MUT_LAUNCH(1, 1); }
         else if (nt == 2) { MUT_LAUNCH_1(2); }
         else if (nt == 3 && W == 1) { MUT_LAUNCH_1(3); }
-        else if (nt == 3 && W == 2) { MUT_LAUNCH(3, 2); }
-        else if (nt == 3 && W == 4) { MUT_LAUNCH(3, 4); }
+        else if (nt == 3 && W == 2) { MUT_LAUNCH_H(3, 2); }
+        else if (nt == 3 && W == 4) { MUT_LAUNCH_H(3, 4); }
         else if (nt == 3) { MUT_LAUNCH_W(3, 8); }
         else if (W == 1) { MUT_LAUNCH_1(4); }
-        else if (W == 2) { MUT_LAUNCH(4, 2); }
-        else if (W == 4) { MUT_LAUNCH(4, 4); }
+        else if (W == 2) { MUT_LAUNCH_H(4, 2); }
+        else if (W == 4) { MUT_LAUNCH_H(4, 4); }
         else { MUT_LAUNCH_W(4, 8); }
 #undef MUT_LAUNCH
 #undef MUT_LAUNCH_1
+#undef MUT_LAUNCH_H
+#undef MUT_SHARE
+#undef MUT_HALF_OK
 #undef MUT_LAUNCH_W
 #undef MUT_LAUNCH_R
         FMM_LAUNCH_CHECK(c, "p2p_mutual_kernel");

@@ -622,12 +622,16 @@ def test_kd_order_with_li_rebuilt_by_the_leaf_blocks(fmm, monkeypatch, N, N0, st
 @pytest.mark.parametrize("N,N0,cube", [(10000, 729, True), (40000, 729, True), (5003, 640, False), (200000, 900, True), (9000, 1000, False),
                                        (5008, 343, True),
                                        # leaves of 1025 .. 2048 particles: two target passes per block (1250, 2048, 1025 / 1026, 1563)
-                                       (20000, 1331, True), (8192, 2048, False), (4101, 1100, False), (100000, 1600, True)])
+                                       (20000, 1331, True), (8192, 2048, False), (4101, 1100, False), (100000, 1600, True),
+                                       # every warp's share ends in more than 15 particles: still the RAGGED kernels (700; 1400 in two passes)
+                                       (11200, 700, False), (5600, 1400, True), (44800, 700, True)])
 def test_ragged_leaves_in_the_mutual_near_field(fmm, N, N0, cube):
     """Leaves that leave whole warp-slots of an eight-warp near-field block empty (625 particles in 8 x 32 x 3 slots, 782 or 879
     in 8 x 32 x 4, ...): the warps with an empty last slot run the shorter loops and the slot assignment rotates with the block
     index (p2p_mutual_kernel, RAGGED); with and without the row split; (313 in 4 x 32 x 3) keeps the plain kernel; leaves of
-    more than 1,024 particles are worked on in two passes whose reaction sums add up in the same segments.
+    more than 1,024 particles are worked on in two passes whose reaction sums add up in the same segments.  Where every warp's
+    equal share of the leaf ends in 1 .. 15 particles (313 = 4 x 79, 625 = 8 x 79, 782 = 8 x 98, ...) the half-rate last slot
+    of test_half_rate_tail_slot_of_one_warp_leaves is used instead, with per-warp shares.
     Fields against the oracle, and the same bits from one evaluation to the next."""
     w = workloads.paper_cube(N=N, order_n=2) if cube else workloads.config(2, N=N)
     plan = fmm.fmm_plan_create(*w.arrays(), w.q, order_n=2, leaf_size=N0, theta=0.5)
