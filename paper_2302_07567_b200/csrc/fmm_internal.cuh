@@ -94,6 +94,9 @@ struct fmm_plan {
     int stop_level, early_leaves;
     int maxleaf;            // largest leaf: N0 with early leaves, else ceil(N / 2^kappa)
 #define FMM_MUTUAL_MAX_LEAF 2048  // the mutual near field holds a leaf's targets in registers: 1024 per pass, at most two passes
+#define FMM_MUTUAL_MIN_LEAF 24    // below that (one target per lane, lanes idle) the gather of many tiny reaction segments in L2P costs more
+                                  // than the shared evaluations save: N = 1.28e6, leaves of 20: P2P + L2P 3.54 ms mutual, 3.26 ms one-sided
+                                  // (leaves of 10: 4.68 / 3.99; leaves of 39: 3.48 / 4.42)
     double theta, gamma_bar, gamma_bar_param;
     fmm_hdr *hdr;           // device
     int ranges_done;        // node_lo / node_hi are filled (they depend on N and N0 only)

@@ -533,7 +533,7 @@ int dtt_build_lists(fmm_plan *p)
     const int rows_len = (int)p->nodes + 2;
     const int64_t maxleaf = p->maxleaf;
     // the mean-gamma kernel is antisymmetric in the pair, the source-momentum kernel (D depends on p_j) is not
-    const bool mutual = !(p->flags & FMM_KERNEL_SOURCE_MOMENTUM) && maxleaf <= FMM_MUTUAL_MAX_LEAF;
+    const bool mutual = !(p->flags & FMM_KERNEL_SOURCE_MOMENTUM) && maxleaf <= FMM_MUTUAL_MAX_LEAF && maxleaf >= FMM_MUTUAL_MIN_LEAF;
     dtt_counters h;
     fmm_hdr hh;
     int64_t cap = p->leaves * 128;  // first guess; enlarged until nothing overflows, and kept by the plan
